@@ -1,0 +1,335 @@
+// ORACLE (test infrastructure) — grid driver and the C entry points that tests/_orc.py loads with
+// ctypes.  Time stepping follows DESIGN.md §3 C-12 (predictor/corrector = one zone-cycle,
+// PAPER.md:41, 141) and C-14 (harmonic Courant dt, PAPER.md:93 fn. 2).
+#include "orc_grid.hpp"
+#include <algorithm>
+#include <cstring>
+#include <new>
+
+namespace orc {
+
+static const double PI = 3.14159265358979323846;
+
+static bool params_ok(const Params& p, std::string& why) {
+  for (int d = 0; d < 3; d++) {
+    if (p.n[d] < 1) { why = "n[d] < 1"; return false; }
+    if (!(p.xmax[d] > p.xmin[d])) { why = "xmax <= xmin"; return false; }
+    if ((p.bc_lo[d] == 0) != (p.bc_hi[d] == 0)) { why = "periodic must be set on both sides"; return false; }
+  }
+  if (p.metric == 1 && !(p.xmin[0] > 0.0)) { why = "r_in <= 0"; return false; }
+  if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0)) { why = "gamma_ad/cour"; return false; }
+  return true;
+}
+
+// internal-coordinate extents: x1 = ln r for the Kerr-Schild map
+static void internal_extent(const Params& p, double lo[3], double hi[3]) {
+  for (int d = 0; d < 3; d++) { lo[d] = p.xmin[d]; hi[d] = p.xmax[d]; }
+  if (p.metric == 1) { lo[0] = std::log(p.xmin[0]); hi[0] = std::log(p.xmax[0]); }
+}
+
+static Grid* grid_new(const Params& par) {
+  Grid* g = new Grid();
+  g->par = par;
+  g->t = 0.0;
+  g->dt = 0.0;
+  g->have_state = false;
+  g->stats = Stats{0, 0, 0, 0};
+  if (!params_ok(par, g->err)) { delete g; return nullptr; }
+  double lo[3], hi[3];
+  internal_extent(par, lo, hi);
+  g->blocks.resize(1);
+  Block& b = g->blocks[0];
+  for (int d = 0; d < 3; d++) {
+    b.n[d] = par.n[d];
+    b.I0[d] = 0;
+    b.dx[d] = (hi[d] - lo[d]) / par.n[d];
+    b.x0[d] = lo[d];
+    b.phys_lo[d] = b.phys_hi[d] = true;
+  }
+  b.lev1 = 0;
+  b.tau = 0;
+  block_init(par, b);
+  return g;
+}
+
+// one stage of C-12 on the single block
+static void stage(Grid& g, Fields& src, const Fields& base, Fields& out, double dts) {
+  Block& b = g.blocks[0];
+  fill_physical_bc(g.par, b, src);
+  compute_Bc(b, src, false);
+  flux_pass(g.par, b, src);
+  ct_edges(g.par, b, src);
+  update(g.par, b, src, base, out, dts, g.stats);
+}
+
+static void full_step(Grid& g) {
+  Block& b = g.blocks[0];
+  const double dt = g.dt;
+  stage(g, b.sn, b.sn, b.sh, 0.5 * dt);     // predictor: src = base = n, dt/2 -> n+1/2
+  stage(g, b.sh, b.sn, b.snew, dt);         // corrector: src = n+1/2, base = n, dt -> n+1
+  for (int c = 0; c < 5; c++) b.sn.P[c].swap(b.snew.P[c]);
+  for (int c = 0; c < 3; c++) { b.sn.Bc[c].swap(b.snew.Bc[c]); b.sn.Bf[c].swap(b.snew.Bf[c]); }
+  g.t += dt;
+  g.dt = dt_from_ctop(g.par, b);            // C-14: corrector ctop of step n sets dt of step n+1
+}
+
+static bool state_finite(const Grid& g) {
+  const Block& b = g.blocks[0];
+  for (int i = 0; i < b.n[0]; i++)
+    for (int j = 0; j < b.n[1]; j++)
+      for (int k = 0; k < b.n[2]; k++) {
+        const size_t z = b.idx(i, j, k);
+        for (int c = 0; c < 5; c++)
+          if (!std::isfinite(b.sn.P[c][z])) return false;
+      }
+  return true;
+}
+
+}  // namespace orc
+
+using namespace orc;
+
+extern "C" {
+
+int orc_sizeof_params() { return (int)sizeof(Params); }
+
+void* orc_grid_create(const Params* p) {
+  if (!p) return nullptr;
+  try { return grid_new(*p); } catch (const std::bad_alloc&) { return nullptr; }
+}
+
+void orc_grid_destroy(void* h) { delete (Grid*)h; }
+
+// hydro[c]: N1*N2*N3 active zones, x3 fastest.  bface[d]: d-faces, extent n[d]+1 along d; NULL -> 0.
+int orc_set_prims(void* h, const double* const hydro[5], const double* const bface[3]) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  for (int c = 0; c < 5; c++)
+    for (int i = 0; i < b.n[0]; i++)
+      for (int j = 0; j < b.n[1]; j++)
+        for (int k = 0; k < b.n[2]; k++)
+          b.sn.P[c][b.idx(i, j, k)] = hydro[c][((size_t)i * b.n[1] + j) * b.n[2] + k];
+  for (int d = 0; d < 3; d++) {
+    int m[3] = {b.n[0], b.n[1], b.n[2]};
+    m[d] += 1;
+    std::fill(b.sn.Bf[d].begin(), b.sn.Bf[d].end(), 0.0);
+    if (!bface || !bface[d]) continue;
+    for (int i = 0; i < m[0]; i++)
+      for (int j = 0; j < m[1]; j++)
+        for (int k = 0; k < m[2]; k++) {
+          double v = bface[d][((size_t)i * m[1] + j) * m[2] + k];
+          if (d == 1 && b.pole2[j + NG]) v = 0.0;   // C-12: Bf2 on the pole face is 0
+          b.sn.Bf[d][b.idx(i, j, k)] = v;
+        }
+  }
+  fill_physical_bc(g.par, b, b.sn);
+  compute_Bc(b, b.sn, false);
+  flux_pass(g.par, b, b.sn);               // C-14: one flux pass sets dt of step 0
+  g.dt = dt_from_ctop(g.par, b);
+  g.t = 0.0;
+  g.have_state = true;
+  g.stats = Stats{0, 0, 0, 0};
+  return state_finite(g) ? 0 : 5;
+}
+
+int orc_step(void* h, int nsteps, double* t_out, double* dt_last) {
+  Grid& g = *(Grid*)h;
+  if (!g.have_state) return 4;
+  double dtl = 0.0;
+  for (int s = 0; s < nsteps; s++) {
+    dtl = g.dt;
+    full_step(g);
+  }
+  if (t_out) *t_out = g.t;
+  if (dt_last) *dt_last = dtl;
+  return state_finite(g) ? 0 : 5;
+}
+
+double orc_get_dt(void* h) { return ((Grid*)h)->dt; }
+void orc_set_dt(void* h, double dt) { ((Grid*)h)->dt = dt; }
+
+int orc_get_prims(void* h, double* const prims[8]) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  for (int c = 0; c < 8; c++) {
+    const std::vector<double>& a = (c < 5) ? b.sn.P[c] : b.sn.Bc[c - 5];
+    for (int i = 0; i < b.n[0]; i++)
+      for (int j = 0; j < b.n[1]; j++)
+        for (int k = 0; k < b.n[2]; k++)
+          prims[c][((size_t)i * b.n[1] + j) * b.n[2] + k] = a[b.idx(i, j, k)];
+  }
+  return 0;
+}
+
+int orc_get_bface(void* h, double* const bface[3]) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  for (int d = 0; d < 3; d++) {
+    int m[3] = {b.n[0], b.n[1], b.n[2]};
+    m[d] += 1;
+    for (int i = 0; i < m[0]; i++)
+      for (int j = 0; j < m[1]; j++)
+        for (int k = 0; k < m[2]; k++)
+          bface[d][((size_t)i * m[1] + j) * m[2] + k] = b.sn.Bf[d][b.idx(i, j, k)];
+  }
+  return 0;
+}
+
+// C-11: max over zones of |div| / sum_d (|Bf+| + |Bf-|)/(2 dx^d), zones with a denominator below
+// 1e-12 of its global maximum count 0.
+int orc_divb(void* h, double* out) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
+  double denmax = 0.0;
+  for (int pass = 0; pass < 2; pass++) {
+    double worst = 0.0;
+    for (int i = 0; i < b.n[0]; i++)
+      for (int j = 0; j < b.n[1]; j++)
+        for (int k = 0; k < b.n[2]; k++) {
+          const size_t z = b.idx(i, j, k);
+          double div = 0.0, den = 0.0;
+          for (int d = 0; d < 3; d++) {
+            const double lo = b.sn.Bf[d][z], hi = b.sn.Bf[d][z + str[d]];
+            div += (hi - lo) / b.dx[d];
+            den += (std::fabs(hi) + std::fabs(lo)) / (2.0 * b.dx[d]);
+          }
+          if (pass == 0) denmax = std::max(denmax, den);
+          else if (den > 1e-12 * denmax) worst = std::max(worst, std::fabs(div) / den);
+        }
+    if (pass == 1) *out = worst;
+  }
+  return 0;
+}
+
+int orc_get_stats(void* h, long long counts[4]) {
+  Grid& g = *(Grid*)h;
+  counts[0] = g.stats.c2p_fail; counts[1] = g.stats.rho_floor;
+  counts[2] = g.stats.u_floor;  counts[3] = g.stats.gam_ceil;
+  g.stats = Stats{0, 0, 0, 0};
+  return 0;
+}
+
+// Face fluxes / EMFs of the most recent flux pass, for face-by-face parity (debug access).
+// which: 0..4 hydro flux F^d[c]; 5,6 the two face EMFs E_e, E_f with (d,e,f) cyclic.
+int orc_get_face(void* h, int d, int which, double* out) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  static const int CY[3][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}};
+  const std::vector<double>& a = (which < 5) ? b.F[d][which] : b.Ef[d][CY[d][which - 4]];
+  int m[3] = {b.n[0], b.n[1], b.n[2]};
+  m[d] += 1;
+  for (int i = 0; i < m[0]; i++)
+    for (int j = 0; j < m[1]; j++)
+      for (int k = 0; k < m[2]; k++) out[((size_t)i * m[1] + j) * m[2] + k] = a[b.idx(i, j, k)];
+  return 0;
+}
+
+// Conserved totals over active zones: sum of U[c] dV for c = 0..4 (P10), U from sn.
+int orc_totals(void* h, double tot[5]) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  for (int c = 0; c < 5; c++) tot[c] = 0.0;
+  const double dV = b.dx[0] * b.dx[1] * b.dx[2];
+  for (int i = 0; i < b.n[0]; i++)
+    for (int j = 0; j < b.n[1]; j++) {
+      const Geom& G = b.gc[b.idx2(i, j)];
+      for (int k = 0; k < b.n[2]; k++) {
+        const size_t z = b.idx(i, j, k);
+        double P[8], U[8];
+        for (int c = 0; c < 5; c++) P[c] = b.sn.P[c][z];
+        for (int c = 0; c < 3; c++) P[5 + c] = b.sn.Bc[c][z];
+        State S;
+        get_state(P, G, S);
+        prim_to_U(P, S, G, g.par.gamma_ad, U);
+        for (int c = 0; c < 5; c++) tot[c] += U[c] * dV;
+      }
+    }
+  return 0;
+}
+
+// ---- per-zone entry points for the pins -------------------------------------------------------
+void orc_geom_at(int metric, double a, double x1, double x2, Geom* G) { geom_at(metric, a, x1, x2, *G); }
+void orc_conn_at(int metric, double a, double x1, double x2, double* conn64) {
+  conn_at(metric, a, x1, x2, *(double(*)[4][4][4])conn64);
+}
+void orc_gcov_derivs(int metric, double a, double x1, double x2, double* g, double* d1, double* d2) {
+  gcov_and_derivs(metric, a, x1, x2, *(double(*)[4][4])g, *(double(*)[4][4])d1, *(double(*)[4][4])d2);
+}
+void orc_prim_to_UF(const double* P, const Geom* G, double gam, int dir, double* U, double* F) {
+  State S;
+  get_state(P, *G, S);
+  prim_to_U(P, S, *G, gam, U);
+  if (dir >= 1) prim_to_F(P, S, *G, gam, dir, F);
+}
+void orc_state(const double* P, const Geom* G, double* ucon, double* ucov, double* bcon, double* bcov,
+               double* bsq) {
+  State S;
+  get_state(P, *G, S);
+  for (int m = 0; m < 4; m++) { ucon[m] = S.ucon[m]; ucov[m] = S.ucov[m]; bcon[m] = S.bcon[m]; bcov[m] = S.bcov[m]; }
+  *bsq = S.bsq;
+}
+void orc_wavespeeds(const double* P, const Geom* G, double gam, int dir, double* vmin, double* vmax) {
+  State S;
+  get_state(P, *G, S);
+  wavespeeds(P, S, *G, gam, dir, *vmin, *vmax);
+}
+void orc_source(const double* P, const Geom* G, const double* conn64, double gam, double* S5) {
+  State S;
+  get_state(P, *G, S);
+  source(P, S, *G, *(const double(*)[4][4][4])conn64, gam, S5);
+}
+int orc_con2prim(const double* U5, const double* Bc, const Geom* G, double gam, const double* Pguess,
+                 double* Pout, int* iters) {
+  return con2prim(U5, Bc, *G, gam, Pguess, Pout, iters);
+}
+void orc_ppm_zone(const double* a5, double* aL, double* aR) { ppm_zone(a5, *aL, *aR); }
+void orc_plm_zone(const double* a3, double* aL, double* aR) { plm_zone(a3, *aL, *aR); }
+void orc_hll(const double* UL, const double* UR, const double* FL, const double* FR, double cmin,
+             double cmax, double* F) { hll(UL, UR, FL, FR, cmin, cmax, F); }
+
+}  // extern "C"
+
+// ---- debug access for the CT pins (P8): run fill + flux + CT on the current state --------------
+extern "C" {
+int orc_debug_emf(void* h) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  fill_physical_bc(g.par, b, b.sn);
+  compute_Bc(b, b.sn, false);
+  flux_pass(g.par, b, b.sn);
+  ct_edges(g.par, b, b.sn);
+  return 0;
+}
+// edge EMF E_f on edges (extent n+1 along the two directions != f), x3 fastest
+int orc_get_edge(void* h, int f, double* out) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  int m[3] = {b.n[0] + 1, b.n[1] + 1, b.n[2] + 1};
+  m[f] -= 1;
+  for (int i = 0; i < m[0]; i++)
+    for (int j = 0; j < m[1]; j++)
+      for (int k = 0; k < m[2]; k++)
+        out[((size_t)i * m[1] + j) * m[2] + k] = b.Ee[f][b.idx(i, j, k)];
+  return 0;
+}
+// centre EMF E^c_f on active zones
+int orc_get_centre_emf(void* h, int f, double* out) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  for (int i = 0; i < b.n[0]; i++)
+    for (int j = 0; j < b.n[1]; j++)
+      for (int k = 0; k < b.n[2]; k++)
+        out[((size_t)i * b.n[1] + j) * b.n[2] + k] = b.Cc[f][b.idx(i, j, k)];
+  return 0;
+}
+void orc_get_ctop(void* h, double* c3) {
+  Grid& g = *(Grid*)h;
+  for (int d = 0; d < 3; d++) c3[d] = g.blocks[0].ctop[d];
+}
+}
+
+// failure-code histogram of con2prim since creation (debug): codes 1..4
+extern "C" void orc_get_fail_hist(long long h4[4]) {
+  for (int c = 0; c < 4; c++) h4[c] = orc::g_fail_hist[c];
+}

@@ -1,0 +1,328 @@
+// ORACLE (test infrastructure) — the per-block stage: boundary fill, reconstruct + HLL, CT,
+// source + update + inversion, Courant dt.  DESIGN.md §3 C-5..C-14.
+#include "orc_grid.hpp"
+#include <algorithm>
+#include <cstring>
+
+namespace orc {
+
+long long g_fail_hist[4] = {0, 0, 0, 0};  // debug: con2prim failure codes seen
+
+static const int CYC[3][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}};  // (d, e, f) cyclic
+
+void block_init(const Params& par, Block& b) {
+  for (int d = 0; d < 3; d++) b.e[d] = b.n[d] + 2 * NG + 1;
+  const size_t n2d = (size_t)b.e[0] * b.e[1];
+  b.gc.resize(n2d);
+  b.gf1.resize(n2d);
+  b.gf2.resize(n2d);
+  b.conn.assign(n2d * 64, 0.0);
+  b.pole2.assign(b.e[1], 0);
+  b.mrow.assign(b.e[1], 1);
+  for (int j = -NG; j <= b.n[1] + NG; j++) {
+    const long long J = b.I0[1] + j;
+    if (par.metric == 1 && (J == 0 || J == par.n[1])) b.pole2[j + NG] = 1;
+  }
+  for (int i = -NG; i <= b.n[0] + NG; i++)
+    for (int j = -NG; j <= b.n[1] + NG; j++) {
+      const size_t q = b.idx2(i, j);
+      geom_at(par.metric, par.a, b.xc(0, i), b.xc(1, j), b.gc[q]);
+      geom_at(par.metric, par.a, b.xf(0, i), b.xc(1, j), b.gf1[q]);
+      geom_at(par.metric, par.a, b.xc(0, i), b.xf(1, j), b.gf2[q]);
+      if (b.pole2[j + NG]) b.gf2[q].gdet = 0.0;
+      double c[4][4][4];
+      conn_at(par.metric, par.a, b.xc(0, i), b.xc(1, j), c);
+      std::memcpy(&b.conn[q * 64], c, sizeof(c));
+    }
+  const size_t n = b.size();
+  b.sn.alloc(n);
+  b.sh.alloc(n);
+  b.snew.alloc(n);
+  for (int d = 0; d < 3; d++) {
+    for (int c = 0; c < 5; c++) b.F[d][c].assign(n, 0.0);
+    for (int c = 0; c < 3; c++) b.Ef[d][c].assign(n, 0.0);
+    b.Ee[d].assign(n, 0.0);
+    b.Cc[d].assign(n, 0.0);
+    b.ctop[d] = 0.0;
+  }
+}
+
+// ---- physical boundaries (C-12) -------------------------------------------------------------------
+// kind: 0 centred along d, 1 staggered along d (a d-face array); sgn: reflection sign
+static void fill_dim(const Block& b, std::vector<double>& a, int d, int bc_lo, int bc_hi,
+                     bool do_lo, bool do_hi, bool stag, double sgn) {
+  const int n = b.n[d];
+  const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
+  const int o1 = (d + 1) % 3, o2 = (d + 2) % 3;
+  for (int p = 0; p < b.e[o1]; p++)
+    for (int q = 0; q < b.e[o2]; q++) {
+      double* base = a.data() + (size_t)p * str[o1] + (size_t)q * str[o2] + (size_t)NG * str[d];
+      auto at = [&](int i) -> double& { return base[(ptrdiff_t)i * str[d]]; };
+      for (int m = 1; m <= NG; m++) {
+        if (do_lo) {
+          const int g = -m;
+          if (bc_lo == 0) at(g) = at(((g % n) + n) % n);
+          else if (bc_lo == 1) at(g) = at(0);
+          else at(g) = sgn * (stag ? at(m) : at(m - 1));
+        }
+        if (do_hi) {
+          const int g = stag ? n + m : n - 1 + m;
+          if (bc_hi == 0) at(g) = stag ? at(m % n == 0 ? n : m % n) : at((g % n + n) % n);
+          else if (bc_hi == 1) at(g) = stag ? at(n) : at(n - 1);
+          else at(g) = sgn * (stag ? at(n - m) : at(n - m));
+        }
+      }
+      if (stag) {  // a reflecting wall carries no normal flux: the wall face itself is 0
+        if (do_lo && bc_lo == 2) at(0) = 0.0;
+        if (do_hi && bc_hi == 2) at(n) = 0.0;
+      }
+    }
+}
+
+void fill_physical_bc(const Params& par, Block& b, Fields& s) {
+  for (int d = 0; d < 3; d++) {  // order x1, x2, x3 so that edge and corner ghosts are defined
+    const bool lo = b.phys_lo[d], hi = b.phys_hi[d];
+    if (!lo && !hi) continue;
+    const int bl = par.bc_lo[d], bh = par.bc_hi[d];
+    for (int c = 0; c < 5; c++)
+      fill_dim(b, s.P[c], d, bl, bh, lo, hi, false, (c == 2 + d) ? -1.0 : 1.0);
+    for (int c = 0; c < 3; c++)
+      fill_dim(b, s.Bf[c], d, bl, bh, lo, hi, c == d, (c == d) ? -1.0 : 1.0);
+  }
+}
+
+// C-10: B^d_c = (Bf^d_- + Bf^d_+) / (2 g_c)
+void compute_Bc(const Block& b, Fields& s, bool active_only) {
+  const int lo = active_only ? 0 : -NG;
+  const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
+#pragma omp parallel for collapse(2)
+  for (int i = lo; i < b.n[0] - lo; i++)
+    for (int j = lo; j < b.n[1] - lo; j++) {
+      const double g = b.gc[b.idx2(i, j)].gdet;
+      for (int k = lo; k < b.n[2] - lo; k++) {
+        const size_t z = b.idx(i, j, k);
+        for (int d = 0; d < 3; d++)
+          s.Bc[d][z] = (s.Bf[d][z] + s.Bf[d][z + str[d]]) / (2.0 * g);
+      }
+    }
+}
+
+// ---- reconstruct + HLL on one face (C-5, C-6, C-7) -------------------------------------------------
+// face on the low side of zone (i,j,k) along d; `st` = stencil stride along d (1; m in derefined rows)
+static void face_flux(const Params& par, Block& b, const Fields& s, int d, int i, int j, int k,
+                      int st, double* ctop) {
+  const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
+  const size_t z = b.idx(i, j, k);
+  const ptrdiff_t sd = (ptrdiff_t)str[d] * st;
+  const int e = CYC[d][1], f = CYC[d][2];
+  const Geom& G = (d == 0) ? b.gf1[b.idx2(i, j)] : (d == 1) ? b.gf2[b.idx2(i, j)] : b.gc[b.idx2(i, j)];
+  if (d == 1 && b.pole2[j + NG]) {  // C-7: pole faces carry no flux; no state is evaluated
+    for (int c = 0; c < 5; c++) b.F[d][c][z] = 0.0;
+    b.Ef[d][e][z] = b.Ef[d][f][z] = 0.0;
+    return;
+  }
+  double PL[8], PR[8];
+  const double* var[7] = {s.P[0].data(), s.P[1].data(), s.P[2].data(), s.P[3].data(),
+                          s.P[4].data(), s.Bc[e].data(), s.Bc[f].data()};
+  const int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
+  for (int v = 0; v < 7; v++) {
+    const double* a = var[v] + z;
+    double aL, aR, dummy;
+    if (par.recon == 0) {
+      const double l5[5] = {a[-3 * sd], a[-2 * sd], a[-sd], a[0], a[sd]};
+      const double r5[5] = {a[-2 * sd], a[-sd], a[0], a[sd], a[2 * sd]};
+      ppm_zone(l5, dummy, aR);  // left of the face: a_R of zone j-1
+      ppm_zone(r5, aL, dummy);  // right of the face: a_L of zone j
+    } else {
+      const double l3[3] = {a[-2 * sd], a[-sd], a[0]};
+      const double r3[3] = {a[-sd], a[0], a[sd]};
+      plm_zone(l3, dummy, aR);
+      plm_zone(r3, aL, dummy);
+    }
+    PL[slot[v]] = aR;
+    PR[slot[v]] = aL;
+  }
+  PL[5 + d] = PR[5 + d] = s.Bf[d][z] / G.gdet;  // C-5: normal field is single-valued at the face
+  State SL, SR;
+  get_state(PL, G, SL);
+  get_state(PR, G, SR);
+  double UL[8], UR[8], FL[8], FR[8], Fh[8];
+  prim_to_U(PL, SL, G, par.gamma_ad, UL);
+  prim_to_U(PR, SR, G, par.gamma_ad, UR);
+  prim_to_F(PL, SL, G, par.gamma_ad, d + 1, FL);
+  prim_to_F(PR, SR, G, par.gamma_ad, d + 1, FR);
+  double vminL, vmaxL, vminR, vmaxR;
+  wavespeeds(PL, SL, G, par.gamma_ad, d + 1, vminL, vmaxL);
+  wavespeeds(PR, SR, G, par.gamma_ad, d + 1, vminR, vmaxR);
+  const double cmax = std::max(0.0, std::max(vmaxL, vmaxR));
+  const double cmin = std::max(0.0, std::max(-vminL, -vminR));
+  hll(UL, UR, FL, FR, cmin, cmax, Fh);
+  for (int c = 0; c < 5; c++) b.F[d][c][z] = Fh[c];
+  // C-8: on a d-face, E_f = -F^d(B^e), E_e = +F^d(B^f)
+  b.Ef[d][f][z] = -Fh[5 + e];
+  b.Ef[d][e][z] = Fh[5 + f];
+  if (ctop) *ctop = std::max(cmax, cmin);
+}
+
+void flux_pass(const Params& par, Block& b, const Fields& src) {
+  for (int d = 0; d < 3; d++) {
+    int lo[3] = {-1, -1, -1}, hi[3] = {b.n[0], b.n[1], b.n[2]};  // one transverse ghost layer (CT)
+    lo[d] = 0;
+    hi[d] = b.n[d];
+    double cmaxd = 0.0;
+#pragma omp parallel for collapse(2) reduction(max : cmaxd)
+    for (int i = lo[0]; i <= hi[0]; i++)
+      for (int j = lo[1]; j <= hi[1]; j++)
+        for (int k = lo[2]; k <= hi[2]; k++) {
+          double ct = 0.0;
+          face_flux(par, b, src, d, i, j, k, 1, &ct);
+          const int id[3] = {i, j, k};
+          bool act = true;  // C-14: the Courant maximum runs over the faces of ACTIVE zones
+          for (int t = 0; t < 3; t++)
+            if (t != d && (id[t] < 0 || id[t] >= b.n[t])) act = false;
+          if (act) cmaxd = std::max(cmaxd, ct);
+        }
+    b.ctop[d] = cmaxd;
+  }
+}
+
+// ---- constrained transport (C-8, C-9) -------------------------------------------------------------
+static inline double up(double m, double lo, double hi) {
+  return m > 0.0 ? lo : (m < 0.0 ? hi : 0.5 * (lo + hi));
+}
+
+void ct_edges(const Params& par, Block& b, const Fields& s) {
+  const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
+  // centre EMFs E^c_k = -eps_{kmn} v^m Bdens^n on active zones plus one ghost layer
+#pragma omp parallel for collapse(2)
+  for (int i = -1; i <= b.n[0]; i++)
+    for (int j = -1; j <= b.n[1]; j++)
+      for (int k = -1; k <= b.n[2]; k++) {
+        const size_t z = b.idx(i, j, k);
+        const Geom& G = b.gc[b.idx2(i, j)];
+        double P[8];
+        for (int c = 0; c < 5; c++) P[c] = s.P[c][z];
+        for (int c = 0; c < 3; c++) P[5 + c] = s.Bc[c][z];
+        State S;
+        get_state(P, G, S);
+        const double v[3] = {S.ucon[1] / S.ucon[0], S.ucon[2] / S.ucon[0], S.ucon[3] / S.ucon[0]};
+        const double B[3] = {G.gdet * P[5], G.gdet * P[6], G.gdet * P[7]};
+        b.Cc[0][z] = -(v[1] * B[2] - v[2] * B[1]);
+        b.Cc[1][z] = -(v[2] * B[0] - v[0] * B[2]);
+        b.Cc[2][z] = -(v[0] * B[1] - v[1] * B[0]);
+      }
+  // edge EMF E_f at (d-1/2, e-1/2), (d,e,f) cyclic
+  for (int f = 0; f < 3; f++) {
+    const int d = CYC[f][1], e = CYC[f][2];
+    const ptrdiff_t sD = str[d], sE = str[e];
+    const std::vector<double>&X = b.Ef[d][f], &Y = b.Ef[e][f], &C = b.Cc[f];
+    const std::vector<double>&md = b.F[d][0], &me = b.F[e][0];
+    int hi[3] = {b.n[0], b.n[1], b.n[2]};
+    hi[f] = b.n[f] - 1;
+#pragma omp parallel for collapse(2)
+    for (int i = 0; i <= hi[0]; i++)
+      for (int j = 0; j <= hi[1]; j++)
+        for (int k = 0; k <= hi[2]; k++) {
+          const size_t z = b.idx(i, j, k);
+          // C-9: edges on the polar axis carry E1 = E3 = 0 exactly
+          if (f != 1 && b.pole2[j + NG]) { b.Ee[f][z] = 0.0; continue; }
+          const double E =
+              0.25 * (X[z] + X[z - sE] + Y[z] + Y[z - sD]) +
+              0.25 * (up(md[z - sE], Y[z - sD] - C[z - sD - sE], Y[z] - C[z - sE]) -
+                      up(md[z], C[z - sD] - Y[z - sD], C[z] - Y[z])) +
+              0.25 * (up(me[z - sD], X[z - sE] - C[z - sD - sE], X[z] - C[z - sD]) -
+                      up(me[z], C[z - sE] - X[z - sE], C[z] - X[z]));
+          b.Ee[f][z] = E;
+        }
+  }
+  (void)par;
+}
+
+// ---- floors and ceiling (C-13; PAPER.md:59 says only "below a certain threshold") -----------------
+void floors_and_ceiling(const Params& par, const Geom& G, double r, double P[5], Stats& st) {
+  const double rfl = par.rho_fl_coef * std::pow(r, par.rho_fl_pow);
+  const double ufl = par.u_fl_coef * std::pow(r, par.u_fl_pow);
+  if (P[0] < rfl) { P[0] = rfl; st.rho_floor++; }
+  if (P[1] < ufl) { P[1] = ufl; st.u_floor++; }
+  double q = 0.0;
+  for (int i = 1; i < 4; i++)
+    for (int j = 1; j < 4; j++) q += G.gcov[i][j] * P[1 + i] * P[1 + j];
+  const double gamma = std::sqrt(1.0 + q);
+  if (gamma > par.gamma_max) {
+    const double fac = std::sqrt((par.gamma_max * par.gamma_max - 1.0) / (gamma * gamma - 1.0));
+    for (int i = 2; i < 5; i++) P[i] *= fac;
+    st.gam_ceil++;
+  }
+}
+
+// ---- B update, source, conservative update, inversion (C-10, C-12, C-13) ---------------------------
+void update(const Params& par, Block& b, const Fields& src, const Fields& base, Fields& out,
+            double dt, Stats& st) {
+  const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
+  // C-10: Bf^d -= dt [ (E_f(e+) - E_f(e-))/dx^e - (E_e(f+) - E_e(f-))/dx^f ]
+  for (int d = 0; d < 3; d++) {
+    const int e = CYC[d][1], f = CYC[d][2];
+    int hi[3] = {b.n[0] - 1, b.n[1] - 1, b.n[2] - 1};
+    hi[d] = b.n[d];
+#pragma omp parallel for collapse(2)
+    for (int i = 0; i <= hi[0]; i++)
+      for (int j = 0; j <= hi[1]; j++)
+        for (int k = 0; k <= hi[2]; k++) {
+          const size_t z = b.idx(i, j, k);
+          if (d == 1 && b.pole2[j + NG]) { out.Bf[d][z] = 0.0; continue; }
+          const double curl = (b.Ee[f][z + str[e]] - b.Ee[f][z]) / b.dx[e] -
+                              (b.Ee[e][z + str[f]] - b.Ee[e][z]) / b.dx[f];
+          out.Bf[d][z] = base.Bf[d][z] - dt * curl;
+        }
+  }
+  compute_Bc(b, out, true);
+  long long nfail = 0, nrf = 0, nuf = 0, ngc = 0;
+#pragma omp parallel for collapse(2) reduction(+ : nfail, nrf, nuf, ngc)
+  for (int i = 0; i < b.n[0]; i++)
+    for (int j = 0; j < b.n[1]; j++) {
+      const Geom& G = b.gc[b.idx2(i, j)];
+      const double(*conn)[4][4] = (const double(*)[4][4]) & b.conn[b.idx2(i, j) * 64];
+      const double r = (par.metric == 1) ? std::exp(b.xc(0, i)) : 1.0;
+      for (int k = 0; k < b.n[2]; k++) {
+        const size_t z = b.idx(i, j, k);
+        double Pb[8], Ps[8], Ub[8], Ssrc[5], U[5];
+        for (int c = 0; c < 5; c++) { Pb[c] = base.P[c][z]; Ps[c] = src.P[c][z]; }
+        for (int c = 0; c < 3; c++) { Pb[5 + c] = base.Bc[c][z]; Ps[5 + c] = src.Bc[c][z]; }
+        State Sb, Ss;
+        get_state(Pb, G, Sb);
+        prim_to_U(Pb, Sb, G, par.gamma_ad, Ub);
+        get_state(Ps, G, Ss);
+        source(Ps, Ss, G, conn, par.gamma_ad, Ssrc);
+        for (int c = 0; c < 5; c++) {
+          double div = 0.0;
+          for (int d = 0; d < 3; d++) div += (b.F[d][c][z + str[d]] - b.F[d][c][z]) / b.dx[d];
+          U[c] = Ub[c] - dt * div + dt * Ssrc[c];
+        }
+        const double Bn[3] = {out.Bc[0][z], out.Bc[1][z], out.Bc[2][z]};
+        double Pn[5];
+        int rc = con2prim(U, Bn, G, par.gamma_ad, Ps, Pn, nullptr);
+        if (rc != 0) {
+#pragma omp atomic
+          g_fail_hist[rc - 1]++;
+        }
+        if (rc != 0) {  // C-13: keep the source state's hydro primitives, count the failure
+          nfail++;
+          for (int c = 0; c < 5; c++) Pn[c] = Ps[c];
+        }
+        Stats loc = {0, 0, 0, 0};
+        floors_and_ceiling(par, G, r, Pn, loc);
+        nrf += loc.rho_floor; nuf += loc.u_floor; ngc += loc.gam_ceil;
+        for (int c = 0; c < 5; c++) out.P[c][z] = Pn[c];
+      }
+    }
+  st.c2p_fail += nfail; st.rho_floor += nrf; st.u_floor += nuf; st.gam_ceil += ngc;
+}
+
+// C-14 (PAPER.md:93 fn. 2): 1/dt = sum_d 1/dt_d, dt_d = C dx^d / max ctop_d
+double dt_from_ctop(const Params& par, const Block& b) {
+  double s = 0.0;
+  for (int d = 0; d < 3; d++) s += b.ctop[d] / b.dx[d];
+  return par.cour / s;
+}
+
+}  // namespace orc

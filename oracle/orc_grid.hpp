@@ -1,0 +1,72 @@
+// ORACLE (test infrastructure) — block data structure and the per-block stage (C-5..C-14).
+#pragma once
+#include "orc.hpp"
+
+namespace orc {
+
+struct Fields {                    // one time level of one block ("flat arrays")
+  std::vector<double> P[5];        // rho, u, ut1, ut2, ut3 at zone centres
+  std::vector<double> Bc[3];       // cell-centred B^i (C-10)
+  std::vector<double> Bf[3];       // densitised face field g*B^d on d-faces
+  void alloc(size_t n) {
+    for (auto& v : P) v.assign(n, 0.0);
+    for (auto& v : Bc) v.assign(n, 0.0);
+    for (auto& v : Bf) v.assign(n, 0.0);
+  }
+};
+
+struct Block {
+  int n[3];                        // active zones
+  int e[3];                        // padded extents n + 2NG + 1 (the +1 holds the last face/edge)
+  long long I0[3];                 // global index of local zone 0, in zones of this block's level
+  int lev1;                        // x1 refinement level (0 or 1), C-16
+  double dx[3];
+  double x0[3];                    // internal-coordinate origin of the GLOBAL grid
+  bool phys_lo[3], phys_hi[3];     // side lies on the domain boundary
+  int tau;                         // LAT time level (C-17)
+  std::vector<int> mrow;           // phi-derefinement factor per local x2 row incl. ghosts (C-15)
+
+  std::vector<Geom> gc, gf1, gf2;  // 2-D tables over (i,j) incl. ghosts: centres, x1-, x2-faces
+  std::vector<double> conn;        // Gamma at centres, 64 per (i,j)
+  std::vector<char> pole2;         // x2-face row j lies on the polar axis
+
+  Fields sn, sh, snew;             // time n, n+1/2 and the state being written
+  std::vector<double> F[3][5];     // hydro fluxes on d-faces
+  std::vector<double> Ef[3][3];    // Ef[d][c]: E_c on d-faces, c != d (C-8)
+  std::vector<double> Ee[3];       // edge EMFs (C-9)
+  std::vector<double> Cc[3];       // centre EMFs (C-8)
+  double ctop[3];
+
+  size_t size() const { return (size_t)e[0] * e[1] * e[2]; }
+  size_t idx(int i, int j, int k) const {
+    return ((size_t)(i + NG) * e[1] + (j + NG)) * e[2] + (k + NG);
+  }
+  size_t idx2(int i, int j) const { return (size_t)(i + NG) * e[1] + (j + NG); }
+  double xc(int d, int i) const { return x0[d] + ((double)(I0[d] + i) + 0.5) * dx[d]; }
+  double xf(int d, int i) const { return x0[d] + (double)(I0[d] + i) * dx[d]; }
+};
+
+extern long long g_fail_hist[4];
+struct Stats { long long c2p_fail, rho_floor, u_floor, gam_ceil; };
+
+struct Grid {
+  Params par;
+  std::vector<Block> blocks;
+  double t, dt;
+  bool have_state;
+  Stats stats;
+  std::string err;
+};
+
+void block_init(const Params& par, Block& b);           // geometry tables, allocation
+void fill_physical_bc(const Params& par, Block& b, Fields& s);
+void compute_Bc(const Block& b, Fields& s, bool active_only);
+void flux_pass(const Params& par, Block& b, const Fields& src);
+void ct_edges(const Params& par, Block& b, const Fields& src);
+// out may alias base (every zone/face reads only its own base value)
+void update(const Params& par, Block& b, const Fields& src, const Fields& base, Fields& out,
+            double dt, Stats& st);
+double dt_from_ctop(const Params& par, const Block& b);
+void floors_and_ceiling(const Params& par, const Geom& G, double r, double P[5], Stats& st);
+
+}  // namespace orc

@@ -1,0 +1,251 @@
+// ORACLE (test infrastructure) — per-zone physics: C-2..C-7, C-12 (source), C-13 of DESIGN.md §3.
+// PAPER.md:45-47 (Eq. 1: dU/dt = -dF^i/dx^i + S; U conserved, F fluxes, S the warping source);
+// PAPER.md:41 (HLLE, PPM); PAPER.md:49 (Newton-Raphson inversion, Noble et al. 2006).
+#include "orc.hpp"
+#include <algorithm>
+
+namespace orc {
+
+// C-2 four-velocity from primitives, C-3 magnetic four-vector
+void get_state(const double P[8], const Geom& G, State& S) {
+  double q = 0.0;
+  for (int i = 1; i < 4; i++)
+    for (int j = 1; j < 4; j++) q += G.gcov[i][j] * P[1 + i] * P[1 + j];
+  S.gamma = std::sqrt(1.0 + q);
+  S.ucon[0] = S.gamma / G.alpha;
+  for (int i = 1; i < 4; i++) S.ucon[i] = P[1 + i] - S.gamma * G.beta[i - 1] / G.alpha;
+  for (int m = 0; m < 4; m++) {
+    double acc = 0.0;
+    for (int n = 0; n < 4; n++) acc += G.gcov[m][n] * S.ucon[n];
+    S.ucov[m] = acc;
+  }
+  S.bcon[0] = P[5] * S.ucov[1] + P[6] * S.ucov[2] + P[7] * S.ucov[3];
+  for (int i = 1; i < 4; i++) S.bcon[i] = (P[4 + i] + S.bcon[0] * S.ucon[i]) / S.ucon[0];
+  for (int m = 0; m < 4; m++) {
+    double acc = 0.0;
+    for (int n = 0; n < 4; n++) acc += G.gcov[m][n] * S.bcon[n];
+    S.bcov[m] = acc;
+  }
+  S.bsq = 0.0;
+  for (int m = 0; m < 4; m++) S.bsq += S.bcon[m] * S.bcov[m];
+}
+
+// C-4: T^mu_nu = (w + b^2) u^mu u_nu + (p + b^2/2) delta^mu_nu - b^mu b_nu for fixed mu
+static void mhd_row(const double P[8], const State& S, double gam, int mu, double T[4]) {
+  const double p = (gam - 1.0) * P[1];
+  const double w = P[0] + P[1] + p;
+  const double eta = w + S.bsq;
+  const double ptot = p + 0.5 * S.bsq;
+  for (int nu = 0; nu < 4; nu++)
+    T[nu] = eta * S.ucon[mu] * S.ucov[nu] + (mu == nu ? ptot : 0.0) - S.bcon[mu] * S.bcov[nu];
+}
+
+// C-4: U = g (rho u^t, T^t_t + rho u^t, T^t_1, T^t_2, T^t_3, B^1, B^2, B^3)
+void prim_to_U(const double P[8], const State& S, const Geom& G, double gam, double U[8]) {
+  double T[4];
+  mhd_row(P, S, gam, 0, T);
+  const double D = P[0] * S.ucon[0];
+  U[0] = G.gdet * D;
+  U[1] = G.gdet * (T[0] + D);
+  U[2] = G.gdet * T[1];
+  U[3] = G.gdet * T[2];
+  U[4] = G.gdet * T[3];
+  for (int i = 0; i < 3; i++) U[5 + i] = G.gdet * P[5 + i];
+}
+
+// C-4: F^d = g (rho u^d, T^d_t + rho u^d, T^d_i, b^i u^d - b^d u^i)
+void prim_to_F(const double P[8], const State& S, const Geom& G, double gam, int dir, double F[8]) {
+  double T[4];
+  mhd_row(P, S, gam, dir, T);
+  const double m = P[0] * S.ucon[dir];
+  F[0] = G.gdet * m;
+  F[1] = G.gdet * (T[0] + m);
+  F[2] = G.gdet * T[1];
+  F[3] = G.gdet * T[2];
+  F[4] = G.gdet * T[3];
+  for (int i = 1; i < 4; i++)
+    F[4 + i] = G.gdet * (S.bcon[i] * S.ucon[dir] - S.bcon[dir] * S.ucon[i]);
+}
+
+// C-6: bounds on the fast-wave coordinate speeds along `dir`
+void wavespeeds(const double P[8], const State& S, const Geom& G, double gam, int dir,
+                double& vmin, double& vmax) {
+  const double p = (gam - 1.0) * P[1];
+  const double w = P[0] + P[1] + p;
+  const double cs2 = gam * p / w;
+  const double va2 = S.bsq / (S.bsq + w);
+  double cm2 = cs2 + va2 - cs2 * va2;
+  cm2 = std::min(std::max(cm2, 0.0), 1.0);
+  const double A = G.gcon[dir][dir], Bq = G.gcon[0][0], C = G.gcon[0][dir];
+  const double ut = S.ucon[0], ud = S.ucon[dir];
+  const double a2 = ut * ut - (Bq + ut * ut) * cm2;
+  const double a1 = 2.0 * (ud * ut - (C + ud * ut) * cm2);
+  const double a0 = ud * ud - (A + ud * ud) * cm2;
+  const double disc = std::sqrt(std::max(a1 * a1 - 4.0 * a2 * a0, 0.0));
+  const double v1 = (a1 + disc) / (2.0 * a2);
+  const double v2 = (a1 - disc) / (2.0 * a2);
+  vmax = std::max(v1, v2);
+  vmin = std::min(v1, v2);
+}
+
+// C-7 HLL(E) flux for all 8 rows (the row of the face-normal field is identically 0).
+// DESIGN.md §3 C-7a: a mass flux smaller than 1e-12 of the magnitude of its own HLL terms is
+// rounding noise and is flushed to exactly 0, so that the upwind selector of C-9 sees a tie.
+void hll(const double UL[8], const double UR[8], const double FL[8], const double FR[8],
+         double cmin, double cmax, double F[8]) {
+  const double sum = cmax + cmin;
+  if (sum < 1e-300) {
+    for (int c = 0; c < 8; c++) F[c] = 0.5 * (FL[c] + FR[c]);
+  } else {
+    for (int c = 0; c < 8; c++)
+      F[c] = (cmax * FL[c] + cmin * FR[c] - cmax * cmin * (UR[c] - UL[c])) / sum;
+    const double mag = (cmax * std::fabs(FL[0]) + cmin * std::fabs(FR[0]) +
+                        cmax * cmin * (std::fabs(UR[0]) + std::fabs(UL[0]))) / sum;
+    if (std::fabs(F[0]) <= 1e-12 * mag) F[0] = 0.0;
+  }
+}
+
+// C-12: S_nu = g T^kappa_lambda Gamma^lambda_{nu kappa}, nu = 0..3 ; S(rho) = 0.
+// Rows follow U: (0, S_t, S_1, S_2, S_3).
+void source(const double P[8], const State& S, const Geom& G, const double conn[4][4][4],
+            double gam, double Ssrc[5]) {
+  double T[4][4];
+  for (int k = 0; k < 4; k++) mhd_row(P, S, gam, k, T[k]);
+  Ssrc[0] = 0.0;
+  for (int nu = 0; nu < 4; nu++) {
+    double acc = 0.0;
+    for (int k = 0; k < 4; k++)
+      for (int l = 0; l < 4; l++) acc += T[k][l] * conn[l][nu][k];
+    Ssrc[1 + nu] = G.gdet * acc;
+  }
+}
+
+// C-13 conserved -> primitive: 2-unknown (W, v^2) Newton-Raphson of Noble et al. 2006
+// (PAPER.md:49).  U: densitised hydro rows; Bc: cell-centred B^i of the NEW field.
+// Failure codes: 1 no convergence, 2 non-finite.  A converged root with rho <= 0 or u < 0 is NOT a
+// failure: the floors that follow repair it (DESIGN.md §3 S-8).
+int con2prim(const double U[5], const double Bc[3], const Geom& G, double gam,
+             const double Pguess[5], double Pout[5], int* iters) {
+  const double ig = 1.0 / G.gdet;
+  const double alpha = G.alpha;
+  // undensitise; remove rho u^t from the energy row (C-4)
+  const double rhout = U[0] * ig;
+  double Tt[4] = {U[1] * ig - rhout, U[2] * ig, U[3] * ig, U[4] * ig};
+  const double D = alpha * rhout;
+  double Qcov[4], Qcon[4], Bs[4] = {0.0, alpha * Bc[0], alpha * Bc[1], alpha * Bc[2]};
+  for (int m = 0; m < 4; m++) Qcov[m] = alpha * Tt[m];
+  for (int m = 0; m < 4; m++) {
+    double acc = 0.0;
+    for (int n = 0; n < 4; n++) acc += G.gcon[m][n] * Qcov[n];
+    Qcon[m] = acc;
+  }
+  double ncon[4];
+  for (int m = 0; m < 4; m++) ncon[m] = -alpha * G.gcon[m][0];
+  double Qdotn = 0.0, QQ = 0.0;
+  for (int m = 0; m < 4; m++) {
+    Qdotn += Qcov[m] * ncon[m];
+    QQ += Qcov[m] * Qcon[m];
+  }
+  const double Qtsq = QQ + Qdotn * Qdotn;
+  double QdB = 0.0, Bsq = 0.0;
+  for (int i = 1; i < 4; i++) {
+    QdB += Qcov[i] * Bs[i];
+    for (int j = 1; j < 4; j++) Bsq += G.gcov[i][j] * Bs[i] * Bs[j];
+  }
+  const double QdB2 = QdB * QdB;
+  const double cg = (gam - 1.0) / gam;
+
+  // guess from P_src: W0 = (rho + gamma_ad u) gamma^2, v2_0 = 1 - 1/gamma^2
+  double q = 0.0;
+  for (int i = 1; i < 4; i++)
+    for (int j = 1; j < 4; j++) q += G.gcov[i][j] * Pguess[1 + i] * Pguess[1 + j];
+  const double g2 = 1.0 + q;
+  double W = (Pguess[0] + gam * Pguess[1]) * g2;
+  double v2 = 1.0 - 1.0 / g2;
+  v2 = std::min(std::max(v2, 0.0), 1.0 - 1e-15);
+
+  int extra = -1, it = 0;
+  bool conv = false;
+  for (it = 0; it < 30; it++) {
+    const double omv = 1.0 - v2;
+    const double sq = std::sqrt(omv);
+    const double p = cg * (W * omv - D * sq);
+    const double dpdW = cg * omv;
+    const double dpdv = cg * (-W + D / (2.0 * sq));
+    const double BW = Bsq + W;
+    const double W2 = W * W, W3 = W2 * W;
+    const double f1 = Qtsq - v2 * BW * BW + QdB2 * (Bsq + 2.0 * W) / W2;
+    const double f2 = -Qdotn - 0.5 * Bsq * (1.0 + v2) + QdB2 / (2.0 * W2) - W + p;
+    const double j11 = -2.0 * v2 * BW - 2.0 * QdB2 * BW / W3;
+    const double j12 = -BW * BW;
+    const double j21 = -QdB2 / W3 - 1.0 + dpdW;
+    const double j22 = -0.5 * Bsq + dpdv;
+    const double det = j11 * j22 - j12 * j21;
+    const double dW = -(j22 * f1 - j12 * f2) / det;
+    const double dv = -(-j21 * f1 + j11 * f2) / det;
+    if (!std::isfinite(dW) || !std::isfinite(dv)) {
+      if (iters) *iters = it;
+      return 2;
+    }
+    W = std::fabs(W + dW);
+    v2 = std::min(std::max(v2 + dv, 0.0), 1.0 - 1e-15);
+    if (extra >= 0) {
+      if (++extra >= 2) { conv = true; it++; break; }
+    } else if (std::fabs(dW) <= 1e-12 * std::fabs(W) && std::fabs(dv) <= 1e-12) {
+      extra = 0;  // converged: take 2 more iterations (C-13)
+    }
+  }
+  if (iters) *iters = it;
+  if (!conv) return 1;
+  const double gamma = 1.0 / std::sqrt(1.0 - v2);
+  const double rho = D / gamma;
+  const double u = (W / (gamma * gamma) - rho) / gam;
+  if (!std::isfinite(rho) || !std::isfinite(u) || !std::isfinite(W)) return 2;
+  Pout[0] = rho;
+  Pout[1] = u;
+  for (int i = 1; i < 4; i++) {
+    const double Qt = Qcon[i] + Qdotn * ncon[i];
+    Pout[1 + i] = gamma / (W + Bsq) * (Qt + QdB * Bs[i] / W);
+  }
+  return 0;
+}
+
+// C-5 PPM (Colella & Woodward 1984) on a uniform grid, zone j = a[2]
+static double ppm_slope(double am, double a0, double ap) {
+  const double dl = a0 - am, dr = ap - a0;
+  if (dl * dr <= 0.0) return 0.0;
+  const double dc = 0.5 * (ap - am);
+  const double lim = std::min(std::fabs(dc), std::min(2.0 * std::fabs(dl), 2.0 * std::fabs(dr)));
+  return dc > 0.0 ? lim : -lim;
+}
+
+void ppm_zone(const double a[5], double& aL, double& aR) {
+  const double dm_m = ppm_slope(a[0], a[1], a[2]);
+  const double dm_0 = ppm_slope(a[1], a[2], a[3]);
+  const double dm_p = ppm_slope(a[2], a[3], a[4]);
+  aL = a[1] + 0.5 * (a[2] - a[1]) - (dm_0 - dm_m) / 6.0;  // a_{j-1/2}
+  aR = a[2] + 0.5 * (a[3] - a[2]) - (dm_p - dm_0) / 6.0;  // a_{j+1/2}
+  const double aj = a[2];
+  if ((aR - aj) * (aj - aL) <= 0.0) {
+    aL = aR = aj;
+  } else {
+    const double d = aR - aL;
+    const double c = aj - 0.5 * (aL + aR);
+    if (d * c > d * d / 6.0) aL = 3.0 * aj - 2.0 * aR;
+    else if (d * c < -d * d / 6.0) aR = 3.0 * aj - 2.0 * aL;
+  }
+}
+
+void plm_zone(const double a[3], double& aL, double& aR) {
+  // MC limiter: minmod(2(a_j - a_{j-1}), (a_{j+1} - a_{j-1})/2, 2(a_{j+1} - a_j))
+  const double dl = 2.0 * (a[1] - a[0]), dr = 2.0 * (a[2] - a[1]), dc = 0.5 * (a[2] - a[0]);
+  double s = 0.0;
+  if (dl * dr > 0.0) {
+    s = std::min(std::fabs(dc), std::min(std::fabs(dl), std::fabs(dr)));
+    if (dc < 0.0) s = -s;
+  }
+  aL = a[1] - 0.5 * s;
+  aR = a[1] + 0.5 * s;
+}
+
+}  // namespace orc
