@@ -1,0 +1,139 @@
+/* hamr.h — C ABI of the B200-native H-AMR hot path (Liska et al., arXiv:1912.10192).
+ *
+ * What the library computes: the per-zone GRMHD conservative update
+ *     d_t(sqrt(-g) U) + d_i(sqrt(-g) F^i) = sqrt(-g) S ,  div B = 0          (Eq. 1)
+ * on a grid uniform in the internal coordinates x1 = ln r, x2 = theta, x3 = phi of a Kerr-Schild
+ * foliation, with HLLE fluxes and PPM reconstruction, a staggered
+ * constrained-transport magnetic field with velocity-upwinded EMFs, source terms at
+ * zone centres, a Newton-Raphson conserved-to-primitive inversion,
+ * floors, a 2nd-order predictor/corrector and the harmonic
+ * Courant time step (PAPER.md:93 fn. 2).  The readings of every point the paper leaves open are
+ * in DESIGN.md §3.  Every step runs in hand-written CUDA kernels for sm_100a; there is no CPU path.
+ *
+ * Conventions
+ *  - all floating point is IEEE fp64; units G = c = M = 1;
+ *  - all arrays are SoA, dense, index order [i1][i2][i3] with i3 fastest, ACTIVE zones only (the
+ *    library owns the ghost zones);
+ *  - primitives: rho, u, ut1, ut2, ut3 (ut^i = spatial 4-velocity projected normal to the lapse
+ *    observer, C-2), cell-centred B^i;  face field Bf^d = sqrt(-g) B^d on d-faces, with
+ *    shapes (N1+1,N2,N3), (N1,N2+1,N3), (N1,N2,N3+1);
+ *  - pointers are HOST pointers unless the function name ends in _dev, in which case they are
+ *    DEVICE pointers read or written on the grid's stream;
+ *  - the caller owns every array it passes; the library copies in or out before returning
+ *    (host variants synchronise the grid's stream; _dev variants and hamr_step_async do not);
+ *  - every call returns a hamr_status, never throws, never aborts; no global state;
+ *  - one CUDA stream per grid; a grid must not be used from two host threads at once.
+ */
+#ifndef HAMR_H
+#define HAMR_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hamr_grid hamr_grid; /* opaque; owns (or borrows, see hamr_grid_create_in) device memory */
+
+typedef enum {
+  HAMR_OK = 0,
+  HAMR_EINVAL = 1,     /* bad argument or parameter set                                         */
+  HAMR_ENOMEM = 2,     /* device or host allocation failed / arena too small                    */
+  HAMR_ECUDA = 3,      /* a CUDA call failed; hamr_last_error() has the text                    */
+  HAMR_ESTATE = 4,     /* call out of order, e.g. hamr_step before hamr_set_prims               */
+  HAMR_ENONFINITE = 5  /* NaN/Inf detected in the evolved primitives; the grid is unusable      */
+} hamr_status;
+
+typedef enum { HAMR_METRIC_MINKOWSKI = 0, HAMR_METRIC_KERR_SCHILD = 1 } hamr_metric_t;
+typedef enum { HAMR_BC_PERIODIC = 0, HAMR_BC_OUTFLOW = 1, HAMR_BC_POLAR_REFLECT = 2 } hamr_bc_t;
+typedef enum { HAMR_RECON_PPM = 0, HAMR_RECON_PLM_MC = 1 } hamr_recon_t;
+
+/* Parameter block (plain data).  The coordinate map follows the metric: Minkowski = Cartesian box
+ * (x^i linear), Kerr-Schild = (ln r, theta, phi). */
+typedef struct {
+  int metric;            /* hamr_metric_t                                                        */
+  int recon;             /* hamr_recon_t (PPM; PLM+MC is the allowed alternative)   */
+  int n[3];              /* base zones N1, N2, N3                                                */
+  int bc_lo[3], bc_hi[3];/* hamr_bc_t per side; periodic must be set on both sides of a dim     */
+  int nb[3];             /* block size; {0,0,0} = one block (block-structured grid: DESIGN.md §9)*/
+  int n_deref;           /* number of phi-derefinement thresholds, 0 = none       */
+  int deref_factor[4];
+  int lat_max_level;     /* local adaptive time-stepping levels; 0 = global dt    */
+  int pad_;
+  double a;              /* black-hole spin (ignored for Minkowski)                              */
+  double xmin[3], xmax[3]; /* PHYSICAL extents: (r_in, r_out), (0, pi), (0, 2pi), or the box     */
+  double gamma_ad;       /* adiabatic index, p = (gamma_ad - 1) u                                */
+  double cour;           /* Courant factor C of dt_d = C dx^d / max ctop_d (PAPER.md:93 fn. 2)   */
+  double rho_fl_coef, rho_fl_pow, u_fl_coef, u_fl_pow; /* floor = coef * r^pow (r = 1 Cartesian) */
+  double gamma_max;      /* Lorentz-factor ceiling                                               */
+  double deref_theta_deg[4];
+  double r_refine_max;   /* r-refinement radius; <= 0 = none                       */
+} hamr_params;
+
+/* ---- life cycle ------------------------------------------------------------------------------ */
+/* Builds the grid: allocates all device arrays (cudaMalloc, own stream) and runs the metric
+ * precompute kernel (g_{mu nu}, g^{mu nu}, sqrt(-g), lapse, shift at centres and faces, metric
+ * derivatives for the source).  *out is NULL on failure. */
+int hamr_grid_create(const hamr_params* p, hamr_grid** out);
+/* Bytes of device memory a grid with these parameters needs. */
+int hamr_workspace_bytes(const hamr_params* p, size_t* bytes);
+/* Same as hamr_grid_create, but the device arrays live in caller-owned device memory `arena`
+ * (>= hamr_workspace_bytes, 256-byte aligned; e.g. a torch CUDA tensor) and all work is issued on
+ * the caller's `cuda_stream` (a cudaStream_t cast to void*; NULL = the legacy default stream).
+ * The arena must outlive the grid; hamr_grid_destroy does not free it. */
+int hamr_grid_create_in(const hamr_params* p, void* arena, size_t arena_bytes, void* cuda_stream,
+                        hamr_grid** out);
+int hamr_grid_destroy(hamr_grid* g);
+
+/* ---- state in -------------------------------------------------------------------------------- */
+/* Sets the state at t = 0: hydro[c] = rho, u, ut1, ut2, ut3 at zone centres (N1*N2*N3 each);
+ * bface[d] = sqrt(-g) B^d on d-faces (NULL, or NULL entries, = 0).  Fills ghosts, derives the
+ * cell-centred field (C-10) and runs one flux pass to set the first dt (C-14).
+ * Returns HAMR_ENONFINITE if the input contains NaN/Inf. */
+int hamr_set_prims(hamr_grid* g, const double* const hydro[5], const double* const bface[3]);
+int hamr_set_prims_dev(hamr_grid* g, const double* const hydro[5], const double* const bface[3]);
+
+/* ---- the hot path ---------------------------------------------------------------------------- */
+/* Advances nsteps full steps (predictor + corrector = one zone-cycle each): ghost
+ * fill, reconstruct + HLL per direction, CT EMFs + face-B update, source + update, con2prim +
+ * floors, Courant dt reduction — all on the device.  t_out / dt_last_out (host, may be NULL)
+ * receive the time reached and the dt of the last step; the call synchronises the stream. */
+int hamr_step(hamr_grid* g, int nsteps, double* t_out, double* dt_last_out);
+/* Enqueues nsteps steps and returns without synchronising (errors surface at the next sync). */
+int hamr_step_async(hamr_grid* g, int nsteps);
+int hamr_sync(hamr_grid* g); /* waits for the stream; reports HAMR_ENONFINITE / HAMR_ECUDA */
+
+/* ---- state out ------------------------------------------------------------------------------- */
+int hamr_get_prims(hamr_grid* g, double* const prims[8]); /* 5 hydro + cell-centred B^i */
+int hamr_get_prims_dev(hamr_grid* g, double* const prims[8]);
+int hamr_get_bface(hamr_grid* g, double* const bface[3]);
+/* max over zones of |div| / sum_d (|Bf+| + |Bf-|)/(2 dx^d), div = sum_d (Bf^d_+ - Bf^d_-)/dx^d;
+ * zones whose denominator is below 1e-12 of its global maximum count 0 (C-11). */
+int hamr_divb(hamr_grid* g, double* max_norm_divb);
+/* counts since the last call: con2prim failures, rho-floor, u-floor, gamma-ceiling hits */
+int hamr_get_stats(hamr_grid* g, long long counts[4]);
+int hamr_get_time(hamr_grid* g, double* t, double* dt_next);
+int hamr_set_dt(hamr_grid* g, double dt_next); /* overrides the next step's dt (run-to-time) */
+const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the next call on g */
+
+/* ---- block-structured grid (BASELINE.json cfg 4) ------------------ */
+int hamr_num_blocks(const hamr_grid* g);
+int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int n[3],
+                    int* time_level);
+
+/* ---- diagnostics used by the parity tests (not part of the hot path) -------------------------- */
+/* Runs ghost fill + flux pass + CT EMFs on the current state (no update). */
+int hamr_debug_emf(hamr_grid* g);
+/* which 0..4: hydro flux F^d[c] of the last flux pass; 5, 6: the two face EMFs E_e, E_f with
+ * (d, e, f) cyclic (C-8).  out: d-face array, extent n[d]+1 along d. */
+int hamr_get_face(hamr_grid* g, int d, int which, double* out);
+/* edge EMF E_f (extent n+1 along the two directions != f). */
+int hamr_get_edge(hamr_grid* g, int f, double* out);
+int hamr_get_ctop(hamr_grid* g, double ctop[3]); /* per-direction max signal speed of the last corrector pass */
+/* conserved totals sum_zones U[c] dV, c = 0..4, of the current state */
+int hamr_totals(hamr_grid* g, double tot[5]);
+/* kernel launches issued on this grid's stream since creation */
+int hamr_launch_count(const hamr_grid* g, long long* n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HAMR_H */

@@ -1,0 +1,490 @@
+// api.cu — the C-ABI of libhamr (include/hamr.h): grid life cycle, state in/out, the step driver.
+// The time integrator is the 2nd-order predictor/corrector of PAPER.md:41, 141 (C-12):
+//   predictor: src = base = state n,  dt/2 -> n+1/2 ;  corrector: src = n+1/2, base = n, dt -> n+1,
+// each stage = ghost fill -> reconstruct+HLL x3 -> CT EMFs -> B update + source + update + inversion.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "hamr_host.h"
+
+using namespace hamr;
+
+namespace {
+
+constexpr int N_STATE_ARR = 11, N_ARR = 3 * N_STATE_ARR + 15 + 3 + 3 + 3 + 3;
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+bool params_ok(const hamr_params& p, std::string& why) {
+  for (int d = 0; d < 3; d++) {
+    if (p.n[d] < 1) { why = "n[d] < 1"; return false; }
+    if (!(p.xmax[d] > p.xmin[d])) { why = "xmax <= xmin"; return false; }
+    if (p.bc_lo[d] < 0 || p.bc_lo[d] > 2 || p.bc_hi[d] < 0 || p.bc_hi[d] > 2) { why = "bad boundary kind"; return false; }
+    if ((p.bc_lo[d] == HAMR_BC_PERIODIC) != (p.bc_hi[d] == HAMR_BC_PERIODIC)) {
+      why = "periodic must be set on both sides";
+      return false;
+    }
+    if (p.bc_lo[d] != HAMR_BC_PERIODIC && p.n[d] < NG) { why = "non-periodic dimension needs n >= 3"; return false; }
+  }
+  if (p.metric != HAMR_METRIC_MINKOWSKI && p.metric != HAMR_METRIC_KERR_SCHILD) { why = "bad metric"; return false; }
+  if (p.recon != HAMR_RECON_PPM && p.recon != HAMR_RECON_PLM_MC) { why = "bad recon"; return false; }
+  if (p.metric == HAMR_METRIC_KERR_SCHILD && !(p.xmin[0] > 0.0)) { why = "r_in <= 0"; return false; }
+  if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0) || !(p.gamma_max > 1.0)) { why = "gamma_ad / cour / gamma_max"; return false; }
+  if (p.nb[0] || p.nb[1] || p.nb[2] || p.n_deref || p.lat_max_level || p.r_refine_max > 0.0) {
+    why = "block-structured grid (nb, deref, r_refine, LAT) is not available in this build";
+    return false;
+  }
+  return true;
+}
+
+void make_layout(const hamr_params& p, Lay& L) {
+  for (int d = 0; d < 3; d++) L.n[d] = p.n[d];
+  L.e1 = p.n[0] + 2 * NG + 1;
+  L.e2 = p.n[1] + 2 * NG + 1;
+  L.p3 = (int)align_up((size_t)p.n[2] + 2 * NG + 1, 16);
+  L.S2 = L.p3;
+  L.S1 = L.e2 * L.p3;
+  L.off0 = ((long long)NG * L.e2 + NG) * L.p3 + NG + LEAD;
+  L.len = (long long)align_up((size_t)L.e1 * L.e2 * L.p3 + 32, 32);
+  L.n2d = L.e1 * L.e2;
+}
+
+struct ArenaPlan {
+  size_t arr, tabs, scal, cnt, stage, total;
+  size_t stage_doubles;
+};
+
+ArenaPlan plan_arena(const Lay& L) {
+  ArenaPlan a;
+  size_t off = 0;
+  a.arr = off; off += (size_t)N_ARR * L.len * 8;
+  a.tabs = off; off += align_up(((size_t)3 * NGEO + 2 * NDG) * L.n2d * 8 + (size_t)2 * L.e1 * 8, 256);
+  a.scal = off; off += 256;
+  a.cnt = off; off += 256;
+  a.stage_doubles = (size_t)8 * (L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);
+  a.stage = off; off += align_up(a.stage_doubles * 8, 256);
+  a.total = off;
+  return a;
+}
+
+int fail(hamr_grid* g, int code, const char* what, cudaError_t e = cudaSuccess) {
+  if (g) {
+    g->err = what;
+    if (e != cudaSuccess) { g->err += ": "; g->err += cudaGetErrorString(e); }
+  }
+  return code;
+}
+
+#define CK(call)                                                    \
+  do {                                                              \
+    cudaError_t e_ = (call);                                        \
+    if (e_ != cudaSuccess) return fail(g, HAMR_ECUDA, #call, e_);   \
+  } while (0)
+
+int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* stream, bool own,
+                  hamr_grid** out) {
+  if (out) *out = nullptr;
+  if (!p || !out) return HAMR_EINVAL;
+  std::string why;
+  if (!params_ok(*p, why)) return HAMR_EINVAL;
+  hamr_grid* g = new (std::nothrow) hamr_grid();
+  if (!g) return HAMR_ENOMEM;
+  g->par = *p;
+  Dev& D = g->D;
+  std::memset(&D, 0, sizeof(D));
+  make_layout(*p, D.L);
+  const ArenaPlan ap = plan_arena(D.L);
+  g->own_arena = own;
+  g->own_stream = own;
+  g->arena = nullptr;
+  g->stream = nullptr;
+  g->h_pinned = nullptr;
+  g->have_state = false;
+  g->dead = false;
+  g->launches = 0;
+  g->isn = 0; g->ish = 1; g->inew = 2;
+  cudaError_t e;
+  if (own) {
+    if ((e = cudaStreamCreateWithFlags(&g->stream, cudaStreamNonBlocking)) != cudaSuccess) { delete g; return HAMR_ECUDA; }
+    if ((e = cudaMalloc(&g->arena, ap.total)) != cudaSuccess) {
+      cudaStreamDestroy(g->stream);
+      delete g;
+      return e == cudaErrorMemoryAllocation ? HAMR_ENOMEM : HAMR_ECUDA;
+    }
+    g->arena_bytes = ap.total;
+  } else {
+    if (!arena || ((uintptr_t)arena & 255) != 0) { delete g; return HAMR_EINVAL; }
+    if (arena_bytes < ap.total) { delete g; return HAMR_ENOMEM; }
+    g->arena = arena;
+    g->arena_bytes = arena_bytes;
+    g->stream = (cudaStream_t)stream;
+  }
+  if ((e = cudaMallocHost((void**)&g->h_pinned, 64 * sizeof(double))) != cudaSuccess) {
+    if (own) { cudaFree(g->arena); cudaStreamDestroy(g->stream); }
+    delete g;
+    return HAMR_ECUDA;
+  }
+  // internal coordinates: x1 = ln r on the Kerr-Schild map
+  double lo[3], hi[3];
+  for (int d = 0; d < 3; d++) { lo[d] = p->xmin[d]; hi[d] = p->xmax[d]; }
+  if (p->metric == HAMR_METRIC_KERR_SCHILD) { lo[0] = std::log(p->xmin[0]); hi[0] = std::log(p->xmax[0]); }
+  D.metric = p->metric;
+  D.recon = p->recon;
+  for (int d = 0; d < 3; d++) {
+    D.bc_lo[d] = p->bc_lo[d];
+    D.bc_hi[d] = p->bc_hi[d];
+    D.dx[d] = (hi[d] - lo[d]) / p->n[d];
+    D.x0[d] = lo[d];
+  }
+  D.a = p->a; D.gam = p->gamma_ad; D.cour = p->cour; D.gamma_max = p->gamma_max;
+  D.rho_fl_coef = p->rho_fl_coef; D.rho_fl_pow = p->rho_fl_pow;
+  D.u_fl_coef = p->u_fl_coef; D.u_fl_pow = p->u_fl_pow;
+
+  char* base = (char*)g->arena;
+  double* arr = (double*)(base + ap.arr);
+  int ia = 0;
+  auto next = [&]() { return arr + (size_t)(ia++) * D.L.len; };
+  for (int s = 0; s < 3; s++) {
+    for (int c = 0; c < 5; c++) g->s[s].P[c] = next();
+    for (int c = 0; c < 3; c++) g->s[s].Bc[c] = next();
+    for (int c = 0; c < 3; c++) g->s[s].Bf[c] = next();
+  }
+  for (int d = 0; d < 3; d++) for (int c = 0; c < 5; c++) D.F[d][c] = next();
+  for (int d = 0; d < 3; d++) D.EfA[d] = next();
+  for (int d = 0; d < 3; d++) D.EfB[d] = next();
+  for (int d = 0; d < 3; d++) D.Ee[d] = next();
+  for (int d = 0; d < 3; d++) D.Cc[d] = next();
+  double* tabs = (double*)(base + ap.tabs);
+  double* gc = tabs;
+  double* gf1 = gc + (size_t)NGEO * D.L.n2d;
+  double* gf2 = gf1 + (size_t)NGEO * D.L.n2d;
+  double* dgc = gf2 + (size_t)NGEO * D.L.n2d;
+  double* rfl = dgc + (size_t)2 * NDG * D.L.n2d;
+  double* ufl = rfl + D.L.e1;
+  D.gc = gc; D.gf1 = gf1; D.gf2 = gf2; D.dgc = dgc; D.rho_fl = rfl; D.u_fl = ufl;
+  D.scal = (double*)(base + ap.scal);
+  D.cnt = (unsigned long long*)(base + ap.cnt);
+  g->stage = (double*)(base + ap.stage);
+  g->stage_doubles = ap.stage_doubles;
+
+  e = cudaMemsetAsync(g->arena, 0, ap.total, g->stream);
+  if (e == cudaSuccess) {
+    launch_geometry(g, gc, gf1, gf2, dgc, rfl, ufl);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
+  if (e != cudaSuccess) {
+    cudaFreeHost(g->h_pinned);
+    if (own) { cudaFree(g->arena); cudaStreamDestroy(g->stream); }
+    delete g;
+    return HAMR_ECUDA;
+  }
+  *out = g;
+  return HAMR_OK;
+}
+
+// reads n device scalars into host memory (synchronises)
+int read_scal(hamr_grid* g, int first, int n, double* out) {
+  CK(cudaMemcpyAsync(g->h_pinned, g->D.scal + first, n * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  for (int c = 0; c < n; c++) out[c] = g->h_pinned[c];
+  return HAMR_OK;
+}
+
+int check_state(hamr_grid* g) {  // after a sync point: non-finite flag, sticky CUDA errors
+  unsigned long long* h = (unsigned long long*)(g->h_pinned + 32);
+  CK(cudaMemcpyAsync(h, g->D.cnt + N_NONFINITE, sizeof(unsigned long long), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  CK(cudaGetLastError());
+  if (*h != 0) {
+    g->dead = true;
+    return fail(g, HAMR_ENONFINITE, "non-finite primitives detected");
+  }
+  return HAMR_OK;
+}
+
+void enqueue_stage(hamr_grid* g, const Fields& src, const Fields& base, const Fields& out, double dtfac,
+                   bool same, bool want_ctop) {
+  launch_ghosts(g, src, false);
+  launch_flux(g, src, want_ctop);
+  launch_ct(g, src);
+  launch_update(g, src, base, out, dtfac, same);
+}
+
+void enqueue_step(hamr_grid* g) {
+  const Fields& sn = g->s[g->isn];
+  const Fields& sh = g->s[g->ish];
+  const Fields& sw = g->s[g->inew];
+  enqueue_stage(g, sn, sn, sh, 0.5, true, false);
+  enqueue_stage(g, sh, sn, sw, 1.0, false, true);
+  const int tmp = g->isn; g->isn = g->inew; g->inew = tmp;
+  launch_dt(g, 1);  // C-14: the corrector's ctop of step n sets dt of step n+1
+}
+
+int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* const bface[3], bool dev) {
+  if (!g) return HAMR_EINVAL;
+  if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
+  if (!hydro) return fail(g, HAMR_EINVAL, "hydro is NULL");
+  for (int c = 0; c < 5; c++) if (!hydro[c]) return fail(g, HAMR_EINVAL, "hydro[c] is NULL");
+  const Lay& L = g->D.L;
+  const Fields& sn = g->s[g->isn];
+  const size_t nz = (size_t)L.n[0] * L.n[1] * L.n[2];
+  for (int c = 0; c < 5; c++) {
+    const double* src = hydro[c];
+    if (!dev) {
+      double* st = g->stage + (size_t)c * nz;
+      CK(cudaMemcpyAsync(st, hydro[c], nz * 8, cudaMemcpyHostToDevice, g->stream));
+      src = st;
+    }
+    launch_pack(g, src, sn.P[c], -1, false);
+  }
+  size_t off = 5 * nz;
+  for (int d = 0; d < 3; d++) {
+    int m[3] = {L.n[0], L.n[1], L.n[2]};
+    m[d] += 1;
+    const size_t nf = (size_t)m[0] * m[1] * m[2];
+    const double* src = (bface && bface[d]) ? bface[d] : nullptr;
+    if (src && !dev) {
+      if (off + nf > g->stage_doubles) return fail(g, HAMR_ENOMEM, "staging buffer too small");
+      double* st = g->stage + off;
+      CK(cudaMemcpyAsync(st, src, nf * 8, cudaMemcpyHostToDevice, g->stream));
+      src = st;
+      off += nf;
+    }
+    launch_pack(g, src, sn.Bf[d], d, d == 1);
+  }
+  CK(cudaMemsetAsync(g->D.scal, 0, NSCAL * sizeof(double), g->stream));
+  CK(cudaMemsetAsync(g->D.cnt, 0, NCNT * sizeof(unsigned long long), g->stream));
+  launch_ghosts(g, sn, true);
+  launch_flux(g, sn, true);   // C-14: one flux pass sets dt of step 0
+  launch_dt(g, 0);
+  launch_check_finite(g, sn);
+  g->have_state = true;
+  CK(cudaGetLastError());
+  if (dev) return HAMR_OK;
+  return check_state(g);
+}
+
+int get_dense(hamr_grid* g, const double* padded, double* out, int stag, bool dev, size_t stage_off) {
+  const Lay& L = g->D.L;
+  int m[3] = {L.n[0], L.n[1], L.n[2]};
+  if (stag >= 0) m[stag] += 1;
+  const size_t nf = (size_t)m[0] * m[1] * m[2];
+  if (dev) {
+    launch_unpack(g, padded, out, m);
+  } else {
+    double* st = g->stage + stage_off;
+    launch_unpack(g, padded, st, m);
+    CK(cudaMemcpyAsync(out, st, nf * 8, cudaMemcpyDeviceToHost, g->stream));
+  }
+  return HAMR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int hamr_workspace_bytes(const hamr_params* p, size_t* bytes) {
+  std::string why;
+  if (!p || !bytes || !params_ok(*p, why)) return HAMR_EINVAL;
+  Lay L;
+  make_layout(*p, L);
+  *bytes = plan_arena(L).total;
+  return HAMR_OK;
+}
+
+int hamr_grid_create(const hamr_params* p, hamr_grid** out) {
+  return create_common(p, nullptr, 0, nullptr, true, out);
+}
+
+int hamr_grid_create_in(const hamr_params* p, void* arena, size_t arena_bytes, void* cuda_stream,
+                        hamr_grid** out) {
+  return create_common(p, arena, arena_bytes, cuda_stream, false, out);
+}
+
+int hamr_grid_destroy(hamr_grid* g) {
+  if (!g) return HAMR_EINVAL;
+  cudaStreamSynchronize(g->stream);
+  cudaFreeHost(g->h_pinned);
+  if (g->own_arena) cudaFree(g->arena);
+  if (g->own_stream) cudaStreamDestroy(g->stream);
+  delete g;
+  return HAMR_OK;
+}
+
+int hamr_set_prims(hamr_grid* g, const double* const hydro[5], const double* const bface[3]) {
+  return set_prims_common(g, hydro, bface, false);
+}
+int hamr_set_prims_dev(hamr_grid* g, const double* const hydro[5], const double* const bface[3]) {
+  return set_prims_common(g, hydro, bface, true);
+}
+
+int hamr_step_async(hamr_grid* g, int nsteps) {
+  if (!g || nsteps < 0) return HAMR_EINVAL;
+  if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "hamr_step before hamr_set_prims");
+  for (int s = 0; s < nsteps; s++) enqueue_step(g);
+  CK(cudaGetLastError());
+  return HAMR_OK;
+}
+
+int hamr_sync(hamr_grid* g) {
+  if (!g) return HAMR_EINVAL;
+  return check_state(g);
+}
+
+int hamr_step(hamr_grid* g, int nsteps, double* t_out, double* dt_last_out) {
+  int rc = hamr_step_async(g, nsteps);
+  if (rc != HAMR_OK) return rc;
+  double v[6];
+  rc = read_scal(g, 0, 6, v);
+  if (rc != HAMR_OK) return rc;
+  if (t_out) *t_out = v[S_T];
+  if (dt_last_out) *dt_last_out = v[S_DTLAST];
+  return check_state(g);
+}
+
+int hamr_get_prims(hamr_grid* g, double* const prims[8]) {
+  if (!g || !prims) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  const Fields& sn = g->s[g->isn];
+  const size_t nz = (size_t)g->D.L.n[0] * g->D.L.n[1] * g->D.L.n[2];
+  for (int c = 0; c < 8; c++) {
+    if (!prims[c]) continue;
+    int rc = get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], prims[c], -1, false, (size_t)c * nz);
+    if (rc != HAMR_OK) return rc;
+  }
+  CK(cudaStreamSynchronize(g->stream));
+  return HAMR_OK;
+}
+
+int hamr_get_prims_dev(hamr_grid* g, double* const prims[8]) {
+  if (!g || !prims) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  const Fields& sn = g->s[g->isn];
+  for (int c = 0; c < 8; c++)
+    if (prims[c]) get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], prims[c], -1, true, 0);
+  CK(cudaGetLastError());
+  return HAMR_OK;
+}
+
+int hamr_get_bface(hamr_grid* g, double* const bface[3]) {
+  if (!g || !bface) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  const Fields& sn = g->s[g->isn];
+  const Lay& L = g->D.L;
+  size_t off = 0;
+  for (int d = 0; d < 3; d++) {
+    if (!bface[d]) continue;
+    int rc = get_dense(g, sn.Bf[d], bface[d], d, false, off);
+    if (rc != HAMR_OK) return rc;
+    off += (size_t)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);
+  }
+  CK(cudaStreamSynchronize(g->stream));
+  return HAMR_OK;
+}
+
+int hamr_divb(hamr_grid* g, double* out) {
+  if (!g || !out) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  launch_divb(g, g->s[g->isn]);
+  return read_scal(g, S_DIVB, 1, out);
+}
+
+int hamr_get_stats(hamr_grid* g, long long counts[4]) {
+  if (!g || !counts) return HAMR_EINVAL;
+  unsigned long long* h = (unsigned long long*)(g->h_pinned + 32);
+  CK(cudaMemcpyAsync(h, g->D.cnt, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaMemsetAsync(g->D.cnt, 0, 4 * sizeof(unsigned long long), g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  for (int c = 0; c < 4; c++) counts[c] = (long long)h[c];
+  return HAMR_OK;
+}
+
+int hamr_get_time(hamr_grid* g, double* t, double* dt_next) {
+  if (!g) return HAMR_EINVAL;
+  double v[2];
+  int rc = read_scal(g, S_T, 2, v);
+  if (rc != HAMR_OK) return rc;
+  if (t) *t = v[0];
+  if (dt_next) *dt_next = v[1];
+  return HAMR_OK;
+}
+
+int hamr_set_dt(hamr_grid* g, double dt) {
+  if (!g || !(dt > 0.0)) return HAMR_EINVAL;
+  g->h_pinned[48] = dt;
+  CK(cudaMemcpyAsync(g->D.scal + S_DT, g->h_pinned + 48, sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return HAMR_OK;
+}
+
+const char* hamr_last_error(const hamr_grid* g) { return g ? g->err.c_str() : "null grid"; }
+
+int hamr_num_blocks(const hamr_grid* g) { return g ? 1 : 0; }
+
+int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int n[3], int* time_level) {
+  if (!g || b != 0) return HAMR_EINVAL;
+  for (int d = 0; d < 3; d++) {
+    if (x_lo) x_lo[d] = g->D.x0[d];
+    if (dx) dx[d] = g->D.dx[d];
+    if (n) n[d] = g->D.L.n[d];
+  }
+  if (time_level) *time_level = 0;
+  return HAMR_OK;
+}
+
+int hamr_debug_emf(hamr_grid* g) {
+  if (!g) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  const Fields& sn = g->s[g->isn];
+  launch_ghosts(g, sn, false);
+  launch_zero_ctop(g);
+  launch_flux(g, sn, true);
+  launch_ct(g, sn);
+  launch_dt(g, 2);
+  CK(cudaStreamSynchronize(g->stream));
+  CK(cudaGetLastError());
+  return HAMR_OK;
+}
+
+int hamr_get_face(hamr_grid* g, int d, int which, double* out) {
+  if (!g || !out || d < 0 || d > 2 || which < 0 || which > 6) return HAMR_EINVAL;
+  const double* a = which < 5 ? g->D.F[d][which] : (which == 5 ? g->D.EfA[d] : g->D.EfB[d]);
+  int rc = get_dense(g, a, out, d, false, 0);
+  if (rc != HAMR_OK) return rc;
+  CK(cudaStreamSynchronize(g->stream));
+  return HAMR_OK;
+}
+
+int hamr_get_edge(hamr_grid* g, int f, double* out) {
+  if (!g || !out || f < 0 || f > 2) return HAMR_EINVAL;
+  const Lay& L = g->D.L;
+  int m[3] = {L.n[0] + 1, L.n[1] + 1, L.n[2] + 1};
+  m[f] -= 1;
+  launch_unpack(g, g->D.Ee[f], g->stage, m);
+  CK(cudaMemcpyAsync(out, g->stage, (size_t)m[0] * m[1] * m[2] * 8, cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return HAMR_OK;
+}
+
+int hamr_get_ctop(hamr_grid* g, double ctop[3]) {
+  if (!g || !ctop) return HAMR_EINVAL;
+  return read_scal(g, S_CTOPL0, 3, ctop);
+}
+
+int hamr_totals(hamr_grid* g, double tot[5]) {
+  if (!g || !tot) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  launch_totals(g, g->s[g->isn]);
+  return read_scal(g, S_TOT0, 5, tot);
+}
+
+int hamr_launch_count(const hamr_grid* g, long long* n) {
+  if (!g || !n) return HAMR_EINVAL;
+  *n = g->launches;
+  return HAMR_OK;
+}
+
+}  // extern "C"

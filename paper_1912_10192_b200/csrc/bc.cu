@@ -1,0 +1,108 @@
+// bc.cu — physical boundary fill (C-12) and cell-centred B in ghosts (C-10).
+// Boundaries (BASELINE.json cfg 0; PAPER.md:79 discusses the polar boundary): outflow copies the
+// nearest active zone / boundary face, polar reflect mirrors about the axis with ut^2, Bf^2
+// changing sign, periodic wraps.  The fill order x1, x2, x3 of the definition (edge and corner
+// ghosts take values already filled along earlier dimensions) is reproduced in ONE launch by
+// composing the three index maps: every ghost value is a signed copy of one active value.
+#include "hamr_host.h"
+
+namespace hamr {
+
+__device__ __forceinline__ int pmod(int g, int n) {
+  int r = g % n;
+  return r < 0 ? r + n : r;
+}
+
+// source index along one dimension for padded index g; `stag`: the array is a face array along
+// this dimension (active faces 0..n) else zone-centred (active 0..n-1).  flip is set when the
+// value comes from a reflection.
+__device__ __forceinline__ int map_idx(int g, int n, int bc_lo, int bc_hi, bool stag, bool& flip) {
+  const int hi = stag ? n : n - 1;
+  if (g >= 0 && g <= hi) return g;
+  if (g < 0) {
+    const int m = -g;
+    if (bc_lo == HAMR_BC_PERIODIC) return pmod(g, n);
+    if (bc_lo == HAMR_BC_OUTFLOW) return 0;
+    flip = true;
+    return stag ? m : m - 1;
+  }
+  const int m = g - hi;
+  if (bc_hi == HAMR_BC_PERIODIC) return stag ? ((m % n == 0) ? n : m % n) : g % n;
+  if (bc_hi == HAMR_BC_OUTFLOW) return hi;
+  flip = true;
+  return n - m;
+}
+
+// value of array `a` (vector component vc = -1 scalar / 0..2; face array along sd = -1 / 0..2) at
+// any padded location, as the fill would leave it
+__device__ __forceinline__ double ghost_value(const Dev& D, const double* __restrict__ a, int vc, int sd,
+                                              int i, int j, int k) {
+  const Lay& L = D.L;
+  bool f0 = false, f1 = false, f2 = false;
+  const int si = map_idx(i, L.n[0], D.bc_lo[0], D.bc_hi[0], sd == 0, f0);
+  const int sj = map_idx(j, L.n[1], D.bc_lo[1], D.bc_hi[1], sd == 1, f1);
+  const int sk = map_idx(k, L.n[2], D.bc_lo[2], D.bc_hi[2], sd == 2, f2);
+  double v = a[L.idx(si, sj, sk)];
+  // a reflecting wall carries no normal flux: the wall face itself is 0
+  if (sd == 0 && ((si == 0 && D.bc_lo[0] == HAMR_BC_POLAR_REFLECT) || (si == L.n[0] && D.bc_hi[0] == HAMR_BC_POLAR_REFLECT))) v = 0.0;
+  if (sd == 1 && ((sj == 0 && D.bc_lo[1] == HAMR_BC_POLAR_REFLECT) || (sj == L.n[1] && D.bc_hi[1] == HAMR_BC_POLAR_REFLECT))) v = 0.0;
+  if (sd == 2 && ((sk == 0 && D.bc_lo[2] == HAMR_BC_POLAR_REFLECT) || (sk == L.n[2] && D.bc_hi[2] == HAMR_BC_POLAR_REFLECT))) v = 0.0;
+  const bool neg = (vc == 0 && f0) || (vc == 1 && f1) || (vc == 2 && f2);
+  return neg ? -v : v;
+}
+
+// One thread per padded location.  Writes ghost P, ghost Bf and Bc of ghost zones (of all zones if
+// `all` is set: used once for the initial state).
+__global__ void __launch_bounds__(256) k_ghosts(Dev D, Fields s, int all) {
+  const Lay& L = D.L;
+  const int e3 = L.n[2] + 2 * NG + 1;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long tot = (long long)L.e1 * L.e2 * e3;
+  if (t >= tot) return;
+  const int k = (int)(t % e3) - NG;
+  const int j = (int)((t / e3) % L.e2) - NG;
+  const int i = (int)(t / ((long long)e3 * L.e2)) - NG;
+  const int id[3] = {i, j, k};
+  bool in_c[3], extra[3];
+  for (int d = 0; d < 3; d++) {
+    in_c[d] = id[d] >= 0 && id[d] < L.n[d];
+    extra[d] = id[d] == L.n[d] + NG;
+  }
+  const bool zone_active = in_c[0] && in_c[1] && in_c[2];
+  const bool zone_slot = !(extra[0] || extra[1] || extra[2]);
+  if (zone_active && !all) {
+    // interior: only wall faces of reflecting boundaries need attention
+    for (int d = 0; d < 3; d++)
+      if (id[d] == 0 && D.bc_lo[d] == HAMR_BC_POLAR_REFLECT) s.Bf[d][L.idx(i, j, k)] = 0.0;
+    return;
+  }
+  const long long z = L.idx(i, j, k);
+  if (zone_slot && !zone_active) {
+    for (int c = 0; c < 5; c++) s.P[c][z] = ghost_value(D, s.P[c], c - 2, -1, i, j, k);
+  }
+  double lo[3], hi[3];
+  for (int d = 0; d < 3; d++) {
+    // face array along d: valid slot if the transverse indices are zone slots
+    const int o1 = (d + 1) % 3, o2 = (d + 2) % 3;
+    if (extra[o1] || extra[o2]) { lo[d] = hi[d] = 0.0; continue; }
+    lo[d] = ghost_value(D, s.Bf[d], d, d, i, j, k);
+    const bool face_active = in_c[o1] && in_c[o2] && id[d] >= 0 && id[d] <= L.n[d];
+    const bool wall = face_active && ((id[d] == 0 && D.bc_lo[d] == HAMR_BC_POLAR_REFLECT) ||
+                                      (id[d] == L.n[d] && D.bc_hi[d] == HAMR_BC_POLAR_REFLECT));
+    if (!face_active || wall) s.Bf[d][z] = lo[d];  // ghost_value returns 0 on a reflecting wall
+    if (!extra[d]) hi[d] = ghost_value(D, s.Bf[d], d, d, i + (d == 0), j + (d == 1), k + (d == 2));
+  }
+  if (zone_slot) {
+    const double g = __ldg(D.gc + GDET * L.n2d + L.idx2(i, j));
+    for (int d = 0; d < 3; d++) s.Bc[d][z] = (lo[d] + hi[d]) / (2.0 * g);
+  }
+}
+
+void launch_ghosts(hamr_grid* g, const Fields& s, bool all) {
+  const Lay& L = g->D.L;
+  const long long tot = (long long)L.e1 * L.e2 * (L.n[2] + 2 * NG + 1);
+  k_ghosts<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s, all ? 1 : 0);
+  g->launches++;
+}
+
+}  // namespace hamr

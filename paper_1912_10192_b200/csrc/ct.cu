@@ -1,0 +1,89 @@
+// ct.cu — constrained transport: centre EMFs and velocity-upwinded edge EMFs.
+// "magnetic fields are evolved on a staggered grid, where the electric fields have been
+// velocity upwinded to add dissipation (Gardiner & Stone 2005)".  DESIGN.md C-8 (centre EMF
+// E^c_k = -eps_kmn v^m (g B^n)), C-9 (edge EMF from 4 face EMFs, 4 centre EMFs and the sign of the
+// HLL mass fluxes; edges on the polar axis carry E1 = E3 = 0).
+#include "hamr_host.h"
+
+namespace hamr {
+
+// centre EMFs on active zones plus one ghost layer
+__global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s) {
+  const Lay& L = Dv.L;
+  const int c2 = L.n[2] + 2, c1 = L.n[1] + 2;
+  const long long tot = (long long)(L.n[0] + 2) * c1 * c2;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= tot) return;
+  const int k = (int)(t % c2) - 1;
+  const int j = (int)((t / c2) % c1) - 1;
+  const int i = (int)(t / ((long long)c2 * c1)) - 1;
+  const long long z = L.idx(i, j, k);
+  const int q = L.idx2(i, j);
+  const double* gc = Dv.gc;
+  const int n2d = L.n2d;
+  const double c11 = __ldg(gc + C11 * n2d + q), c13 = __ldg(gc + C13 * n2d + q), c22 = __ldg(gc + C22 * n2d + q),
+               c33 = __ldg(gc + C33 * n2d + q), gdet = __ldg(gc + GDET * n2d + q),
+               ialpha = __ldg(gc + IALPHA * n2d + q), boa = __ldg(gc + BOA * n2d + q);
+  const double v1 = s.P[2][z], v2 = s.P[3][z], v3 = s.P[4][z];
+  const double gam = sqrt(1.0 + (c11 * v1 * v1 + c22 * v2 * v2 + c33 * v3 * v3 + 2.0 * (c13 * v1 * v3)));
+  const double iut = 1.0 / (gam * ialpha);
+  const double w1 = (v1 - gam * boa) * iut, w2 = v2 * iut, w3 = v3 * iut;  // v^i = u^i / u^t
+  const double B1 = gdet * s.Bc[0][z], B2 = gdet * s.Bc[1][z], B3 = gdet * s.Bc[2][z];
+  Dv.Cc[0][z] = -(w2 * B3 - w3 * B2);
+  Dv.Cc[1][z] = -(w3 * B1 - w1 * B3);
+  Dv.Cc[2][z] = -(w1 * B2 - w2 * B1);
+}
+
+__device__ __forceinline__ double up(double m, double lo, double hi) {
+  return m > 0.0 ? lo : (m < 0.0 ? hi : 0.5 * (lo + hi));
+}
+
+// E_f at edge (d-1/2, e-1/2) of zone z, (f, d, e) cyclic.  X = E_f on d-faces, Y = E_f on e-faces,
+// C = centre E_f, md / me = HLL mass fluxes through d- / e-faces.
+__device__ __forceinline__ double edge_emf(const double* __restrict__ X, const double* __restrict__ Y,
+                                           const double* __restrict__ C, const double* __restrict__ md,
+                                           const double* __restrict__ me, long long z, long long sD,
+                                           long long sE) {
+  const double Xz = X[z], Xe = X[z - sE], Yz = Y[z], Yd = Y[z - sD];
+  const double Cz = C[z], Cd = C[z - sD], Ce = C[z - sE], Cde = C[z - sD - sE];
+  return 0.25 * (Xz + Xe + Yz + Yd) +
+         0.25 * (up(md[z - sE], Yd - Cde, Yz - Ce) - up(md[z], Cd - Yd, Cz - Yz)) +
+         0.25 * (up(me[z - sD], Xe - Cde, Xz - Cd) - up(me[z], Ce - Xe, Cz - Xz));
+}
+
+// one thread per zone corner: the three edge EMFs on the low edges of zone (i,j,k), 0 <= idx <= n
+__global__ void __launch_bounds__(128) k_edge_emf(Dev Dv) {
+  const Lay& L = Dv.L;
+  const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
+  const long long tot = (long long)(L.n[0] + 1) * c1 * c2;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= tot) return;
+  const int k = (int)(t % c2);
+  const int j = (int)((t / c2) % c1);
+  const int i = (int)(t / ((long long)c2 * c1));
+  const long long z = L.idx(i, j, k);
+  const bool pole = Dv.metric == HAMR_METRIC_KERR_SCHILD && (j == 0 || j == L.n[1]);
+  const long long S[3] = {L.S1, L.S2, 1};
+  const int id[3] = {i, j, k};
+#pragma unroll
+  for (int f = 0; f < 3; f++) {
+    const int d = (f + 1) % 3, e = (f + 2) % 3;
+    if (id[f] >= L.n[f]) continue;
+    double E = 0.0;
+    if (!(f != 1 && pole))
+      // X = E_f on d-faces: f = d + 2 -> EfB[d];  Y = E_f on e-faces: f = e + 1 -> EfA[e]
+      E = edge_emf(Dv.EfB[d], Dv.EfA[e], Dv.Cc[f], Dv.F[d][0], Dv.F[e][0], z, S[d], S[e]);
+    Dv.Ee[f][z] = E;
+  }
+}
+
+void launch_ct(hamr_grid* g, const Fields& src) {
+  const Lay& L = g->D.L;
+  long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 2);
+  k_centre_emf<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(g->D, src);
+  tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);
+  k_edge_emf<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(g->D);
+  g->launches += 2;
+}
+
+}  // namespace hamr

@@ -1,0 +1,289 @@
+"""Thin ctypes binding of libhamr.so (include/hamr.h).  Argument marshalling only: every step of the
+hot path runs in the CUDA kernels behind the C-ABI.  There is no CPU fallback: if the library is
+missing or fails to load, importing the binding's entry points raises.
+
+Names mirror the C calls: hamr_grid_create -> Grid(...), hamr_set_prims -> Grid.set_prims,
+hamr_step -> Grid.step, hamr_get_prims -> Grid.get_prims, hamr_divb -> Grid.divb, ...
+PyTorch is used only for device memory and streams (Grid(..., torch_arena=True) places every
+device array of the grid inside one torch CUDA tensor and issues all work on torch's current stream).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhamr.so")
+_LIB = None
+
+c_double_p = C.POINTER(C.c_double)
+
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENONFINITE = range(6)
+_STATUS = {0: "HAMR_OK", 1: "HAMR_EINVAL", 2: "HAMR_ENOMEM", 3: "HAMR_ECUDA", 4: "HAMR_ESTATE",
+           5: "HAMR_ENONFINITE"}
+
+# every symbol include/hamr.h declares (checked by tests/test_abi.py against the header text)
+SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "hamr_grid_destroy",
+           "hamr_set_prims", "hamr_set_prims_dev", "hamr_step", "hamr_step_async", "hamr_sync",
+           "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
+           "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
+           "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
+           "hamr_launch_count"]
+
+
+class HamrError(RuntimeError):
+    def __init__(self, code, msg=""):
+        self.code = code
+        super().__init__(f"{_STATUS.get(code, code)}: {msg}")
+
+
+class Params(C.Structure):
+    """hamr_params of include/hamr.h"""
+    _fields_ = [("metric", C.c_int), ("recon", C.c_int), ("n", C.c_int * 3),
+                ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3), ("nb", C.c_int * 3),
+                ("n_deref", C.c_int), ("deref_factor", C.c_int * 4),
+                ("lat_max_level", C.c_int), ("pad_", C.c_int),
+                ("a", C.c_double), ("xmin", C.c_double * 3), ("xmax", C.c_double * 3),
+                ("gamma_ad", C.c_double), ("cour", C.c_double),
+                ("rho_fl_coef", C.c_double), ("rho_fl_pow", C.c_double),
+                ("u_fl_coef", C.c_double), ("u_fl_pow", C.c_double), ("gamma_max", C.c_double),
+                ("deref_theta_deg", C.c_double * 4), ("r_refine_max", C.c_double)]
+
+
+def lib():
+    """Loads libhamr.so; raises if it has not been built (python -m paper_1912_10192_b200.build)."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python paper_1912_10192_b200/build.py` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp = C.c_void_p
+        L.hamr_grid_create.argtypes = [C.POINTER(Params), C.POINTER(vp)]
+        L.hamr_workspace_bytes.argtypes = [C.POINTER(Params), C.POINTER(C.c_size_t)]
+        L.hamr_grid_create_in.argtypes = [C.POINTER(Params), vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.hamr_grid_destroy.argtypes = [vp]
+        L.hamr_set_prims.argtypes = [vp, C.POINTER(c_double_p), C.POINTER(c_double_p)]
+        L.hamr_set_prims_dev.argtypes = [vp, C.POINTER(c_double_p), C.POINTER(c_double_p)]
+        L.hamr_step.argtypes = [vp, C.c_int, c_double_p, c_double_p]
+        L.hamr_step_async.argtypes = [vp, C.c_int]
+        L.hamr_sync.argtypes = [vp]
+        L.hamr_get_prims.argtypes = [vp, C.POINTER(c_double_p)]
+        L.hamr_get_prims_dev.argtypes = [vp, C.POINTER(c_double_p)]
+        L.hamr_get_bface.argtypes = [vp, C.POINTER(c_double_p)]
+        L.hamr_divb.argtypes = [vp, c_double_p]
+        L.hamr_get_stats.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.hamr_get_time.argtypes = [vp, c_double_p, c_double_p]
+        L.hamr_set_dt.argtypes = [vp, C.c_double]
+        L.hamr_last_error.argtypes = [vp]
+        L.hamr_last_error.restype = C.c_char_p
+        L.hamr_num_blocks.argtypes = [vp]
+        L.hamr_block_info.argtypes = [vp, C.c_int, c_double_p, c_double_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.hamr_debug_emf.argtypes = [vp]
+        L.hamr_get_face.argtypes = [vp, C.c_int, C.c_int, c_double_p]
+        L.hamr_get_edge.argtypes = [vp, C.c_int, c_double_p]
+        L.hamr_get_ctop.argtypes = [vp, c_double_p]
+        L.hamr_totals.argtypes = [vp, c_double_p]
+        L.hamr_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
+        for s in SYMBOLS:
+            if s != "hamr_last_error":
+                getattr(L, s).restype = C.c_int
+        _LIB = L
+    return _LIB
+
+
+def pack_params(p: dict) -> Params:
+    q = Params()
+    q.metric, q.recon = int(p["metric"]), int(p["recon"])
+    for d in range(3):
+        q.n[d] = int(p["n"][d])
+        q.bc_lo[d], q.bc_hi[d] = int(p["bc_lo"][d]), int(p["bc_hi"][d])
+        q.nb[d] = int(p["nb"][d])
+        q.xmin[d], q.xmax[d] = float(p["xmin"][d]), float(p["xmax"][d])
+    q.n_deref = len(p["deref_factor"])
+    for i, (t, f) in enumerate(zip(p["deref_theta_deg"], p["deref_factor"])):
+        q.deref_theta_deg[i], q.deref_factor[i] = float(t), int(f)
+    q.lat_max_level = int(p["lat_max_level"])
+    q.a = float(p["a"])
+    q.gamma_ad, q.cour = float(p["gamma_ad"]), float(p["cour"])
+    q.rho_fl_coef, q.rho_fl_pow = float(p["rho_fl_coef"]), float(p["rho_fl_pow"])
+    q.u_fl_coef, q.u_fl_pow = float(p["u_fl_coef"]), float(p["u_fl_pow"])
+    q.gamma_max = float(p["gamma_max"])
+    q.r_refine_max = float(p["r_refine_max"])
+    return q
+
+
+def _dp(a):
+    return a.ctypes.data_as(c_double_p)
+
+
+def _arr(x):
+    return np.ascontiguousarray(np.asarray(x, dtype=np.float64))
+
+
+class Grid:
+    """hamr_grid handle.  p: parameter dict as produced by paper_1912_10192_b200.inputs.*_params."""
+
+    def __init__(self, p: dict, torch_arena: bool = False):
+        self.L = lib()
+        self.p = p
+        self.n = tuple(int(v) for v in p["n"])
+        self._par = pack_params(p)
+        self._arena = None
+        h = C.c_void_p(None)
+        if torch_arena:
+            import torch
+            nbytes = C.c_size_t(0)
+            rc = self.L.hamr_workspace_bytes(C.byref(self._par), C.byref(nbytes))
+            if rc != OK:
+                raise HamrError(rc, "hamr_workspace_bytes")
+            self._arena = torch.empty(nbytes.value + 256, dtype=torch.uint8, device="cuda")
+            ptr = (self._arena.data_ptr() + 255) // 256 * 256
+            stream = torch.cuda.current_stream().cuda_stream
+            rc = self.L.hamr_grid_create_in(C.byref(self._par), C.c_void_p(ptr), C.c_size_t(nbytes.value),
+                                            C.c_void_p(stream), C.byref(h))
+        else:
+            rc = self.L.hamr_grid_create(C.byref(self._par), C.byref(h))
+        if rc != OK or not h.value:
+            raise HamrError(rc, "hamr_grid_create")
+        self.h = h
+
+    # -- life cycle ---------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.hamr_grid_destroy(self.h)
+            self.h = None
+            self._arena = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ck(self, rc):
+        if rc != OK:
+            raise HamrError(rc, (self.L.hamr_last_error(self.h) or b"").decode())
+
+    def _fshape(self, d):
+        s = list(self.n)
+        s[d] += 1
+        return tuple(s)
+
+    # -- state in -----------------------------------------------------------------------------------
+    def set_prims(self, hydro, bface=None):
+        hy = [_arr(h) for h in hydro]
+        assert len(hy) == 5 and all(h.shape == self.n for h in hy)
+        hp = (c_double_p * 5)(*[_dp(h) for h in hy])
+        if bface is None:
+            rc = self.L.hamr_set_prims(self.h, hp, None)
+        else:
+            bf = [_arr(b) for b in bface]
+            assert all(bf[d].shape == self._fshape(d) for d in range(3))
+            bp = (c_double_p * 3)(*[_dp(b) for b in bf])
+            rc = self.L.hamr_set_prims(self.h, hp, bp)
+        return rc
+
+    def set_prims_dev(self, hydro, bface=None):
+        """hydro / bface: torch CUDA float64 contiguous tensors (device pointers are passed through)."""
+        hp = (c_double_p * 5)(*[C.cast(C.c_void_p(t.data_ptr()), c_double_p) for t in hydro])
+        bp = None
+        if bface is not None:
+            bp = (c_double_p * 3)(*[C.cast(C.c_void_p(t.data_ptr()), c_double_p) for t in bface])
+        return self.L.hamr_set_prims_dev(self.h, hp, bp)
+
+    # -- the hot path -------------------------------------------------------------------------------
+    def step(self, nsteps=1):
+        t, dt = C.c_double(0), C.c_double(0)
+        self._ck(self.L.hamr_step(self.h, C.c_int(nsteps), C.byref(t), C.byref(dt)))
+        return t.value, dt.value
+
+    def step_async(self, nsteps=1):
+        self._ck(self.L.hamr_step_async(self.h, C.c_int(nsteps)))
+
+    def sync(self):
+        self._ck(self.L.hamr_sync(self.h))
+
+    # -- state out ----------------------------------------------------------------------------------
+    def get_prims(self):
+        out = [np.empty(self.n) for _ in range(8)]
+        self._ck(self.L.hamr_get_prims(self.h, (c_double_p * 8)(*[_dp(o) for o in out])))
+        return out
+
+    def get_prims_dev(self, out):
+        pp = (c_double_p * 8)(*[C.cast(C.c_void_p(t.data_ptr()), c_double_p) for t in out])
+        self._ck(self.L.hamr_get_prims_dev(self.h, pp))
+
+    def get_bface(self):
+        out = [np.empty(self._fshape(d)) for d in range(3)]
+        self._ck(self.L.hamr_get_bface(self.h, (c_double_p * 3)(*[_dp(o) for o in out])))
+        return out
+
+    def divb(self):
+        v = C.c_double(0)
+        self._ck(self.L.hamr_divb(self.h, C.byref(v)))
+        return v.value
+
+    def stats(self):
+        c = (C.c_longlong * 4)()
+        self._ck(self.L.hamr_get_stats(self.h, c))
+        return tuple(c[:])
+
+    @property
+    def t(self):
+        t = C.c_double(0)
+        self._ck(self.L.hamr_get_time(self.h, C.byref(t), None))
+        return t.value
+
+    @property
+    def dt(self):
+        dt = C.c_double(0)
+        self._ck(self.L.hamr_get_time(self.h, None, C.byref(dt)))
+        return dt.value
+
+    @dt.setter
+    def dt(self, v):
+        self._ck(self.L.hamr_set_dt(self.h, C.c_double(v)))
+
+    def num_blocks(self):
+        return self.L.hamr_num_blocks(self.h)
+
+    def block_info(self, b):
+        lo, dx = np.zeros(3), np.zeros(3)
+        n = (C.c_int * 3)()
+        tl = C.c_int(0)
+        self._ck(self.L.hamr_block_info(self.h, b, _dp(lo), _dp(dx), n, C.byref(tl)))
+        return lo, dx, tuple(n[:]), tl.value
+
+    # -- diagnostics --------------------------------------------------------------------------------
+    def debug_emf(self):
+        self._ck(self.L.hamr_debug_emf(self.h))
+
+    def get_face(self, d, which):
+        out = np.empty(self._fshape(d))
+        self._ck(self.L.hamr_get_face(self.h, d, which, _dp(out)))
+        return out
+
+    def get_edge(self, f):
+        s = [v + 1 for v in self.n]
+        s[f] -= 1
+        out = np.empty(tuple(s))
+        self._ck(self.L.hamr_get_edge(self.h, f, _dp(out)))
+        return out
+
+    def ctop(self):
+        c = np.zeros(3)
+        self._ck(self.L.hamr_get_ctop(self.h, _dp(c)))
+        return c
+
+    def totals(self):
+        t = np.zeros(5)
+        self._ck(self.L.hamr_totals(self.h, _dp(t)))
+        return t
+
+    def launch_count(self):
+        n = C.c_longlong(0)
+        self._ck(self.L.hamr_launch_count(self.h, C.byref(n)))
+        return n.value

@@ -1,0 +1,42 @@
+"""Error norms for GPU <-> oracle parity (reading S-21)."""
+import numpy as np
+
+from paper_1912_10192_b200 import inputs as I
+
+
+def centre_gcov_diag_and_norm(p, vec):
+    """sqrt(g_ii) per component and ||q|| = sqrt(g_ij q^i q^j) at zone centres for a vector field
+    vec = [q1, q2, q3] (each (N1,N2,N3))."""
+    n = p["n"]
+    if p["metric"] == I.METRIC_MINKOWSKI:
+        sg = [np.ones(n)] * 3
+        nrm = np.sqrt(vec[0] ** 2 + vec[1] ** 2 + vec[2] ** 2)
+        return sg, nrm
+    xc, _, _ = I.grid_coords(p)
+    r2, th2 = np.meshgrid(np.exp(xc[0]), xc[1], indexing="ij")
+    g = I.ks_gcov(p["a"], r2, th2)[:, :, None, :, :]
+    q = np.stack(vec, axis=-1)
+    nrm2 = np.einsum("...i,...ij,...j->...", q, g[..., 1:, 1:], q)
+    sg = [np.sqrt(np.broadcast_to(g[..., 1 + i, 1 + i], n)) for i in range(3)]
+    return sg, np.sqrt(np.maximum(nrm2, 0.0))
+
+
+def parity_errors(p, ref, got):
+    """max relative error per primitive group: rho, u (pointwise relative), ut and B (component
+    error in orthonormal-like units against max(||q||, 1e-3 max ||q||))."""
+    out = {}
+    for name, c in (("rho", 0), ("u", 1)):
+        out[name] = float(np.max(np.abs(got[c] - ref[c]) / np.abs(ref[c])))
+    for name, c0 in (("ut", 2), ("B", 5)):
+        sg, nrm = centre_gcov_diag_and_norm(p, ref[c0:c0 + 3])
+        scale = np.maximum(nrm, 1e-3 * nrm.max())
+        if nrm.max() == 0.0:
+            out[name] = float(max(np.max(np.abs(got[c0 + i] - ref[c0 + i])) for i in range(3)))
+            continue
+        out[name] = float(max(np.max(np.abs(got[c0 + i] - ref[c0 + i]) * sg[i] / scale) for i in range(3)))
+    return out
+
+
+def rel_max(ref, got):
+    s = np.abs(ref).max()
+    return float(np.abs(got - ref).max() / (s if s > 0 else 1.0))

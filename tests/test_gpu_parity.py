@@ -1,0 +1,177 @@
+"""GPU <-> oracle parity through the C-ABI (BASELINE.json north_star: max relative error <= 1e-10 on all
+primitives after 1 step, <= 1e-7 after 10 steps, div B <= 1e-12, zero inversion failures).
+Same seeded inputs to both sides; element-by-element comparison.  Needs a B200."""
+import numpy as np
+import pytest
+
+from paper_1912_10192_b200 import inputs as I
+from tests._parity import parity_errors, rel_max
+
+pytestmark = pytest.mark.gpu
+
+TOL_1, TOL_10, TOL_DIVB = 1e-10, 1e-7, 1e-12
+
+
+@pytest.fixture(scope="module")
+def H():
+    from paper_1912_10192_b200 import build, hamr
+    build.build_lib()
+    hamr.lib()
+    return hamr
+
+
+def _pair(H, orc, p, hyd, bf):
+    g = H.Grid(p)
+    o = orc.OrcGrid(p)
+    assert g.set_prims(hyd, bf) == 0
+    assert o.set_prims(hyd, bf) == 0
+    return g, o
+
+
+def _cases():
+    c = {}
+    p = I.torus_params()                                        # BASELINE cfg 0
+    c["cfg0_torus"] = (p, lambda: I.fm_torus(p, seed=0))
+    q = I.minkowski_params(n=(40, 24, 36))                      # ragged sizes: several tiles + tails
+    c["minkowski_ragged"] = (q, lambda: I.minkowski_waves(q, seed=1, amp=1e-2, noise=1e-3))
+    r = I.torus_params(n=(24, 16, 8), recon=I.RECON_PLM)
+    c["torus_plm"] = (r, lambda: I.fm_torus(r, seed=5))
+    s = I.minkowski_params(n=(32, 32, 32))                      # BASELINE cfg 1 at oracle-friendly size
+    c["cfg1_waves"] = (s, lambda: I.minkowski_waves(s, seed=1))
+    return c
+
+
+CASES = _cases()
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_face_fluxes_emfs_and_ctop_match(H, orc, name):
+    p, gen = CASES[name]
+    hyd, bf = gen()
+    g, o = _pair(H, orc, p, hyd, bf)
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt          # first dt from the initial flux pass (C-14)
+    g.debug_emf()
+    o.debug_emf()
+    for d in range(3):
+        for which in range(7):
+            a, b = o.get_face(d, which), g.get_face(d, which)
+            assert rel_max(a, b) <= 1e-12, (name, d, which, rel_max(a, b))
+            if which == 0:   # the upwind selector of CT sees the SIGN of the mass flux: must agree exactly
+                assert np.array_equal(np.sign(a), np.sign(b)), (name, d)
+    for f in range(3):
+        a, b = o.get_edge(f), g.get_edge(f)
+        assert rel_max(a, b) <= 1e-12, (name, f, rel_max(a, b))
+    assert np.allclose(g.ctop(), o.ctop(), rtol=1e-13, atol=0)
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_parity_after_1_and_10_steps(H, orc, name):
+    p, gen = CASES[name]
+    hyd, bf = gen()
+    g, o = _pair(H, orc, p, hyd, bf)
+    tg, dtg = g.step(1)
+    to, dto = o.step(1)
+    assert abs(tg - to) <= 1e-13 * to and abs(dtg - dto) <= 1e-13 * dto
+    e1 = parity_errors(p, o.get_prims(), g.get_prims())
+    assert max(e1.values()) <= TOL_1, (name, e1)
+    for a, b in zip(o.get_bface(), g.get_bface()):
+        assert rel_max(a, b) <= TOL_1
+    g.step(9)
+    o.step(9)
+    e10 = parity_errors(p, o.get_prims(), g.get_prims())
+    assert max(e10.values()) <= TOL_10, (name, e10)
+    assert g.divb() <= TOL_DIVB and o.divb() <= TOL_DIVB
+    sg, so = g.stats(), o.stats()
+    assert sg[0] == 0 and so[0] == 0                 # parity runs must report zero inversion failures
+    print(name, "1 step", e1, "10 steps", e10, "floors gpu/orc", sg, so)
+
+
+def test_divb_and_conservation_minkowski(H):
+    p = I.minkowski_params(n=(24, 20, 28))
+    hyd, bf = I.minkowski_waves(p, seed=1, amp=1e-2, noise=1e-3)
+    g = H.Grid(p)
+    assert g.set_prims(hyd, bf) == 0
+    assert g.divb() < 1e-13
+    t0 = g.totals()
+    g.step(30)
+    t1 = g.totals()
+    assert g.divb() < TOL_DIVB and g.stats()[0] == 0
+    assert abs(t1[0] - t0[0]) < 1e-13 * abs(t0[0])
+    assert abs(t1[1] - t0[1]) < 1e-13 * abs(t0[1])
+    assert np.all(np.abs(t1[2:] - t0[2:]) < 1e-13 * abs(t0[1]))
+    b0 = [b.sum() for b in bf]
+    b1 = [b.sum() for b in g.get_bface()]
+    assert np.allclose(b0, b1, rtol=1e-13)
+
+
+def test_edge_cases(H, orc):
+    # phi slab (N3 = 1), no magnetic field, minimum sizes
+    p = I.torus_params(n=(16, 8, 1))
+    hyd, _ = I.fm_torus(p, pert=0.0, with_B=False)
+    g, o = _pair(H, orc, p, hyd, None)
+    g.step(3)
+    o.step(3)
+    e = parity_errors(p, o.get_prims(), g.get_prims())
+    assert max(e.values()) <= 1e-9, e
+    # smallest non-periodic extents
+    q = I.torus_params(n=(3, 3, 3))
+    hyd, bf = I.fm_torus(q, seed=7)
+    g, o = _pair(H, orc, q, hyd, bf)
+    g.step(2)
+    o.step(2)
+    assert max(parity_errors(q, o.get_prims(), g.get_prims()).values()) <= 1e-9
+    # call order and bad input
+    g2 = H.Grid(q)
+    with pytest.raises(H.HamrError) as ei:
+        g2.step(1)
+    assert ei.value.code == H.ESTATE
+    hyd[0] = hyd[0].copy()
+    hyd[0][1, 1, 1] = np.nan
+    assert g2.set_prims(hyd, bf) == H.ENONFINITE
+    # zero steps is a no-op
+    g3 = H.Grid(q)
+    hyd, bf = I.fm_torus(q, seed=7)
+    g3.set_prims(hyd, bf)
+    t, _ = g3.step(0)
+    assert t == 0.0
+    for a, b in zip(g3.get_prims()[:5], hyd):
+        assert np.array_equal(a, b)
+
+
+def test_device_pointer_path_and_torch_arena(H, orc):
+    import torch
+    p = I.torus_params(n=(24, 12, 16))
+    hyd, bf = I.fm_torus(p, seed=3)
+    g = H.Grid(p, torch_arena=True)
+    hd = [torch.from_numpy(np.ascontiguousarray(h)).cuda() for h in hyd]
+    bd = [torch.from_numpy(np.ascontiguousarray(b)).cuda() for b in bf]
+    assert g.set_prims_dev(hd, bd) == 0
+    g.step(2)
+    out = [torch.empty(p["n"], dtype=torch.float64, device="cuda") for _ in range(8)]
+    g.get_prims_dev(out)
+    torch.cuda.synchronize()
+    g2 = H.Grid(p)
+    g2.set_prims(hyd, bf)
+    g2.step(2)
+    ref = g2.get_prims()
+    for a, b in zip(ref, out):
+        assert np.array_equal(a, b.cpu().numpy())     # same kernels, same inputs: bitwise
+    assert g.launch_count() > 0
+
+
+def test_full_size_headline_config_one_step(H, orc):
+    """BASELINE cfg 2 (256x128x128 Kerr torus) in the launch configuration bench.py times: every
+    zone compared against the oracle after one step; properties after more steps."""
+    p = I.torus_params(n=(256, 128, 128), r_out=1000.0)
+    hyd, bf = I.fm_torus(p, seed=2)
+    g, o = _pair(H, orc, p, hyd, bf)
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt
+    g.step(1)
+    o.step(1)
+    e1 = parity_errors(p, o.get_prims(), g.get_prims())
+    print("cfg2 1 step", e1)
+    assert max(e1.values()) <= TOL_1, e1
+    o.close()
+    g.step(9)
+    assert g.divb() <= TOL_DIVB
+    assert g.stats()[0] == 0
