@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py — zone-cycles/s of the fp64 GRMHD step on B200 (BASELINE.json metric), the HBM/ALU roofline
+fraction of the dominant kernel, the end-to-end number through the C-ABI with host buffers, and the
+CPU oracle timed beside it.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg3]
+
+A "step" is one full pass of the hot path over the whole grid: hamr_step(1) = predictor + corrector
+= one zone-cycle per zone.  Default workload: BASELINE.json configs[2], the 256x128x128
+Kerr Fishbone-Moncrief torus (the config the metric is quoted on).  Inputs are seeded and synthetic
+(paper_1912_10192_b200/inputs.py); the state (2.4 GB of fp64 arrays) is far larger than the 126 MB L2.
+N > 1: the path does not shard ("replicas only"): every rank runs an independent replica.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "zone_cycles_per_sec"
+UNIT = "zone-cycles/s"
+
+
+def workload(name):
+    from paper_1912_10192_b200 import inputs as I
+    if name == "cfg2":
+        p = I.torus_params(n=(256, 128, 128), r_out=1000.0)
+        return p, (lambda: I.fm_torus(p, seed=2)), "BASELINE cfg2: Kerr FM torus 256x128x128 fp64, a=0.9375, PPM+HLL+CT"
+    if name == "cfg0":
+        p = I.torus_params()
+        return p, (lambda: I.fm_torus(p, seed=0)), "BASELINE cfg0: tiny Kerr FM torus 32x16x16"
+    if name == "cfg1":
+        p = I.minkowski_params(n=(128, 128, 128))
+        return p, (lambda: I.minkowski_waves(p, seed=1)), "BASELINE cfg1: Minkowski periodic 128^3 linear waves"
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """samples nvidia-smi clocks / throttle reasons while the timed region runs"""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# algorithmic doubles per unit of each kernel class: (reads + writes) per face / zone
+ALG_DOUBLES = {"flux_x1": 16, "flux_x2": 16, "flux_x3": 16,   # 9 r (P5, 2 transverse Bc, Bf^d) + 7 w (F5, 2 EMFs)
+               # update: r src P5+Bc3 (+ base P5+Bc3 in the corrector), base Bf3, Ee3, F15; w P5, Bc3, Bf3
+               "update_predictor": 8 + 3 + 3 + 15 + 11, "update_corrector": 8 + 8 + 3 + 3 + 15 + 11,
+               "centre_emf": 6 + 3, "edge_emf": 6 + 3 + 3 + 3, "ghosts": 0, "dt": 0, "other": 0}
+
+
+def units_per_launch(cls, n):
+    n1, n2, n3 = n
+    if cls == "flux_x1":
+        return (n1 + 1) * (n2 + 2) * (n3 + 2)
+    if cls == "flux_x2":
+        return (n1 + 2) * (n2 + 1) * (n3 + 2)
+    if cls == "flux_x3":
+        return (n1 + 2) * (n2 + 2) * (n3 + 1)
+    if cls == "centre_emf":
+        return (n1 + 2) * (n2 + 2) * (n3 + 2)
+    if cls == "edge_emf":
+        return (n1 + 1) * (n2 + 1) * (n3 + 1)
+    return n1 * n2 * n3
+
+
+def cpu_oracle_time(p, gen, steps):
+    """times the oracle as it stands on the host cores: `steps` full steps of the workload"""
+    from tests import _orc
+    hyd, bf = gen()
+    o = _orc.OrcGrid(p)
+    o.set_prims(hyd, bf)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    cores = int(_orc.lib().orc_omp_threads())
+    o.close()
+    nz = int(np.prod(p["n"]))
+    return nz * steps / dt, dt, cores
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import __graft_entry__ as ge
+    subprocess.check_call(["make", "-s", "-C", os.path.join(ROOT, "oracle")])
+    p, gen, desc = workload(args.workload)
+    from tests import _orc
+    hyd, bf = gen()
+    o = _orc.OrcGrid(p)
+    o.set_prims(hyd, bf)
+    for _ in range(args.warmup):
+        o.step(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(1)
+    dt = time.perf_counter() - t0
+    cores = int(_orc.lib().orc_omp_threads())
+    nz = int(np.prod(p["n"]))
+    val = nz * args.steps / dt
+    sample = f"{args.steps} full oracle steps of the whole {p['n'][0]}x{p['n'][1]}x{p['n'][2]} grid per timed step"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="hamr", choices=["hamr", "reference"])
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if args.steps is None:
+            args.steps = 5
+        args.warmup = min(args.warmup, 1) if args.warmup else 0
+        return run_reference(args)
+    if args.steps is None:
+        args.steps = 20
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    import __graft_entry__ as ge
+    if rank == 0:
+        ge.build()
+    if world > 1:
+        dist.barrier()
+    from paper_1912_10192_b200 import hamr
+
+    p, gen, desc = workload(args.workload)
+    n = tuple(p["n"])
+    nz = int(np.prod(n))
+    hyd, bf = gen()
+    g = hamr.Grid(p, torch_arena=True)        # device memory and stream from torch; all math in libhamr
+    hd = [torch.from_numpy(np.ascontiguousarray(h)).cuda() for h in hyd]
+    bd = [torch.from_numpy(np.ascontiguousarray(b)).cuda() for b in bf]
+    assert g.set_prims_dev(hd, bd) == 0
+    g.sync()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput ---------------------------------------------------------------
+    for _ in range(args.warmup):
+        g.step_async(1)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = g.launch_count()
+    g.profile_begin()                          # per-kernel CUDA event pairs on the launching stream
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        g.step_async(1)
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    prof = g.profile_end()
+    clocks = sampler.stop()
+    launches = g.launch_count() - l0
+    g.sync()
+    tms = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    ms_max = float(tms.item())
+    value = world * nz * args.steps / (ms_max * 1e-3)
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned): set_prims + step + get_prims -----
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    hh = [pin(h) for h in hyd]
+    bh = [pin(b) for b in bf]
+    outs = [torch.empty(n, dtype=torch.float64).pin_memory().numpy() for _ in range(8)]
+    C = hamr.C
+    hp = (hamr.c_double_p * 5)(*[hamr._dp(h) for h in hh])
+    bp = (hamr.c_double_p * 3)(*[hamr._dp(b) for b in bh])
+    op = (hamr.c_double_p * 8)(*[hamr._dp(o) for o in outs])
+    L = hamr.lib()
+
+    def e2e_step():
+        rc = L.hamr_set_prims(g.h, hp, bp)
+        rc |= L.hamr_step(g.h, 1, None, None)
+        rc |= L.hamr_get_prims(g.h, op)
+        assert rc == 0, rc
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    ev0.record()
+    for _ in range(args.e2e_steps):
+        e2e_step()
+    ev1.record()
+    barrier()
+    e2e_ms = max(ev0.elapsed_time(ev1), 1e3 * (time.perf_counter() - t0))
+    tms = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    e2e_val = world * nz * args.e2e_steps / (float(tms.item()) * 1e-3)
+    h2d = sum(a.nbytes for a in hh) + sum(a.nbytes for a in bh)
+    d2h = sum(a.nbytes for a in outs)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel ------------------------------------------------------------
+    hbm_peak, peak_src = peaks()
+    kern = {k: {"ms_total": v[0], "launches": v[1], "ms_avg": v[0] / v[1] if v[1] else 0.0,
+                "share": v[0] / ms if ms else 0.0} for k, v in prof.items() if v[1]}
+    for k, d in kern.items():
+        by = ALG_DOUBLES.get(k, 0) * 8 * units_per_launch(k, n)
+        d["alg_bytes"] = by
+        d["gbs"] = by / (d["ms_avg"] * 1e-3) / 1e9 if d["ms_avg"] > 0 else 0.0
+    dom = max(kern, key=lambda k: kern[k]["ms_total"])
+    roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": hbm_peak, "unit": "GB/s",
+            "frac": kern[dom]["gbs"] / hbm_peak, "traffic": None, "peak_source": peak_src,
+            "share_of_step": kern[dom]["share"],
+            "whole_step": {"alg_bytes_per_zone_cycle_floor": 440,
+                           "frac_of_hbm_at_floor": 440.0 * value / world / 1e9 / hbm_peak,
+                           "alg_bytes_per_zone_cycle_pipeline": sum(d["alg_bytes"] * d["launches"] for d in kern.values()) / (nz * args.steps),
+                           "frac_of_hbm_pipeline": sum(d["alg_bytes"] * d["launches"] for d in kern.values()) / (ms * 1e-3) / 1e9 / hbm_peak},
+            "kernels": {k: {"ms_avg": round(d["ms_avg"], 4), "share": round(d["share"], 4),
+                            "gbs": round(d["gbs"], 1), "launches": d["launches"]} for k, d in kern.items()}}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        subprocess.check_call(["make", "-s", "-C", os.path.join(ROOT, "oracle")])
+        steps_cpu = 3 if args.workload == "cfg2" else 2
+        v, secs, cores = cpu_oracle_time(p, gen, steps_cpu)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{steps_cpu} full steps of the same {n[0]}x{n[1]}x{n[2]} workload ({secs:.1f} s)"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "zones": nz, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "inputs (2.4 GB state) larger than L2; no flush needed", "timing": "CUDA events on the launching (torch current) stream"},
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": args.e2e_steps, "what": "hamr_set_prims(host) + hamr_step(1) + hamr_get_prims(host), pinned buffers"},
+            "gpu_launches": launches,
+            "roofline": roof, "cpu_baseline": cpu}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -130,6 +130,14 @@ int hamr_get_edge(hamr_grid* g, int f, double* out);
 int hamr_get_ctop(hamr_grid* g, double ctop[3]); /* per-direction max signal speed of the last corrector pass */
 /* conserved totals sum_zones U[c] dV, c = 0..4, of the current state */
 int hamr_totals(hamr_grid* g, double tot[5]);
+/* Per-kernel device timers.  Between hamr_profile_begin and hamr_profile_end every kernel launch on
+ * the grid's stream is bracketed by a CUDA event pair; _end synchronises and returns, per kernel
+ * class c < HAMR_NKCLASS, the summed device time ms[c] and the number of launches count[c].
+ * nclass must be >= HAMR_NKCLASS. */
+#define HAMR_NKCLASS 10
+int hamr_profile_begin(hamr_grid* g);
+int hamr_profile_end(hamr_grid* g, int nclass, double ms[], long long count[]);
+const char* hamr_profile_class_name(int c); /* "" if out of range */
 /* kernel launches issued on this grid's stream since creation */
 int hamr_launch_count(const hamr_grid* g, long long* n);
 

@@ -333,3 +333,7 @@ void orc_get_ctop(void* h, double* c3) {
 extern "C" void orc_get_fail_hist(long long h4[4]) {
   for (int c = 0; c < 4; c++) h4[c] = orc::g_fail_hist[c];
 }
+
+// number of OpenMP threads the oracle's loops use (reported by bench.py's cpu_baseline leg)
+#include <omp.h>
+extern "C" int orc_omp_threads() { return omp_get_max_threads(); }

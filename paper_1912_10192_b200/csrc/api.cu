@@ -103,6 +103,8 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   g->have_state = false;
   g->dead = false;
   g->launches = 0;
+  g->prof = false;
+  g->ev_used = 0;
   g->isn = 0; g->ish = 1; g->inew = 2;
   cudaError_t e;
   if (own) {
@@ -307,6 +309,7 @@ int hamr_grid_destroy(hamr_grid* g) {
   if (!g) return HAMR_EINVAL;
   cudaStreamSynchronize(g->stream);
   cudaFreeHost(g->h_pinned);
+  for (cudaEvent_t e : g->ev) cudaEventDestroy(e);
   if (g->own_arena) cudaFree(g->arena);
   if (g->own_stream) cudaStreamDestroy(g->stream);
   delete g;
@@ -479,6 +482,35 @@ int hamr_totals(hamr_grid* g, double tot[5]) {
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
   launch_totals(g, g->s[g->isn]);
   return read_scal(g, S_TOT0, 5, tot);
+}
+
+int hamr_profile_begin(hamr_grid* g) {
+  if (!g) return HAMR_EINVAL;
+  CK(cudaStreamSynchronize(g->stream));
+  g->ev_used = 0;
+  g->prof = true;
+  return HAMR_OK;
+}
+
+int hamr_profile_end(hamr_grid* g, int nclass, double ms[], long long count[]) {
+  if (!g || !ms || !count || nclass < NKCLASS) return HAMR_EINVAL;
+  g->prof = false;
+  CK(cudaStreamSynchronize(g->stream));
+  for (int c = 0; c < nclass; c++) { ms[c] = 0.0; count[c] = 0; }
+  for (size_t i = 0; i < g->ev_used; i++) {
+    float t = 0.f;
+    CK(cudaEventElapsedTime(&t, g->ev[2 * i], g->ev[2 * i + 1]));
+    ms[g->ev_cls[i]] += (double)t;
+    count[g->ev_cls[i]]++;
+  }
+  g->ev_used = 0;
+  return HAMR_OK;
+}
+
+const char* hamr_profile_class_name(int c) {
+  static const char* names[NKCLASS] = {"ghosts", "flux_x1", "flux_x2", "flux_x3", "centre_emf", "edge_emf",
+                                       "update_predictor", "update_corrector", "dt", "other"};
+  return (c >= 0 && c < NKCLASS) ? names[c] : "";
 }
 
 int hamr_launch_count(const hamr_grid* g, long long* n) {

@@ -101,8 +101,8 @@ __global__ void __launch_bounds__(256) k_ghosts(Dev D, Fields s, int all) {
 void launch_ghosts(hamr_grid* g, const Fields& s, bool all) {
   const Lay& L = g->D.L;
   const long long tot = (long long)L.e1 * L.e2 * (L.n[2] + 2 * NG + 1);
+  Launch l_(g, K_GHOSTS);
   k_ghosts<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s, all ? 1 : 0);
-  g->launches++;
 }
 
 }  // namespace hamr

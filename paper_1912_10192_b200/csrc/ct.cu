@@ -80,10 +80,13 @@ __global__ void __launch_bounds__(128) k_edge_emf(Dev Dv) {
 void launch_ct(hamr_grid* g, const Fields& src) {
   const Lay& L = g->D.L;
   long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 2);
-  k_centre_emf<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(g->D, src);
+  {
+    Launch l_(g, K_CEMF);
+    k_centre_emf<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(g->D, src);
+  }
   tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);
+  Launch l_(g, K_EDGE);
   k_edge_emf<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(g->D);
-  g->launches += 2;
 }
 
 }  // namespace hamr

@@ -143,11 +143,11 @@ static void launch_flux_d(hamr_grid* g, const Fields& src, bool want_ctop) {
   long long tot = 1;
   for (int d = 0; d < 3; d++) tot *= (d == D) ? L.n[d] + 1 : L.n[d] + 2;
   const unsigned nb = (unsigned)((tot + 127) / 128);
+  Launch l_(g, K_FLUX1 + D);
   if (g->D.recon == HAMR_RECON_PPM)
     k_flux<D, HAMR_RECON_PPM><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
   else
     k_flux<D, HAMR_RECON_PLM_MC><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
-  g->launches++;
 }
 
 void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop) {

@@ -108,8 +108,8 @@ __global__ void k_geometry(Dev D, double* gc, double* gf1, double* gf2, double* 
 void launch_geometry(hamr_grid* g, double* gc, double* gf1, double* gf2, double* dgc, double* rho_fl,
                      double* u_fl) {
   const int n = g->D.L.n2d;
+  Launch l_(g, K_OTHER);
   k_geometry<<<(n + 127) / 128, 128, 0, g->stream>>>(g->D, gc, gf1, gf2, dgc, rho_fl, u_fl);
-  g->launches++;
 }
 
 }  // namespace hamr

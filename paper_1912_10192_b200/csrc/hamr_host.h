@@ -1,6 +1,7 @@
 // hamr_host.h — host-side grid object and kernel launchers of libhamr (internal; product code).
 #pragma once
 #include <string>
+#include <vector>
 #include "../../include/hamr.h"
 #include "hamr_dev.cuh"
 
@@ -43,6 +44,11 @@ struct Dev {                 // everything a kernel may need, passed by value
 
 }  // namespace hamr
 
+namespace hamr {
+// kernel classes for the per-kernel timers (hamr_profile_*)
+enum KClass { K_GHOSTS = 0, K_FLUX1, K_FLUX2, K_FLUX3, K_CEMF, K_EDGE, K_UPDATE_P, K_UPDATE_C, K_DT, K_OTHER, NKCLASS };
+}
+
 struct hamr_grid {
   hamr_params par;
   hamr::Dev D;
@@ -58,7 +64,39 @@ struct hamr_grid {
   bool have_state, dead;
   long long launches;
   std::string err;
+  // per-kernel timers: CUDA event pairs on the grid's stream around every launch while enabled
+  bool prof;
+  std::vector<cudaEvent_t> ev;   // pairs: start, stop
+  std::vector<int> ev_cls;
+  size_t ev_used;
 };
+
+namespace hamr {
+// brackets one kernel launch with an event pair when profiling is on; always counts the launch
+struct Launch {
+  hamr_grid* g;
+  bool on;
+  Launch(hamr_grid* g_, int cls) : g(g_), on(g_->prof) {
+    g->launches++;
+    if (!on) return;
+    if (g->ev_used * 2 + 2 > g->ev.size()) {
+      cudaEvent_t a, b;
+      cudaEventCreate(&a);
+      cudaEventCreate(&b);
+      g->ev.push_back(a);
+      g->ev.push_back(b);
+      g->ev_cls.push_back(cls);
+    }
+    g->ev_cls[g->ev_used] = cls;
+    cudaEventRecord(g->ev[g->ev_used * 2], g->stream);
+  }
+  ~Launch() {
+    if (!on) return;
+    cudaEventRecord(g->ev[g->ev_used * 2 + 1], g->stream);
+    g->ev_used++;
+  }
+};
+}
 
 namespace hamr {
 

@@ -27,8 +27,8 @@ __global__ void k_zero_ctop(Dev Dv) {
 }
 
 void launch_dt(hamr_grid* g, int mode) {
+  Launch l_(g, K_DT);
   k_dt<<<1, 1, 0, g->stream>>>(g->D, mode);
-  g->launches++;
 }
 
 // dense (m0, m1, m2), x3 fastest  ->  padded array; zero_pole: Bf^2 on the polar axis is 0 (C-12)
@@ -54,15 +54,15 @@ void launch_pack(hamr_grid* g, const double* dense, double* padded, int stag, bo
   int m[3] = {g->D.L.n[0], g->D.L.n[1], g->D.L.n[2]};
   if (stag >= 0) m[stag] += 1;
   const long long tot = (long long)m[0] * m[1] * m[2];
+  Launch l_(g, K_OTHER);
   k_pack<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, dense, padded, m[0], m[1], m[2],
                                                                  zero_pole ? 1 : 0);
-  g->launches++;
 }
 
 void launch_unpack(hamr_grid* g, const double* padded, double* dense, const int m[3]) {
   const long long tot = (long long)m[0] * m[1] * m[2];
+  Launch l_(g, K_OTHER);
   k_unpack<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, padded, dense, m[0], m[1], m[2]);
-  g->launches++;
 }
 
 // C-11, two passes: max denominator, then max |div| / den over zones with den > 1e-12 denmax
@@ -96,10 +96,11 @@ void launch_divb(hamr_grid* g, const Fields& s) {
   const Lay& L = g->D.L;
   const long long tot = (long long)L.n[0] * L.n[1] * L.n[2];
   const unsigned nb = (unsigned)((tot + 255) / 256);
+  Launch l_(g, K_OTHER);
+  g->launches += 2;
   k_zero_scal<<<1, 1, 0, g->stream>>>(g->D, S_DENMAX, 2);
   k_divb<<<nb, 256, 0, g->stream>>>(g->D, s, 0);
   k_divb<<<nb, 256, 0, g->stream>>>(g->D, s, 1);
-  g->launches += 3;
 }
 
 // sum over active zones of U[c] dV (conservation diagnostic, P10)
@@ -131,9 +132,10 @@ __global__ void k_totals(Dev Dv, Fields s) {
 void launch_totals(hamr_grid* g, const Fields& s) {
   const Lay& L = g->D.L;
   const long long tot = (long long)L.n[0] * L.n[1] * L.n[2];
+  Launch l_(g, K_OTHER);
+  g->launches += 1;
   k_zero_scal<<<1, 1, 0, g->stream>>>(g->D, S_TOT0, 5);
   k_totals<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s);
-  g->launches += 2;
 }
 
 __global__ void k_check_finite(Dev Dv, Fields s) {
@@ -154,13 +156,13 @@ __global__ void k_check_finite(Dev Dv, Fields s) {
 void launch_check_finite(hamr_grid* g, const Fields& s) {
   const Lay& L = g->D.L;
   const long long tot = (long long)L.n[0] * L.n[1] * L.n[2];
+  Launch l_(g, K_OTHER);
   k_check_finite<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s);
-  g->launches++;
 }
 
 void launch_zero_ctop(hamr_grid* g) {
+  Launch l_(g, K_OTHER);
   k_zero_ctop<<<1, 1, 0, g->stream>>>(g->D);
-  g->launches++;
 }
 
 }  // namespace hamr

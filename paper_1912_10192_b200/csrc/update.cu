@@ -228,9 +228,9 @@ void launch_update(hamr_grid* g, const Fields& src, const Fields& base, const Fi
   const Lay& L = g->D.L;
   const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);
   const unsigned nb = (unsigned)((tot + 127) / 128);
+  Launch l_(g, src_is_base ? K_UPDATE_P : K_UPDATE_C);
   if (src_is_base) k_update<true><<<nb, 128, 0, g->stream>>>(g->D, src, base, out, dtfac);
   else k_update<false><<<nb, 128, 0, g->stream>>>(g->D, src, base, out, dtfac);
-  g->launches++;
 }
 
 }  // namespace hamr

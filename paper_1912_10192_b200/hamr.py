@@ -30,7 +30,8 @@ SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "h
            "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
            "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
            "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
-           "hamr_launch_count"]
+           "hamr_profile_begin", "hamr_profile_end", "hamr_profile_class_name", "hamr_launch_count"]
+NKCLASS = 10
 
 
 class HamrError(RuntimeError):
@@ -87,8 +88,12 @@ def lib():
         L.hamr_get_ctop.argtypes = [vp, c_double_p]
         L.hamr_totals.argtypes = [vp, c_double_p]
         L.hamr_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.hamr_profile_begin.argtypes = [vp]
+        L.hamr_profile_end.argtypes = [vp, C.c_int, c_double_p, C.POINTER(C.c_longlong)]
+        L.hamr_profile_class_name.argtypes = [C.c_int]
+        L.hamr_profile_class_name.restype = C.c_char_p
         for s in SYMBOLS:
-            if s != "hamr_last_error":
+            if s not in ("hamr_last_error", "hamr_profile_class_name"):
                 getattr(L, s).restype = C.c_int
         _LIB = L
     return _LIB
@@ -282,6 +287,16 @@ class Grid:
         t = np.zeros(5)
         self._ck(self.L.hamr_totals(self.h, _dp(t)))
         return t
+
+    def profile_begin(self):
+        self._ck(self.L.hamr_profile_begin(self.h))
+
+    def profile_end(self):
+        """{kernel class: (summed device ms, launches)} since profile_begin"""
+        ms = (C.c_double * NKCLASS)()
+        cnt = (C.c_longlong * NKCLASS)()
+        self._ck(self.L.hamr_profile_end(self.h, NKCLASS, ms, cnt))
+        return {self.L.hamr_profile_class_name(c).decode(): (ms[c], cnt[c]) for c in range(NKCLASS)}
 
     def launch_count(self):
         n = C.c_longlong(0)
