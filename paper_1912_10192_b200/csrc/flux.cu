@@ -5,131 +5,229 @@
 // field from the staggered face B, U/F of both states (C-4), fast-speed bounds (C-6), HLL flux of
 // the 5 hydro rows and the 2 transverse-B rows (= face EMFs, C-7/C-8), and the per-direction
 // maximum signal speed for the Courant step (C-14).
+//
+// The kernels are bound by the FP64 pipe (64 lanes per SM), not by HBM, so the
+// design minimises fp64 instructions per face:
+//  * every zone's parabola is built ONCE and shared by its two faces: along x1 / x2 a thread
+//    marches along the sweep direction carrying the previous zone's right edge in registers (loads
+//    stay coalesced along x3); along x3 neighbouring lanes exchange the edge with a warp shuffle;
+//  * reconstruction is branch-free (selects, no divergence), divisions by constants are
+//    multiplications, each state needs 3 reciprocals and 2 square roots in total.
 #include "hamr_host.h"
 
 namespace hamr {
 
-// HLL for one row
-__device__ __forceinline__ double hll1(double UL, double UR, double FL, double FR, double cmin, double cmax,
-                                       double cc, double isum, bool avg) {
-  return avg ? 0.5 * (FL + FR) : (cmax * FL + cmin * FR - cc * (UR - UL)) * isum;
+constexpr double SIXTH = 1.0 / 6.0;
+
+// ---- C-5 reconstruction, branch-free ----------------------------------------------------------------
+// van Leer / CW84 limited slope from dl = a_j - a_{j-1}, dr = a_{j+1} - a_j, dc = (a_{j+1} - a_{j-1})/2
+__device__ __forceinline__ double lim_slope(double dl, double dr, double dc) {
+  const double lim = dmin(fabs(dc), 2.0 * dmin(fabs(dl), fabs(dr)));
+  return (dl * dr > 0.0) ? copysign(lim, dc) : 0.0;
 }
 
-// Physics of one face along direction D (0..2) from the two reconstructed states.
-// Fh[0..4]: hydro flux; EA = E_e, EB = E_f on the face with (D, e, f) cyclic; returns ctop.
+// parabola edges (aL at j-1/2, aR at j+1/2) of zone j from a0..a4 = a[j-2..j+2]
+__device__ __forceinline__ void ppm_edges(double a0, double a1, double a2, double a3, double a4, double& aL,
+                                          double& aR) {
+  const double d10 = a1 - a0, d21 = a2 - a1, d32 = a3 - a2, d43 = a4 - a3;
+  const double dm_m = lim_slope(d10, d21, 0.5 * (a2 - a0));
+  const double dm_0 = lim_slope(d21, d32, 0.5 * (a3 - a1));
+  const double dm_p = lim_slope(d32, d43, 0.5 * (a4 - a2));
+  double l = a1 + 0.5 * d21 - (dm_0 - dm_m) * SIXTH;
+  double r = a2 + 0.5 * d32 - (dm_p - dm_0) * SIXTH;
+  // monotonise
+  const bool flat = (r - a2) * (a2 - l) <= 0.0;
+  const double d = r - l;
+  const double c = a2 - 0.5 * (l + r);
+  const double dc = d * c, dd6 = d * d * SIXTH;
+  const bool over = dc > dd6, under = dc < -dd6;
+  const double nl = 3.0 * a2 - 2.0 * r, nr = 3.0 * a2 - 2.0 * l;
+  aL = flat ? a2 : (over ? nl : l);
+  aR = flat ? a2 : ((!over && under) ? nr : r);
+}
+
+// PLM with the MC limiter: minmod(2(a1-a0), (a2-a0)/2, 2(a2-a1))
+__device__ __forceinline__ void plm_edges(double a0, double a1, double a2, double& aL, double& aR) {
+  const double s = lim_slope(a1 - a0, a2 - a1, 0.5 * (a2 - a0));
+  aL = a1 - 0.5 * s;
+  aR = a1 + 0.5 * s;
+}
+
+template <int RECON>
+__device__ __forceinline__ void zone_edges(const double* __restrict__ a, int sd, double& aL, double& aR) {
+  if (RECON == HAMR_RECON_PPM) ppm_edges(a[-2 * sd], a[-sd], a[0], a[sd], a[2 * sd], aL, aR);
+  else plm_edges(a[-sd], a[0], a[sd], aL, aR);
+}
+
+// ---- C-2..C-7 on one face ------------------------------------------------------------------------------
+// the subset of the face geometry the flux needs
+struct FGeo {
+  double c00, c01, c03, c11, c13, c22, c33;  // g_{mu nu}
+  double k00, kdd, k0d;                      // g^{tt}, g^{dd}, g^{td}
+  double gdet, igdet, ialpha, boa;
+};
+
 template <int D>
-__device__ __forceinline__ double face_physics(const double PL[8], const double PR[8], const Geo& G,
-                                               double gam_ad, double Fh[5], double& EA, double& EB) {
+__device__ __forceinline__ FGeo load_fgeo(const double* __restrict__ tab, int n2d, int q) {
+  FGeo G;
+  G.c00 = __ldg(tab + C00 * n2d + q); G.c01 = __ldg(tab + C01 * n2d + q);
+  G.c03 = __ldg(tab + C03 * n2d + q); G.c11 = __ldg(tab + C11 * n2d + q);
+  G.c13 = __ldg(tab + C13 * n2d + q); G.c22 = __ldg(tab + C22 * n2d + q);
+  G.c33 = __ldg(tab + C33 * n2d + q);
+  G.k00 = __ldg(tab + K00 * n2d + q);
+  G.kdd = __ldg(tab + (D == 0 ? K11 : (D == 1 ? K22 : K33)) * n2d + q);
+  G.k0d = (D == 0) ? __ldg(tab + K01 * n2d + q) : 0.0;  // g^{t2} = g^{t3} = 0 for both metrics
+  G.gdet = __ldg(tab + GDET * n2d + q); G.igdet = __ldg(tab + IGDET * n2d + q);
+  G.ialpha = __ldg(tab + IALPHA * n2d + q); G.boa = __ldg(tab + BOA * n2d + q);
+  return G;
+}
+
+// one side of the face: U and F rows (without the sqrt(-g) factor, applied after HLL) and speed bounds
+template <int D>
+__device__ __forceinline__ void side_state(const double P[8], const FGeo& G, double gam_ad, double U[7],
+                                           double F[7], double& vmin, double& vmax) {
   constexpr int dir = D + 1, e = (D + 1) % 3, f = (D + 2) % 3;
-  const double A = (D == 0) ? G.k11 : (D == 1 ? G.k22 : G.k33);
-  const double Cq = (D == 0) ? G.k01 : 0.0;
-  double UL[7], UR[7], FL[7], FR[7];
-  double vminL, vmaxL, vminR, vmaxR;
+  // C-2
+  const double q = G.c11 * P[2] * P[2] + G.c22 * P[3] * P[3] + G.c33 * P[4] * P[4] + 2.0 * (G.c13 * P[2] * P[4]);
+  const double gam = sqrt(1.0 + q);
+  double u[4], ul[4], b[4], bl[4];
+  u[0] = gam * G.ialpha;
+  u[1] = P[2] - gam * G.boa;
+  u[2] = P[3];
+  u[3] = P[4];
+  ul[0] = G.c00 * u[0] + G.c01 * u[1] + G.c03 * u[3];
+  ul[1] = G.c01 * u[0] + G.c11 * u[1] + G.c13 * u[3];
+  ul[2] = G.c22 * u[2];
+  ul[3] = G.c03 * u[0] + G.c13 * u[1] + G.c33 * u[3];
+  // C-3
+  b[0] = P[5] * ul[1] + P[6] * ul[2] + P[7] * ul[3];
+  const double iut = 1.0 / u[0];
+  b[1] = (P[5] + b[0] * u[1]) * iut;
+  b[2] = (P[6] + b[0] * u[2]) * iut;
+  b[3] = (P[7] + b[0] * u[3]) * iut;
+  bl[0] = G.c00 * b[0] + G.c01 * b[1] + G.c03 * b[3];
+  bl[1] = G.c01 * b[0] + G.c11 * b[1] + G.c13 * b[3];
+  bl[2] = G.c22 * b[2];
+  bl[3] = G.c03 * b[0] + G.c13 * b[1] + G.c33 * b[3];
+  const double bsq = b[0] * bl[0] + b[1] * bl[1] + b[2] * bl[2] + b[3] * bl[3];
+  // C-4
+  const double p = (gam_ad - 1.0) * P[1];
+  const double w = P[0] + P[1] + p;
+  const double eta = w + bsq;
+  const double ptot = p + 0.5 * bsq;
+  const double eu0 = eta * u[0], eud = eta * u[dir];
+  const double Dn = P[0] * u[0], m = P[0] * u[dir];
+  U[0] = Dn;
+  U[1] = eu0 * ul[0] + ptot - b[0] * bl[0] + Dn;
+  F[0] = m;
+  F[1] = eud * ul[0] - b[dir] * bl[0] + m;
 #pragma unroll
-  for (int side = 0; side < 2; side++) {
-    const double* P = side ? PR : PL;
-    double* U = side ? UR : UL;
-    double* F = side ? FR : FL;
-    St S;
-    get_state(P, G, S);
-    const double p = (gam_ad - 1.0) * P[1];
-    const double eta = P[0] + P[1] + p + S.bsq;
-    const double ptot = p + 0.5 * S.bsq;
-    const double eu0 = eta * S.ucon[0], eud = eta * S.ucon[dir];
-    const double b0 = S.bcon[0], bd = S.bcon[dir];
-    const double Dn = P[0] * S.ucon[0], m = P[0] * S.ucon[dir];
-    U[0] = G.gdet * Dn;
-    U[1] = G.gdet * (eu0 * S.ucov[0] + ptot - b0 * S.bcov[0] + Dn);
-    F[0] = G.gdet * m;
-    F[1] = G.gdet * (eud * S.ucov[0] - bd * S.bcov[0] + m);
-#pragma unroll
-    for (int c = 1; c < 4; c++) {
-      U[1 + c] = G.gdet * (eu0 * S.ucov[c] - b0 * S.bcov[c]);
-      F[1 + c] = G.gdet * (eud * S.ucov[c] + (c == dir ? ptot : 0.0) - bd * S.bcov[c]);
-    }
-    // transverse field rows: U = g B^i, F = g (b^i u^d - b^d u^i)
-    U[5] = G.gdet * P[5 + e];
-    U[6] = G.gdet * P[5 + f];
-    F[5] = G.gdet * (S.bcon[1 + e] * S.ucon[dir] - bd * S.ucon[1 + e]);
-    F[6] = G.gdet * (S.bcon[1 + f] * S.ucon[dir] - bd * S.ucon[1 + f]);
-    wavespeeds(P, S, gam_ad, A, G.k00, Cq, dir, side ? vminR : vminL, side ? vmaxR : vmaxL);
+  for (int c = 1; c < 4; c++) {
+    U[1 + c] = eu0 * ul[c] - b[0] * bl[c];
+    F[1 + c] = eud * ul[c] + (c == dir ? ptot : 0.0) - b[dir] * bl[c];
   }
-  const double cmax = fmax(0.0, fmax(vmaxL, vmaxR));
-  const double cmin = fmax(0.0, fmax(-vminL, -vminR));
+  U[5] = P[5 + e];
+  U[6] = P[5 + f];
+  F[5] = b[1 + e] * u[dir] - b[dir] * u[1 + e];
+  F[6] = b[1 + f] * u[dir] - b[dir] * u[1 + f];
+  // C-6: c_m^2 = c_s^2 + v_A^2 - c_s^2 v_A^2 with c_s^2 = gamma p / w, v_A^2 = b^2 / (b^2 + w)
+  const double gp = gam_ad * p;
+  double cm2 = (gp * eta + bsq * (w - gp)) / (w * eta);
+  cm2 = dmin(dmax(cm2, 0.0), 1.0);
+  const double ut2 = u[0] * u[0], udt = u[dir] * u[0], ud2 = u[dir] * u[dir];
+  const double a2 = ut2 - (G.k00 + ut2) * cm2;
+  const double a1 = 2.0 * (udt - (G.k0d + udt) * cm2);
+  const double a0 = ud2 - (G.kdd + ud2) * cm2;
+  const double disc = sqrt(dmax(a1 * a1 - 4.0 * a2 * a0, 0.0));
+  const double i2 = 1.0 / (2.0 * a2);
+  const double v1 = (a1 + disc) * i2, v2 = (a1 - disc) * i2;
+  vmax = dmax(v1, v2);
+  vmin = dmin(v1, v2);
+}
+
+// HLL (C-7) from the two states; writes the 7 outputs of the face; returns ctop
+template <int D>
+__device__ __forceinline__ double face_flux(const double PL[8], const double PR[8], const FGeo& G, double gam_ad,
+                                            const Dev& Dv, int z) {
+  double UL[7], UR[7], FL[7], FR[7], vminL, vmaxL, vminR, vmaxR;
+  side_state<D>(PL, G, gam_ad, UL, FL, vminL, vmaxL);
+  side_state<D>(PR, G, gam_ad, UR, FR, vminR, vmaxR);
+  const double cmax = dmax(0.0, dmax(vmaxL, vmaxR));
+  const double cmin = dmax(0.0, dmax(-vminL, -vminR));
   const double sum = cmax + cmin;
   const bool avg = sum < 1e-300;
   const double isum = avg ? 0.0 : 1.0 / sum;
-  const double cc = cmax * cmin;
+  // F = g [cmax FL + cmin FR - cmax cmin (UR - UL)] / (cmax + cmin);  average if both speeds vanish
+  const double wl = avg ? 0.5 * G.gdet : cmax * isum * G.gdet;
+  const double wr = avg ? 0.5 * G.gdet : cmin * isum * G.gdet;
+  const double wc = avg ? 0.0 : cmax * cmin * isum * G.gdet;
+  double Fh[7];
 #pragma unroll
-  for (int c = 0; c < 5; c++) Fh[c] = hll1(UL[c], UR[c], FL[c], FR[c], cmin, cmax, cc, isum, avg);
-  const double Fe = hll1(UL[5], UR[5], FL[5], FR[5], cmin, cmax, cc, isum, avg);
-  const double Ff = hll1(UL[6], UR[6], FL[6], FR[6], cmin, cmax, cc, isum, avg);
-  if (!avg) {
-    // C-7a: a mass flux below 1e-12 of the magnitude of its own HLL terms is rounding noise and is
-    // flushed to exactly 0, so that the upwind selector of C-9 sees a tie
-    const double mag = (cmax * fabs(FL[0]) + cmin * fabs(FR[0]) + cc * (fabs(UR[0]) + fabs(UL[0]))) * isum;
-    if (fabs(Fh[0]) <= 1e-12 * mag) Fh[0] = 0.0;
-  }
-  EB = -Fe;  // C-8: on a d-face, E_f = -F^d(B^e)
-  EA = Ff;   //                    E_e = +F^d(B^f)
-  return fmax(cmax, cmin);
+  for (int c = 0; c < 7; c++) Fh[c] = wl * FL[c] + wr * FR[c] - wc * (UR[c] - UL[c]);
+  // C-7a: a mass flux below 1e-12 of the magnitude of its own HLL terms is rounding noise and is
+  // flushed to exactly 0, so that the upwind selector of C-9 sees a tie
+  const double mag = wl * fabs(FL[0]) + wr * fabs(FR[0]) + wc * (fabs(UR[0]) + fabs(UL[0]));
+  if (!avg && fabs(Fh[0]) <= 1e-12 * mag) Fh[0] = 0.0;
+#pragma unroll
+  for (int c = 0; c < 5; c++) Dv.F[D][c][z] = Fh[c];
+  Dv.EfB[D][z] = -Fh[5];  // C-8: on a d-face, E_f = -F^d(B^e)
+  Dv.EfA[D][z] = Fh[6];   //                    E_e = +F^d(B^f)
+  return dmax(cmax, cmin);
 }
 
-// v1: one thread per face, stencil read straight from global memory (L1/L2 catch the reuse).
+__device__ __forceinline__ void zero_face(const Dev& Dv, int D, int z) {
+  for (int c = 0; c < 5; c++) Dv.F[D][c][z] = 0.0;
+  Dv.EfA[D][z] = 0.0;
+  Dv.EfB[D][z] = 0.0;
+}
+
+// ---- sweeps along x1 / x2: a thread marches along the sweep direction ---------------------------------
+// grid.x covers the flattened transverse index (other, k), k fastest; grid.y the segments of SEG faces.
+constexpr int SEG = 16;
+
 template <int D, int RECON>
-__global__ void __launch_bounds__(128) k_flux(Dev Dv, Fields s, int want_ctop) {
+__global__ void __launch_bounds__(128) k_flux_march(Dev Dv, Fields s, int want_ctop) {
+  static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   const Lay& L = Dv.L;
+  constexpr int O = 1 - D;          // the other non-x3 dimension
   constexpr int e = (D + 1) % 3, f = (D + 2) % 3;
-  // box of faces: 0..n along D, one transverse ghost layer on each side (needed by CT)
-  int lo[3] = {-1, -1, -1}, cntd[3];
-  lo[D] = 0;
-  for (int d = 0; d < 3; d++) cntd[d] = (d == D) ? L.n[d] + 1 : L.n[d] + 2;
-  const long long tot = (long long)cntd[0] * cntd[1] * cntd[2];
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int ck = L.n[2] + 2;
+  const int tf = blockIdx.x * blockDim.x + threadIdx.x;
   double ctop = 0.0;
-  if (t < tot) {
-    const int k = (int)(t % cntd[2]) + lo[2];
-    const int j = (int)((t / cntd[2]) % cntd[1]) + lo[1];
-    const int i = (int)(t / ((long long)cntd[2] * cntd[1])) + lo[0];
-    const long long z = L.idx(i, j, k);
-    const int q = L.idx2(i, j);
-    const bool pole = (D == 1) && Dv.metric == HAMR_METRIC_KERR_SCHILD && (j == 0 || j == L.n[1]);
-    double Fh[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, EA = 0.0, EB = 0.0;
-    if (!pole) {  // C-7: pole faces carry no flux and no state is evaluated there
-      const Geo G = load_geo(D == 0 ? Dv.gf1 : (D == 1 ? Dv.gf2 : Dv.gc), L.n2d, q);
-      const long long sd = (D == 0) ? L.S1 : (D == 1 ? L.S2 : 1);
-      double PL[8], PR[8];
-      const double* var[7] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[e], s.Bc[f]};
-      const int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
+  if (tf < (L.n[O] + 2) * ck) {
+    const int k = tf % ck - 1, o = tf / ck - 1;
+    const int f0 = blockIdx.y * SEG, f1 = min(f0 + SEG, L.n[D] + 1);
+    const int sd = (D == 0) ? L.S1 : L.S2;
+    const bool act = o >= 0 && o < L.n[O] && k >= 0 && k < L.n[2];  // C-14: faces of ACTIVE zones
+    const bool ks = Dv.metric == HAMR_METRIC_KERR_SCHILD;
+    const double* var[7] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[e], s.Bc[f]};
+    constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
+    int z = (int)L.idx(D == 0 ? f0 - 1 : o, D == 0 ? o : f0 - 1, k);
+    double PL[8], PR[8];
+    // right edges of the zone below the first face
 #pragma unroll
-      for (int v = 0; v < 7; v++) {
-        const double* a = var[v] + z;
-        double aL, aR, dummy;
-        if (RECON == HAMR_RECON_PPM) {
-          const double m3 = a[-3 * sd], m2 = a[-2 * sd], m1 = a[-sd], c0 = a[0], p1 = a[sd], p2 = a[2 * sd];
-          ppm_zone(m3, m2, m1, c0, p1, dummy, aR);  // left of the face: a_R of zone j-1
-          ppm_zone(m2, m1, c0, p1, p2, aL, dummy);  // right of the face: a_L of zone j
-        } else {
-          const double m2 = a[-2 * sd], m1 = a[-sd], c0 = a[0], p1 = a[sd];
-          plm_zone(m2, m1, c0, dummy, aR);
-          plm_zone(m1, c0, p1, aL, dummy);
-        }
-        PL[slot[v]] = aR;
-        PR[slot[v]] = aL;
-      }
-      PL[5 + D] = PR[5 + D] = s.Bf[D][z] / G.gdet;  // C-5: the normal field is single-valued at the face
-      const double ct = face_physics<D>(PL, PR, G, Dv.gam, Fh, EA, EB);
-      // C-14: the Courant maximum runs over the faces of ACTIVE zones
-      const int id[3] = {i, j, k};
-      bool act = true;
-      for (int d = 0; d < 3; d++)
-        if (d != D && (id[d] < 0 || id[d] >= L.n[d])) act = false;
-      if (act) ctop = ct;
+    for (int v = 0; v < 7; v++) {
+      double aL;
+      zone_edges<RECON>(var[v] + z, sd, aL, PL[slot[v]]);
     }
+    for (int fc = f0; fc < f1; fc++) {
+      z += sd;
+      double carry[7];
 #pragma unroll
-    for (int c = 0; c < 5; c++) Dv.F[D][c][z] = Fh[c];
-    Dv.EfA[D][z] = EA;
-    Dv.EfB[D][z] = EB;
+      for (int v = 0; v < 7; v++) zone_edges<RECON>(var[v] + z, sd, PR[slot[v]], carry[v]);
+      const bool pole = (D == 1) && ks && (fc == 0 || fc == L.n[1]);
+      if (pole) {  // C-7: pole faces carry no flux and no state is evaluated there
+        zero_face(Dv, D, z);
+      } else {
+        const int q = (D == 0) ? L.idx2(fc, o) : L.idx2(o, fc);
+        const FGeo G = load_fgeo<D>(D == 0 ? Dv.gf1 : Dv.gf2, L.n2d, q);
+        PL[5 + D] = PR[5 + D] = s.Bf[D][z] * G.igdet;  // C-5: the normal field is single-valued at the face
+        const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
+        if (act) ctop = dmax(ctop, ct);
+      }
+#pragma unroll
+      for (int v = 0; v < 7; v++) PL[slot[v]] = carry[v];
+    }
   }
   if (want_ctop) {
     ctop = warp_max(ctop);
@@ -137,23 +235,70 @@ __global__ void __launch_bounds__(128) k_flux(Dev Dv, Fields s, int want_ctop) {
   }
 }
 
+// ---- sweep along x3: one lane per zone, the right edge comes from the neighbouring lane ---------------
+// Zones (i, j, k) with i, j in [-1, n], k in [-1, n3] are flattened with k fastest; a warp owns 31
+// consecutive zones plus one leading helper zone that only supplies its right edges.
+template <int RECON>
+__global__ void __launch_bounds__(128) k_flux_x3(Dev Dv, Fields s, int want_ctop) {
+  constexpr int D = 2;
+  const Lay& L = Dv.L;
+  const int ck = L.n[2] + 2, cj = L.n[1] + 2;
+  const long long tot = (long long)(L.n[0] + 2) * cj * ck;
+  const int lane = threadIdx.x & 31;
+  const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  long long t = warp * 31 + lane - 1;
+  const bool valid = t >= 0 && t < tot;
+  t = t < 0 ? 0 : (t >= tot ? tot - 1 : t);  // clamped lanes compute on a real zone and store nothing
+  const int k = (int)(t % ck) - 1;
+  const int j = (int)((t / ck) % cj) - 1;
+  const int i = (int)(t / ((long long)ck * cj)) - 1;
+  const int z = (int)L.idx(i, j, k);
+  const double* var[7] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[0], s.Bc[1]};
+  double PL[8], PR[8];
+#pragma unroll
+  for (int v = 0; v < 7; v++) {
+    double aR;
+    zone_edges<RECON>(var[v] + z, 1, PR[v], aR);
+    PL[v] = __shfl_up_sync(0xffffffffu, aR, 1);  // right edge of zone k-1 = left state of face k-1/2
+  }
+  double ctop = 0.0;
+  if (valid && lane > 0 && k >= 0) {
+    const FGeo G = load_fgeo<D>(Dv.gc, L.n2d, L.idx2(i, j));
+    PL[7] = PR[7] = s.Bf[2][z] * G.igdet;
+    const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
+    if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct;
+  }
+  if (want_ctop) {
+    ctop = warp_max(ctop);
+    if (lane == 0 && ctop > 0.0) atomic_max_pos(Dv.scal + S_CTOP0 + D, ctop);
+  }
+}
+
 template <int D>
-static void launch_flux_d(hamr_grid* g, const Fields& src, bool want_ctop) {
+static void launch_march(hamr_grid* g, const Fields& src, bool want_ctop) {
   const Lay& L = g->D.L;
-  long long tot = 1;
-  for (int d = 0; d < 3; d++) tot *= (d == D) ? L.n[d] + 1 : L.n[d] + 2;
-  const unsigned nb = (unsigned)((tot + 127) / 128);
+  const int O = 1 - D;
+  const int ntr = (L.n[O] + 2) * (L.n[2] + 2);
+  dim3 grid((ntr + 127) / 128, (L.n[D] + 1 + SEG - 1) / SEG);
   Launch l_(g, K_FLUX1 + D);
   if (g->D.recon == HAMR_RECON_PPM)
-    k_flux<D, HAMR_RECON_PPM><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
+    k_flux_march<D, HAMR_RECON_PPM><<<grid, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
   else
-    k_flux<D, HAMR_RECON_PLM_MC><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
+    k_flux_march<D, HAMR_RECON_PLM_MC><<<grid, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
 }
 
 void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop) {
-  launch_flux_d<0>(g, src, want_ctop);
-  launch_flux_d<1>(g, src, want_ctop);
-  launch_flux_d<2>(g, src, want_ctop);
+  launch_march<0>(g, src, want_ctop);
+  launch_march<1>(g, src, want_ctop);
+  const Lay& L = g->D.L;
+  const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 2);
+  const long long warps = (tot + 30) / 31 + 1;
+  const unsigned nb = (unsigned)((warps + 3) / 4);
+  Launch l_(g, K_FLUX3);
+  if (g->D.recon == HAMR_RECON_PPM)
+    k_flux_x3<HAMR_RECON_PPM><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
+  else
+    k_flux_x3<HAMR_RECON_PLM_MC><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
 }
 
 }  // namespace hamr

@@ -75,6 +75,7 @@ __device__ static void store_geo(double* tab, int n2d, int q, const Geo& G) {
   tab[K13 * n2d + q] = G.k13; tab[K22 * n2d + q] = G.k22; tab[K33 * n2d + q] = G.k33;
   tab[GDET * n2d + q] = G.gdet; tab[ALPHA * n2d + q] = G.alpha; tab[IALPHA * n2d + q] = G.ialpha;
   tab[BOA * n2d + q] = G.boa;
+  tab[IGDET * n2d + q] = G.gdet > 0.0 ? 1.0 / G.gdet : 0.0;
 }
 
 __global__ void k_geometry(Dev D, double* gc, double* gf1, double* gf2, double* dgc, double* rho_fl,

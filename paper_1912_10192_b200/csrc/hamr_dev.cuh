@@ -42,6 +42,7 @@ enum GeoComp {
   C00 = 0, C01, C03, C11, C13, C22, C33,  // covariant metric
   K00, K01, K11, K13, K22, K33,           // contravariant metric
   GDET, ALPHA, IALPHA, BOA,               // sqrt(-g), lapse, 1/lapse, beta^1/lapse
+  IGDET,                                  // 1/sqrt(-g) (0 on the polar axis)
   NGEO
 };
 // centre-only extras: x1- and x2-derivatives of the 7 covariant components (for the source, C-12)
@@ -50,7 +51,7 @@ enum DgComp { D00 = 0, D01, D03, D11, D13, D22, D33, NDG };
 struct Geo {
   double c00, c01, c03, c11, c13, c22, c33;
   double k00, k01, k11, k13, k22, k33;
-  double gdet, alpha, ialpha, boa;
+  double gdet, alpha, ialpha, boa, igdet;
 };
 
 __device__ __forceinline__ Geo load_geo(const double* __restrict__ tab, int n2d, int q) {
@@ -64,6 +65,7 @@ __device__ __forceinline__ Geo load_geo(const double* __restrict__ tab, int n2d,
   G.k22 = __ldg(tab + K22 * n2d + q); G.k33 = __ldg(tab + K33 * n2d + q);
   G.gdet = __ldg(tab + GDET * n2d + q); G.alpha = __ldg(tab + ALPHA * n2d + q);
   G.ialpha = __ldg(tab + IALPHA * n2d + q); G.boa = __ldg(tab + BOA * n2d + q);
+  G.igdet = __ldg(tab + IGDET * n2d + q);
   return G;
 }
 
@@ -183,6 +185,10 @@ __device__ __forceinline__ void plm_zone(double a0, double a1, double a2, double
 __device__ __forceinline__ void atomic_max_pos(double* addr, double v) {
   atomicMax(reinterpret_cast<unsigned long long*>(addr), (unsigned long long)__double_as_longlong(v));
 }
+
+// plain compare-select min / max (no NaN special-casing, unlike fmin / fmax)
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 
 __device__ __forceinline__ double warp_max(double v) {
 #pragma unroll
