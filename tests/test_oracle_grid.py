@@ -2,7 +2,20 @@
 import numpy as np
 import pytest
 
+import os
+
 from paper_1912_10192_b200 import inputs as I
+
+
+def _golden(name):
+    """name -> value pairs of a text fixture under tests/golden/ (each file cites its source)"""
+    out = {}
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()
+                out[k] = float(v)
+    return out
 
 
 def run_to(g, T):
@@ -97,9 +110,9 @@ def test_p9_p10_conservation_and_divb_minkowski(orc):
 # ---- P11: second-order convergence of linear fast + Alfven waves -------------------------------------------
 def test_p11_phase_speeds_closed_form():
     em = I.flat_eigenmodes()
-    assert np.isclose(em["fast"][0], 0.6620283526406386, rtol=1e-13)
-    assert np.isclose(em["alfven"][0], 0.5857789663852442, rtol=1e-13)
-    assert np.isclose(em["slow"][0], 0.45692145405745066, rtol=1e-13)
+    gold = _golden("cfg1_wave_speeds.txt")
+    for name in ("fast", "alfven", "slow"):
+        assert np.isclose(em[name][0], gold[name], rtol=1e-13), name
     # Alfven mode is incompressible and transverse
     r = em["alfven"][1]
     assert abs(r[0]) < 1e-12 and abs(r[1]) < 1e-12 and abs(r[2:5].sum()) < 1e-12 and abs(r[5:8].sum()) < 1e-12
@@ -132,9 +145,10 @@ def test_p11_linear_wave_convergence(orc, modes):
 def test_p12_fm_initial_data_identities():
     a, gam = 0.9375, 13.0 / 9.0
     rho, u, ut, uphi, inside, info = I.fm_torus_point(a, gam, np.array([12.0, 9.3]), np.array([np.pi / 2, 1.45]))
-    assert np.isclose(info["l"], 4.28128446853189, rtol=1e-13)
-    assert np.isclose(info["hmax"] - 1, 0.0169982893680827, rtol=1e-11)
-    assert np.isclose(info["rho_max"], 41.36891956734738, rtol=1e-10)
+    gold = _golden("fm_torus_constants.txt")
+    assert np.isclose(info["l"], gold["l"], rtol=1e-13)
+    assert np.isclose(info["hmax"] - 1, gold["hmax_m1"], rtol=1e-11)
+    assert np.isclose(info["rho_max"], gold["rho_max"], rtol=1e-10)
     assert np.isclose(rho[0], 1.0, rtol=1e-12) and inside.all()
     # u^t u_phi = l everywhere in the torus (constant angular momentum), checked in KS
     g = I.ks_gcov(a, np.array([9.3]), np.array([1.45]))[0]
