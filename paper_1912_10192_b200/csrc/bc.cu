@@ -51,17 +51,10 @@ __device__ __forceinline__ double ghost_value(const Dev& D, const double* __rest
   return neg ? -v : v;
 }
 
-// One thread per padded location.  Writes ghost P, ghost Bf and Bc of ghost zones (of all zones if
-// `all` is set: used once for the initial state).
-__global__ void __launch_bounds__(256) k_ghosts(Dev D, Fields s, int all) {
+// One padded location (i,j,k).  Writes ghost P, ghost Bf and Bc of ghost zones (of all zones if `all`
+// is set: used once for the initial state).
+__device__ __forceinline__ void ghost_cell(const Dev& D, const Fields& s, int all, int i, int j, int k) {
   const Lay& L = D.L;
-  const int e3 = L.n[2] + 2 * NG + 1;
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long tot = (long long)L.e1 * L.e2 * e3;
-  if (t >= tot) return;
-  const int k = (int)(t % e3) - NG;
-  const int j = (int)((t / e3) % L.e2) - NG;
-  const int i = (int)(t / ((long long)e3 * L.e2)) - NG;
   const int id[3] = {i, j, k};
   bool in_c[3], extra[3];
   for (int d = 0; d < 3; d++) {
@@ -98,11 +91,68 @@ __global__ void __launch_bounds__(256) k_ghosts(Dev D, Fields s, int all) {
   }
 }
 
+// every padded location (initial state; grids with a reflecting x1 or x3 wall)
+__global__ void __launch_bounds__(256) k_ghosts(Dev D, Fields s, int all) {
+  const Lay& L = D.L;
+  const int e3 = L.n[2] + 2 * NG + 1;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long tot = (long long)L.e1 * L.e2 * e3;
+  if (t >= tot) return;
+  ghost_cell(D, s, all, (int)(t / ((long long)e3 * L.e2)) - NG, (int)((t / e3) % L.e2) - NG, (int)(t % e3) - NG);
+}
+
+// The ghost shell only (the per-stage fill; ~12 % of the padded grid for cfg 2):
+//  part A: (i,j) columns with i or j outside the active range (plus the j = 0 wall row of a reflecting
+//          axis): every k;   part B: active (i,j) columns: the 2 NG + 1 ghost slots in k.
+__global__ void __launch_bounds__(256) k_ghosts_shell(Dev D, Fields s, int nj, long long nA) {
+  const Lay& L = D.L;
+  const int e3 = L.n[2] + 2 * NG + 1;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < nA) {
+    const int k = (int)(t % e3) - NG;
+    long long row = t / e3;
+    int i, j;
+    const long long lo_rows = (long long)NG * L.e2, mid_rows = (long long)L.n[0] * nj;
+    if (row < lo_rows) {
+      i = (int)(row / L.e2) - NG; j = (int)(row % L.e2) - NG;
+    } else if (row < lo_rows + mid_rows) {
+      row -= lo_rows;
+      i = (int)(row / nj);
+      const int q = (int)(row % nj);  // -3, -2, -1, [0,] n2 .. n2 + 3
+      j = q < NG ? q - NG : (nj == 2 * NG + 2 ? (q == NG ? 0 : L.n[1] + q - NG - 1) : L.n[1] + q - NG);
+    } else {
+      row -= lo_rows + mid_rows;
+      i = L.n[0] + (int)(row / L.e2); j = (int)(row % L.e2) - NG;
+    }
+    ghost_cell(D, s, 0, i, j, k);
+    return;
+  }
+  const long long u = t - nA;
+  const long long nB = (long long)L.n[0] * L.n[1] * 8;
+  if (u >= nB) return;
+  const int q = (int)(u & 7);
+  if (q == 7) return;
+  const long long col = u >> 3;
+  const int i = (int)(col / L.n[1]), j = (int)(col % L.n[1]);
+  if (nj == 2 * NG + 2 && j == 0) return;  // the wall row was done in part A
+  const int k = q < NG ? q - NG : L.n[2] + q - NG;
+  ghost_cell(D, s, 0, i, j, k);
+}
+
 void launch_ghosts(hamr_grid* g, const Fields& s, bool all) {
   const Lay& L = g->D.L;
-  const long long tot = (long long)L.e1 * L.e2 * (L.n[2] + 2 * NG + 1);
+  const int e3 = L.n[2] + 2 * NG + 1;
   Launch l_(g, K_GHOSTS);
-  k_ghosts<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s, all ? 1 : 0);
+  if (all || g->D.bc_lo[0] == HAMR_BC_POLAR_REFLECT || g->D.bc_lo[2] == HAMR_BC_POLAR_REFLECT) {
+    const long long tot = (long long)L.e1 * L.e2 * e3;
+    k_ghosts<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s, all ? 1 : 0);
+    return;
+  }
+  const int nj = 2 * NG + 1 + (g->D.bc_lo[1] == HAMR_BC_POLAR_REFLECT ? 1 : 0);
+  const long long rows = (long long)(2 * NG + 1) * L.e2 + (long long)L.n[0] * nj;
+  const long long nA = rows * e3;
+  const long long tot = nA + (long long)L.n[0] * L.n[1] * 8;
+  k_ghosts_shell<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s, nj, nA);
 }
 
 }  // namespace hamr

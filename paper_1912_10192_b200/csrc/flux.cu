@@ -26,6 +26,23 @@ __device__ __forceinline__ double lim_slope(double dl, double dr, double dc) {
   return (dl * dr > 0.0) ? copysign(lim, dc) : 0.0;
 }
 
+// interface value a_{j+1/2} from a_j, d = a_{j+1} - a_j and the limited slopes of zones j and j+1
+__device__ __forceinline__ double ppm_iface(double aj, double d, double dm_j, double dm_jp) {
+  return aj + 0.5 * d - (dm_jp - dm_j) * SIXTH;
+}
+
+// monotonised parabola edges of a zone with mean a and interface values l (low side), r (high side)
+__device__ __forceinline__ void ppm_mono(double l, double a, double r, double& aL, double& aR) {
+  const bool flat = (r - a) * (a - l) <= 0.0;
+  const double d = r - l;
+  const double c = a - 0.5 * (l + r);
+  const double dc = d * c, dd6 = d * d * SIXTH;
+  const bool over = dc > dd6, under = dc < -dd6;
+  const double nl = 3.0 * a - 2.0 * r, nr = 3.0 * a - 2.0 * l;
+  aL = flat ? a : (over ? nl : l);
+  aR = flat ? a : ((!over && under) ? nr : r);
+}
+
 // parabola edges (aL at j-1/2, aR at j+1/2) of zone j from a0..a4 = a[j-2..j+2]
 __device__ __forceinline__ void ppm_edges(double a0, double a1, double a2, double a3, double a4, double& aL,
                                           double& aR) {
@@ -33,17 +50,7 @@ __device__ __forceinline__ void ppm_edges(double a0, double a1, double a2, doubl
   const double dm_m = lim_slope(d10, d21, 0.5 * (a2 - a0));
   const double dm_0 = lim_slope(d21, d32, 0.5 * (a3 - a1));
   const double dm_p = lim_slope(d32, d43, 0.5 * (a4 - a2));
-  double l = a1 + 0.5 * d21 - (dm_0 - dm_m) * SIXTH;
-  double r = a2 + 0.5 * d32 - (dm_p - dm_0) * SIXTH;
-  // monotonise
-  const bool flat = (r - a2) * (a2 - l) <= 0.0;
-  const double d = r - l;
-  const double c = a2 - 0.5 * (l + r);
-  const double dc = d * c, dd6 = d * d * SIXTH;
-  const bool over = dc > dd6, under = dc < -dd6;
-  const double nl = 3.0 * a2 - 2.0 * r, nr = 3.0 * a2 - 2.0 * l;
-  aL = flat ? a2 : (over ? nl : l);
-  aR = flat ? a2 : ((!over && under) ? nr : r);
+  ppm_mono(ppm_iface(a1, d21, dm_m, dm_0), a2, ppm_iface(a2, d32, dm_0, dm_p), aL, aR);
 }
 
 // PLM with the MC limiter: minmod(2(a1-a0), (a2-a0)/2, 2(a2-a1))
@@ -64,7 +71,7 @@ __device__ __forceinline__ void zone_edges(const double* __restrict__ a, int sd,
 struct FGeo {
   double c00, c01, c03, c11, c13, c22, c33;  // g_{mu nu}
   double k00, kdd, k0d;                      // g^{tt}, g^{dd}, g^{td}
-  double gdet, igdet, ialpha, boa;
+  double gdet, igdet, alpha, ialpha, boa;
 };
 
 template <int D>
@@ -78,6 +85,7 @@ __device__ __forceinline__ FGeo load_fgeo(const double* __restrict__ tab, int n2
   G.kdd = __ldg(tab + (D == 0 ? K11 : (D == 1 ? K22 : K33)) * n2d + q);
   G.k0d = (D == 0) ? __ldg(tab + K01 * n2d + q) : 0.0;  // g^{t2} = g^{t3} = 0 for both metrics
   G.gdet = __ldg(tab + GDET * n2d + q); G.igdet = __ldg(tab + IGDET * n2d + q);
+  G.alpha = __ldg(tab + ALPHA * n2d + q);
   G.ialpha = __ldg(tab + IALPHA * n2d + q); G.boa = __ldg(tab + BOA * n2d + q);
   return G;
 }
@@ -89,7 +97,9 @@ __device__ __forceinline__ void side_state(const double P[8], const FGeo& G, dou
   constexpr int dir = D + 1, e = (D + 1) % 3, f = (D + 2) % 3;
   // C-2
   const double q = G.c11 * P[2] * P[2] + G.c22 * P[3] * P[3] + G.c33 * P[4] * P[4] + 2.0 * (G.c13 * P[2] * P[4]);
-  const double gam = sqrt(1.0 + q);
+  const double q1 = 1.0 + q;
+  const double rg = rsqrt(q1);  // gamma = q1 rg and 1/u^t = alpha/gamma = alpha rg share one special-function call
+  const double gam = q1 * rg;
   double u[4], ul[4], b[4], bl[4];
   u[0] = gam * G.ialpha;
   u[1] = P[2] - gam * G.boa;
@@ -101,7 +111,7 @@ __device__ __forceinline__ void side_state(const double P[8], const FGeo& G, dou
   ul[3] = G.c03 * u[0] + G.c13 * u[1] + G.c33 * u[3];
   // C-3
   b[0] = P[5] * ul[1] + P[6] * ul[2] + P[7] * ul[3];
-  const double iut = 1.0 / u[0];
+  const double iut = G.alpha * rg;
   b[1] = (P[5] + b[0] * u[1]) * iut;
   b[2] = (P[6] + b[0] * u[2]) * iut;
   b[3] = (P[7] + b[0] * u[3]) * iut;
@@ -131,13 +141,14 @@ __device__ __forceinline__ void side_state(const double P[8], const FGeo& G, dou
   F[5] = b[1 + e] * u[dir] - b[dir] * u[1 + e];
   F[6] = b[1 + f] * u[dir] - b[dir] * u[1 + f];
   // C-6: c_m^2 = c_s^2 + v_A^2 - c_s^2 v_A^2 with c_s^2 = gamma p / w, v_A^2 = b^2 / (b^2 + w)
+  // = N / Dq with Dq = w (w + b^2) > 0; the quadratic is multiplied through by Dq (same roots, no division)
   const double gp = gam_ad * p;
-  double cm2 = (gp * eta + bsq * (w - gp)) / (w * eta);
-  cm2 = dmin(dmax(cm2, 0.0), 1.0);
+  const double Dq = w * eta;
+  const double N = dmin(dmax(gp * eta + bsq * (w - gp), 0.0), Dq);  // clamp c_m^2 to [0, 1]
   const double ut2 = u[0] * u[0], udt = u[dir] * u[0], ud2 = u[dir] * u[dir];
-  const double a2 = ut2 - (G.k00 + ut2) * cm2;
-  const double a1 = 2.0 * (udt - (G.k0d + udt) * cm2);
-  const double a0 = ud2 - (G.kdd + ud2) * cm2;
+  const double a2 = ut2 * Dq - (G.k00 + ut2) * N;
+  const double a1 = 2.0 * (udt * Dq - (G.k0d + udt) * N);
+  const double a0 = ud2 * Dq - (G.kdd + ud2) * N;
   const double disc = sqrt(dmax(a1 * a1 - 4.0 * a2 * a0, 0.0));
   const double i2 = 1.0 / (2.0 * a2);
   const double v1 = (a1 + disc) * i2, v2 = (a1 - disc) * i2;
@@ -182,11 +193,25 @@ __device__ __forceinline__ void zero_face(const Dev& Dv, int D, int z) {
 }
 
 // ---- sweeps along x1 / x2: a thread marches along the sweep direction ---------------------------------
-// grid.x covers the flattened transverse index (other, k), k fastest; grid.y the segments of SEG faces.
-constexpr int SEG = 16;
-
+// grid.x covers the flattened transverse index (other, k), k fastest; grid.y the segments of `seg` faces.
+// PPM: the thread carries, per variable, a_j, a_{j+1}, the limited slope of zone j and the interface
+// value a_{j-1/2}; each step loads ONE new value a_{j+2}, builds ONE new slope and ONE new interface
+// value (the expressions are those of ppm_edges, so the result is bitwise the same).
+#ifndef HAMR_MARCH_RELOAD
+#define HAMR_MARCH_RELOAD 1  // 1: re-read a_j, a_{j+1} from L1 each step instead of carrying them in registers (measured faster)
+#endif
+#ifndef HAMR_MARCH_MINB
+#define HAMR_MARCH_MINB 4  // 128 regs/thread: measured best of 1/3/4 on cfg 2 (profiles/)
+#endif
+#ifndef HAMR_MARCH_UNROLL
+#define HAMR_MARCH_UNROLL 1
+#endif
+constexpr int MARCH_UNROLL = HAMR_MARCH_UNROLL;
+#ifndef HAMR_X3_MINB
+#define HAMR_X3_MINB 5
+#endif
 template <int D, int RECON>
-__global__ void __launch_bounds__(128) k_flux_march(Dev Dv, Fields s, int want_ctop) {
+__global__ void __launch_bounds__(128, HAMR_MARCH_MINB) k_flux_march(Dev Dv, Fields s, int seg, int want_ctop) {
   static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   const Lay& L = Dv.L;
   constexpr int O = 1 - D;          // the other non-x3 dimension
@@ -196,7 +221,7 @@ __global__ void __launch_bounds__(128) k_flux_march(Dev Dv, Fields s, int want_c
   double ctop = 0.0;
   if (tf < (L.n[O] + 2) * ck) {
     const int k = tf % ck - 1, o = tf / ck - 1;
-    const int f0 = blockIdx.y * SEG, f1 = min(f0 + SEG, L.n[D] + 1);
+    const int f0 = blockIdx.y * seg, f1 = min(f0 + seg, L.n[D] + 1);
     const int sd = (D == 0) ? L.S1 : L.S2;
     const bool act = o >= 0 && o < L.n[O] && k >= 0 && k < L.n[2];  // C-14: faces of ACTIVE zones
     const bool ks = Dv.metric == HAMR_METRIC_KERR_SCHILD;
@@ -204,17 +229,49 @@ __global__ void __launch_bounds__(128) k_flux_march(Dev Dv, Fields s, int want_c
     constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
     int z = (int)L.idx(D == 0 ? f0 - 1 : o, D == 0 ? o : f0 - 1, k);
     double PL[8], PR[8];
-    // right edges of the zone below the first face
+    double a0[7], a1[7], dm[7], il[7];  // PPM marching state (unused for PLM)
+    // the zone below the first face: its right edge, and the marching state of the next zone
 #pragma unroll
     for (int v = 0; v < 7; v++) {
-      double aL;
-      zone_edges<RECON>(var[v] + z, sd, aL, PL[slot[v]]);
+      const double* a = var[v] + z;
+      if (RECON == HAMR_RECON_PPM) {
+        const double m2 = a[-2 * sd], m1 = a[-sd], c0 = a[0], p1 = a[sd], p2 = a[2 * sd];
+        const double d10 = m1 - m2, d21 = c0 - m1, d32 = p1 - c0, d43 = p2 - p1;
+        const double dm_m = lim_slope(d10, d21, 0.5 * (c0 - m2));
+        const double dm_0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
+        const double dm_p = lim_slope(d32, d43, 0.5 * (p2 - c0));
+        const double r = ppm_iface(c0, d32, dm_0, dm_p);
+        double aL;
+        ppm_mono(ppm_iface(m1, d21, dm_m, dm_0), c0, r, aL, PL[slot[v]]);
+        a0[v] = p1; a1[v] = p2; dm[v] = dm_p; il[v] = r;
+      } else {
+        double aL;
+        plm_edges(a[-sd], a[0], a[sd], aL, PL[slot[v]]);
+      }
     }
+#pragma unroll MARCH_UNROLL
     for (int fc = f0; fc < f1; fc++) {
       z += sd;
       double carry[7];
 #pragma unroll
-      for (int v = 0; v < 7; v++) zone_edges<RECON>(var[v] + z, sd, PR[slot[v]], carry[v]);
+      for (int v = 0; v < 7; v++) {
+        const double* a = var[v] + z;
+        if (RECON == HAMR_RECON_PPM) {
+          const double a2 = a[2 * sd];
+#if HAMR_MARCH_RELOAD
+          const double c0 = a[0], c1 = a[sd];
+#else
+          const double c0 = a0[v], c1 = a1[v];
+#endif
+          const double d21 = c1 - c0, d32 = a2 - c1;
+          const double dmp = lim_slope(d21, d32, 0.5 * (a2 - c0));
+          const double r = ppm_iface(c0, d21, dm[v], dmp);
+          ppm_mono(il[v], c0, r, PR[slot[v]], carry[v]);
+          a0[v] = c1; a1[v] = a2; dm[v] = dmp; il[v] = r;
+        } else {
+          plm_edges(a[-sd], a[0], a[sd], PR[slot[v]], carry[v]);
+        }
+      }
       const bool pole = (D == 1) && ks && (fc == 0 || fc == L.n[1]);
       if (pole) {  // C-7: pole faces carry no flux and no state is evaluated there
         zero_face(Dv, D, z);
@@ -235,21 +292,26 @@ __global__ void __launch_bounds__(128) k_flux_march(Dev Dv, Fields s, int want_c
   }
 }
 
-// ---- sweep along x3: one lane per zone, the right edge comes from the neighbouring lane ---------------
-// Zones (i, j, k) with i, j in [-1, n], k in [-1, n3] are flattened with k fastest; a warp owns 31
-// consecutive zones plus one leading helper zone that only supplies its right edges.
+// ---- sweep along x3: one lane per zone, neighbouring lanes exchange slopes and edges -------------------
+// Zones (i, j, k) with i, j in [-1, n], k in [-HLO, n3 + HHI - 1] are flattened with k fastest.  A warp
+// owns 32 consecutive zones of which the first HLO and the last HHI only help.
+// PPM (HLO = 2, HHI = 1): every lane builds the limited slope of ITS zone once; slopes, interface
+// values and right edges travel between lanes by warp shuffle.  PLM (HLO = 1, HHI = 0).
 template <int RECON>
-__global__ void __launch_bounds__(128) k_flux_x3(Dev Dv, Fields s, int want_ctop) {
+__global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s, int want_ctop) {
   constexpr int D = 2;
+  constexpr int HLO = (RECON == HAMR_RECON_PPM) ? 2 : 1, HHI = (RECON == HAMR_RECON_PPM) ? 1 : 0;
+  constexpr int OWN = 32 - HLO - HHI;
+  constexpr unsigned FULL = 0xffffffffu;
   const Lay& L = Dv.L;
-  const int ck = L.n[2] + 2, cj = L.n[1] + 2;
+  const int ck = L.n[2] + 1 + HLO + HHI, cj = L.n[1] + 2;
   const long long tot = (long long)(L.n[0] + 2) * cj * ck;
   const int lane = threadIdx.x & 31;
   const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  long long t = warp * 31 + lane - 1;
+  long long t = warp * OWN + lane - HLO;
   const bool valid = t >= 0 && t < tot;
   t = t < 0 ? 0 : (t >= tot ? tot - 1 : t);  // clamped lanes compute on a real zone and store nothing
-  const int k = (int)(t % ck) - 1;
+  const int k = (int)(t % ck) - HLO;
   const int j = (int)((t / ck) % cj) - 1;
   const int i = (int)(t / ((long long)ck * cj)) - 1;
   const int z = (int)L.idx(i, j, k);
@@ -257,12 +319,23 @@ __global__ void __launch_bounds__(128) k_flux_x3(Dev Dv, Fields s, int want_ctop
   double PL[8], PR[8];
 #pragma unroll
   for (int v = 0; v < 7; v++) {
+    const double* a = var[v] + z;
     double aR;
-    zone_edges<RECON>(var[v] + z, 1, PR[v], aR);
-    PL[v] = __shfl_up_sync(0xffffffffu, aR, 1);  // right edge of zone k-1 = left state of face k-1/2
+    if (RECON == HAMR_RECON_PPM) {
+      const double m1 = a[-1], c0 = a[0], p1 = a[1];
+      const double d21 = c0 - m1, d32 = p1 - c0;
+      const double dm0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
+      const double dmp = __shfl_down_sync(FULL, dm0, 1);         // slope of zone k+1
+      const double r = ppm_iface(c0, d32, dm0, dmp);             // a_{k+1/2}
+      const double l = __shfl_up_sync(FULL, r, 1);               // a_{k-1/2}, built by lane-1 from the same expression
+      ppm_mono(l, c0, r, PR[v], aR);
+    } else {
+      plm_edges(a[-1], a[0], a[1], PR[v], aR);
+    }
+    PL[v] = __shfl_up_sync(FULL, aR, 1);  // right edge of zone k-1 = left state of face k-1/2
   }
   double ctop = 0.0;
-  if (valid && lane > 0 && k >= 0) {
+  if (valid && lane >= HLO && lane < 32 - HHI && k >= 0 && k <= L.n[2]) {
     const FGeo G = load_fgeo<D>(Dv.gc, L.n2d, L.idx2(i, j));
     PL[7] = PR[7] = s.Bf[2][z] * G.igdet;
     const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
@@ -274,31 +347,67 @@ __global__ void __launch_bounds__(128) k_flux_x3(Dev Dv, Fields s, int want_ctop
   }
 }
 
+// picks the number of faces per marching segment so that the grid fills whole waves of resident
+// blocks (148 SMs x blocks per SM) with little prologue overhead
+template <int D, int RECON>
+static int pick_segment(const Lay& L, int nbx) {
+  static int cached_seg = 0, cached_key = -1;
+  const int nf = L.n[D] + 1;
+  const int key = nf * 4096 + nbx;
+  if (key == cached_key) return cached_seg;
+  int dev = 0, sms = 148, per_sm = 2;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_flux_march<D, RECON>, 128, 0);
+  if (per_sm < 1) per_sm = 1;
+  const double slots = (double)sms * per_sm;
+  double best = -1.0;
+  int best_seg = nf < 16 ? nf : 16;
+  for (int nseg = 1; nseg <= nf && nseg <= 64; nseg++) {
+    const int seg = (nf + nseg - 1) / nseg;
+    if (seg < 8 && nseg > 1) break;
+    const int ns = (nf + seg - 1) / seg;
+    const double blocks = (double)nbx * ns;
+    const double waves = ceil(blocks / slots);
+    // useful work / occupied slots-time: wave fill x (faces / (faces + one prologue zone per segment))
+    const double eff = blocks / (waves * slots) * ((double)nf / ((double)ns * (seg + 1)));
+    if (eff > best) { best = eff; best_seg = seg; }
+  }
+  cached_key = key;
+  cached_seg = best_seg;
+  return best_seg;
+}
+
 template <int D>
 static void launch_march(hamr_grid* g, const Fields& src, bool want_ctop) {
   const Lay& L = g->D.L;
   const int O = 1 - D;
   const int ntr = (L.n[O] + 2) * (L.n[2] + 2);
-  dim3 grid((ntr + 127) / 128, (L.n[D] + 1 + SEG - 1) / SEG);
+  const int nbx = (ntr + 127) / 128;
   Launch l_(g, K_FLUX1 + D);
-  if (g->D.recon == HAMR_RECON_PPM)
-    k_flux_march<D, HAMR_RECON_PPM><<<grid, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
-  else
-    k_flux_march<D, HAMR_RECON_PLM_MC><<<grid, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
+  if (g->D.recon == HAMR_RECON_PPM) {
+    const int seg = pick_segment<D, HAMR_RECON_PPM>(L, nbx);
+    dim3 grid(nbx, (L.n[D] + 1 + seg - 1) / seg);
+    k_flux_march<D, HAMR_RECON_PPM><<<grid, 128, 0, g->stream>>>(g->D, src, seg, want_ctop ? 1 : 0);
+  } else {
+    const int seg = pick_segment<D, HAMR_RECON_PLM_MC>(L, nbx);
+    dim3 grid(nbx, (L.n[D] + 1 + seg - 1) / seg);
+    k_flux_march<D, HAMR_RECON_PLM_MC><<<grid, 128, 0, g->stream>>>(g->D, src, seg, want_ctop ? 1 : 0);
+  }
 }
 
 void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop) {
   launch_march<0>(g, src, want_ctop);
   launch_march<1>(g, src, want_ctop);
   const Lay& L = g->D.L;
-  const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 2);
-  const long long warps = (tot + 30) / 31 + 1;
+  const bool ppm = g->D.recon == HAMR_RECON_PPM;
+  const int own = ppm ? 29 : 31, halo = ppm ? 3 : 1;
+  const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 1 + halo);
+  const long long warps = (tot + own - 1) / own + 1;
   const unsigned nb = (unsigned)((warps + 3) / 4);
   Launch l_(g, K_FLUX3);
-  if (g->D.recon == HAMR_RECON_PPM)
-    k_flux_x3<HAMR_RECON_PPM><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
-  else
-    k_flux_x3<HAMR_RECON_PLM_MC><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
+  if (ppm) k_flux_x3<HAMR_RECON_PPM><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
+  else k_flux_x3<HAMR_RECON_PLM_MC><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
 }
 
 }  // namespace hamr
