@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cstring>
 #include <new>
+#include <stdexcept>
 
 namespace orc {
 
@@ -35,6 +36,13 @@ static Grid* grid_new(const Params& par) {
   g->have_state = false;
   g->stats = Stats{0, 0, 0, 0};
   if (!params_ok(par, g->err)) { delete g; return nullptr; }
+  g->multi = par.nb[0] > 0 || par.nb[1] > 0 || par.nb[2] > 0 || par.n_deref > 0 ||
+             par.lat_max_level > 0 || par.r_refine_max > 0.0;
+  if (g->multi) {
+    try { blocks_build(*g); } catch (const std::exception& e) { delete g; return nullptr; }
+    return g;
+  }
+  g->nslot[0] = g->nslot[1] = g->nslot[2] = 1;
   double lo[3], hi[3];
   internal_extent(par, lo, hi);
   g->blocks.resize(1);
@@ -74,15 +82,47 @@ static void full_step(Grid& g) {
 }
 
 static bool state_finite(const Grid& g) {
-  const Block& b = g.blocks[0];
-  for (int i = 0; i < b.n[0]; i++)
-    for (int j = 0; j < b.n[1]; j++)
-      for (int k = 0; k < b.n[2]; k++) {
-        const size_t z = b.idx(i, j, k);
-        for (int c = 0; c < 5; c++)
-          if (!std::isfinite(b.sn.P[c][z])) return false;
-      }
+  for (const Block& b : g.blocks)
+    for (int i = 0; i < b.n[0]; i++)
+      for (int j = 0; j < b.n[1]; j++)
+        for (int k = 0; k < b.n[2]; k++) {
+          const size_t z = b.idx(i, j, k);
+          for (int c = 0; c < 5; c++)
+            if (!std::isfinite(b.sn.P[c][z])) return false;
+        }
   return true;
+}
+
+// dense <-> block transfers.  Global arrays (orc_set_prims etc.) exist for grids without x1
+// refinement: block b holds the sub-box starting at I0.  stag = -1 zone-centred, else the face dim.
+static void scatter(const Grid& g, Block& b, std::vector<double>& dst, const double* src, int stag,
+                    bool global) {
+  int m[3] = {b.n[0], b.n[1], b.n[2]}, M[3] = {g.par.n[0], g.par.n[1], g.par.n[2]};
+  if (stag >= 0) { m[stag] += 1; M[stag] += 1; }
+  for (int i = 0; i < m[0]; i++)
+    for (int j = 0; j < m[1]; j++)
+      for (int k = 0; k < m[2]; k++) {
+        double v = global ? src[((size_t)(b.I0[0] + i) * M[1] + (b.I0[1] + j)) * M[2] + (b.I0[2] + k)]
+                          : src[((size_t)i * m[1] + j) * m[2] + k];
+        if (stag == 1 && b.pole2[j + NG]) v = 0.0;      // C-12: Bf2 on the pole face is 0
+        dst[b.idx(i, j, k)] = v;
+      }
+}
+static void gather(const Grid& g, const Block& b, const std::vector<double>& src, double* dst, int stag,
+                   bool global) {
+  int m[3] = {b.n[0], b.n[1], b.n[2]}, M[3] = {g.par.n[0], g.par.n[1], g.par.n[2]};
+  if (stag >= 0) { m[stag] += 1; M[stag] += 1; }
+  for (int i = 0; i < m[0]; i++)
+    for (int j = 0; j < m[1]; j++)
+      for (int k = 0; k < m[2]; k++) {
+        const double v = src[b.idx(i, j, k)];
+        if (global) dst[((size_t)(b.I0[0] + i) * M[1] + (b.I0[1] + j)) * M[2] + (b.I0[2] + k)] = v;
+        else dst[((size_t)i * m[1] + j) * m[2] + k] = v;
+      }
+}
+static bool has_refinement(const Grid& g) {
+  for (const Block& b : g.blocks) if (b.lev1) return true;
+  return false;
 }
 
 }  // namespace orc
@@ -103,6 +143,21 @@ void orc_grid_destroy(void* h) { delete (Grid*)h; }
 // hydro[c]: N1*N2*N3 active zones, x3 fastest.  bface[d]: d-faces, extent n[d]+1 along d; NULL -> 0.
 int orc_set_prims(void* h, const double* const hydro[5], const double* const bface[3]) {
   Grid& g = *(Grid*)h;
+  if (g.multi) {
+    if (has_refinement(g)) return 1;   // refined grids are set block by block
+    for (Block& b : g.blocks) {
+      for (int c = 0; c < 5; c++) scatter(g, b, b.sn.P[c], hydro[c], -1, true);
+      for (int d = 0; d < 3; d++) {
+        std::fill(b.sn.Bf[d].begin(), b.sn.Bf[d].end(), 0.0);
+        if (bface && bface[d]) scatter(g, b, b.sn.Bf[d], bface[d], d, true);
+      }
+    }
+    blocks_initial_dt(g);
+    g.t = 0.0;
+    g.have_state = true;
+    g.stats = Stats{0, 0, 0, 0};
+    return state_finite(g) ? 0 : 5;
+  }
   Block& b = g.blocks[0];
   for (int c = 0; c < 5; c++)
     for (int i = 0; i < b.n[0]; i++)
@@ -138,7 +193,8 @@ int orc_step(void* h, int nsteps, double* t_out, double* dt_last) {
   double dtl = 0.0;
   for (int s = 0; s < nsteps; s++) {
     dtl = g.dt;
-    full_step(g);
+    if (g.multi) blocks_coarse_step(g);
+    else full_step(g);
   }
   if (t_out) *t_out = g.t;
   if (dt_last) *dt_last = dtl;
@@ -150,6 +206,12 @@ void orc_set_dt(void* h, double dt) { ((Grid*)h)->dt = dt; }
 
 int orc_get_prims(void* h, double* const prims[8]) {
   Grid& g = *(Grid*)h;
+  if (g.multi) {
+    if (has_refinement(g)) return 1;
+    for (const Block& b : g.blocks)
+      for (int c = 0; c < 8; c++) gather(g, b, (c < 5) ? b.sn.P[c] : b.sn.Bc[c - 5], prims[c], -1, true);
+    return 0;
+  }
   Block& b = g.blocks[0];
   for (int c = 0; c < 8; c++) {
     const std::vector<double>& a = (c < 5) ? b.sn.P[c] : b.sn.Bc[c - 5];
@@ -163,6 +225,13 @@ int orc_get_prims(void* h, double* const prims[8]) {
 
 int orc_get_bface(void* h, double* const bface[3]) {
   Grid& g = *(Grid*)h;
+  if (g.multi) {
+    if (has_refinement(g)) return 1;
+    // a face shared by two blocks is written twice; orc_bface_mismatch() reports whether the copies agree
+    for (const Block& b : g.blocks)
+      for (int d = 0; d < 3; d++) gather(g, b, b.sn.Bf[d], bface[d], d, true);
+    return 0;
+  }
   Block& b = g.blocks[0];
   for (int d = 0; d < 3; d++) {
     int m[3] = {b.n[0], b.n[1], b.n[2]};
@@ -179,11 +248,11 @@ int orc_get_bface(void* h, double* const bface[3]) {
 // 1e-12 of its global maximum count 0.
 int orc_divb(void* h, double* out) {
   Grid& g = *(Grid*)h;
-  Block& b = g.blocks[0];
-  const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
   double denmax = 0.0;
   for (int pass = 0; pass < 2; pass++) {
     double worst = 0.0;
+    for (const Block& b : g.blocks) {
+    const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
     for (int i = 0; i < b.n[0]; i++)
       for (int j = 0; j < b.n[1]; j++)
         for (int k = 0; k < b.n[2]; k++) {
@@ -197,6 +266,7 @@ int orc_divb(void* h, double* out) {
           if (pass == 0) denmax = std::max(denmax, den);
           else if (den > 1e-12 * denmax) worst = std::max(worst, std::fabs(div) / den);
         }
+    }
     if (pass == 1) *out = worst;
   }
   return 0;
@@ -228,8 +298,8 @@ int orc_get_face(void* h, int d, int which, double* out) {
 // Conserved totals over active zones: sum of U[c] dV for c = 0..4 (P10), U from sn.
 int orc_totals(void* h, double tot[5]) {
   Grid& g = *(Grid*)h;
-  Block& b = g.blocks[0];
   for (int c = 0; c < 5; c++) tot[c] = 0.0;
+  for (const Block& b : g.blocks) {
   const double dV = b.dx[0] * b.dx[1] * b.dx[2];
   for (int i = 0; i < b.n[0]; i++)
     for (int j = 0; j < b.n[1]; j++) {
@@ -245,7 +315,86 @@ int orc_totals(void* h, double tot[5]) {
         for (int c = 0; c < 5; c++) tot[c] += U[c] * dV;
       }
     }
+  }
   return 0;
+}
+
+// ---- block enumeration (C-16, C-17) -------------------------------------------------------------
+int orc_num_blocks(void* h) { return (int)((Grid*)h)->blocks.size(); }
+// x_lo: internal coordinates of the block's low corner
+int orc_block_info(void* h, int bi, double x_lo[3], double dx[3], int n[3], int* tau, int* lev1) {
+  Grid& g = *(Grid*)h;
+  if (bi < 0 || bi >= (int)g.blocks.size()) return 1;
+  const Block& b = g.blocks[bi];
+  for (int d = 0; d < 3; d++) { x_lo[d] = b.xf(d, 0); dx[d] = b.dx[d]; n[d] = b.n[d]; }
+  *tau = b.tau;
+  *lev1 = b.lev1;
+  return 0;
+}
+int orc_set_block_prims(void* h, int bi, const double* const hydro[5], const double* const bface[3]) {
+  Grid& g = *(Grid*)h;
+  if (!g.multi || bi < 0 || bi >= (int)g.blocks.size()) return 1;
+  Block& b = g.blocks[bi];
+  for (int c = 0; c < 5; c++) scatter(g, b, b.sn.P[c], hydro[c], -1, false);
+  for (int d = 0; d < 3; d++) {
+    std::fill(b.sn.Bf[d].begin(), b.sn.Bf[d].end(), 0.0);
+    if (bface && bface[d]) scatter(g, b, b.sn.Bf[d], bface[d], d, false);
+  }
+  return 0;
+}
+// test hook: prescribe the LAT level of every block (NULL: back to Courant-based levels)
+int orc_force_levels(void* h, const int* tau) {
+  Grid& g = *(Grid*)h;
+  g.forced_tau.clear();
+  if (tau) g.forced_tau.assign(tau, tau + g.blocks.size());
+  return 0;
+}
+// after every block has been set: ghost fill, first dt and time levels
+int orc_blocks_commit(void* h) {
+  Grid& g = *(Grid*)h;
+  if (!g.multi) return 1;
+  blocks_initial_dt(g);
+  g.t = 0.0;
+  g.have_state = true;
+  g.stats = Stats{0, 0, 0, 0};
+  return state_finite(g) ? 0 : 5;
+}
+int orc_get_block_prims(void* h, int bi, double* const prims[8]) {
+  Grid& g = *(Grid*)h;
+  if (bi < 0 || bi >= (int)g.blocks.size()) return 1;
+  const Block& b = g.blocks[bi];
+  for (int c = 0; c < 8; c++) gather(g, b, (c < 5) ? b.sn.P[c] : b.sn.Bc[c - 5], prims[c], -1, false);
+  return 0;
+}
+int orc_get_block_bface(void* h, int bi, double* const bface[3]) {
+  Grid& g = *(Grid*)h;
+  if (bi < 0 || bi >= (int)g.blocks.size()) return 1;
+  const Block& b = g.blocks[bi];
+  for (int d = 0; d < 3; d++) gather(g, b, b.sn.Bf[d], bface[d], d, false);
+  return 0;
+}
+// largest difference between the two copies of a face field value on faces shared by two blocks
+double orc_bface_mismatch(void* h) {
+  Grid& g = *(Grid*)h;
+  double worst = 0.0;
+  for (const Block& b : g.blocks)
+    for (int d = 0; d < 3; d++) {
+      int o[3] = {0, 0, 0};
+      o[d] = 1;
+      const int qi = b.nbr[o[0] + 1][o[1] + 1][o[2] + 1];
+      if (qi < 0 || g.blocks[qi].lev1 != b.lev1) continue;
+      const Block& q = g.blocks[qi];
+      const int e = (d + 1) % 3, f = (d + 2) % 3;
+      for (int p = 0; p < b.n[e]; p++)
+        for (int r = 0; r < b.n[f]; r++) {
+          int lb[3], lq[3];
+          lb[d] = b.n[d]; lb[e] = p; lb[f] = r;
+          lq[d] = 0; lq[e] = p; lq[f] = r;
+          worst = std::max(worst, std::fabs(b.sn.Bf[d][b.idx(lb[0], lb[1], lb[2])] -
+                                            q.sn.Bf[d][q.idx(lq[0], lq[1], lq[2])]));
+        }
+    }
+  return worst;
 }
 
 // ---- per-zone entry points for the pins -------------------------------------------------------

@@ -1,0 +1,449 @@
+// ORACLE (test infrastructure) — block-structured grid: block lattice, ghost exchange between
+// blocks, local adaptive time-stepping with flux / EMF correction.  DESIGN.md §9 (C-16, C-17);
+// PAPER.md:71 (blocks, boundary-cell transfer), PAPER.md:105 (LAT: per-block dt in factors of 2),
+// PAPER.md:137 (flux / EMF synchronisation between time levels, correction added to the coarse
+// block's boundary cells, extra inversion there).
+#include "orc_grid.hpp"
+#include <algorithm>
+#include <cstring>
+#include <stdexcept>
+
+namespace orc {
+
+static const int CYC[3][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}};  // (d, e, f) cyclic
+
+// ---- block lattice (C-16) -----------------------------------------------------------------------
+void blocks_build(Grid& g) {
+  const Params& par = g.par;
+  double lo[3], hi[3], dx0[3];
+  int nb[3], NB[3];
+  for (int d = 0; d < 3; d++) { lo[d] = par.xmin[d]; hi[d] = par.xmax[d]; }
+  if (par.metric == 1) { lo[0] = std::log(par.xmin[0]); hi[0] = std::log(par.xmax[0]); }
+  for (int d = 0; d < 3; d++) {
+    nb[d] = par.nb[d] > 0 ? par.nb[d] : par.n[d];
+    if (par.n[d] % nb[d] != 0) throw std::runtime_error("n[d] is not a multiple of nb[d]");
+    NB[d] = par.n[d] / nb[d];
+    dx0[d] = (hi[d] - lo[d]) / par.n[d];
+  }
+  // x1 slots: a base block column whose x1-centre has r < r_refine_max is replaced by two children
+  // with dx1/2 (C-16; PAPER.md:71 per-dimension splitting)
+  struct Slot { int col, lev, child; };
+  std::vector<Slot> slots;
+  bool seen_coarse = false;
+  for (int col = 0; col < NB[0]; col++) {
+    bool refined = false;
+    if (par.r_refine_max > 0.0 && par.metric == 1) {
+      const double xc = lo[0] + ((double)col + 0.5) * nb[0] * dx0[0];
+      refined = std::exp(xc) < par.r_refine_max;
+    }
+    if (refined && seen_coarse) throw std::runtime_error("refined columns must be contiguous from r_in");
+    if (refined) { slots.push_back({col, 1, 0}); slots.push_back({col, 1, 1}); }
+    else { slots.push_back({col, 0, 0}); seen_coarse = true; }
+  }
+  g.nslot[0] = (int)slots.size(); g.nslot[1] = NB[1]; g.nslot[2] = NB[2];
+  g.lattice.assign((size_t)g.nslot[0] * NB[1] * NB[2], -1);
+  g.blocks.clear();
+  g.blocks.resize(g.lattice.size());
+  int id = 0;
+  for (int s = 0; s < g.nslot[0]; s++)
+    for (int bj = 0; bj < NB[1]; bj++)
+      for (int bk = 0; bk < NB[2]; bk++, id++) {
+        Block& b = g.blocks[id];
+        g.lattice[((size_t)s * NB[1] + bj) * NB[2] + bk] = id;
+        b.slot[0] = s; b.slot[1] = bj; b.slot[2] = bk;
+        b.lev1 = slots[s].lev;
+        for (int d = 0; d < 3; d++) { b.n[d] = nb[d]; b.dx[d] = dx0[d]; b.x0[d] = lo[d]; }
+        b.I0[0] = slots[s].lev ? (long long)(2 * slots[s].col + slots[s].child) * nb[0]
+                               : (long long)slots[s].col * nb[0];
+        if (b.lev1) b.dx[0] = dx0[0] / 2.0;
+        b.I0[1] = (long long)bj * nb[1];
+        b.I0[2] = (long long)bk * nb[2];
+        for (int d = 0; d < 3; d++) {
+          // periodic dimensions are closed through the neighbour table, not through fill_physical_bc
+          b.phys_lo[d] = b.slot[d] == 0 && par.bc_lo[d] != 0;
+          b.phys_hi[d] = b.slot[d] == g.nslot[d] - 1 && par.bc_hi[d] != 0;
+        }
+        b.tau = 0; b.tb_u = 0; b.dt_u = 2; b.has_new = false;
+      }
+  for (Block& b : g.blocks) {
+    for (int o0 = -1; o0 <= 1; o0++)
+      for (int o1 = -1; o1 <= 1; o1++)
+        for (int o2 = -1; o2 <= 1; o2++) {
+          const int o[3] = {o0, o1, o2};
+          int s[3];
+          bool inside = true;
+          for (int d = 0; d < 3; d++) {
+            s[d] = b.slot[d] + o[d];
+            if (s[d] < 0 || s[d] >= g.nslot[d]) {
+              if (par.bc_lo[d] == 0) s[d] = (s[d] + g.nslot[d]) % g.nslot[d];
+              else inside = false;
+            }
+          }
+          b.nbr[o0 + 1][o1 + 1][o2 + 1] =
+              inside ? g.lattice[((size_t)s[0] * g.nslot[1] + s[1]) * g.nslot[2] + s[2]] : -1;
+        }
+  }
+  for (Block& b : g.blocks) {
+    // C-16 ghost geometry on a refined x1 level uses the block's own (fine or coarse) spacing
+    if (b.lev1) {
+      // pole2 / geometry use global x2 index and the block's own x1 spacing: block_init reads
+      // I0 and dx, which are already those of the block's level
+    }
+    block_init(par, b);
+    const size_t n = b.size();
+    for (int d = 0; d < 3; d++) {
+      for (int c = 0; c < 5; c++) { b.FA[d][c].assign(n, 0.0); b.FA2[d][c].assign(n, 0.0); }
+      b.EA[d].assign(n, 0.0);
+      b.EA2[d].assign(n, 0.0);
+      b.ctop_last[d] = 0.0;
+    }
+  }
+}
+
+// ---- ghost exchange (C-16 same-level copy; C-17 time interpolation) ----------------------------------
+// value at integer time s_u (units of dt_0/2) of an array of block q given its three time levels
+static inline double sample(const Block& q, const std::vector<double>& an, const std::vector<double>& ah,
+                            const std::vector<double>& aw, size_t z, long long s_u) {
+  if (s_u == q.tb_u) return an[z];                       // a completed state: copy
+  if (q.has_new) {                                       // completed states bracket s: linear in time
+    const double w = (double)(s_u - q.tb_u) / (double)q.dt_u;
+    return (1.0 - w) * an[z] + w * aw[z];
+  }
+  const double w = (double)(s_u - q.tb_u) / (double)(q.dt_u / 2);  // state n and its predictor state
+  return (1.0 - w) * an[z] + w * ah[z];
+}
+
+static void exchange_block(Grid& g, Block& b, Fields& dst, long long s_u) {
+  auto off = [](int idx, int n, bool face) { return idx < 0 ? -1 : (idx > (face ? n : n - 1) ? 1 : 0); };
+  for (int i = -NG; i < b.n[0] + NG + 1; i++)
+    for (int j = -NG; j < b.n[1] + NG + 1; j++)
+      for (int k = -NG; k < b.n[2] + NG + 1; k++) {
+        const int id[3] = {i, j, k};
+        const size_t z = b.idx(i, j, k);
+        // a = 0: zone-centred hydro primitives; a = 1 + d: the d-face field
+        for (int a = 0; a < 4; a++) {
+          int o[3], lq[3];
+          bool ghost = false, valid = true;
+          for (int d = 0; d < 3; d++) {
+            const bool face = (a == 1 + d);
+            if (!face && id[d] > b.n[d] + NG - 1) valid = false;  // index n+3 exists for faces only
+            o[d] = off(id[d], b.n[d], face);
+            if (o[d] != 0) ghost = true;
+          }
+          if (!valid) continue;
+          int qi = b.nbr[o[0] + 1][o[1] + 1][o[2] + 1];   // the block itself if no offset
+          if (qi < 0) continue;                          // outside the domain: physical boundary
+          for (int d = 0; d < 3; d++) lq[d] = id[d] - o[d] * b.n[d];
+          // C-17: a face on the plane between two blocks on different time levels has ONE value in
+          // every stage source, that of the finer block (own boundary faces included)
+          if (a > 0 && (id[a - 1] == 0 || id[a - 1] == b.n[a - 1])) {
+            const int d = a - 1;
+            int o2[3] = {o[0], o[1], o[2]};
+            o2[d] = id[d] == 0 ? -1 : 1;
+            const int q2 = b.nbr[o2[0] + 1][o2[1] + 1][o2[2] + 1];
+            if (q2 >= 0 && g.blocks[q2].tau < g.blocks[qi].tau && g.blocks[q2].lev1 == g.blocks[qi].lev1) {
+              qi = q2;
+              lq[d] = id[d] == 0 ? b.n[d] : 0;
+              ghost = true;
+            }
+          }
+          if (!ghost) continue;
+          const Block& q = g.blocks[qi];
+          if (q.lev1 != b.lev1) continue;                // coarse <-> fine: exchange_refined()
+          const size_t zq = q.idx(lq[0], lq[1], lq[2]);
+          if (a == 0) {
+            for (int c = 0; c < 5; c++) dst.P[c][z] = sample(q, q.sn.P[c], q.sh.P[c], q.snew.P[c], zq, s_u);
+          } else {
+            const int d = a - 1;
+            dst.Bf[d][z] = sample(q, q.sn.Bf[d], q.sh.Bf[d], q.snew.Bf[d], zq, s_u);
+          }
+        }
+      }
+}
+
+// ---- one stage of C-12 on every block of one time level ------------------------------------------------
+static void stage_level(Grid& g, int tau, bool corrector) {
+  for (Block& b : g.blocks) {
+    if (b.tau != tau) continue;
+    Fields& src = corrector ? b.sh : b.sn;
+    exchange_block(g, b, src, b.tb_u + (corrector ? b.dt_u / 2 : 0));
+    fill_physical_bc(g.par, b, src);
+    compute_Bc(b, src, false);
+  }
+  for (Block& b : g.blocks) {
+    if (b.tau != tau) continue;
+    Fields& src = corrector ? b.sh : b.sn;
+    flux_pass(g.par, b, src);
+    ct_edges(g.par, b, src);
+    const double dtb = g.dt * (double)(b.dt_u / 2);      // dt_b = 2^tau dt_0
+    if (corrector) {
+      // C-17 registers: R1 = dt_b * (F, E) of this corrector; R2 accumulates the two steps that
+      // make up one step of a neighbour on the next coarser level
+      const bool first = (b.tb_u % (2 * b.dt_u)) == 0;
+      const size_t n = b.size();
+      for (int d = 0; d < 3; d++) {
+        for (int c = 0; c < 5; c++)
+          for (size_t z = 0; z < n; z++) {
+            const double v = dtb * b.F[d][c][z];
+            b.FA[d][c][z] = v;
+            b.FA2[d][c][z] = first ? v : b.FA2[d][c][z] + v;
+          }
+        for (size_t z = 0; z < n; z++) {
+          const double v = dtb * b.Ee[d][z];
+          b.EA[d][z] = v;
+          b.EA2[d][z] = first ? v : b.EA2[d][z] + v;
+        }
+        b.ctop_last[d] = b.ctop[d];
+      }
+    }
+    update(g.par, b, src, b.sn, corrector ? b.snew : b.sh, corrector ? dtb : 0.5 * dtb, g.stats);
+  }
+  if (corrector)
+    for (Block& b : g.blocks)
+      if (b.tau == tau) b.has_new = true;
+}
+
+// ---- C-17 correct(tau-1 -> tau) ---------------------------------------------------------------------
+// For every block c on level tau with a neighbour on level tau-1 (across a face, edge or corner):
+//  * edge EMFs on c's boundary that a finer block shares are replaced by the finer block's
+//    time-integrated EMF; every active face of c touching a replaced edge is rebuilt from the base
+//    field with the corrected EMFs; the normal field on a face shared with a finer block is copied;
+//  * the flux difference on faces shared with a finer block is added to c's boundary zones;
+//  * the touched zones are re-inverted.
+static void correct_level(Grid& g, int tau) {
+  const Params& par = g.par;
+  for (Block& c : g.blocks) {
+    if (c.tau != tau) continue;
+    bool any = false;
+    for (int a = 0; a < 27; a++) {
+      const int q = (&c.nbr[0][0][0])[a];
+      if (q >= 0 && g.blocks[q].tau == tau - 1) any = true;
+    }
+    if (!any) continue;
+    const int str[3] = {c.e[1] * c.e[2], c.e[2], 1};
+    const size_t n = c.size();
+    std::vector<double> EC[3];
+    std::vector<char> erep[3], ftouch[3], zmask(n, 0);
+    std::vector<double> dU[5];
+    for (int d = 0; d < 3; d++) { EC[d] = c.EA[d]; erep[d].assign(n, 0); ftouch[d].assign(n, 0); }
+    for (int cc = 0; cc < 5; cc++) dU[cc].assign(n, 0.0);
+    // (1) replace boundary edge EMFs by the finer sharer's accumulated value
+    for (int f = 0; f < 3; f++) {
+      const int d = CYC[f][1], e = CYC[f][2];
+      int hi[3] = {c.n[0], c.n[1], c.n[2]};
+      hi[f] = c.n[f] - 1;
+      for (int i = 0; i <= hi[0]; i++)
+        for (int j = 0; j <= hi[1]; j++)
+          for (int k = 0; k <= hi[2]; k++) {
+            const int id[3] = {i, j, k};
+            const int od = id[d] == 0 ? -1 : (id[d] == c.n[d] ? 1 : 0);
+            const int oe = id[e] == 0 ? -1 : (id[e] == c.n[e] ? 1 : 0);
+            if (od == 0 && oe == 0) continue;
+            const int cand[3][2] = {{od, 0}, {0, oe}, {od, oe}};
+            for (int t = 0; t < 3; t++) {
+              if (cand[t][0] == 0 && cand[t][1] == 0) continue;
+              int o[3] = {0, 0, 0};
+              o[d] = cand[t][0]; o[e] = cand[t][1];
+              const int qi = c.nbr[o[0] + 1][o[1] + 1][o[2] + 1];
+              if (qi < 0) continue;
+              const Block& q = g.blocks[qi];
+              if (q.tau != tau - 1) continue;
+              int lq[3] = {i, j, k};
+              lq[d] -= o[d] * c.n[d];
+              lq[e] -= o[e] * c.n[e];
+              const size_t z = c.idx(i, j, k);
+              EC[f][z] = q.EA2[f][q.idx(lq[0], lq[1], lq[2])];
+              erep[f][z] = 1;
+              break;
+            }
+          }
+    }
+    // (2) rebuild every active face touching a replaced edge: Bf = base - curl(EC)   (C-10 with dt E -> EC)
+    for (int d = 0; d < 3; d++) {
+      const int e = CYC[d][1], f = CYC[d][2];
+      int hi[3] = {c.n[0] - 1, c.n[1] - 1, c.n[2] - 1};
+      hi[d] = c.n[d];
+      for (int i = 0; i <= hi[0]; i++)
+        for (int j = 0; j <= hi[1]; j++)
+          for (int k = 0; k <= hi[2]; k++) {
+            const size_t z = c.idx(i, j, k);
+            if (!(erep[f][z] || erep[f][z + str[e]] || erep[e][z] || erep[e][z + str[f]])) continue;
+            if (d == 1 && c.pole2[j + NG]) continue;
+            const double curl = (EC[f][z + str[e]] - EC[f][z]) / c.dx[e] - (EC[e][z + str[f]] - EC[e][z]) / c.dx[f];
+            c.snew.Bf[d][z] = c.sn.Bf[d][z] - curl;
+            ftouch[d][z] = 1;
+          }
+    }
+    // (3) faces shared with a finer face-neighbour: copy its normal field, add the flux difference
+    for (int d = 0; d < 3; d++)
+      for (int side = 0; side < 2; side++) {
+        int o[3] = {0, 0, 0};
+        o[d] = side ? 1 : -1;
+        const int qi = c.nbr[o[0] + 1][o[1] + 1][o[2] + 1];
+        if (qi < 0) continue;
+        const Block& q = g.blocks[qi];
+        if (q.tau != tau - 1) continue;
+        const int e = CYC[d][1], f = CYC[d][2];
+        for (int p = 0; p < c.n[e]; p++)
+          for (int r = 0; r < c.n[f]; r++) {
+            int lc[3], lq[3], lz[3];
+            lc[d] = side ? c.n[d] : 0; lc[e] = p; lc[f] = r;        // c's boundary face
+            lq[d] = side ? 0 : q.n[d]; lq[e] = p; lq[f] = r;        // the same face in q
+            lz[d] = side ? c.n[d] - 1 : 0; lz[e] = p; lz[f] = r;    // c's boundary zone
+            const size_t zf = c.idx(lc[0], lc[1], lc[2]), zq = q.idx(lq[0], lq[1], lq[2]);
+            const size_t zz = c.idx(lz[0], lz[1], lz[2]);
+            c.snew.Bf[d][zf] = q.sn.Bf[d][zq];   // q has completed both steps: its sn is at c's new time
+            ftouch[d][zf] = 1;
+            for (int cc = 0; cc < 5; cc++) {
+              const double dF = q.FA2[d][cc][zq] - c.FA[d][cc][zf];
+              // U_new = U - (dt F_hi - dt F_lo)/dx: the high face enters with -, the low face with +
+              dU[cc][zz] += (side ? -dF : dF) / c.dx[d];
+            }
+            zmask[zz] = 1;
+          }
+      }
+    // zones with a touched face
+    for (int d = 0; d < 3; d++)
+      for (int i = 0; i < c.n[0]; i++)
+        for (int j = 0; j < c.n[1]; j++)
+          for (int k = 0; k < c.n[2]; k++) {
+            const size_t z = c.idx(i, j, k);
+            if (ftouch[d][z] || ftouch[d][z + str[d]]) zmask[z] = 1;
+          }
+    // (4) re-invert: U = U(P^{n+1}, old B_c) + dU with the rebuilt B_c
+    for (int i = 0; i < c.n[0]; i++)
+      for (int j = 0; j < c.n[1]; j++) {
+        const Geom& G = c.gc[c.idx2(i, j)];
+        const double r = (par.metric == 1) ? std::exp(c.xc(0, i)) : 1.0;
+        for (int k = 0; k < c.n[2]; k++) {
+          const size_t z = c.idx(i, j, k);
+          if (!zmask[z]) continue;
+          double P[8], U[8], Bn[3], Pn[5];
+          for (int cc = 0; cc < 5; cc++) P[cc] = c.snew.P[cc][z];
+          for (int cc = 0; cc < 3; cc++) P[5 + cc] = c.snew.Bc[cc][z];
+          State S;
+          get_state(P, G, S);
+          prim_to_U(P, S, G, par.gamma_ad, U);
+          for (int cc = 0; cc < 5; cc++) U[cc] += dU[cc][z];
+          for (int d = 0; d < 3; d++) {
+            Bn[d] = (c.snew.Bf[d][z] + c.snew.Bf[d][z + str[d]]) / (2.0 * G.gdet);
+            c.snew.Bc[d][z] = Bn[d];
+          }
+          int rc = con2prim(U, Bn, G, par.gamma_ad, P, Pn, nullptr);
+          if (rc != 0) {
+            g.stats.c2p_fail++;
+            for (int cc = 0; cc < 5; cc++) Pn[cc] = P[cc];
+          }
+          floors_and_ceiling(par, G, r, Pn, g.stats);
+          for (int cc = 0; cc < 5; cc++) c.snew.P[cc][z] = Pn[cc];
+        }
+      }
+  }
+}
+
+static void rotate_level(Grid& g, int tau) {
+  for (Block& b : g.blocks) {
+    if (b.tau != tau) continue;
+    for (int c = 0; c < 5; c++) b.sn.P[c].swap(b.snew.P[c]);
+    for (int c = 0; c < 3; c++) { b.sn.Bc[c].swap(b.snew.Bc[c]); b.sn.Bf[c].swap(b.snew.Bf[c]); }
+    b.tb_u += b.dt_u;
+    b.has_new = false;
+  }
+}
+
+// C-17: advance(tau) = predictor, first half of the finer levels, corrector, second half, correction
+static void advance(Grid& g, int tau) {
+  stage_level(g, tau, false);
+  if (tau > 0) advance(g, tau - 1);
+  stage_level(g, tau, true);
+  if (tau > 0) {
+    advance(g, tau - 1);
+    correct_level(g, tau);
+  }
+  rotate_level(g, tau);
+}
+
+// ---- time step and time levels (C-14, C-17) ---------------------------------------------------------------
+static void assign_levels(Grid& g) {
+  const Params& par = g.par;
+  const int tmax = par.lat_max_level;
+  if (tmax <= 0) {
+    // global step: per-direction maximum over the whole grid, then the harmonic sum (C-14)
+    double s = 0.0;
+    for (int d = 0; d < 3; d++) {
+      double m = 0.0;
+      for (const Block& b : g.blocks) m = std::max(m, b.ctop_last[d] / b.dx[d]);
+      s += m;
+    }
+    g.dt = par.cour / s;
+    for (Block& b : g.blocks) { b.tau = 0; }
+  } else {
+    // per-block Courant step, levels in factors of 2 relative to the smallest
+    std::vector<double> dtb(g.blocks.size());
+    double dt0 = 1e300;
+    for (size_t i = 0; i < g.blocks.size(); i++) {
+      dtb[i] = dt_from_ctop(par, g.blocks[i]);
+      dt0 = std::min(dt0, dtb[i]);
+    }
+    if (!g.forced_tau.empty()) {
+      // test hook: prescribed levels; dt_0 is the largest step every block can take on its level
+      dt0 = 1e300;
+      for (size_t i = 0; i < g.blocks.size(); i++) {
+        g.blocks[i].tau = std::min(tmax, std::max(0, g.forced_tau[i]));
+        dt0 = std::min(dt0, dtb[i] / (double)(1 << g.blocks[i].tau));
+      }
+    } else {
+      for (size_t i = 0; i < g.blocks.size(); i++) {
+        int tau = 0;
+        double lim = 2.0 * dt0;
+        while (tau < tmax && dtb[i] >= lim) { tau++; lim *= 2.0; }
+        g.blocks[i].tau = tau;
+      }
+    }
+    // neighbours across faces, edges and corners differ by at most one level: lower until they do
+    for (bool changed = true; changed;) {
+      changed = false;
+      std::vector<int> nt(g.blocks.size());
+      for (size_t i = 0; i < g.blocks.size(); i++) {
+        const Block& b = g.blocks[i];
+        int t = b.tau;
+        for (int a = 0; a < 27; a++) {
+          const int q = (&b.nbr[0][0][0])[a];
+          if (q >= 0) t = std::min(t, g.blocks[q].tau + 1);
+        }
+        nt[i] = t;
+        if (t != b.tau) changed = true;
+      }
+      for (size_t i = 0; i < g.blocks.size(); i++) g.blocks[i].tau = nt[i];
+    }
+    g.dt = dt0;
+  }
+  for (Block& b : g.blocks) {
+    b.tb_u = 0;
+    b.dt_u = 2LL << b.tau;
+    b.has_new = false;
+  }
+}
+
+void blocks_initial_dt(Grid& g) {
+  for (Block& b : g.blocks) { b.tau = 0; b.tb_u = 0; b.dt_u = 2; b.has_new = false; }
+  for (Block& b : g.blocks) {
+    exchange_block(g, b, b.sn, 0);
+    fill_physical_bc(g.par, b, b.sn);
+    compute_Bc(b, b.sn, false);
+  }
+  for (Block& b : g.blocks) {
+    flux_pass(g.par, b, b.sn);                 // C-14: one flux pass sets the first dt
+    for (int d = 0; d < 3; d++) b.ctop_last[d] = b.ctop[d];
+  }
+  assign_levels(g);
+}
+
+void blocks_coarse_step(Grid& g) {
+  const int tmax = std::max(0, g.par.lat_max_level);
+  advance(g, tmax);
+  g.t += g.dt * (double)(1 << tmax);
+  assign_levels(g);
+}
+
+}  // namespace orc

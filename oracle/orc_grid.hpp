@@ -31,6 +31,16 @@ struct Block {
   std::vector<char> pole2;         // x2-face row j lies on the polar axis
 
   Fields sn, sh, snew;             // time n, n+1/2 and the state being written
+  // ---- block-structured grid (C-16, C-17; orc_blocks.cpp) ----
+  int slot[3];                     // position in the block lattice (x1 slot, x2 block, x3 block)
+  int nbr[3][3][3];                // neighbour block ids by offset (-1: outside the domain)
+  long long tb_u, dt_u;            // LAT: time of sn and own step, in units of (finest dt)/2
+  bool has_new;                    // snew holds the completed state at tb_u + dt_u
+  std::vector<double> FA[3][5];    // flux register R1: dt_b * F of the latest corrector (C-17)
+  std::vector<double> EA[3];       // EMF register R1: dt_b * E_edge of the latest corrector
+  std::vector<double> FA2[3][5];   // R2: R1 summed over the two steps inside one step of the next
+  std::vector<double> EA2[3];      //     coarser time level
+  double ctop_last[3];             // ctop of this block's most recent corrector (or initial) pass
   std::vector<double> F[3][5];     // hydro fluxes on d-faces
   std::vector<double> Ef[3][3];    // Ef[d][c]: E_c on d-faces, c != d (C-8)
   std::vector<double> Ee[3];       // edge EMFs (C-9)
@@ -52,11 +62,21 @@ struct Stats { long long c2p_fail, rho_floor, u_floor, gam_ceil; };
 struct Grid {
   Params par;
   std::vector<Block> blocks;
-  double t, dt;
+  double t, dt;                    // dt: the global step, or the finest-level step dt_0 under LAT
   bool have_state;
   Stats stats;
   std::string err;
+  int nslot[3];                    // block lattice extents
+  std::vector<int> lattice;        // block id by (slot1, slot2, slot3)
+  bool multi;                      // more than one block, or any of deref / refine / LAT
+  std::vector<int> forced_tau;     // test hook: fixed time levels instead of the Courant-based ones
 };
+
+// orc_blocks.cpp (C-15..C-17)
+void blocks_build(Grid& g);                       // block lattice, neighbours, geometry
+void blocks_exchange(Grid& g, int level, int stage_half);  // ghost fill of the level's stage source
+void blocks_initial_dt(Grid& g);                  // flux pass on every block, first dt / levels
+void blocks_coarse_step(Grid& g);                 // one (coarse) step: advance(tau_max)
 
 void block_init(const Params& par, Block& b);           // geometry tables, allocation
 void fill_physical_bc(const Params& par, Block& b, Fields& s);

@@ -54,8 +54,14 @@ def lib():
         L.orc_set_dt.argtypes = [C.c_void_p, C.c_double]
         for name in ("orc_set_prims", "orc_step", "orc_get_prims", "orc_get_bface", "orc_divb",
                      "orc_get_stats", "orc_get_face", "orc_totals", "orc_debug_emf", "orc_get_edge",
-                     "orc_get_centre_emf", "orc_get_ctop"):
+                     "orc_get_centre_emf", "orc_get_ctop", "orc_block_info", "orc_set_block_prims",
+                     "orc_get_block_prims", "orc_get_block_bface"):
             getattr(L, name).argtypes = None
+        L.orc_bface_mismatch.restype = C.c_double
+        L.orc_bface_mismatch.argtypes = [C.c_void_p]
+        L.orc_num_blocks.argtypes = [C.c_void_p]
+        L.orc_blocks_commit.argtypes = [C.c_void_p]
+        L.orc_force_levels.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
         L.orc_geom_at.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.POINTER(Geom)]
         L.orc_conn_at.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, c_double_p]
         L.orc_gcov_derivs.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, c_double_p,
@@ -209,6 +215,60 @@ class OrcGrid:
         c = np.zeros(3)
         self.L.orc_get_ctop(self.h, _dp(c))
         return c
+
+    # ---- block-structured grid ----
+    def num_blocks(self):
+        return self.L.orc_num_blocks(self.h)
+
+    def block_info(self, b):
+        xlo, dx = (C.c_double * 3)(), (C.c_double * 3)()
+        n = (C.c_int * 3)()
+        tau, lev = C.c_int(0), C.c_int(0)
+        rc = self.L.orc_block_info(self.h, C.c_int(b), xlo, dx, n, C.byref(tau), C.byref(lev))
+        assert rc == 0
+        return dict(x_lo=np.array(xlo[:]), dx=np.array(dx[:]), n=tuple(n[:]), tau=tau.value, lev1=lev.value)
+
+    def levels(self):
+        return np.array([self.block_info(b)["tau"] for b in range(self.num_blocks())])
+
+    def force_levels(self, tau):
+        if tau is None:
+            return self.L.orc_force_levels(self.h, None)
+        a = (C.c_int * len(tau))(*[int(t) for t in tau])
+        return self.L.orc_force_levels(self.h, a)
+
+    def set_block_prims(self, b, hydro, bface=None):
+        hy = [_arr(h) for h in hydro]
+        hp = (c_double_p * 5)(*[_dp(h) for h in hy])
+        if bface is None:
+            return self.L.orc_set_block_prims(self.h, C.c_int(b), hp, None)
+        bf = [_arr(x) for x in bface]
+        bp = (c_double_p * 3)(*[_dp(x) for x in bf])
+        return self.L.orc_set_block_prims(self.h, C.c_int(b), hp, bp)
+
+    def commit(self):
+        return self.L.orc_blocks_commit(self.h)
+
+    def get_block_prims(self, b):
+        n = self.block_info(b)["n"]
+        out = [np.empty(n) for _ in range(8)]
+        rc = self.L.orc_get_block_prims(self.h, C.c_int(b), (c_double_p * 8)(*[_dp(o) for o in out]))
+        assert rc == 0
+        return out
+
+    def get_block_bface(self, b):
+        n = list(self.block_info(b)["n"])
+        out = []
+        for d in range(3):
+            s = list(n)
+            s[d] += 1
+            out.append(np.empty(tuple(s)))
+        rc = self.L.orc_get_block_bface(self.h, C.c_int(b), (c_double_p * 3)(*[_dp(o) for o in out]))
+        assert rc == 0
+        return out
+
+    def bface_mismatch(self):
+        return self.L.orc_bface_mismatch(self.h)
 
 
 # ---- per-zone helpers for the pins ---------------------------------------------------------------
