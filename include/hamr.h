@@ -115,9 +115,23 @@ int hamr_set_dt(hamr_grid* g, double dt_next); /* overrides the next step's dt (
 const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the next call on g */
 
 /* ---- block-structured grid (BASELINE.json cfg 4) ------------------ */
+/* A grid with nb != {0,0,0} or lat_max_level > 0 is cut into blocks of nb zones (nb[d] = 0: the whole
+ * extent; nb[d] must divide n[d] and be >= 3).  Blocks exchange ghost zones directly;
+ * with lat_max_level = L > 0 every block steps with dt_0 * 2^tau, tau <= L chosen from its own Courant
+ * limit at every coarse step, neighbours differing by at most one level; ghosts of a
+ * block on another time level are interpolated in time, and at the end of each coarse block's step
+ * its boundary zones are corrected with the finer neighbour's accumulated fluxes and EMFs and
+ * inverted again (C-16, C-17).  On such a grid hamr_step(nsteps) takes
+ * nsteps COARSE steps of 2^L finest steps each; set / get calls take the same global arrays.
+ * All kernels of a stage run once over all blocks of a time level (no per-block launches). */
 int hamr_num_blocks(const hamr_grid* g);
+/* x_lo: internal coordinates of the block's low corner; time_level: its current LAT level tau */
 int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int n[3],
                     int* time_level);
+/* Test hook: prescribes the LAT level of every block (tau[hamr_num_blocks], clamped to
+ * 0..lat_max_level, then lowered until neighbours differ by at most one); NULL restores the
+ * Courant-based choice.  Takes effect at the next hamr_set_prims / coarse step.  The caller keeps tau. */
+int hamr_set_levels(hamr_grid* g, const int* tau);
 
 /* ---- diagnostics used by the parity tests (not part of the hot path) -------------------------- */
 /* Runs ghost fill + flux pass + CT EMFs on the current state (no update). */

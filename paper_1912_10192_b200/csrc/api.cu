@@ -13,6 +13,9 @@ using namespace hamr;
 namespace {
 
 constexpr int N_STATE_ARR = 11, N_ARR = 3 * N_STATE_ARR + 15 + 3 + 3 + 3 + 3;
+constexpr int N_REG_ARR = 15 + 3;  // LAT flux / EMF registers (C-17)
+
+bool is_block_grid(const hamr_params& p) { return p.nb[0] > 0 || p.nb[1] > 0 || p.nb[2] > 0 || p.lat_max_level > 0; }
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -31,39 +34,66 @@ bool params_ok(const hamr_params& p, std::string& why) {
   if (p.recon != HAMR_RECON_PPM && p.recon != HAMR_RECON_PLM_MC) { why = "bad recon"; return false; }
   if (p.metric == HAMR_METRIC_KERR_SCHILD && !(p.xmin[0] > 0.0)) { why = "r_in <= 0"; return false; }
   if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0) || !(p.gamma_max > 1.0)) { why = "gamma_ad / cour / gamma_max"; return false; }
-  if (p.nb[0] || p.nb[1] || p.nb[2] || p.n_deref || p.lat_max_level || p.r_refine_max > 0.0) {
-    why = "block-structured grid (nb, deref, r_refine, LAT) is not available in this build";
+  if (p.n_deref || p.r_refine_max > 0.0) {
+    why = "phi-derefinement and r-refinement are not available in this build (DESIGN.md section 9)";
     return false;
+  }
+  if (p.lat_max_level < 0 || p.lat_max_level > 3) { why = "lat_max_level must be 0..3"; return false; }
+  if (is_block_grid(p)) {
+    int ns[3], bn[3];
+    if (p.nb[0] < 0 || p.nb[1] < 0 || p.nb[2] < 0 || blk_count(p, ns, bn) <= 0) {
+      why = "block size must divide n and be >= 3";
+      return false;
+    }
   }
   return true;
 }
 
-void make_layout(const hamr_params& p, Lay& L) {
-  for (int d = 0; d < 3; d++) L.n[d] = p.n[d];
-  L.e1 = p.n[0] + 2 * NG + 1;
-  L.e2 = p.n[1] + 2 * NG + 1;
-  L.p3 = (int)align_up((size_t)p.n[2] + 2 * NG + 1, 16);
+// Layout of one padded block (monolithic grid: the one block).  On a block grid every array holds nblk
+// blocks of blen doubles back to back and the geometry tables are global.
+struct GridShape {
+  int nblk;        // 0: monolithic
+  int blen;        // doubles per block per array
+  int te1, te2;    // extents of the geometry tables
+  int narr;        // fp64 arrays of Lay::len doubles
+};
+
+bool make_layout(const hamr_params& p, Lay& L, GridShape& G) {
+  int ns[3], bn[3] = {p.n[0], p.n[1], p.n[2]};
+  G.nblk = is_block_grid(p) ? blk_count(p, ns, bn) : 0;
+  for (int d = 0; d < 3; d++) L.n[d] = bn[d];
+  L.e1 = bn[0] + 2 * NG + 1;
+  L.e2 = bn[1] + 2 * NG + 1;
+  L.p3 = (int)align_up((size_t)bn[2] + 2 * NG + 1, 16);
   L.S2 = L.p3;
   L.S1 = L.e2 * L.p3;
   L.off0 = ((long long)NG * L.e2 + NG) * L.p3 + NG + LEAD;
-  L.len = (long long)align_up((size_t)L.e1 * L.e2 * L.p3 + 32, 32);
-  L.n2d = L.e1 * L.e2;
+  const long long blen = (long long)align_up((size_t)L.e1 * L.e2 * L.p3 + 32, 32);
+  L.len = blen * (G.nblk > 0 ? G.nblk : 1);
+  if (L.len >= (1LL << 31)) return false;   // kernels index one array with 32-bit offsets
+  G.blen = (int)blen;
+  G.te1 = p.n[0] + 2 * NG + 1;
+  G.te2 = p.n[1] + 2 * NG + 1;
+  L.n2d = G.te1 * G.te2;
+  G.narr = N_ARR + ((G.nblk > 0 && p.lat_max_level > 0) ? N_REG_ARR : 0);
+  return true;
 }
 
 struct ArenaPlan {
-  size_t arr, tabs, scal, cnt, stage, total;
+  size_t arr, tabs, scal, cnt, stage, blk, total;
   size_t stage_doubles;
 };
 
-ArenaPlan plan_arena(const Lay& L) {
+ArenaPlan plan_arena(const hamr_params& p, const Lay& L, const GridShape& G) {
   ArenaPlan a;
   size_t off = 0;
-  a.arr = off; off += (size_t)N_ARR * L.len * 8;
-  a.tabs = off; off += align_up(((size_t)3 * NGEO + 2 * NDG) * L.n2d * 8 + (size_t)2 * L.e1 * 8, 256);
+  a.arr = off; off += (size_t)G.narr * L.len * 8;
+  a.tabs = off; off += align_up(((size_t)3 * NGEO + 2 * NDG) * L.n2d * 8 + (size_t)2 * G.te1 * 8, 256);
   a.scal = off; off += 256;
   a.cnt = off; off += 256;
-  a.stage_doubles = (size_t)8 * (L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);
+  a.stage_doubles = (size_t)8 * (p.n[0] + 1) * (p.n[1] + 1) * (p.n[2] + 1);
   a.stage = off; off += align_up(a.stage_doubles * 8, 256);
+  a.blk = off; off += G.nblk > 0 ? blk_table_bytes(G.nblk) : 0;
   a.total = off;
   return a;
 }
@@ -93,8 +123,13 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   g->par = *p;
   Dev& D = g->D;
   std::memset(&D, 0, sizeof(D));
-  make_layout(*p, D.L);
-  const ArenaPlan ap = plan_arena(D.L);
+  GridShape gs;
+  if (!make_layout(*p, D.L, gs)) { delete g; return HAMR_EINVAL; }
+  const ArenaPlan ap = plan_arena(*p, D.L, gs);
+  g->bh.on = false;
+  g->bh.nblk = 0;
+  g->bh.h_ctop = nullptr;
+  g->bh.h_ints = nullptr;
   g->own_arena = own;
   g->own_stream = own;
   g->arena = nullptr;
@@ -157,13 +192,23 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   for (int d = 0; d < 3; d++) D.EfB[d] = next();
   for (int d = 0; d < 3; d++) D.Ee[d] = next();
   for (int d = 0; d < 3; d++) D.Cc[d] = next();
+  if (gs.narr > N_ARR) {
+    for (int d = 0; d < 3; d++) for (int c = 0; c < 5; c++) D.B.FA2[d][c] = next();
+    for (int d = 0; d < 3; d++) D.B.EA2[d] = next();
+  }
+  D.B.nblk = gs.nblk;
+  D.B.blen = gs.blen;
+  D.B.ge2 = gs.te2;
+  D.B.n2g = p->n[1];
+  D.B.tlev = 0;
+  D.B.flev = 0;
   double* tabs = (double*)(base + ap.tabs);
   double* gc = tabs;
   double* gf1 = gc + (size_t)NGEO * D.L.n2d;
   double* gf2 = gf1 + (size_t)NGEO * D.L.n2d;
   double* dgc = gf2 + (size_t)NGEO * D.L.n2d;
   double* rfl = dgc + (size_t)2 * NDG * D.L.n2d;
-  double* ufl = rfl + D.L.e1;
+  double* ufl = rfl + gs.te1;
   D.gc = gc; D.gf1 = gf1; D.gf2 = gf2; D.dgc = dgc; D.rho_fl = rfl; D.u_fl = ufl;
   D.scal = (double*)(base + ap.scal);
   D.cnt = (unsigned long long*)(base + ap.cnt);
@@ -172,12 +217,15 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
 
   e = cudaMemsetAsync(g->arena, 0, ap.total, g->stream);
   if (e == cudaSuccess) {
-    launch_geometry(g, gc, gf1, gf2, dgc, rfl, ufl);
+    launch_geometry_tab(g, gs.te1, gs.te2, D.L.n2d, D.dx[0], p->n[1], gc, gf1, gf2, dgc, rfl, ufl);
     e = cudaGetLastError();
   }
+  if (e == cudaSuccess && gs.nblk > 0 && blk_setup(g, base + ap.blk) != HAMR_OK) e = cudaErrorUnknown;
   if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
   if (e != cudaSuccess) {
     cudaFreeHost(g->h_pinned);
+    if (g->bh.h_ctop) cudaFreeHost(g->bh.h_ctop);
+    if (g->bh.h_ints) cudaFreeHost(g->bh.h_ints);
     if (own) { cudaFree(g->arena); cudaStreamDestroy(g->stream); }
     delete g;
     return HAMR_ECUDA;
@@ -229,9 +277,14 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
   if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
   if (!hydro) return fail(g, HAMR_EINVAL, "hydro is NULL");
   for (int c = 0; c < 5; c++) if (!hydro[c]) return fail(g, HAMR_EINVAL, "hydro[c] is NULL");
-  const Lay& L = g->D.L;
+  const bool blk = g->bh.on;
+  const int* N = g->par.n;
+  if (blk) {
+    g->isn = 0; g->ish = 1; g->inew = 2;
+    CK(cudaMemsetAsync(g->D.B.cur, 0, (size_t)g->bh.nblk * sizeof(int), g->stream));
+  }
   const Fields& sn = g->s[g->isn];
-  const size_t nz = (size_t)L.n[0] * L.n[1] * L.n[2];
+  const size_t nz = (size_t)N[0] * N[1] * N[2];
   for (int c = 0; c < 5; c++) {
     const double* src = hydro[c];
     if (!dev) {
@@ -239,11 +292,12 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
       CK(cudaMemcpyAsync(st, hydro[c], nz * 8, cudaMemcpyHostToDevice, g->stream));
       src = st;
     }
-    launch_pack(g, src, sn.P[c], -1, false);
+    if (blk) blk_pack(g, src, c, -1, false);
+    else launch_pack(g, src, sn.P[c], -1, false);
   }
   size_t off = 5 * nz;
   for (int d = 0; d < 3; d++) {
-    int m[3] = {L.n[0], L.n[1], L.n[2]};
+    int m[3] = {N[0], N[1], N[2]};
     m[d] += 1;
     const size_t nf = (size_t)m[0] * m[1] * m[2];
     const double* src = (bface && bface[d]) ? bface[d] : nullptr;
@@ -254,30 +308,41 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
       src = st;
       off += nf;
     }
-    launch_pack(g, src, sn.Bf[d], d, d == 1);
+    if (blk) blk_pack(g, src, 5 + d, d, d == 1);
+    else launch_pack(g, src, sn.Bf[d], d, d == 1);
   }
   CK(cudaMemsetAsync(g->D.scal, 0, NSCAL * sizeof(double), g->stream));
   CK(cudaMemsetAsync(g->D.cnt, 0, NCNT * sizeof(unsigned long long), g->stream));
-  launch_ghosts(g, sn, true);
-  launch_flux(g, sn, true);   // C-14: one flux pass sets dt of step 0
-  launch_dt(g, 0);
-  launch_check_finite(g, sn);
+  if (blk) {
+    const int rc = blk_initial(g);
+    if (rc != HAMR_OK) return fail(g, rc, "block grid initialisation failed");
+    blk_check_finite(g);
+  } else {
+    launch_ghosts(g, sn, true);
+    launch_flux(g, sn, true);   // C-14: one flux pass sets dt of step 0
+    launch_dt(g, 0);
+    launch_check_finite(g, sn);
+  }
   g->have_state = true;
   CK(cudaGetLastError());
   if (dev) return HAMR_OK;
   return check_state(g);
 }
 
-int get_dense(hamr_grid* g, const double* padded, double* out, int stag, bool dev, size_t stage_off) {
-  const Lay& L = g->D.L;
-  int m[3] = {L.n[0], L.n[1], L.n[2]};
+// kind (block grids): 0..4 P, 5..7 Bc, 8..10 Bf of the current state
+int get_dense(hamr_grid* g, const double* padded, double* out, int stag, bool dev, size_t stage_off, int kind = -1) {
+  const int* N = g->par.n;
+  int m[3] = {N[0], N[1], N[2]};
   if (stag >= 0) m[stag] += 1;
   const size_t nf = (size_t)m[0] * m[1] * m[2];
+  if (g->bh.on && kind < 0) return fail(g, HAMR_ESTATE, "not available on a block-structured grid");
   if (dev) {
-    launch_unpack(g, padded, out, m);
+    if (g->bh.on) blk_unpack(g, kind, out);
+    else launch_unpack(g, padded, out, m);
   } else {
     double* st = g->stage + stage_off;
-    launch_unpack(g, padded, st, m);
+    if (g->bh.on) blk_unpack(g, kind, st);
+    else launch_unpack(g, padded, st, m);
     CK(cudaMemcpyAsync(out, st, nf * 8, cudaMemcpyDeviceToHost, g->stream));
   }
   return HAMR_OK;
@@ -291,8 +356,9 @@ int hamr_workspace_bytes(const hamr_params* p, size_t* bytes) {
   std::string why;
   if (!p || !bytes || !params_ok(*p, why)) return HAMR_EINVAL;
   Lay L;
-  make_layout(*p, L);
-  *bytes = plan_arena(L).total;
+  GridShape gs;
+  if (!make_layout(*p, L, gs)) return HAMR_EINVAL;
+  *bytes = plan_arena(*p, L, gs).total;
   return HAMR_OK;
 }
 
@@ -309,6 +375,8 @@ int hamr_grid_destroy(hamr_grid* g) {
   if (!g) return HAMR_EINVAL;
   cudaStreamSynchronize(g->stream);
   cudaFreeHost(g->h_pinned);
+  if (g->bh.h_ctop) cudaFreeHost(g->bh.h_ctop);
+  if (g->bh.h_ints) cudaFreeHost(g->bh.h_ints);
   for (cudaEvent_t e : g->ev) cudaEventDestroy(e);
   if (g->own_arena) cudaFree(g->arena);
   if (g->own_stream) cudaStreamDestroy(g->stream);
@@ -327,7 +395,12 @@ int hamr_step_async(hamr_grid* g, int nsteps) {
   if (!g || nsteps < 0) return HAMR_EINVAL;
   if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
   if (!g->have_state) return fail(g, HAMR_ESTATE, "hamr_step before hamr_set_prims");
-  for (int s = 0; s < nsteps; s++) enqueue_step(g);
+  if (g->bh.on) {
+    const int rc = blk_step(g, nsteps);
+    if (rc != HAMR_OK) return fail(g, rc, "block grid step failed");
+  } else {
+    for (int s = 0; s < nsteps; s++) enqueue_step(g);
+  }
   CK(cudaGetLastError());
   return HAMR_OK;
 }
@@ -352,10 +425,10 @@ int hamr_get_prims(hamr_grid* g, double* const prims[8]) {
   if (!g || !prims) return HAMR_EINVAL;
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
   const Fields& sn = g->s[g->isn];
-  const size_t nz = (size_t)g->D.L.n[0] * g->D.L.n[1] * g->D.L.n[2];
+  const size_t nz = (size_t)g->par.n[0] * g->par.n[1] * g->par.n[2];
   for (int c = 0; c < 8; c++) {
     if (!prims[c]) continue;
-    int rc = get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], prims[c], -1, false, (size_t)c * nz);
+    int rc = get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], prims[c], -1, false, (size_t)c * nz, c);
     if (rc != HAMR_OK) return rc;
   }
   CK(cudaStreamSynchronize(g->stream));
@@ -367,7 +440,7 @@ int hamr_get_prims_dev(hamr_grid* g, double* const prims[8]) {
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
   const Fields& sn = g->s[g->isn];
   for (int c = 0; c < 8; c++)
-    if (prims[c]) get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], prims[c], -1, true, 0);
+    if (prims[c]) get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], prims[c], -1, true, 0, c);
   CK(cudaGetLastError());
   return HAMR_OK;
 }
@@ -376,13 +449,13 @@ int hamr_get_bface(hamr_grid* g, double* const bface[3]) {
   if (!g || !bface) return HAMR_EINVAL;
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
   const Fields& sn = g->s[g->isn];
-  const Lay& L = g->D.L;
+  const int* N = g->par.n;
   size_t off = 0;
   for (int d = 0; d < 3; d++) {
     if (!bface[d]) continue;
-    int rc = get_dense(g, sn.Bf[d], bface[d], d, false, off);
+    int rc = get_dense(g, sn.Bf[d], bface[d], d, false, off, 8 + d);
     if (rc != HAMR_OK) return rc;
-    off += (size_t)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);
+    off += (size_t)(N[0] + 1) * (N[1] + 1) * (N[2] + 1);
   }
   CK(cudaStreamSynchronize(g->stream));
   return HAMR_OK;
@@ -391,7 +464,8 @@ int hamr_get_bface(hamr_grid* g, double* const bface[3]) {
 int hamr_divb(hamr_grid* g, double* out) {
   if (!g || !out) return HAMR_EINVAL;
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
-  launch_divb(g, g->s[g->isn]);
+  if (g->bh.on) blk_divb(g);
+  else launch_divb(g, g->s[g->isn]);
   return read_scal(g, S_DIVB, 1, out);
 }
 
@@ -425,22 +499,29 @@ int hamr_set_dt(hamr_grid* g, double dt) {
 
 const char* hamr_last_error(const hamr_grid* g) { return g ? g->err.c_str() : "null grid"; }
 
-int hamr_num_blocks(const hamr_grid* g) { return g ? 1 : 0; }
+int hamr_num_blocks(const hamr_grid* g) { return g ? (g->bh.on ? g->bh.nblk : 1) : 0; }
 
 int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int n[3], int* time_level) {
-  if (!g || b != 0) return HAMR_EINVAL;
+  if (!g || b < 0 || b >= hamr_num_blocks(g)) return HAMR_EINVAL;
   for (int d = 0; d < 3; d++) {
-    if (x_lo) x_lo[d] = g->D.x0[d];
-    if (dx) dx[d] = g->D.dx[d];
+    const double dxd = (d == 0 && g->bh.on && g->bh.lev1[b]) ? 0.5 * g->D.dx[0] : g->D.dx[d];
+    if (x_lo) x_lo[d] = g->D.x0[d] + (g->bh.on ? g->bh.I0[(size_t)b * 3 + d] * dxd : 0.0);
+    if (dx) dx[d] = dxd;
     if (n) n[d] = g->D.L.n[d];
   }
-  if (time_level) *time_level = 0;
+  if (time_level) *time_level = g->bh.on ? g->bh.tau[b] : 0;
   return HAMR_OK;
+}
+
+int hamr_set_levels(hamr_grid* g, const int* tau) {
+  if (!g || !g->bh.on) return HAMR_EINVAL;
+  return blk_set_levels(g, tau);
 }
 
 int hamr_debug_emf(hamr_grid* g) {
   if (!g) return HAMR_EINVAL;
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  if (g->bh.on) return fail(g, HAMR_ESTATE, "not available on a block-structured grid");
   const Fields& sn = g->s[g->isn];
   launch_ghosts(g, sn, false);
   launch_zero_ctop(g);
@@ -463,6 +544,7 @@ int hamr_get_face(hamr_grid* g, int d, int which, double* out) {
 
 int hamr_get_edge(hamr_grid* g, int f, double* out) {
   if (!g || !out || f < 0 || f > 2) return HAMR_EINVAL;
+  if (g->bh.on) return fail(g, HAMR_ESTATE, "not available on a block-structured grid");
   const Lay& L = g->D.L;
   int m[3] = {L.n[0] + 1, L.n[1] + 1, L.n[2] + 1};
   m[f] -= 1;
@@ -480,7 +562,8 @@ int hamr_get_ctop(hamr_grid* g, double ctop[3]) {
 int hamr_totals(hamr_grid* g, double tot[5]) {
   if (!g || !tot) return HAMR_EINVAL;
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
-  launch_totals(g, g->s[g->isn]);
+  if (g->bh.on) blk_totals(g);
+  else launch_totals(g, g->s[g->isn]);
   return read_scal(g, S_TOT0, 5, tot);
 }
 

@@ -1,0 +1,942 @@
+// blocks.cu — block-structured grid on one GPU.
+// the grid is a set of blocks that "directly transfer boundary cells" to one another;
+// local adaptive time-stepping — every block steps with its own dt, a power of two
+// times the smallest; at the interface between time levels the fluxes and EMFs of the
+// finer block are accumulated and the coarse block's boundary zones are corrected with the
+// difference, "an additional conserved to primitive variable inversion needs to be performed for
+// these boundary cells".  Readings C-16 (same-level ghost copy, physical boundaries on the blocks
+// that touch the domain edge) and C-17 (schedule, time-interpolated ghosts, registers, correction).
+//
+// B200 design: blocks are far too small to fill the GPU one at a time (16^3 zones; PAPER.md:185
+// wants >~50^3 per launch), so every kernel of a stage is launched ONCE for all blocks of a time
+// level: arrays hold the padded blocks back to back, a launch carries the list of its blocks, and
+// a thread finds its block from its flat index.  No stream-per-block, no host loop over blocks.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include "hamr_host.h"
+
+namespace hamr {
+
+// the three buffer sets of the state arrays; a block's time-n state is s[cur], its predictor state
+// s[1], the state being written by its corrector s[2 - cur]
+struct Bufs { Fields s[3]; };
+
+// LAT clock of every time level (C-17), in units of (finest dt)/2: time of the level's time-n state,
+// its step, and whether its corrector has completed (so that s[2 - cur] holds the state at tb + dt)
+struct LevT { long long tb[4]; int dtu[4]; int hasnew[4]; };
+
+__device__ __forceinline__ const double* buf_arr(const Bufs& B, int buf, int kind) {
+  // kind 0..4: hydro primitive; 5..7: face field along kind - 5
+  const Fields& f0 = B.s[0];
+  const Fields& f1 = B.s[1];
+  const Fields& f2 = B.s[2];
+  const double* a0 = kind < 5 ? f0.P[kind] : f0.Bf[kind - 5];
+  const double* a1 = kind < 5 ? f1.P[kind] : f1.Bf[kind - 5];
+  const double* a2 = kind < 5 ? f2.P[kind] : f2.Bf[kind - 5];
+  return buf == 0 ? a0 : (buf == 1 ? a1 : a2);
+}
+
+template <typename T>
+__device__ __forceinline__ T pick4(const T v[4], int i) {
+  return i == 0 ? v[0] : (i == 1 ? v[1] : (i == 2 ? v[2] : v[3]));
+}
+
+// C-17: value at time s_u of array `kind` of block q at local offset zl, from q's three time levels:
+// a completed state at s_u is copied; completed states bracketing s_u are interpolated linearly in
+// time; otherwise the time-n state and the predictor state at tb + dt/2 are
+__device__ __forceinline__ double blk_sample(const Dev& Dv, const Bufs& B, const LevT& lt, int kind, int q,
+                                             int zl, long long s_u) {
+  const int tq = Dv.B.tau[q], cq = Dv.B.cur[q];
+  const long long tb = pick4(lt.tb, tq);
+  const int dtu = pick4(lt.dtu, tq);
+  const long long z = (long long)q * Dv.B.blen + zl;
+  const double an = buf_arr(B, cq, kind)[z];
+  if (s_u == tb) return an;
+  if (pick4(lt.hasnew, tq)) {
+    const double w = (double)(s_u - tb) / (double)dtu;
+    return (1.0 - w) * an + w * buf_arr(B, 2 - cq, kind)[z];
+  }
+  const double w = (double)(s_u - tb) / (double)(dtu / 2);
+  return (1.0 - w) * an + w * buf_arr(B, 1, kind)[z];
+}
+
+// Value that the ghost fill of C-16 / C-12 leaves at padded index id[] of array `kind` of block b:
+// the per-dimension physical-boundary maps (outflow copy, polar mirror; fill order x1, x2, x3) are
+// composed with the neighbour lookup, so that every ghost value is ONE signed sample of an active
+// value.  own_buf: the buffer holding b's stage source.  mod: the value differs from what b's own
+// active storage holds (a ghost, a reflecting wall face, or a boundary face owned by a finer block).
+__device__ __forceinline__ double blk_gval(const Dev& Dv, const Bufs& B, const LevT& lt, int b, int own_buf,
+                                           int kind, const int id[3], long long s_u, bool& mod) {
+  const Lay& L = Dv.L;
+  const int sd = kind >= 5 ? kind - 5 : -1;                    // staggered along sd
+  const int vc = kind >= 5 ? kind - 5 : (kind >= 2 ? kind - 2 : -1);  // component flipped by a mirror along vc
+  const int phys = __ldg(Dv.B.phys + b);
+  int m[3], o[3];
+  bool neg = false, zero = false;
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    const int n = L.n[d], hi = (sd == d) ? n : n - 1, g = id[d];
+    m[d] = g; o[d] = 0;
+    if (g < 0) {
+      if (phys & (1 << d)) {
+        if (Dv.bc_lo[d] == HAMR_BC_OUTFLOW) m[d] = 0;
+        else { m[d] = (sd == d) ? -g : -g - 1; if (vc == d) neg = !neg; }
+      } else o[d] = -1;
+    } else if (g > hi) {
+      if (phys & (8 << d)) {
+        if (Dv.bc_hi[d] == HAMR_BC_OUTFLOW) m[d] = hi;
+        else { m[d] = n - (g - hi); if (vc == d) neg = !neg; }
+      } else o[d] = 1;
+    }
+    // a reflecting wall carries no normal flux: the wall face itself is 0
+    if (sd == d && ((m[d] == 0 && (phys & (1 << d)) && Dv.bc_lo[d] == HAMR_BC_POLAR_REFLECT) ||
+                    (m[d] == n && (phys & (8 << d)) && Dv.bc_hi[d] == HAMR_BC_POLAR_REFLECT)))
+      zero = true;
+  }
+  const int* nb = Dv.B.nbr + b * 27;
+  int q = (o[0] == 0 && o[1] == 0 && o[2] == 0) ? b : __ldg(nb + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
+  int lq[3] = {m[0] - o[0] * L.n[0], m[1] - o[1] * L.n[1], m[2] - o[2] * L.n[2]};
+  bool ghost = (o[0] | o[1] | o[2]) != 0;
+  // C-17: a face on the plane between two blocks on different time levels has ONE value in every stage
+  // source, that of the finer block
+  if (sd >= 0 && (m[sd] == 0 || m[sd] == L.n[sd])) {
+    int o2[3] = {o[0], o[1], o[2]};
+    o2[sd] = m[sd] == 0 ? -1 : 1;
+    const int q2 = __ldg(nb + (o2[0] + 1) * 9 + (o2[1] + 1) * 3 + (o2[2] + 1));
+    if (q2 >= 0 && q >= 0 && Dv.B.tau[q2] < Dv.B.tau[q]) {
+      q = q2;
+      lq[sd] = m[sd] == 0 ? L.n[sd] : 0;
+      ghost = true;
+    }
+  }
+  mod = ghost || zero || neg || m[0] != id[0] || m[1] != id[1] || m[2] != id[2];
+  if (zero) return 0.0;
+  double v;
+  const int zl = (int)L.idx(lq[0], lq[1], lq[2]);
+  if (!ghost) v = buf_arr(B, own_buf, kind)[(long long)b * Dv.B.blen + zl];
+  else v = blk_sample(Dv, B, lt, kind, q, zl, s_u);
+  return neg ? -v : v;
+}
+
+// Ghost fill of the stage source of every listed block: neighbour exchange with time interpolation
+// (C-16, C-17), physical boundaries (C-12), cell-centred B wherever a face changed (C-10).
+// role: 0 the source is the block's time-n state, 1 its predictor state.  all: also derive B_c on the
+// active zones (initial state).  zero_ctop: reset the block's Courant maxima (before a corrector pass).
+__global__ void __launch_bounds__(256) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, int role, long long s_u_base,
+                                                    int all, int zero_ctop) {
+  const Lay& L = Dv.L;
+  const int e3 = L.n[2] + 2 * NG + 1;
+  const long long per = (long long)L.e1 * L.e2 * e3;
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= per * Dv.B.nact) return;
+  const int bslot = (int)(t / per);
+  t -= bslot * per;
+  const int b = __ldg(Dv.B.list + bslot);
+  if (zero_ctop && t == 0) Dv.B.ctopb[b * 3] = Dv.B.ctopb[b * 3 + 1] = Dv.B.ctopb[b * 3 + 2] = 0.0;
+  const int id[3] = {(int)(t / ((long long)e3 * L.e2)) - NG, (int)((t / e3) % L.e2) - NG, (int)(t % e3) - NG};
+  // zones two or more layers inside the block have nothing to do
+  bool deep = true;
+  for (int d = 0; d < 3; d++) deep = deep && id[d] >= 1 && id[d] <= L.n[d] - 2;
+  if (deep && !all) return;
+  const int cur = Dv.B.cur[b];
+  const int own = role == 0 ? cur : 1;
+  // s_u: the listed blocks share one time level, hence one clock
+  const long long s_u = s_u_base;
+  bool in_c[3], extra[3];
+  for (int d = 0; d < 3; d++) { in_c[d] = id[d] >= 0 && id[d] < L.n[d]; extra[d] = id[d] == L.n[d] + NG; }
+  const bool zone_active = in_c[0] && in_c[1] && in_c[2];
+  const bool zone_slot = !(extra[0] || extra[1] || extra[2]);
+  const long long z = (long long)b * Dv.B.blen + L.idx(id[0], id[1], id[2]);
+  const Fields& dst = B.s[0];  // pointer selection below
+  (void)dst;
+  if (zone_slot && !zone_active) {
+#pragma unroll
+    for (int c = 0; c < 5; c++) {
+      bool mod;
+      const double v = blk_gval(Dv, B, lt, b, own, c, id, s_u, mod);
+      const_cast<double*>(buf_arr(B, own, c))[z] = v;
+    }
+  }
+  double lo[3], hi[3];
+  bool anymod = false;
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    const int o1 = (d + 1) % 3, o2 = (d + 2) % 3;
+    if (extra[o1] || extra[o2]) { lo[d] = hi[d] = 0.0; continue; }
+    bool mod;
+    lo[d] = blk_gval(Dv, B, lt, b, own, 5 + d, id, s_u, mod);
+    if (mod) { const_cast<double*>(buf_arr(B, own, 5 + d))[z] = lo[d]; anymod = true; }
+    hi[d] = 0.0;
+    if (!extra[d]) {
+      int idp[3] = {id[0], id[1], id[2]};
+      idp[d] += 1;
+      hi[d] = blk_gval(Dv, B, lt, b, own, 5 + d, idp, s_u, mod);
+      anymod = anymod || mod;
+    }
+  }
+  if (zone_slot && (!zone_active || all || anymod)) {
+    const int4 inf = __ldg(Dv.B.info + b);
+    const double g = __ldg(Dv.gc + inf.y * Dv.B.tlev + GDET * L.n2d + inf.x + id[0] * Dv.B.ge2 + id[1]);
+    const Fields& f = B.s[0];
+    (void)f;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+      double* bc = own == 0 ? B.s[0].Bc[d] : (own == 1 ? B.s[1].Bc[d] : B.s[2].Bc[d]);
+      bc[z] = (lo[d] + hi[d]) / (2.0 * g);
+    }
+  }
+}
+
+// C-17 registers: R2 = sum over the steps inside one step of the next coarser level of dt_b F and
+// dt_b E of the corrector pass, on the faces and edges of the block boundary only.
+__global__ void __launch_bounds__(128) k_blk_registers(Dev Dv, int first, double dtfac) {
+  const Lay& L = Dv.L;
+  const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
+  const long long per = (long long)(L.n[0] + 1) * c1 * c2;
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= per * Dv.B.nact) return;
+  const int bslot = (int)(t / per);
+  t -= bslot * per;
+  const int b = __ldg(Dv.B.list + bslot);
+  const int id[3] = {(int)(t / ((long long)c2 * c1)), (int)((t / c2) % c1), (int)(t % c2)};
+  bool onb[3];
+  for (int d = 0; d < 3; d++) onb[d] = id[d] == 0 || id[d] == L.n[d];
+  if (!(onb[0] || onb[1] || onb[2])) return;
+  const long long z = (long long)b * Dv.B.blen + L.idx(id[0], id[1], id[2]);
+  const double dtb = dtfac * Dv.scal[S_DT];
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    const int e = (d + 1) % 3, f = (d + 2) % 3;
+    if (onb[d] && id[e] < L.n[e] && id[f] < L.n[f]) {  // a boundary face along d
+#pragma unroll
+      for (int c = 0; c < 5; c++) {
+        const double v = dtb * Dv.F[d][c][z];
+        Dv.B.FA2[d][c][z] = first ? v : Dv.B.FA2[d][c][z] + v;
+      }
+    }
+    // edge along d lies on the boundary if either transverse index does
+    if (id[d] < L.n[d] && (onb[e] || onb[f])) {
+      const double v = dtb * Dv.Ee[d][z];
+      Dv.B.EA2[d][z] = first ? v : Dv.B.EA2[d][z] + v;
+    }
+  }
+}
+
+// time-integrated EMF on edge f at index id[] of block c (time level tc, step dtc): the accumulated
+// register of a block on level tc - 1 that shares the edge (across the face, the other face, or the
+// diagonal, in that order), else the block's own dtc * E.  rep: the former.
+__device__ __forceinline__ double blk_edge_ec(const Dev& Dv, int c, int tc, int f, const int id[3], double dtc,
+                                              bool& rep) {
+  const Lay& L = Dv.L;
+  const int d = (f + 1) % 3, e = (f + 2) % 3;
+  const int od = id[d] == 0 ? -1 : (id[d] == L.n[d] ? 1 : 0);
+  const int oe = id[e] == 0 ? -1 : (id[e] == L.n[e] ? 1 : 0);
+  rep = false;
+  if (od != 0 || oe != 0) {
+    const int cand[3][2] = {{od, 0}, {0, oe}, {od, oe}};
+#pragma unroll
+    for (int t = 0; t < 3; t++) {
+      if (cand[t][0] == 0 && cand[t][1] == 0) continue;
+      int o[3] = {0, 0, 0};
+      o[d] = cand[t][0]; o[e] = cand[t][1];
+      const int q = __ldg(Dv.B.nbr + c * 27 + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
+      if (q < 0 || Dv.B.tau[q] != tc - 1) continue;
+      int lq[3] = {id[0], id[1], id[2]};
+      lq[d] -= o[d] * L.n[d];
+      lq[e] -= o[e] * L.n[e];
+      rep = true;
+      return Dv.B.EA2[f][(long long)q * Dv.B.blen + L.idx(lq[0], lq[1], lq[2])];
+    }
+  }
+  return dtc * Dv.Ee[f][(long long)c * Dv.B.blen + L.idx(id[0], id[1], id[2])];
+}
+
+// is the d-face at id[] of block c rebuilt by the correction, and with what?  Returns true and the new
+// value: base - curl(EC) if one of its four edges is shared with a finer block; the finer face
+// neighbour's own normal field on a face shared with it (C-17 correct(), steps 1-3 for the field).
+__device__ __forceinline__ bool blk_face_corr(const Dev& Dv, const Bufs& B, int c, int tc, int curc, int d,
+                                              const int id[3], double dtc, bool want_value, double& val) {
+  const Lay& L = Dv.L;
+  const int e = (d + 1) % 3, f = (d + 2) % 3;
+  // shared with a finer face neighbour: copy its field (it has completed both steps: its time-n state
+  // is at the coarse block's new time)
+  if (id[d] == 0 || id[d] == L.n[d]) {
+    int o[3] = {0, 0, 0};
+    o[d] = id[d] == 0 ? -1 : 1;
+    const int q = __ldg(Dv.B.nbr + c * 27 + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
+    if (q >= 0 && Dv.B.tau[q] == tc - 1) {
+      if (want_value) {
+        int lq[3] = {id[0], id[1], id[2]};
+        lq[d] = id[d] == 0 ? L.n[d] : 0;
+        val = buf_arr(B, Dv.B.cur[q], 5 + d)[(long long)q * Dv.B.blen + L.idx(lq[0], lq[1], lq[2])];
+      }
+      return true;
+    }
+  }
+  const int4 inf = __ldg(Dv.B.info + c);
+  if (d == 1 && Dv.metric == HAMR_METRIC_KERR_SCHILD && (inf.w + id[1] == 0 || inf.w + id[1] == Dv.B.n2g))
+    return false;  // pole faces stay 0
+  int ie[3] = {id[0], id[1], id[2]}, jf[3] = {id[0], id[1], id[2]};
+  ie[e] += 1;
+  jf[f] += 1;
+  bool r0, r1, r2, r3;
+  const double Ef0 = blk_edge_ec(Dv, c, tc, f, id, dtc, r0), Ef1 = blk_edge_ec(Dv, c, tc, f, ie, dtc, r1);
+  const double Ee0 = blk_edge_ec(Dv, c, tc, e, id, dtc, r2), Ee1 = blk_edge_ec(Dv, c, tc, e, jf, dtc, r3);
+  if (!(r0 || r1 || r2 || r3)) return false;
+  if (want_value) {
+    const double dxd[3] = {inf.y ? 0.5 * Dv.dx[0] : Dv.dx[0], Dv.dx[1], Dv.dx[2]};
+    const double curl = (Ef1 - Ef0) / dxd[e] - (Ee1 - Ee0) / dxd[f];
+    val = buf_arr(B, curc, 5 + d)[(long long)c * Dv.B.blen + L.idx(id[0], id[1], id[2])] - curl;
+  }
+  return true;
+}
+
+// correct(tau-1 -> tau), field part: rewrites the faces of the listed (level tau) blocks' new state
+__global__ void __launch_bounds__(128) k_blk_correct_faces(Dev Dv, Bufs B, int tc, double dtfac) {
+  const Lay& L = Dv.L;
+  const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
+  const long long per = (long long)(L.n[0] + 1) * c1 * c2;
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= per * Dv.B.nact) return;
+  const int bslot = (int)(t / per);
+  t -= bslot * per;
+  const int c = __ldg(Dv.B.list + bslot);
+  const int id[3] = {(int)(t / ((long long)c2 * c1)), (int)((t / c2) % c1), (int)(t % c2)};
+  // only faces within one zone of the block boundary can be touched
+  bool near = false;
+  for (int d = 0; d < 3; d++) near = near || id[d] <= 1 || id[d] >= L.n[d] - 1;
+  if (!near) return;
+  const int curc = Dv.B.cur[c];
+  const double dtc = dtfac * Dv.scal[S_DT];
+  const long long z = (long long)c * Dv.B.blen + L.idx(id[0], id[1], id[2]);
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    const int e = (d + 1) % 3, f = (d + 2) % 3;
+    if (id[e] >= L.n[e] || id[f] >= L.n[f]) continue;
+    double v;
+    if (blk_face_corr(Dv, B, c, tc, curc, d, id, dtc, true, v))
+      const_cast<double*>(buf_arr(B, 2 - curc, 5 + d))[z] = v;
+  }
+}
+
+// correct(tau-1 -> tau), zone part: flux difference into the boundary zones, new cell-centred field,
+// re-inversion of every touched zone
+__global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int tc, double dtfac) {
+  const Lay& L = Dv.L;
+  const long long per = (long long)L.n[0] * L.n[1] * L.n[2];
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0;
+  if (t < per * Dv.B.nact) {
+    const int bslot = (int)(t / per);
+    t -= bslot * per;
+    const int c = __ldg(Dv.B.list + bslot);
+    const int id[3] = {(int)(t / ((long long)L.n[2] * L.n[1])), (int)((t / L.n[2]) % L.n[1]), (int)(t % L.n[2])};
+    bool near = false;
+    for (int d = 0; d < 3; d++) near = near || id[d] == 0 || id[d] == L.n[d] - 1;
+    if (near) {
+      const int curc = Dv.B.cur[c];
+      const double dtc = dtfac * Dv.scal[S_DT];
+      const int4 inf = __ldg(Dv.B.info + c);
+      const double dxd[3] = {inf.y ? 0.5 * Dv.dx[0] : Dv.dx[0], Dv.dx[1], Dv.dx[2]};
+      const long long S[3] = {L.S1, L.S2, 1};
+      const long long z = (long long)c * Dv.B.blen + L.idx(id[0], id[1], id[2]);
+      bool touched = false;
+      double dU[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+      for (int d = 0; d < 3; d++) {
+#pragma unroll
+        for (int side = 0; side < 2; side++) {
+          int fi[3] = {id[0], id[1], id[2]};
+          fi[d] += side;
+          double dummy;
+          if (blk_face_corr(Dv, B, c, tc, curc, d, fi, dtc, false, dummy)) touched = true;
+          // flux difference on a face shared with a finer face neighbour
+          if ((side == 0 && id[d] == 0) || (side == 1 && id[d] == L.n[d] - 1)) {
+            int o[3] = {0, 0, 0};
+            o[d] = side ? 1 : -1;
+            const int q = __ldg(Dv.B.nbr + c * 27 + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
+            if (q >= 0 && Dv.B.tau[q] == tc - 1) {
+              int lq[3] = {id[0], id[1], id[2]};
+              lq[d] = side ? 0 : L.n[d];
+              const long long zq = (long long)q * Dv.B.blen + L.idx(lq[0], lq[1], lq[2]);
+              const long long zf = z + side * S[d];
+#pragma unroll
+              for (int cc = 0; cc < 5; cc++) {
+                const double dF = Dv.B.FA2[d][cc][zq] - dtc * Dv.F[d][cc][zf];
+                // U_new = U - (dt F_hi - dt F_lo)/dx: the high face enters with -, the low face with +
+                dU[cc] += (side ? -dF : dF) / dxd[d];
+              }
+              touched = true;
+            }
+          }
+        }
+      }
+      if (touched) {
+        const int q2 = inf.x + id[0] * Dv.B.ge2 + id[1];
+        const Geo G = load_geo(Dv.gc + inf.y * Dv.B.tlev, L.n2d, q2);
+        double P[8], U[5], Bn[3], Pn[5];
+        const int nw = 2 - curc;
+#pragma unroll
+        for (int cc = 0; cc < 5; cc++) P[cc] = buf_arr(B, nw, cc)[z];
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+          double* bc = nw == 0 ? B.s[0].Bc[d] : B.s[2].Bc[d];
+          P[5 + d] = bc[z];
+          const double* bf = buf_arr(B, nw, 5 + d);
+          Bn[d] = (bf[z] + bf[z + S[d]]) / (2.0 * G.gdet);
+          bc[z] = Bn[d];
+        }
+        St Sx;
+        get_state(P, G, Sx);
+        prim_to_U5(P, Sx, G.gdet, Dv.gam, U);
+#pragma unroll
+        for (int cc = 0; cc < 5; cc++) U[cc] += dU[cc];
+        if (con2prim(U, Bn, G, Dv.gam, P, Pn) != 0) {
+          nfail = 1;
+#pragma unroll
+          for (int cc = 0; cc < 5; cc++) Pn[cc] = P[cc];
+        }
+        const int fi = inf.z + id[0] + NG + inf.y * Dv.B.flev;
+        floors_ceiling(G, __ldg(Dv.rho_fl + fi), __ldg(Dv.u_fl + fi), Dv.gamma_max, Pn, nrf, nuf, ngc);
+#pragma unroll
+        for (int cc = 0; cc < 5; cc++) {
+          const_cast<double*>(buf_arr(B, nw, cc))[z] = Pn[cc];
+          if (!isfinite(Pn[cc])) bad = 1;
+        }
+      }
+    }
+  }
+  const unsigned m_f = __ballot_sync(0xffffffffu, nfail), m_r = __ballot_sync(0xffffffffu, nrf),
+                 m_u = __ballot_sync(0xffffffffu, nuf), m_g = __ballot_sync(0xffffffffu, ngc),
+                 m_b = __ballot_sync(0xffffffffu, bad);
+  if ((threadIdx.x & 31) == 0) {
+    if (m_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)__popc(m_f));
+    if (m_r) atomicAdd(Dv.cnt + N_RHOFL, (unsigned long long)__popc(m_r));
+    if (m_u) atomicAdd(Dv.cnt + N_UFL, (unsigned long long)__popc(m_u));
+    if (m_g) atomicAdd(Dv.cnt + N_GCEIL, (unsigned long long)__popc(m_g));
+    if (m_b) atomicAdd(Dv.cnt + N_NONFINITE, (unsigned long long)__popc(m_b));
+  }
+}
+
+// the listed blocks finished a step: their new state becomes their time-n state
+__global__ void k_blk_rotate(Dev Dv) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= Dv.B.nact) return;
+  const int b = Dv.B.list[t];
+  Dv.B.cur[b] = 2 - Dv.B.cur[b];
+}
+
+// C-14 on a block grid with one global dt: per-direction maximum of ctop / dx over the blocks, then
+// the harmonic sum (PAPER.md:93 fn. 2).  One CTA.  mode 0: set dt; 1: advance t by the dt just used first.
+__global__ void __launch_bounds__(256) k_blk_dt(Dev Dv, int mode) {
+  __shared__ double sm[3][8];
+  double m[3] = {0.0, 0.0, 0.0};
+  for (int b = threadIdx.x; b < Dv.B.nblk; b += blockDim.x) {
+    const int lev = Dv.B.info[b].y;
+    m[0] = fmax(m[0], Dv.B.ctopb[b * 3] / (lev ? 0.5 * Dv.dx[0] : Dv.dx[0]));
+    m[1] = fmax(m[1], Dv.B.ctopb[b * 3 + 1] / Dv.dx[1]);
+    m[2] = fmax(m[2], Dv.B.ctopb[b * 3 + 2] / Dv.dx[2]);
+  }
+  for (int d = 0; d < 3; d++) {
+    m[d] = warp_max(m[d]);
+    if ((threadIdx.x & 31) == 0) sm[d][threadIdx.x >> 5] = m[d];
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double* s = Dv.scal;
+    if (mode == 1) { s[S_T] += s[S_DT]; s[S_DTLAST] = s[S_DT]; }
+    double sum = 0.0;
+    for (int d = 0; d < 3; d++) {
+      double v = 0.0;
+      for (int w = 0; w < (int)(blockDim.x >> 5); w++) v = fmax(v, sm[d][w]);
+      sum += v;
+    }
+    s[S_DT] = Dv.cour / sum;
+  }
+}
+
+// LAT: one coarse step of 2^tmax finest steps has been taken; the host sets the next dt_0
+__global__ void k_blk_time(Dev Dv, double fac) {
+  Dv.scal[S_T] += fac * Dv.scal[S_DT];
+  Dv.scal[S_DTLAST] = Dv.scal[S_DT];
+}
+
+// dense global arrays <-> blocks (grids without x1 refinement).  stag: -1 zone-centred, else the face dim;
+// a face shared by two blocks is stored in both.
+__global__ void __launch_bounds__(256) k_blk_pack(Dev Dv, const double* __restrict__ dense, double* __restrict__ s0,
+                                                  double* __restrict__ s2, int stag, int zero_pole, int ng0, int ng1,
+                                                  int ng2) {
+  const Lay& L = Dv.L;
+  int m[3] = {L.n[0], L.n[1], L.n[2]};
+  int M[3] = {ng0, ng1, ng2};
+  if (stag >= 0) { m[stag] += 1; M[stag] += 1; }
+  const long long per = (long long)m[0] * m[1] * m[2];
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= per * Dv.B.nblk) return;
+  const int b = (int)(t / per);
+  t -= b * per;
+  const int k = (int)(t % m[2]), j = (int)((t / m[2]) % m[1]), i = (int)(t / ((long long)m[2] * m[1]));
+  const int4 inf = __ldg(Dv.B.info + b);
+  const int K0 = __ldg(Dv.B.K0 + b);
+  double v = dense ? dense[((long long)(inf.z + i) * M[1] + (inf.w + j)) * M[2] + (K0 + k)] : 0.0;
+  if (zero_pole && Dv.metric == HAMR_METRIC_KERR_SCHILD && (inf.w + j == 0 || inf.w + j == Dv.B.n2g)) v = 0.0;
+  (Dv.B.cur[b] ? s2 : s0)[(long long)b * Dv.B.blen + L.idx(i, j, k)] = v;
+}
+
+__global__ void __launch_bounds__(256) k_blk_unpack(Dev Dv, const double* __restrict__ s0, const double* __restrict__ s2,
+                                                    double* __restrict__ dense, int stag, int ng0, int ng1, int ng2) {
+  const Lay& L = Dv.L;
+  int m[3] = {L.n[0], L.n[1], L.n[2]};
+  int M[3] = {ng0, ng1, ng2};
+  if (stag >= 0) { m[stag] += 1; M[stag] += 1; }
+  const long long per = (long long)m[0] * m[1] * m[2];
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= per * Dv.B.nblk) return;
+  const int b = (int)(t / per);
+  t -= b * per;
+  const int k = (int)(t % m[2]), j = (int)((t / m[2]) % m[1]), i = (int)(t / ((long long)m[2] * m[1]));
+  const int4 inf = __ldg(Dv.B.info + b);
+  const int K0 = __ldg(Dv.B.K0 + b);
+  dense[((long long)(inf.z + i) * M[1] + (inf.w + j)) * M[2] + (K0 + k)] =
+      (Dv.B.cur[b] ? s2 : s0)[(long long)b * Dv.B.blen + L.idx(i, j, k)];
+}
+
+// ---- diagnostics on a block grid (C-11 div B, conserved totals, finite check) ----------------------------
+__global__ void __launch_bounds__(256) k_blk_diag(Dev Dv, Bufs B, int what) {
+  // what 0: max denominator of C-11; 1: max |div| / den; 2: conserved totals; 3: finite check
+  const Lay& L = Dv.L;
+  const long long per = (long long)L.n[0] * L.n[1] * L.n[2];
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  double val = 0.0, U[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  int bad = 0;
+  if (t < per * Dv.B.nblk) {
+    const int b = (int)(t / per);
+    t -= b * per;
+    const int k = (int)(t % L.n[2]), j = (int)((t / L.n[2]) % L.n[1]), i = (int)(t / ((long long)L.n[2] * L.n[1]));
+    const long long z = (long long)b * Dv.B.blen + L.idx(i, j, k);
+    const long long S[3] = {L.S1, L.S2, 1};
+    const int cur = Dv.B.cur[b];
+    const int4 inf = __ldg(Dv.B.info + b);
+    const double dxd[3] = {inf.y ? 0.5 * Dv.dx[0] : Dv.dx[0], Dv.dx[1], Dv.dx[2]};
+    const Fields& s = cur ? B.s[2] : B.s[0];
+    if (what <= 1) {
+      double div = 0.0, den = 0.0;
+      for (int d = 0; d < 3; d++) {
+        const double lo = s.Bf[d][z], hi = s.Bf[d][z + S[d]];
+        div += (hi - lo) / dxd[d];
+        den += (fabs(hi) + fabs(lo)) / (2.0 * dxd[d]);
+      }
+      if (what == 0) val = den;
+      else if (den > 1e-12 * Dv.scal[S_DENMAX]) val = fabs(div) / den;
+    } else if (what == 2) {
+      const Geo G = load_geo(Dv.gc + inf.y * Dv.B.tlev, L.n2d, inf.x + i * Dv.B.ge2 + j);
+      double P[8];
+      for (int c = 0; c < 5; c++) P[c] = s.P[c][z];
+      for (int c = 0; c < 3; c++) P[5 + c] = s.Bc[c][z];
+      St Sx;
+      get_state(P, G, Sx);
+      prim_to_U5(P, Sx, G.gdet, Dv.gam, U);
+      const double dV = dxd[0] * dxd[1] * dxd[2];
+      for (int c = 0; c < 5; c++) U[c] *= dV;
+    } else {
+      for (int c = 0; c < 5; c++) bad |= !isfinite(s.P[c][z]);
+      for (int c = 0; c < 3; c++) bad |= !isfinite(s.Bc[c][z]);
+    }
+  }
+  if (what <= 1) {
+    val = warp_max(val);
+    if ((threadIdx.x & 31) == 0 && val > 0.0) atomic_max_pos(Dv.scal + (what == 0 ? S_DENMAX : S_DIVB), val);
+  } else if (what == 2) {
+    for (int c = 0; c < 5; c++) {
+      double v = U[c];
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      if ((threadIdx.x & 31) == 0) atomicAdd(Dv.scal + S_TOT0 + c, v);
+    }
+  } else {
+    const unsigned m = __ballot_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(Dv.cnt + N_NONFINITE, (unsigned long long)__popc(m));
+  }
+}
+
+__global__ void k_blk_zero_scal(Dev Dv, int first, int count) {
+  for (int c = 0; c < count; c++) Dv.scal[first + c] = 0.0;
+}
+
+// ==== host side ==============================================================================================
+
+static Bufs bufs_of(const hamr_grid* g) {
+  Bufs B;
+  for (int i = 0; i < 3; i++) B.s[i] = g->s[i];
+  return B;
+}
+
+static LevT clocks_of(const hamr_grid* g) {
+  LevT lt;
+  for (int i = 0; i < 4; i++) { lt.tb[i] = g->bh.tb_u[i]; lt.dtu[i] = g->bh.dt_u[i]; lt.hasnew[i] = g->bh.has_new[i]; }
+  return lt;
+}
+
+// Dev of a launch over the blocks of list `which` (0..3: time level; 4: every block)
+static Dev dev_list(const hamr_grid* g, int which) {
+  Dev D = g->D;
+  D.B.list = g->bh.d_lists + (size_t)which * g->bh.nblk;
+  D.B.nact = which == 4 ? g->bh.nblk : g->bh.nlist[which];
+  return D;
+}
+
+int blk_count(const hamr_params& p, int nslot[3], int bn[3]) {
+  long long nb = 1;
+  for (int d = 0; d < 3; d++) {
+    bn[d] = p.nb[d] > 0 ? p.nb[d] : p.n[d];
+    if (bn[d] < NG || p.n[d] % bn[d] != 0) return 0;
+    nslot[d] = p.n[d] / bn[d];
+    nb *= nslot[d];
+  }
+  return nb > (1 << 20) ? 0 : (int)nb;
+}
+
+size_t blk_table_bytes(int nblk) {
+  // info (int4), nbr (27), phys, K0, tau, cur, 5 lists, 4 correction lists, ctopb (3 doubles)
+  return ((size_t)nblk * (16 + 4 * (27 + 4 + 5 + 4) + 24) + 1024 + 255) / 256 * 256;
+}
+
+// C-16: block lattice, neighbour table (periodic dimensions close through it), per-block table offsets
+int blk_setup(hamr_grid* g, void* tables) {
+  BlkHost& H = g->bh;
+  const hamr_params& p = g->par;
+  int bn[3];
+  const int nblk = blk_count(p, H.nslot, bn);
+  if (nblk <= 0) return HAMR_EINVAL;
+  H.on = true;
+  H.nblk = nblk;
+  H.tmax = p.lat_max_level > 0 ? p.lat_max_level : 0;
+  H.nbr.assign((size_t)nblk * 27, -1);
+  H.lev1.assign(nblk, 0);
+  H.tau.assign(nblk, 0);
+  H.I0.assign((size_t)nblk * 3, 0);
+  H.forced.clear();
+  BlkDev& B = g->D.B;
+  const int ge2 = p.n[1] + 2 * NG + 1;
+  std::vector<int> info((size_t)nblk * 4), phys(nblk), K0(nblk);
+  auto id_of = [&](int s0, int s1, int s2) { return (s0 * H.nslot[1] + s1) * H.nslot[2] + s2; };
+  for (int s0 = 0; s0 < H.nslot[0]; s0++)
+    for (int s1 = 0; s1 < H.nslot[1]; s1++)
+      for (int s2 = 0; s2 < H.nslot[2]; s2++) {
+        const int b = id_of(s0, s1, s2);
+        const int sl[3] = {s0, s1, s2};
+        const int I0[3] = {s0 * bn[0], s1 * bn[1], s2 * bn[2]};
+        for (int d = 0; d < 3; d++) H.I0[(size_t)b * 3 + d] = I0[d];
+        info[(size_t)b * 4 + 0] = (I0[0] + NG) * ge2 + I0[1] + NG;
+        info[(size_t)b * 4 + 1] = 0;
+        info[(size_t)b * 4 + 2] = I0[0];
+        info[(size_t)b * 4 + 3] = I0[1];
+        K0[b] = I0[2];
+        int ph = 0;
+        for (int d = 0; d < 3; d++) {
+          if (sl[d] == 0 && p.bc_lo[d] != HAMR_BC_PERIODIC) ph |= 1 << d;
+          if (sl[d] == H.nslot[d] - 1 && p.bc_hi[d] != HAMR_BC_PERIODIC) ph |= 8 << d;
+        }
+        phys[b] = ph;
+        for (int o0 = -1; o0 <= 1; o0++)
+          for (int o1 = -1; o1 <= 1; o1++)
+            for (int o2 = -1; o2 <= 1; o2++) {
+              const int o[3] = {o0, o1, o2};
+              int q[3];
+              bool inside = true;
+              for (int d = 0; d < 3; d++) {
+                q[d] = sl[d] + o[d];
+                if (q[d] < 0 || q[d] >= H.nslot[d]) {
+                  if (p.bc_lo[d] == HAMR_BC_PERIODIC) q[d] = (q[d] + H.nslot[d]) % H.nslot[d];
+                  else inside = false;
+                }
+              }
+              H.nbr[(size_t)b * 27 + (o0 + 1) * 9 + (o1 + 1) * 3 + (o2 + 1)] = inside ? id_of(q[0], q[1], q[2]) : -1;
+            }
+      }
+  char* t = (char*)tables;
+  auto take = [&](size_t bytes) { char* r = t; t += (bytes + 15) / 16 * 16; return r; };
+  int4* d_info = (int4*)take((size_t)nblk * 16);
+  int* d_nbr = (int*)take((size_t)nblk * 27 * 4);
+  int* d_phys = (int*)take((size_t)nblk * 4);
+  int* d_K0 = (int*)take((size_t)nblk * 4);
+  B.tau = (int*)take((size_t)nblk * 4);
+  B.cur = (int*)take((size_t)nblk * 4);
+  H.d_lists = (int*)take((size_t)nblk * 5 * 4);
+  H.d_clists = (int*)take((size_t)nblk * 4 * 4);
+  B.ctopb = (double*)take((size_t)nblk * 24);
+  B.info = d_info; B.nbr = d_nbr; B.phys = d_phys; B.K0 = d_K0;
+  B.list = H.d_lists; B.nact = 0;
+  if (cudaMallocHost((void**)&H.h_ctop, (size_t)nblk * 3 * sizeof(double)) != cudaSuccess) return HAMR_ECUDA;
+  if (cudaMallocHost((void**)&H.h_ints, (size_t)nblk * 10 * sizeof(int)) != cudaSuccess) return HAMR_ECUDA;
+  std::vector<int> all(nblk);
+  for (int b = 0; b < nblk; b++) all[b] = b;
+  cudaStream_t st = g->stream;
+  cudaError_t e = cudaSuccess;
+  auto up = [&](void* dst, const void* src, size_t bytes) {
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st);
+  };
+  up(d_info, info.data(), (size_t)nblk * 16);
+  up(d_nbr, H.nbr.data(), (size_t)nblk * 27 * 4);
+  up(d_phys, phys.data(), (size_t)nblk * 4);
+  up(d_K0, K0.data(), (size_t)nblk * 4);
+  up(H.d_lists, all.data(), (size_t)nblk * 4);                       // level 0 list (every block at tau = 0)
+  up(H.d_lists + (size_t)4 * nblk, all.data(), (size_t)nblk * 4);    // the list of every block
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);               // the host vectors go out of scope
+  for (int i = 0; i < 4; i++) { H.nlist[i] = 0; H.nclist[i] = 0; H.tb_u[i] = 0; H.dt_u[i] = 2 << i; H.has_new[i] = 0; }
+  H.nlist[0] = nblk;
+  H.dt0 = 0.0;
+  return e == cudaSuccess ? HAMR_OK : HAMR_ECUDA;
+}
+
+void blk_pack(hamr_grid* g, const double* dense, int kind, int stag, bool zero_pole) {
+  const Dev D = dev_list(g, 4);
+  const Lay& L = D.L;
+  int m[3] = {L.n[0], L.n[1], L.n[2]};
+  if (stag >= 0) m[stag] += 1;
+  const long long tot = (long long)m[0] * m[1] * m[2] * D.B.nblk;
+  double* a0 = kind < 5 ? g->s[0].P[kind] : g->s[0].Bf[kind - 5];
+  double* a2 = kind < 5 ? g->s[2].P[kind] : g->s[2].Bf[kind - 5];
+  Launch l_(g, K_OTHER);
+  k_blk_pack<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(D, dense, a0, a2, stag, zero_pole ? 1 : 0,
+                                                                   g->par.n[0], g->par.n[1], g->par.n[2]);
+}
+
+void blk_unpack(hamr_grid* g, int kind, double* dense) {
+  const Dev D = dev_list(g, 4);
+  const Lay& L = D.L;
+  const int stag = kind >= 8 ? kind - 8 : -1;
+  int m[3] = {L.n[0], L.n[1], L.n[2]};
+  if (stag >= 0) m[stag] += 1;
+  const long long tot = (long long)m[0] * m[1] * m[2] * D.B.nblk;
+  auto arr = [&](int buf) -> const double* {
+    const Fields& f = g->s[buf];
+    return kind < 5 ? f.P[kind] : (kind < 8 ? f.Bc[kind - 5] : f.Bf[kind - 8]);
+  };
+  Launch l_(g, K_OTHER);
+  k_blk_unpack<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(D, arr(0), arr(2), dense, stag, g->par.n[0],
+                                                                     g->par.n[1], g->par.n[2]);
+}
+
+static void blk_ghosts(hamr_grid* g, const Dev& D, int role, long long s_u, bool all, bool zero_ctop) {
+  if (D.B.nact == 0) return;
+  const Lay& L = D.L;
+  const long long tot = (long long)L.e1 * L.e2 * (L.n[2] + 2 * NG + 1) * D.B.nact;
+  Launch l_(g, K_GHOSTS);
+  k_blk_ghosts<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(D, bufs_of(g), clocks_of(g), role, s_u,
+                                                                     all ? 1 : 0, zero_ctop ? 1 : 0);
+}
+
+// one stage of C-12 on every block of time level tau (C-17)
+static void blk_stage(hamr_grid* g, int tau, bool corrector) {
+  BlkHost& H = g->bh;
+  const Dev D = dev_list(g, tau);
+  if (D.B.nact > 0) {
+    const long long s_u = H.tb_u[tau] + (corrector ? H.dt_u[tau] / 2 : 0);
+    blk_ghosts(g, D, corrector ? 1 : 0, s_u, false, corrector);
+    const Fields& s0 = g->s[0];
+    const Fields& s1 = g->s[1];
+    const Fields& s2 = g->s[2];
+    launch_flux_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2, corrector);
+    launch_ct_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2);
+    const double lev_fac = (double)(1 << tau);   // dt_b = 2^tau dt_0
+    if (corrector && tau < H.tmax) {
+      const int first = (H.tb_u[tau] % (2LL * H.dt_u[tau])) == 0 ? 1 : 0;
+      const Lay& L = D.L;
+      const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1) * D.B.nact;
+      Launch l_(g, K_OTHER);
+      k_blk_registers<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, first, lev_fac);
+    }
+    if (!corrector) {
+      const Roles ra = {s0, s0, s1}, rb = {s2, s2, s1};
+      launch_update_on(g, D, ra, rb, 0.5 * lev_fac, true);
+    } else {
+      const Roles ra = {s1, s0, s2}, rb = {s1, s2, s0};
+      launch_update_on(g, D, ra, rb, lev_fac, false);
+    }
+  }
+  if (corrector) H.has_new[tau] = 1;
+}
+
+// C-17 correct(tau-1 -> tau) on the level-tau blocks that touch a level tau-1 block
+static void blk_correct(hamr_grid* g, int tau) {
+  BlkHost& H = g->bh;
+  if (H.nclist[tau] == 0) return;
+  Dev D = g->D;
+  D.B.list = H.d_clists + (size_t)tau * H.nblk;
+  D.B.nact = H.nclist[tau];
+  const Lay& L = D.L;
+  const double lev_fac = (double)(1 << tau);
+  long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1) * D.B.nact;
+  {
+    Launch l_(g, K_OTHER);
+    k_blk_correct_faces<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, bufs_of(g), tau, lev_fac);
+  }
+  tot = (long long)L.n[0] * L.n[1] * L.n[2] * D.B.nact;
+  Launch l_(g, K_OTHER);
+  k_blk_correct_zones<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, bufs_of(g), tau, lev_fac);
+}
+
+static void blk_rotate(hamr_grid* g, int tau) {
+  BlkHost& H = g->bh;
+  const Dev D = dev_list(g, tau);
+  if (D.B.nact > 0) {
+    Launch l_(g, K_OTHER);
+    k_blk_rotate<<<(D.B.nact + 127) / 128, 128, 0, g->stream>>>(D);
+  }
+  H.tb_u[tau] += H.dt_u[tau];
+  H.has_new[tau] = 0;
+}
+
+// C-17: advance(tau) = predictor, first half of the finer levels, corrector, second half, correction
+static void blk_advance(hamr_grid* g, int tau) {
+  blk_stage(g, tau, false);
+  if (tau > 0) blk_advance(g, tau - 1);
+  blk_stage(g, tau, true);
+  if (tau > 0) {
+    blk_advance(g, tau - 1);
+    blk_correct(g, tau);
+  }
+  blk_rotate(g, tau);
+}
+
+// C-14 / C-17: the next dt and, under LAT, every block's time level.  after_step: a coarse step was just taken.
+static int blk_assign(hamr_grid* g, bool after_step) {
+  BlkHost& H = g->bh;
+  const int nblk = H.nblk;
+  cudaStream_t st = g->stream;
+  if (H.tmax == 0) {  // one global dt, found on the device; every block stays on level 0
+    Launch l_(g, K_DT);
+    k_blk_dt<<<1, 256, 0, st>>>(dev_list(g, 4), after_step ? 1 : 0);
+    for (int i = 0; i < 4; i++) { H.tb_u[i] = 0; H.dt_u[i] = 2 << i; H.has_new[i] = 0; }
+    return HAMR_OK;
+  }
+  if (after_step) {
+    Launch l_(g, K_DT);
+    k_blk_time<<<1, 1, 0, st>>>(g->D, (double)(1 << H.tmax));
+  }
+  if (cudaMemcpyAsync(H.h_ctop, g->D.B.ctopb, (size_t)nblk * 24, cudaMemcpyDeviceToHost, st) != cudaSuccess) return HAMR_ECUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return HAMR_ECUDA;
+  // per-block Courant step (PAPER.md:93 fn. 2), levels in factors of two above the smallest
+  std::vector<double> dtb(nblk);
+  double dt0 = 1e300;
+  for (int b = 0; b < nblk; b++) {
+    double s = 0.0;
+    for (int d = 0; d < 3; d++) {
+      const double dx = (d == 0 && H.lev1[b]) ? 0.5 * g->D.dx[0] : g->D.dx[d];
+      s += H.h_ctop[(size_t)b * 3 + d] / dx;
+    }
+    dtb[b] = g->D.cour / s;
+    dt0 = std::min(dt0, dtb[b]);
+  }
+  if (!H.forced.empty()) {
+    dt0 = 1e300;
+    for (int b = 0; b < nblk; b++) {
+      H.tau[b] = std::min(H.tmax, std::max(0, H.forced[b]));
+      dt0 = std::min(dt0, dtb[b] / (double)(1 << H.tau[b]));
+    }
+  } else {
+    for (int b = 0; b < nblk; b++) {
+      int tau = 0;
+      double lim = 2.0 * dt0;
+      while (tau < H.tmax && dtb[b] >= lim) { tau++; lim *= 2.0; }
+      H.tau[b] = tau;
+    }
+  }
+  // neighbours across faces, edges and corners differ by at most one level
+  std::vector<int> nt(nblk);
+  for (bool changed = true; changed;) {
+    changed = false;
+    for (int b = 0; b < nblk; b++) {
+      int t = H.tau[b];
+      for (int a = 0; a < 27; a++) {
+        const int q = H.nbr[(size_t)b * 27 + a];
+        if (q >= 0) t = std::min(t, H.tau[q] + 1);
+      }
+      nt[b] = t;
+      if (t != H.tau[b]) changed = true;
+    }
+    H.tau = nt;
+  }
+  // lists per level; correction lists; upload
+  int* hl = H.h_ints;                       // [4][nblk] lists, [4][nblk] correction lists, [nblk] tau
+  for (int i = 0; i < 4; i++) { H.nlist[i] = 0; H.nclist[i] = 0; }
+  for (int b = 0; b < nblk; b++) {
+    const int t = H.tau[b];
+    hl[(size_t)t * nblk + H.nlist[t]++] = b;
+    bool any = false;
+    for (int a = 0; a < 27 && !any; a++) {
+      const int q = H.nbr[(size_t)b * 27 + a];
+      any = q >= 0 && H.tau[q] == t - 1;
+    }
+    if (any) hl[(size_t)(4 + t) * nblk + H.nclist[t]++] = b;
+    hl[(size_t)8 * nblk + b] = t;
+  }
+  cudaError_t e = cudaMemcpyAsync(H.d_lists, hl, (size_t)4 * nblk * 4, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(H.d_clists, hl + (size_t)4 * nblk, (size_t)4 * nblk * 4, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(g->D.B.tau, hl + (size_t)8 * nblk, (size_t)nblk * 4, cudaMemcpyHostToDevice, st);
+  H.dt0 = dt0;
+  g->h_pinned[56] = dt0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(g->D.scal + S_DT, g->h_pinned + 56, sizeof(double), cudaMemcpyHostToDevice, st);
+  for (int i = 0; i < 4; i++) { H.tb_u[i] = 0; H.dt_u[i] = 2 << i; H.has_new[i] = 0; }
+  return e == cudaSuccess ? HAMR_OK : HAMR_ECUDA;
+}
+
+int blk_set_levels(hamr_grid* g, const int* tau) {
+  BlkHost& H = g->bh;
+  if (!H.on) return HAMR_EINVAL;
+  H.forced.clear();
+  if (tau) H.forced.assign(tau, tau + H.nblk);
+  return HAMR_OK;
+}
+
+// after the state has been packed: every block on level 0, ghost fill, one flux pass for the first dt (C-14)
+int blk_initial(hamr_grid* g) {
+  BlkHost& H = g->bh;
+  cudaStream_t st = g->stream;
+  std::fill(H.tau.begin(), H.tau.end(), 0);
+  for (int i = 0; i < 4; i++) { H.nlist[i] = 0; H.nclist[i] = 0; H.tb_u[i] = 0; H.dt_u[i] = 2 << i; H.has_new[i] = 0; }
+  H.nlist[0] = H.nblk;
+  if (cudaMemsetAsync(g->D.B.tau, 0, (size_t)H.nblk * 4, st) != cudaSuccess) return HAMR_ECUDA;
+  // level-0 list = every block
+  if (cudaMemcpyAsync(H.d_lists, H.d_lists + (size_t)4 * H.nblk, (size_t)H.nblk * 4, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+    return HAMR_ECUDA;
+  const Dev D = dev_list(g, 4);
+  blk_ghosts(g, D, 0, 0, true, true);
+  launch_flux_on(g, D, g->s[0], g->s[2], true);
+  return blk_assign(g, false);
+}
+
+int blk_step(hamr_grid* g, int nsteps) {
+  for (int s = 0; s < nsteps; s++) {
+    blk_advance(g, g->bh.tmax);
+    const int rc = blk_assign(g, true);
+    if (rc != HAMR_OK) return rc;
+  }
+  return HAMR_OK;
+}
+
+static void blk_diag(hamr_grid* g, int what) {
+  const Dev D = dev_list(g, 4);
+  const Lay& L = D.L;
+  const long long tot = (long long)L.n[0] * L.n[1] * L.n[2] * D.B.nblk;
+  Launch l_(g, K_OTHER);
+  k_blk_diag<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(D, bufs_of(g), what);
+}
+
+void blk_divb(hamr_grid* g) {
+  g->launches++;
+  k_blk_zero_scal<<<1, 1, 0, g->stream>>>(g->D, S_DENMAX, 2);
+  blk_diag(g, 0);
+  blk_diag(g, 1);
+}
+
+void blk_totals(hamr_grid* g) {
+  g->launches++;
+  k_blk_zero_scal<<<1, 1, 0, g->stream>>>(g->D, S_TOT0, 5);
+  blk_diag(g, 2);
+}
+
+void blk_check_finite(hamr_grid* g) { blk_diag(g, 3); }
+
+}  // namespace hamr

@@ -8,19 +8,26 @@
 namespace hamr {
 
 // centre EMFs on active zones plus one ghost layer
-__global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s) {
+template <bool BLK>
+__global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s0, Fields s2) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + 2, c1 = L.n[1] + 2;
-  const long long tot = (long long)(L.n[0] + 2) * c1 * c2;
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= tot) return;
+  const long long per = (long long)(L.n[0] + 2) * c1 * c2;
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (BLK ? per * Dv.B.nact : per)) return;
+  int bslot = 0;
+  if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
+  const BCtx C = blk_ctx<BLK>(Dv, bslot);
   const int k = (int)(t % c2) - 1;
   const int j = (int)((t / c2) % c1) - 1;
   const int i = (int)(t / ((long long)c2 * c1)) - 1;
-  const long long z = L.idx(i, j, k);
-  const int q = L.idx2(i, j);
-  const double* gc = Dv.gc;
+  const long long z = C.zoff + L.idx(i, j, k);
+  const int q = C.q0 + i * (BLK ? Dv.B.ge2 : L.e2) + j;
+  const double* gc = Dv.gc + (BLK ? C.lev * Dv.B.tlev : 0);
   const int n2d = L.n2d;
+  Fields s;
+  for (int c = 2; c < 5; c++) s.P[c] = selp<BLK>(s0.P[c], s2.P[c], C.cur);
+  for (int c = 0; c < 3; c++) s.Bc[c] = selp<BLK>(s0.Bc[c], s2.Bc[c], C.cur);
   const double c11 = __ldg(gc + C11 * n2d + q), c13 = __ldg(gc + C13 * n2d + q), c22 = __ldg(gc + C22 * n2d + q),
                c33 = __ldg(gc + C33 * n2d + q), gdet = __ldg(gc + GDET * n2d + q),
                ialpha = __ldg(gc + IALPHA * n2d + q), boa = __ldg(gc + BOA * n2d + q);
@@ -52,17 +59,21 @@ __device__ __forceinline__ double edge_emf(const double* __restrict__ X, const d
 }
 
 // one thread per zone corner: the three edge EMFs on the low edges of zone (i,j,k), 0 <= idx <= n
+template <bool BLK>
 __global__ void __launch_bounds__(128) k_edge_emf(Dev Dv) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
-  const long long tot = (long long)(L.n[0] + 1) * c1 * c2;
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= tot) return;
+  const long long per = (long long)(L.n[0] + 1) * c1 * c2;
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (BLK ? per * Dv.B.nact : per)) return;
+  int bslot = 0;
+  if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
+  const BCtx C = blk_ctx<BLK>(Dv, bslot);
   const int k = (int)(t % c2);
   const int j = (int)((t / c2) % c1);
   const int i = (int)(t / ((long long)c2 * c1));
-  const long long z = L.idx(i, j, k);
-  const bool pole = Dv.metric == HAMR_METRIC_KERR_SCHILD && (j == 0 || j == L.n[1]);
+  const long long z = C.zoff + L.idx(i, j, k);
+  const bool pole = Dv.metric == HAMR_METRIC_KERR_SCHILD && (C.J0 + j == 0 || C.J0 + j == (BLK ? Dv.B.n2g : L.n[1]));
   const long long S[3] = {L.S1, L.S2, 1};
   const int id[3] = {i, j, k};
 #pragma unroll
@@ -77,16 +88,23 @@ __global__ void __launch_bounds__(128) k_edge_emf(Dev Dv) {
   }
 }
 
-void launch_ct(hamr_grid* g, const Fields& src) {
-  const Lay& L = g->D.L;
-  long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 2);
+void launch_ct_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2) {
+  const Lay& L = Dv.L;
+  const bool blk = Dv.B.nblk > 0;
+  if (blk && Dv.B.nact == 0) return;
+  const long long mult = blk ? Dv.B.nact : 1;
+  long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 2) * mult;
   {
     Launch l_(g, K_CEMF);
-    k_centre_emf<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(g->D, src);
+    if (blk) k_centre_emf<true><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
+    else k_centre_emf<false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
   }
-  tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);
+  tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1) * mult;
   Launch l_(g, K_EDGE);
-  k_edge_emf<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(g->D);
+  if (blk) k_edge_emf<true><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv);
+  else k_edge_emf<false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv);
 }
+
+void launch_ct(hamr_grid* g, const Fields& src) { launch_ct_on(g, g->D, src, src); }
 
 }  // namespace hamr

@@ -192,6 +192,24 @@ __device__ __forceinline__ void zero_face(const Dev& Dv, int D, int z) {
   Dv.EfB[D][z] = 0.0;
 }
 
+// C-14 / H5: per-direction maximum signal speed: warp-shuffle max, then one atomic max per warp on the
+// bit pattern of the positive double.  BLK: one maximum per block (a warp may straddle two blocks).
+template <bool BLK>
+__device__ __forceinline__ void ctop_commit(const Dev& Dv, int D, int b, double ctop) {
+  if (!BLK) {
+    ctop = warp_max(ctop);
+    if ((threadIdx.x & 31) == 0 && ctop > 0.0) atomic_max_pos(Dv.scal + S_CTOP0 + D, ctop);
+    return;
+  }
+  const int b0 = __shfl_sync(0xffffffffu, b, 0);
+  if (__all_sync(0xffffffffu, b == b0)) {
+    ctop = warp_max(ctop);
+    if ((threadIdx.x & 31) == 0 && ctop > 0.0) atomic_max_pos(Dv.B.ctopb + b0 * 3 + D, ctop);
+  } else if (ctop > 0.0) {
+    atomic_max_pos(Dv.B.ctopb + b * 3 + D, ctop);
+  }
+}
+
 // ---- sweeps along x1 / x2: a thread marches along the sweep direction ---------------------------------
 // grid.x covers the flattened transverse index (other, k), k fastest; grid.y the segments of `seg` faces.
 // PPM: the thread carries, per variable, a_j, a_{j+1}, the limited slope of zone j and the interface
@@ -210,24 +228,38 @@ constexpr int MARCH_UNROLL = HAMR_MARCH_UNROLL;
 #ifndef HAMR_X3_MINB
 #define HAMR_X3_MINB 5
 #endif
-template <int D, int RECON>
-__global__ void __launch_bounds__(128, HAMR_MARCH_MINB) k_flux_march(Dev Dv, Fields s, int seg, int want_ctop) {
+// BLK: the launch covers the blocks of Dv.B.list (block-structured grid, H7); s / s2 are the buffer sets
+// holding the stage source of blocks with cur == 0 / cur == 2.
+template <int D, int RECON, bool BLK>
+__global__ void __launch_bounds__(128, HAMR_MARCH_MINB) k_flux_march(Dev Dv, Fields s, Fields s2, int seg,
+                                                                      int want_ctop) {
   static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   const Lay& L = Dv.L;
   constexpr int O = 1 - D;          // the other non-x3 dimension
   constexpr int e = (D + 1) % 3, f = (D + 2) % 3;
   const int ck = L.n[2] + 2;
-  const int tf = blockIdx.x * blockDim.x + threadIdx.x;
+  const int ntr = (L.n[O] + 2) * ck;
+  int tf = blockIdx.x * blockDim.x + threadIdx.x;
+  int bslot = 0;
+  if (BLK) { bslot = tf / ntr; tf -= bslot * ntr; }
+  const bool live = BLK ? bslot < Dv.B.nact : tf < ntr;
+  const BCtx C = blk_ctx<BLK>(Dv, BLK ? min(bslot, Dv.B.nact - 1) : 0);
+  const int ge2 = BLK ? Dv.B.ge2 : L.e2, n2g = BLK ? Dv.B.n2g : L.n[1];
   double ctop = 0.0;
-  if (tf < (L.n[O] + 2) * ck) {
+  if (live) {
     const int k = tf % ck - 1, o = tf / ck - 1;
     const int f0 = blockIdx.y * seg, f1 = min(f0 + seg, L.n[D] + 1);
     const int sd = (D == 0) ? L.S1 : L.S2;
     const bool act = o >= 0 && o < L.n[O] && k >= 0 && k < L.n[2];  // C-14: faces of ACTIVE zones
     const bool ks = Dv.metric == HAMR_METRIC_KERR_SCHILD;
-    const double* var[7] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[e], s.Bc[f]};
+    const double* var[7] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
+                            selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),
+                            selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[e], s2.Bc[e], C.cur),
+                            selp<BLK>(s.Bc[f], s2.Bc[f], C.cur)};
+    const double* bfn = selp<BLK>(s.Bf[D], s2.Bf[D], C.cur);
+    const double* gtab = (D == 0 ? Dv.gf1 : Dv.gf2) + (BLK ? C.lev * Dv.B.tlev : 0);
     constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
-    int z = (int)L.idx(D == 0 ? f0 - 1 : o, D == 0 ? o : f0 - 1, k);
+    int z = C.zoff + (int)L.idx(D == 0 ? f0 - 1 : o, D == 0 ? o : f0 - 1, k);
     double PL[8], PR[8];
     double a0[7], a1[7], dm[7], il[7];  // PPM marching state (unused for PLM)
     // the zone below the first face: its right edge, and the marching state of the next zone
@@ -272,13 +304,13 @@ __global__ void __launch_bounds__(128, HAMR_MARCH_MINB) k_flux_march(Dev Dv, Fie
           plm_edges(a[-sd], a[0], a[sd], PR[slot[v]], carry[v]);
         }
       }
-      const bool pole = (D == 1) && ks && (fc == 0 || fc == L.n[1]);
+      const bool pole = (D == 1) && ks && (C.J0 + fc == 0 || C.J0 + fc == n2g);
       if (pole) {  // C-7: pole faces carry no flux and no state is evaluated there
         zero_face(Dv, D, z);
       } else {
-        const int q = (D == 0) ? L.idx2(fc, o) : L.idx2(o, fc);
-        const FGeo G = load_fgeo<D>(D == 0 ? Dv.gf1 : Dv.gf2, L.n2d, q);
-        PL[5 + D] = PR[5 + D] = s.Bf[D][z] * G.igdet;  // C-5: the normal field is single-valued at the face
+        const int q = C.q0 + ((D == 0) ? fc * ge2 + o : o * ge2 + fc);
+        const FGeo G = load_fgeo<D>(gtab, L.n2d, q);
+        PL[5 + D] = PR[5 + D] = bfn[z] * G.igdet;  // C-5: the normal field is single-valued at the face
         const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
         if (act) ctop = dmax(ctop, ct);
       }
@@ -286,10 +318,7 @@ __global__ void __launch_bounds__(128, HAMR_MARCH_MINB) k_flux_march(Dev Dv, Fie
       for (int v = 0; v < 7; v++) PL[slot[v]] = carry[v];
     }
   }
-  if (want_ctop) {
-    ctop = warp_max(ctop);
-    if ((threadIdx.x & 31) == 0 && ctop > 0.0) atomic_max_pos(Dv.scal + S_CTOP0 + D, ctop);
-  }
+  if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
 }
 
 // ---- sweep along x3: one lane per zone, neighbouring lanes exchange slopes and edges -------------------
@@ -297,25 +326,32 @@ __global__ void __launch_bounds__(128, HAMR_MARCH_MINB) k_flux_march(Dev Dv, Fie
 // owns 32 consecutive zones of which the first HLO and the last HHI only help.
 // PPM (HLO = 2, HHI = 1): every lane builds the limited slope of ITS zone once; slopes, interface
 // values and right edges travel between lanes by warp shuffle.  PLM (HLO = 1, HHI = 0).
-template <int RECON>
-__global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s, int want_ctop) {
+template <int RECON, bool BLK>
+__global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s, Fields s2, int want_ctop) {
   constexpr int D = 2;
   constexpr int HLO = (RECON == HAMR_RECON_PPM) ? 2 : 1, HHI = (RECON == HAMR_RECON_PPM) ? 1 : 0;
   constexpr int OWN = 32 - HLO - HHI;
   constexpr unsigned FULL = 0xffffffffu;
   const Lay& L = Dv.L;
   const int ck = L.n[2] + 1 + HLO + HHI, cj = L.n[1] + 2;
-  const long long tot = (long long)(L.n[0] + 2) * cj * ck;
+  const long long per = (long long)(L.n[0] + 2) * cj * ck;
+  const long long tot = BLK ? per * Dv.B.nact : per;
   const int lane = threadIdx.x & 31;
   const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   long long t = warp * OWN + lane - HLO;
   const bool valid = t >= 0 && t < tot;
   t = t < 0 ? 0 : (t >= tot ? tot - 1 : t);  // clamped lanes compute on a real zone and store nothing
+  int bslot = 0;
+  if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
+  const BCtx C = blk_ctx<BLK>(Dv, bslot);
   const int k = (int)(t % ck) - HLO;
   const int j = (int)((t / ck) % cj) - 1;
   const int i = (int)(t / ((long long)ck * cj)) - 1;
-  const int z = (int)L.idx(i, j, k);
-  const double* var[7] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[0], s.Bc[1]};
+  const int z = C.zoff + (int)L.idx(i, j, k);
+  const double* var[7] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
+                          selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),
+                          selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[0], s2.Bc[0], C.cur),
+                          selp<BLK>(s.Bc[1], s2.Bc[1], C.cur)};
   double PL[8], PR[8];
 #pragma unroll
   for (int v = 0; v < 7; v++) {
@@ -336,29 +372,28 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
   }
   double ctop = 0.0;
   if (valid && lane >= HLO && lane < 32 - HHI && k >= 0 && k <= L.n[2]) {
-    const FGeo G = load_fgeo<D>(Dv.gc, L.n2d, L.idx2(i, j));
-    PL[7] = PR[7] = s.Bf[2][z] * G.igdet;
+    const int ge2 = BLK ? Dv.B.ge2 : L.e2;
+    const FGeo G = load_fgeo<D>(Dv.gc + (BLK ? C.lev * Dv.B.tlev : 0), L.n2d, C.q0 + i * ge2 + j);
+    PL[7] = PR[7] = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z] * G.igdet;
     const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
     if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct;
   }
-  if (want_ctop) {
-    ctop = warp_max(ctop);
-    if (lane == 0 && ctop > 0.0) atomic_max_pos(Dv.scal + S_CTOP0 + D, ctop);
-  }
+  if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
 }
 
 // picks the number of faces per marching segment so that the grid fills whole waves of resident
 // blocks (148 SMs x blocks per SM) with little prologue overhead
-template <int D, int RECON>
+template <int D, int RECON, bool BLK>
 static int pick_segment(const Lay& L, int nbx) {
-  static int cached_seg = 0, cached_key = -1;
+  static int cached_seg = 0;
+  static long long cached_key = -1;
   const int nf = L.n[D] + 1;
-  const int key = nf * 4096 + nbx;
+  const long long key = (long long)nf * (1LL << 32) + nbx;
   if (key == cached_key) return cached_seg;
   int dev = 0, sms = 148, per_sm = 2;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_flux_march<D, RECON>, 128, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_flux_march<D, RECON, BLK>, 128, 0);
   if (per_sm < 1) per_sm = 1;
   const double slots = (double)sms * per_sm;
   double best = -1.0;
@@ -378,36 +413,46 @@ static int pick_segment(const Lay& L, int nbx) {
   return best_seg;
 }
 
-template <int D>
-static void launch_march(hamr_grid* g, const Fields& src, bool want_ctop) {
-  const Lay& L = g->D.L;
+template <int D, int RECON, bool BLK>
+static void launch_march_t(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
+  const Lay& L = Dv.L;
   const int O = 1 - D;
-  const int ntr = (L.n[O] + 2) * (L.n[2] + 2);
-  const int nbx = (ntr + 127) / 128;
-  Launch l_(g, K_FLUX1 + D);
-  if (g->D.recon == HAMR_RECON_PPM) {
-    const int seg = pick_segment<D, HAMR_RECON_PPM>(L, nbx);
-    dim3 grid(nbx, (L.n[D] + 1 + seg - 1) / seg);
-    k_flux_march<D, HAMR_RECON_PPM><<<grid, 128, 0, g->stream>>>(g->D, src, seg, want_ctop ? 1 : 0);
-  } else {
-    const int seg = pick_segment<D, HAMR_RECON_PLM_MC>(L, nbx);
-    dim3 grid(nbx, (L.n[D] + 1 + seg - 1) / seg);
-    k_flux_march<D, HAMR_RECON_PLM_MC><<<grid, 128, 0, g->stream>>>(g->D, src, seg, want_ctop ? 1 : 0);
-  }
+  const long long ntr = (long long)(L.n[O] + 2) * (L.n[2] + 2) * (BLK ? Dv.B.nact : 1);
+  const int nbx = (int)((ntr + 127) / 128);
+  const int seg = pick_segment<D, RECON, BLK>(L, nbx);
+  dim3 grid(nbx, (L.n[D] + 1 + seg - 1) / seg);
+  k_flux_march<D, RECON, BLK><<<grid, 128, 0, g->stream>>>(Dv, src, src2, seg, want_ctop ? 1 : 0);
 }
 
-void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop) {
-  launch_march<0>(g, src, want_ctop);
-  launch_march<1>(g, src, want_ctop);
-  const Lay& L = g->D.L;
-  const bool ppm = g->D.recon == HAMR_RECON_PPM;
+template <int D>
+static void launch_march(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
+  Launch l_(g, K_FLUX1 + D);
+  const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
+  if (ppm && !blk) launch_march_t<D, HAMR_RECON_PPM, false>(g, Dv, src, src2, want_ctop);
+  else if (ppm) launch_march_t<D, HAMR_RECON_PPM, true>(g, Dv, src, src2, want_ctop);
+  else if (!blk) launch_march_t<D, HAMR_RECON_PLM_MC, false>(g, Dv, src, src2, want_ctop);
+  else launch_march_t<D, HAMR_RECON_PLM_MC, true>(g, Dv, src, src2, want_ctop);
+}
+
+// src / src2: the stage source in the buffer sets of blocks with cur == 0 / 2 (monolithic: src2 unused)
+void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
+  if (Dv.B.nblk > 0 && Dv.B.nact == 0) return;
+  launch_march<0>(g, Dv, src, src2, want_ctop);
+  launch_march<1>(g, Dv, src, src2, want_ctop);
+  const Lay& L = Dv.L;
+  const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
   const int own = ppm ? 29 : 31, halo = ppm ? 3 : 1;
-  const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 1 + halo);
+  const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 1 + halo) * (blk ? Dv.B.nact : 1);
   const long long warps = (tot + own - 1) / own + 1;
   const unsigned nb = (unsigned)((warps + 3) / 4);
   Launch l_(g, K_FLUX3);
-  if (ppm) k_flux_x3<HAMR_RECON_PPM><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
-  else k_flux_x3<HAMR_RECON_PLM_MC><<<nb, 128, 0, g->stream>>>(g->D, src, want_ctop ? 1 : 0);
+  const int wc = want_ctop ? 1 : 0;
+  if (ppm && !blk) k_flux_x3<HAMR_RECON_PPM, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+  else if (ppm) k_flux_x3<HAMR_RECON_PPM, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+  else if (!blk) k_flux_x3<HAMR_RECON_PLM_MC, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+  else k_flux_x3<HAMR_RECON_PLM_MC, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
 }
+
+void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop) { launch_flux_on(g, g->D, src, src, want_ctop); }
 
 }  // namespace hamr

@@ -78,27 +78,28 @@ __device__ static void store_geo(double* tab, int n2d, int q, const Geo& G) {
   tab[IGDET * n2d + q] = G.gdet > 0.0 ? 1.0 / G.gdet : 0.0;
 }
 
-__global__ void k_geometry(Dev D, double* gc, double* gf1, double* gf2, double* dgc, double* rho_fl,
-                           double* u_fl) {
+// e1 x e2 table entries; entry (ti, tj) is the zone with index (ti - NG, tj - NG) counted from the
+// domain's low corner in zones of spacing dx1 (the table of one x1 refinement level), n2glob zones in x2
+__global__ void k_geometry(Dev D, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
+                           double* gf2, double* dgc, double* rho_fl, double* u_fl) {
   const int q = blockIdx.x * blockDim.x + threadIdx.x;
-  const Lay& L = D.L;
-  if (q >= L.n2d) return;
-  const int i = q / L.e2 - NG, j = q % L.e2 - NG;
-  const double xc1 = D.x0[0] + ((double)i + 0.5) * D.dx[0], xf1 = D.x0[0] + (double)i * D.dx[0];
+  if (q >= e1 * e2) return;
+  const int i = q / e2 - NG, j = q % e2 - NG;
+  const double xc1 = D.x0[0] + ((double)i + 0.5) * dx1, xf1 = D.x0[0] + (double)i * dx1;
   const double xc2 = D.x0[1] + ((double)j + 0.5) * D.dx[1], xf2 = D.x0[1] + (double)j * D.dx[1];
   Geo G;
   double d1[NDG], d2[NDG];
   metric_at(D.metric, D.a, xc1, xc2, G, d1, d2);
-  store_geo(gc, L.n2d, q, G);
+  store_geo(gc, n2d, q, G);
   for (int c = 0; c < NDG; c++) {
-    dgc[c * L.n2d + q] = d1[c];
-    dgc[(NDG + c) * L.n2d + q] = d2[c];
+    dgc[c * n2d + q] = d1[c];
+    dgc[(NDG + c) * n2d + q] = d2[c];
   }
   metric_at(D.metric, D.a, xf1, xc2, G, d1, d2);
-  store_geo(gf1, L.n2d, q, G);
+  store_geo(gf1, n2d, q, G);
   metric_at(D.metric, D.a, xc1, xf2, G, d1, d2);
-  if (D.metric == HAMR_METRIC_KERR_SCHILD && (j == 0 || j == L.n[1])) G.gdet = 0.0;  // pole faces (C-7)
-  store_geo(gf2, L.n2d, q, G);
+  if (D.metric == HAMR_METRIC_KERR_SCHILD && (j == 0 || j == n2glob)) G.gdet = 0.0;  // pole faces (C-7)
+  store_geo(gf2, n2d, q, G);
   if (j == -NG) {  // floors depend on x1 only (C-13): coef * r^pow, r = 1 on the Cartesian map
     const double r = (D.metric == HAMR_METRIC_KERR_SCHILD) ? exp(xc1) : 1.0;
     rho_fl[i + NG] = D.rho_fl_coef * pow(r, D.rho_fl_pow);
@@ -106,11 +107,17 @@ __global__ void k_geometry(Dev D, double* gc, double* gf1, double* gf2, double* 
   }
 }
 
+void launch_geometry_tab(hamr_grid* g, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
+                         double* gf2, double* dgc, double* rho_fl, double* u_fl) {
+  Launch l_(g, K_OTHER);
+  k_geometry<<<(e1 * e2 + 127) / 128, 128, 0, g->stream>>>(g->D, e1, e2, n2d, dx1, n2glob, gc, gf1, gf2, dgc,
+                                                         rho_fl, u_fl);
+}
+
 void launch_geometry(hamr_grid* g, double* gc, double* gf1, double* gf2, double* dgc, double* rho_fl,
                      double* u_fl) {
-  const int n = g->D.L.n2d;
-  Launch l_(g, K_OTHER);
-  k_geometry<<<(n + 127) / 128, 128, 0, g->stream>>>(g->D, gc, gf1, gf2, dgc, rho_fl, u_fl);
+  const Lay& L = g->D.L;
+  launch_geometry_tab(g, L.e1, L.e2, L.n2d, g->D.dx[0], L.n[1], gc, gf1, gf2, dgc, rho_fl, u_fl);
 }
 
 }  // namespace hamr

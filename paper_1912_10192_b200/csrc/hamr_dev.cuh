@@ -196,4 +196,90 @@ __device__ __forceinline__ double warp_max(double v) {
   return v;
 }
 
+// C-13: 2-unknown (W = w gamma^2, v^2) Newton-Raphson.  U: densitised hydro rows; Bc: NEW cell-centred
+// field; Pg: guess (the stage's source state).  Returns 0 ok, 1 no convergence, 2 non-finite.
+__device__ __forceinline__ int con2prim(const double U[5], const double Bc[3], const Geo& G, double gam_ad,
+                                        const double Pg[5], double Pout[5]) {
+  const double ig = 1.0 / G.gdet;
+  const double alpha = G.alpha;
+  const double rhout = U[0] * ig;
+  const double D = alpha * rhout;
+  // Q_mu = alpha T^t_mu with rho u^t removed from the energy row (C-4)
+  const double Q0 = alpha * (U[1] * ig - rhout), Q1 = alpha * (U[2] * ig), Q2 = alpha * (U[3] * ig),
+               Q3 = alpha * (U[4] * ig);
+  const double B1 = alpha * Bc[0], B2 = alpha * Bc[1], B3 = alpha * Bc[2];
+  const double Qc0 = G.k00 * Q0 + G.k01 * Q1;
+  const double Qc1 = G.k01 * Q0 + G.k11 * Q1 + G.k13 * Q3;
+  const double Qc2 = G.k22 * Q2;
+  const double Qc3 = G.k13 * Q1 + G.k33 * Q3;
+  const double n0 = -alpha * G.k00, n1 = -alpha * G.k01;  // n^mu = -alpha g^{mu t}; n^2 = n^3 = 0
+  const double Qdotn = Q0 * n0 + Q1 * n1;
+  const double QQ = Q0 * Qc0 + Q1 * Qc1 + Q2 * Qc2 + Q3 * Qc3;
+  const double Qtsq = QQ + Qdotn * Qdotn;
+  const double QdB = Q1 * B1 + Q2 * B2 + Q3 * B3;
+  const double Bsq = vsq_tilde(G, B1, B2, B3);
+  const double QdB2 = QdB * QdB;
+  const double cg = (gam_ad - 1.0) / gam_ad;
+
+  const double g2 = 1.0 + vsq_tilde(G, Pg[2], Pg[3], Pg[4]);
+  double W = (Pg[0] + gam_ad * Pg[1]) * g2;
+  double v2 = 1.0 - 1.0 / g2;
+  v2 = fmin(fmax(v2, 0.0), 1.0 - 1e-15);
+
+  int extra = -1;
+  bool conv = false;
+  for (int it = 0; it < 30; it++) {
+    const double omv = 1.0 - v2;
+    const double sq = sqrt(omv);
+    const double p = cg * (W * omv - D * sq);
+    const double dpdW = cg * omv;
+    const double dpdv = cg * (-W + D / (2.0 * sq));
+    const double BW = Bsq + W;
+    const double iW = 1.0 / W;
+    const double iW2 = iW * iW, iW3 = iW2 * iW;
+    const double f1 = Qtsq - v2 * BW * BW + QdB2 * (Bsq + 2.0 * W) * iW2;
+    const double f2 = -Qdotn - 0.5 * Bsq * (1.0 + v2) + 0.5 * QdB2 * iW2 - W + p;
+    const double j11 = -2.0 * v2 * BW - 2.0 * QdB2 * BW * iW3;
+    const double j12 = -BW * BW;
+    const double j21 = -QdB2 * iW3 - 1.0 + dpdW;
+    const double j22 = -0.5 * Bsq + dpdv;
+    const double idet = 1.0 / (j11 * j22 - j12 * j21);
+    const double dW = -(j22 * f1 - j12 * f2) * idet;
+    const double dv = -(-j21 * f1 + j11 * f2) * idet;
+    if (!isfinite(dW) || !isfinite(dv)) return 2;
+    W = fabs(W + dW);
+    v2 = fmin(fmax(v2 + dv, 0.0), 1.0 - 1e-15);
+    if (extra >= 0) {
+      if (++extra >= 2) { conv = true; break; }
+    } else if (fabs(dW) <= 1e-12 * fabs(W) && fabs(dv) <= 1e-12) {
+      extra = 0;  // converged: take 2 more iterations so the result does not depend on the guess
+    }
+  }
+  if (!conv) return 1;
+  const double gamma = 1.0 / sqrt(1.0 - v2);
+  const double rho = D / gamma;
+  const double u = (W / (gamma * gamma) - rho) / gam_ad;
+  if (!isfinite(rho) || !isfinite(u) || !isfinite(W)) return 2;
+  Pout[0] = rho;
+  Pout[1] = u;
+  const double fac = gamma / (W + Bsq), qw = QdB / W;
+  Pout[2] = fac * (Qc1 + Qdotn * n1 + qw * B1);
+  Pout[3] = fac * (Qc2 + qw * B2);
+  Pout[4] = fac * (Qc3 + qw * B3);
+  return 0;
+}
+
+// floors and Lorentz-factor ceiling on primitives (C-13)
+__device__ __forceinline__ void floors_ceiling(const Geo& G, double rfl, double ufl, double gamma_max, double Pn[5],
+                                               int& nrf, int& nuf, int& ngc) {
+  if (Pn[0] < rfl) { Pn[0] = rfl; nrf = 1; }
+  if (Pn[1] < ufl) { Pn[1] = ufl; nuf = 1; }
+  const double gamma = sqrt(1.0 + vsq_tilde(G, Pn[2], Pn[3], Pn[4]));
+  if (gamma > gamma_max) {
+    const double fac = sqrt((gamma_max * gamma_max - 1.0) / (gamma * gamma - 1.0));
+    Pn[2] *= fac; Pn[3] *= fac; Pn[4] *= fac;
+    ngc = 1;
+  }
+}
+
 }  // namespace hamr

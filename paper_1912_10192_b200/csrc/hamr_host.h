@@ -20,8 +20,31 @@ enum Scal { S_T = 0, S_DT, S_CTOP0, S_CTOP1, S_CTOP2, S_DTLAST, S_DENMAX, S_DIVB
 // device counters
 enum Cnt { N_C2PFAIL = 0, N_RHOFL, N_UFL, N_GCEIL, N_NONFINITE, NCNT = 8 };
 
+// Block-structured grid: every per-variable array holds nblk
+// padded blocks back to back (block b at doubles [b*blen, (b+1)*blen)); a launch works on the blocks
+// listed in `list` (all blocks of one time level).  nblk == 0: monolithic grid.
+struct BlkDev {
+  int nblk;                  // blocks on the grid
+  int nact;                  // blocks in this launch
+  int blen;                  // doubles per block per array
+  int ge2;                   // row pitch of the (global, per x1-level) geometry tables
+  int n2g;                   // global N2 (pole faces: J == 0 or J == n2g)
+  int tlev, flev;            // offset in doubles of the level-1 geometry / floor tables
+  const int* list;           // [nact] block ids of this launch
+  const int4* info;          // [nblk] {table index of local zone (0,0), x1 level, I0, J0}
+  const int* nbr;            // [nblk][27] neighbour block by offset, -1 outside the domain
+  const int* phys;           // [nblk] bit d: low side of dim d is a physical boundary, bit 3+d: high side
+  const int* K0;             // [nblk] global x3 index of local zone 0
+  int* tau;                  // [nblk] LAT time level (C-17)
+  int* cur;                  // [nblk] which of the 3 buffers holds the block's time-n state (0 or 2)
+  double* ctopb;             // [nblk][3] max signal speed of the block's last corrector pass (C-14)
+  double* FA2[3][5];         // flux registers: dt_b F summed over the steps inside one coarser step (C-17)
+  double* EA2[3];            // EMF registers
+};
+
 struct Dev {                 // everything a kernel may need, passed by value
   Lay L;
+  BlkDev B;
   int metric, recon;
   int bc_lo[3], bc_hi[3];
   double dx[3], x0[3];       // internal-coordinate spacing and origin
@@ -42,6 +65,30 @@ struct Dev {                 // everything a kernel may need, passed by value
   unsigned long long* cnt;   // [NCNT]
 };
 
+// the three roles of a stage (C-12) in the buffer sets of blocks with cur == 0 (a) / cur == 2 (b)
+struct Roles { Fields src, base, out; };
+
+// per-thread view of the block a BLK kernel thread works on (monolithic: constants)
+struct BCtx { int b, zoff, q0, lev, cur, I0, J0; };
+template <bool BLK>
+__device__ __forceinline__ BCtx blk_ctx(const Dev& Dv, int slot) {
+  BCtx c;
+  if (BLK) {
+    c.b = __ldg(Dv.B.list + slot);
+    const int4 inf = __ldg(Dv.B.info + c.b);
+    c.zoff = c.b * Dv.B.blen; c.q0 = inf.x; c.lev = inf.y; c.I0 = inf.z; c.J0 = inf.w;
+    c.cur = Dv.B.cur[c.b];
+  } else {
+    c.b = 0; c.zoff = 0; c.q0 = NG * Dv.L.e2 + NG; c.lev = 0; c.cur = 0; c.I0 = 0; c.J0 = 0;
+  }
+  return c;
+}
+// buffer selection: a block's time-n state lives in buffer set a (cur == 0) or b (cur == 2)
+template <bool BLK>
+__device__ __forceinline__ const double* selp(const double* a, const double* b, int cur) { return (BLK && cur) ? b : a; }
+template <bool BLK>
+__device__ __forceinline__ double* selp(double* a, double* b, int cur) { return (BLK && cur) ? b : a; }
+
 }  // namespace hamr
 
 namespace hamr {
@@ -49,8 +96,32 @@ namespace hamr {
 enum KClass { K_GHOSTS = 0, K_FLUX1, K_FLUX2, K_FLUX3, K_CEMF, K_EDGE, K_UPDATE_P, K_UPDATE_C, K_DT, K_OTHER, NKCLASS };
 }
 
+namespace hamr {
+// host side of the block-structured grid (blocks.cu)
+struct BlkHost {
+  bool on;                   // block-structured grid (more than one block, or LAT)
+  int nblk, tmax;            // blocks; highest LAT level (0: one global dt)
+  int nslot[3];              // block lattice extents
+  std::vector<int> nbr;      // [nblk][27] host mirror of the neighbour table
+  std::vector<int> lev1;     // [nblk] x1 refinement level
+  std::vector<int> tau;      // [nblk] current time level
+  std::vector<int> I0;       // [nblk][3]
+  std::vector<int> forced;   // test hook: prescribed time levels (empty: Courant-based)
+  int* d_lists;              // device [5][nblk]: blocks of level 0..3, then every block
+  int* d_clists;             // device [4][nblk]: blocks of level tau with a neighbour on tau - 1
+  int nlist[4], nclist[4];
+  long long tb_u[4];         // LAT clocks per level, units of (finest dt)/2 (C-17)
+  int dt_u[4];
+  int has_new[4];
+  double* h_ctop;            // pinned [nblk][3]
+  int* h_ints;               // pinned [6][nblk]
+  double dt0;                // host copy of the finest step (LAT)
+};
+}
+
 struct hamr_grid {
   hamr_params par;
+  hamr::BlkHost bh;
   hamr::Dev D;
   hamr::Fields s[3];         // rotating: sn (time n), sh (n+1/2), snew
   int isn, ish, inew;
@@ -115,5 +186,23 @@ void launch_divb(hamr_grid* g, const Fields& s);
 void launch_totals(hamr_grid* g, const Fields& s);
 void launch_check_finite(hamr_grid* g, const Fields& s);
 void launch_zero_ctop(hamr_grid* g);
+void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop);
+void launch_ct_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2);
+void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles& rb, double dtfac, bool same);
+void launch_geometry_tab(hamr_grid* g, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
+                         double* gf2, double* dgc, double* rho_fl, double* u_fl);
+
+// blocks.cu: block-structured grid (H7)
+int blk_count(const hamr_params& p, int nslot[3], int bn[3]);       // number of blocks (0 if invalid)
+size_t blk_table_bytes(int nblk);                                   // device bytes of the block tables
+int blk_setup(hamr_grid* g, void* tables);                          // lattice, neighbour tables, lists
+void blk_pack(hamr_grid* g, const double* dense, int kind, int stag, bool zero_pole);  // kind: 0..4 P, 5..7 Bf
+void blk_unpack(hamr_grid* g, int kind, double* dense);             // kind: 0..4 P, 5..7 Bc, 8..10 Bf
+int blk_initial(hamr_grid* g);                                      // ghosts, first flux pass, dt / levels
+int blk_step(hamr_grid* g, int nsteps);                             // nsteps coarse steps
+int blk_set_levels(hamr_grid* g, const int* tau);
+void blk_divb(hamr_grid* g);
+void blk_totals(hamr_grid* g);
+void blk_check_finite(hamr_grid* g);
 
 }  // namespace hamr

@@ -29,6 +29,7 @@ SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "h
            "hamr_set_prims", "hamr_set_prims_dev", "hamr_step", "hamr_step_async", "hamr_sync",
            "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
            "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
+           "hamr_set_levels",
            "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
            "hamr_profile_begin", "hamr_profile_end", "hamr_profile_class_name", "hamr_launch_count"]
 NKCLASS = 10
@@ -82,6 +83,7 @@ def lib():
         L.hamr_last_error.restype = C.c_char_p
         L.hamr_num_blocks.argtypes = [vp]
         L.hamr_block_info.argtypes = [vp, C.c_int, c_double_p, c_double_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.hamr_set_levels.argtypes = [vp, C.POINTER(C.c_int)]
         L.hamr_debug_emf.argtypes = [vp]
         L.hamr_get_face.argtypes = [vp, C.c_int, C.c_int, c_double_p]
         L.hamr_get_edge.argtypes = [vp, C.c_int, c_double_p]
@@ -254,6 +256,16 @@ class Grid:
 
     def num_blocks(self):
         return self.L.hamr_num_blocks(self.h)
+
+    def set_levels(self, tau):
+        if tau is None:
+            self._ck(self.L.hamr_set_levels(self.h, None))
+        else:
+            assert len(tau) == self.num_blocks()
+            self._ck(self.L.hamr_set_levels(self.h, (C.c_int * len(tau))(*[int(v) for v in tau])))
+
+    def levels(self):
+        return [self.block_info(b)[3] for b in range(self.num_blocks())]
 
     def block_info(self, b):
         lo, dx = np.zeros(3), np.zeros(3)
