@@ -42,38 +42,26 @@ __device__ __forceinline__ T pick4(const T v[4], int i) {
   return i == 0 ? v[0] : (i == 1 ? v[1] : (i == 2 ? v[2] : v[3]));
 }
 
-// C-17: value at time s_u of array `kind` of block q at local offset zl, from q's three time levels:
-// a completed state at s_u is copied; completed states bracketing s_u are interpolated linearly in
-// time; otherwise the time-n state and the predictor state at tb + dt/2 are
-__device__ __forceinline__ double blk_sample(const Dev& Dv, const Bufs& B, const LevT& lt, int kind, int q,
-                                             int zl, long long s_u) {
-  const int tq = Dv.B.tau[q], cq = Dv.B.cur[q];
-  const long long tb = pick4(lt.tb, tq);
-  const int dtu = pick4(lt.dtu, tq);
-  const long long z = (long long)q * Dv.B.blen + zl;
-  const double an = buf_arr(B, cq, kind)[z];
-  if (s_u == tb) return an;
-  if (pick4(lt.hasnew, tq)) {
-    const double w = (double)(s_u - tb) / (double)dtu;
-    return (1.0 - w) * an + w * buf_arr(B, 2 - cq, kind)[z];
-  }
-  const double w = (double)(s_u - tb) / (double)(dtu / 2);
-  return (1.0 - w) * an + w * buf_arr(B, 1, kind)[z];
-}
-
-// Value that the ghost fill of C-16 / C-12 leaves at padded index id[] of array `kind` of block b:
+// Where the ghost fill of C-16 / C-12 takes the value at padded index id[] of an array of block b from:
 // the per-dimension physical-boundary maps (outflow copy, polar mirror; fill order x1, x2, x3) are
-// composed with the neighbour lookup, so that every ghost value is ONE signed sample of an active
-// value.  own_buf: the buffer holding b's stage source.  mod: the value differs from what b's own
-// active storage holds (a ghost, a reflecting wall face, or a boundary face owned by a finer block).
-__device__ __forceinline__ double blk_gval(const Dev& Dv, const Bufs& B, const LevT& lt, int b, int own_buf,
-                                           int kind, const int id[3], long long s_u, bool& mod) {
+// composed with the neighbour lookup, so that every ghost value is ONE signed sample of an active value.
+struct GSrc {
+  int q;        // block holding the value
+  int zl;       // offset of the value inside that block
+  int negmask;  // bit d: a mirror along d was applied (the component along d changes sign)
+  bool ghost;   // sampled from a neighbour (else read from b's own active storage)
+  bool zero;    // a reflecting wall face: the value is 0
+  bool mod;     // differs from what b's own storage holds at id[]
+};
+
+// sd: the array is staggered along sd (-1: zone-centred)
+// norule: every neighbour is on b's own time level, so no face is owned by a finer block
+__device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, const int id[3], bool norule) {
   const Lay& L = Dv.L;
-  const int sd = kind >= 5 ? kind - 5 : -1;                    // staggered along sd
-  const int vc = kind >= 5 ? kind - 5 : (kind >= 2 ? kind - 2 : -1);  // component flipped by a mirror along vc
-  const int phys = __ldg(Dv.B.phys + b);
   int m[3], o[3];
-  bool neg = false, zero = false;
+  GSrc s;
+  s.negmask = 0;
+  s.zero = false;
 #pragma unroll
   for (int d = 0; d < 3; d++) {
     const int n = L.n[d], hi = (sd == d) ? n : n - 1, g = id[d];
@@ -81,105 +69,223 @@ __device__ __forceinline__ double blk_gval(const Dev& Dv, const Bufs& B, const L
     if (g < 0) {
       if (phys & (1 << d)) {
         if (Dv.bc_lo[d] == HAMR_BC_OUTFLOW) m[d] = 0;
-        else { m[d] = (sd == d) ? -g : -g - 1; if (vc == d) neg = !neg; }
+        else { m[d] = (sd == d) ? -g : -g - 1; s.negmask |= 1 << d; }
       } else o[d] = -1;
     } else if (g > hi) {
       if (phys & (8 << d)) {
         if (Dv.bc_hi[d] == HAMR_BC_OUTFLOW) m[d] = hi;
-        else { m[d] = n - (g - hi); if (vc == d) neg = !neg; }
+        else { m[d] = n - (g - hi); s.negmask |= 1 << d; }
       } else o[d] = 1;
     }
     // a reflecting wall carries no normal flux: the wall face itself is 0
     if (sd == d && ((m[d] == 0 && (phys & (1 << d)) && Dv.bc_lo[d] == HAMR_BC_POLAR_REFLECT) ||
                     (m[d] == n && (phys & (8 << d)) && Dv.bc_hi[d] == HAMR_BC_POLAR_REFLECT)))
-      zero = true;
+      s.zero = true;
   }
   const int* nb = Dv.B.nbr + b * 27;
-  int q = (o[0] == 0 && o[1] == 0 && o[2] == 0) ? b : __ldg(nb + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
+  s.ghost = (o[0] | o[1] | o[2]) != 0;
+  s.q = s.ghost ? __ldg(nb + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1)) : b;
   int lq[3] = {m[0] - o[0] * L.n[0], m[1] - o[1] * L.n[1], m[2] - o[2] * L.n[2]};
-  bool ghost = (o[0] | o[1] | o[2]) != 0;
   // C-17: a face on the plane between two blocks on different time levels has ONE value in every stage
   // source, that of the finer block
-  if (sd >= 0 && (m[sd] == 0 || m[sd] == L.n[sd])) {
+  if (!norule && sd >= 0 && (m[sd] == 0 || m[sd] == L.n[sd])) {
     int o2[3] = {o[0], o[1], o[2]};
     o2[sd] = m[sd] == 0 ? -1 : 1;
     const int q2 = __ldg(nb + (o2[0] + 1) * 9 + (o2[1] + 1) * 3 + (o2[2] + 1));
-    if (q2 >= 0 && q >= 0 && Dv.B.tau[q2] < Dv.B.tau[q]) {
-      q = q2;
+    if (q2 >= 0 && s.q >= 0 && Dv.B.tau[q2] < Dv.B.tau[s.q]) {
+      s.q = q2;
       lq[sd] = m[sd] == 0 ? L.n[sd] : 0;
-      ghost = true;
+      s.ghost = true;
     }
   }
-  mod = ghost || zero || neg || m[0] != id[0] || m[1] != id[1] || m[2] != id[2];
-  if (zero) return 0.0;
+  s.mod = s.ghost || s.zero || (sd >= 0 && ((s.negmask >> sd) & 1)) || m[0] != id[0] || m[1] != id[1] || m[2] != id[2];
+  s.zl = (int)L.idx(lq[0], lq[1], lq[2]);
+  return s;
+}
+
+// C-17 time sampling of block q at time s_u: which buffers and with what weight
+struct QTime { int b0, b1; double w; };  // value = (1 - w) a[b0] + w a[b1]; b1 < 0: a plain copy of a[b0]
+__device__ __forceinline__ QTime blk_qtime(const Dev& Dv, const LevT& lt, int q, long long s_u) {
+  const int tq = Dv.B.tau[q], cq = Dv.B.cur[q];
+  const long long tb = pick4(lt.tb, tq);
+  const int dtu = pick4(lt.dtu, tq);
+  QTime t;
+  t.b0 = cq; t.b1 = -1; t.w = 0.0;
+  if (s_u == tb) return t;                                  // a completed state: copy
+  if (pick4(lt.hasnew, tq)) {                               // completed states bracket s_u
+    t.b1 = 2 - cq;
+    t.w = (double)(s_u - tb) / (double)dtu;
+  } else {                                                  // the time-n state and the predictor state
+    t.b1 = 1;
+    t.w = (double)(s_u - tb) / (double)(dtu / 2);
+  }
+  return t;
+}
+
+__device__ __forceinline__ double blk_fetch(const Dev& Dv, const Bufs& B, int b, int own_buf, int kind,
+                                            const GSrc& s, const QTime& qt) {
+  if (s.zero) return 0.0;
+  const int vc = kind >= 5 ? kind - 5 : (kind >= 2 ? kind - 2 : -1);
   double v;
-  const int zl = (int)L.idx(lq[0], lq[1], lq[2]);
-  if (!ghost) v = buf_arr(B, own_buf, kind)[(long long)b * Dv.B.blen + zl];
-  else v = blk_sample(Dv, B, lt, kind, q, zl, s_u);
-  return neg ? -v : v;
+  if (!s.ghost) {
+    v = buf_arr(B, own_buf, kind)[(long long)b * Dv.B.blen + s.zl];
+  } else {
+    const long long z = (long long)s.q * Dv.B.blen + s.zl;
+    v = buf_arr(B, qt.b0, kind)[z];
+    if (qt.b1 >= 0) v = (1.0 - qt.w) * v + qt.w * buf_arr(B, qt.b1, kind)[z];
+  }
+  return (vc >= 0 && ((s.negmask >> vc) & 1)) ? -v : v;
 }
 
 // Ghost fill of the stage source of every listed block: neighbour exchange with time interpolation
 // (C-16, C-17), physical boundaries (C-12), cell-centred B wherever a face changed (C-10).
 // role: 0 the source is the block's time-n state, 1 its predictor state.  all: also derive B_c on the
 // active zones (initial state).  zero_ctop: reset the block's Courant maxima (before a corrector pass).
-__global__ void __launch_bounds__(256) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, int role, long long s_u_base,
-                                                    int all, int zero_ctop) {
+// Block flags (host, per level assignment): bit 0 "simple": no physical side and all 26 neighbours on
+// the block's own time level -> every ghost value (B_c included) is a plain copy of the neighbour's
+// stage source; bit 1: some neighbour is on a finer time level (only then can an ACTIVE face change).
+__global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, int role, long long s_u, int all,
+                                                    int zero_ctop) {
+  // grid: x covers the padded locations of one block, y the blocks of the launch; 32-bit index arithmetic
   const Lay& L = Dv.L;
   const int e3 = L.n[2] + 2 * NG + 1;
-  const long long per = (long long)L.e1 * L.e2 * e3;
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= per * Dv.B.nact) return;
-  const int bslot = (int)(t / per);
-  t -= bslot * per;
-  const int b = __ldg(Dv.B.list + bslot);
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (unsigned)(L.e1 * L.e2 * e3)) return;
+  const int b = __ldg(Dv.B.list + blockIdx.y);
   if (zero_ctop && t == 0) Dv.B.ctopb[b * 3] = Dv.B.ctopb[b * 3 + 1] = Dv.B.ctopb[b * 3 + 2] = 0.0;
-  const int id[3] = {(int)(t / ((long long)e3 * L.e2)) - NG, (int)((t / e3) % L.e2) - NG, (int)(t % e3) - NG};
-  // zones two or more layers inside the block have nothing to do
-  bool deep = true;
-  for (int d = 0; d < 3; d++) deep = deep && id[d] >= 1 && id[d] <= L.n[d] - 2;
-  if (deep && !all) return;
-  const int cur = Dv.B.cur[b];
-  const int own = role == 0 ? cur : 1;
-  // s_u: the listed blocks share one time level, hence one clock
-  const long long s_u = s_u_base;
+  const unsigned tj = t / (unsigned)e3, ti = tj / (unsigned)L.e2;
+  const int id[3] = {(int)ti - NG, (int)(tj - ti * L.e2) - NG, (int)(t - tj * e3) - NG};
   bool in_c[3], extra[3];
+#pragma unroll
   for (int d = 0; d < 3; d++) { in_c[d] = id[d] >= 0 && id[d] < L.n[d]; extra[d] = id[d] == L.n[d] + NG; }
   const bool zone_active = in_c[0] && in_c[1] && in_c[2];
   const bool zone_slot = !(extra[0] || extra[1] || extra[2]);
-  const long long z = (long long)b * Dv.B.blen + L.idx(id[0], id[1], id[2]);
-  const Fields& dst = B.s[0];  // pointer selection below
-  (void)dst;
-  if (zone_slot && !zone_active) {
+  // Which ghosts anything reads: a sweep along d reads zones up to NG deep along d but only one layer out
+  // in the other two dimensions (the transverse ghost layer whose face EMFs feed C-9), and the centre EMFs
+  // are needed one layer out.  Ghost zones more than one layer out in two or more dimensions are never
+  // read and are left alone; ghost FACE storage is only read as the normal field of faces 0..n along d
+  // in that one transverse layer (a ghost zone's B_c is built here from the fetched face values).
+  int ndeep = 0;
+  bool shell1[3];
 #pragma unroll
-    for (int c = 0; c < 5; c++) {
-      bool mod;
-      const double v = blk_gval(Dv, B, lt, b, own, c, id, s_u, mod);
-      const_cast<double*>(buf_arr(B, own, c))[z] = v;
+  for (int d = 0; d < 3; d++) {
+    ndeep += (id[d] < -1 || id[d] > L.n[d]) ? 1 : 0;
+    shell1[d] = id[d] >= -1 && id[d] <= L.n[d];
+  }
+  if (ndeep >= 2) return;
+  const int flags = Dv.B.flags[b];
+  if (zone_active && !all && !(flags & 2)) return;   // no finer neighbour: active storage is final
+  const int cur = Dv.B.cur[b];
+  const int own = role == 0 ? cur : 1;
+  const long long z = (long long)b * Dv.B.blen + L.idx(id[0], id[1], id[2]);
+  const int* nb = Dv.B.nbr + b * 27;
+
+  if ((flags & 1) && !all) {
+    // ---- fast path: plain copies from same-level neighbours ------------------------------------------
+    int oc[3], lc[3];
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+      oc[d] = id[d] < 0 ? -1 : (id[d] >= L.n[d] ? 1 : 0);
+      lc[d] = id[d] - oc[d] * L.n[d];
     }
+    // all loads are issued before the first store (the stores may alias the loads as far as the compiler
+    // knows; interleaving them would serialise eleven DRAM round trips)
+    const Fields& fo = own == 0 ? B.s[0] : (own == 1 ? B.s[1] : B.s[2]);
+    double vP[5], vB[3], vF[3];
+    bool wF[3];
+    if (zone_slot) {
+      const int q = __ldg(nb + (oc[0] + 1) * 9 + (oc[1] + 1) * 3 + (oc[2] + 1));
+      const int bq = role == 0 ? Dv.B.cur[q] : 1;
+      const long long zq = (long long)q * Dv.B.blen + L.idx(lc[0], lc[1], lc[2]);
+      const Fields& fq = bq == 0 ? B.s[0] : (bq == 1 ? B.s[1] : B.s[2]);
+#pragma unroll
+      for (int c = 0; c < 5; c++) vP[c] = fq.P[c][zq];
+#pragma unroll
+      for (int c = 0; c < 3; c++) vB[c] = fq.Bc[c][zq];
+    }
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+      const int o1 = (d + 1) % 3, o2 = (d + 2) % 3;
+      int of[3] = {oc[0], oc[1], oc[2]}, lf[3] = {lc[0], lc[1], lc[2]};
+      if (id[d] == L.n[d]) { of[d] = 0; lf[d] = id[d]; }    // the block's own high face
+      wF[d] = shell1[o1] && shell1[o2] && id[d] >= 0 && id[d] <= L.n[d] && (of[0] | of[1] | of[2]) != 0;
+      vF[d] = 0.0;
+      if (wF[d]) {
+        const int q = __ldg(nb + (of[0] + 1) * 9 + (of[1] + 1) * 3 + (of[2] + 1));
+        const int bq = role == 0 ? Dv.B.cur[q] : 1;
+        vF[d] = buf_arr(B, bq, 5 + d)[(long long)q * Dv.B.blen + L.idx(lf[0], lf[1], lf[2])];
+      }
+    }
+    if (zone_slot) {
+#pragma unroll
+      for (int c = 0; c < 5; c++) fo.P[c][z] = vP[c];
+#pragma unroll
+      for (int c = 0; c < 3; c++) fo.Bc[c][z] = vB[c];
+    }
+#pragma unroll
+    for (int d = 0; d < 3; d++)
+      if (wF[d]) fo.Bf[d][z] = vF[d];
+    return;
+  }
+
+  // ---- general path --------------------------------------------------------------------------------
+  // zones two or more layers inside the block have nothing to do
+  bool deep = true;
+#pragma unroll
+  for (int d = 0; d < 3; d++) deep = deep && id[d] >= 1 && id[d] <= L.n[d] - 2;
+  if (deep && !all) return;
+  const int phys = __ldg(Dv.B.phys + b);
+  // bit 2: all neighbours on the block's own level: no finer-block faces, and every sample is a plain copy
+  // of the neighbour's stage source (its time-n state for a predictor, its predictor state for a corrector)
+  const bool same = (flags & 4) != 0;
+  int lastq = -1;
+  QTime qt;
+  qt.b0 = 0; qt.b1 = -1; qt.w = 0.0;
+  auto qtime = [&](int q) {
+    QTime r;
+    if (same) { r.b0 = role == 0 ? Dv.B.cur[q] : 1; r.b1 = -1; r.w = 0.0; return r; }
+    return blk_qtime(Dv, lt, q, s_u);
+  };
+  // loads first, stores last (see the fast path)
+  double vP[5];
+  const bool wP = zone_slot && !zone_active;
+  if (wP) {
+    const GSrc s = blk_src(Dv, b, phys, -1, id, same);
+    if (s.ghost) { qt = qtime(s.q); lastq = s.q; }
+#pragma unroll
+    for (int c = 0; c < 5; c++) vP[c] = blk_fetch(Dv, B, b, own, c, s, qt);
   }
   double lo[3], hi[3];
+  bool wF[3] = {false, false, false};
   bool anymod = false;
 #pragma unroll
   for (int d = 0; d < 3; d++) {
     const int o1 = (d + 1) % 3, o2 = (d + 2) % 3;
     if (extra[o1] || extra[o2]) { lo[d] = hi[d] = 0.0; continue; }
-    bool mod;
-    lo[d] = blk_gval(Dv, B, lt, b, own, 5 + d, id, s_u, mod);
-    if (mod) { const_cast<double*>(buf_arr(B, own, 5 + d))[z] = lo[d]; anymod = true; }
+    GSrc s = blk_src(Dv, b, phys, d, id, same);
+    if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
+    lo[d] = blk_fetch(Dv, B, b, own, 5 + d, s, qt);
+    if (s.mod) { wF[d] = shell1[o1] && shell1[o2] && id[d] >= 0 && id[d] <= L.n[d]; anymod = true; }
     hi[d] = 0.0;
     if (!extra[d]) {
       int idp[3] = {id[0], id[1], id[2]};
       idp[d] += 1;
-      hi[d] = blk_gval(Dv, B, lt, b, own, 5 + d, idp, s_u, mod);
-      anymod = anymod || mod;
+      s = blk_src(Dv, b, phys, d, idp, same);
+      if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
+      hi[d] = blk_fetch(Dv, B, b, own, 5 + d, s, qt);
+      anymod = anymod || s.mod;
     }
   }
+  if (wP) {
+#pragma unroll
+    for (int c = 0; c < 5; c++) const_cast<double*>(buf_arr(B, own, c))[z] = vP[c];
+  }
+#pragma unroll
+  for (int d = 0; d < 3; d++)
+    if (wF[d]) const_cast<double*>(buf_arr(B, own, 5 + d))[z] = lo[d];
   if (zone_slot && (!zone_active || all || anymod)) {
     const int4 inf = __ldg(Dv.B.info + b);
     const double g = __ldg(Dv.gc + inf.y * Dv.B.tlev + GDET * L.n2d + inf.x + id[0] * Dv.B.ge2 + id[1]);
-    const Fields& f = B.s[0];
-    (void)f;
 #pragma unroll
     for (int d = 0; d < 3; d++) {
       double* bc = own == 0 ? B.s[0].Bc[d] : (own == 1 ? B.s[1].Bc[d] : B.s[2].Bc[d]);
@@ -193,13 +299,14 @@ __global__ void __launch_bounds__(256) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, int
 __global__ void __launch_bounds__(128) k_blk_registers(Dev Dv, int first, double dtfac) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
-  const long long per = (long long)(L.n[0] + 1) * c1 * c2;
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned per = (unsigned)(L.n[0] + 1) * c1 * c2;
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= per * Dv.B.nact) return;
   const int bslot = (int)(t / per);
   t -= bslot * per;
   const int b = __ldg(Dv.B.list + bslot);
-  const int id[3] = {(int)(t / ((long long)c2 * c1)), (int)((t / c2) % c1), (int)(t % c2)};
+  const unsigned tj = t / (unsigned)c2, ti = tj / (unsigned)c1;
+  const int id[3] = {(int)ti, (int)(tj - ti * c1), (int)(t - tj * c2)};
   bool onb[3];
   for (int d = 0; d < 3; d++) onb[d] = id[d] == 0 || id[d] == L.n[d];
   if (!(onb[0] || onb[1] || onb[2])) return;
@@ -296,13 +403,14 @@ __device__ __forceinline__ bool blk_face_corr(const Dev& Dv, const Bufs& B, int 
 __global__ void __launch_bounds__(128) k_blk_correct_faces(Dev Dv, Bufs B, int tc, double dtfac) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
-  const long long per = (long long)(L.n[0] + 1) * c1 * c2;
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned per = (unsigned)(L.n[0] + 1) * c1 * c2;
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= per * Dv.B.nact) return;
   const int bslot = (int)(t / per);
   t -= bslot * per;
   const int c = __ldg(Dv.B.list + bslot);
-  const int id[3] = {(int)(t / ((long long)c2 * c1)), (int)((t / c2) % c1), (int)(t % c2)};
+  const unsigned tj = t / (unsigned)c2, ti = tj / (unsigned)c1;
+  const int id[3] = {(int)ti, (int)(tj - ti * c1), (int)(t - tj * c2)};
   // only faces within one zone of the block boundary can be touched
   bool near = false;
   for (int d = 0; d < 3; d++) near = near || id[d] <= 1 || id[d] >= L.n[d] - 1;
@@ -324,14 +432,15 @@ __global__ void __launch_bounds__(128) k_blk_correct_faces(Dev Dv, Bufs B, int t
 // re-inversion of every touched zone
 __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int tc, double dtfac) {
   const Lay& L = Dv.L;
-  const long long per = (long long)L.n[0] * L.n[1] * L.n[2];
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned per = (unsigned)L.n[0] * L.n[1] * L.n[2];
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0;
   if (t < per * Dv.B.nact) {
     const int bslot = (int)(t / per);
     t -= bslot * per;
     const int c = __ldg(Dv.B.list + bslot);
-    const int id[3] = {(int)(t / ((long long)L.n[2] * L.n[1])), (int)((t / L.n[2]) % L.n[1]), (int)(t % L.n[2])};
+    const unsigned tj = t / (unsigned)L.n[2], ti = tj / (unsigned)L.n[1];
+    const int id[3] = {(int)ti, (int)(tj - ti * L.n[1]), (int)(t - tj * L.n[2])};
     bool near = false;
     for (int d = 0; d < 3; d++) near = near || id[d] == 0 || id[d] == L.n[d] - 1;
     if (near) {
@@ -585,6 +694,23 @@ static Dev dev_list(const hamr_grid* g, int which) {
   return D;
 }
 
+// per-block ghost-fill flags from the current time levels (see k_blk_ghosts) into pinned memory, then upload
+static cudaError_t blk_upload_flags(hamr_grid* g) {
+  BlkHost& H = g->bh;
+  int* hf = H.h_ints + (size_t)9 * H.nblk;
+  for (int b = 0; b < H.nblk; b++) {
+    bool same = true, finer = false;
+    for (int a = 0; a < 27; a++) {
+      const int q = H.nbr[(size_t)b * 27 + a];
+      if (q < 0) continue;
+      if (H.tau[q] != H.tau[b]) same = false;
+      if (H.tau[q] < H.tau[b]) finer = true;
+    }
+    hf[b] = ((same && H.phys[b] == 0) ? 1 : 0) | (finer ? 2 : 0) | (same ? 4 : 0);
+  }
+  return cudaMemcpyAsync(g->D.B.flags, hf, (size_t)H.nblk * 4, cudaMemcpyHostToDevice, g->stream);
+}
+
 int blk_count(const hamr_params& p, int nslot[3], int bn[3]) {
   long long nb = 1;
   for (int d = 0; d < 3; d++) {
@@ -597,8 +723,8 @@ int blk_count(const hamr_params& p, int nslot[3], int bn[3]) {
 }
 
 size_t blk_table_bytes(int nblk) {
-  // info (int4), nbr (27), phys, K0, tau, cur, 5 lists, 4 correction lists, ctopb (3 doubles)
-  return ((size_t)nblk * (16 + 4 * (27 + 4 + 5 + 4) + 24) + 1024 + 255) / 256 * 256;
+  // info (int4), nbr (27), phys, K0, tau, cur, flags, 5 lists, 4 correction lists, ctopb (3 doubles)
+  return ((size_t)nblk * (16 + 4 * (27 + 5 + 5 + 4) + 24) + 1024 + 255) / 256 * 256;
 }
 
 // C-16: block lattice, neighbour table (periodic dimensions close through it), per-block table offsets
@@ -616,6 +742,7 @@ int blk_setup(hamr_grid* g, void* tables) {
   H.tau.assign(nblk, 0);
   H.I0.assign((size_t)nblk * 3, 0);
   H.forced.clear();
+  H.phys.clear();
   BlkDev& B = g->D.B;
   const int ge2 = p.n[1] + 2 * NG + 1;
   std::vector<int> info((size_t)nblk * 4), phys(nblk), K0(nblk);
@@ -638,6 +765,7 @@ int blk_setup(hamr_grid* g, void* tables) {
           if (sl[d] == H.nslot[d] - 1 && p.bc_hi[d] != HAMR_BC_PERIODIC) ph |= 8 << d;
         }
         phys[b] = ph;
+        H.phys.push_back(ph);
         for (int o0 = -1; o0 <= 1; o0++)
           for (int o1 = -1; o1 <= 1; o1++)
             for (int o2 = -1; o2 <= 1; o2++) {
@@ -664,6 +792,7 @@ int blk_setup(hamr_grid* g, void* tables) {
   B.cur = (int*)take((size_t)nblk * 4);
   H.d_lists = (int*)take((size_t)nblk * 5 * 4);
   H.d_clists = (int*)take((size_t)nblk * 4 * 4);
+  B.flags = (int*)take((size_t)nblk * 4);
   B.ctopb = (double*)take((size_t)nblk * 24);
   B.info = d_info; B.nbr = d_nbr; B.phys = d_phys; B.K0 = d_K0;
   B.list = H.d_lists; B.nact = 0;
@@ -682,6 +811,9 @@ int blk_setup(hamr_grid* g, void* tables) {
   up(d_K0, K0.data(), (size_t)nblk * 4);
   up(H.d_lists, all.data(), (size_t)nblk * 4);                       // level 0 list (every block at tau = 0)
   up(H.d_lists + (size_t)4 * nblk, all.data(), (size_t)nblk * 4);    // the list of every block
+  if (e == cudaSuccess) e = cudaMemsetAsync(B.tau, 0, (size_t)nblk * 4, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(B.cur, 0, (size_t)nblk * 4, st);
+  if (e == cudaSuccess) e = blk_upload_flags(g);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);               // the host vectors go out of scope
   for (int i = 0; i < 4; i++) { H.nlist[i] = 0; H.nclist[i] = 0; H.tb_u[i] = 0; H.dt_u[i] = 2 << i; H.has_new[i] = 0; }
   H.nlist[0] = nblk;
@@ -721,10 +853,15 @@ void blk_unpack(hamr_grid* g, int kind, double* dense) {
 static void blk_ghosts(hamr_grid* g, const Dev& D, int role, long long s_u, bool all, bool zero_ctop) {
   if (D.B.nact == 0) return;
   const Lay& L = D.L;
-  const long long tot = (long long)L.e1 * L.e2 * (L.n[2] + 2 * NG + 1) * D.B.nact;
+  const int per = L.e1 * L.e2 * (L.n[2] + 2 * NG + 1);
   Launch l_(g, K_GHOSTS);
-  k_blk_ghosts<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(D, bufs_of(g), clocks_of(g), role, s_u,
-                                                                     all ? 1 : 0, zero_ctop ? 1 : 0);
+  for (int first = 0; first < D.B.nact; first += 65535) {   // grid.y limit
+    Dev Dc = D;
+    Dc.B.list = D.B.list + first;
+    Dc.B.nact = std::min(65535, D.B.nact - first);
+    k_blk_ghosts<<<dim3((per + 255) / 256, Dc.B.nact), 256, 0, g->stream>>>(Dc, bufs_of(g), clocks_of(g), role, s_u,
+                                                                         all ? 1 : 0, zero_ctop ? 1 : 0);
+  }
 }
 
 // one stage of C-12 on every block of time level tau (C-17)
@@ -875,6 +1012,7 @@ static int blk_assign(hamr_grid* g, bool after_step) {
   cudaError_t e = cudaMemcpyAsync(H.d_lists, hl, (size_t)4 * nblk * 4, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(H.d_clists, hl + (size_t)4 * nblk, (size_t)4 * nblk * 4, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(g->D.B.tau, hl + (size_t)8 * nblk, (size_t)nblk * 4, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = blk_upload_flags(g);
   H.dt0 = dt0;
   g->h_pinned[56] = dt0;
   if (e == cudaSuccess) e = cudaMemcpyAsync(g->D.scal + S_DT, g->h_pinned + 56, sizeof(double), cudaMemcpyHostToDevice, st);
@@ -898,6 +1036,8 @@ int blk_initial(hamr_grid* g) {
   for (int i = 0; i < 4; i++) { H.nlist[i] = 0; H.nclist[i] = 0; H.tb_u[i] = 0; H.dt_u[i] = 2 << i; H.has_new[i] = 0; }
   H.nlist[0] = H.nblk;
   if (cudaMemsetAsync(g->D.B.tau, 0, (size_t)H.nblk * 4, st) != cudaSuccess) return HAMR_ECUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return HAMR_ECUDA;   // the pinned staging area is reused
+  if (blk_upload_flags(g) != cudaSuccess) return HAMR_ECUDA;
   // level-0 list = every block
   if (cudaMemcpyAsync(H.d_lists, H.d_lists + (size_t)4 * H.nblk, (size_t)H.nblk * 4, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
     return HAMR_ECUDA;

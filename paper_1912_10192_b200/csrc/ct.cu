@@ -12,15 +12,16 @@ template <bool BLK>
 __global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s0, Fields s2) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + 2, c1 = L.n[1] + 2;
-  const long long per = (long long)(L.n[0] + 2) * c1 * c2;
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned per = (unsigned)(L.n[0] + 2) * c1 * c2;
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= (BLK ? per * Dv.B.nact : per)) return;
   int bslot = 0;
   if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
   const BCtx C = blk_ctx<BLK>(Dv, bslot);
-  const int k = (int)(t % c2) - 1;
-  const int j = (int)((t / c2) % c1) - 1;
-  const int i = (int)(t / ((long long)c2 * c1)) - 1;
+  const unsigned tj = t / (unsigned)c2, ti = tj / (unsigned)c1;
+  const int k = (int)(t - tj * c2) - 1;
+  const int j = (int)(tj - ti * c1) - 1;
+  const int i = (int)ti - 1;
   const long long z = C.zoff + L.idx(i, j, k);
   const int q = C.q0 + i * (BLK ? Dv.B.ge2 : L.e2) + j;
   const double* gc = Dv.gc + (BLK ? C.lev * Dv.B.tlev : 0);
@@ -63,15 +64,16 @@ template <bool BLK>
 __global__ void __launch_bounds__(128) k_edge_emf(Dev Dv) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
-  const long long per = (long long)(L.n[0] + 1) * c1 * c2;
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned per = (unsigned)(L.n[0] + 1) * c1 * c2;
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= (BLK ? per * Dv.B.nact : per)) return;
   int bslot = 0;
   if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
   const BCtx C = blk_ctx<BLK>(Dv, bslot);
-  const int k = (int)(t % c2);
-  const int j = (int)((t / c2) % c1);
-  const int i = (int)(t / ((long long)c2 * c1));
+  const unsigned tj = t / (unsigned)c2, ti = tj / (unsigned)c1;
+  const int k = (int)(t - tj * c2);
+  const int j = (int)(tj - ti * c1);
+  const int i = (int)ti;
   const long long z = C.zoff + L.idx(i, j, k);
   const bool pole = Dv.metric == HAMR_METRIC_KERR_SCHILD && (C.J0 + j == 0 || C.J0 + j == (BLK ? Dv.B.n2g : L.n[1]));
   const long long S[3] = {L.S1, L.S2, 1};

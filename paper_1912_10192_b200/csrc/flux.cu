@@ -334,19 +334,22 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
   constexpr unsigned FULL = 0xffffffffu;
   const Lay& L = Dv.L;
   const int ck = L.n[2] + 1 + HLO + HHI, cj = L.n[1] + 2;
-  const long long per = (long long)(L.n[0] + 2) * cj * ck;
-  const long long tot = BLK ? per * Dv.B.nact : per;
+  // 32-bit index arithmetic (the launcher guarantees tot < 2^31): 64-bit division is emulated
+  const int per = (L.n[0] + 2) * cj * ck;
+  const int tot = BLK ? per * Dv.B.nact : per;
   const int lane = threadIdx.x & 31;
-  const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  long long t = warp * OWN + lane - HLO;
-  const bool valid = t >= 0 && t < tot;
-  t = t < 0 ? 0 : (t >= tot ? tot - 1 : t);  // clamped lanes compute on a real zone and store nothing
+  const int warp = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  int ts = warp * OWN + lane - HLO;
+  const bool valid = ts >= 0 && ts < tot;
+  ts = ts < 0 ? 0 : (ts >= tot ? tot - 1 : ts);  // clamped lanes compute on a real zone and store nothing
+  unsigned t = (unsigned)ts;
   int bslot = 0;
-  if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
+  if (BLK) { bslot = (int)(t / (unsigned)per); t -= bslot * per; }
   const BCtx C = blk_ctx<BLK>(Dv, bslot);
-  const int k = (int)(t % ck) - HLO;
-  const int j = (int)((t / ck) % cj) - 1;
-  const int i = (int)(t / ((long long)ck * cj)) - 1;
+  const unsigned tj = t / (unsigned)ck, ti = tj / (unsigned)cj;
+  const int k = (int)(t - tj * ck) - HLO;
+  const int j = (int)(tj - ti * cj) - 1;
+  const int i = (int)ti - 1;
   const int z = C.zoff + (int)L.idx(i, j, k);
   const double* var[7] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
                           selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),

@@ -37,6 +37,7 @@ struct BlkDev {
   const int* K0;             // [nblk] global x3 index of local zone 0
   int* tau;                  // [nblk] LAT time level (C-17)
   int* cur;                  // [nblk] which of the 3 buffers holds the block's time-n state (0 or 2)
+  int* flags;                // [nblk] bit 0: ghost fill is a plain copy; bit 1: has a finer-level neighbour
   double* ctopb;             // [nblk][3] max signal speed of the block's last corrector pass (C-14)
   double* FA2[3][5];         // flux registers: dt_b F summed over the steps inside one coarser step (C-17)
   double* EA2[3];            // EMF registers
@@ -106,6 +107,7 @@ struct BlkHost {
   std::vector<int> lev1;     // [nblk] x1 refinement level
   std::vector<int> tau;      // [nblk] current time level
   std::vector<int> I0;       // [nblk][3]
+  std::vector<int> phys;     // [nblk] physical-boundary sides
   std::vector<int> forced;   // test hook: prescribed time levels (empty: Courant-based)
   int* d_lists;              // device [5][nblk]: blocks of level 0..3, then every block
   int* d_clists;             // device [4][nblk]: blocks of level tau with a neighbour on tau - 1

@@ -32,8 +32,9 @@ template <bool SAME, bool BLK>  // SAME: predictor, source state == base state
 __global__ void __launch_bounds__(128) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
-  const long long per = (long long)(L.n[0] + 1) * c1 * c2;
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  // 32-bit index arithmetic throughout: 64-bit division is emulated (~100 instructions each)
+  const unsigned per = (unsigned)(L.n[0] + 1) * c1 * c2;
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = t < (BLK ? per * Dv.B.nact : per);
   int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0;
   if (valid) {
@@ -42,9 +43,10 @@ __global__ void __launch_bounds__(128) k_update(Dev Dv, Roles ra, Roles rb, doub
     const BCtx C = blk_ctx<BLK>(Dv, bslot);
     const Fields src = pick_fields<BLK>(ra.src, rb.src, C.cur), base = pick_fields<BLK>(ra.base, rb.base, C.cur),
                  out = pick_fields<BLK>(ra.out, rb.out, C.cur);
-    const int k = (int)(t % c2);
-    const int j = (int)((t / c2) % c1);
-    const int i = (int)(t / ((long long)c2 * c1));
+    const unsigned tj = t / (unsigned)c2;
+    const int k = (int)(t - tj * c2);
+    const int i = (int)(tj / (unsigned)c1);
+    const int j = (int)(tj - i * c1);
     const long long z = C.zoff + L.idx(i, j, k);
     const double dt = dtfac * Dv.scal[S_DT];
     const long long S[3] = {L.S1, L.S2, 1};
