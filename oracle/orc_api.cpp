@@ -151,6 +151,7 @@ int orc_set_prims(void* h, const double* const hydro[5], const double* const bfa
         std::fill(b.sn.Bf[d].begin(), b.sn.Bf[d].end(), 0.0);
         if (bface && bface[d]) scatter(g, b, b.sn.Bf[d], bface[d], d, true);
       }
+      deref_project(g.par, b, b.sn);
     }
     blocks_initial_dt(g);
     g.t = 0.0;

@@ -40,6 +40,13 @@ void blocks_build(Grid& g) {
     if (refined) { slots.push_back({col, 1, 0}); slots.push_back({col, 1, 1}); }
     else { slots.push_back({col, 0, 0}); seen_coarse = true; }
   }
+  if (par.n_deref > 0) {
+    // C-15: the strided x3 stencil of a derefined row wraps inside the block
+    if (NB[2] != 1 || par.bc_lo[2] != 0) throw std::runtime_error("phi-derefinement needs blocks that span a periodic x3");
+    for (int t = 0; t < par.n_deref && t < 4; t++)
+      if (par.deref_factor[t] < 1 || par.n[2] % par.deref_factor[t] != 0)
+        throw std::runtime_error("deref factor must divide n3");
+  }
   g.nslot[0] = (int)slots.size(); g.nslot[1] = NB[1]; g.nslot[2] = NB[2];
   g.lattice.assign((size_t)g.nslot[0] * NB[1] * NB[2], -1);
   g.blocks.clear();
@@ -174,7 +181,9 @@ static void stage_level(Grid& g, int tau, bool corrector) {
     if (b.tau != tau) continue;
     Fields& src = corrector ? b.sh : b.sn;
     flux_pass(g.par, b, src);
+    deref_fix_fluxes(g.par, b);
     ct_edges(g.par, b, src);
+    deref_fix_edges(g.par, b);
     const double dtb = g.dt * (double)(b.dt_u / 2);      // dt_b = 2^tau dt_0
     if (corrector) {
       // C-17 registers: R1 = dt_b * (F, E) of this corrector; R2 accumulates the two steps that
@@ -338,6 +347,7 @@ static void correct_level(Grid& g, int tau) {
           for (int cc = 0; cc < 5; cc++) c.snew.P[cc][z] = Pn[cc];
         }
       }
+    deref_sync_groups(par, c, c.snew);
   }
 }
 

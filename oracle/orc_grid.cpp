@@ -10,6 +10,24 @@ long long g_fail_hist[4] = {0, 0, 0, 0};  // debug: con2prim failure codes seen
 
 static const int CYC[3][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}};  // (d, e, f) cyclic
 
+// C-15: phi-derefinement factor of global x2 row J by its zone-centre polar angle: the largest factor
+// whose threshold (degrees from either pole) the row lies inside.  Rows beyond a pole (ghosts) take
+// the factor of their mirror image (of their periodic image if x2 is periodic).
+int deref_factor_of_row(const Params& par, long long J) {
+  if (par.n_deref <= 0) return 1;
+  const long long N2 = par.n[1];
+  if (par.bc_lo[1] == 0) J = ((J % N2) + N2) % N2;   // periodic x2: the image row
+  if (J < 0) J = -J - 1;                              // beyond a pole: the mirror row
+  if (J >= N2) J = 2 * N2 - 1 - J;
+  if (J < 0 || J >= N2) return 1;
+  // polar angle of the zone centre in degrees; on the Cartesian map the x2 extent plays (0, 180)
+  const double th = ((double)J + 0.5) / (double)N2 * 180.0;
+  int m = 1;
+  for (int t = 0; t < par.n_deref && t < 4; t++)
+    if (th < par.deref_theta_deg[t] || th > 180.0 - par.deref_theta_deg[t]) m = std::max(m, (int)par.deref_factor[t]);
+  return m;
+}
+
 void block_init(const Params& par, Block& b) {
   for (int d = 0; d < 3; d++) b.e[d] = b.n[d] + 2 * NG + 1;
   const size_t n2d = (size_t)b.e[0] * b.e[1];
@@ -22,6 +40,7 @@ void block_init(const Params& par, Block& b) {
   for (int j = -NG; j <= b.n[1] + NG; j++) {
     const long long J = b.I0[1] + j;
     if (par.metric == 1 && (J == 0 || J == par.n[1])) b.pole2[j + NG] = 1;
+    b.mrow[j + NG] = deref_factor_of_row(par, J);
   }
   for (int i = -NG; i <= b.n[0] + NG; i++)
     for (int j = -NG; j <= b.n[1] + NG; j++) {
@@ -99,21 +118,25 @@ void compute_Bc(const Block& b, Fields& s, bool active_only) {
   for (int i = lo; i < b.n[0] - lo; i++)
     for (int j = lo; j < b.n[1] - lo; j++) {
       const double g = b.gc[b.idx2(i, j)].gdet;
+      const int m = b.mrow[j + NG], n3 = b.n[2];
       for (int k = lo; k < b.n[2] - lo; k++) {
         const size_t z = b.idx(i, j, k);
         for (int d = 0; d < 3; d++)
           s.Bc[d][z] = (s.Bf[d][z] + s.Bf[d][z + str[d]]) / (2.0 * g);
+        if (m > 1) {
+          // C-15 (iii): in a derefined row B_c^3 is the GROUP's value, from the group's two outer x3-faces
+          const int kk = ((k % n3) + n3) % n3, k0 = kk - kk % m;
+          s.Bc[2][z] = (s.Bf[2][b.idx(i, j, k0)] + s.Bf[2][b.idx(i, j, k0 + m)]) / (2.0 * g);
+        }
       }
     }
 }
 
 // ---- reconstruct + HLL on one face (C-5, C-6, C-7) -------------------------------------------------
-// face on the low side of zone (i,j,k) along d; `st` = stencil stride along d (1; m in derefined rows)
-static void face_flux(const Params& par, Block& b, const Fields& s, int d, int i, int j, int k,
-                      int st, double* ctop) {
-  const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
-  const size_t z = b.idx(i, j, k);
-  const ptrdiff_t sd = (ptrdiff_t)str[d] * st;
+// face on the low side of zone z along d.  st6[v][0..5]: the six zone values a[j-3 .. j+2] of the
+// seven reconstructed variables around the face (j = the zone on the high side).
+static void face_flux_core(const Params& par, Block& b, const Fields& s, int d, int i, int j, size_t z,
+                           const double st6[7][6], double* ctop) {
   const int e = CYC[d][1], f = CYC[d][2];
   const Geom& G = (d == 0) ? b.gf1[b.idx2(i, j)] : (d == 1) ? b.gf2[b.idx2(i, j)] : b.gc[b.idx2(i, j)];
   if (d == 1 && b.pole2[j + NG]) {  // C-7: pole faces carry no flux; no state is evaluated
@@ -122,22 +145,16 @@ static void face_flux(const Params& par, Block& b, const Fields& s, int d, int i
     return;
   }
   double PL[8], PR[8];
-  const double* var[7] = {s.P[0].data(), s.P[1].data(), s.P[2].data(), s.P[3].data(),
-                          s.P[4].data(), s.Bc[e].data(), s.Bc[f].data()};
   const int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
   for (int v = 0; v < 7; v++) {
-    const double* a = var[v] + z;
+    const double* a = st6[v];
     double aL, aR, dummy;
     if (par.recon == 0) {
-      const double l5[5] = {a[-3 * sd], a[-2 * sd], a[-sd], a[0], a[sd]};
-      const double r5[5] = {a[-2 * sd], a[-sd], a[0], a[sd], a[2 * sd]};
-      ppm_zone(l5, dummy, aR);  // left of the face: a_R of zone j-1
-      ppm_zone(r5, aL, dummy);  // right of the face: a_L of zone j
+      ppm_zone(a, dummy, aR);      // left of the face: a_R of zone j-1 from a[j-3 .. j+1]
+      ppm_zone(a + 1, aL, dummy);  // right of the face: a_L of zone j from a[j-2 .. j+2]
     } else {
-      const double l3[3] = {a[-2 * sd], a[-sd], a[0]};
-      const double r3[3] = {a[-sd], a[0], a[sd]};
-      plm_zone(l3, dummy, aR);
-      plm_zone(r3, aL, dummy);
+      plm_zone(a + 1, dummy, aR);  // a[j-2 .. j]
+      plm_zone(a + 2, aL, dummy);  // a[j-1 .. j+1]
     }
     PL[slot[v]] = aR;
     PR[slot[v]] = aL;
@@ -164,6 +181,37 @@ static void face_flux(const Params& par, Block& b, const Fields& s, int d, int i
   if (ctop) *ctop = std::max(cmax, cmin);
 }
 
+static void face_flux(const Params& par, Block& b, const Fields& s, int d, int i, int j, int k,
+                      double* ctop) {
+  const int str[3] = {b.e[1] * b.e[2], b.e[2], 1};
+  const size_t z = b.idx(i, j, k);
+  const ptrdiff_t sd = str[d];
+  const int e = CYC[d][1], f = CYC[d][2];
+  const double* var[7] = {s.P[0].data(), s.P[1].data(), s.P[2].data(), s.P[3].data(),
+                          s.P[4].data(), s.Bc[e].data(), s.Bc[f].data()};
+  double st6[7][6];
+  for (int v = 0; v < 7; v++)
+    for (int t = 0; t < 6; t++) st6[v][t] = var[v][(ptrdiff_t)z + (t - 3) * sd];
+  face_flux_core(par, b, s, d, i, j, z, st6, ctop);
+}
+
+// C-15 (ii): x3-face on a group boundary of a phi-derefined row (k a multiple of m): the stencil takes
+// one value per GROUP, i.e. zones k + t m, t = -3..2, wrapped periodically (the block spans all of x3).
+static void face_flux_x3_deref(const Params& par, Block& b, const Fields& s, int i, int j, int k, int m,
+                               double* ctop) {
+  const size_t z = b.idx(i, j, k);
+  const int n3 = b.n[2];
+  const double* var[7] = {s.P[0].data(), s.P[1].data(), s.P[2].data(), s.P[3].data(),
+                          s.P[4].data(), s.Bc[0].data(), s.Bc[1].data()};
+  double st6[7][6];
+  for (int v = 0; v < 7; v++)
+    for (int t = 0; t < 6; t++) {
+      const int kk = (((k + (t - 3) * m) % n3) + n3) % n3;
+      st6[v][t] = var[v][b.idx(i, j, kk)];
+    }
+  face_flux_core(par, b, s, 2, i, j, z, st6, ctop);
+}
+
 void flux_pass(const Params& par, Block& b, const Fields& src) {
   for (int d = 0; d < 3; d++) {
     int lo[3] = {-1, -1, -1}, hi[3] = {b.n[0], b.n[1], b.n[2]};  // one transverse ghost layer (CT)
@@ -175,7 +223,16 @@ void flux_pass(const Params& par, Block& b, const Fields& src) {
       for (int j = lo[1]; j <= hi[1]; j++)
         for (int k = lo[2]; k <= hi[2]; k++) {
           double ct = 0.0;
-          face_flux(par, b, src, d, i, j, k, 1, &ct);
+          const int m = b.mrow[j + NG];
+          if (d == 2 && m > 1) {
+            // C-15 (ii): fluxes only on group-boundary faces (the others are interpolated by
+            // deref_fix_fluxes); the Courant limit of the row uses the group width m dx3
+            if (k < 0 || k > b.n[2] || k % m != 0) continue;
+            face_flux_x3_deref(par, b, src, i, j, k, m, &ct);
+            ct /= (double)m;
+          } else {
+            face_flux(par, b, src, d, i, j, k, &ct);
+          }
           const int id[3] = {i, j, k};
           bool act = true;  // C-14: the Courant maximum runs over the faces of ACTIVE zones
           for (int t = 0; t < 3; t++)
@@ -184,6 +241,118 @@ void flux_pass(const Params& par, Block& b, const Fields& src) {
         }
     b.ctop[d] = cmaxd;
   }
+}
+
+// ---- phi-derefinement fix-ups (C-15; "averages the fluxes ... over 2^n cells") --------------
+// Everything is stored on the fine grid.  After the flux pass the face quantities of derefined rows are
+// given the group structure: x1- and x2-face values become their group mean, x3-face values between
+// group boundaries the linear interpolation of the two boundary faces.  With one value per fine face
+// and per fine edge, the unchanged update conserves and the unchanged CT keeps div B per FINE zone.
+static inline int face2_factor(const Block& b, int j) {  // x2-face j lies between rows j-1 and j
+  return std::max(b.mrow[j - 1 + NG], b.mrow[j + NG]);
+}
+
+static void group_mean(std::vector<double>& a, const Block& b, int i, int j, int m) {
+  const int n3 = b.n[2];
+  for (int k0 = 0; k0 < n3; k0 += m) {
+    double sum = 0.0;
+    for (int r = 0; r < m; r++) sum += a[b.idx(i, j, k0 + r)];
+    const double mean = sum / (double)m;
+    for (int r = 0; r < m; r++) a[b.idx(i, j, k0 + r)] = mean;
+  }
+  a[b.idx(i, j, -1)] = a[b.idx(i, j, n3 - 1)];  // the periodic transverse ghost layer (feeds C-9)
+  a[b.idx(i, j, n3)] = a[b.idx(i, j, 0)];
+}
+
+static void group_interp(std::vector<double>& a, const Block& b, int i, int j, int m) {
+  const int n3 = b.n[2];
+  for (int k0 = 0; k0 < n3; k0 += m) {
+    const double lo = a[b.idx(i, j, k0)], hi = a[b.idx(i, j, k0 + m)];
+    for (int r = 1; r < m; r++) a[b.idx(i, j, k0 + r)] = lo + ((double)r / (double)m) * (hi - lo);
+  }
+}
+
+void deref_fix_fluxes(const Params& par, Block& b) {
+  if (par.n_deref <= 0) return;
+  for (int i = -1; i <= b.n[0]; i++)
+    for (int j = -1; j <= b.n[1]; j++) {
+      const int m = b.mrow[j + NG];
+      if (m > 1 && i >= 0) {          // x1-faces of the row
+        for (int c = 0; c < 5; c++) group_mean(b.F[0][c], b, i, j, m);
+        group_mean(b.Ef[0][1], b, i, j, m);
+        group_mean(b.Ef[0][2], b, i, j, m);
+      }
+      if (m > 1) {                    // x3-faces of the row: in-group faces
+        for (int c = 0; c < 5; c++) group_interp(b.F[2][c], b, i, j, m);
+        group_interp(b.Ef[2][0], b, i, j, m);
+        group_interp(b.Ef[2][1], b, i, j, m);
+      }
+      if (j >= 0) {                   // x2-face between rows j-1 and j: the coarser of the two groupings
+        const int M = face2_factor(b, j);
+        if (M > 1) {
+          for (int c = 0; c < 5; c++) group_mean(b.F[1][c], b, i, j, M);
+          group_mean(b.Ef[1][2], b, i, j, M);
+          group_mean(b.Ef[1][0], b, i, j, M);
+        }
+      }
+    }
+}
+
+// C-15 (iv): E3 is a group mean; E1 and E2 exist on group-boundary phi-edges, the ones in between are
+// their linear interpolation.  Edges on an x2-face row use the coarser grouping of the two rows.
+void deref_fix_edges(const Params& par, Block& b) {
+  if (par.n_deref <= 0) return;
+  const int n3 = b.n[2];
+  for (int i = 0; i <= b.n[0]; i++)
+    for (int j = 0; j <= b.n[1]; j++) {
+      const int m = b.mrow[j + NG], M = face2_factor(b, j);
+      if (M > 1) {                                         // E3 at (i-1/2, j-1/2, k)
+        for (int k0 = 0; k0 < n3; k0 += M) {
+          double sum = 0.0;
+          for (int r = 0; r < M; r++) sum += b.Ee[2][b.idx(i, j, k0 + r)];
+          for (int r = 0; r < M; r++) b.Ee[2][b.idx(i, j, k0 + r)] = sum / (double)M;
+        }
+      }
+      if (M > 1 && i < b.n[0]) group_interp(b.Ee[0], b, i, j, M);   // E1 at (i, j-1/2, k-1/2)
+      if (m > 1 && j < b.n[1]) group_interp(b.Ee[1], b, i, j, m);   // E2 at (i-1/2, j, k-1/2)
+    }
+}
+
+// C-15 (v): one inversion per group: the group's first member's result is the group's
+void deref_sync_groups(const Params& par, Block& b, Fields& s) {
+  if (par.n_deref <= 0) return;
+  for (int i = 0; i < b.n[0]; i++)
+    for (int j = 0; j < b.n[1]; j++) {
+      const int m = b.mrow[j + NG];
+      if (m <= 1) continue;
+      for (int k = 0; k < b.n[2]; k++) {
+        if (k % m == 0) continue;
+        const size_t z = b.idx(i, j, k), z0 = b.idx(i, j, k - k % m);
+        for (int c = 0; c < 5; c++) s.P[c][z] = s.P[c][z0];
+        for (int c = 0; c < 3; c++) s.Bc[c][z] = s.Bc[c][z0];
+      }
+    }
+}
+
+// C-15 (i): puts an initial state onto the invariant: hydro primitives become their group mean; the
+// x3-face field between group boundaries the linear interpolation of the boundary faces.  The face
+// fields Bf1, Bf2 are expected to be group-uniform already (true for any axisymmetric field).
+void deref_project(const Params& par, Block& b, Fields& s) {
+  if (par.n_deref <= 0) return;
+  for (int i = 0; i <= b.n[0]; i++)
+    for (int j = 0; j < b.n[1]; j++) {
+      const int m = b.mrow[j + NG];
+      if (m <= 1) continue;
+      if (i < b.n[0]) {
+        for (int c = 0; c < 5; c++)
+          for (int k0 = 0; k0 < b.n[2]; k0 += m) {
+            double sum = 0.0;
+            for (int r = 0; r < m; r++) sum += s.P[c][b.idx(i, j, k0 + r)];
+            for (int r = 0; r < m; r++) s.P[c][b.idx(i, j, k0 + r)] = sum / (double)m;
+          }
+        group_interp(s.Bf[2], b, i, j, m);
+      }
+    }
 }
 
 // ---- constrained transport (C-8, C-9) -------------------------------------------------------------
@@ -316,6 +485,7 @@ void update(const Params& par, Block& b, const Fields& src, const Fields& base, 
       }
     }
   st.c2p_fail += nfail; st.rho_floor += nrf; st.u_floor += nuf; st.gam_ceil += ngc;
+  deref_sync_groups(par, b, out);
 }
 
 // C-14 (PAPER.md:93 fn. 2): 1/dt = sum_d 1/dt_d, dt_d = C dx^d / max ctop_d

@@ -87,6 +87,12 @@ void ct_edges(const Params& par, Block& b, const Fields& src);
 void update(const Params& par, Block& b, const Fields& src, const Fields& base, Fields& out,
             double dt, Stats& st);
 double dt_from_ctop(const Params& par, const Block& b);
+// C-15 phi-derefinement (orc_grid.cpp)
+int deref_factor_of_row(const Params& par, long long J);
+void deref_fix_fluxes(const Params& par, Block& b);
+void deref_fix_edges(const Params& par, Block& b);
+void deref_sync_groups(const Params& par, Block& b, Fields& s);
+void deref_project(const Params& par, Block& b, Fields& s);
 void floors_and_ceiling(const Params& par, const Geom& G, double r, double P[5], Stats& st);
 
 }  // namespace orc

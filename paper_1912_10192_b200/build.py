@@ -33,6 +33,7 @@ def _stale(target: str, deps) -> bool:
 
 def build_lib(verbose: bool = False, force: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
+    extra = os.environ.get("HAMR_EXTRA_NVCC_FLAGS", "").split()   # tuning experiments (-DHAMR_...=n)
     nvcc = _nvcc()
     hdrs = [os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
     jobs = []
@@ -44,7 +45,7 @@ def build_lib(verbose: bool = False, force: bool = False) -> str:
 
     def compile_one(job):
         src, obj = job
-        r = subprocess.run([nvcc] + NVCC_FLAGS + ["-c", src, "-o", obj], capture_output=True, text=True)
+        r = subprocess.run([nvcc] + NVCC_FLAGS + extra + ["-c", src, "-o", obj], capture_output=True, text=True)
         log = r.stdout + r.stderr
         with open(obj + ".log", "w") as f:
             f.write(log)

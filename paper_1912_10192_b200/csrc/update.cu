@@ -28,8 +28,14 @@ __device__ __forceinline__ Fields pick_fields(const Fields& a, const Fields& b, 
   return f;
 }
 
+#ifndef HAMR_UPD_RELOAD
+#define HAMR_UPD_RELOAD 1  // measured on cfg 2: 0.561 -> 0.516 ms (predictor) together with HAMR_UPD_MINB 6
+#endif
+#ifndef HAMR_UPD_MINB
+#define HAMR_UPD_MINB 6  // 80 regs (72 B spilled); 4 / 5 measured 4 % / 7 % slower with the reload, 8 slower still
+#endif
 template <bool SAME, bool BLK>  // SAME: predictor, source state == base state
-__global__ void __launch_bounds__(128) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
+__global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
   // 32-bit index arithmetic throughout: 64-bit division is emulated (~100 instructions each)
@@ -131,16 +137,38 @@ __global__ void __launch_bounds__(128) k_update(Dev Dv, Roles ra, Roles rb, doub
         U[c] = U[c] - dt * div + dt * sc;
       }
       double Pn[5];
+#if HAMR_UPD_RELOAD
+      // the geometry record and the guess are re-read (L1 / L2 hits) instead of being kept in registers
+      // across the flux divergence: lower register pressure, more resident warps
+      const double* gtab = Dv.gc + tl;
+      asm volatile("" : "+l"(gtab));
+      const Geo G2 = load_geo(gtab, L.n2d, q);
+      const double* sp[5] = {src.P[0], src.P[1], src.P[2], src.P[3], src.P[4]};
+      double Pg[5];
+#pragma unroll
+      for (int c = 0; c < 5; c++) { const double* a = sp[c]; asm volatile("" : "+l"(a)); Pg[c] = a[z]; }
+      const int rc = con2prim(U, Bn, G2, Dv.gam, Pg, Pn);
+      if (rc != 0) {
+        nfail = 1;
+#pragma unroll
+        for (int c = 0; c < 5; c++) Pn[c] = Pg[c];
+      }
+#define G G2
+#else
       const int rc = con2prim(U, Bn, G, Dv.gam, Ps, Pn);
       if (rc != 0) {  // C-13: keep the source state's hydro primitives, count the failure
         nfail = 1;
 #pragma unroll
         for (int c = 0; c < 5; c++) Pn[c] = Ps[c];
       }
+#endif
       // floors and Lorentz-factor ceiling (C-13)
       const int fi = C.I0 + i + NG + (BLK ? C.lev * Dv.B.flev : 0);
       const double rfl = __ldg(Dv.rho_fl + fi), ufl = __ldg(Dv.u_fl + fi);
       floors_ceiling(G, rfl, ufl, Dv.gamma_max, Pn, nrf, nuf, ngc);
+#if HAMR_UPD_RELOAD
+#undef G
+#endif
 #pragma unroll
       for (int c = 0; c < 5; c++) {
         out.P[c][z] = Pn[c];
