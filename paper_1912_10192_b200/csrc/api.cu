@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 #include "hamr_host.h"
 
 using namespace hamr;
@@ -34,9 +35,17 @@ bool params_ok(const hamr_params& p, std::string& why) {
   if (p.recon != HAMR_RECON_PPM && p.recon != HAMR_RECON_PLM_MC) { why = "bad recon"; return false; }
   if (p.metric == HAMR_METRIC_KERR_SCHILD && !(p.xmin[0] > 0.0)) { why = "r_in <= 0"; return false; }
   if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0) || !(p.gamma_max > 1.0)) { why = "gamma_ad / cour / gamma_max"; return false; }
-  if (p.n_deref || p.r_refine_max > 0.0) {
-    why = "phi-derefinement and r-refinement are not available in this build (DESIGN.md section 9)";
+  if (p.r_refine_max > 0.0) {
+    why = "r-refinement is not available in this build (DESIGN.md section 9)";
     return false;
+  }
+  if (p.n_deref < 0 || p.n_deref > 4) { why = "n_deref must be 0..4"; return false; }
+  if (p.n_deref > 0) {
+    // C-15: the strided x3 stencil of a derefined row wraps inside the grid / block
+    if (p.bc_lo[2] != HAMR_BC_PERIODIC) { why = "phi-derefinement needs a periodic x3"; return false; }
+    if (p.nb[2] != 0 && p.nb[2] != p.n[2]) { why = "phi-derefinement needs blocks that span x3"; return false; }
+    for (int t = 0; t < p.n_deref; t++)
+      if (p.deref_factor[t] < 1 || p.n[2] % p.deref_factor[t] != 0) { why = "deref factor must divide n3"; return false; }
   }
   if (p.lat_max_level < 0 || p.lat_max_level > 3) { why = "lat_max_level must be 0..3"; return false; }
   if (is_block_grid(p)) {
@@ -80,7 +89,7 @@ bool make_layout(const hamr_params& p, Lay& L, GridShape& G) {
 }
 
 struct ArenaPlan {
-  size_t arr, tabs, scal, cnt, stage, blk, total;
+  size_t arr, tabs, scal, cnt, stage, blk, mrow, total;
   size_t stage_doubles;
 };
 
@@ -94,6 +103,7 @@ ArenaPlan plan_arena(const hamr_params& p, const Lay& L, const GridShape& G) {
   a.stage_doubles = (size_t)8 * (p.n[0] + 1) * (p.n[1] + 1) * (p.n[2] + 1);
   a.stage = off; off += align_up(a.stage_doubles * 8, 256);
   a.blk = off; off += G.nblk > 0 ? blk_table_bytes(G.nblk) : 0;
+  a.mrow = off; off += p.n_deref > 0 ? align_up((size_t)G.te2 * sizeof(int), 256) : 0;
   a.total = off;
   return a;
 }
@@ -221,6 +231,16 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
     e = cudaGetLastError();
   }
   if (e == cudaSuccess && gs.nblk > 0 && blk_setup(g, base + ap.blk) != HAMR_OK) e = cudaErrorUnknown;
+  if (e == cudaSuccess && p->n_deref > 0) {   // C-15: derefinement factor per global x2 row incl. ghosts
+    std::vector<int> mrow(gs.te2);
+    bool any = false;
+    for (int t = 0; t < gs.te2; t++) { mrow[t] = deref_row_factor(*p, (long long)t - NG); any = any || mrow[t] > 1; }
+    if (any) {
+      e = cudaMemcpyAsync(base + ap.mrow, mrow.data(), (size_t)gs.te2 * sizeof(int), cudaMemcpyHostToDevice, g->stream);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
+      D.mrow = (const int*)(base + ap.mrow);
+    }
+  }
   if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
   if (e != cudaSuccess) {
     cudaFreeHost(g->h_pinned);
@@ -259,7 +279,9 @@ void enqueue_stage(hamr_grid* g, const Fields& src, const Fields& base, const Fi
   launch_ghosts(g, src, false);
   launch_flux(g, src, want_ctop);
   launch_ct(g, src);
+  launch_deref_fix_edges(g, g->D);
   launch_update(g, src, base, out, dtfac, same);
+  launch_deref_sync(g, g->D, out, out);
 }
 
 void enqueue_step(hamr_grid* g) {
@@ -318,6 +340,7 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
     if (rc != HAMR_OK) return fail(g, rc, "block grid initialisation failed");
     blk_check_finite(g);
   } else {
+    launch_deref_project(g, g->D, sn, sn);
     launch_ghosts(g, sn, true);
     launch_flux(g, sn, true);   // C-14: one flux pass sets dt of step 0
     launch_dt(g, 0);
@@ -527,6 +550,7 @@ int hamr_debug_emf(hamr_grid* g) {
   launch_zero_ctop(g);
   launch_flux(g, sn, true);
   launch_ct(g, sn);
+  launch_deref_fix_edges(g, g->D);
   launch_dt(g, 2);
   CK(cudaStreamSynchronize(g->stream));
   CK(cudaGetLastError());

@@ -87,6 +87,13 @@ __device__ __forceinline__ void ghost_cell(const Dev& D, const Fields& s, int al
   }
   if (zone_slot) {
     const double g = __ldg(D.gc + GDET * L.n2d + L.idx2(i, j));
+    if (D.mrow && __ldg(D.mrow + j + NG) > 1) {
+      // C-15: B_c^3 of a phi-derefined row is the group's value, from the group's two outer x3-faces
+      const int m = __ldg(D.mrow + j + NG), n3 = L.n[2];
+      const int kk = ((k % n3) + n3) % n3, k0 = kk - kk % m;
+      lo[2] = ghost_value(D, s.Bf[2], 2, 2, i, j, k0);
+      hi[2] = ghost_value(D, s.Bf[2], 2, 2, i, j, k0 + m);
+    }
     for (int d = 0; d < 3; d++) s.Bc[d][z] = (lo[d] + hi[d]) / (2.0 * g);
   }
 }

@@ -286,6 +286,19 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
   if (zone_slot && (!zone_active || all || anymod)) {
     const int4 inf = __ldg(Dv.B.info + b);
     const double g = __ldg(Dv.gc + inf.y * Dv.B.tlev + GDET * L.n2d + inf.x + id[0] * Dv.B.ge2 + id[1]);
+    if (Dv.mrow && __ldg(Dv.mrow + inf.w + id[1] + NG) > 1) {
+      // C-15: B_c^3 of a phi-derefined row is the group's value (the block spans all of x3)
+      const int m = __ldg(Dv.mrow + inf.w + id[1] + NG), n3 = L.n[2];
+      const int kk = ((id[2] % n3) + n3) % n3, k0 = kk - kk % m;
+      int ig[3] = {id[0], id[1], k0};
+      GSrc s = blk_src(Dv, b, phys, 2, ig, same);
+      if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
+      lo[2] = blk_fetch(Dv, B, b, own, 7, s, qt);
+      ig[2] = k0 + m;
+      s = blk_src(Dv, b, phys, 2, ig, same);
+      if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
+      hi[2] = blk_fetch(Dv, B, b, own, 7, s, qt);
+    }
 #pragma unroll
     for (int d = 0; d < 3; d++) {
       double* bc = own == 0 ? B.s[0].Bc[d] : (own == 1 ? B.s[1].Bc[d] : B.s[2].Bc[d]);
@@ -876,6 +889,7 @@ static void blk_stage(hamr_grid* g, int tau, bool corrector) {
     const Fields& s2 = g->s[2];
     launch_flux_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2, corrector);
     launch_ct_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2);
+    launch_deref_fix_edges(g, D);
     const double lev_fac = (double)(1 << tau);   // dt_b = 2^tau dt_0
     if (corrector && tau < H.tmax) {
       const int first = (H.tb_u[tau] % (2LL * H.dt_u[tau])) == 0 ? 1 : 0;
@@ -887,9 +901,11 @@ static void blk_stage(hamr_grid* g, int tau, bool corrector) {
     if (!corrector) {
       const Roles ra = {s0, s0, s1}, rb = {s2, s2, s1};
       launch_update_on(g, D, ra, rb, 0.5 * lev_fac, true);
+      launch_deref_sync(g, D, s1, s1);
     } else {
       const Roles ra = {s1, s0, s2}, rb = {s1, s2, s0};
       launch_update_on(g, D, ra, rb, lev_fac, false);
+      launch_deref_sync(g, D, s2, s0);
     }
   }
   if (corrector) H.has_new[tau] = 1;
@@ -910,8 +926,11 @@ static void blk_correct(hamr_grid* g, int tau) {
     k_blk_correct_faces<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, bufs_of(g), tau, lev_fac);
   }
   tot = (long long)L.n[0] * L.n[1] * L.n[2] * D.B.nact;
-  Launch l_(g, K_OTHER);
-  k_blk_correct_zones<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, bufs_of(g), tau, lev_fac);
+  {
+    Launch l_(g, K_OTHER);
+    k_blk_correct_zones<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, bufs_of(g), tau, lev_fac);
+  }
+  launch_deref_sync(g, D, g->s[2], g->s[0]);   // the corrected new state of a block with cur == 0 / 2
 }
 
 static void blk_rotate(hamr_grid* g, int tau) {
@@ -1042,6 +1061,7 @@ int blk_initial(hamr_grid* g) {
   if (cudaMemcpyAsync(H.d_lists, H.d_lists + (size_t)4 * H.nblk, (size_t)H.nblk * 4, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
     return HAMR_ECUDA;
   const Dev D = dev_list(g, 4);
+  launch_deref_project(g, D, g->s[0], g->s[2]);
   blk_ghosts(g, D, 0, 0, true, true);
   launch_flux_on(g, D, g->s[0], g->s[2], true);
   return blk_assign(g, false);

@@ -1,0 +1,190 @@
+// deref.cu — phi-derefinement of the polar rows ("internal SMR"; DESIGN.md §9 C-15).
+// near the poles the grid is derefined in phi; the code "averages the fluxes and conserved
+// quantities ... over 2^n cells" and adapts the reconstruction to the larger cell spacing.
+//
+// Reading (C-15): a row with factor m treats every aligned group of m phi-zones as one zone, but all
+// arrays stay on the FINE grid.  After the flux kernels the face values of derefined rows are given the
+// group structure (x1-/x2-face values -> group mean; x3-face values between group boundaries -> linear
+// interpolation of the boundary faces, which flux.cu: k_deref_x3 computes with a strided stencil), after
+// the edge-EMF kernel likewise (E3 -> group mean, E1 / E2 between group-boundary edges -> interpolation).
+// Every fine face and fine edge then carries ONE value, so the unchanged update conserves and the
+// unchanged CT keeps div B per fine zone; the hydro state of a group is that of its first member.
+// An x2-face (and its edges) between two rows uses the coarser of the two rows' groupings.
+//
+// All of this touches ~17 % of the rows of BASELINE cfg 4 and is HBM-bound streaming work; one thread
+// owns one group of one (i, j) column, so no two threads touch the same value.
+#include "hamr_host.h"
+
+namespace hamr {
+
+// C-15: factor of global x2 row J by the polar angle of its zone centre (degrees; on the Cartesian map the
+// x2 extent stands for (0, 180)): the largest factor whose threshold the row lies inside.  Rows beyond a
+// pole take their mirror row's factor, rows beyond a periodic x2 boundary their image's.
+int deref_row_factor(const hamr_params& p, long long J) {
+  if (p.n_deref <= 0) return 1;
+  const long long N2 = p.n[1];
+  if (p.bc_lo[1] == HAMR_BC_PERIODIC) J = ((J % N2) + N2) % N2;
+  if (J < 0) J = -J - 1;
+  if (J >= N2) J = 2 * N2 - 1 - J;
+  if (J < 0 || J >= N2) return 1;
+  const double th = ((double)J + 0.5) / (double)N2 * 180.0;
+  int m = 1;
+  for (int t = 0; t < p.n_deref && t < 4; t++)
+    if ((th < p.deref_theta_deg[t] || th > 180.0 - p.deref_theta_deg[t]) && p.deref_factor[t] > m) m = p.deref_factor[t];
+  return m;
+}
+
+// thread -> (block, i, j, k) over i in [ilo, n1 + ihi), j in [jlo, n2 + jhi), k in [0, n3)
+struct DIdx { int i, j, k; bool valid; BCtx C; };
+template <bool BLK>
+__device__ __forceinline__ DIdx deref_idx(const Dev& Dv, int ilo, int ihi, int jlo, int jhi) {
+  const Lay& L = Dv.L;
+  const int ci = L.n[0] + ihi - ilo, cj = L.n[1] + jhi - jlo, ck = L.n[2];
+  const unsigned per = (unsigned)ci * cj * ck;
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  DIdx r;
+  r.valid = t < (BLK ? per * Dv.B.nact : per);
+  if (!r.valid) t = 0;
+  int bslot = 0;
+  if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
+  r.C = blk_ctx<BLK>(Dv, bslot);
+  const unsigned tj = t / (unsigned)ck, ti = tj / (unsigned)cj;
+  r.k = (int)(t - tj * ck);
+  r.j = (int)(tj - ti * cj) + jlo;
+  r.i = (int)ti + ilo;
+  return r;
+}
+
+// group mean in place (members z0 .. z0 + m - 1), summed in member order; wrap: also the periodic
+// transverse ghost layer (k = -1 <- n3 - 1, k = n3 <- 0), which feeds the edge EMFs of C-9
+__device__ __forceinline__ void group_mean(double* __restrict__ a, long long zrow, int k0, int m, int n3, bool wrap) {
+  double sum = 0.0;
+  for (int r = 0; r < m; r++) sum += a[zrow + k0 + r];
+  const double mean = sum / (double)m;
+  for (int r = 0; r < m; r++) a[zrow + k0 + r] = mean;
+  if (wrap && k0 == 0) a[zrow + n3] = mean;
+  if (wrap && k0 + m == n3) a[zrow - 1] = mean;
+}
+
+// members 1 .. m-1 become the linear interpolation of the values at k0 and k0 + m
+__device__ __forceinline__ void group_interp(double* __restrict__ a, long long zrow, int k0, int m) {
+  const double lo = a[zrow + k0], hi = a[zrow + k0 + m];
+  for (int r = 1; r < m; r++) a[zrow + k0 + r] = lo + ((double)r / (double)m) * (hi - lo);
+}
+
+// C-15 (iii): after the three flux kernels
+template <bool BLK>
+__global__ void __launch_bounds__(128) k_deref_fix_flux(Dev Dv) {
+  const Lay& L = Dv.L;
+  const DIdx T = deref_idx<BLK>(Dv, -1, 1, -1, 1);   // i, j in [-1, n]: the transverse ghost layer included
+  if (!T.valid) return;
+  const int i = T.i, j = T.j, k = T.k, n3 = L.n[2];
+  const int m = __ldg(Dv.mrow + T.C.J0 + j + NG);
+  const int M = max(m, __ldg(Dv.mrow + T.C.J0 + j - 1 + NG));   // x2-face j lies between rows j-1 and j
+  const long long zrow = T.C.zoff + L.idx(i, j, 0);
+  if (m > 1 && k % m == 0) {
+    if (i >= 0) {                      // x1-faces of the row
+#pragma unroll
+      for (int c = 0; c < 5; c++) group_mean(Dv.F[0][c], zrow, k, m, n3, true);
+      group_mean(Dv.EfA[0], zrow, k, m, n3, true);
+      group_mean(Dv.EfB[0], zrow, k, m, n3, true);
+    }
+#pragma unroll
+    for (int c = 0; c < 5; c++) group_interp(Dv.F[2][c], zrow, k, m);   // x3-faces inside the group
+    group_interp(Dv.EfA[2], zrow, k, m);
+    group_interp(Dv.EfB[2], zrow, k, m);
+  }
+  if (j >= 0 && M > 1 && k % M == 0) {  // x2-face on the low side of row j
+#pragma unroll
+    for (int c = 0; c < 5; c++) group_mean(Dv.F[1][c], zrow, k, M, n3, true);
+    group_mean(Dv.EfA[1], zrow, k, M, n3, true);
+    group_mean(Dv.EfB[1], zrow, k, M, n3, true);
+  }
+}
+
+// C-15 (iv): after the edge-EMF kernel
+template <bool BLK>
+__global__ void __launch_bounds__(128) k_deref_fix_edges(Dev Dv) {
+  const Lay& L = Dv.L;
+  const DIdx T = deref_idx<BLK>(Dv, 0, 1, 0, 1);     // i in [0, n1], j in [0, n2]
+  if (!T.valid) return;
+  const int i = T.i, j = T.j, k = T.k, n3 = L.n[2];
+  const int m = __ldg(Dv.mrow + T.C.J0 + j + NG);
+  const int M = max(m, __ldg(Dv.mrow + T.C.J0 + j - 1 + NG));
+  const long long zrow = T.C.zoff + L.idx(i, j, 0);
+  if (M > 1 && k % M == 0) {
+    group_mean(Dv.Ee[2], zrow, k, M, n3, false);                 // E3 at (i-1/2, j-1/2, k)
+    if (i < L.n[0]) group_interp(Dv.Ee[0], zrow, k, M);          // E1 at (i, j-1/2, k-1/2)
+  }
+  if (m > 1 && k % m == 0 && j < L.n[1]) group_interp(Dv.Ee[1], zrow, k, m);   // E2 at (i-1/2, j, k-1/2)
+}
+
+// C-15 (v): one inversion per group: the first member's primitives and B_c are the group's
+template <bool BLK>
+__global__ void __launch_bounds__(128) k_deref_sync(Dev Dv, Fields o0, Fields o2) {
+  const Lay& L = Dv.L;
+  const DIdx T = deref_idx<BLK>(Dv, 0, 0, 0, 0);
+  if (!T.valid) return;
+  const int m = __ldg(Dv.mrow + T.C.J0 + T.j + NG);
+  const int r = T.k % m;
+  if (m == 1 || r == 0) return;
+  const long long z = T.C.zoff + L.idx(T.i, T.j, T.k);
+#pragma unroll
+  for (int c = 0; c < 5; c++) { double* a = selp<BLK>(o0.P[c], o2.P[c], T.C.cur); a[z] = a[z - r]; }
+#pragma unroll
+  for (int c = 0; c < 3; c++) { double* a = selp<BLK>(o0.Bc[c], o2.Bc[c], T.C.cur); a[z] = a[z - r]; }
+}
+
+// C-15 (i): puts an initial state onto the invariant: hydro primitives -> group mean, x3-face field between
+// group boundaries -> interpolation.  Bf1, Bf2 are expected to be group-uniform (any axisymmetric field is).
+template <bool BLK>
+__global__ void __launch_bounds__(128) k_deref_project(Dev Dv, Fields s0, Fields s2) {
+  const Lay& L = Dv.L;
+  const DIdx T = deref_idx<BLK>(Dv, 0, 0, 0, 0);
+  if (!T.valid) return;
+  const int m = __ldg(Dv.mrow + T.C.J0 + T.j + NG);
+  if (m == 1 || T.k % m != 0) return;
+  const long long zrow = T.C.zoff + L.idx(T.i, T.j, 0);
+#pragma unroll
+  for (int c = 0; c < 5; c++) group_mean(selp<BLK>(s0.P[c], s2.P[c], T.C.cur), zrow, T.k, m, L.n[2], false);
+  group_interp(selp<BLK>(s0.Bf[2], s2.Bf[2], T.C.cur), zrow, T.k, m);
+}
+
+static unsigned nblocks_for(const Dev& Dv, int ci, int cj) {
+  const long long tot = (long long)ci * cj * Dv.L.n[2] * (Dv.B.nblk > 0 ? Dv.B.nact : 1);
+  return (unsigned)((tot + 127) / 128);
+}
+
+void launch_deref_fix_flux(hamr_grid* g, const Dev& Dv) {
+  if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
+  Launch l_(g, K_OTHER);
+  const unsigned nb = nblocks_for(Dv, Dv.L.n[0] + 2, Dv.L.n[1] + 2);
+  if (Dv.B.nblk > 0) k_deref_fix_flux<true><<<nb, 128, 0, g->stream>>>(Dv);
+  else k_deref_fix_flux<false><<<nb, 128, 0, g->stream>>>(Dv);
+}
+
+void launch_deref_fix_edges(hamr_grid* g, const Dev& Dv) {
+  if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
+  Launch l_(g, K_OTHER);
+  const unsigned nb = nblocks_for(Dv, Dv.L.n[0] + 1, Dv.L.n[1] + 1);
+  if (Dv.B.nblk > 0) k_deref_fix_edges<true><<<nb, 128, 0, g->stream>>>(Dv);
+  else k_deref_fix_edges<false><<<nb, 128, 0, g->stream>>>(Dv);
+}
+
+void launch_deref_sync(hamr_grid* g, const Dev& Dv, const Fields& out, const Fields& out2) {
+  if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
+  Launch l_(g, K_OTHER);
+  const unsigned nb = nblocks_for(Dv, Dv.L.n[0], Dv.L.n[1]);
+  if (Dv.B.nblk > 0) k_deref_sync<true><<<nb, 128, 0, g->stream>>>(Dv, out, out2);
+  else k_deref_sync<false><<<nb, 128, 0, g->stream>>>(Dv, out, out2);
+}
+
+void launch_deref_project(hamr_grid* g, const Dev& Dv, const Fields& s, const Fields& s2) {
+  if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
+  Launch l_(g, K_OTHER);
+  const unsigned nb = nblocks_for(Dv, Dv.L.n[0], Dv.L.n[1]);
+  if (Dv.B.nblk > 0) k_deref_project<true><<<nb, 128, 0, g->stream>>>(Dv, s, s2);
+  else k_deref_project<false><<<nb, 128, 0, g->stream>>>(Dv, s, s2);
+}
+
+}  // namespace hamr

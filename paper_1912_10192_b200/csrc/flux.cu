@@ -374,7 +374,9 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
     PL[v] = __shfl_up_sync(FULL, aR, 1);  // right edge of zone k-1 = left state of face k-1/2
   }
   double ctop = 0.0;
-  if (valid && lane >= HLO && lane < 32 - HHI && k >= 0 && k <= L.n[2]) {
+  // C-15: the x3-faces of a phi-derefined row are computed by k_deref_x3 with a strided stencil
+  const bool fine_row = Dv.mrow == nullptr || __ldg(Dv.mrow + C.J0 + j + NG) == 1;
+  if (valid && fine_row && lane >= HLO && lane < 32 - HHI && k >= 0 && k <= L.n[2]) {
     const int ge2 = BLK ? Dv.B.ge2 : L.e2;
     const FGeo G = load_fgeo<D>(Dv.gc + (BLK ? C.lev * Dv.B.tlev : 0), L.n2d, C.q0 + i * ge2 + j);
     PL[7] = PR[7] = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z] * G.igdet;
@@ -382,6 +384,79 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
     if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct;
   }
   if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
+}
+
+// ---- C-15 (ii): x3-faces of phi-derefined rows -----------------------------------------------------------
+// "PPM ... modified for the increased cell spacing".  In a row with factor m the flux exists on
+// group-boundary faces only (k a multiple of m); its stencil takes one value per group, zones k + t m,
+// t = -3..2, wrapped periodically (the grid or block spans all of x3); the Courant limit uses m dx3.
+// One thread per group-boundary face; rows with m = 1 return at once.
+template <int RECON, bool BLK>
+__global__ void __launch_bounds__(128) k_deref_x3(Dev Dv, Fields s, Fields s2, int want_ctop) {
+  constexpr int D = 2;
+  const Lay& L = Dv.L;
+  const int ck = L.n[2] + 1, cj = L.n[1] + 2;
+  const unsigned per = (unsigned)(L.n[0] + 2) * cj * ck;
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = t < (BLK ? per * Dv.B.nact : per);
+  if (!valid) t = 0;
+  int bslot = 0;
+  if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
+  const BCtx C = blk_ctx<BLK>(Dv, bslot);
+  const unsigned tj = t / (unsigned)ck, ti = tj / (unsigned)cj;
+  const int k = (int)(t - tj * ck), j = (int)(tj - ti * cj) - 1, i = (int)ti - 1;
+  const int m = __ldg(Dv.mrow + C.J0 + j + NG);
+  double ctop = 0.0;
+  if (valid && m > 1 && k % m == 0) {
+    const int n3 = L.n[2];
+    const int zrow = C.zoff + (int)L.idx(i, j, 0);
+    const double* var[7] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
+                            selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),
+                            selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[0], s2.Bc[0], C.cur),
+                            selp<BLK>(s.Bc[1], s2.Bc[1], C.cur)};
+    int kk[6];
+#pragma unroll
+    for (int q = 0; q < 6; q++) {
+      int w = (k + (q - 3) * m) % n3;
+      kk[q] = w < 0 ? w + n3 : w;
+    }
+    double PL[8], PR[8];
+#pragma unroll
+    for (int v = 0; v < 7; v++) {
+      const double* a = var[v] + zrow;
+      const double a0 = a[kk[0]], a1 = a[kk[1]], a2 = a[kk[2]], a3 = a[kk[3]], a4 = a[kk[4]], a5 = a[kk[5]];
+      double dum;
+      if (RECON == HAMR_RECON_PPM) {
+        ppm_edges(a0, a1, a2, a3, a4, dum, PL[v]);   // left of the face: a_R of group k/m - 1
+        ppm_edges(a1, a2, a3, a4, a5, PR[v], dum);   // right of the face: a_L of group k/m
+      } else {
+        plm_edges(a1, a2, a3, dum, PL[v]);
+        plm_edges(a2, a3, a4, PR[v], dum);
+      }
+    }
+    const int ge2 = BLK ? Dv.B.ge2 : L.e2;
+    const FGeo G = load_fgeo<D>(Dv.gc + (BLK ? C.lev * Dv.B.tlev : 0), L.n2d, C.q0 + i * ge2 + j);
+    const int z = zrow + k;
+    PL[7] = PR[7] = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z] * G.igdet;
+    const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
+    if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct / (double)m;
+  }
+  if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
+}
+
+void launch_deref_x3(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
+  if (!Dv.mrow) return;
+  const Lay& L = Dv.L;
+  const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
+  if (blk && Dv.B.nact == 0) return;
+  const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 1) * (blk ? Dv.B.nact : 1);
+  const unsigned nb = (unsigned)((tot + 127) / 128);
+  const int wc = want_ctop ? 1 : 0;
+  Launch l_(g, K_FLUX3);
+  if (ppm && !blk) k_deref_x3<HAMR_RECON_PPM, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+  else if (ppm) k_deref_x3<HAMR_RECON_PPM, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+  else if (!blk) k_deref_x3<HAMR_RECON_PLM_MC, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+  else k_deref_x3<HAMR_RECON_PLM_MC, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
 }
 
 // picks the number of faces per marching segment so that the grid fills whole waves of resident
@@ -448,12 +523,18 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
   const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 1 + halo) * (blk ? Dv.B.nact : 1);
   const long long warps = (tot + own - 1) / own + 1;
   const unsigned nb = (unsigned)((warps + 3) / 4);
-  Launch l_(g, K_FLUX3);
   const int wc = want_ctop ? 1 : 0;
-  if (ppm && !blk) k_flux_x3<HAMR_RECON_PPM, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
-  else if (ppm) k_flux_x3<HAMR_RECON_PPM, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
-  else if (!blk) k_flux_x3<HAMR_RECON_PLM_MC, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
-  else k_flux_x3<HAMR_RECON_PLM_MC, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+  {
+    Launch l_(g, K_FLUX3);
+    if (ppm && !blk) k_flux_x3<HAMR_RECON_PPM, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (ppm) k_flux_x3<HAMR_RECON_PPM, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (!blk) k_flux_x3<HAMR_RECON_PLM_MC, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else k_flux_x3<HAMR_RECON_PLM_MC, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+  }
+  if (Dv.mrow) {  // C-15: strided x3 fluxes of the derefined rows, then the group structure on all face values
+    launch_deref_x3(g, Dv, src, src2, want_ctop);
+    launch_deref_fix_flux(g, Dv);
+  }
 }
 
 void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop) { launch_flux_on(g, g->D, src, src, want_ctop); }

@@ -62,6 +62,7 @@ struct Dev {                 // everything a kernel may need, passed by value
   double* EfB[3];            // on d-faces: E_f
   double* Ee[3];             // edge EMFs (C-9)
   double* Cc[3];             // centre EMFs (C-8)
+  const int* mrow;           // phi-derefinement factor per global x2 row incl. ghosts (C-15); NULL: none
   double* scal;              // [NSCAL]
   unsigned long long* cnt;   // [NCNT]
 };
@@ -191,6 +192,13 @@ void launch_zero_ctop(hamr_grid* g);
 void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop);
 void launch_ct_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2);
 void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles& rb, double dtfac, bool same);
+// deref.cu / flux.cu: phi-derefinement (C-15)
+void launch_deref_x3(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop);
+void launch_deref_fix_flux(hamr_grid* g, const Dev& Dv);
+void launch_deref_fix_edges(hamr_grid* g, const Dev& Dv);
+void launch_deref_sync(hamr_grid* g, const Dev& Dv, const Fields& out, const Fields& out2);
+void launch_deref_project(hamr_grid* g, const Dev& Dv, const Fields& s, const Fields& s2);
+int deref_row_factor(const hamr_params& p, long long J);
 void launch_geometry_tab(hamr_grid* g, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
                          double* gf2, double* dgc, double* rho_fl, double* u_fl);
 

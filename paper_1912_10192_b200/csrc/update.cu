@@ -76,11 +76,20 @@ __global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra,
       {
         const double h0 = bf_new<0>(Dv, base.Bf[0], z + S[0], dt, S, idx);
         const double h1 = (ks && Jg + 1 == n2g) ? 0.0 : bf_new<1>(Dv, base.Bf[1], z + S[1], dt, S, idx);
-        const double h2 = bf_new<2>(Dv, base.Bf[2], z + S[2], dt, S, idx);
+        double h2 = bf_new<2>(Dv, base.Bf[2], z + S[2], dt, S, idx), l2 = lo[2];
+        if (Dv.mrow) {
+          // C-15: in a phi-derefined row B_c^3 is the GROUP's value, from the group's two outer x3-faces
+          const int m = __ldg(Dv.mrow + Jg + NG);
+          if (m > 1) {
+            const long long zg = z - (k % m);
+            l2 = bf_new<2>(Dv, base.Bf[2], zg, dt, S, idx);
+            h2 = bf_new<2>(Dv, base.Bf[2], zg + m, dt, S, idx);
+          }
+        }
         const double i2g = 1.0 / (2.0 * G.gdet);
         Bn[0] = (lo[0] + h0) * i2g;
         Bn[1] = (lo[1] + h1) * i2g;
-        Bn[2] = (lo[2] + h2) * i2g;
+        Bn[2] = (l2 + h2) * i2g;
       }
       double Ps[8], U[5], Ssrc1, Ssrc2;
 #pragma unroll
