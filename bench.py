@@ -3,7 +3,7 @@
 fraction of the dominant kernel, the end-to-end number through the C-ABI with host buffers, and the
 CPU oracle timed beside it.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg3]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg4b]
 
 A "step" is one full pass of the hot path over the whole grid: hamr_step(1) = predictor + corrector
 = one zone-cycle per zone.  Default workload: BASELINE.json configs[2], the 256x128x128
@@ -42,6 +42,13 @@ def workload(name):
     if name == "cfg1":
         p = I.minkowski_params(n=(128, 128, 128))
         return p, (lambda: I.minkowski_waves(p, seed=1)), "BASELINE cfg1: Minkowski periodic 128^3 linear waves"
+    if name == "cfg4b":
+        # the part of BASELINE cfg 4 that is built: cfg 2's torus (seed 4) on 16 x 16 x 128
+        # blocks, phi-derefined by 2 / 4 within 15 / 5 degrees of the poles, LAT levels 1, 2, 4; no r-refinement
+        p = I.torus_params(n=(256, 128, 128), r_out=1000.0, nb=(16, 16, 128), lat_max_level=2,
+                           deref_theta_deg=(15.0, 5.0), deref_factor=(2, 4))
+        return p, (lambda: I.fm_torus(p, seed=4)), ("BASELINE cfg4 without r-refinement: Kerr FM torus 256x128x128 in 16x16x128 "
+                                                     "blocks, phi-derefinement 2x/4x, LAT levels 1/2/4")
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -114,6 +121,13 @@ ALG_DOUBLES = {"flux_x1": 16, "flux_x2": 16, "flux_x3": 16,   # 9 r (P5, 2 trans
                "centre_emf": 6 + 3, "edge_emf": 6 + 3 + 3 + 3, "ghosts": 0, "dt": 0, "other": 0}
 
 
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel class from the round's
+# `ncu --set full` capture of this same command on cfg 2 (profiles/r1c_ncu_full_cfg2.md)
+NCU_TRAFFIC_SOURCE = "profiles/r1c_ncu_full_cfg2.md"
+NCU_TRAFFIC = {"flux_x1": 612235336, "flux_x2": 594134716, "flux_x3": 537716000, "centre_emf": 318640136, "edge_emf": 535194424, "update_predictor": 1382105232, "update_corrector": 1657781416, "ghosts": 139616240}
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+
 def units_per_launch(cls, n):
     n1, n2, n3 = n
     if cls == "flux_x1":
@@ -140,7 +154,7 @@ def cpu_oracle_time(p, gen, steps):
     dt = time.perf_counter() - t0
     cores = int(_orc.lib().orc_omp_threads())
     o.close()
-    nz = int(np.prod(p["n"]))
+    nz = int(np.prod(p["n"])) * 2 ** int(p["lat_max_level"])   # effective zone-cycles per (coarse) step
     return nz * steps / dt, dt, cores
 
 
@@ -162,7 +176,7 @@ def run_reference(args):
         o.step(1)
     dt = time.perf_counter() - t0
     cores = int(_orc.lib().orc_omp_threads())
-    nz = int(np.prod(p["n"]))
+    nz = int(np.prod(p["n"])) * 2 ** int(p["lat_max_level"])
     val = nz * args.steps / dt
     sample = f"{args.steps} full oracle steps of the whole {p['n'][0]}x{p['n'][1]}x{p['n'][2]} grid per timed step"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
@@ -213,6 +227,8 @@ def main():
     p, gen, desc = workload(args.workload)
     n = tuple(p["n"])
     nz = int(np.prod(n))
+    blocky = any(p["nb"]) or p["lat_max_level"] > 0
+    fin = 2 ** int(p["lat_max_level"])        # finest steps per hamr_step on a LAT grid
     hyd, bf = gen()
     g = hamr.Grid(p, torch_arena=True)        # device memory and stream from torch; all math in libhamr
     hd = [torch.from_numpy(np.ascontiguousarray(h)).cuda() for h in hyd]
@@ -249,7 +265,12 @@ def main():
     if world > 1:
         dist.all_reduce(tms, op=dist.ReduceOp.MAX)
     ms_max = float(tms.item())
-    value = world * nz * args.steps / (ms_max * 1e-3)
+    # LAT: "effective" zone-cycles (zones x finest-level steps, the paper's convention)
+    value = world * nz * fin * args.steps / (ms_max * 1e-3)
+    performed = None
+    if blocky:
+        lv = np.array(g.levels())
+        performed = world * nz * float(np.mean(fin / 2.0 ** lv)) * args.steps / (ms_max * 1e-3)
 
     # ---- end to end through the C-ABI with HOST buffers (pinned): set_prims + step + get_prims -----
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
@@ -279,7 +300,7 @@ def main():
     tms = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    e2e_val = world * nz * args.e2e_steps / (float(tms.item()) * 1e-3)
+    e2e_val = world * nz * fin * args.e2e_steps / (float(tms.item()) * 1e-3)
     h2d = sum(a.nbytes for a in hh) + sum(a.nbytes for a in bh)
     d2h = sum(a.nbytes for a in outs)
 
@@ -293,16 +314,20 @@ def main():
     kern = {k: {"ms_total": v[0], "launches": v[1], "ms_avg": v[0] / v[1] if v[1] else 0.0,
                 "share": v[0] / ms if ms else 0.0} for k, v in prof.items() if v[1]}
     for k, d in kern.items():
-        by = ALG_DOUBLES.get(k, 0) * 8 * units_per_launch(k, n)
+        # per-launch algorithmic bytes are defined for the monolithic launch shape only
+        by = 0 if blocky else ALG_DOUBLES.get(k, 0) * 8 * units_per_launch(k, n)
         d["alg_bytes"] = by
         d["gbs"] = by / (d["ms_avg"] * 1e-3) / 1e9 if d["ms_avg"] > 0 else 0.0
     dom = max(kern, key=lambda k: kern[k]["ms_total"])
     roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": hbm_peak, "unit": "GB/s",
-            "frac": kern[dom]["gbs"] / hbm_peak, "traffic": None, "peak_source": peak_src,
+            "frac": kern[dom]["gbs"] / hbm_peak, "traffic": NCU_TRAFFIC.get(dom) if args.workload == "cfg2" else None,
+            "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": peak_src,
+            "fp64_pipe": {"peak_tflops_derived": FP64_PEAK_TFLOPS, "note": "148 SMs x 64 DFMA lanes x 2 x 1.965 GHz; "
+                          "per-kernel FP64 pipe utilisation from ncu is in profiles/ (DESIGN.md section 7)"},
             "share_of_step": kern[dom]["share"],
             "whole_step": {"alg_bytes_per_zone_cycle_floor": 440,
                            "frac_of_hbm_at_floor": 440.0 * value / world / 1e9 / hbm_peak,
-                           "alg_bytes_per_zone_cycle_pipeline": sum(d["alg_bytes"] * d["launches"] for d in kern.values()) / (nz * args.steps),
+                           "alg_bytes_per_zone_cycle_pipeline": sum(d["alg_bytes"] * d["launches"] for d in kern.values()) / (nz * fin * args.steps),
                            "frac_of_hbm_pipeline": sum(d["alg_bytes"] * d["launches"] for d in kern.values()) / (ms * 1e-3) / 1e9 / hbm_peak},
             "kernels": {k: {"ms_avg": round(d["ms_avg"], 4), "share": round(d["share"], 4),
                             "gbs": round(d["gbs"], 1), "launches": d["launches"]} for k, d in kern.items()}}
@@ -310,7 +335,7 @@ def main():
     cpu = None
     if not args.no_cpu_baseline:
         subprocess.check_call(["make", "-s", "-C", os.path.join(ROOT, "oracle")])
-        steps_cpu = 3 if args.workload == "cfg2" else 2
+        steps_cpu = 3 if args.workload == "cfg2" else (1 if args.workload == "cfg4b" else 2)
         v, secs, cores = cpu_oracle_time(p, gen, steps_cpu)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"{steps_cpu} full steps of the same {n[0]}x{n[1]}x{n[2]} workload ({secs:.1f} s)"}
@@ -318,7 +343,9 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": desc, "zones": nz, "parallelism": "replicas only" if world > 1 else "1 GPU",
+            "config": {"workload": desc, "zones": nz, "blocks": g.num_blocks(), "finest_steps_per_step": fin,
+                       "performed_zone_updates_per_sec": performed,
+                       "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs (2.4 GB state) larger than L2; no flush needed", "timing": "CUDA events on the launching (torch current) stream"},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
