@@ -354,6 +354,7 @@ int orc_force_levels(void* h, const int* tau) {
 int orc_blocks_commit(void* h) {
   Grid& g = *(Grid*)h;
   if (!g.multi) return 1;
+  for (Block& b : g.blocks) deref_project(g.par, b, b.sn);
   blocks_initial_dt(g);
   g.t = 0.0;
   g.have_state = true;

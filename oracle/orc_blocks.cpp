@@ -32,9 +32,10 @@ void blocks_build(Grid& g) {
   bool seen_coarse = false;
   for (int col = 0; col < NB[0]; col++) {
     bool refined = false;
-    if (par.r_refine_max > 0.0 && par.metric == 1) {
+    if (par.r_refine_max > 0.0) {
+      // centre of the column: r on the Kerr-Schild map, x1 itself on the Cartesian map
       const double xc = lo[0] + ((double)col + 0.5) * nb[0] * dx0[0];
-      refined = std::exp(xc) < par.r_refine_max;
+      refined = (par.metric == 1 ? std::exp(xc) : xc) < par.r_refine_max;
     }
     if (refined && seen_coarse) throw std::runtime_error("refined columns must be contiguous from r_in");
     if (refined) { slots.push_back({col, 1, 0}); slots.push_back({col, 1, 1}); }
@@ -168,12 +169,131 @@ static void exchange_block(Grid& g, Block& b, Fields& dst, long long s_u) {
       }
 }
 
+// ---- ghost exchange across the x1 refinement interface (C-16) ------------------------------------------------
+// A refined block has dx1/2 and unchanged dx2, dx3, so only the x1 index changes meaning across the
+// interface.  kind: 0..4 hydro primitive, 5 + d the d-face field.  All reads go through sample().
+static double sample_kind(const Block& q, int kind, int i, int j, int k, long long s_u) {
+  const size_t z = q.idx(i, j, k);
+  if (kind < 5) return sample(q, q.sn.P[kind], q.sh.P[kind], q.snew.P[kind], z, s_u);
+  const int d = kind - 5;
+  return sample(q, q.sn.Bf[d], q.sh.Bf[d], q.snew.Bf[d], z, s_u);
+}
+
+// C-16 restriction: coarse value = arithmetic mean of the two fine values it covers (primitives and
+// densitised transverse faces alike)
+static double restrict2(const Block& qf, int kind, int i0, int j, int k, long long s_u) {
+  return 0.5 * (sample_kind(qf, kind, i0, j, k, s_u) + sample_kind(qf, kind, i0 + 1, j, k, s_u));
+}
+
+static void exchange_refined(Grid& g, Block& b, Fields& dst, long long s_u) {
+  for (int side = 0; side < 2; side++) {
+    const int o0 = side ? 1 : -1;
+    for (int o1 = -1; o1 <= 1; o1++)
+      for (int o2 = -1; o2 <= 1; o2++) {
+        const int qi = b.nbr[o0 + 1][o1 + 1][o2 + 1];
+        if (qi < 0 || g.blocks[qi].lev1 == b.lev1) continue;
+        const Block& q = g.blocks[qi];
+        // the block on b's own side of the interface in the same transverse position (b itself for
+        // o1 = o2 = 0): it covers the zones just outside q
+        const int ri = b.nbr[1][o1 + 1][o2 + 1];
+        const Block& r = g.blocks[ri];
+        const int n0 = b.n[0];
+        // ranges of the padded indices that fall into q
+        auto range = [&](int o, int n, int& lo, int& hi, bool face) {
+          if (o < 0) { lo = -NG; hi = -1; }
+          else if (o > 0) { lo = face ? n + 1 : n; hi = face ? n + NG : n + NG - 1; }
+          else { lo = 0; hi = face ? n : n - 1; }
+        };
+        for (int kind = 0; kind < 8; kind++) {
+          if (kind > 0 && kind < 5) continue;          // the five hydro variables share kind 0's geometry
+          const int fd = kind >= 5 ? kind - 5 : -1;    // face direction
+          int lo[3], hi[3];
+          range(o0, b.n[0], lo[0], hi[0], fd == 0);
+          range(o1, b.n[1], lo[1], hi[1], fd == 1);
+          range(o2, b.n[2], lo[2], hi[2], fd == 2);
+          for (int i = lo[0]; i <= hi[0]; i++)
+            for (int j = lo[1]; j <= hi[1]; j++)
+              for (int k = lo[2]; k <= hi[2]; k++) {
+                const int lj = j - o1 * b.n[1], lk = k - o2 * b.n[2];
+                const int nk = kind == 0 ? 5 : 1;
+                for (int c = 0; c < nk; c++) {
+                  const int kd = kind == 0 ? c : kind;
+                  double v;
+                  if (b.lev1 == 0) {
+                    // ---- coarse ghost from fine data
+                    if (fd == 0) {               // normal face: coincident fine face, copied
+                      const int t = side ? i - n0 : -i;            // 1..3 coarse faces from the interface
+                      v = sample_kind(q, kd, side ? 2 * t : n0 - 2 * t, lj, lk, s_u);
+                    } else {                     // zones and transverse faces: mean of the two fine ones
+                      const int t = side ? i - n0 : -1 - i;        // 0..2 coarse zones from the interface
+                      v = restrict2(q, kd, side ? 2 * t : n0 - 2 * t - 2, lj, lk, s_u);
+                    }
+                  } else {
+                    // ---- fine ghost from coarse data
+                    if (fd == 0) {
+                      // normal faces: coincident ones copied, in-between ones the mean of their neighbours
+                      const int t = side ? i - n0 : -i;            // 1..3 fine faces from the interface
+                      const int c0 = side ? t / 2 : n0 - t / 2;    // coarse face at or just inside
+                      if (t % 2 == 0) v = sample_kind(q, kd, c0, lj, lk, s_u);
+                      else v = 0.5 * (sample_kind(q, kd, c0, lj, lk, s_u) +
+                                      sample_kind(q, kd, side ? c0 + 1 : c0 - 1, lj, lk, s_u));
+                    } else {
+                      // zones and transverse faces: piecewise linear in x1 with the MC-limited slope,
+                      // evaluated a quarter of a coarse zone off the coarse centre
+                      const int t = side ? i - n0 : -1 - i;        // 0..2 fine zones from the interface
+                      const int ic = side ? t / 2 : n0 - 1 - t / 2;
+                      const bool high_half = side ? (t % 2 == 1) : (t % 2 == 0);
+                      double a3[3];
+                      for (int w = -1; w <= 1; w++) {
+                        const int iw = ic + w;
+                        if (iw >= 0 && iw < n0) a3[w + 1] = sample_kind(q, kd, iw, lj, lk, s_u);
+                        else a3[w + 1] = restrict2(r, kd, side ? n0 - 2 : 0, lj, lk, s_u);  // covered by fine zones
+                      }
+                      double aL, aR;
+                      plm_zone(a3, aL, aR);
+                      v = 0.5 * (a3[1] + (high_half ? aR : aL));
+                    }
+                  }
+                  if (kind == 0) dst.P[c][b.idx(i, j, k)] = v;
+                  else dst.Bf[fd][b.idx(i, j, k)] = v;
+                }
+              }
+        }
+      }
+  }
+}
+
+// C-16: where a coarse and a fine block on the same time level share the x1 interface, the fine block's
+// F^1 and the edge EMFs E_2, E_3 lying in the interface plane are authoritative: the coarse block
+// overwrites its own with them before its update (equal face areas and edge lengths: plain copies).
+static void interface_agreement(Grid& g, int tau) {
+  for (Block& c : g.blocks) {
+    if (c.tau != tau || c.lev1 != 0) continue;
+    for (int side = 0; side < 2; side++) {
+      const int qi = c.nbr[side ? 2 : 0][1][1];
+      if (qi < 0) continue;
+      const Block& q = g.blocks[qi];
+      if (q.lev1 == c.lev1 || q.tau != c.tau) continue;
+      const int ic = side ? c.n[0] : 0, iq = side ? 0 : q.n[0];
+      for (int j = 0; j <= c.n[1]; j++)
+        for (int k = 0; k <= c.n[2]; k++) {
+          const size_t zc = c.idx(ic, j, k), zq = q.idx(iq, j, k);
+          if (j < c.n[1] && k < c.n[2])
+            for (int cc = 0; cc < 5; cc++) c.F[0][cc][zc] = q.F[0][cc][zq];
+          if (j < c.n[1]) c.Ee[1][zc] = q.Ee[1][zq];   // E2 on edges along x2 at (i-1/2, k-1/2)
+          if (k < c.n[2]) c.Ee[2][zc] = q.Ee[2][zq];   // E3 on edges along x3 at (i-1/2, j-1/2)
+        }
+    }
+  }
+}
+
 // ---- one stage of C-12 on every block of one time level ------------------------------------------------
 static void stage_level(Grid& g, int tau, bool corrector) {
   for (Block& b : g.blocks) {
     if (b.tau != tau) continue;
     Fields& src = corrector ? b.sh : b.sn;
     exchange_block(g, b, src, b.tb_u + (corrector ? b.dt_u / 2 : 0));
+    exchange_refined(g, b, src, b.tb_u + (corrector ? b.dt_u / 2 : 0));
     fill_physical_bc(g.par, b, src);
     compute_Bc(b, src, false);
   }
@@ -184,6 +304,11 @@ static void stage_level(Grid& g, int tau, bool corrector) {
     deref_fix_fluxes(g.par, b);
     ct_edges(g.par, b, src);
     deref_fix_edges(g.par, b);
+  }
+  interface_agreement(g, tau);
+  for (Block& b : g.blocks) {
+    if (b.tau != tau) continue;
+    Fields& src = corrector ? b.sh : b.sn;
     const double dtb = g.dt * (double)(b.dt_u / 2);      // dt_b = 2^tau dt_0
     if (corrector) {
       // C-17 registers: R1 = dt_b * (F, E) of this corrector; R2 accumulates the two steps that
@@ -439,6 +564,7 @@ void blocks_initial_dt(Grid& g) {
   for (Block& b : g.blocks) { b.tau = 0; b.tb_u = 0; b.dt_u = 2; b.has_new = false; }
   for (Block& b : g.blocks) {
     exchange_block(g, b, b.sn, 0);
+    exchange_refined(g, b, b.sn, 0);
     fill_physical_bc(g.par, b, b.sn);
     compute_Bc(b, b.sn, false);
   }

@@ -169,8 +169,11 @@ def grid_coords(p: dict):
 
 
 def fm_torus(p: dict, seed: int = 0, pert: float = 0.02, beta: float = 100.0, with_B: bool = True,
-             r_in: float = 6.0, r_max: float = 12.0):
-    """BASELINE.json cfg 0 / cfg 2 initial data.  Returns (hydro[5], bface[3])."""
+             r_in: float = 6.0, r_max: float = 12.0, bfac=None, zidx=None, ret_bfac: bool = False):
+    """BASELINE.json cfg 0 / cfg 2 initial data.  Returns (hydro[5], bface[3]).
+    bfac: field normalisation to use instead of the grid's own (blocks of one grid share the base
+    grid's); zidx: zone indices keying the pressure perturbation (default: this grid's own);
+    ret_bfac: also return the normalisation."""
     a, gam = p["a"], p["gamma_ad"]
     n = p["n"]
     xc, xf, dx = grid_coords(p)
@@ -212,13 +215,53 @@ def fm_torus(p: dict, seed: int = 0, pert: float = 0.02, beta: float = 100.0, wi
         bcon[..., 3] = (bt * ucon[..., 3]) / ucon[..., 0]
         bsq = np.einsum("...m,...mn,...n->...", bcon, g, bcon)
         pmax = ((gam - 1.0) * u).max()
-        if bsq.max() > 0.0:
+        fac = bfac
+        if fac is None and bsq.max() > 0.0:
             fac = np.sqrt(pmax / (0.5 * bsq.max() * beta))
+        if fac is not None:
             bface[0][:] = (fac * B1)[:, :, None]
             bface[1][:] = (fac * B2)[:, :, None]
+        bfac = fac
     if pert != 0.0:
-        hyd[1] = hyd[1] * (1.0 + pert * rand_pm1(seed, zone_index(n)))
+        hyd[1] = hyd[1] * (1.0 + pert * rand_pm1(seed, zone_index(n) if zidx is None else zidx))
+    if ret_bfac:
+        return hyd, bface, bfac
     return hyd, bface
+
+
+def block_as_grid(p: dict, x_lo, dx, n) -> dict:
+    """parameter dict describing ONE block (internal-coordinate corner x_lo, spacing dx, n zones) as a
+    grid of its own, for sampling analytic initial data on the blocks of a refined grid"""
+    lo = np.array(x_lo, dtype=np.float64)
+    hi = lo + np.array(dx, dtype=np.float64) * np.array(n, dtype=np.float64)
+    if p["metric"] == METRIC_KS:
+        lo[0], hi[0] = np.exp(lo[0]), np.exp(hi[0])
+    return dict(p, n=tuple(int(v) for v in n), xmin=tuple(lo), xmax=tuple(hi), nb=(0, 0, 0),
+                r_refine_max=0.0, lat_max_level=0, deref_theta_deg=(), deref_factor=())
+
+
+def base_zone_index(p: dict, x_lo, dx, n) -> np.ndarray:
+    """index of the BASE-grid zone containing each zone of a block (both children of a refined zone share
+    it), for perturbations that must not depend on the decomposition"""
+    xc0, _, dx0 = grid_coords(dict(p, nb=(0, 0, 0)))
+    lo0 = [xc0[d][0] - 0.5 * dx0[d] for d in range(3)]
+    idx = []
+    for d in range(3):
+        xc = np.array(x_lo[d]) + (np.arange(int(n[d])) + 0.5) * dx[d]
+        idx.append(np.floor((xc - lo0[d]) / dx0[d]).astype(np.int64))
+    N = p["n"]
+    return ((idx[0][:, None, None] * N[1] + idx[1][None, :, None]) * N[2] + idx[2][None, None, :]).astype(np.uint64)
+
+
+def fm_torus_blocks(p: dict, infos, seed: int = 0, pert: float = 0.02, beta: float = 100.0):
+    """cfg 4: the torus sampled on every block of a (possibly x1-refined) block grid.  infos: per block
+    (x_lo, dx, n) in internal coordinates.  Field normalisation from the base grid."""
+    _, _, bfac = fm_torus(dict(p, nb=(0, 0, 0), r_refine_max=0.0), seed, pert=0.0, beta=beta, ret_bfac=True)
+    out = []
+    for x_lo, dx, n in infos:
+        pg = block_as_grid(p, x_lo, dx, n)
+        out.append(fm_torus(pg, seed, pert, beta, bfac=bfac, zidx=base_zone_index(p, x_lo, dx, n)))
+    return out
 
 
 # ------------------------------------------------------------------------------------------------
@@ -284,14 +327,15 @@ def flat_eigenmodes(gam=4.0 / 3.0, rho=1.0, u=3.0, B=(1.0, np.sqrt(2.0), 0.5), k
 
 
 def minkowski_waves(p: dict, seed: int = 1, amp: float = 1e-6, noise: float = 1e-8,
-                    modes=("fast", "alfven"), t: float = 0.0, B0=(1.0, np.sqrt(2.0), 0.5)):
+                    modes=("fast", "alfven"), t: float = 0.0, B0=(1.0, np.sqrt(2.0), 0.5), box=None):
     """cfg 1: background rho=1, p=1, B0, superposed eigenmodes cos(k.x - omega t), k = 2 pi (1,1,1)
     on the unit cube; face B from an edge vector potential (discretely divergence-free); density
     white noise `noise` from `seed`.  `t` translates the modes (the exact linear solution, P11)."""
     gam = p["gamma_ad"]
     n = p["n"]
     xc, xf, dx = grid_coords(p)
-    L = np.array(p["xmax"]) - np.array(p["xmin"])
+    # box: extent of the periodic box when p describes only a block of it (block_as_grid)
+    L = np.array(p["xmax"]) - np.array(p["xmin"]) if box is None else np.array(box, dtype=np.float64)
     k = 2.0 * np.pi / L
     kmag = np.linalg.norm(k)
     u0 = 1.0 / (gam - 1.0)
@@ -318,10 +362,10 @@ def minkowski_waves(p: dict, seed: int = 1, amp: float = 1e-6, noise: float = 1e
         bface[0] = bface[0] + (A3[:, 1:, :] - A3[:, :-1, :]) / dx[1] - (A2[:, :, 1:] - A2[:, :, :-1]) / dx[2]
         bface[1] = bface[1] + (A1[:, :, 1:] - A1[:, :, :-1]) / dx[2] - (A3[1:, :, :] - A3[:-1, :, :]) / dx[0]
         bface[2] = bface[2] + (A2[1:, :, :] - A2[:-1, :, :]) / dx[0] - (A1[:, 1:, :] - A1[:, :-1, :]) / dx[1]
-    # periodic images must be bitwise identical
-    bface[0][-1] = bface[0][0]
-    bface[1][:, -1] = bface[1][:, 0]
-    bface[2][:, :, -1] = bface[2][:, :, 0]
+    if box is None:   # periodic images must be bitwise identical
+        bface[0][-1] = bface[0][0]
+        bface[1][:, -1] = bface[1][:, 0]
+        bface[2][:, :, -1] = bface[2][:, :, 0]
     if noise != 0.0:
         hyd[0] = hyd[0] * (1.0 + noise * rand_pm1(seed, zone_index(n)))
     return hyd, bface
