@@ -128,6 +128,20 @@ int hamr_num_blocks(const hamr_grid* g);
 /* x_lo: internal coordinates of the block's low corner; time_level: its current LAT level tau */
 int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int n[3],
                     int* time_level);
+/* One x1 refinement level (PAPER.md:71 per-dimension refinement; C-16): with r_refine_max > 0 every
+ * block column whose x1-centre has r < r_refine_max (x1 < r_refine_max on the Cartesian map) is replaced by
+ * two blocks of nb zones with dx1 / 2; such columns must be contiguous from the low x1 side and nb[0] >= 6.
+ * Ghost zones across the coarse/fine interface are restricted (mean of the two fine values) or prolonged
+ * (piecewise linear in x1, MC-limited); the coarse block takes the fine block's interface fluxes and EMFs.
+ * A refined grid has no global zone array: its state is set and read block by block.  Arrays are dense,
+ * block-local, x3 fastest: hydro[c] nb0*nb1*nb2, bface[d] with nb[d]+1 along d (NULL = 0); the caller keeps
+ * them.  After the last hamr_set_block_prims, hamr_blocks_commit fills ghosts, projects onto the
+ * derefinement invariant, and finds the first dt and time levels (HAMR_ENONFINITE on NaN/Inf input).
+ * Also valid on unrefined block grids. */
+int hamr_set_block_prims(hamr_grid* g, int b, const double* const hydro[5], const double* const bface[3]);
+int hamr_blocks_commit(hamr_grid* g);
+int hamr_get_block_prims(hamr_grid* g, int b, double* const prims[8]);   /* 5 hydro + cell-centred B^i */
+int hamr_get_block_bface(hamr_grid* g, int b, double* const bface[3]);
 /* Test hook: prescribes the LAT level of every block (tau[hamr_num_blocks], clamped to
  * 0..lat_max_level, then lowered until neighbours differ by at most one); NULL restores the
  * Courant-based choice.  Takes effect at the next hamr_set_prims / coarse step.  The caller keeps tau. */

@@ -38,6 +38,8 @@ void blocks_build(Grid& g) {
       refined = (par.metric == 1 ? std::exp(xc) : xc) < par.r_refine_max;
     }
     if (refined && seen_coarse) throw std::runtime_error("refined columns must be contiguous from r_in");
+    // a coarse ghost layer of NG zones is the restriction of 2 NG fine zones of ONE neighbour
+    if (refined && nb[0] < 2 * NG) throw std::runtime_error("x1 refinement needs nb[0] >= 6");
     if (refined) { slots.push_back({col, 1, 0}); slots.push_back({col, 1, 1}); }
     else { slots.push_back({col, 0, 0}); seen_coarse = true; }
   }

@@ -17,6 +17,7 @@ constexpr int N_STATE_ARR = 11, N_ARR = 3 * N_STATE_ARR + 15 + 3 + 3 + 3 + 3;
 constexpr int N_REG_ARR = 15 + 3;  // LAT flux / EMF registers (C-17)
 
 bool is_block_grid(const hamr_params& p) { return p.nb[0] > 0 || p.nb[1] > 0 || p.nb[2] > 0 || p.lat_max_level > 0; }
+bool params_ok(const hamr_params& p, std::string& why);
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -35,10 +36,7 @@ bool params_ok(const hamr_params& p, std::string& why) {
   if (p.recon != HAMR_RECON_PPM && p.recon != HAMR_RECON_PLM_MC) { why = "bad recon"; return false; }
   if (p.metric == HAMR_METRIC_KERR_SCHILD && !(p.xmin[0] > 0.0)) { why = "r_in <= 0"; return false; }
   if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0) || !(p.gamma_max > 1.0)) { why = "gamma_ad / cour / gamma_max"; return false; }
-  if (p.r_refine_max > 0.0) {
-    why = "r-refinement is not available in this build (DESIGN.md section 9)";
-    return false;
-  }
+  if (p.r_refine_max > 0.0 && !is_block_grid(p)) { why = "x1 refinement needs a block grid (nb)"; return false; }
   if (p.n_deref < 0 || p.n_deref > 4) { why = "n_deref must be 0..4"; return false; }
   if (p.n_deref > 0) {
     // C-15: the strided x3 stencil of a derefined row wraps inside the grid / block
@@ -64,6 +62,7 @@ struct GridShape {
   int nblk;        // 0: monolithic
   int blen;        // doubles per block per array
   int te1, te2;    // extents of the geometry tables
+  int nlev;        // x1 refinement levels carrying a table set (1 or 2, C-16)
   int narr;        // fp64 arrays of Lay::len doubles
 };
 
@@ -81,7 +80,8 @@ bool make_layout(const hamr_params& p, Lay& L, GridShape& G) {
   L.len = blen * (G.nblk > 0 ? G.nblk : 1);
   if (L.len >= (1LL << 31)) return false;   // kernels index one array with 32-bit offsets
   G.blen = (int)blen;
-  G.te1 = p.n[0] + 2 * NG + 1;
+  G.nlev = (G.nblk > 0 && blk_has_refinement(p)) ? 2 : 1;
+  G.te1 = G.nlev * p.n[0] + 2 * NG + 1;   // the level-1 table is indexed in fine zones
   G.te2 = p.n[1] + 2 * NG + 1;
   L.n2d = G.te1 * G.te2;
   G.narr = N_ARR + ((G.nblk > 0 && p.lat_max_level > 0) ? N_REG_ARR : 0);
@@ -97,7 +97,7 @@ ArenaPlan plan_arena(const hamr_params& p, const Lay& L, const GridShape& G) {
   ArenaPlan a;
   size_t off = 0;
   a.arr = off; off += (size_t)G.narr * L.len * 8;
-  a.tabs = off; off += align_up(((size_t)3 * NGEO + 2 * NDG) * L.n2d * 8 + (size_t)2 * G.te1 * 8, 256);
+  a.tabs = off; off += align_up((size_t)G.nlev * (((size_t)3 * NGEO + 2 * NDG) * L.n2d * 8 + (size_t)2 * G.te1 * 8), 256);
   a.scal = off; off += 256;
   a.cnt = off; off += 256;
   a.stage_doubles = (size_t)8 * (p.n[0] + 1) * (p.n[1] + 1) * (p.n[2] + 1);
@@ -146,6 +146,7 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   g->stream = nullptr;
   g->h_pinned = nullptr;
   g->have_state = false;
+  g->blocks_open = false;
   g->dead = false;
   g->launches = 0;
   g->prof = false;
@@ -210,14 +211,15 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   D.B.blen = gs.blen;
   D.B.ge2 = gs.te2;
   D.B.n2g = p->n[1];
-  D.B.tlev = 0;
-  D.B.flev = 0;
+  // geometry tables: [level][gc | gf1 | gf2 | dgc], then the floor tables [level][rho | u]
+  D.B.tlev = (int)(((size_t)3 * NGEO + 2 * NDG) * D.L.n2d);
+  D.B.flev = 2 * gs.te1;
   double* tabs = (double*)(base + ap.tabs);
   double* gc = tabs;
   double* gf1 = gc + (size_t)NGEO * D.L.n2d;
   double* gf2 = gf1 + (size_t)NGEO * D.L.n2d;
   double* dgc = gf2 + (size_t)NGEO * D.L.n2d;
-  double* rfl = dgc + (size_t)2 * NDG * D.L.n2d;
+  double* rfl = tabs + (size_t)gs.nlev * D.B.tlev;
   double* ufl = rfl + gs.te1;
   D.gc = gc; D.gf1 = gf1; D.gf2 = gf2; D.dgc = dgc; D.rho_fl = rfl; D.u_fl = ufl;
   D.scal = (double*)(base + ap.scal);
@@ -228,6 +230,9 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   e = cudaMemsetAsync(g->arena, 0, ap.total, g->stream);
   if (e == cudaSuccess) {
     launch_geometry_tab(g, gs.te1, gs.te2, D.L.n2d, D.dx[0], p->n[1], gc, gf1, gf2, dgc, rfl, ufl);
+    if (gs.nlev > 1)   // C-16: the refined level's tables, dx1 / 2
+      launch_geometry_tab(g, gs.te1, gs.te2, D.L.n2d, 0.5 * D.dx[0], p->n[1], gc + D.B.tlev, gf1 + D.B.tlev,
+                          gf2 + D.B.tlev, dgc + D.B.tlev, rfl + D.B.flev, ufl + D.B.flev);
     e = cudaGetLastError();
   }
   if (e == cudaSuccess && gs.nblk > 0 && blk_setup(g, base + ap.blk) != HAMR_OK) e = cudaErrorUnknown;
@@ -301,6 +306,7 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
   for (int c = 0; c < 5; c++) if (!hydro[c]) return fail(g, HAMR_EINVAL, "hydro[c] is NULL");
   const bool blk = g->bh.on;
   const int* N = g->par.n;
+  if (blk && g->bh.refined) return fail(g, HAMR_ESTATE, "a grid with x1 refinement is set block by block (hamr_set_block_prims)");
   if (blk) {
     g->isn = 0; g->ish = 1; g->inew = 2;
     CK(cudaMemsetAsync(g->D.B.cur, 0, (size_t)g->bh.nblk * sizeof(int), g->stream));
@@ -359,6 +365,7 @@ int get_dense(hamr_grid* g, const double* padded, double* out, int stag, bool de
   if (stag >= 0) m[stag] += 1;
   const size_t nf = (size_t)m[0] * m[1] * m[2];
   if (g->bh.on && kind < 0) return fail(g, HAMR_ESTATE, "not available on a block-structured grid");
+  if (g->bh.on && g->bh.refined) return fail(g, HAMR_ESTATE, "a grid with x1 refinement is read block by block (hamr_get_block_prims)");
   if (dev) {
     if (g->bh.on) blk_unpack(g, kind, out);
     else launch_unpack(g, padded, out, m);
@@ -535,6 +542,80 @@ int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int
   if (time_level) *time_level = g->bh.on ? g->bh.tau[b] : 0;
   return HAMR_OK;
 }
+
+// ---- block-by-block state access (required on grids with x1 refinement) ---------------------------------
+int hamr_set_block_prims(hamr_grid* g, int b, const double* const hydro[5], const double* const bface[3]) {
+  if (!g || !g->bh.on || b < 0 || b >= g->bh.nblk || !hydro) return HAMR_EINVAL;
+  if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
+  for (int c = 0; c < 5; c++) if (!hydro[c]) return fail(g, HAMR_EINVAL, "hydro[c] is NULL");
+  const Lay& L = g->D.L;
+  if (!g->blocks_open) {   // first block of a new state: every block back to buffer set 0
+    CK(cudaMemsetAsync(g->D.B.cur, 0, (size_t)g->bh.nblk * sizeof(int), g->stream));
+    g->blocks_open = true;
+    g->have_state = false;
+  }
+  const size_t nz = (size_t)L.n[0] * L.n[1] * L.n[2];
+  size_t off = 0;
+  for (int c = 0; c < 5; c++) {
+    double* st = g->stage + off;
+    CK(cudaMemcpyAsync(st, hydro[c], nz * 8, cudaMemcpyHostToDevice, g->stream));
+    blk_pack_one(g, b, st, c, -1, false);
+    off += nz;
+  }
+  for (int d = 0; d < 3; d++) {
+    int m[3] = {L.n[0], L.n[1], L.n[2]};
+    m[d] += 1;
+    const size_t nf = (size_t)m[0] * m[1] * m[2];
+    const double* src = (bface && bface[d]) ? bface[d] : nullptr;
+    if (src) {
+      double* st = g->stage + off;
+      CK(cudaMemcpyAsync(st, src, nf * 8, cudaMemcpyHostToDevice, g->stream));
+      src = st;
+      off += nf;
+    }
+    blk_pack_one(g, b, src, 5 + d, d, d == 1);
+  }
+  CK(cudaStreamSynchronize(g->stream));   // the staging area is reused by the next call
+  return HAMR_OK;
+}
+
+int hamr_blocks_commit(hamr_grid* g) {
+  if (!g || !g->bh.on) return HAMR_EINVAL;
+  if (!g->blocks_open) return fail(g, HAMR_ESTATE, "hamr_blocks_commit without hamr_set_block_prims");
+  g->blocks_open = false;
+  g->isn = 0; g->ish = 1; g->inew = 2;
+  CK(cudaMemsetAsync(g->D.scal, 0, NSCAL * sizeof(double), g->stream));
+  CK(cudaMemsetAsync(g->D.cnt, 0, NCNT * sizeof(unsigned long long), g->stream));
+  const int rc = blk_initial(g);
+  if (rc != HAMR_OK) return fail(g, rc, "block grid initialisation failed");
+  blk_check_finite(g);
+  g->have_state = true;
+  CK(cudaGetLastError());
+  return check_state(g);
+}
+
+static int get_block(hamr_grid* g, int b, int kind0, int nkind, double* const out[]) {
+  if (!g || !g->bh.on || b < 0 || b >= g->bh.nblk || !out) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  const Lay& L = g->D.L;
+  size_t off = 0;
+  for (int c = 0; c < nkind; c++) {
+    if (!out[c]) continue;
+    const int kind = kind0 + c, stag = kind >= 8 ? kind - 8 : -1;
+    int m[3] = {L.n[0], L.n[1], L.n[2]};
+    if (stag >= 0) m[stag] += 1;
+    const size_t nf = (size_t)m[0] * m[1] * m[2];
+    double* st = g->stage + off;
+    blk_unpack_one(g, b, kind, st);
+    CK(cudaMemcpyAsync(out[c], st, nf * 8, cudaMemcpyDeviceToHost, g->stream));
+    off += nf;
+  }
+  CK(cudaStreamSynchronize(g->stream));
+  return HAMR_OK;
+}
+
+int hamr_get_block_prims(hamr_grid* g, int b, double* const prims[8]) { return get_block(g, b, 0, 8, prims); }
+int hamr_get_block_bface(hamr_grid* g, int b, double* const bface[3]) { return get_block(g, b, 8, 3, bface); }
 
 int hamr_set_levels(hamr_grid* g, const int* tau) {
   if (!g || !g->bh.on) return HAMR_EINVAL;

@@ -52,6 +52,11 @@ struct GSrc {
   bool ghost;   // sampled from a neighbour (else read from b's own active storage)
   bool zero;    // a reflecting wall face: the value is 0
   bool mod;     // differs from what b's own storage holds at id[]
+  // C-16: the neighbour is on the other x1 refinement level: the value is a restriction / prolongation
+  bool ref;
+  int rq;       // the block on b's own side of the interface in the same transverse position
+  int side;     // the neighbour lies on the high (1) or low (0) x1 side
+  int mi, lj, lk;  // b's padded x1 index of the value; the neighbour's transverse indices
 };
 
 // sd: the array is staggered along sd (-1: zone-centred)
@@ -92,7 +97,7 @@ __device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, 
     int o2[3] = {o[0], o[1], o[2]};
     o2[sd] = m[sd] == 0 ? -1 : 1;
     const int q2 = __ldg(nb + (o2[0] + 1) * 9 + (o2[1] + 1) * 3 + (o2[2] + 1));
-    if (q2 >= 0 && s.q >= 0 && Dv.B.tau[q2] < Dv.B.tau[s.q]) {
+    if (q2 >= 0 && s.q >= 0 && Dv.B.tau[q2] < Dv.B.tau[s.q] && Dv.B.info[q2].y == Dv.B.info[s.q].y) {
       s.q = q2;
       lq[sd] = m[sd] == 0 ? L.n[sd] : 0;
       s.ghost = true;
@@ -100,6 +105,13 @@ __device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, 
   }
   s.mod = s.ghost || s.zero || (sd >= 0 && ((s.negmask >> sd) & 1)) || m[0] != id[0] || m[1] != id[1] || m[2] != id[2];
   s.zl = (int)L.idx(lq[0], lq[1], lq[2]);
+  s.ref = false;
+  if (!norule && o[0] != 0 && s.q >= 0 && Dv.B.info[s.q].y != Dv.B.info[b].y) {
+    s.ref = true;
+    s.rq = __ldg(nb + 9 + (o[1] + 1) * 3 + (o[2] + 1));
+    s.side = o[0] > 0 ? 1 : 0;
+    s.mi = m[0]; s.lj = lq[1]; s.lk = lq[2];
+  }
   return s;
 }
 
@@ -120,6 +132,68 @@ __device__ __forceinline__ QTime blk_qtime(const Dev& Dv, const LevT& lt, int q,
     t.w = (double)(s_u - tb) / (double)(dtu / 2);
   }
   return t;
+}
+
+__device__ __forceinline__ double blk_at(const Dev& Dv, const Bufs& B, int kind, int q, const QTime& t, int i, int j,
+                                        int k) {
+  const long long z = (long long)q * Dv.B.blen + Dv.L.idx(i, j, k);
+  double v = buf_arr(B, t.b0, kind)[z];
+  if (t.b1 >= 0) v = (1.0 - t.w) * v + t.w * buf_arr(B, t.b1, kind)[z];
+  return v;
+}
+
+// C-16 ghost value across the x1 refinement interface.  levb: b's level.  Coarse ghosts: zones and
+// transverse faces are the mean of the two fine values they cover, normal faces the coincident fine face.
+// Fine ghosts: zones and transverse faces are piecewise linear in x1 with the MC-limited slope of the
+// coarse values (the coarse value beyond the interface is the restriction of the fine block rq), a quarter
+// of a coarse zone off the coarse centre; normal faces copy coincident coarse faces, in-between ones are
+// the mean of their two coarse neighbours.
+__device__ __forceinline__ double blk_fetch_ref(const Dev& Dv, const Bufs& B, const LevT& lt, int levb, int kind,
+                                                const GSrc& s, long long s_u) {
+  if (s.zero) return 0.0;
+  const int n0 = Dv.L.n[0];
+  const bool hi = s.side != 0, normal = kind == 5;
+  const int i = s.mi, j = s.lj, k = s.lk, q = s.q;
+  const QTime tq = blk_qtime(Dv, lt, q, s_u);
+  double v;
+  if (levb == 0) {
+    if (normal) {
+      const int t = hi ? i - n0 : -i;                       // 1..3 coarse faces from the interface
+      v = blk_at(Dv, B, kind, q, tq, hi ? 2 * t : n0 - 2 * t, j, k);
+    } else {
+      const int t = hi ? i - n0 : -1 - i;                   // 0..2 coarse zones from the interface
+      const int i0 = hi ? 2 * t : n0 - 2 * t - 2;
+      v = 0.5 * (blk_at(Dv, B, kind, q, tq, i0, j, k) + blk_at(Dv, B, kind, q, tq, i0 + 1, j, k));
+    }
+  } else {
+    if (normal) {
+      const int t = hi ? i - n0 : -i;                       // 1..3 fine faces from the interface
+      const int c0 = hi ? t / 2 : n0 - t / 2;
+      v = blk_at(Dv, B, kind, q, tq, c0, j, k);
+      if (t & 1) v = 0.5 * (v + blk_at(Dv, B, kind, q, tq, hi ? c0 + 1 : c0 - 1, j, k));
+    } else {
+      const int t = hi ? i - n0 : -1 - i;                   // 0..2 fine zones from the interface
+      const int ic = hi ? t / 2 : n0 - 1 - t / 2;
+      const bool high_half = hi ? (t & 1) != 0 : (t & 1) == 0;
+      double a3[3];
+#pragma unroll
+      for (int w = -1; w <= 1; w++) {
+        const int iw = ic + w;
+        if (iw >= 0 && iw < n0) {
+          a3[w + 1] = blk_at(Dv, B, kind, q, tq, iw, j, k);
+        } else {                                            // covered by two fine zones of rq
+          const QTime tr = blk_qtime(Dv, lt, s.rq, s_u);
+          const int i0 = hi ? n0 - 2 : 0;
+          a3[w + 1] = 0.5 * (blk_at(Dv, B, kind, s.rq, tr, i0, j, k) + blk_at(Dv, B, kind, s.rq, tr, i0 + 1, j, k));
+        }
+      }
+      double aL, aR;
+      plm_zone(a3[0], a3[1], a3[2], aL, aR);
+      v = 0.5 * (a3[1] + (high_half ? aR : aL));
+    }
+  }
+  const int vc = kind >= 5 ? kind - 5 : (kind >= 2 ? kind - 2 : -1);
+  return (vc >= 0 && ((s.negmask >> vc) & 1)) ? -v : v;
 }
 
 __device__ __forceinline__ double blk_fetch(const Dev& Dv, const Bufs& B, int b, int own_buf, int kind,
@@ -241,6 +315,10 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
   int lastq = -1;
   QTime qt;
   qt.b0 = 0; qt.b1 = -1; qt.w = 0.0;
+  const int levb = Dv.B.info[b].y;
+  auto fetch = [&](int kind, const GSrc& gs) {
+    return gs.ref ? blk_fetch_ref(Dv, B, lt, levb, kind, gs, s_u) : blk_fetch(Dv, B, b, own, kind, gs, qt);
+  };
   auto qtime = [&](int q) {
     QTime r;
     if (same) { r.b0 = role == 0 ? Dv.B.cur[q] : 1; r.b1 = -1; r.w = 0.0; return r; }
@@ -253,7 +331,7 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
     const GSrc s = blk_src(Dv, b, phys, -1, id, same);
     if (s.ghost) { qt = qtime(s.q); lastq = s.q; }
 #pragma unroll
-    for (int c = 0; c < 5; c++) vP[c] = blk_fetch(Dv, B, b, own, c, s, qt);
+    for (int c = 0; c < 5; c++) vP[c] = fetch(c, s);
   }
   double lo[3], hi[3];
   bool wF[3] = {false, false, false};
@@ -264,7 +342,7 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
     if (extra[o1] || extra[o2]) { lo[d] = hi[d] = 0.0; continue; }
     GSrc s = blk_src(Dv, b, phys, d, id, same);
     if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
-    lo[d] = blk_fetch(Dv, B, b, own, 5 + d, s, qt);
+    lo[d] = fetch(5 + d, s);
     if (s.mod) { wF[d] = shell1[o1] && shell1[o2] && id[d] >= 0 && id[d] <= L.n[d]; anymod = true; }
     hi[d] = 0.0;
     if (!extra[d]) {
@@ -272,7 +350,7 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
       idp[d] += 1;
       s = blk_src(Dv, b, phys, d, idp, same);
       if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
-      hi[d] = blk_fetch(Dv, B, b, own, 5 + d, s, qt);
+      hi[d] = fetch(5 + d, s);
       anymod = anymod || s.mod;
     }
   }
@@ -293,11 +371,11 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
       int ig[3] = {id[0], id[1], k0};
       GSrc s = blk_src(Dv, b, phys, 2, ig, same);
       if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
-      lo[2] = blk_fetch(Dv, B, b, own, 7, s, qt);
+      lo[2] = fetch(7, s);
       ig[2] = k0 + m;
       s = blk_src(Dv, b, phys, 2, ig, same);
       if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
-      hi[2] = blk_fetch(Dv, B, b, own, 7, s, qt);
+      hi[2] = fetch(7, s);
     }
 #pragma unroll
     for (int d = 0; d < 3; d++) {
@@ -685,6 +763,53 @@ __global__ void k_blk_zero_scal(Dev Dv, int first, int count) {
   for (int c = 0; c < count; c++) Dv.scal[first + c] = 0.0;
 }
 
+// C-16: where a coarse and a fine block on the same time level share the x1 interface, the fine block's F^1
+// and the edge EMFs E_2, E_3 lying in the interface plane are authoritative: the coarse block overwrites its
+// own with them before its update (equal face areas and edge lengths: plain copies).
+__global__ void __launch_bounds__(128) k_blk_iface(Dev Dv) {
+  const Lay& L = Dv.L;
+  const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
+  const unsigned per = 2u * c1 * c2;
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= per * Dv.B.nact) return;
+  const int bslot = (int)(t / per);
+  t -= bslot * per;
+  const int c = __ldg(Dv.B.list + bslot);
+  if (Dv.B.info[c].y != 0) return;
+  const int side = (int)(t / (unsigned)(c1 * c2));
+  t -= side * c1 * c2;
+  const int j = (int)(t / (unsigned)c2), k = (int)(t - (t / (unsigned)c2) * c2);
+  const int q = __ldg(Dv.B.nbr + c * 27 + (side ? 2 : 0) * 9 + 4);
+  if (q < 0 || Dv.B.info[q].y == 0 || Dv.B.tau[q] != Dv.B.tau[c]) return;
+  const long long zc = (long long)c * Dv.B.blen + L.idx(side ? L.n[0] : 0, j, k);
+  const long long zq = (long long)q * Dv.B.blen + L.idx(side ? 0 : L.n[0], j, k);
+  if (j < L.n[1] && k < L.n[2]) {
+#pragma unroll
+    for (int cc = 0; cc < 5; cc++) Dv.F[0][cc][zc] = Dv.F[0][cc][zq];
+  }
+  if (j < L.n[1]) Dv.Ee[1][zc] = Dv.Ee[1][zq];
+  if (k < L.n[2]) Dv.Ee[2][zc] = Dv.Ee[2][zq];
+}
+
+// one block's dense arrays <-> its padded storage (grids with x1 refinement are set and read block by block)
+__global__ void __launch_bounds__(256) k_blk_pack1(Dev Dv, int b, const double* __restrict__ dense, double* __restrict__ s0,
+                                                   double* __restrict__ s2, int stag, int zero_pole, int unpack) {
+  const Lay& L = Dv.L;
+  int m[3] = {L.n[0], L.n[1], L.n[2]};
+  if (stag >= 0) m[stag] += 1;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (unsigned)(m[0] * m[1] * m[2])) return;
+  const unsigned tj = t / (unsigned)m[2], ti = tj / (unsigned)m[1];
+  const int k = (int)(t - tj * m[2]), j = (int)(tj - ti * m[1]), i = (int)ti;
+  double* a = Dv.B.cur[b] ? s2 : s0;
+  const long long z = (long long)b * Dv.B.blen + L.idx(i, j, k);
+  if (unpack) { const_cast<double*>(dense)[t] = a[z]; return; }
+  double v = dense ? dense[t] : 0.0;
+  const int J = Dv.B.info[b].w + j;
+  if (zero_pole && Dv.metric == HAMR_METRIC_KERR_SCHILD && (J == 0 || J == Dv.B.n2g)) v = 0.0;
+  a[z] = v;
+}
+
 // ==== host side ==============================================================================================
 
 static Bufs bufs_of(const hamr_grid* g) {
@@ -716,12 +841,32 @@ static cudaError_t blk_upload_flags(hamr_grid* g) {
     for (int a = 0; a < 27; a++) {
       const int q = H.nbr[(size_t)b * 27 + a];
       if (q < 0) continue;
-      if (H.tau[q] != H.tau[b]) same = false;
+      if (H.tau[q] != H.tau[b] || H.lev1[q] != H.lev1[b]) same = false;
       if (H.tau[q] < H.tau[b]) finer = true;
     }
     hf[b] = ((same && H.phys[b] == 0) ? 1 : 0) | (finer ? 2 : 0) | (same ? 4 : 0);
   }
   return cudaMemcpyAsync(g->D.B.flags, hf, (size_t)H.nblk * 4, cudaMemcpyHostToDevice, g->stream);
+}
+
+// C-16 x1 slots: a base block column whose x1-centre has r < r_refine_max (x1 itself on the Cartesian map)
+// is replaced by two children with dx1 / 2 (per-dimension splitting).  Returns the number of
+// refined columns (they must be contiguous from the low x1 side), -1 if they are not.
+static int blk_refined_columns(const hamr_params& p, int ncol, int bn0) {
+  if (!(p.r_refine_max > 0.0)) return 0;
+  const bool ks = p.metric == HAMR_METRIC_KERR_SCHILD;
+  const double lo = ks ? std::log(p.xmin[0]) : p.xmin[0], hi = ks ? std::log(p.xmax[0]) : p.xmax[0];
+  const double dx0 = (hi - lo) / p.n[0];
+  int nref = 0;
+  bool seen_coarse = false;
+  for (int col = 0; col < ncol; col++) {
+    const double xc = lo + ((double)col + 0.5) * bn0 * dx0;
+    const bool refined = (ks ? std::exp(xc) : xc) < p.r_refine_max;
+    if (refined && seen_coarse) return -1;
+    if (refined) nref++;
+    else seen_coarse = true;
+  }
+  return nref;
 }
 
 int blk_count(const hamr_params& p, int nslot[3], int bn[3]) {
@@ -730,9 +875,19 @@ int blk_count(const hamr_params& p, int nslot[3], int bn[3]) {
     bn[d] = p.nb[d] > 0 ? p.nb[d] : p.n[d];
     if (bn[d] < NG || p.n[d] % bn[d] != 0) return 0;
     nslot[d] = p.n[d] / bn[d];
-    nb *= nslot[d];
   }
+  const int nref = blk_refined_columns(p, nslot[0], bn[0]);
+  if (nref < 0) return 0;
+  if (nref > 0 && bn[0] < 2 * NG) return 0;   // a coarse ghost layer of 3 zones covers 6 fine zones
+  nslot[0] += nref;
+  for (int d = 0; d < 3; d++) nb *= nslot[d];
   return nb > (1 << 20) ? 0 : (int)nb;
+}
+
+int blk_has_refinement(const hamr_params& p) {
+  int ns[3], bn[3];
+  if (blk_count(p, ns, bn) <= 0) return 0;
+  return blk_refined_columns(p, p.n[0] / bn[0], bn[0]) > 0 ? 1 : 0;
 }
 
 size_t blk_table_bytes(int nblk) {
@@ -760,15 +915,20 @@ int blk_setup(hamr_grid* g, void* tables) {
   const int ge2 = p.n[1] + 2 * NG + 1;
   std::vector<int> info((size_t)nblk * 4), phys(nblk), K0(nblk);
   auto id_of = [&](int s0, int s1, int s2) { return (s0 * H.nslot[1] + s1) * H.nslot[2] + s2; };
+  const int nref = blk_refined_columns(p, p.n[0] / bn[0], bn[0]);   // slots 0 .. 2 nref - 1 are fine children
+  H.refined = nref > 0;
   for (int s0 = 0; s0 < H.nslot[0]; s0++)
     for (int s1 = 0; s1 < H.nslot[1]; s1++)
       for (int s2 = 0; s2 < H.nslot[2]; s2++) {
         const int b = id_of(s0, s1, s2);
         const int sl[3] = {s0, s1, s2};
-        const int I0[3] = {s0 * bn[0], s1 * bn[1], s2 * bn[2]};
+        // x1 index of the block's first zone in zones of its own level
+        const int lev = s0 < 2 * nref ? 1 : 0;
+        const int I0[3] = {lev ? s0 * bn[0] : (s0 - nref) * bn[0], s1 * bn[1], s2 * bn[2]};
+        H.lev1[b] = lev;
         for (int d = 0; d < 3; d++) H.I0[(size_t)b * 3 + d] = I0[d];
         info[(size_t)b * 4 + 0] = (I0[0] + NG) * ge2 + I0[1] + NG;
-        info[(size_t)b * 4 + 1] = 0;
+        info[(size_t)b * 4 + 1] = lev;
         info[(size_t)b * 4 + 2] = I0[0];
         info[(size_t)b * 4 + 3] = I0[1];
         K0[b] = I0[2];
@@ -863,6 +1023,31 @@ void blk_unpack(hamr_grid* g, int kind, double* dense) {
                                                                      g->par.n[1], g->par.n[2]);
 }
 
+void blk_pack_one(hamr_grid* g, int b, const double* dense, int kind, int stag, bool zero_pole) {
+  const Lay& L = g->D.L;
+  int m[3] = {L.n[0], L.n[1], L.n[2]};
+  if (stag >= 0) m[stag] += 1;
+  const int tot = m[0] * m[1] * m[2];
+  double* a0 = kind < 5 ? g->s[0].P[kind] : g->s[0].Bf[kind - 5];
+  double* a2 = kind < 5 ? g->s[2].P[kind] : g->s[2].Bf[kind - 5];
+  Launch l_(g, K_OTHER);
+  k_blk_pack1<<<(tot + 255) / 256, 256, 0, g->stream>>>(g->D, b, dense, a0, a2, stag, zero_pole ? 1 : 0, 0);
+}
+
+void blk_unpack_one(hamr_grid* g, int b, int kind, double* dense) {
+  const Lay& L = g->D.L;
+  const int stag = kind >= 8 ? kind - 8 : -1;
+  int m[3] = {L.n[0], L.n[1], L.n[2]};
+  if (stag >= 0) m[stag] += 1;
+  const int tot = m[0] * m[1] * m[2];
+  auto arr = [&](int buf) -> double* {
+    const Fields& f = g->s[buf];
+    return kind < 5 ? f.P[kind] : (kind < 8 ? f.Bc[kind - 5] : f.Bf[kind - 8]);
+  };
+  Launch l_(g, K_OTHER);
+  k_blk_pack1<<<(tot + 255) / 256, 256, 0, g->stream>>>(g->D, b, dense, arr(0), arr(2), stag, 0, 1);
+}
+
 static void blk_ghosts(hamr_grid* g, const Dev& D, int role, long long s_u, bool all, bool zero_ctop) {
   if (D.B.nact == 0) return;
   const Lay& L = D.L;
@@ -890,6 +1075,12 @@ static void blk_stage(hamr_grid* g, int tau, bool corrector) {
     launch_flux_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2, corrector);
     launch_ct_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2);
     launch_deref_fix_edges(g, D);
+    if (H.refined) {   // C-16: same-time flux / EMF agreement on the refinement interface
+      const Lay& L = D.L;
+      const long long tot = 2LL * (L.n[1] + 1) * (L.n[2] + 1) * D.B.nact;
+      Launch l_(g, K_OTHER);
+      k_blk_iface<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D);
+    }
     const double lev_fac = (double)(1 << tau);   // dt_b = 2^tau dt_0
     if (corrector && tau < H.tmax) {
       const int first = (H.tb_u[tau] % (2LL * H.dt_u[tau])) == 0 ? 1 : 0;

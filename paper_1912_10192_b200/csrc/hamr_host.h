@@ -102,6 +102,7 @@ namespace hamr {
 // host side of the block-structured grid (blocks.cu)
 struct BlkHost {
   bool on;                   // block-structured grid (more than one block, or LAT)
+  bool refined;              // some block columns carry the x1 refinement level (C-16)
   int nblk, tmax;            // blocks; highest LAT level (0: one global dt)
   int nslot[3];              // block lattice extents
   std::vector<int> nbr;      // [nblk][27] host mirror of the neighbour table
@@ -136,6 +137,7 @@ struct hamr_grid {
   size_t stage_doubles;
   double* h_pinned;          // small pinned host buffer for scalar read-back
   bool have_state, dead;
+  bool blocks_open;          // hamr_set_block_prims calls are being collected; hamr_blocks_commit closes
   long long launches;
   std::string err;
   // per-kernel timers: CUDA event pairs on the grid's stream around every launch while enabled
@@ -204,6 +206,9 @@ void launch_geometry_tab(hamr_grid* g, int e1, int e2, int n2d, double dx1, int 
 
 // blocks.cu: block-structured grid (H7)
 int blk_count(const hamr_params& p, int nslot[3], int bn[3]);       // number of blocks (0 if invalid)
+int blk_has_refinement(const hamr_params& p);
+void blk_pack_one(hamr_grid* g, int b, const double* dense, int kind, int stag, bool zero_pole);
+void blk_unpack_one(hamr_grid* g, int b, int kind, double* dense);
 size_t blk_table_bytes(int nblk);                                   // device bytes of the block tables
 int blk_setup(hamr_grid* g, void* tables);                          // lattice, neighbour tables, lists
 void blk_pack(hamr_grid* g, const double* dense, int kind, int stag, bool zero_pole);  // kind: 0..4 P, 5..7 Bf

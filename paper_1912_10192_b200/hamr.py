@@ -29,7 +29,8 @@ SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "h
            "hamr_set_prims", "hamr_set_prims_dev", "hamr_step", "hamr_step_async", "hamr_sync",
            "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
            "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
-           "hamr_set_levels",
+           "hamr_set_levels", "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
+           "hamr_get_block_bface",
            "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
            "hamr_profile_begin", "hamr_profile_end", "hamr_profile_class_name", "hamr_launch_count"]
 NKCLASS = 10
@@ -84,6 +85,10 @@ def lib():
         L.hamr_num_blocks.argtypes = [vp]
         L.hamr_block_info.argtypes = [vp, C.c_int, c_double_p, c_double_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.hamr_set_levels.argtypes = [vp, C.POINTER(C.c_int)]
+        L.hamr_set_block_prims.argtypes = [vp, C.c_int, C.POINTER(c_double_p), C.POINTER(c_double_p)]
+        L.hamr_blocks_commit.argtypes = [vp]
+        L.hamr_get_block_prims.argtypes = [vp, C.c_int, C.POINTER(c_double_p)]
+        L.hamr_get_block_bface.argtypes = [vp, C.c_int, C.POINTER(c_double_p)]
         L.hamr_debug_emf.argtypes = [vp]
         L.hamr_get_face.argtypes = [vp, C.c_int, C.c_int, c_double_p]
         L.hamr_get_edge.argtypes = [vp, C.c_int, c_double_p]
@@ -256,6 +261,30 @@ class Grid:
 
     def num_blocks(self):
         return self.L.hamr_num_blocks(self.h)
+
+    def set_block_prims(self, b, hydro, bface=None):
+        hy = [_arr(h) for h in hydro]
+        hp = (c_double_p * 5)(*[_dp(h) for h in hy])
+        bp = None
+        if bface is not None:
+            bf = [_arr(x) for x in bface]
+            bp = (c_double_p * 3)(*[_dp(x) for x in bf])
+        return self.L.hamr_set_block_prims(self.h, int(b), hp, bp)
+
+    def commit(self):
+        return self.L.hamr_blocks_commit(self.h)
+
+    def get_block_prims(self, b):
+        n = self.block_info(b)[2]
+        out = [np.empty(n) for _ in range(8)]
+        self._ck(self.L.hamr_get_block_prims(self.h, int(b), (c_double_p * 8)(*[_dp(o) for o in out])))
+        return out
+
+    def get_block_bface(self, b):
+        n = self.block_info(b)[2]
+        out = [np.empty(tuple(n[e] + (e == d) for e in range(3))) for d in range(3)]
+        self._ck(self.L.hamr_get_block_bface(self.h, int(b), (c_double_p * 3)(*[_dp(o) for o in out])))
+        return out
 
     def set_levels(self, tau):
         if tau is None:

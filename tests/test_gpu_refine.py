@@ -1,0 +1,107 @@
+"""GPU <-> oracle parity on grids with the x1 refinement level (DESIGN.md §9 C-16;
+PAPER.md:71, 137): restricted / prolonged ghosts across the coarse-fine interface, interface flux and EMF
+agreement, alone, with LAT, and with phi-derefinement (the full feature set of BASELINE cfg 4).  Needs a B200."""
+import numpy as np
+import pytest
+
+from paper_1912_10192_b200 import inputs as I
+from tests._parity import parity_errors
+
+pytestmark = pytest.mark.gpu
+
+TOL_1, TOL_10, TOL_DIVB = 1e-10, 1e-7, 1e-12
+
+
+@pytest.fixture(scope="module")
+def H():
+    from paper_1912_10192_b200 import build, hamr
+    build.build_lib()
+    hamr.lib()
+    return hamr
+
+
+def _infos(o):
+    out = []
+    for b in range(o.num_blocks()):
+        d = o.block_info(b)
+        out.append((d["x_lo"], d["dx"], d["n"]))
+    return out
+
+
+def _set_both(g, o, data):
+    for b, (hyd, bf) in enumerate(data):
+        assert g.set_block_prims(b, hyd, bf) == 0 and o.set_block_prims(b, hyd, bf) == 0
+    assert g.commit() == 0 and o.commit() == 0
+
+
+def _check_blocks(p, infos, o, g, tol):
+    worst = {}
+    for b, (x_lo, dx, n) in enumerate(infos):
+        pg = I.block_as_grid(p, x_lo, dx, n)
+        e = parity_errors(pg, o.get_block_prims(b), g.get_block_prims(b))
+        for k, v in e.items():
+            worst[k] = max(worst.get(k, 0.0), v)
+        for a, c in zip(o.get_block_bface(b), g.get_block_bface(b)):
+            assert np.abs(a - c).max() <= tol * max(np.abs(a).max(), 1e-300)
+    assert max(worst.values()) <= tol, worst
+    assert g.divb() <= TOL_DIVB and g.stats()[0] == 0
+
+
+def test_refined_lattice_matches_oracle(H, orc):
+    p = I.torus_params(n=(32, 16, 16), nb=(8, 8, 8), r_refine_max=4.0)
+    g, o = H.Grid(p), orc.OrcGrid(p)
+    assert g.num_blocks() == o.num_blocks() and g.num_blocks() > 4 * 2 * 2
+    for b in range(g.num_blocks()):
+        lo, dx, n, _ = g.block_info(b)
+        d = o.block_info(b)
+        assert np.allclose(lo, d["x_lo"], rtol=0, atol=1e-13) and np.allclose(dx, d["dx"], rtol=1e-14) and n == d["n"]
+
+
+@pytest.mark.parametrize("lat", [0, 1])
+def test_refined_minkowski_waves(H, orc, lat):
+    p = I.minkowski_params(n=(16, 8, 8), nb=(8, 4, 4), r_refine_max=0.5, lat_max_level=lat)   # 2 interfaces
+    g, o = H.Grid(p), orc.OrcGrid(p)
+    infos = _infos(o)
+    if lat:
+        lv = [0 if o.block_info(b)["lev1"] else 1 for b in range(o.num_blocks())]
+        o.force_levels(lv)
+        g.set_levels(lv)
+    data = [I.minkowski_waves(I.block_as_grid(p, *inf), amp=1e-2, noise=0.0, box=(1.0, 1.0, 1.0)) for inf in infos]
+    _set_both(g, o, data)
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt
+    if lat:
+        assert g.levels() == list(o.levels()) and len(set(g.levels())) == 2
+    t0 = g.totals()
+    g.step(1)
+    o.step(1)
+    _check_blocks(p, infos, o, g, TOL_1 * (2 if lat else 1))
+    g.step(5)
+    o.step(5)
+    _check_blocks(p, infos, o, g, TOL_10)
+    t1 = g.totals()
+    assert np.abs(t1 - t0).max() / max(t0[0], abs(t0[1])) < 1e-13   # conservative through both interfaces
+
+
+@pytest.mark.parametrize("extra", [dict(), dict(lat_max_level=2),
+                                   dict(nb=(8, 4, 16), lat_max_level=1, deref_theta_deg=(30.0, 12.0), deref_factor=(2, 4))])
+def test_refined_torus(H, orc, extra):
+    """cfg 0 torus with the block columns inside r < 4 refined (the horizon region), outflow / polar / periodic
+    boundaries on the edge blocks; last case: every feature of BASELINE cfg 4 at once"""
+    kw = dict(nb=(8, 8, 8), r_refine_max=4.0)
+    kw.update(extra)
+    p = I.torus_params(n=(32, 16, 16), **kw)
+    g, o = H.Grid(p), orc.OrcGrid(p)
+    infos = _infos(o)
+    assert any(o.block_info(b)["lev1"] for b in range(o.num_blocks()))
+    _set_both(g, o, I.fm_torus_blocks(p, infos, seed=4))
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt
+    if "lat_max_level" in extra:
+        assert g.levels() == list(o.levels())
+    g.step(1)
+    o.step(1)
+    fin = 2 ** extra.get("lat_max_level", 0)
+    _check_blocks(p, infos, o, g, TOL_1 * fin)
+    if g.levels() == list(o.levels()):
+        g.step(3)
+        o.step(3)
+        _check_blocks(p, infos, o, g, TOL_10)

@@ -26,7 +26,7 @@ def _set_blocks(g, p, fn):
     assert g.commit() == 0
 
 
-def _refined_box(n=(16, 8, 8), nb=(4, 4, 4), **kw):
+def _refined_box(n=(16, 8, 8), nb=(8, 4, 4), **kw):
     # periodic unit cube, columns with x1-centre < 0.5 refined: two coarse/fine interfaces (one through the wrap)
     return I.minkowski_params(n=n, nb=nb, r_refine_max=0.5, **kw)
 
@@ -34,9 +34,9 @@ def _refined_box(n=(16, 8, 8), nb=(4, 4, 4), **kw):
 def test_refined_lattice(orc):
     p = _refined_box()
     g = orc.OrcGrid(p)
-    assert g.num_blocks() == (2 * 2 + 2) * 2 * 2
+    assert g.num_blocks() == (2 * 1 + 1) * 2 * 2
     lev = [g.block_info(b)["lev1"] for b in range(g.num_blocks())]
-    assert sorted(set(lev)) == [0, 1] and sum(lev) == 4 * 4
+    assert sorted(set(lev)) == [0, 1] and sum(lev) == 2 * 4
     for b in range(g.num_blocks()):
         d = g.block_info(b)
         assert abs(d["dx"][0] - (1 / 32 if d["lev1"] else 1 / 16)) < 1e-15
@@ -82,7 +82,7 @@ def test_refinement_conserves_and_keeps_divb(orc, lat):
 
 
 def _wave_error(orc, N, T=0.25):
-    p = _refined_box(n=(N, N // 2, N // 2), nb=(N // 4, N // 4, N // 4))
+    p = _refined_box(n=(N, N // 2, N // 2), nb=(N // 2, N // 4, N // 4))
     g = orc.OrcGrid(p)
     _set_blocks(g, p, lambda pg: I.minkowski_waves(pg, amp=1e-6, noise=0.0, modes=("fast",), box=(1.0, 1.0, 1.0)))
     t = 0.0
