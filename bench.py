@@ -3,7 +3,7 @@
 fraction of the dominant kernel, the end-to-end number through the C-ABI with host buffers, and the
 CPU oracle timed beside it.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg4b]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg4b|cfg4]
 
 A "step" is one full pass of the hot path over the whole grid: hamr_step(1) = predictor + corrector
 = one zone-cycle per zone.  Default workload: BASELINE.json configs[2], the 256x128x128
@@ -49,6 +49,14 @@ def workload(name):
                            deref_theta_deg=(15.0, 5.0), deref_factor=(2, 4))
         return p, (lambda: I.fm_torus(p, seed=4)), ("BASELINE cfg4 without r-refinement: Kerr FM torus 256x128x128 in 16x16x128 "
                                                      "blocks, phi-derefinement 2x/4x, LAT levels 1/2/4")
+    if name == "cfg4":
+        # BASELINE cfg 4 with blocks that span phi: 16 x 16 x 128 blocks, phi-derefined 2x / 4x
+        # within 15 / 5 degrees of the poles, one x1 refinement level for r < 20 (184 blocks, 6 029 312 zones),
+        # LAT levels 1, 2, 4; torus data sampled per block, seed 4.  gen() returns the per-block data.
+        p = I.torus_params(n=(256, 128, 128), r_out=1000.0, nb=(16, 16, 128), lat_max_level=2, r_refine_max=20.0,
+                           deref_theta_deg=(15.0, 5.0), deref_factor=(2, 4))
+        return p, (lambda infos: I.fm_torus_blocks(p, infos, seed=4)), ("BASELINE cfg4: Kerr FM torus, base 256x128x128 in "
+                   "16x16x128 blocks, one x1 refinement level r<20, phi-derefinement 2x/4x, LAT levels 1/2/4")
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -143,18 +151,33 @@ def units_per_launch(cls, n):
     return n1 * n2 * n3
 
 
+def oracle_set(o, p, gen):
+    """initial state into an oracle grid (block by block on a refined grid); returns the number of zones"""
+    if p["r_refine_max"] > 0:
+        infos = []
+        for b in range(o.num_blocks()):
+            d = o.block_info(b)
+            infos.append((d["x_lo"], d["dx"], d["n"]))
+        for b, (hb, fb) in enumerate(gen(infos)):
+            assert o.set_block_prims(b, hb, fb) == 0
+        assert o.commit() == 0
+        return sum(int(np.prod(i[2])) for i in infos)
+    hyd, bf = gen()
+    assert o.set_prims(hyd, bf) == 0
+    return int(np.prod(p["n"]))
+
+
 def cpu_oracle_time(p, gen, steps):
     """times the oracle as it stands on the host cores: `steps` full steps of the workload"""
     from tests import _orc
-    hyd, bf = gen()
     o = _orc.OrcGrid(p)
-    o.set_prims(hyd, bf)
+    nz = oracle_set(o, p, gen)
     t0 = time.perf_counter()
     o.step(steps)
     dt = time.perf_counter() - t0
     cores = int(_orc.lib().orc_omp_threads())
     o.close()
-    nz = int(np.prod(p["n"])) * 2 ** int(p["lat_max_level"])   # effective zone-cycles per (coarse) step
+    nz = nz * 2 ** int(p["lat_max_level"])   # effective zone-cycles per (coarse) step
     return nz * steps / dt, dt, cores
 
 
@@ -166,9 +189,8 @@ def run_reference(args):
     subprocess.check_call(["make", "-s", "-C", os.path.join(ROOT, "oracle")])
     p, gen, desc = workload(args.workload)
     from tests import _orc
-    hyd, bf = gen()
     o = _orc.OrcGrid(p)
-    o.set_prims(hyd, bf)
+    nz0 = oracle_set(o, p, gen)
     for _ in range(args.warmup):
         o.step(1)
     t0 = time.perf_counter()
@@ -176,7 +198,7 @@ def run_reference(args):
         o.step(1)
     dt = time.perf_counter() - t0
     cores = int(_orc.lib().orc_omp_threads())
-    nz = int(np.prod(p["n"])) * 2 ** int(p["lat_max_level"])
+    nz = nz0 * 2 ** int(p["lat_max_level"])
     val = nz * args.steps / dt
     sample = f"{args.steps} full oracle steps of the whole {p['n'][0]}x{p['n'][1]}x{p['n'][2]} grid per timed step"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
@@ -229,11 +251,20 @@ def main():
     nz = int(np.prod(n))
     blocky = any(p["nb"]) or p["lat_max_level"] > 0
     fin = 2 ** int(p["lat_max_level"])        # finest steps per hamr_step on a LAT grid
-    hyd, bf = gen()
     g = hamr.Grid(p, torch_arena=True)        # device memory and stream from torch; all math in libhamr
-    hd = [torch.from_numpy(np.ascontiguousarray(h)).cuda() for h in hyd]
-    bd = [torch.from_numpy(np.ascontiguousarray(b)).cuda() for b in bf]
-    assert g.set_prims_dev(hd, bd) == 0
+    refined = p["r_refine_max"] > 0
+    if refined:                               # a refined grid has no global zone array: block-by-block state
+        infos = [g.block_info(b)[:3] for b in range(g.num_blocks())]
+        bdata = gen(infos)
+        nz = sum(int(np.prod(i[2])) for i in infos)
+        for b, (hb, fb) in enumerate(bdata):
+            assert g.set_block_prims(b, hb, fb) == 0
+        assert g.commit() == 0
+    else:
+        hyd, bf = gen()
+        hd = [torch.from_numpy(np.ascontiguousarray(h)).cuda() for h in hyd]
+        bd = [torch.from_numpy(np.ascontiguousarray(b)).cuda() for b in bf]
+        assert g.set_prims_dev(hd, bd) == 0
     g.sync()
 
     def barrier():
@@ -274,20 +305,39 @@ def main():
 
     # ---- end to end through the C-ABI with HOST buffers (pinned): set_prims + step + get_prims -----
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
-    hh = [pin(h) for h in hyd]
-    bh = [pin(b) for b in bf]
-    outs = [torch.empty(n, dtype=torch.float64).pin_memory().numpy() for _ in range(8)]
     C = hamr.C
-    hp = (hamr.c_double_p * 5)(*[hamr._dp(h) for h in hh])
-    bp = (hamr.c_double_p * 3)(*[hamr._dp(b) for b in bh])
-    op = (hamr.c_double_p * 8)(*[hamr._dp(o) for o in outs])
     L = hamr.lib()
+    if refined:
+        hh = [pin(h) for hb, fb in bdata for h in hb]
+        bh = [pin(f) for hb, fb in bdata for f in fb]
+        nbk = g.num_blocks()
+        outs = [torch.empty(infos[b][2], dtype=torch.float64).pin_memory().numpy() for b in range(nbk) for _ in range(8)]
+        hps = [(hamr.c_double_p * 5)(*[hamr._dp(h) for h in hh[5 * b:5 * b + 5]]) for b in range(nbk)]
+        bps = [(hamr.c_double_p * 3)(*[hamr._dp(f) for f in bh[3 * b:3 * b + 3]]) for b in range(nbk)]
+        ops = [(hamr.c_double_p * 8)(*[hamr._dp(o) for o in outs[8 * b:8 * b + 8]]) for b in range(nbk)]
 
-    def e2e_step():
-        rc = L.hamr_set_prims(g.h, hp, bp)
-        rc |= L.hamr_step(g.h, 1, None, None)
-        rc |= L.hamr_get_prims(g.h, op)
-        assert rc == 0, rc
+        def e2e_step():
+            rc = 0
+            for b in range(nbk):
+                rc |= L.hamr_set_block_prims(g.h, b, hps[b], bps[b])
+            rc |= L.hamr_blocks_commit(g.h)
+            rc |= L.hamr_step(g.h, 1, None, None)
+            for b in range(nbk):
+                rc |= L.hamr_get_block_prims(g.h, b, ops[b])
+            assert rc == 0, rc
+    else:
+        hh = [pin(h) for h in hyd]
+        bh = [pin(b) for b in bf]
+        outs = [torch.empty(n, dtype=torch.float64).pin_memory().numpy() for _ in range(8)]
+        hp = (hamr.c_double_p * 5)(*[hamr._dp(h) for h in hh])
+        bp = (hamr.c_double_p * 3)(*[hamr._dp(b) for b in bh])
+        op = (hamr.c_double_p * 8)(*[hamr._dp(o) for o in outs])
+
+        def e2e_step():
+            rc = L.hamr_set_prims(g.h, hp, bp)
+            rc |= L.hamr_step(g.h, 1, None, None)
+            rc |= L.hamr_get_prims(g.h, op)
+            assert rc == 0, rc
     e2e_step()
     barrier()
     t0 = time.perf_counter()
@@ -309,6 +359,9 @@ def main():
             dist.destroy_process_group()
         return
 
+    nb_ws = C.c_size_t(0)
+    L.hamr_workspace_bytes(C.byref(g._par), C.byref(nb_ws))
+    ws_gb = nb_ws.value / 1e9
     # ---- roofline of the dominant kernel ------------------------------------------------------------
     hbm_peak, peak_src = peaks()
     kern = {k: {"ms_total": v[0], "launches": v[1], "ms_avg": v[0] / v[1] if v[1] else 0.0,
@@ -335,10 +388,10 @@ def main():
     cpu = None
     if not args.no_cpu_baseline:
         subprocess.check_call(["make", "-s", "-C", os.path.join(ROOT, "oracle")])
-        steps_cpu = 3 if args.workload == "cfg2" else (1 if args.workload == "cfg4b" else 2)
+        steps_cpu = 3 if args.workload == "cfg2" else (1 if args.workload in ("cfg4b", "cfg4") else 2)
         v, secs, cores = cpu_oracle_time(p, gen, steps_cpu)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"{steps_cpu} full steps of the same {n[0]}x{n[1]}x{n[2]} workload ({secs:.1f} s)"}
+               "sample": f"{steps_cpu} full {'coarse ' if fin > 1 else ''}steps of the same workload, all {nz} zones ({secs:.1f} s)"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
@@ -346,10 +399,12 @@ def main():
             "config": {"workload": desc, "zones": nz, "blocks": g.num_blocks(), "finest_steps_per_step": fin,
                        "performed_zone_updates_per_sec": performed,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "l2": "inputs (2.4 GB state) larger than L2; no flush needed", "timing": "CUDA events on the launching (torch current) stream"},
+                       "l2": f"state arrays ({ws_gb:.1f} GB workspace) far larger than the 126 MB L2; no flush needed",
+                       "timing": "CUDA events on the launching (torch current) stream"},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": args.e2e_steps, "what": "hamr_set_prims(host) + hamr_step(1) + hamr_get_prims(host), pinned buffers"},
+                    "steps": args.e2e_steps, "what": ("hamr_set_block_prims x blocks + hamr_blocks_commit + hamr_step(1) + hamr_get_block_prims x blocks"
+                             if refined else "hamr_set_prims(host) + hamr_step(1) + hamr_get_prims(host)") + ", pinned buffers"},
             "gpu_launches": launches,
             "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line))
