@@ -151,6 +151,19 @@ def units_per_launch(cls, n):
     return n1 * n2 * n3
 
 
+def replica_throughput(ms_local, units_per_rank, world, device):
+    """Whole-job value of N independent replicas ("replicas only"): the timed region of
+    every rank, the MAX over ranks (one scalar all-reduce of the TIMING, not a data-path collective), and
+    world x units / that time.  Returns (value per second, max ms).  Covered on CPU by a world_size-2 gloo test."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    return world * units_per_rank / (ms_max * 1e-3), ms_max
+
+
 def oracle_set(o, p, gen):
     """initial state into an oracle grid (block by block on a refined grid); returns the number of zones"""
     if p["r_refine_max"] > 0:
@@ -292,12 +305,8 @@ def main():
     clocks = sampler.stop()
     launches = g.launch_count() - l0
     g.sync()
-    tms = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    ms_max = float(tms.item())
     # LAT: "effective" zone-cycles (zones x finest-level steps, the paper's convention)
-    value = world * nz * fin * args.steps / (ms_max * 1e-3)
+    value, ms_max = replica_throughput(ms, nz * fin * args.steps, world, "cuda")
     performed = None
     if blocky:
         lv = np.array(g.levels())
@@ -347,10 +356,7 @@ def main():
     ev1.record()
     barrier()
     e2e_ms = max(ev0.elapsed_time(ev1), 1e3 * (time.perf_counter() - t0))
-    tms = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    e2e_val = world * nz * fin * args.e2e_steps / (float(tms.item()) * 1e-3)
+    e2e_val, _ = replica_throughput(e2e_ms, nz * fin * args.e2e_steps, world, "cuda")
     h2d = sum(a.nbytes for a in hh) + sum(a.nbytes for a in bh)
     d2h = sum(a.nbytes for a in outs)
 
