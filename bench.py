@@ -3,7 +3,7 @@
 fraction of the dominant kernel, the end-to-end number through the C-ABI with host buffers, and the
 CPU oracle timed beside it.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg4b|cfg4]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg3|cfg4b|cfg4]
 
 A "step" is one full pass of the hot path over the whole grid: hamr_step(1) = predictor + corrector
 = one zone-cycle per zone.  Default workload: BASELINE.json configs[2], the 256x128x128
@@ -42,6 +42,10 @@ def workload(name):
     if name == "cfg1":
         p = I.minkowski_params(n=(128, 128, 128))
         return p, (lambda: I.minkowski_waves(p, seed=1)), "BASELINE cfg1: Minkowski periodic 128^3 linear waves"
+    if name == "cfg3":
+        p = I.tilted_disk_params()
+        return p, (lambda: I.tilted_disk(p, seed=3)), ("BASELINE cfg3: tilted thin disk 512x256x256 fp64 (synthetic stand-in: "
+                                                        "h/r=0.03, tilt 65 deg, toroidal field beta=10)")
     if name == "cfg4b":
         # the part of BASELINE cfg 4 that is built: cfg 2's torus (seed 4) on 16 x 16 x 128
         # blocks, phi-derefined by 2 / 4 within 15 / 5 degrees of the poles, LAT levels 1, 2, 4; no r-refinement

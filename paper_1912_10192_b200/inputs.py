@@ -369,3 +369,109 @@ def minkowski_waves(p: dict, seed: int = 1, amp: float = 1e-6, noise: float = 1e
     if noise != 0.0:
         hyd[0] = hyd[0] * (1.0 + noise * rand_pm1(seed, zone_index(n)))
     return hyd, bface
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json cfg 3: tilted thin disk.  The paper's model is unpublished ("in prep."), so
+# this is a synthetic stand-in with the same load pattern: a thin (h/r = 0.03), strongly magnetised sheet
+# inclined by 65 degrees that crosses the polar rows.  Not an equilibrium.
+# ------------------------------------------------------------------------------------------------
+def tilted_disk_params(n=(512, 256, 256), **kw) -> dict:
+    return base_params(n=tuple(n), xmax=(1000.0, np.pi, 2.0 * np.pi), **kw)
+
+
+def _disk_frame(r, th, ph, tilt):
+    """Cartesian-like position from the KS spatial coordinates, and cylindrical (R', z') about the axis
+    z' = (sin tilt, 0, cos tilt)."""
+    st, ct = np.sin(th), np.cos(th)
+    x, y, z = r * st * np.cos(ph), r * st * np.sin(ph), r * ct
+    ax = np.array([np.sin(tilt), 0.0, np.cos(tilt)])
+    zp = x * ax[0] + z * ax[2]
+    Rp = np.sqrt(np.maximum(r * r - zp * zp, 0.0))
+    return (x, y, z), ax, Rp, zp
+
+
+def _disk_density(Rp, zp, hr, r_in, r_out):
+    Rs = np.maximum(Rp, 1e-3 * r_in)
+    H = hr * Rs
+    taper = np.where(Rp < 0.9 * r_out, 1.0, 0.5 * (1.0 + np.cos(np.pi * np.clip((Rp - 0.9 * r_out) / (0.1 * r_out), 0.0, 1.0))))
+    taper = taper * np.clip((Rp - r_in) / (0.1 * r_in), 0.0, 1.0)      # smooth inner edge over 10 % of r_in
+    rho = (r_in / Rs) * np.exp(-np.minimum(0.5 * (zp / H) ** 2, 700.0)) * taper
+    p = rho * hr * hr / Rs                                             # c_s = (h/r) v_K
+    return rho, p
+
+
+def tilted_disk(p: dict, seed: int = 3, pert: float = 0.01, beta: float = 10.0, hr: float = 0.03,
+                tilt_deg: float = 65.0, r_in: float = 10.0, r_out: float = 100.0):
+    """cfg 3 stand-in.  Density (R'/r_in)^-1 exp(-z'^2 / 2H^2), H = hr R', between r_in and r_out (tapered);
+    p = rho hr^2 / R'; circular motion Omega = R'^-1.5 about the tilted axis; field from the vector
+    potential A = R'^2.5 p z'-hat (purely toroidal in the disk frame), discrete curl on the grid edges,
+    scaled to p_max / (b^2/2)_max = beta; rho x (1 + pert U) from seed; floors elsewhere.
+    Returns (hydro[5], bface[3])."""
+    a, gam, n = p["a"], p["gamma_ad"], p["n"]
+    tilt = np.deg2rad(tilt_deg)
+    xc, xf, dx = grid_coords(p)
+    cen = [np.exp(xc[0])[:, None, None], xc[1][None, :, None], xc[2][None, None, :]]
+    fac = [np.exp(xf[0])[:, None, None], xf[1][None, :, None], xf[2][None, None, :]]
+    r, th, ph = np.broadcast_arrays(*cen)
+    (x, y, z), ax, Rp, zp = _disk_frame(r, th, ph, tilt)
+    rho_d, p_d = _disk_density(Rp, zp, hr, r_in, r_out)
+    rho_fl = p["rho_fl_coef"] * r ** p["rho_fl_pow"]
+    u_fl = p["u_fl_coef"] * r ** p["u_fl_pow"]
+    inside = rho_d > rho_fl
+    rho = np.where(inside, rho_d, rho_fl)
+    u = np.where(inside, np.maximum(p_d / (gam - 1.0), u_fl), u_fl)
+    # coordinate velocity of the rotation Omega z'-hat x r:  r-dot = 0
+    Om = np.maximum(Rp, r_in) ** -1.5
+    vx, vy, vz = Om * (ax[1] * z - ax[2] * y), Om * (ax[2] * x - ax[0] * z), Om * (ax[0] * y - ax[1] * x)
+    st = np.maximum(np.sin(th), 1e-12)
+    v2 = -vz / (r * st)                                   # theta-dot
+    v3 = (x * vy - y * vx) / np.maximum(x * x + y * y, 1e-30)   # phi-dot
+    g = ks_gcov(a, r, th)
+    nrm = g[..., 0, 0] + 2.0 * g[..., 0, 3] * v3 + g[..., 2, 2] * v2 * v2 + g[..., 3, 3] * v3 * v3
+    ok = inside & (nrm < -1e-6)
+    ut = np.where(ok, 1.0 / np.sqrt(np.maximum(-nrm, 1e-6)), 0.0)
+    alpha, beta1, gdet = ks_lapse_shift(a, r, th)
+    hyd = [rho, u, np.where(ok, ut * beta1, 0.0), np.where(ok, ut * v2, 0.0), np.where(ok, ut * v3, 0.0)]
+    hyd = [np.ascontiguousarray(h) for h in hyd]
+
+    def A_cov(d, rr, tt, pp):      # covariant component d of A = A_z' z'-hat in (ln r, theta, phi)
+        rr, tt, pp = np.broadcast_arrays(rr, tt, pp)
+        _, _, Rq, zq = _disk_frame(rr, tt, pp, tilt)
+        # A_z' = R'^2.5 p: b^2 / p stays bounded in the wings of the Gaussian (a potential ~ sqrt(p) would make
+        # the low-density surface layers magnetically dominated, because surfaces of constant z'/R' flare)
+        Az = Rq ** 2.5 * _disk_density(Rq, zq, hr, r_in, r_out)[1]
+        s, c, sp, cp = np.sin(tt), np.cos(tt), np.sin(pp), np.cos(pp)
+        if d == 0:      # A . d r-vec / d ln r = r A . r-hat
+            return Az * rr * (ax[0] * s * cp + ax[2] * c)
+        if d == 1:      # r A . theta-hat
+            return Az * rr * (ax[0] * c * cp - ax[2] * s)
+        return Az * rr * s * (-ax[0] * sp)                 # r sin(theta) A . phi-hat
+    A1 = A_cov(0, cen[0], fac[1], fac[2])                  # (N1, N2+1, N3+1)
+    A2 = A_cov(1, fac[0], cen[1], fac[2])                  # (N1+1, N2, N3+1)
+    A3 = A_cov(2, fac[0], fac[1], cen[2])                  # (N1+1, N2+1, N3)
+    bface = [(A3[:, 1:, :] - A3[:, :-1, :]) / dx[1] - (A2[:, :, 1:] - A2[:, :, :-1]) / dx[2],
+             (A1[:, :, 1:] - A1[:, :, :-1]) / dx[2] - (A3[1:, :, :] - A3[:-1, :, :]) / dx[0],
+             (A2[1:, :, :] - A2[:-1, :, :]) / dx[0] - (A1[:, 1:, :] - A1[:, :-1, :]) / dx[1]]
+    del A1, A2, A3
+    bface[2][:, :, -1] = bface[2][:, :, 0]                 # periodic images bitwise identical
+    # normalisation: p_max / (b^2 / 2)_max = beta, b^2 from the face-mean field and the disk velocity
+    Bc = [0.5 * (bface[0][1:] + bface[0][:-1]) / gdet, 0.5 * (bface[1][:, 1:] + bface[1][:, :-1]) / gdet,
+          0.5 * (bface[2][:, :, 1:] + bface[2][:, :, :-1]) / gdet]
+    ucon = np.zeros(r.shape + (4,))
+    ucon[..., 0] = np.where(ok, ut, 1.0 / alpha)
+    ucon[..., 1] = np.where(ok, 0.0, -beta1 / alpha)
+    ucon[..., 2] = hyd[3]
+    ucon[..., 3] = hyd[4]
+    ucov = np.einsum("...mn,...n->...m", g, ucon)
+    bt = Bc[0] * ucov[..., 1] + Bc[1] * ucov[..., 2] + Bc[2] * ucov[..., 3]
+    bcon = np.zeros_like(ucon)
+    bcon[..., 0] = bt
+    for i in range(3):
+        bcon[..., 1 + i] = (Bc[i] + bt * ucon[..., 1 + i]) / ucon[..., 0]
+    bsq = np.einsum("...m,...mn,...n->...", bcon, g, bcon)
+    fac_b = np.sqrt(((gam - 1.0) * u).max() / (0.5 * bsq.max() * beta)) if bsq.max() > 0 else 0.0
+    bface = [np.ascontiguousarray(fac_b * b) for b in bface]
+    if pert != 0.0:
+        hyd[0] = hyd[0] * (1.0 + pert * rand_pm1(seed, zone_index(n)))
+    return hyd, bface
