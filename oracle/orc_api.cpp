@@ -18,6 +18,12 @@ static bool params_ok(const Params& p, std::string& why) {
     if ((p.bc_lo[d] == 0) != (p.bc_hi[d] == 0)) { why = "periodic must be set on both sides"; return false; }
   }
   if (p.metric == 1 && !(p.xmin[0] > 0.0)) { why = "r_in <= 0"; return false; }
+  if (p.bc_lo[1] == 3 || p.bc_hi[1] == 3) {   // NEXT-1 transmissive pole
+    if (p.bc_lo[1] != p.bc_hi[1] || p.bc_lo[2] != 0 || p.n[2] % 2 != 0 || (p.nb[2] != 0 && p.nb[2] != p.n[2])) {
+      why = "transmissive poles need both poles, periodic even x3, blocks spanning x3";
+      return false;
+    }
+  }
   if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0)) { why = "gamma_ad/cour"; return false; }
   return true;
 }
@@ -488,3 +494,16 @@ extern "C" void orc_get_fail_hist(long long h4[4]) {
 // number of OpenMP threads the oracle's loops use (reported by bench.py's cpu_baseline leg)
 #include <omp.h>
 extern "C" int orc_omp_threads() { return omp_get_max_threads(); }
+
+// debug access for the boundary pins: fills the ghosts of the single block's current state and returns one
+// full padded array (kind 0..4 hydro, 5..7 Bc, 8..10 Bf), extents n + 2 NG + 1 per dimension, x3 fastest
+extern "C" int orc_get_padded(void* h, int kind, double* out) {
+  Grid& g = *(Grid*)h;
+  if (g.multi || kind < 0 || kind > 10) return 1;
+  Block& b = g.blocks[0];
+  fill_physical_bc(g.par, b, b.sn);
+  compute_Bc(b, b.sn, false);
+  const std::vector<double>& a = kind < 5 ? b.sn.P[kind] : (kind < 8 ? b.sn.Bc[kind - 5] : b.sn.Bf[kind - 8]);
+  std::memcpy(out, a.data(), a.size() * sizeof(double));
+  return 0;
+}

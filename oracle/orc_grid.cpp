@@ -98,11 +98,40 @@ static void fill_dim(const Block& b, std::vector<double>& a, int d, int bc_lo, i
     }
 }
 
+// NEXT-1 transmissive pole: the zone beyond the pole at (theta_ghost = -theta', phi) IS the zone
+// at (theta', phi + pi).  Along the extended meridian the theta basis vector reverses, the r and phi ones do
+// not, so the ghost takes the mirror row's value half a turn away, with the x2 components (ut^2, Bf^2)
+// changing sign; Bf^2 on the pole face is 0 (zero area).  Needs an even N3, a periodic x3 of extent 2 pi and
+// a block that spans x3.  stag2 / stag3: the array is staggered along x2 / x3.
+static void fill_polar_transmit(const Block& b, std::vector<double>& a, bool do_lo, bool do_hi, bool stag2,
+                                bool stag3, double sgn) {
+  const int n2 = b.n[1], n3 = b.n[2], half = n3 / 2;
+  for (int i = -NG; i < b.n[0] + NG + 1; i++)
+    for (int k = -NG; k < n3 + NG + 1; k++) {
+      const int ks = ((k % n3) + n3 + half) % n3;   // a face index n3 is face 0
+      (void)stag3;
+      for (int m = 1; m <= NG; m++) {
+        if (do_lo) a[b.idx(i, -m, k)] = sgn * a[b.idx(i, stag2 ? m : m - 1, ks)];
+        if (do_hi) a[b.idx(i, stag2 ? n2 + m : n2 - 1 + m, k)] = sgn * a[b.idx(i, n2 - m, ks)];
+      }
+      if (stag2) {
+        if (do_lo) a[b.idx(i, 0, k)] = 0.0;
+        if (do_hi) a[b.idx(i, n2, k)] = 0.0;
+      }
+    }
+}
+
 void fill_physical_bc(const Params& par, Block& b, Fields& s) {
   for (int d = 0; d < 3; d++) {  // order x1, x2, x3 so that edge and corner ghosts are defined
     const bool lo = b.phys_lo[d], hi = b.phys_hi[d];
     if (!lo && !hi) continue;
     const int bl = par.bc_lo[d], bh = par.bc_hi[d];
+    if (d == 1 && (bl == 3 || bh == 3)) {
+      // both poles transmissive (a mix with another kind on the other pole is not supported)
+      for (int c = 0; c < 5; c++) fill_polar_transmit(b, s.P[c], lo, hi, false, false, c == 3 ? -1.0 : 1.0);
+      for (int c = 0; c < 3; c++) fill_polar_transmit(b, s.Bf[c], lo, hi, c == 1, c == 2, c == 1 ? -1.0 : 1.0);
+      continue;
+    }
     for (int c = 0; c < 5; c++)
       fill_dim(b, s.P[c], d, bl, bh, lo, hi, false, (c == 2 + d) ? -1.0 : 1.0);
     for (int c = 0; c < 3; c++)

@@ -25,12 +25,22 @@ bool params_ok(const hamr_params& p, std::string& why) {
   for (int d = 0; d < 3; d++) {
     if (p.n[d] < 1) { why = "n[d] < 1"; return false; }
     if (!(p.xmax[d] > p.xmin[d])) { why = "xmax <= xmin"; return false; }
-    if (p.bc_lo[d] < 0 || p.bc_lo[d] > 2 || p.bc_hi[d] < 0 || p.bc_hi[d] > 2) { why = "bad boundary kind"; return false; }
+    if (p.bc_lo[d] < 0 || p.bc_lo[d] > 3 || p.bc_hi[d] < 0 || p.bc_hi[d] > 3) { why = "bad boundary kind"; return false; }
+    if (d != 1 && (p.bc_lo[d] == HAMR_BC_POLAR_TRANSMIT || p.bc_hi[d] == HAMR_BC_POLAR_TRANSMIT)) {
+      why = "the transmissive polar boundary applies to x2 only";
+      return false;
+    }
     if ((p.bc_lo[d] == HAMR_BC_PERIODIC) != (p.bc_hi[d] == HAMR_BC_PERIODIC)) {
       why = "periodic must be set on both sides";
       return false;
     }
     if (p.bc_lo[d] != HAMR_BC_PERIODIC && p.n[d] < NG) { why = "non-periodic dimension needs n >= 3"; return false; }
+  }
+  if (p.bc_lo[1] == HAMR_BC_POLAR_TRANSMIT || p.bc_hi[1] == HAMR_BC_POLAR_TRANSMIT) {
+    if (p.bc_lo[1] != p.bc_hi[1] || p.bc_lo[2] != HAMR_BC_PERIODIC || p.n[2] % 2 != 0 || (p.nb[2] != 0 && p.nb[2] != p.n[2])) {
+      why = "transmissive poles need both poles, a periodic even x3 and blocks that span x3";
+      return false;
+    }
   }
   if (p.metric != HAMR_METRIC_MINKOWSKI && p.metric != HAMR_METRIC_KERR_SCHILD) { why = "bad metric"; return false; }
   if (p.recon != HAMR_RECON_PPM && p.recon != HAMR_RECON_PLM_MC) { why = "bad recon"; return false; }

@@ -41,12 +41,14 @@ __device__ __forceinline__ double ghost_value(const Dev& D, const double* __rest
   bool f0 = false, f1 = false, f2 = false;
   const int si = map_idx(i, L.n[0], D.bc_lo[0], D.bc_hi[0], sd == 0, f0);
   const int sj = map_idx(j, L.n[1], D.bc_lo[1], D.bc_hi[1], sd == 1, f1);
-  const int sk = map_idx(k, L.n[2], D.bc_lo[2], D.bc_hi[2], sd == 2, f2);
+  int sk = map_idx(k, L.n[2], D.bc_lo[2], D.bc_hi[2], sd == 2, f2);
+  // NEXT-1 transmissive pole: the zone beyond the pole is the mirror row's zone half a turn away
+  if (f1 && D.bc_lo[1] == HAMR_BC_POLAR_TRANSMIT) sk = (sk % L.n[2] + L.n[2] / 2) % L.n[2];
   double v = a[L.idx(si, sj, sk)];
   // a reflecting wall carries no normal flux: the wall face itself is 0
-  if (sd == 0 && ((si == 0 && D.bc_lo[0] == HAMR_BC_POLAR_REFLECT) || (si == L.n[0] && D.bc_hi[0] == HAMR_BC_POLAR_REFLECT))) v = 0.0;
-  if (sd == 1 && ((sj == 0 && D.bc_lo[1] == HAMR_BC_POLAR_REFLECT) || (sj == L.n[1] && D.bc_hi[1] == HAMR_BC_POLAR_REFLECT))) v = 0.0;
-  if (sd == 2 && ((sk == 0 && D.bc_lo[2] == HAMR_BC_POLAR_REFLECT) || (sk == L.n[2] && D.bc_hi[2] == HAMR_BC_POLAR_REFLECT))) v = 0.0;
+  if (sd == 0 && ((si == 0 && D.bc_lo[0] >= HAMR_BC_POLAR_REFLECT) || (si == L.n[0] && D.bc_hi[0] >= HAMR_BC_POLAR_REFLECT))) v = 0.0;
+  if (sd == 1 && ((sj == 0 && D.bc_lo[1] >= HAMR_BC_POLAR_REFLECT) || (sj == L.n[1] && D.bc_hi[1] >= HAMR_BC_POLAR_REFLECT))) v = 0.0;
+  if (sd == 2 && ((sk == 0 && D.bc_lo[2] >= HAMR_BC_POLAR_REFLECT) || (sk == L.n[2] && D.bc_hi[2] >= HAMR_BC_POLAR_REFLECT))) v = 0.0;
   const bool neg = (vc == 0 && f0) || (vc == 1 && f1) || (vc == 2 && f2);
   return neg ? -v : v;
 }
@@ -66,7 +68,7 @@ __device__ __forceinline__ void ghost_cell(const Dev& D, const Fields& s, int al
   if (zone_active && !all) {
     // interior: only wall faces of reflecting boundaries need attention
     for (int d = 0; d < 3; d++)
-      if (id[d] == 0 && D.bc_lo[d] == HAMR_BC_POLAR_REFLECT) s.Bf[d][L.idx(i, j, k)] = 0.0;
+      if (id[d] == 0 && D.bc_lo[d] >= HAMR_BC_POLAR_REFLECT) s.Bf[d][L.idx(i, j, k)] = 0.0;
     return;
   }
   const long long z = L.idx(i, j, k);
@@ -80,8 +82,8 @@ __device__ __forceinline__ void ghost_cell(const Dev& D, const Fields& s, int al
     if (extra[o1] || extra[o2]) { lo[d] = hi[d] = 0.0; continue; }
     lo[d] = ghost_value(D, s.Bf[d], d, d, i, j, k);
     const bool face_active = in_c[o1] && in_c[o2] && id[d] >= 0 && id[d] <= L.n[d];
-    const bool wall = face_active && ((id[d] == 0 && D.bc_lo[d] == HAMR_BC_POLAR_REFLECT) ||
-                                      (id[d] == L.n[d] && D.bc_hi[d] == HAMR_BC_POLAR_REFLECT));
+    const bool wall = face_active && ((id[d] == 0 && D.bc_lo[d] >= HAMR_BC_POLAR_REFLECT) ||
+                                      (id[d] == L.n[d] && D.bc_hi[d] >= HAMR_BC_POLAR_REFLECT));
     if (!face_active || wall) s.Bf[d][z] = lo[d];  // ghost_value returns 0 on a reflecting wall
     if (!extra[d]) hi[d] = ghost_value(D, s.Bf[d], d, d, i + (d == 0), j + (d == 1), k + (d == 2));
   }
@@ -150,12 +152,12 @@ void launch_ghosts(hamr_grid* g, const Fields& s, bool all) {
   const Lay& L = g->D.L;
   const int e3 = L.n[2] + 2 * NG + 1;
   Launch l_(g, K_GHOSTS);
-  if (all || g->D.bc_lo[0] == HAMR_BC_POLAR_REFLECT || g->D.bc_lo[2] == HAMR_BC_POLAR_REFLECT) {
+  if (all || g->D.bc_lo[0] >= HAMR_BC_POLAR_REFLECT || g->D.bc_lo[2] >= HAMR_BC_POLAR_REFLECT) {
     const long long tot = (long long)L.e1 * L.e2 * e3;
     k_ghosts<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s, all ? 1 : 0);
     return;
   }
-  const int nj = 2 * NG + 1 + (g->D.bc_lo[1] == HAMR_BC_POLAR_REFLECT ? 1 : 0);
+  const int nj = 2 * NG + 1 + (g->D.bc_lo[1] >= HAMR_BC_POLAR_REFLECT ? 1 : 0);
   const long long rows = (long long)(2 * NG + 1) * L.e2 + (long long)L.n[0] * nj;
   const long long nA = rows * e3;
   const long long tot = nA + (long long)L.n[0] * L.n[1] * 8;

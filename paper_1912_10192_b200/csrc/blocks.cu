@@ -83,9 +83,15 @@ __device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, 
       } else o[d] = 1;
     }
     // a reflecting wall carries no normal flux: the wall face itself is 0
-    if (sd == d && ((m[d] == 0 && (phys & (1 << d)) && Dv.bc_lo[d] == HAMR_BC_POLAR_REFLECT) ||
-                    (m[d] == n && (phys & (8 << d)) && Dv.bc_hi[d] == HAMR_BC_POLAR_REFLECT)))
+    if (sd == d && ((m[d] == 0 && (phys & (1 << d)) && Dv.bc_lo[d] >= HAMR_BC_POLAR_REFLECT) ||
+                    (m[d] == n && (phys & (8 << d)) && Dv.bc_hi[d] >= HAMR_BC_POLAR_REFLECT)))
       s.zero = true;
+  }
+  // NEXT-1 transmissive pole: the mirror row's zone half a turn away in x3 (the block spans x3)
+  if (((s.negmask >> 1) & 1) && Dv.bc_lo[1] == HAMR_BC_POLAR_TRANSMIT) {
+    const int n3 = L.n[2];
+    m[2] = (((id[2] % n3) + n3) % n3 + n3 / 2) % n3;
+    o[2] = 0;
   }
   const int* nb = Dv.B.nbr + b * 27;
   s.ghost = (o[0] | o[1] | o[2]) != 0;

@@ -41,7 +41,7 @@ def zone_index(n) -> np.ndarray:
 # ------------------------------------------------------------------------------------------------
 # parameter sets (plain dicts; each binding packs its own struct)
 # ------------------------------------------------------------------------------------------------
-BC_PERIODIC, BC_OUTFLOW, BC_POLAR = 0, 1, 2
+BC_PERIODIC, BC_OUTFLOW, BC_POLAR, BC_POLAR_TRANSMIT = 0, 1, 2, 3
 METRIC_MINKOWSKI, METRIC_KS = 0, 1
 RECON_PPM, RECON_PLM = 0, 1
 

@@ -217,6 +217,14 @@ class OrcGrid:
         return c
 
     # ---- block-structured grid ----
+    def get_padded(self, kind):
+        """full padded array (ghosts filled) of a monolithic grid: kind 0..4 hydro, 5..7 Bc, 8..10 Bf"""
+        e = tuple(v + 7 for v in self.n)
+        out = np.empty(e)
+        self.L.orc_get_padded.argtypes = [C.c_void_p, C.c_int, c_double_p]
+        assert self.L.orc_get_padded(self.h, int(kind), _dp(out)) == 0
+        return out
+
     def num_blocks(self):
         return self.L.orc_num_blocks(self.h)
 
