@@ -3,7 +3,7 @@
 fraction of the dominant kernel, the end-to-end number through the C-ABI with host buffers, and the
 CPU oracle timed beside it.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg3|cfg4b|cfg4]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg3|cfg4b|cfg4|paper150]
 
 A "step" is one full pass of the hot path over the whole grid: hamr_step(1) = predictor + corrector
 = one zone-cycle per zone.  Default workload: BASELINE.json configs[2], the 256x128x128
@@ -42,6 +42,10 @@ def workload(name):
     if name == "cfg1":
         p = I.minkowski_params(n=(128, 128, 128))
         return p, (lambda: I.minkowski_waves(p, seed=1)), "BASELINE cfg1: Minkowski periodic 128^3 linear waves"
+    if name == "paper150":
+        # the paper's own single-GPU benchmark shape (one 150^3 block, no AMR / SMR / LAT): context
+        p = I.torus_params(n=(150, 150, 150), r_out=1000.0)
+        return p, (lambda: I.fm_torus(p, seed=2)), "paper's single-GPU shape: one 150^3 Kerr-Schild block (FM torus data)"
     if name == "cfg3":
         p = I.tilted_disk_params()
         return p, (lambda: I.tilted_disk(p, seed=3)), ("BASELINE cfg3: tilted thin disk 512x256x256 fp64 (synthetic stand-in: "
@@ -138,6 +142,7 @@ ALG_DOUBLES = {"flux_x1": 16, "flux_x2": 16, "flux_x3": 16,   # 9 r (P5, 2 trans
 NCU_TRAFFIC_SOURCE = "profiles/r1c_ncu_full_cfg2.md"
 NCU_TRAFFIC = {"flux_x1": 612235336, "flux_x2": 594134716, "flux_x3": 537716000, "centre_emf": 318640136, "edge_emf": 535194424, "update_predictor": 1382105232, "update_corrector": 1657781416, "ghosts": 139616240}
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+PAPER_V100_150CUBED = 0.85e8   # ~0.85e8 zone-cycles/s, 1 V100, one 150^3 block
 
 
 def units_per_launch(cls, n):
@@ -405,7 +410,8 @@ def main():
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": (value / PAPER_V100_150CUBED if args.workload == "paper150" else None),
+            "dtype": "f64", "data": "synthetic",
             "config": {"workload": desc, "zones": nz, "blocks": g.num_blocks(), "finest_steps_per_step": fin,
                        "performed_zone_updates_per_sec": performed,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
