@@ -150,3 +150,45 @@ def test_lat_courant_levels_torus(H, orc):
         g.step(2)
         o.step(2)
         _check(p, o, g, TOL_10)
+
+
+def test_block_grid_parameter_and_call_order_errors(H):
+    """error behaviour of the block-structured entry points (include/hamr.h): EINVAL for parameter sets the
+    build does not support, ESTATE for calls out of order; nothing throws, nothing aborts"""
+    base = I.torus_params(n=(32, 16, 16))
+    bad = [dict(nb=(5, 4, 4)),                                                     # does not divide n
+           dict(nb=(2, 4, 4)),                                                     # block smaller than the ghost depth
+           dict(nb=(8, 4, 8), deref_theta_deg=(30.0,), deref_factor=(2,)),         # derefined rows need blocks spanning x3
+           dict(deref_theta_deg=(30.0,), deref_factor=(3,)),                       # factor must divide N3
+           dict(nb=(4, 4, 16), r_refine_max=4.0),                                  # refinement needs nb[0] >= 6
+           dict(r_refine_max=4.0),                                                 # refinement needs a block grid
+           dict(lat_max_level=5),
+           dict(bc_lo=(I.BC_OUTFLOW, I.BC_POLAR_TRANSMIT, I.BC_PERIODIC))]         # transmissive on one pole only
+    for kw in bad:
+        with pytest.raises(H.HamrError) as ei:
+            H.Grid(dict(base, **kw))
+        assert ei.value.code == H.EINVAL, kw
+    g = H.Grid(dict(base, nb=(8, 8, 8), r_refine_max=4.0))
+    hyd, bf = I.fm_torus(base, seed=0)
+    assert g.set_prims(hyd, bf) == H.ESTATE          # a refined grid is set block by block
+    assert g.commit() == H.ESTATE                    # nothing was set
+    with pytest.raises(H.HamrError) as ei:
+        g.step(1)
+    assert ei.value.code == H.ESTATE
+    u = H.Grid(dict(base, nb=(8, 8, 8)))             # unrefined block grid: both ways of setting agree
+    assert u.set_prims(hyd, bf) == 0
+    ref = u.get_prims()
+    v = H.Grid(dict(base, nb=(8, 8, 8)))
+    for b in range(v.num_blocks()):
+        lo, dx, n, _ = v.block_info(b)
+        i0 = [int(round((lo[d] - u.block_info(0)[0][d]) / dx[d])) for d in range(3)]
+        sl = tuple(slice(i0[d], i0[d] + n[d]) for d in range(3))
+        fsl = [tuple(slice(i0[e], i0[e] + n[e] + (e == d)) for e in range(3)) for d in range(3)]
+        assert v.set_block_prims(b, [h[sl] for h in hyd], [bf[d][fsl[d]] for d in range(3)]) == 0
+    assert v.commit() == 0
+    for a, b_ in zip(ref, v.get_prims()):
+        assert np.array_equal(a, b_)
+    got = v.get_block_prims(3)
+    lo, dx, n, _ = v.block_info(3)
+    i0 = [int(round((lo[d] - v.block_info(0)[0][d]) / dx[d])) for d in range(3)]
+    assert np.array_equal(got[0], ref[0][tuple(slice(i0[d], i0[d] + n[d]) for d in range(3))])
