@@ -45,10 +45,13 @@ void blocks_build(Grid& g) {
   }
   if (par.n_deref > 0) {
     // C-15: the strided x3 stencil of a derefined row wraps inside the block
-    if (NB[2] != 1 || par.bc_lo[2] != 0) throw std::runtime_error("phi-derefinement needs blocks that span a periodic x3");
-    for (int t = 0; t < par.n_deref && t < 4; t++)
-      if (par.deref_factor[t] < 1 || par.n[2] % par.deref_factor[t] != 0)
-        throw std::runtime_error("deref factor must divide n3");
+    // C-15: groups never straddle blocks and a ghost depth of 3 groups fits one neighbour; factors are powers of 2
+    if (par.bc_lo[2] != 0) throw std::runtime_error("phi-derefinement needs a periodic x3");
+    for (int t = 0; t < par.n_deref && t < 4; t++) {
+      const int f = par.deref_factor[t];
+      if (f < 1 || (f & (f - 1)) != 0 || nb[2] % f != 0 || nb[2] < 3 * f)
+        throw std::runtime_error("deref factor must be a power of two with 3 factor <= nb[2], dividing it");
+    }
   }
   g.nslot[0] = (int)slots.size(); g.nslot[1] = NB[1]; g.nslot[2] = NB[2];
   g.lattice.assign((size_t)g.nslot[0] * NB[1] * NB[2], -1);
@@ -144,6 +147,13 @@ static void exchange_block(Grid& g, Block& b, Fields& dst, long long s_u) {
           int qi = b.nbr[o[0] + 1][o[1] + 1][o[2] + 1];   // the block itself if no offset
           if (qi < 0) continue;                          // outside the domain: physical boundary
           for (int d = 0; d < 3; d++) lq[d] = id[d] - o[d] * b.n[d];
+          // C-15: the phi-ghost slots of a derefined row are in group units
+          if (o[2] != 0) {
+            // an x2-face array follows the grouping of its face, the coarser of the two rows it separates
+            const int mg = a == 2 ? std::max(b.mrow[std::max(j - 1, -NG) + NG], b.mrow[j + NG]) : b.mrow[j + NG];
+            int o2;
+            if (mg > 1) lq[2] = deref_ghost_k(k, b.n[2], mg, a == 3, o2);
+          }
           // C-17: a face on the plane between two blocks on different time levels has ONE value in
           // every stage source, that of the finer block (own boundary faces included)
           if (a > 0 && (id[a - 1] == 0 || id[a - 1] == b.n[a - 1])) {
@@ -216,7 +226,10 @@ static void exchange_refined(Grid& g, Block& b, Fields& dst, long long s_u) {
           for (int i = lo[0]; i <= hi[0]; i++)
             for (int j = lo[1]; j <= hi[1]; j++)
               for (int k = lo[2]; k <= hi[2]; k++) {
-                const int lj = j - o1 * b.n[1], lk = k - o2 * b.n[2];
+                int o2u;
+                const int lj = j - o1 * b.n[1];
+                const int mg = fd == 1 ? std::max(b.mrow[std::max(j - 1, -NG) + NG], b.mrow[j + NG]) : b.mrow[j + NG];
+                const int lk = o2 != 0 ? deref_ghost_k(k, b.n[2], mg, fd == 2, o2u) : k;
                 const int nk = kind == 0 ? 5 : 1;
                 for (int c = 0; c < nk; c++) {
                   const int kd = kind == 0 ? c : kind;
@@ -289,6 +302,40 @@ static void interface_agreement(Grid& g, int tau) {
   }
 }
 
+// C-15: the x1- and x2-face fluxes of a derefined row in the transverse phi-ghost layer (k = -1 and k = n3;
+// they feed the edge EMFs of C-9 on the block's phi-boundary) must be the phi-neighbour's group means, not
+// this block's own per-zone values: where rows with different factors meet, the mean changes the value.
+// Same-level neighbours only (across time levels the LAT correction makes the shared edges agree).
+static void deref_exchange_flux_layers(Grid& g, int tau) {
+  if (g.par.n_deref <= 0) return;
+  for (Block& b : g.blocks) {
+    if (b.tau != tau) continue;
+    const int n3 = b.n[2];
+    for (int side = 0; side < 2; side++) {
+      const int qi = b.nbr[1][1][side ? 2 : 0];
+      if (qi < 0) continue;
+      const Block& q = g.blocks[qi];
+      if (q.tau != b.tau || q.lev1 != b.lev1) continue;
+      const int kd = side ? n3 : -1, ks = side ? 0 : n3 - 1;
+      for (int i = 0; i <= b.n[0]; i++)
+        for (int j = 0; j <= b.n[1]; j++) {
+          const int m = b.mrow[j + NG], M = std::max(m, b.mrow[j - 1 + NG]);
+          const size_t zd = b.idx(i, j, kd), zs = q.idx(i, j, ks);
+          if (m > 1 && j < b.n[1]) {
+            for (int c = 0; c < 5; c++) b.F[0][c][zd] = q.F[0][c][zs];
+            b.Ef[0][1][zd] = q.Ef[0][1][zs];
+            b.Ef[0][2][zd] = q.Ef[0][2][zs];
+          }
+          if (M > 1 && i < b.n[0]) {
+            for (int c = 0; c < 5; c++) b.F[1][c][zd] = q.F[1][c][zs];
+            b.Ef[1][2][zd] = q.Ef[1][2][zs];
+            b.Ef[1][0][zd] = q.Ef[1][0][zs];
+          }
+        }
+    }
+  }
+}
+
 // ---- one stage of C-12 on every block of one time level ------------------------------------------------
 static void stage_level(Grid& g, int tau, bool corrector) {
   for (Block& b : g.blocks) {
@@ -304,6 +351,11 @@ static void stage_level(Grid& g, int tau, bool corrector) {
     Fields& src = corrector ? b.sh : b.sn;
     flux_pass(g.par, b, src);
     deref_fix_fluxes(g.par, b);
+  }
+  deref_exchange_flux_layers(g, tau);
+  for (Block& b : g.blocks) {
+    if (b.tau != tau) continue;
+    Fields& src = corrector ? b.sh : b.sn;
     ct_edges(g.par, b, src);
     deref_fix_edges(g.par, b);
   }

@@ -107,18 +107,28 @@ static void fill_polar_transmit(const Block& b, std::vector<double>& a, bool do_
                                 bool stag3, double sgn) {
   const int n2 = b.n[1], n3 = b.n[2], half = n3 / 2;
   for (int i = -NG; i < b.n[0] + NG + 1; i++)
-    for (int k = -NG; k < n3 + NG + 1; k++) {
-      const int ks = ((k % n3) + n3 + half) % n3;   // a face index n3 is face 0
-      (void)stag3;
-      for (int m = 1; m <= NG; m++) {
-        if (do_lo) a[b.idx(i, -m, k)] = sgn * a[b.idx(i, stag2 ? m : m - 1, ks)];
-        if (do_hi) a[b.idx(i, stag2 ? n2 + m : n2 - 1 + m, k)] = sgn * a[b.idx(i, n2 - m, ks)];
+    for (int g = 1; g <= NG; g++)
+      for (int side = 0; side < 2; side++) {
+        if (!(side ? do_hi : do_lo)) continue;
+        const int jg = side ? (stag2 ? n2 + g : n2 - 1 + g) : -g;      // the ghost row (or x2-face)
+        const int js = side ? n2 - g : (stag2 ? g : g - 1);            // its mirror image
+        // factor of the SOURCE row's x3 grouping: a phi-ghost slot holds a whole group (C-15); an x2-face
+        // array follows the grouping of its face (the coarser of its two rows)
+        const int m = stag2 ? std::max(b.mrow[js - 1 + NG], b.mrow[js + NG]) : b.mrow[js + NG];
+        for (int k = -NG; k < n3 + NG + 1; k++) {
+          int o2;
+          int kz = deref_ghost_k(k, n3, m, stag3, o2);                // fine x3 index, possibly beyond the block
+          kz = ((kz + o2 * n3) % n3 + n3) % n3;                        // periodic: back into the block
+          const int ks = (kz + half) % n3;                             // half a turn away; face n3 is face 0
+          a[b.idx(i, jg, k)] = sgn * a[b.idx(i, js, ks)];
+        }
       }
-      if (stag2) {
+  if (stag2)
+    for (int i = -NG; i < b.n[0] + NG + 1; i++)
+      for (int k = -NG; k < n3 + NG + 1; k++) {
         if (do_lo) a[b.idx(i, 0, k)] = 0.0;
         if (do_hi) a[b.idx(i, n2, k)] = 0.0;
       }
-    }
 }
 
 void fill_physical_bc(const Params& par, Block& b, Fields& s) {
@@ -152,9 +162,20 @@ void compute_Bc(const Block& b, Fields& s, bool active_only) {
         const size_t z = b.idx(i, j, k);
         for (int d = 0; d < 3; d++)
           s.Bc[d][z] = (s.Bf[d][z] + s.Bf[d][z + str[d]]) / (2.0 * g);
-        if (m > 1) {
+        if (k < 0 || k >= n3) {
+          // a phi-ghost slot holds a whole group of THIS row; the two x2-faces of the zone are stored in the
+          // grouping of their own faces
+          const int Mlo = std::max(b.mrow[std::max(j - 1, -NG) + NG], m);
+          const int Mhi = std::max(m, b.mrow[std::min(j + 1, b.n[1] + NG) + NG]);
+          if (Mlo != m || Mhi != m) {
+            const double flo = s.Bf[1][b.idx(i, j, deref_face2_slot(k, n3, m, Mlo))];
+            const double fhi = s.Bf[1][b.idx(i, j + 1, deref_face2_slot(k, n3, m, Mhi))];
+            s.Bc[1][z] = (flo + fhi) / (2.0 * g);
+          }
+        } else if (m > 1) {
           // C-15 (iii): in a derefined row B_c^3 is the GROUP's value, from the group's two outer x3-faces
-          const int kk = ((k % n3) + n3) % n3, k0 = kk - kk % m;
+          // (a phi-ghost zone holds a whole group and its two ghost faces are that group's outer faces)
+          const int k0 = k - k % m;
           s.Bc[2][z] = (s.Bf[2][b.idx(i, j, k0)] + s.Bf[2][b.idx(i, j, k0 + m)]) / (2.0 * g);
         }
       }
@@ -225,7 +246,7 @@ static void face_flux(const Params& par, Block& b, const Fields& s, int d, int i
 }
 
 // C-15 (ii): x3-face on a group boundary of a phi-derefined row (k a multiple of m): the stencil takes
-// one value per GROUP, i.e. zones k + t m, t = -3..2, wrapped periodically (the block spans all of x3).
+// one value per GROUP, i.e. zones k + t m, t = -3..2; beyond the block the phi-ghost zones hold groups.
 static void face_flux_x3_deref(const Params& par, Block& b, const Fields& s, int i, int j, int k, int m,
                                double* ctop) {
   const size_t z = b.idx(i, j, k);
@@ -235,7 +256,9 @@ static void face_flux_x3_deref(const Params& par, Block& b, const Fields& s, int
   double st6[7][6];
   for (int v = 0; v < 7; v++)
     for (int t = 0; t < 6; t++) {
-      const int kk = (((k + (t - 3) * m) % n3) + n3) % n3;
+      int kk = k + (t - 3) * m;                      // first zone of the group, in fine zones
+      if (kk < 0) kk = kk / m;                       // groups beyond the low edge: ghost zones -1, -2, -3
+      else if (kk >= n3) kk = n3 + (kk - n3) / m;    // beyond the high edge: ghost zones n3, n3 + 1, n3 + 2
       st6[v][t] = var[v][b.idx(i, j, kk)];
     }
   face_flux_core(par, b, s, 2, i, j, z, st6, ctop);
@@ -281,16 +304,20 @@ static inline int face2_factor(const Block& b, int j) {  // x2-face j lies betwe
   return std::max(b.mrow[j - 1 + NG], b.mrow[j + NG]);
 }
 
+// pairwise (tree) sum of m = 2^p values: the mean of m IDENTICAL values is then that value exactly, so group
+// quantities that are already uniform are left bit-for-bit alone (blocks that share a group boundary stay
+// consistent)
+static double tree_sum(const double* v, int m) {
+  if (m == 1) return v[0];
+  return tree_sum(v, m / 2) + tree_sum(v + m / 2, m / 2);
+}
+
 static void group_mean(std::vector<double>& a, const Block& b, int i, int j, int m) {
   const int n3 = b.n[2];
   for (int k0 = 0; k0 < n3; k0 += m) {
-    double sum = 0.0;
-    for (int r = 0; r < m; r++) sum += a[b.idx(i, j, k0 + r)];
-    const double mean = sum / (double)m;
+    const double mean = tree_sum(&a[b.idx(i, j, k0)], m) / (double)m;
     for (int r = 0; r < m; r++) a[b.idx(i, j, k0 + r)] = mean;
   }
-  a[b.idx(i, j, -1)] = a[b.idx(i, j, n3 - 1)];  // the periodic transverse ghost layer (feeds C-9)
-  a[b.idx(i, j, n3)] = a[b.idx(i, j, 0)];
 }
 
 static void group_interp(std::vector<double>& a, const Block& b, int i, int j, int m) {
@@ -338,7 +365,7 @@ void deref_fix_edges(const Params& par, Block& b) {
       if (M > 1) {                                         // E3 at (i-1/2, j-1/2, k)
         for (int k0 = 0; k0 < n3; k0 += M) {
           double sum = 0.0;
-          for (int r = 0; r < M; r++) sum += b.Ee[2][b.idx(i, j, k0 + r)];
+          sum = tree_sum(&b.Ee[2][b.idx(i, j, k0)], M);
           for (int r = 0; r < M; r++) b.Ee[2][b.idx(i, j, k0 + r)] = sum / (double)M;
         }
       }
@@ -348,18 +375,30 @@ void deref_fix_edges(const Params& par, Block& b) {
 }
 
 // C-15 (v): one inversion per group: the group's first member's result is the group's
+// The whole invariant (i) is re-imposed EXACTLY after every update: hydro and B_c of a group are its first
+// member's; Bf1 (row grouping) and Bf2 (the coarser grouping of the two rows of its face) likewise; Bf3 on
+// in-group faces is re-interpolated from the group's outer faces.  The update leaves all of these true to
+// round-off only (the interpolated EMFs differ in the last bit between members); making them exact keeps
+// neighbouring blocks, which recompute shared faces from copies of each other's groups, bit-for-bit
+// consistent, and costs div B nothing beyond round-off that does not accumulate.
 void deref_sync_groups(const Params& par, Block& b, Fields& s) {
   if (par.n_deref <= 0) return;
-  for (int i = 0; i < b.n[0]; i++)
-    for (int j = 0; j < b.n[1]; j++) {
-      const int m = b.mrow[j + NG];
-      if (m <= 1) continue;
+  for (int i = 0; i <= b.n[0]; i++)
+    for (int j = 0; j <= b.n[1]; j++) {
+      const int m = b.mrow[j + NG], M = face2_factor(b, j);
       for (int k = 0; k < b.n[2]; k++) {
-        if (k % m == 0) continue;
-        const size_t z = b.idx(i, j, k), z0 = b.idx(i, j, k - k % m);
-        for (int c = 0; c < 5; c++) s.P[c][z] = s.P[c][z0];
-        for (int c = 0; c < 3; c++) s.Bc[c][z] = s.Bc[c][z0];
+        const size_t z = b.idx(i, j, k);
+        if (m > 1 && k % m != 0 && j < b.n[1]) {
+          const size_t z0 = b.idx(i, j, k - k % m);
+          s.Bf[0][z] = s.Bf[0][z0];
+          if (i < b.n[0]) {
+            for (int c = 0; c < 5; c++) s.P[c][z] = s.P[c][z0];
+            for (int c = 0; c < 3; c++) s.Bc[c][z] = s.Bc[c][z0];
+          }
+        }
+        if (M > 1 && k % M != 0 && i < b.n[0]) s.Bf[1][z] = s.Bf[1][b.idx(i, j, k - k % M)];
       }
+      if (m > 1 && i < b.n[0] && j < b.n[1]) group_interp(s.Bf[2], b, i, j, m);
     }
 }
 
@@ -375,13 +414,13 @@ void deref_project(const Params& par, Block& b, Fields& s) {
       if (i < b.n[0]) {
         for (int c = 0; c < 5; c++)
           for (int k0 = 0; k0 < b.n[2]; k0 += m) {
-            double sum = 0.0;
-            for (int r = 0; r < m; r++) sum += s.P[c][b.idx(i, j, k0 + r)];
+            const double sum = tree_sum(&s.P[c][b.idx(i, j, k0)], m);
             for (int r = 0; r < m; r++) s.P[c][b.idx(i, j, k0 + r)] = sum / (double)m;
           }
         group_interp(s.Bf[2], b, i, j, m);
       }
     }
+  deref_sync_groups(par, b, s);   // Bf1, Bf2 onto their first member as well
 }
 
 // ---- constrained transport (C-8, C-9) -------------------------------------------------------------

@@ -87,6 +87,26 @@ void ct_edges(const Params& par, Block& b, const Fields& src);
 void update(const Params& par, Block& b, const Fields& src, const Fields& base, Fields& out,
             double dt, Stats& st);
 double dt_from_ctop(const Params& par, const Block& b);
+// C-15: the phi-ghost slots of a row with factor m are in GROUP units: ghost zone -g holds group -g (the
+// neighbour's zones n3 - g m ...), ghost zone n3 - 1 + g holds group g - 1 beyond the edge (the neighbour's zone
+// (g - 1) m); ghost x3-faces likewise hold group-boundary faces.  Returns the neighbour offset o2 and the x3
+// index inside the neighbour.  m = 1: the ordinary ghost zones.  Needs n3 >= 3 m.
+inline int deref_ghost_k(int k, int n3, int m, bool face3, int& o2) {
+  const int hi = face3 ? n3 : n3 - 1;
+  if (k < 0) { o2 = -1; return n3 + k * m; }
+  if (k > hi) { o2 = 1; return face3 ? (k - n3) * m : (k - n3) * m; }
+  o2 = 0;
+  return k;
+}
+// C-15: an x2-face array (Bf2) follows the grouping of its FACE (the coarser of the two rows it separates), so
+// its phi-ghost slots are in units of that grouping.  A zone row with factor m whose ghost slot k holds one of
+// ITS groups finds the face value that covers that group in this slot of the face array with grouping M >= m.
+inline int deref_face2_slot(int k, int n3, int m, int M) {
+  if (M == m) return k;
+  if (k < 0) { const int g = -k; return -((g * m + M - 1) / M); }     // group -g of the row lies in face group -ceil(g m / M)
+  if (k >= n3) { const int g = k - n3; return n3 + (g * m) / M; }     // group g beyond the edge: face group floor(g m / M)
+  return k;
+}
 // C-15 phi-derefinement (orc_grid.cpp)
 int deref_factor_of_row(const Params& par, long long J);
 void deref_fix_fluxes(const Params& par, Block& b);

@@ -59,10 +59,10 @@ def test_p14_deref_everywhere_is_the_coarse_phi_grid(orc, m):
 
 
 def test_p14_axisymmetric_data_do_not_notice(orc):
-    p0 = I.torus_params(n=(16, 16, 8))
+    p0 = I.torus_params(n=(16, 16, 16))
     p1 = dict(p0, deref_theta_deg=(30.0, 12.0), deref_factor=(2, 4))
     hyd, bf = I.fm_torus(p0, seed=0, pert=0.0)   # no phi-dependent perturbation
-    a, b = orc.OrcGrid(dict(p0, nb=(16, 16, 8))), orc.OrcGrid(p1)
+    a, b = orc.OrcGrid(dict(p0, nb=(16, 16, 16))), orc.OrcGrid(p1)
     assert a.set_prims(hyd, bf) == 0 and b.set_prims(hyd, bf) == 0
     assert b.dt > a.dt                       # the derefined polar rows no longer set the Courant step
     for _ in range(3):
@@ -126,3 +126,38 @@ def test_p14_torus_mixed_rows_with_blocks_and_lat(orc):
     g.step(2)
     _group_checks(g.get_prims(), g.get_bface(), mrow)
     assert g.divb() <= 1e-12 and g.stats()[0] == 0
+
+
+def test_p14_blocks_that_cut_phi_equal_blocks_that_span_it_bitwise(orc):
+    """phi-ghost zones of derefined rows are held in GROUP units and the group invariants are exact, so a grid whose
+    blocks cut x3 (BASELINE cfg 4's 16^3 blocks) reproduces the phi-spanning decomposition bit for bit, shared
+    faces included; mixed rows (m = 4, 2, 1), phi-dependent data"""
+    n = (8, 16, 32)
+    res = []
+    for nb in ((8, 16, 32), (4, 8, 16), (8, 4, 16)):
+        p = I.minkowski_params(n=n, nb=nb, deref_theta_deg=(45.0, 22.6), deref_factor=(2, 4))
+        hyd, bf = I.minkowski_waves(p, seed=1, amp=2e-2, noise=1e-2)
+        bf = [np.full_like(b, v) for b, v in zip(bf, (1.0, np.sqrt(2.0), 0.5))]
+        g = orc.OrcGrid(p)
+        assert g.set_prims(hyd, bf) == 0
+        t0 = g.totals()
+        g.step(5)
+        assert np.abs(g.totals() - t0).max() / max(t0[0], abs(t0[1])) < 1e-13
+        assert g.divb() <= 1e-12 and g.bface_mismatch() == 0.0
+        res.append(g.get_prims() + g.get_bface())
+    for r in res[1:]:
+        for a, b in zip(res[0], r):
+            assert np.array_equal(a, b)
+
+
+def test_p14_phi_cut_blocks_torus_with_lat(orc):
+    p = I.torus_params(n=(32, 16, 32), nb=(8, 4, 16), lat_max_level=1, deref_theta_deg=(30.0, 12.0), deref_factor=(2, 4))
+    hyd, bf = I.fm_torus(p, seed=4)
+    a, b = orc.OrcGrid(p), orc.OrcGrid(dict(p, nb=(8, 4, 32)))
+    assert a.set_prims(hyd, bf) == 0 and b.set_prims(hyd, bf) == 0
+    a.step(2)
+    b.step(2)
+    assert len(set(a.levels())) == 2
+    for x, y in zip(a.get_prims() + a.get_bface(), b.get_prims() + b.get_bface()):
+        assert np.array_equal(x, y)
+    assert a.divb() <= 1e-12 and a.bface_mismatch() == 0.0 and a.stats()[0] == 0
