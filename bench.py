@@ -58,13 +58,13 @@ def workload(name):
         return p, (lambda: I.fm_torus(p, seed=4)), ("BASELINE cfg4 without r-refinement: Kerr FM torus 256x128x128 in 16x16x128 "
                                                      "blocks, phi-derefinement 2x/4x, LAT levels 1/2/4")
     if name == "cfg4":
-        # BASELINE cfg 4 with blocks that span phi: 16 x 16 x 128 blocks, phi-derefined 2x / 4x
-        # within 15 / 5 degrees of the poles, one x1 refinement level for r < 20 (184 blocks, 6 029 312 zones),
-        # LAT levels 1, 2, 4; torus data sampled per block, seed 4.  gen() returns the per-block data.
-        p = I.torus_params(n=(256, 128, 128), r_out=1000.0, nb=(16, 16, 128), lat_max_level=2, r_refine_max=20.0,
+        # BASELINE cfg 4: base 256x128x128 in 16^3 blocks, phi-derefined 2x / 4x within 15 / 5
+        # degrees of the poles, one x1 refinement level for r < 20 (1472 blocks, 6 029 312 zones), LAT levels 1, 2, 4;
+        # torus data sampled per block, seed 4.  gen() returns the per-block data.
+        p = I.torus_params(n=(256, 128, 128), r_out=1000.0, nb=(16, 16, 16), lat_max_level=2, r_refine_max=20.0,
                            deref_theta_deg=(15.0, 5.0), deref_factor=(2, 4))
         return p, (lambda infos: I.fm_torus_blocks(p, infos, seed=4)), ("BASELINE cfg4: Kerr FM torus, base 256x128x128 in "
-                   "16x16x128 blocks, one x1 refinement level r<20, phi-derefinement 2x/4x, LAT levels 1/2/4")
+                   "16^3 blocks (1472), one x1 refinement level r<20, phi-derefinement 2x/4x, LAT levels 1/2/4")
     raise SystemExit(f"unknown workload {name}")
 
 

@@ -51,9 +51,15 @@ bool params_ok(const hamr_params& p, std::string& why) {
   if (p.n_deref > 0) {
     // C-15: the strided x3 stencil of a derefined row wraps inside the grid / block
     if (p.bc_lo[2] != HAMR_BC_PERIODIC) { why = "phi-derefinement needs a periodic x3"; return false; }
-    if (p.nb[2] != 0 && p.nb[2] != p.n[2]) { why = "phi-derefinement needs blocks that span x3"; return false; }
-    for (int t = 0; t < p.n_deref; t++)
-      if (p.deref_factor[t] < 1 || p.n[2] % p.deref_factor[t] != 0) { why = "deref factor must divide n3"; return false; }
+    // groups never straddle blocks and a ghost depth of 3 groups fits one neighbour; factors are powers of two
+    const int nb3 = p.nb[2] > 0 ? p.nb[2] : p.n[2];
+    for (int t = 0; t < p.n_deref; t++) {
+      const int f = p.deref_factor[t];
+      if (f < 1 || f > 16 || (f & (f - 1)) != 0 || nb3 % f != 0 || nb3 < 3 * f) {
+        why = "deref factor must be a power of two <= 16 that divides nb[2], with 3 factor <= nb[2]";
+        return false;
+      }
+    }
   }
   if (p.lat_max_level < 0 || p.lat_max_level > 3) { why = "lat_max_level must be 0..3"; return false; }
   if (is_block_grid(p)) {
@@ -357,6 +363,7 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
     blk_check_finite(g);
   } else {
     launch_deref_project(g, g->D, sn, sn);
+    launch_deref_sync(g, g->D, sn, sn);
     launch_ghosts(g, sn, true);
     launch_flux(g, sn, true);   // C-14: one flux pass sets dt of step 0
     launch_dt(g, 0);

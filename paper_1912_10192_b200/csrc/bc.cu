@@ -42,6 +42,12 @@ __device__ __forceinline__ double ghost_value(const Dev& D, const double* __rest
   const int si = map_idx(i, L.n[0], D.bc_lo[0], D.bc_hi[0], sd == 0, f0);
   const int sj = map_idx(j, L.n[1], D.bc_lo[1], D.bc_hi[1], sd == 1, f1);
   int sk = map_idx(k, L.n[2], D.bc_lo[2], D.bc_hi[2], sd == 2, f2);
+  if (D.mrow && D.bc_lo[2] == HAMR_BC_PERIODIC && (k < 0 || k > (sd == 2 ? L.n[2] : L.n[2] - 1))) {
+    // C-15: the phi-ghost slots of a derefined row hold whole groups; an x2-face array follows its face's grouping
+    const int mj = __ldg(D.mrow + j + NG);
+    const int mg = sd == 1 ? max(mj, __ldg(D.mrow + max(j - 1, -NG) + NG)) : mj;
+    if (mg > 1) sk = deref_ghost_k(k, L.n[2], mg);
+  }
   // NEXT-1 transmissive pole: the zone beyond the pole is the mirror row's zone half a turn away
   if (f1 && D.bc_lo[1] == HAMR_BC_POLAR_TRANSMIT) sk = (sk % L.n[2] + L.n[2] / 2) % L.n[2];
   double v = a[L.idx(si, sj, sk)];
@@ -89,12 +95,20 @@ __device__ __forceinline__ void ghost_cell(const Dev& D, const Fields& s, int al
   }
   if (zone_slot) {
     const double g = __ldg(D.gc + GDET * L.n2d + L.idx2(i, j));
-    if (D.mrow && __ldg(D.mrow + j + NG) > 1) {
-      // C-15: B_c^3 of a phi-derefined row is the group's value, from the group's two outer x3-faces
+    if (D.mrow) {
       const int m = __ldg(D.mrow + j + NG), n3 = L.n[2];
-      const int kk = ((k % n3) + n3) % n3, k0 = kk - kk % m;
-      lo[2] = ghost_value(D, s.Bf[2], 2, 2, i, j, k0);
-      hi[2] = ghost_value(D, s.Bf[2], 2, 2, i, j, k0 + m);
+      if (k >= 0 && k < n3) {
+        if (m > 1) {   // C-15: B_c^3 of a phi-derefined row is the group's value, from the group's two outer x3-faces
+          const int k0 = k - k % m;
+          lo[2] = ghost_value(D, s.Bf[2], 2, 2, i, j, k0);
+          hi[2] = ghost_value(D, s.Bf[2], 2, 2, i, j, k0 + m);
+        }
+      } else {
+        // a phi-ghost slot holds a whole group of THIS row; its two x2-faces are stored in their faces' groupings
+        const int Mlo = max(m, __ldg(D.mrow + max(j - 1, -NG) + NG)), Mhi = max(m, __ldg(D.mrow + min(j + 1, L.n[1] + NG) + NG));
+        if (Mlo != m) lo[1] = ghost_value(D, s.Bf[1], 1, 1, i, j, deref_face2_slot(k, n3, m, Mlo));
+        if (Mhi != m) hi[1] = ghost_value(D, s.Bf[1], 1, 1, i, j + 1, deref_face2_slot(k, n3, m, Mhi));
+      }
     }
     for (int d = 0; d < 3; d++) s.Bc[d][z] = (lo[d] + hi[d]) / (2.0 * g);
   }

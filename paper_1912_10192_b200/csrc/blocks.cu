@@ -87,16 +87,24 @@ __device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, 
                     (m[d] == n && (phys & (8 << d)) && Dv.bc_hi[d] >= HAMR_BC_POLAR_REFLECT)))
       s.zero = true;
   }
+  // C-15: the phi-ghost slots of a derefined row hold whole groups; an x2-face array follows its face's grouping
+  int kz = m[2] - o[2] * L.n[2];            // x3 index inside the block that holds the value
+  if (Dv.mrow && o[2] != 0) {
+    const int J = Dv.B.info[b].w + id[1];
+    const int mj = __ldg(Dv.mrow + J + NG);
+    const int mg = sd == 1 ? max(mj, __ldg(Dv.mrow + max(J - 1, -NG) + NG)) : mj;
+    if (mg > 1) kz = deref_ghost_k(id[2], L.n[2], mg);
+  }
   // NEXT-1 transmissive pole: the mirror row's zone half a turn away in x3 (the block spans x3)
   if (((s.negmask >> 1) & 1) && Dv.bc_lo[1] == HAMR_BC_POLAR_TRANSMIT) {
     const int n3 = L.n[2];
-    m[2] = (((id[2] % n3) + n3) % n3 + n3 / 2) % n3;
+    kz = (kz % n3 + n3 / 2) % n3;
     o[2] = 0;
   }
   const int* nb = Dv.B.nbr + b * 27;
   s.ghost = (o[0] | o[1] | o[2]) != 0;
   s.q = s.ghost ? __ldg(nb + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1)) : b;
-  int lq[3] = {m[0] - o[0] * L.n[0], m[1] - o[1] * L.n[1], m[2] - o[2] * L.n[2]};
+  int lq[3] = {m[0] - o[0] * L.n[0], m[1] - o[1] * L.n[1], kz};
   // C-17: a face on the plane between two blocks on different time levels has ONE value in every stage
   // source, that of the finer block
   if (!norule && sd >= 0 && (m[sd] == 0 || m[sd] == L.n[sd])) {
@@ -109,7 +117,7 @@ __device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, 
       s.ghost = true;
     }
   }
-  s.mod = s.ghost || s.zero || (sd >= 0 && ((s.negmask >> sd) & 1)) || m[0] != id[0] || m[1] != id[1] || m[2] != id[2];
+  s.mod = s.ghost || s.zero || (sd >= 0 && ((s.negmask >> sd) & 1)) || m[0] != id[0] || m[1] != id[1] || kz != id[2];
   s.zl = (int)L.idx(lq[0], lq[1], lq[2]);
   s.ref = false;
   if (!norule && o[0] != 0 && s.q >= 0 && Dv.B.info[s.q].y != Dv.B.info[b].y) {
@@ -273,6 +281,14 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
     const Fields& fo = own == 0 ? B.s[0] : (own == 1 ? B.s[1] : B.s[2]);
     double vP[5], vB[3], vF[3];
     bool wF[3];
+    // C-15: phi-ghost slots of derefined rows are in group units (x2-face arrays: their face's grouping)
+    int mj = 1, Mj = 1;
+    if (Dv.mrow && oc[2] != 0) {
+      const int J = Dv.B.info[b].w + id[1];
+      mj = __ldg(Dv.mrow + J + NG);
+      Mj = max(mj, __ldg(Dv.mrow + max(J - 1, -NG) + NG));
+      if (mj > 1) lc[2] = deref_ghost_k(id[2], L.n[2], mj);
+    }
     if (zone_slot) {
       const int q = __ldg(nb + (oc[0] + 1) * 9 + (oc[1] + 1) * 3 + (oc[2] + 1));
       const int bq = role == 0 ? Dv.B.cur[q] : 1;
@@ -287,6 +303,7 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
     for (int d = 0; d < 3; d++) {
       const int o1 = (d + 1) % 3, o2 = (d + 2) % 3;
       int of[3] = {oc[0], oc[1], oc[2]}, lf[3] = {lc[0], lc[1], lc[2]};
+      if (d == 1 && oc[2] != 0 && Mj > 1) lf[2] = deref_ghost_k(id[2], L.n[2], Mj);
       if (id[d] == L.n[d]) { of[d] = 0; lf[d] = id[d]; }    // the block's own high face
       wF[d] = shell1[o1] && shell1[o2] && id[d] >= 0 && id[d] <= L.n[d] && (of[0] | of[1] | of[2]) != 0;
       vF[d] = 0.0;
@@ -370,18 +387,38 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
   if (zone_slot && (!zone_active || all || anymod)) {
     const int4 inf = __ldg(Dv.B.info + b);
     const double g = __ldg(Dv.gc + inf.y * Dv.B.tlev + GDET * L.n2d + inf.x + id[0] * Dv.B.ge2 + id[1]);
-    if (Dv.mrow && __ldg(Dv.mrow + inf.w + id[1] + NG) > 1) {
-      // C-15: B_c^3 of a phi-derefined row is the group's value (the block spans all of x3)
-      const int m = __ldg(Dv.mrow + inf.w + id[1] + NG), n3 = L.n[2];
-      const int kk = ((id[2] % n3) + n3) % n3, k0 = kk - kk % m;
-      int ig[3] = {id[0], id[1], k0};
-      GSrc s = blk_src(Dv, b, phys, 2, ig, same);
-      if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
-      lo[2] = fetch(7, s);
-      ig[2] = k0 + m;
-      s = blk_src(Dv, b, phys, 2, ig, same);
-      if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
-      hi[2] = fetch(7, s);
+    if (Dv.mrow) {
+      const int J = inf.w + id[1], n3 = L.n[2];
+      const int m = __ldg(Dv.mrow + J + NG);
+      if (id[2] >= 0 && id[2] < n3) {
+        if (m > 1) {   // C-15: B_c^3 of a phi-derefined row is the group's value, from the group's two outer x3-faces
+          const int k0 = id[2] - id[2] % m;
+          int ig[3] = {id[0], id[1], k0};
+          GSrc s = blk_src(Dv, b, phys, 2, ig, same);
+          if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
+          lo[2] = fetch(7, s);
+          ig[2] = k0 + m;
+          s = blk_src(Dv, b, phys, 2, ig, same);
+          if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
+          hi[2] = fetch(7, s);
+        }
+      } else {
+        // a phi-ghost slot holds a whole group of THIS row; its two x2-faces are stored in their faces' groupings
+        const int Mlo = max(m, __ldg(Dv.mrow + max(J - 1, -NG) + NG));
+        const int Mhi = max(m, __ldg(Dv.mrow + min(J + 1, Dv.B.n2g + NG) + NG));
+        if (Mlo != m) {
+          int ig[3] = {id[0], id[1], deref_face2_slot(id[2], n3, m, Mlo)};
+          const GSrc s = blk_src(Dv, b, phys, 1, ig, same);
+          if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
+          lo[1] = fetch(6, s);
+        }
+        if (Mhi != m) {
+          int ig[3] = {id[0], id[1] + 1, deref_face2_slot(id[2], n3, m, Mhi)};
+          const GSrc s = blk_src(Dv, b, phys, 1, ig, same);
+          if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
+          hi[1] = fetch(6, s);
+        }
+      }
     }
 #pragma unroll
     for (int d = 0; d < 3; d++) {
@@ -1259,6 +1296,7 @@ int blk_initial(hamr_grid* g) {
     return HAMR_ECUDA;
   const Dev D = dev_list(g, 4);
   launch_deref_project(g, D, g->s[0], g->s[2]);
+  launch_deref_sync(g, D, g->s[0], g->s[2]);
   blk_ghosts(g, D, 0, 0, true, true);
   launch_flux_on(g, D, g->s[0], g->s[2], true);
   return blk_assign(g, false);

@@ -55,15 +55,16 @@ __device__ __forceinline__ DIdx deref_idx(const Dev& Dv, int ilo, int ihi, int j
   return r;
 }
 
-// group mean in place (members z0 .. z0 + m - 1), summed in member order; wrap: also the periodic
-// transverse ghost layer (k = -1 <- n3 - 1, k = n3 <- 0), which feeds the edge EMFs of C-9
-__device__ __forceinline__ void group_mean(double* __restrict__ a, long long zrow, int k0, int m, int n3, bool wrap) {
-  double sum = 0.0;
-  for (int r = 0; r < m; r++) sum += a[zrow + k0 + r];
-  const double mean = sum / (double)m;
+// group mean in place (members z0 .. z0 + m - 1, m a power of two <= 16) by a pairwise (tree) sum: the mean of
+// m IDENTICAL values is then that value exactly, so quantities that are already uniform in the group are left
+// bit-for-bit alone and blocks that recompute a shared value from copies of each other's groups agree
+__device__ __forceinline__ void group_mean(double* __restrict__ a, long long zrow, int k0, int m) {
+  double v[16];
+  for (int r = 0; r < m; r++) v[r] = a[zrow + k0 + r];
+  for (int w = 1; w < m; w *= 2)
+    for (int r = 0; r + w < m; r += 2 * w) v[r] = v[r] + v[r + w];
+  const double mean = v[0] / (double)m;
   for (int r = 0; r < m; r++) a[zrow + k0 + r] = mean;
-  if (wrap && k0 == 0) a[zrow + n3] = mean;
-  if (wrap && k0 + m == n3) a[zrow - 1] = mean;
 }
 
 // members 1 .. m-1 become the linear interpolation of the values at k0 and k0 + m
@@ -85,9 +86,9 @@ __global__ void __launch_bounds__(128) k_deref_fix_flux(Dev Dv) {
   if (m > 1 && k % m == 0) {
     if (i >= 0) {                      // x1-faces of the row
 #pragma unroll
-      for (int c = 0; c < 5; c++) group_mean(Dv.F[0][c], zrow, k, m, n3, true);
-      group_mean(Dv.EfA[0], zrow, k, m, n3, true);
-      group_mean(Dv.EfB[0], zrow, k, m, n3, true);
+      for (int c = 0; c < 5; c++) group_mean(Dv.F[0][c], zrow, k, m);
+      group_mean(Dv.EfA[0], zrow, k, m);
+      group_mean(Dv.EfB[0], zrow, k, m);
     }
 #pragma unroll
     for (int c = 0; c < 5; c++) group_interp(Dv.F[2][c], zrow, k, m);   // x3-faces inside the group
@@ -96,9 +97,9 @@ __global__ void __launch_bounds__(128) k_deref_fix_flux(Dev Dv) {
   }
   if (j >= 0 && M > 1 && k % M == 0) {  // x2-face on the low side of row j
 #pragma unroll
-    for (int c = 0; c < 5; c++) group_mean(Dv.F[1][c], zrow, k, M, n3, true);
-    group_mean(Dv.EfA[1], zrow, k, M, n3, true);
-    group_mean(Dv.EfB[1], zrow, k, M, n3, true);
+    for (int c = 0; c < 5; c++) group_mean(Dv.F[1][c], zrow, k, M);
+    group_mean(Dv.EfA[1], zrow, k, M);
+    group_mean(Dv.EfB[1], zrow, k, M);
   }
 }
 
@@ -113,26 +114,81 @@ __global__ void __launch_bounds__(128) k_deref_fix_edges(Dev Dv) {
   const int M = max(m, __ldg(Dv.mrow + T.C.J0 + j - 1 + NG));
   const long long zrow = T.C.zoff + L.idx(i, j, 0);
   if (M > 1 && k % M == 0) {
-    group_mean(Dv.Ee[2], zrow, k, M, n3, false);                 // E3 at (i-1/2, j-1/2, k)
+    group_mean(Dv.Ee[2], zrow, k, M);                            // E3 at (i-1/2, j-1/2, k)
     if (i < L.n[0]) group_interp(Dv.Ee[0], zrow, k, M);          // E1 at (i, j-1/2, k-1/2)
   }
   if (m > 1 && k % m == 0 && j < L.n[1]) group_interp(Dv.Ee[1], zrow, k, m);   // E2 at (i-1/2, j, k-1/2)
 }
 
-// C-15 (v): one inversion per group: the first member's primitives and B_c are the group's
+// C-15 (v) and (i): one inversion per group, and the whole invariant re-imposed EXACTLY after every update: the
+// first member's primitives and B_c are the group's; Bf1 (row grouping) and Bf2 (the grouping of its face)
+// likewise; Bf3 on in-group faces is re-interpolated from the group's outer faces.  The update leaves these true
+// to round-off only; exactness keeps blocks that cut x3 bit-for-bit consistent on the faces they share and
+// costs div B nothing beyond round-off that does not accumulate.
 template <bool BLK>
 __global__ void __launch_bounds__(128) k_deref_sync(Dev Dv, Fields o0, Fields o2) {
   const Lay& L = Dv.L;
-  const DIdx T = deref_idx<BLK>(Dv, 0, 0, 0, 0);
+  const DIdx T = deref_idx<BLK>(Dv, 0, 1, 0, 1);     // i in [0, n1], j in [0, n2]: the high faces included
   if (!T.valid) return;
-  const int m = __ldg(Dv.mrow + T.C.J0 + T.j + NG);
-  const int r = T.k % m;
-  if (m == 1 || r == 0) return;
-  const long long z = T.C.zoff + L.idx(T.i, T.j, T.k);
+  const int i = T.i, j = T.j, k = T.k;
+  const int m = __ldg(Dv.mrow + T.C.J0 + j + NG);
+  const int M = max(m, __ldg(Dv.mrow + T.C.J0 + j - 1 + NG));
+  const long long z = T.C.zoff + L.idx(i, j, k);
+  const int r = k % m, R = k % M;
+  if (m > 1 && r != 0 && j < L.n[1]) {
+    { double* a = selp<BLK>(o0.Bf[0], o2.Bf[0], T.C.cur); a[z] = a[z - r]; }
+    if (i < L.n[0]) {
 #pragma unroll
-  for (int c = 0; c < 5; c++) { double* a = selp<BLK>(o0.P[c], o2.P[c], T.C.cur); a[z] = a[z - r]; }
+      for (int c = 0; c < 5; c++) { double* a = selp<BLK>(o0.P[c], o2.P[c], T.C.cur); a[z] = a[z - r]; }
 #pragma unroll
-  for (int c = 0; c < 3; c++) { double* a = selp<BLK>(o0.Bc[c], o2.Bc[c], T.C.cur); a[z] = a[z - r]; }
+      for (int c = 0; c < 3; c++) { double* a = selp<BLK>(o0.Bc[c], o2.Bc[c], T.C.cur); a[z] = a[z - r]; }
+      double* a = selp<BLK>(o0.Bf[2], o2.Bf[2], T.C.cur);
+      const double lo = a[z - r], hi = a[z - r + m];
+      a[z] = lo + ((double)r / (double)m) * (hi - lo);
+    }
+  }
+  if (M > 1 && R != 0 && i < L.n[0]) { double* a = selp<BLK>(o0.Bf[1], o2.Bf[1], T.C.cur); a[z] = a[z - R]; }
+}
+
+// C-15 (iii): the x1- and x2-face values of derefined rows in the transverse phi-ghost layer (k = -1, k = n3; they
+// feed the edge EMFs of C-9 on the phi-boundary) are the phi-NEIGHBOUR's group means, not this block's own
+// per-zone values: where rows with different factors meet, the mean changes the value.  Same-level neighbours
+// only (across time levels the LAT correction makes shared edges agree); a monolithic grid wraps onto itself.
+template <bool BLK>
+__global__ void __launch_bounds__(128) k_deref_flux_layers(Dev Dv) {
+  const Lay& L = Dv.L;
+  const int c1 = L.n[1] + 1;
+  const unsigned per = 2u * (L.n[0] + 1) * c1;
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (BLK ? per * Dv.B.nact : per)) return;
+  int bslot = 0;
+  if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
+  const BCtx C = blk_ctx<BLK>(Dv, bslot);
+  const int side = (int)(t & 1);
+  t >>= 1;
+  const int j = (int)(t % (unsigned)c1), i = (int)(t / (unsigned)c1), n3 = L.n[2];
+  const int m = __ldg(Dv.mrow + C.J0 + j + NG);
+  const int M = max(m, __ldg(Dv.mrow + C.J0 + j - 1 + NG));
+  if (M == 1) return;
+  int q = C.b;
+  if (BLK) {
+    q = __ldg(Dv.B.nbr + C.b * 27 + 12 + (side ? 2 : 0));       // offset (0, 0, -1) / (0, 0, +1)
+    if (q < 0 || Dv.B.tau[q] != Dv.B.tau[C.b] || Dv.B.info[q].y != C.lev) return;
+  }
+  const long long zd = C.zoff + L.idx(i, j, side ? n3 : -1);
+  const long long zs = (BLK ? (long long)q * Dv.B.blen : 0) + L.idx(i, j, side ? 0 : n3 - 1);
+  if (m > 1 && j < L.n[1]) {
+#pragma unroll
+    for (int c = 0; c < 5; c++) Dv.F[0][c][zd] = Dv.F[0][c][zs];
+    Dv.EfA[0][zd] = Dv.EfA[0][zs];
+    Dv.EfB[0][zd] = Dv.EfB[0][zs];
+  }
+  if (i < L.n[0]) {
+#pragma unroll
+    for (int c = 0; c < 5; c++) Dv.F[1][c][zd] = Dv.F[1][c][zs];
+    Dv.EfA[1][zd] = Dv.EfA[1][zs];
+    Dv.EfB[1][zd] = Dv.EfB[1][zs];
+  }
 }
 
 // C-15 (i): puts an initial state onto the invariant: hydro primitives -> group mean, x3-face field between
@@ -146,7 +202,7 @@ __global__ void __launch_bounds__(128) k_deref_project(Dev Dv, Fields s0, Fields
   if (m == 1 || T.k % m != 0) return;
   const long long zrow = T.C.zoff + L.idx(T.i, T.j, 0);
 #pragma unroll
-  for (int c = 0; c < 5; c++) group_mean(selp<BLK>(s0.P[c], s2.P[c], T.C.cur), zrow, T.k, m, L.n[2], false);
+  for (int c = 0; c < 5; c++) group_mean(selp<BLK>(s0.P[c], s2.P[c], T.C.cur), zrow, T.k, m);
   group_interp(selp<BLK>(s0.Bf[2], s2.Bf[2], T.C.cur), zrow, T.k, m);
 }
 
@@ -163,6 +219,15 @@ void launch_deref_fix_flux(hamr_grid* g, const Dev& Dv) {
   else k_deref_fix_flux<false><<<nb, 128, 0, g->stream>>>(Dv);
 }
 
+void launch_deref_flux_layers(hamr_grid* g, const Dev& Dv) {
+  if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
+  Launch l_(g, K_OTHER);
+  const long long tot = 2LL * (Dv.L.n[0] + 1) * (Dv.L.n[1] + 1) * (Dv.B.nblk > 0 ? Dv.B.nact : 1);
+  const unsigned nb = (unsigned)((tot + 127) / 128);
+  if (Dv.B.nblk > 0) k_deref_flux_layers<true><<<nb, 128, 0, g->stream>>>(Dv);
+  else k_deref_flux_layers<false><<<nb, 128, 0, g->stream>>>(Dv);
+}
+
 void launch_deref_fix_edges(hamr_grid* g, const Dev& Dv) {
   if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
   Launch l_(g, K_OTHER);
@@ -174,7 +239,7 @@ void launch_deref_fix_edges(hamr_grid* g, const Dev& Dv) {
 void launch_deref_sync(hamr_grid* g, const Dev& Dv, const Fields& out, const Fields& out2) {
   if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
   Launch l_(g, K_OTHER);
-  const unsigned nb = nblocks_for(Dv, Dv.L.n[0], Dv.L.n[1]);
+  const unsigned nb = nblocks_for(Dv, Dv.L.n[0] + 1, Dv.L.n[1] + 1);
   if (Dv.B.nblk > 0) k_deref_sync<true><<<nb, 128, 0, g->stream>>>(Dv, out, out2);
   else k_deref_sync<false><<<nb, 128, 0, g->stream>>>(Dv, out, out2);
 }

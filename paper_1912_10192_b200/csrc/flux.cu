@@ -389,7 +389,7 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
 // ---- C-15 (ii): x3-faces of phi-derefined rows -----------------------------------------------------------
 // "PPM ... modified for the increased cell spacing".  In a row with factor m the flux exists on
 // group-boundary faces only (k a multiple of m); its stencil takes one value per group, zones k + t m,
-// t = -3..2, wrapped periodically (the grid or block spans all of x3); the Courant limit uses m dx3.
+// t = -3..2 (beyond the block the phi-ghost zones hold groups, C-15); the Courant limit uses m dx3.
 // One thread per group-boundary face; rows with m = 1 return at once.
 template <int RECON, bool BLK>
 __global__ void __launch_bounds__(128) k_deref_x3(Dev Dv, Fields s, Fields s2, int want_ctop) {
@@ -414,11 +414,11 @@ __global__ void __launch_bounds__(128) k_deref_x3(Dev Dv, Fields s, Fields s2, i
                             selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),
                             selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[0], s2.Bc[0], C.cur),
                             selp<BLK>(s.Bc[1], s2.Bc[1], C.cur)};
-    int kk[6];
+    int kk[6];   // beyond the block the phi-ghost zones hold whole groups: -1, -2, -3 and n3, n3 + 1, n3 + 2
 #pragma unroll
     for (int q = 0; q < 6; q++) {
-      int w = (k + (q - 3) * m) % n3;
-      kk[q] = w < 0 ? w + n3 : w;
+      const int w = k + (q - 3) * m;
+      kk[q] = w < 0 ? w / m : (w >= n3 ? n3 + (w - n3) / m : w);
     }
     double PL[8], PR[8];
 #pragma unroll
@@ -534,6 +534,7 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
   if (Dv.mrow) {  // C-15: strided x3 fluxes of the derefined rows, then the group structure on all face values
     launch_deref_x3(g, Dv, src, src2, want_ctop);
     launch_deref_fix_flux(g, Dv);
+    launch_deref_flux_layers(g, Dv);
   }
 }
 

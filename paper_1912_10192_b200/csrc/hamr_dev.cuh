@@ -282,4 +282,18 @@ __device__ __forceinline__ void floors_ceiling(const Geo& G, double rfl, double 
   }
 }
 
+// ---- C-15: phi-ghost slots of derefined rows are in GROUP units -------------------------------------------
+// x3 index inside the periodic neighbour that ghost slot k of an array whose row (or x2-face) has grouping mg
+// holds: ghost zone -g is group -g (the neighbour's zone n3 - g mg), ghost zone n3 - 1 + g is group g - 1 beyond the
+// edge (its zone (g - 1) mg); x3-faces likewise hold group-boundary faces.  k must lie outside the block.
+__device__ __forceinline__ int deref_ghost_k(int k, int n3, int mg) { return k < 0 ? n3 + k * mg : (k - n3) * mg; }
+// An x2-face array follows the grouping M of its FACE (the coarser of its two rows).  A zone row with factor m whose
+// ghost slot k holds one of ITS groups finds the covering face value in this slot of the face array.
+__device__ __forceinline__ int deref_face2_slot(int k, int n3, int m, int M) {
+  if (M == m) return k;
+  if (k < 0) return -((-k * m + M - 1) / M);
+  if (k >= n3) return n3 + ((k - n3) * m) / M;
+  return k;
+}
+
 }  // namespace hamr

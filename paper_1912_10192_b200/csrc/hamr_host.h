@@ -197,6 +197,7 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
 // deref.cu / flux.cu: phi-derefinement (C-15)
 void launch_deref_x3(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop);
 void launch_deref_fix_flux(hamr_grid* g, const Dev& Dv);
+void launch_deref_flux_layers(hamr_grid* g, const Dev& Dv);
 void launch_deref_fix_edges(hamr_grid* g, const Dev& Dv);
 void launch_deref_sync(hamr_grid* g, const Dev& Dv, const Fields& out, const Fields& out2);
 void launch_deref_project(hamr_grid* g, const Dev& Dv, const Fields& s, const Fields& s2);

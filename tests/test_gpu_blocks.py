@@ -158,7 +158,7 @@ def test_block_grid_parameter_and_call_order_errors(H):
     base = I.torus_params(n=(32, 16, 16))
     bad = [dict(nb=(5, 4, 4)),                                                     # does not divide n
            dict(nb=(2, 4, 4)),                                                     # block smaller than the ghost depth
-           dict(nb=(8, 4, 8), deref_theta_deg=(30.0,), deref_factor=(2,)),         # derefined rows need blocks spanning x3
+           dict(nb=(8, 4, 8), deref_theta_deg=(30.0,), deref_factor=(4,)),         # 3 groups of ghosts must fit one neighbour
            dict(deref_theta_deg=(30.0,), deref_factor=(3,)),                       # factor must divide N3
            dict(nb=(4, 4, 16), r_refine_max=4.0),                                  # refinement needs nb[0] >= 6
            dict(r_refine_max=4.0),                                                 # refinement needs a block grid

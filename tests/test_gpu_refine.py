@@ -108,13 +108,13 @@ def test_refined_torus(H, orc, extra):
 
 
 def test_cfg4_full_size_one_coarse_step(H, orc):
-    """BASELINE cfg 4 at full size in the launch configuration bench.py --workload cfg4 times (184 blocks of
-    16x16x128, 6 029 312 zones, refinement r < 20, derefinement 2x / 4x, LAT levels 1 / 2 / 4): every zone of every
-    block after one coarse step (= 4 finest steps) against the oracle."""
-    p = I.torus_params(n=(256, 128, 128), r_out=1000.0, nb=(16, 16, 128), lat_max_level=2, r_refine_max=20.0,
+    """BASELINE cfg 4 at full size in the launch configuration bench.py --workload cfg4 times (1472 blocks of 16^3,
+    6 029 312 zones, refinement r < 20, derefinement 2x / 4x, LAT levels 1 / 2 / 4): every zone of every block after one
+    coarse step (= 4 finest steps) against the oracle."""
+    p = I.torus_params(n=(256, 128, 128), r_out=1000.0, nb=(16, 16, 16), lat_max_level=2, r_refine_max=20.0,
                        deref_theta_deg=(15.0, 5.0), deref_factor=(2, 4))
     g, o = H.Grid(p), orc.OrcGrid(p)
-    assert g.num_blocks() == o.num_blocks() == 184
+    assert g.num_blocks() == o.num_blocks() == 1472
     infos = _infos(o)
     assert sum(int(np.prod(n)) for _, _, n in infos) == 6029312
     _set_both(g, o, I.fm_torus_blocks(p, infos, seed=4))
