@@ -138,7 +138,9 @@ int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int
  * (piecewise linear in x1, MC-limited); the coarse block takes the fine block's interface fluxes and EMFs.
  * A refined grid has no global zone array: its state is set and read block by block.  Arrays are dense,
  * block-local, x3 fastest: hydro[c] nb0*nb1*nb2, bface[d] with nb[d]+1 along d (NULL = 0); the caller keeps
- * them.  After the last hamr_set_block_prims, hamr_blocks_commit fills ghosts, projects onto the
+ * them and, unlike with the other host calls, must leave them UNCHANGED until hamr_blocks_commit has returned
+ * (the copies of all blocks are queued on the stream and waited for once, in commit; with 1472 blocks a wait
+ * per block would dominate).  After the last hamr_set_block_prims, hamr_blocks_commit fills ghosts, projects onto the
  * derefinement invariant, and finds the first dt and time levels (HAMR_ENONFINITE on NaN/Inf input).
  * Also valid on unrefined block grids. */
 int hamr_set_block_prims(hamr_grid* g, int b, const double* const hydro[5], const double* const bface[3]);

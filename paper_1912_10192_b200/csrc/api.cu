@@ -2,6 +2,7 @@
 // The time integrator is the 2nd-order predictor/corrector of PAPER.md:41, 141 (C-12):
 //   predictor: src = base = state n,  dt/2 -> n+1/2 ;  corrector: src = n+1/2, base = n, dt -> n+1,
 // each stage = ghost fill -> reconstruct+HLL x3 -> CT EMFs -> B update + source + update + inversion.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -117,6 +118,10 @@ ArenaPlan plan_arena(const hamr_params& p, const Lay& L, const GridShape& G) {
   a.scal = off; off += 256;
   a.cnt = off; off += 256;
   a.stage_doubles = (size_t)8 * (p.n[0] + 1) * (p.n[1] + 1) * (p.n[2] + 1);
+  // block-by-block state: every block has its own staging slot, so hamr_set_block_prims need not wait for the
+  // previous block's copies (the stream is synchronised once, in hamr_blocks_commit)
+  if (G.nblk > 0)
+    a.stage_doubles = std::max(a.stage_doubles, (size_t)G.nblk * 8 * (L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1));
   a.stage = off; off += align_up(a.stage_doubles * 8, 256);
   a.blk = off; off += G.nblk > 0 ? blk_table_bytes(G.nblk) : 0;
   a.mrow = off; off += p.n_deref > 0 ? align_up((size_t)G.te2 * sizeof(int), 256) : 0;
@@ -572,7 +577,7 @@ int hamr_set_block_prims(hamr_grid* g, int b, const double* const hydro[5], cons
     g->have_state = false;
   }
   const size_t nz = (size_t)L.n[0] * L.n[1] * L.n[2];
-  size_t off = 0;
+  size_t off = (size_t)b * 8 * (L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);   // the block's own staging slot
   for (int c = 0; c < 5; c++) {
     double* st = g->stage + off;
     CK(cudaMemcpyAsync(st, hydro[c], nz * 8, cudaMemcpyHostToDevice, g->stream));
@@ -592,7 +597,8 @@ int hamr_set_block_prims(hamr_grid* g, int b, const double* const hydro[5], cons
     }
     blk_pack_one(g, b, src, 5 + d, d, d == 1);
   }
-  CK(cudaStreamSynchronize(g->stream));   // the staging area is reused by the next call
+  // the caller's arrays may be pageable: cudaMemcpyAsync from pageable memory returns only after the data
+  // have been staged, so they may be reused on return; the device side completes before hamr_blocks_commit returns
   return HAMR_OK;
 }
 
