@@ -52,6 +52,7 @@ struct GSrc {
   bool ghost;   // sampled from a neighbour (else read from b's own active storage)
   bool zero;    // a reflecting wall face: the value is 0
   bool mod;     // differs from what b's own storage holds at id[]
+  bool moved;   // a physical-boundary map changed the index (outflow copy, mirror, half turn)
   // C-16: the neighbour is on the other x1 refinement level: the value is a restriction / prolongation
   bool ref;
   int rq;       // the block on b's own side of the interface in the same transverse position
@@ -117,6 +118,7 @@ __device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, 
       s.ghost = true;
     }
   }
+  s.moved = m[0] != id[0] || m[1] != id[1] || m[2] != id[2] || s.negmask != 0;
   s.mod = s.ghost || s.zero || (sd >= 0 && ((s.negmask >> sd) & 1)) || m[0] != id[0] || m[1] != id[1] || kz != id[2];
   s.zl = (int)L.idx(lq[0], lq[1], lq[2]);
   s.ref = false;
@@ -225,6 +227,9 @@ __device__ __forceinline__ double blk_fetch(const Dev& Dv, const Bufs& B, int b,
   return (vc >= 0 && ((s.negmask >> vc) & 1)) ? -v : v;
 }
 
+#ifndef HAMR_GHOST_MINB
+#define HAMR_GHOST_MINB 5  // 48 registers; 2 / 3 (104 / 80 registers, no spills) measured 12 % / 3 % slower on cfg 4: occupancy wins
+#endif
 // Ghost fill of the stage source of every listed block: neighbour exchange with time interpolation
 // (C-16, C-17), physical boundaries (C-12), cell-centred B wherever a face changed (C-10).
 // role: 0 the source is the block's time-n state, 1 its predictor state.  all: also derive B_c on the
@@ -232,7 +237,7 @@ __device__ __forceinline__ double blk_fetch(const Dev& Dv, const Bufs& B, int b,
 // Block flags (host, per level assignment): bit 0 "simple": no physical side and all 26 neighbours on
 // the block's own time level -> every ghost value (B_c included) is a plain copy of the neighbour's
 // stage source; bit 1: some neighbour is on a finer time level (only then can an ACTIVE face change).
-__global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, int role, long long s_u, int all,
+__global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, int role, long long s_u, int all,
                                                     int zero_ctop) {
   // grid: x covers the padded locations of one block, y the blocks of the launch; 32-bit index arithmetic
   const Lay& L = Dv.L;
@@ -348,13 +353,25 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
     return blk_qtime(Dv, lt, q, s_u);
   };
   // loads first, stores last (see the fast path)
-  double vP[5];
+  double vP[5], vB[3];
   const bool wP = zone_slot && !zone_active;
+  // pure: a ghost zone that is simply a same-level neighbour's zone (no boundary map, no refinement, no time
+  // interpolation): its B_c is the neighbour's own B_c (same faces, same geometry), which saves the six face
+  // look-ups that would rebuild it.  Safe for the reason the fast path is: every block touching the zones read
+  // here is a neighbour of b on b's own level, so none of them rewrites those zones in this launch.
+  bool pure = false;
   if (wP) {
     const GSrc s = blk_src(Dv, b, phys, -1, id, same);
     if (s.ghost) { qt = qtime(s.q); lastq = s.q; }
 #pragma unroll
     for (int c = 0; c < 5; c++) vP[c] = fetch(c, s);
+    pure = same && !all && s.ghost && !s.ref && !s.moved && !s.zero;
+    if (pure) {
+      const Fields& fq = qt.b0 == 0 ? B.s[0] : (qt.b0 == 1 ? B.s[1] : B.s[2]);
+      const long long zq = (long long)s.q * Dv.B.blen + s.zl;
+#pragma unroll
+      for (int d = 0; d < 3; d++) vB[d] = fq.Bc[d][zq];
+    }
   }
   double lo[3], hi[3];
   bool wF[3] = {false, false, false};
@@ -363,12 +380,14 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
   for (int d = 0; d < 3; d++) {
     const int o1 = (d + 1) % 3, o2 = (d + 2) % 3;
     if (extra[o1] || extra[o2]) { lo[d] = hi[d] = 0.0; continue; }
+    const bool face_read = shell1[o1] && shell1[o2] && id[d] >= 0 && id[d] <= L.n[d];   // a flux kernel reads this face
+    if (pure && !face_read) { lo[d] = hi[d] = 0.0; continue; }
     GSrc s = blk_src(Dv, b, phys, d, id, same);
     if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
     lo[d] = fetch(5 + d, s);
-    if (s.mod) { wF[d] = shell1[o1] && shell1[o2] && id[d] >= 0 && id[d] <= L.n[d]; anymod = true; }
+    if (s.mod) { wF[d] = face_read; anymod = true; }
     hi[d] = 0.0;
-    if (!extra[d]) {
+    if (!extra[d] && !pure) {
       int idp[3] = {id[0], id[1], id[2]};
       idp[d] += 1;
       s = blk_src(Dv, b, phys, d, idp, same);
@@ -384,7 +403,13 @@ __global__ void __launch_bounds__(256, 4) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, 
 #pragma unroll
   for (int d = 0; d < 3; d++)
     if (wF[d]) const_cast<double*>(buf_arr(B, own, 5 + d))[z] = lo[d];
-  if (zone_slot && (!zone_active || all || anymod)) {
+  if (pure) {
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+      double* bc = own == 0 ? B.s[0].Bc[d] : (own == 1 ? B.s[1].Bc[d] : B.s[2].Bc[d]);
+      bc[z] = vB[d];
+    }
+  } else if (zone_slot && (!zone_active || all || anymod)) {
     const int4 inf = __ldg(Dv.B.info + b);
     const double g = __ldg(Dv.gc + inf.y * Dv.B.tlev + GDET * L.n2d + inf.x + id[0] * Dv.B.ge2 + id[1]);
     if (Dv.mrow) {
