@@ -326,22 +326,19 @@ def main():
     C = hamr.C
     L = hamr.lib()
     if refined:
-        hh = [pin(h) for hb, fb in bdata for h in hb]
-        bh = [pin(f) for hb, fb in bdata for f in fb]
+        # every block in one call: the per-block arrays back to back (hamr_set_all_blocks / hamr_get_all_blocks)
+        hh = [pin(np.stack([hb[c] for hb, fb in bdata])) for c in range(5)]
+        bh = [pin(np.stack([fb[c] for hb, fb in bdata])) for c in range(3)]
         nbk = g.num_blocks()
-        outs = [torch.empty(infos[b][2], dtype=torch.float64).pin_memory().numpy() for b in range(nbk) for _ in range(8)]
-        hps = [(hamr.c_double_p * 5)(*[hamr._dp(h) for h in hh[5 * b:5 * b + 5]]) for b in range(nbk)]
-        bps = [(hamr.c_double_p * 3)(*[hamr._dp(f) for f in bh[3 * b:3 * b + 3]]) for b in range(nbk)]
-        ops = [(hamr.c_double_p * 8)(*[hamr._dp(o) for o in outs[8 * b:8 * b + 8]]) for b in range(nbk)]
+        outs = [torch.empty((nbk,) + tuple(infos[0][2]), dtype=torch.float64).pin_memory().numpy() for _ in range(8)]
+        hp = (hamr.c_double_p * 5)(*[hamr._dp(h) for h in hh])
+        bp = (hamr.c_double_p * 3)(*[hamr._dp(f) for f in bh])
+        op = (hamr.c_double_p * 8)(*[hamr._dp(o) for o in outs])
 
         def e2e_step():
-            rc = 0
-            for b in range(nbk):
-                rc |= L.hamr_set_block_prims(g.h, b, hps[b], bps[b])
-            rc |= L.hamr_blocks_commit(g.h)
+            rc = L.hamr_set_all_blocks(g.h, hp, bp)
             rc |= L.hamr_step(g.h, 1, None, None)
-            for b in range(nbk):
-                rc |= L.hamr_get_block_prims(g.h, b, ops[b])
+            rc |= L.hamr_get_all_blocks(g.h, op)
             assert rc == 0, rc
     else:
         hh = [pin(h) for h in hyd]
@@ -419,7 +416,7 @@ def main():
                        "timing": "CUDA events on the launching (torch current) stream"},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": args.e2e_steps, "what": ("hamr_set_block_prims x blocks + hamr_blocks_commit + hamr_step(1) + hamr_get_block_prims x blocks"
+                    "steps": args.e2e_steps, "what": ("hamr_set_all_blocks + hamr_step(1) + hamr_get_all_blocks"
                              if refined else "hamr_set_prims(host) + hamr_step(1) + hamr_get_prims(host)") + ", pinned buffers"},
             "gpu_launches": launches,
             "roofline": roof, "cpu_baseline": cpu}

@@ -146,6 +146,11 @@ int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int
 int hamr_set_block_prims(hamr_grid* g, int b, const double* const hydro[5], const double* const bface[3]);
 int hamr_blocks_commit(hamr_grid* g);
 int hamr_get_block_prims(hamr_grid* g, int b, double* const prims[8]);   /* 5 hydro + cell-centred B^i */
+/* Every block in one call (8 large copies instead of 8 per block): each array holds the per-block dense arrays of
+ * the calls above back to back in block order.  hamr_set_all_blocks includes the commit and copies before it
+ * returns; hamr_get_all_blocks fills prims (NULL entries skipped) and synchronises. */
+int hamr_set_all_blocks(hamr_grid* g, const double* const hydro[5], const double* const bface[3]);
+int hamr_get_all_blocks(hamr_grid* g, double* const prims[8]);
 int hamr_get_block_bface(hamr_grid* g, int b, double* const bface[3]);
 /* Test hook: prescribes the LAT level of every block (tau[hamr_num_blocks], clamped to
  * 0..lat_max_level, then lowered until neighbours differ by at most one); NULL restores the

@@ -602,6 +602,55 @@ int hamr_set_block_prims(hamr_grid* g, int b, const double* const hydro[5], cons
   return HAMR_OK;
 }
 
+// every block in one call: the per-block arrays of hamr_set_block_prims back to back in block order
+int hamr_set_all_blocks(hamr_grid* g, const double* const hydro[5], const double* const bface[3]) {
+  if (!g || !g->bh.on || !hydro) return HAMR_EINVAL;
+  if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
+  for (int c = 0; c < 5; c++) if (!hydro[c]) return fail(g, HAMR_EINVAL, "hydro[c] is NULL");
+  const Lay& L = g->D.L;
+  const size_t nb = (size_t)g->bh.nblk;
+  CK(cudaMemsetAsync(g->D.B.cur, 0, nb * sizeof(int), g->stream));
+  g->have_state = false;
+  const size_t nz = (size_t)L.n[0] * L.n[1] * L.n[2] * nb;
+  size_t off = 0;
+  for (int c = 0; c < 5; c++) {
+    double* st = g->stage + off;
+    CK(cudaMemcpyAsync(st, hydro[c], nz * 8, cudaMemcpyHostToDevice, g->stream));
+    blk_pack_one(g, -1, st, c, -1, false);
+    off += nz;
+  }
+  for (int d = 0; d < 3; d++) {
+    int m[3] = {L.n[0], L.n[1], L.n[2]};
+    m[d] += 1;
+    const size_t nf = (size_t)m[0] * m[1] * m[2] * nb;
+    const double* src = (bface && bface[d]) ? bface[d] : nullptr;
+    if (src) {
+      double* st = g->stage + off;
+      CK(cudaMemcpyAsync(st, src, nf * 8, cudaMemcpyHostToDevice, g->stream));
+      src = st;
+      off += nf;
+    }
+    blk_pack_one(g, -1, src, 5 + d, d, d == 1);
+  }
+  g->blocks_open = true;
+  return hamr_blocks_commit(g);
+}
+
+int hamr_get_all_blocks(hamr_grid* g, double* const prims[8]) {
+  if (!g || !g->bh.on || !prims) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  const Lay& L = g->D.L;
+  const size_t nz = (size_t)L.n[0] * L.n[1] * L.n[2] * g->bh.nblk;
+  for (int c = 0; c < 8; c++) {
+    if (!prims[c]) continue;
+    double* st = g->stage + (size_t)c * nz;
+    blk_unpack_one(g, -1, c, st);
+    CK(cudaMemcpyAsync(prims[c], st, nz * 8, cudaMemcpyDeviceToHost, g->stream));
+  }
+  CK(cudaStreamSynchronize(g->stream));
+  return HAMR_OK;
+}
+
 int hamr_blocks_commit(hamr_grid* g) {
   if (!g || !g->bh.on) return HAMR_EINVAL;
   if (!g->blocks_open) return fail(g, HAMR_ESTATE, "hamr_blocks_commit without hamr_set_block_prims");

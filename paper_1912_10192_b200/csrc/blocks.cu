@@ -865,14 +865,18 @@ __global__ void __launch_bounds__(256) k_blk_pack1(Dev Dv, int b, const double* 
   const Lay& L = Dv.L;
   int m[3] = {L.n[0], L.n[1], L.n[2]};
   if (stag >= 0) m[stag] += 1;
-  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= (unsigned)(m[0] * m[1] * m[2])) return;
+  // b < 0: every block, the dense arrays of the blocks back to back in block order
+  const unsigned per = (unsigned)(m[0] * m[1] * m[2]);
+  const unsigned tg = blockIdx.x * blockDim.x + threadIdx.x;
+  if (tg >= (b < 0 ? per * (unsigned)Dv.B.nblk : per)) return;
+  unsigned t = tg;
+  if (b < 0) { b = (int)(tg / per); t = tg - (unsigned)b * per; }
   const unsigned tj = t / (unsigned)m[2], ti = tj / (unsigned)m[1];
   const int k = (int)(t - tj * m[2]), j = (int)(tj - ti * m[1]), i = (int)ti;
   double* a = Dv.B.cur[b] ? s2 : s0;
   const long long z = (long long)b * Dv.B.blen + L.idx(i, j, k);
-  if (unpack) { const_cast<double*>(dense)[t] = a[z]; return; }
-  double v = dense ? dense[t] : 0.0;
+  if (unpack) { const_cast<double*>(dense)[tg] = a[z]; return; }
+  double v = dense ? dense[tg] : 0.0;
   const int J = Dv.B.info[b].w + j;
   if (zero_pole && Dv.metric == HAMR_METRIC_KERR_SCHILD && (J == 0 || J == Dv.B.n2g)) v = 0.0;
   a[z] = v;
@@ -1095,11 +1099,11 @@ void blk_pack_one(hamr_grid* g, int b, const double* dense, int kind, int stag, 
   const Lay& L = g->D.L;
   int m[3] = {L.n[0], L.n[1], L.n[2]};
   if (stag >= 0) m[stag] += 1;
-  const int tot = m[0] * m[1] * m[2];
+  const long long tot = (long long)m[0] * m[1] * m[2] * (b < 0 ? g->bh.nblk : 1);
   double* a0 = kind < 5 ? g->s[0].P[kind] : g->s[0].Bf[kind - 5];
   double* a2 = kind < 5 ? g->s[2].P[kind] : g->s[2].Bf[kind - 5];
   Launch l_(g, K_OTHER);
-  k_blk_pack1<<<(tot + 255) / 256, 256, 0, g->stream>>>(g->D, b, dense, a0, a2, stag, zero_pole ? 1 : 0, 0);
+  k_blk_pack1<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, b, dense, a0, a2, stag, zero_pole ? 1 : 0, 0);
 }
 
 void blk_unpack_one(hamr_grid* g, int b, int kind, double* dense) {
@@ -1107,13 +1111,13 @@ void blk_unpack_one(hamr_grid* g, int b, int kind, double* dense) {
   const int stag = kind >= 8 ? kind - 8 : -1;
   int m[3] = {L.n[0], L.n[1], L.n[2]};
   if (stag >= 0) m[stag] += 1;
-  const int tot = m[0] * m[1] * m[2];
+  const long long tot = (long long)m[0] * m[1] * m[2] * (b < 0 ? g->bh.nblk : 1);
   auto arr = [&](int buf) -> double* {
     const Fields& f = g->s[buf];
     return kind < 5 ? f.P[kind] : (kind < 8 ? f.Bc[kind - 5] : f.Bf[kind - 8]);
   };
   Launch l_(g, K_OTHER);
-  k_blk_pack1<<<(tot + 255) / 256, 256, 0, g->stream>>>(g->D, b, dense, arr(0), arr(2), stag, 0, 1);
+  k_blk_pack1<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, b, dense, arr(0), arr(2), stag, 0, 1);
 }
 
 static void blk_ghosts(hamr_grid* g, const Dev& D, int role, long long s_u, bool all, bool zero_ctop) {

@@ -30,7 +30,7 @@ SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "h
            "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
            "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
            "hamr_set_levels", "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
-           "hamr_get_block_bface",
+           "hamr_get_block_bface", "hamr_set_all_blocks", "hamr_get_all_blocks",
            "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
            "hamr_profile_begin", "hamr_profile_end", "hamr_profile_class_name", "hamr_launch_count"]
 NKCLASS = 10
@@ -87,6 +87,8 @@ def lib():
         L.hamr_set_levels.argtypes = [vp, C.POINTER(C.c_int)]
         L.hamr_set_block_prims.argtypes = [vp, C.c_int, C.POINTER(c_double_p), C.POINTER(c_double_p)]
         L.hamr_blocks_commit.argtypes = [vp]
+        L.hamr_set_all_blocks.argtypes = [vp, C.POINTER(c_double_p), C.POINTER(c_double_p)]
+        L.hamr_get_all_blocks.argtypes = [vp, C.POINTER(c_double_p)]
         L.hamr_get_block_prims.argtypes = [vp, C.c_int, C.POINTER(c_double_p)]
         L.hamr_get_block_bface.argtypes = [vp, C.c_int, C.POINTER(c_double_p)]
         L.hamr_debug_emf.argtypes = [vp]
@@ -270,6 +272,22 @@ class Grid:
             bf = [_arr(x) for x in bface]
             bp = (c_double_p * 3)(*[_dp(x) for x in bf])
         return self.L.hamr_set_block_prims(self.h, int(b), hp, bp)
+
+    def set_all_blocks(self, hydro, bface=None):
+        """hydro[c] / bface[d]: arrays of shape (nblk, ...) holding every block's dense array"""
+        hy = [_arr(h) for h in hydro]
+        hp = (c_double_p * 5)(*[_dp(h) for h in hy])
+        bp = None
+        if bface is not None:
+            bf = [_arr(x) for x in bface]
+            bp = (c_double_p * 3)(*[_dp(x) for x in bf])
+        return self.L.hamr_set_all_blocks(self.h, hp, bp)
+
+    def get_all_blocks(self):
+        n = self.block_info(0)[2]
+        out = [np.empty((self.num_blocks(),) + tuple(n)) for _ in range(8)]
+        self._ck(self.L.hamr_get_all_blocks(self.h, (c_double_p * 8)(*[_dp(o) for o in out])))
+        return out
 
     def commit(self):
         return self.L.hamr_blocks_commit(self.h)

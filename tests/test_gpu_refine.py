@@ -124,3 +124,26 @@ def test_cfg4_full_size_one_coarse_step(H, orc):
     to, _ = o.step(1)
     assert abs(tg - to) <= 1e-13 * to
     _check_blocks(p, infos, o, g, 4 * TOL_1)
+
+
+def test_all_blocks_calls_equal_block_by_block(H):
+    """hamr_set_all_blocks / hamr_get_all_blocks (one call, arrays of every block back to back) against the
+    block-by-block calls: same state bit for bit"""
+    p = I.torus_params(n=(32, 16, 16), nb=(8, 8, 8), r_refine_max=4.0, lat_max_level=1)
+    a, b = H.Grid(p), H.Grid(p)
+    infos = [a.block_info(q)[:3] for q in range(a.num_blocks())]
+    data = I.fm_torus_blocks(p, infos, seed=4)
+    for q, (hyd, bf) in enumerate(data):
+        assert a.set_block_prims(q, hyd, bf) == 0
+    assert a.commit() == 0
+    hy = [np.stack([d[0][c] for d in data]) for c in range(5)]
+    bf = [np.stack([d[1][c] for d in data]) for c in range(3)]
+    assert b.set_all_blocks(hy, bf) == 0
+    assert a.dt == b.dt
+    a.step(2)
+    b.step(2)
+    allb = b.get_all_blocks()
+    for q in range(a.num_blocks()):
+        one = a.get_block_prims(q)
+        for c in range(8):
+            assert np.array_equal(one[c], allb[c][q])
