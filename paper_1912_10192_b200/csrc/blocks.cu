@@ -901,6 +901,8 @@ static Dev dev_list(const hamr_grid* g, int which) {
   Dev D = g->D;
   D.B.list = g->bh.d_lists + (size_t)which * g->bh.nblk;
   D.B.nact = which == 4 ? g->bh.nblk : g->bh.nlist[which];
+  D.B.dlist = g->bh.d_dlists + (size_t)which * g->bh.nblk;
+  D.B.ndact = g->bh.ndlist[which];
   return D;
 }
 
@@ -941,6 +943,22 @@ static int blk_refined_columns(const hamr_params& p, int ncol, int bn0) {
   return nref;
 }
 
+// per list (time levels 0..3, every block), the blocks that hold phi-derefined rows: the C-15 kernels run on
+// these only.  Uses the pinned staging area (the stream must be idle with respect to it).
+static cudaError_t blk_upload_dlists(hamr_grid* g) {
+  BlkHost& H = g->bh;
+  const int nblk = H.nblk;
+  int* hd = H.h_ints + (size_t)10 * nblk;
+  for (int i = 0; i < 5; i++) H.ndlist[i] = 0;
+  for (int b = 0; b < nblk; b++) {
+    if (!H.hasderef[b]) continue;
+    const int t = H.tau[b];
+    hd[(size_t)t * nblk + H.ndlist[t]++] = b;
+    hd[(size_t)4 * nblk + H.ndlist[4]++] = b;
+  }
+  return cudaMemcpyAsync(H.d_dlists, hd, (size_t)5 * nblk * 4, cudaMemcpyHostToDevice, g->stream);
+}
+
 int blk_count(const hamr_params& p, int nslot[3], int bn[3]) {
   long long nb = 1;
   for (int d = 0; d < 3; d++) {
@@ -964,7 +982,7 @@ int blk_has_refinement(const hamr_params& p) {
 
 size_t blk_table_bytes(int nblk) {
   // info (int4), nbr (27), phys, K0, tau, cur, flags, 5 lists, 4 correction lists, ctopb (3 doubles)
-  return ((size_t)nblk * (16 + 4 * (27 + 5 + 5 + 4) + 24) + 1024 + 255) / 256 * 256;
+  return ((size_t)nblk * (16 + 4 * (27 + 5 + 5 + 4 + 5) + 24) + 1024 + 255) / 256 * 256;
 }
 
 // C-16: block lattice, neighbour table (periodic dimensions close through it), per-block table offsets
@@ -1037,12 +1055,17 @@ int blk_setup(hamr_grid* g, void* tables) {
   B.cur = (int*)take((size_t)nblk * 4);
   H.d_lists = (int*)take((size_t)nblk * 5 * 4);
   H.d_clists = (int*)take((size_t)nblk * 4 * 4);
+  H.d_dlists = (int*)take((size_t)nblk * 5 * 4);
+  H.hasderef.assign(nblk, 0);
+  for (int b = 0; b < nblk; b++)
+    for (int J = H.I0[(size_t)b * 3 + 1] - 1; J <= H.I0[(size_t)b * 3 + 1] + bn[1]; J++)
+      if (deref_row_factor(p, J) > 1) H.hasderef[b] = 1;
   B.flags = (int*)take((size_t)nblk * 4);
   B.ctopb = (double*)take((size_t)nblk * 24);
   B.info = d_info; B.nbr = d_nbr; B.phys = d_phys; B.K0 = d_K0;
   B.list = H.d_lists; B.nact = 0;
   if (cudaMallocHost((void**)&H.h_ctop, (size_t)nblk * 3 * sizeof(double)) != cudaSuccess) return HAMR_ECUDA;
-  if (cudaMallocHost((void**)&H.h_ints, (size_t)nblk * 10 * sizeof(int)) != cudaSuccess) return HAMR_ECUDA;
+  if (cudaMallocHost((void**)&H.h_ints, (size_t)nblk * 16 * sizeof(int)) != cudaSuccess) return HAMR_ECUDA;
   std::vector<int> all(nblk);
   for (int b = 0; b < nblk; b++) all[b] = b;
   cudaStream_t st = g->stream;
@@ -1059,6 +1082,7 @@ int blk_setup(hamr_grid* g, void* tables) {
   if (e == cudaSuccess) e = cudaMemsetAsync(B.tau, 0, (size_t)nblk * 4, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(B.cur, 0, (size_t)nblk * 4, st);
   if (e == cudaSuccess) e = blk_upload_flags(g);
+  if (e == cudaSuccess) e = blk_upload_dlists(g);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);               // the host vectors go out of scope
   for (int i = 0; i < 4; i++) { H.nlist[i] = 0; H.nclist[i] = 0; H.tb_u[i] = 0; H.dt_u[i] = 2 << i; H.has_new[i] = 0; }
   H.nlist[0] = nblk;
@@ -1295,6 +1319,7 @@ static int blk_assign(hamr_grid* g, bool after_step) {
   if (e == cudaSuccess) e = cudaMemcpyAsync(H.d_clists, hl + (size_t)4 * nblk, (size_t)4 * nblk * 4, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(g->D.B.tau, hl + (size_t)8 * nblk, (size_t)nblk * 4, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = blk_upload_flags(g);
+  if (e == cudaSuccess) e = blk_upload_dlists(g);
   H.dt0 = dt0;
   g->h_pinned[56] = dt0;
   if (e == cudaSuccess) e = cudaMemcpyAsync(g->D.scal + S_DT, g->h_pinned + 56, sizeof(double), cudaMemcpyHostToDevice, st);
@@ -1320,6 +1345,7 @@ int blk_initial(hamr_grid* g) {
   if (cudaMemsetAsync(g->D.B.tau, 0, (size_t)H.nblk * 4, st) != cudaSuccess) return HAMR_ECUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return HAMR_ECUDA;   // the pinned staging area is reused
   if (blk_upload_flags(g) != cudaSuccess) return HAMR_ECUDA;
+  if (blk_upload_dlists(g) != cudaSuccess) return HAMR_ECUDA;
   // level-0 list = every block
   if (cudaMemcpyAsync(H.d_lists, H.d_lists + (size_t)4 * H.nblk, (size_t)H.nblk * 4, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
     return HAMR_ECUDA;

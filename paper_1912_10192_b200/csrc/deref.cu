@@ -206,12 +206,20 @@ __global__ void __launch_bounds__(128) k_deref_project(Dev Dv, Fields s0, Fields
   group_interp(selp<BLK>(s0.Bf[2], s2.Bf[2], T.C.cur), zrow, T.k, m);
 }
 
+// the launch of a C-15 kernel: on a block grid only the listed blocks that hold derefined rows
+static Dev deref_dev(const Dev& Dv) {
+  Dev D = Dv;
+  if (Dv.B.nblk > 0 && Dv.B.dlist) { D.B.list = Dv.B.dlist; D.B.nact = Dv.B.ndact; }
+  return D;
+}
+
 static unsigned nblocks_for(const Dev& Dv, int ci, int cj) {
   const long long tot = (long long)ci * cj * Dv.L.n[2] * (Dv.B.nblk > 0 ? Dv.B.nact : 1);
   return (unsigned)((tot + 127) / 128);
 }
 
-void launch_deref_fix_flux(hamr_grid* g, const Dev& Dv) {
+void launch_deref_fix_flux(hamr_grid* g, const Dev& Dv0) {
+  const Dev Dv = deref_dev(Dv0);
   if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
   Launch l_(g, K_OTHER);
   const unsigned nb = nblocks_for(Dv, Dv.L.n[0] + 2, Dv.L.n[1] + 2);
@@ -219,7 +227,8 @@ void launch_deref_fix_flux(hamr_grid* g, const Dev& Dv) {
   else k_deref_fix_flux<false><<<nb, 128, 0, g->stream>>>(Dv);
 }
 
-void launch_deref_flux_layers(hamr_grid* g, const Dev& Dv) {
+void launch_deref_flux_layers(hamr_grid* g, const Dev& Dv0) {
+  const Dev Dv = deref_dev(Dv0);
   if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
   Launch l_(g, K_OTHER);
   const long long tot = 2LL * (Dv.L.n[0] + 1) * (Dv.L.n[1] + 1) * (Dv.B.nblk > 0 ? Dv.B.nact : 1);
@@ -228,7 +237,8 @@ void launch_deref_flux_layers(hamr_grid* g, const Dev& Dv) {
   else k_deref_flux_layers<false><<<nb, 128, 0, g->stream>>>(Dv);
 }
 
-void launch_deref_fix_edges(hamr_grid* g, const Dev& Dv) {
+void launch_deref_fix_edges(hamr_grid* g, const Dev& Dv0) {
+  const Dev Dv = deref_dev(Dv0);
   if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
   Launch l_(g, K_OTHER);
   const unsigned nb = nblocks_for(Dv, Dv.L.n[0] + 1, Dv.L.n[1] + 1);
@@ -236,7 +246,8 @@ void launch_deref_fix_edges(hamr_grid* g, const Dev& Dv) {
   else k_deref_fix_edges<false><<<nb, 128, 0, g->stream>>>(Dv);
 }
 
-void launch_deref_sync(hamr_grid* g, const Dev& Dv, const Fields& out, const Fields& out2) {
+void launch_deref_sync(hamr_grid* g, const Dev& Dv0, const Fields& out, const Fields& out2) {
+  const Dev Dv = deref_dev(Dv0);
   if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
   Launch l_(g, K_OTHER);
   const unsigned nb = nblocks_for(Dv, Dv.L.n[0] + 1, Dv.L.n[1] + 1);
@@ -244,7 +255,8 @@ void launch_deref_sync(hamr_grid* g, const Dev& Dv, const Fields& out, const Fie
   else k_deref_sync<false><<<nb, 128, 0, g->stream>>>(Dv, out, out2);
 }
 
-void launch_deref_project(hamr_grid* g, const Dev& Dv, const Fields& s, const Fields& s2) {
+void launch_deref_project(hamr_grid* g, const Dev& Dv0, const Fields& s, const Fields& s2) {
+  const Dev Dv = deref_dev(Dv0);
   if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
   Launch l_(g, K_OTHER);
   const unsigned nb = nblocks_for(Dv, Dv.L.n[0], Dv.L.n[1]);

@@ -444,8 +444,10 @@ __global__ void __launch_bounds__(128) k_deref_x3(Dev Dv, Fields s, Fields s2, i
   if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
 }
 
-void launch_deref_x3(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
-  if (!Dv.mrow) return;
+void launch_deref_x3(hamr_grid* g, const Dev& Dv0, const Fields& src, const Fields& src2, bool want_ctop) {
+  if (!Dv0.mrow) return;
+  Dev Dv = Dv0;   // on a block grid only the listed blocks that hold derefined rows
+  if (Dv0.B.nblk > 0 && Dv0.B.dlist) { Dv.B.list = Dv0.B.dlist; Dv.B.nact = Dv0.B.ndact; }
   const Lay& L = Dv.L;
   const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
   if (blk && Dv.B.nact == 0) return;

@@ -31,6 +31,8 @@ struct BlkDev {
   int n2g;                   // global N2 (pole faces: J == 0 or J == n2g)
   int tlev, flev;            // offset in doubles of the level-1 geometry / floor tables
   const int* list;           // [nact] block ids of this launch
+  const int* dlist;          // [ndact] those of them that hold phi-derefined rows (C-15 kernels); NULL: use list
+  int ndact;
   const int4* info;          // [nblk] {table index of local zone (0,0), x1 level, I0, J0}
   const int* nbr;            // [nblk][27] neighbour block by offset, -1 outside the domain
   const int* phys;           // [nblk] bit d: low side of dim d is a physical boundary, bit 3+d: high side
@@ -113,12 +115,14 @@ struct BlkHost {
   std::vector<int> forced;   // test hook: prescribed time levels (empty: Courant-based)
   int* d_lists;              // device [5][nblk]: blocks of level 0..3, then every block
   int* d_clists;             // device [4][nblk]: blocks of level tau with a neighbour on tau - 1
-  int nlist[4], nclist[4];
+  int* d_dlists;             // device [5][nblk]: per list, the blocks that hold phi-derefined rows
+  int nlist[4], nclist[4], ndlist[5];
+  std::vector<char> hasderef;  // [nblk] some row of the block (or of its transverse ghost layer) is derefined
   long long tb_u[4];         // LAT clocks per level, units of (finest dt)/2 (C-17)
   int dt_u[4];
   int has_new[4];
   double* h_ctop;            // pinned [nblk][3]
-  int* h_ints;               // pinned [6][nblk]
+  int* h_ints;               // pinned [16][nblk]
   double dt0;                // host copy of the finest step (LAT)
 };
 }
