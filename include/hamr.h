@@ -58,7 +58,7 @@ typedef struct {
   int bc_lo[3], bc_hi[3];/* hamr_bc_t per side; periodic must be set on both sides of a dim     */
   int nb[3];             /* block size; {0,0,0} = one block (block-structured grid: DESIGN.md §9)*/
   int n_deref;           /* number of phi-derefinement thresholds, 0 = none       */
-  int deref_factor[4];
+  int deref_factor[4];   /* derefinement factor per threshold (see "phi-derefinement" below)            */
   int lat_max_level;     /* local adaptive time-stepping levels; 0 = global dt    */
   int pad_;
   double a;              /* black-hole spin (ignored for Minkowski)                              */
@@ -67,8 +67,8 @@ typedef struct {
   double cour;           /* Courant factor C of dt_d = C dx^d / max ctop_d (PAPER.md:93 fn. 2)   */
   double rho_fl_coef, rho_fl_pow, u_fl_coef, u_fl_pow; /* floor = coef * r^pow (r = 1 Cartesian) */
   double gamma_max;      /* Lorentz-factor ceiling                                               */
-  double deref_theta_deg[4];
-  double r_refine_max;   /* r-refinement radius; <= 0 = none                       */
+  double deref_theta_deg[4]; /* thresholds in degrees from either pole                                   */
+  double r_refine_max;   /* x1-refinement radius (see below); <= 0 = none           */
 } hamr_params;
 
 /* ---- life cycle ------------------------------------------------------------------------------ */
@@ -131,6 +131,14 @@ int hamr_num_blocks(const hamr_grid* g);
 /* x_lo: internal coordinates of the block's low corner; time_level: its current LAT level tau */
 int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int n[3],
                     int* time_level);
+/* phi-derefinement of the polar rows (C-15): with n_deref > 0 an x2 row whose zone-centre
+ * polar angle lies within deref_theta_deg[t] degrees of either pole is derefined in x3 by deref_factor[t] (the
+ * largest factor that applies; BASELINE cfg 4: {15, 5} degrees -> {2, 4}).  A row with factor m treats every
+ * aligned group of m phi-zones as one zone: fluxes and EMFs are group means (or interpolated between group
+ * boundaries), the x3 reconstruction takes one value per group, the Courant limit uses m dx3; all arrays keep
+ * the fine shapes.  hamr_set_prims projects the hydro input onto group means; the face field given must be
+ * uniform within groups (any axisymmetric field is).  Needs a periodic x3; factors are powers of two <= 16
+ * that divide the x3 block size nb3 with 3 * factor <= nb3.  Works on monolithic and block grids and under LAT. */
 /* One x1 refinement level (PAPER.md:71 per-dimension refinement; C-16): with r_refine_max > 0 every
  * block column whose x1-centre has r < r_refine_max (x1 < r_refine_max on the Cartesian map) is replaced by
  * two blocks of nb zones with dx1 / 2; such columns must be contiguous from the low x1 side and nb[0] >= 6.
