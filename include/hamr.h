@@ -100,7 +100,10 @@ int hamr_set_prims_dev(hamr_grid* g, const double* const hydro[5], const double*
  * floors, Courant dt reduction — all on the device.  t_out / dt_last_out (host, may be NULL)
  * receive the time reached and the dt of the last step; the call synchronises the stream. */
 int hamr_step(hamr_grid* g, int nsteps, double* t_out, double* dt_last_out);
-/* Enqueues nsteps steps and returns without synchronising (errors surface at the next sync). */
+/* Enqueues nsteps steps and returns without synchronising (errors surface at the next sync).  Exception: on a
+ * grid with lat_max_level > 0 the host reads the per-block Courant limits back once per coarse step to assign
+ * the time levels and build the per-level block lists (one 24 B x blocks copy), so the call waits for all but
+ * the last coarse step. */
 int hamr_step_async(hamr_grid* g, int nsteps);
 int hamr_sync(hamr_grid* g); /* waits for the stream; reports HAMR_ENONFINITE / HAMR_ECUDA */
 
