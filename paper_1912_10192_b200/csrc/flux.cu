@@ -74,19 +74,24 @@ struct FGeo {
   double gdet, igdet, alpha, ialpha, boa;
 };
 
+// from the array-of-records tables (hamr_dev.cuh): one 128-byte line per face record (x1-, x2-faces); the x3 sweep
+// reads the centre record (two lines)
 template <int D>
-__device__ __forceinline__ FGeo load_fgeo(const double* __restrict__ tab, int n2d, int q) {
+__device__ __forceinline__ FGeo load_fgeo(const double* __restrict__ rec) {
   FGeo G;
-  G.c00 = __ldg(tab + C00 * n2d + q); G.c01 = __ldg(tab + C01 * n2d + q);
-  G.c03 = __ldg(tab + C03 * n2d + q); G.c11 = __ldg(tab + C11 * n2d + q);
-  G.c13 = __ldg(tab + C13 * n2d + q); G.c22 = __ldg(tab + C22 * n2d + q);
-  G.c33 = __ldg(tab + C33 * n2d + q);
-  G.k00 = __ldg(tab + K00 * n2d + q);
-  G.kdd = __ldg(tab + (D == 0 ? K11 : (D == 1 ? K22 : K33)) * n2d + q);
-  G.k0d = (D == 0) ? __ldg(tab + K01 * n2d + q) : 0.0;  // g^{t2} = g^{t3} = 0 for both metrics
-  G.gdet = __ldg(tab + GDET * n2d + q); G.igdet = __ldg(tab + IGDET * n2d + q);
-  G.alpha = __ldg(tab + ALPHA * n2d + q);
-  G.ialpha = __ldg(tab + IALPHA * n2d + q); G.boa = __ldg(tab + BOA * n2d + q);
+  if (D < 2) {
+    double v[NREC_F];
+    load_rec(rec, NREC_F, v);
+    G.c00 = v[0]; G.c01 = v[1]; G.c03 = v[2]; G.c11 = v[3]; G.c13 = v[4]; G.c22 = v[5]; G.c33 = v[6];
+    G.k00 = v[7]; G.kdd = v[8]; G.k0d = v[9];
+    G.gdet = v[10]; G.igdet = v[11]; G.alpha = v[12]; G.ialpha = v[13]; G.boa = v[14];
+  } else {
+    double v[18];
+    load_rec(rec, 18, v);
+    G.c00 = v[0]; G.c01 = v[1]; G.c03 = v[2]; G.c11 = v[3]; G.c13 = v[4]; G.c22 = v[5]; G.c33 = v[6];
+    G.k00 = v[7]; G.kdd = v[12]; G.k0d = 0.0;   // g^{33}; g^{t3} = 0 for both metrics
+    G.gdet = v[13]; G.alpha = v[14]; G.ialpha = v[15]; G.boa = v[16]; G.igdet = v[17];
+  }
   return G;
 }
 
@@ -257,7 +262,7 @@ __global__ void __launch_bounds__(128, HAMR_MARCH_MINB) k_flux_march(Dev Dv, Fie
                             selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[e], s2.Bc[e], C.cur),
                             selp<BLK>(s.Bc[f], s2.Bc[f], C.cur)};
     const double* bfn = selp<BLK>(s.Bf[D], s2.Bf[D], C.cur);
-    const double* gtab = (D == 0 ? Dv.gf1 : Dv.gf2) + (BLK ? C.lev * Dv.B.tlev : 0);
+    const double* gtab = (D == 0 ? Dv.gf1A : Dv.gf2A) + (BLK ? C.lev * Dv.B.tlevA : 0);
     constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
     int z = C.zoff + (int)L.idx(D == 0 ? f0 - 1 : o, D == 0 ? o : f0 - 1, k);
     double PL[8], PR[8];
@@ -309,7 +314,7 @@ __global__ void __launch_bounds__(128, HAMR_MARCH_MINB) k_flux_march(Dev Dv, Fie
         zero_face(Dv, D, z);
       } else {
         const int q = C.q0 + ((D == 0) ? fc * ge2 + o : o * ge2 + fc);
-        const FGeo G = load_fgeo<D>(gtab, L.n2d, q);
+        const FGeo G = load_fgeo<D>(gtab + (size_t)q * NREC_F);
         PL[5 + D] = PR[5 + D] = bfn[z] * G.igdet;  // C-5: the normal field is single-valued at the face
         const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
         if (act) ctop = dmax(ctop, ct);
@@ -378,7 +383,7 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
   const bool fine_row = Dv.mrow == nullptr || __ldg(Dv.mrow + C.J0 + j + NG) == 1;
   if (valid && fine_row && lane >= HLO && lane < 32 - HHI && k >= 0 && k <= L.n[2]) {
     const int ge2 = BLK ? Dv.B.ge2 : L.e2;
-    const FGeo G = load_fgeo<D>(Dv.gc + (BLK ? C.lev * Dv.B.tlev : 0), L.n2d, C.q0 + i * ge2 + j);
+    const FGeo G = load_fgeo<D>(Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * ge2 + j) * NREC_C);
     PL[7] = PR[7] = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z] * G.igdet;
     const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
     if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct;
@@ -435,7 +440,7 @@ __global__ void __launch_bounds__(128) k_deref_x3(Dev Dv, Fields s, Fields s2, i
       }
     }
     const int ge2 = BLK ? Dv.B.ge2 : L.e2;
-    const FGeo G = load_fgeo<D>(Dv.gc + (BLK ? C.lev * Dv.B.tlev : 0), L.n2d, C.q0 + i * ge2 + j);
+    const FGeo G = load_fgeo<D>(Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * ge2 + j) * NREC_C);
     const int z = zrow + k;
     PL[7] = PR[7] = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z] * G.igdet;
     const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);

@@ -80,8 +80,16 @@ __device__ static void store_geo(double* tab, int n2d, int q, const Geo& G) {
 
 // e1 x e2 table entries; entry (ti, tj) is the zone with index (ti - NG, tj - NG) counted from the
 // domain's low corner in zones of spacing dx1 (the table of one x1 refinement level), n2glob zones in x2
+// face record of the array-of-records tables (hamr_dev.cuh); kdd / k0d: g^{dd}, g^{td} of the face's direction
+__device__ static void store_face_rec(double* rec, const Geo& G, double kdd, double k0d) {
+  const double v[NREC_F] = {G.c00, G.c01, G.c03, G.c11, G.c13, G.c22, G.c33, G.k00, kdd, k0d, G.gdet,
+                            G.gdet > 0.0 ? 1.0 / G.gdet : 0.0, G.alpha, G.ialpha, G.boa, 0.0};
+  for (int c = 0; c < NREC_F; c++) rec[c] = v[c];
+}
+
 __global__ void k_geometry(Dev D, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
-                           double* gf2, double* dgc, double* rho_fl, double* u_fl) {
+                           double* gf2, double* dgc, double* rho_fl, double* u_fl, double* gcA, double* gf1A,
+                           double* gf2A) {
   const int q = blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= e1 * e2) return;
   const int i = q / e2 - NG, j = q % e2 - NG;
@@ -95,11 +103,18 @@ __global__ void k_geometry(Dev D, int e1, int e2, int n2d, double dx1, int n2glo
     dgc[c * n2d + q] = d1[c];
     dgc[(NDG + c) * n2d + q] = d2[c];
   }
+  {
+    double* rec = gcA + (size_t)q * NREC_C;   // the same numbers, one record per (i, j)
+    for (int c = 0; c < NGEO; c++) rec[c] = gc[c * n2d + q];
+    for (int c = 0; c < NDG; c++) { rec[NGEO + c] = d1[c]; rec[NGEO + NDG + c] = d2[c]; }
+  }
   metric_at(D.metric, D.a, xf1, xc2, G, d1, d2);
   store_geo(gf1, n2d, q, G);
+  store_face_rec(gf1A + (size_t)q * NREC_F, G, G.k11, G.k01);
   metric_at(D.metric, D.a, xc1, xf2, G, d1, d2);
   if (D.metric == HAMR_METRIC_KERR_SCHILD && (j == 0 || j == n2glob)) G.gdet = 0.0;  // pole faces (C-7)
   store_geo(gf2, n2d, q, G);
+  store_face_rec(gf2A + (size_t)q * NREC_F, G, G.k22, 0.0);
   if (j == -NG) {  // floors depend on x1 only (C-13): coef * r^pow, r = 1 on the Cartesian map
     const double r = (D.metric == HAMR_METRIC_KERR_SCHILD) ? exp(xc1) : 1.0;
     rho_fl[i + NG] = D.rho_fl_coef * pow(r, D.rho_fl_pow);
@@ -108,16 +123,11 @@ __global__ void k_geometry(Dev D, int e1, int e2, int n2d, double dx1, int n2glo
 }
 
 void launch_geometry_tab(hamr_grid* g, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
-                         double* gf2, double* dgc, double* rho_fl, double* u_fl) {
+                         double* gf2, double* dgc, double* rho_fl, double* u_fl, double* gcA, double* gf1A,
+                         double* gf2A) {
   Launch l_(g, K_OTHER);
   k_geometry<<<(e1 * e2 + 127) / 128, 128, 0, g->stream>>>(g->D, e1, e2, n2d, dx1, n2glob, gc, gf1, gf2, dgc,
-                                                         rho_fl, u_fl);
-}
-
-void launch_geometry(hamr_grid* g, double* gc, double* gf1, double* gf2, double* dgc, double* rho_fl,
-                     double* u_fl) {
-  const Lay& L = g->D.L;
-  launch_geometry_tab(g, L.e1, L.e2, L.n2d, g->D.dx[0], L.n[1], gc, gf1, gf2, dgc, rho_fl, u_fl);
+                                                         rho_fl, u_fl, gcA, gf1A, gf2A);
 }
 
 }  // namespace hamr

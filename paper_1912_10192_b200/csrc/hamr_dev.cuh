@@ -69,6 +69,31 @@ __device__ __forceinline__ Geo load_geo(const double* __restrict__ tab, int n2d,
   return G;
 }
 
+// The hot kernels read a geometry RECORD with all lanes of a warp on the same (i, j): with the SoA tables that is one
+// cache line (one L2 round trip when it misses L1) per COMPONENT, 15-50 per face or zone.  They therefore read
+// array-of-records copies: a centre record is 32 doubles (the 18 components of Geo in GeoComp order, then the 7 x1-
+// and the 7 x2-derivatives of the covariant metric) = two 128-byte lines; a face record is 16 doubles = one line.
+constexpr int NREC_C = 32, NREC_F = 16;
+// face record: c00 c01 c03 c11 c13 c22 c33 | k00 kdd k0d | gdet igdet alpha ialpha boa | pad
+__device__ __forceinline__ void load_rec(const double* __restrict__ rec, int n, double* v) {
+  const double2* r2 = reinterpret_cast<const double2*>(rec);
+#pragma unroll
+  for (int q = 0; q < n / 2; q++) {
+    const double2 t = __ldg(r2 + q);
+    v[2 * q] = t.x;
+    v[2 * q + 1] = t.y;
+  }
+}
+__device__ __forceinline__ Geo load_geo_rec(const double* __restrict__ rec) {
+  double v[18];
+  load_rec(rec, 18, v);
+  Geo G;
+  G.c00 = v[0]; G.c01 = v[1]; G.c03 = v[2]; G.c11 = v[3]; G.c13 = v[4]; G.c22 = v[5]; G.c33 = v[6];
+  G.k00 = v[7]; G.k01 = v[8]; G.k11 = v[9]; G.k13 = v[10]; G.k22 = v[11]; G.k33 = v[12];
+  G.gdet = v[13]; G.alpha = v[14]; G.ialpha = v[15]; G.boa = v[16]; G.igdet = v[17];
+  return G;
+}
+
 // ---- C-2, C-3: four-velocity and magnetic four-vector -----------------------------------------------
 struct St {
   double ucon[4], ucov[4], bcon[4], bcov[4], bsq;

@@ -30,6 +30,7 @@ struct BlkDev {
   int ge2;                   // row pitch of the (global, per x1-level) geometry tables
   int n2g;                   // global N2 (pole faces: J == 0 or J == n2g)
   int tlev, flev;            // offset in doubles of the level-1 geometry / floor tables
+  int tlevA;                 // the same for the array-of-records copies
   const int* list;           // [nact] block ids of this launch
   const int* dlist;          // [ndact] those of them that hold phi-derefined rows (C-15 kernels); NULL: use list
   int ndact;
@@ -57,6 +58,9 @@ struct Dev {                 // everything a kernel may need, passed by value
   const double* gf1;         // at x1-faces
   const double* gf2;         // at x2-faces (pole rows: gdet = 0)
   const double* dgc;         // [2][NDG][n2d]: d_1 g, d_2 g at centres
+  const double* gcA;         // array-of-records copies for the hot kernels (hamr_dev.cuh): centres [n2d][32],
+  const double* gf1A;        // x1-faces [n2d][16],
+  const double* gf2A;        // x2-faces [n2d][16]
   const double* rho_fl;      // [e1] floor per x1 index
   const double* u_fl;
   double* F[3][5];           // hydro fluxes on d-faces
@@ -181,8 +185,6 @@ struct Launch {
 namespace hamr {
 
 // kernel launchers (each returns after enqueueing on g->stream)
-void launch_geometry(hamr_grid* g, double* gc, double* gf1, double* gf2, double* dgc, double* rho_fl,
-                     double* u_fl);
 void launch_ghosts(hamr_grid* g, const Fields& s, bool bc_active_too);
 void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop);
 void launch_ct(hamr_grid* g, const Fields& src);
@@ -207,7 +209,8 @@ void launch_deref_sync(hamr_grid* g, const Dev& Dv, const Fields& out, const Fie
 void launch_deref_project(hamr_grid* g, const Dev& Dv, const Fields& s, const Fields& s2);
 int deref_row_factor(const hamr_params& p, long long J);
 void launch_geometry_tab(hamr_grid* g, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
-                         double* gf2, double* dgc, double* rho_fl, double* u_fl);
+                         double* gf2, double* dgc, double* rho_fl, double* u_fl, double* gcA, double* gf1A,
+                         double* gf2A);
 
 // blocks.cu: block-structured grid (H7)
 int blk_count(const hamr_params& p, int nslot[3], int bn[3]);       // number of blocks (0 if invalid)

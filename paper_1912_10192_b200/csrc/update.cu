@@ -70,7 +70,8 @@ __global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra,
     if (in0 && in1) { lo[2] = bf_new<2>(Dv, base.Bf[2], z, dt, S, idx); out.Bf[2][z] = lo[2]; }
     if (in0 && in1 && in2) {
       const int q = C.q0 + i * (BLK ? Dv.B.ge2 : L.e2) + j;
-      const Geo G = load_geo(Dv.gc + tl, L.n2d, q);
+      const double* grec = Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)q * NREC_C;
+      const Geo G = load_geo_rec(grec);
       // new cell-centred field from the new faces (the high faces are recomputed, bit-identically)
       double Bn[3];
       {
@@ -114,15 +115,14 @@ __global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra,
         const double T13 = eta * u[1] * u[3] + ptot * G.k13 - b[1] * b[3];
         const double T22 = eta * u[2] * u[2] + ptot * G.k22 - b[2] * b[2];
         const double T33 = eta * u[3] * u[3] + ptot * G.k33 - b[3] * b[3];
-        const double* d1 = Dv.dgc + tl + q;
-        const int n2d = L.n2d;
-        double a1 = 0.5 * (T00 * __ldg(d1 + D00 * n2d) + T11 * __ldg(d1 + D11 * n2d) + T22 * __ldg(d1 + D22 * n2d) +
-                           T33 * __ldg(d1 + D33 * n2d)) +
-                    T01 * __ldg(d1 + D01 * n2d) + T03 * __ldg(d1 + D03 * n2d) + T13 * __ldg(d1 + D13 * n2d);
-        const double* d2 = d1 + NDG * n2d;
-        double a2 = 0.5 * (T00 * __ldg(d2 + D00 * n2d) + T11 * __ldg(d2 + D11 * n2d) + T22 * __ldg(d2 + D22 * n2d) +
-                           T33 * __ldg(d2 + D33 * n2d)) +
-                    T01 * __ldg(d2 + D01 * n2d) + T03 * __ldg(d2 + D03 * n2d) + T13 * __ldg(d2 + D13 * n2d);
+        double dg[2 * NDG];   // d_1 g and d_2 g, in DgComp order, from the zone's record
+        load_rec(grec + NGEO, 2 * NDG, dg);
+        const double* d1 = dg;
+        double a1 = 0.5 * (T00 * d1[D00] + T11 * d1[D11] + T22 * d1[D22] + T33 * d1[D33]) + T01 * d1[D01] +
+                    T03 * d1[D03] + T13 * d1[D13];
+        const double* d2 = dg + NDG;
+        double a2 = 0.5 * (T00 * d2[D00] + T11 * d2[D11] + T22 * d2[D22] + T33 * d2[D33]) + T01 * d2[D01] +
+                    T03 * d2[D03] + T13 * d2[D13];
         Ssrc1 = G.gdet * a1;
         Ssrc2 = G.gdet * a2;
       }
@@ -149,9 +149,9 @@ __global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra,
 #if HAMR_UPD_RELOAD
       // the geometry record and the guess are re-read (L1 / L2 hits) instead of being kept in registers
       // across the flux divergence: lower register pressure, more resident warps
-      const double* gtab = Dv.gc + tl;
+      const double* gtab = grec;
       asm volatile("" : "+l"(gtab));
-      const Geo G2 = load_geo(gtab, L.n2d, q);
+      const Geo G2 = load_geo_rec(gtab);
       const double* sp[5] = {src.P[0], src.P[1], src.P[2], src.P[3], src.P[4]};
       double Pg[5];
 #pragma unroll
