@@ -138,9 +138,9 @@ ALG_DOUBLES = {"flux_x1": 16, "flux_x2": 16, "flux_x3": 16,   # 9 r (P5, 2 trans
 
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel class from the round's
-# `ncu --set full` capture of this same command on cfg 2 (profiles/r1c_ncu_full_cfg2.md)
-NCU_TRAFFIC_SOURCE = "profiles/r1c_ncu_full_cfg2.md"
-NCU_TRAFFIC = {"flux_x1": 612235336, "flux_x2": 594134716, "flux_x3": 537716000, "centre_emf": 318640136, "edge_emf": 535194424, "update_predictor": 1382105232, "update_corrector": 1657781416, "ghosts": 139616240}
+# `ncu --set full` capture of this same command on cfg 2 (profiles/r1e_ncu_full_cfg2.md)
+NCU_TRAFFIC_SOURCE = "profiles/r1e_ncu_full_cfg2.md"
+NCU_TRAFFIC = {"flux_x1": 611919756, "flux_x2": 595946828, "flux_x3": 542627352, "centre_emf": 318860700, "edge_emf": 535477916, "update_predictor": 1377812368, "update_corrector": 1669734608, "ghosts": 139722668}
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 PAPER_V100_150CUBED = 0.85e8   # ~0.85e8 zone-cycles/s, 1 V100, one 150^3 block
 
