@@ -14,8 +14,9 @@ template <int d>
 __device__ __forceinline__ double bf_new(const Dev& Dv, const double* __restrict__ base, long long z, double dt,
                                          const long long S[3], const double idx[3]) {
   constexpr int e = (d + 1) % 3, f = (d + 2) % 3;
-  const double curl = (Dv.Ee[f][z + S[e]] - Dv.Ee[f][z]) * idx[e] - (Dv.Ee[e][z + S[f]] - Dv.Ee[e][z]) * idx[f];
-  return base[z] - dt * curl;
+  const double curl = (__ldg(Dv.Ee[f] + z + S[e]) - __ldg(Dv.Ee[f] + z)) * idx[e] -
+                      (__ldg(Dv.Ee[e] + z + S[f]) - __ldg(Dv.Ee[e] + z)) * idx[f];
+  return __ldg(base + z) - dt * curl;
 }
 
 template <bool BLK>
@@ -94,9 +95,9 @@ __global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra,
       }
       double Ps[8], U[5], Ssrc1, Ssrc2;
 #pragma unroll
-      for (int c = 0; c < 5; c++) Ps[c] = src.P[c][z];
+      for (int c = 0; c < 5; c++) Ps[c] = __ldg(src.P[c] + z);
 #pragma unroll
-      for (int c = 0; c < 3; c++) Ps[5 + c] = src.Bc[c][z];
+      for (int c = 0; c < 3; c++) Ps[5 + c] = __ldg(src.Bc[c] + z);
       {
         St Ss;
         get_state(Ps, G, Ss);
@@ -129,9 +130,9 @@ __global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra,
       if (!SAME) {
         double Pb[8];
 #pragma unroll
-        for (int c = 0; c < 5; c++) Pb[c] = base.P[c][z];
+        for (int c = 0; c < 5; c++) Pb[c] = __ldg(base.P[c] + z);
 #pragma unroll
-        for (int c = 0; c < 3; c++) Pb[5 + c] = base.Bc[c][z];
+        for (int c = 0; c < 3; c++) Pb[5 + c] = __ldg(base.Bc[c] + z);
         St Sb;
         get_state(Pb, G, Sb);
         prim_to_U5(Pb, Sb, G.gdet, Dv.gam, U);
@@ -141,7 +142,7 @@ __global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra,
       for (int c = 0; c < 5; c++) {
         double div = 0.0;
 #pragma unroll
-        for (int d = 0; d < 3; d++) div += (Dv.F[d][c][z + S[d]] - Dv.F[d][c][z]) * idx[d];
+        for (int d = 0; d < 3; d++) div += (__ldg(Dv.F[d][c] + z + S[d]) - __ldg(Dv.F[d][c] + z)) * idx[d];
         const double sc = (c == 2) ? Ssrc1 : (c == 3 ? Ssrc2 : 0.0);
         U[c] = U[c] - dt * div + dt * sc;
       }
