@@ -24,14 +24,13 @@ __global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s0, Fields s2
   const int i = (int)ti - 1;
   const long long z = C.zoff + L.idx(i, j, k);
   const int q = C.q0 + i * (BLK ? Dv.B.ge2 : L.e2) + j;
-  const double* gc = Dv.gc + (BLK ? C.lev * Dv.B.tlev : 0);
-  const int n2d = L.n2d;
   Fields s;
   for (int c = 2; c < 5; c++) s.P[c] = selp<BLK>(s0.P[c], s2.P[c], C.cur);
   for (int c = 0; c < 3; c++) s.Bc[c] = selp<BLK>(s0.Bc[c], s2.Bc[c], C.cur);
-  const double c11 = __ldg(gc + C11 * n2d + q), c13 = __ldg(gc + C13 * n2d + q), c22 = __ldg(gc + C22 * n2d + q),
-               c33 = __ldg(gc + C33 * n2d + q), gdet = __ldg(gc + GDET * n2d + q),
-               ialpha = __ldg(gc + IALPHA * n2d + q), boa = __ldg(gc + BOA * n2d + q);
+  // the zone's geometry record (array-of-records table: two cache lines instead of seven, hamr_dev.cuh)
+  const double* rec = Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)q * NREC_C;
+  const double c11 = __ldg(rec + C11), c13 = __ldg(rec + C13), c22 = __ldg(rec + C22), c33 = __ldg(rec + C33),
+               gdet = __ldg(rec + GDET), ialpha = __ldg(rec + IALPHA), boa = __ldg(rec + BOA);
   const double v1 = s.P[2][z], v2 = s.P[3][z], v3 = s.P[4][z];
   const double gam = sqrt(1.0 + (c11 * v1 * v1 + c22 * v2 * v2 + c33 * v3 * v3 + 2.0 * (c13 * v1 * v3)));
   const double iut = 1.0 / (gam * ialpha);
