@@ -249,7 +249,8 @@ def main():
         args.warmup = min(args.warmup, 1) if args.warmup else 0
         return run_reference(args)
     if args.steps is None:
-        args.steps = 20
+        # BASELINE cfg 2 runs 200 steps (0.6 s on a B200: long enough for the clock sampler to see the load)
+        args.steps = 200 if args.workload in ("cfg2", "cfg1", "cfg0", "paper150") else 20
     args.warmup = max(args.warmup, 3)
 
     import torch
