@@ -6,6 +6,10 @@
 // composing the three index maps: every ghost value is a signed copy of one active value.
 #include "hamr_host.h"
 
+#ifndef HAMR_GHOST_FAST
+#define HAMR_GHOST_FAST 1  // copy path for the periodic x3 slots of the shell fill
+#endif
+
 namespace hamr {
 
 __device__ __forceinline__ int pmod(int g, int n) {
@@ -158,8 +162,31 @@ __global__ void __launch_bounds__(256) k_ghosts_shell(Dev D, Fields s, int nj, l
   const long long col = u >> 3;
   const int i = (int)(col / L.n[1]), j = (int)(col % L.n[1]);
   if (nj == 2 * NG + 2 && j == 0) return;  // the wall row was done in part A
-  const int k = q < NG ? q - NG : L.n[2] + q - NG;
-  ghost_cell(D, s, 0, i, j, k);
+  const int n3 = L.n[2];
+  const int k = q < NG ? q - NG : n3 + q - NG;
+  // periodic x3 on a row that is not derefined and touches no reflecting wall face: the slots are plain
+  // copies of the image zone; same values and the same B_c arithmetic as ghost_cell
+  const bool fast = HAMR_GHOST_FAST && D.bc_lo[2] == HAMR_BC_PERIODIC && !D.mrow && n3 > NG &&
+                    !(j + 1 == L.n[1] && D.bc_hi[1] >= HAMR_BC_POLAR_REFLECT) &&
+                    !(i + 1 == L.n[0] && D.bc_hi[0] >= HAMR_BC_POLAR_REFLECT);
+  if (!fast) { ghost_cell(D, s, 0, i, j, k); return; }
+  if (q == 6) { s.Bf[2][L.idx(i, j, k)] = s.Bf[2][L.idx(i, j, NG)]; return; }
+  const int ks = k < 0 ? k + n3 : k - n3;
+  const long long z = L.idx(i, j, k), zs = L.idx(i, j, ks);
+#pragma unroll
+  for (int c = 0; c < 5; c++) s.P[c][z] = s.P[c][zs];
+  const double lo0 = s.Bf[0][zs], hi0 = s.Bf[0][L.idx(i + 1, j, ks)];
+  const double lo1 = s.Bf[1][zs], hi1 = s.Bf[1][L.idx(i, j + 1, ks)];
+  const int klo = k < 0 ? n3 + k : (k == n3 ? n3 : k - n3);
+  const int khi = k == -1 ? 0 : (k < 0 ? n3 + k + 1 : k + 1 - n3);
+  const double lo2 = s.Bf[2][L.idx(i, j, klo)], hi2 = s.Bf[2][L.idx(i, j, khi)];
+  s.Bf[0][z] = lo0;
+  s.Bf[1][z] = lo1;
+  if (k != n3) s.Bf[2][z] = lo2;
+  const double g2 = 2.0 * __ldg(D.gc + GDET * L.n2d + L.idx2(i, j));
+  s.Bc[0][z] = (lo0 + hi0) / g2;
+  s.Bc[1][z] = (lo1 + hi1) / g2;
+  s.Bc[2][z] = (lo2 + hi2) / g2;
 }
 
 void launch_ghosts(hamr_grid* g, const Fields& s, bool all) {
