@@ -19,8 +19,10 @@ static bool params_ok(const Params& p, std::string& why) {
   }
   if (p.metric == 1 && !(p.xmin[0] > 0.0)) { why = "r_in <= 0"; return false; }
   if (p.bc_lo[1] == 3 || p.bc_hi[1] == 3) {   // NEXT-1 transmissive pole
-    if (p.bc_lo[1] != p.bc_hi[1] || p.bc_lo[2] != 0 || p.n[2] % 2 != 0 || (p.nb[2] != 0 && p.nb[2] != p.n[2])) {
-      why = "transmissive poles need both poles, periodic even x3, blocks spanning x3";
+    // blocks that cut x3 come in an even number, so that half a turn is a whole number of blocks
+    const bool cut_ok = p.nb[2] <= 0 || p.nb[2] == p.n[2] || (p.n[2] % p.nb[2] == 0 && (p.n[2] / p.nb[2]) % 2 == 0);
+    if (p.bc_lo[1] != p.bc_hi[1] || p.bc_lo[2] != 0 || p.n[2] % 2 != 0 || !cut_ok) {
+      why = "transmissive poles need both poles, a periodic even x3 and blocks that span x3 or cut it into an even number";
       return false;
     }
   }
@@ -62,6 +64,7 @@ static Grid* grid_new(const Params& par) {
   }
   b.lev1 = 0;
   b.tau = 0;
+  b.xpole_lo = b.xpole_hi = false;
   block_init(par, b);
   return g;
 }

@@ -77,6 +77,9 @@ void blocks_build(Grid& g) {
           b.phys_hi[d] = b.slot[d] == g.nslot[d] - 1 && par.bc_hi[d] != 0;
         }
         b.tau = 0; b.tb_u = 0; b.dt_u = 2; b.has_new = false;
+        // NEXT-1: with x3 cut into blocks the rows beyond a transmissive pole belong to another block
+        b.xpole_lo = b.phys_lo[1] && par.bc_lo[1] == 3 && NB[2] > 1;
+        b.xpole_hi = b.phys_hi[1] && par.bc_hi[1] == 3 && NB[2] > 1;
       }
   for (Block& b : g.blocks) {
     for (int o0 = -1; o0 <= 1; o0++)
@@ -96,6 +99,14 @@ void blocks_build(Grid& g) {
               inside ? g.lattice[((size_t)s[0] * g.nslot[1] + s[1]) * g.nslot[2] + s[2]] : -1;
         }
   }
+  for (Block& b : g.blocks)
+    for (int o0 = -1; o0 <= 1; o0++)
+      for (int o2 = -1; o2 <= 1; o2++) {
+        const int s0 = b.slot[0] + o0;                   // x1 is never periodic together with a pole
+        const int s2 = ((b.slot[2] + g.nslot[2] / 2 + o2) % g.nslot[2] + g.nslot[2]) % g.nslot[2];
+        const bool inside = s0 >= 0 && s0 < g.nslot[0] && (b.xpole_lo || b.xpole_hi);
+        b.pnbr[o0 + 1][o2 + 1] = inside ? g.lattice[((size_t)s0 * g.nslot[1] + b.slot[1]) * g.nslot[2] + s2] : -1;
+      }
   for (Block& b : g.blocks) {
     // C-16 ghost geometry on a refined x1 level uses the block's own (fine or coarse) spacing
     if (b.lev1) {
@@ -126,6 +137,19 @@ static inline double sample(const Block& q, const std::vector<double>& an, const
   return (1.0 - w) * an[z] + w * ah[z];
 }
 
+// NEXT-1 on blocks that cut x3 (fill_polar_transmit in orc_grid.cpp is the same rule inside one
+// block): ghost row j beyond a transmissive pole is the mirror row of the block half a turn away, at the same
+// local x3 index; ut^2 and Bf^2 change sign.
+static inline bool across_pole(const Block& b, int o1) { return (o1 < 0 && b.xpole_lo) || (o1 > 0 && b.xpole_hi); }
+static inline int pole_mirror(const Block& b, int j, bool face2) {
+  if (j < 0) return face2 ? -j : -j - 1;
+  return b.n[1] - (j - (face2 ? b.n[1] : b.n[1] - 1));
+}
+// x3 grouping of the SOURCE row js (of x2-face js: the coarser of the two rows it separates)
+static inline int pole_group(const Block& b, int js, bool face2) {
+  return face2 ? std::max(b.mrow[js - 1 + NG], b.mrow[js + NG]) : b.mrow[js + NG];
+}
+
 static void exchange_block(Grid& g, Block& b, Fields& dst, long long s_u) {
   auto off = [](int idx, int n, bool face) { return idx < 0 ? -1 : (idx > (face ? n : n - 1) ? 1 : 0); };
   for (int i = -NG; i < b.n[0] + NG + 1; i++)
@@ -144,13 +168,17 @@ static void exchange_block(Grid& g, Block& b, Fields& dst, long long s_u) {
             if (o[d] != 0) ghost = true;
           }
           if (!valid) continue;
-          int qi = b.nbr[o[0] + 1][o[1] + 1][o[2] + 1];   // the block itself if no offset
+          const bool xp = across_pole(b, o[1]);
+          // the block itself if no offset
+          int qi = xp ? b.pnbr[o[0] + 1][o[2] + 1] : b.nbr[o[0] + 1][o[1] + 1][o[2] + 1];
           if (qi < 0) continue;                          // outside the domain: physical boundary
           for (int d = 0; d < 3; d++) lq[d] = id[d] - o[d] * b.n[d];
+          if (xp) lq[1] = pole_mirror(b, j, a == 2);
           // C-15: the phi-ghost slots of a derefined row are in group units
           if (o[2] != 0) {
             // an x2-face array follows the grouping of its face, the coarser of the two rows it separates
-            const int mg = a == 2 ? std::max(b.mrow[std::max(j - 1, -NG) + NG], b.mrow[j + NG]) : b.mrow[j + NG];
+            const int mg = xp ? pole_group(b, lq[1], a == 2)
+                              : (a == 2 ? std::max(b.mrow[std::max(j - 1, -NG) + NG], b.mrow[j + NG]) : b.mrow[j + NG]);
             int o2;
             if (mg > 1) lq[2] = deref_ghost_k(k, b.n[2], mg, a == 3, o2);
           }
@@ -160,7 +188,7 @@ static void exchange_block(Grid& g, Block& b, Fields& dst, long long s_u) {
             const int d = a - 1;
             int o2[3] = {o[0], o[1], o[2]};
             o2[d] = id[d] == 0 ? -1 : 1;
-            const int q2 = b.nbr[o2[0] + 1][o2[1] + 1][o2[2] + 1];
+            const int q2 = xp ? b.pnbr[o2[0] + 1][o2[2] + 1] : b.nbr[o2[0] + 1][o2[1] + 1][o2[2] + 1];
             if (q2 >= 0 && g.blocks[q2].tau < g.blocks[qi].tau && g.blocks[q2].lev1 == g.blocks[qi].lev1) {
               qi = q2;
               lq[d] = id[d] == 0 ? b.n[d] : 0;
@@ -172,10 +200,14 @@ static void exchange_block(Grid& g, Block& b, Fields& dst, long long s_u) {
           if (q.lev1 != b.lev1) continue;                // coarse <-> fine: exchange_refined()
           const size_t zq = q.idx(lq[0], lq[1], lq[2]);
           if (a == 0) {
-            for (int c = 0; c < 5; c++) dst.P[c][z] = sample(q, q.sn.P[c], q.sh.P[c], q.snew.P[c], zq, s_u);
+            for (int c = 0; c < 5; c++) {
+              const double v = sample(q, q.sn.P[c], q.sh.P[c], q.snew.P[c], zq, s_u);
+              dst.P[c][z] = (xp && c == 3) ? -v : v;
+            }
           } else {
             const int d = a - 1;
-            dst.Bf[d][z] = sample(q, q.sn.Bf[d], q.sh.Bf[d], q.snew.Bf[d], zq, s_u);
+            const double v = sample(q, q.sn.Bf[d], q.sh.Bf[d], q.snew.Bf[d], zq, s_u);
+            dst.Bf[d][z] = (xp && d == 1) ? -v : v;
           }
         }
       }
@@ -202,12 +234,13 @@ static void exchange_refined(Grid& g, Block& b, Fields& dst, long long s_u) {
     const int o0 = side ? 1 : -1;
     for (int o1 = -1; o1 <= 1; o1++)
       for (int o2 = -1; o2 <= 1; o2++) {
-        const int qi = b.nbr[o0 + 1][o1 + 1][o2 + 1];
+        const bool xp = across_pole(b, o1);
+        const int qi = xp ? b.pnbr[o0 + 1][o2 + 1] : b.nbr[o0 + 1][o1 + 1][o2 + 1];
         if (qi < 0 || g.blocks[qi].lev1 == b.lev1) continue;
         const Block& q = g.blocks[qi];
         // the block on b's own side of the interface in the same transverse position (b itself for
         // o1 = o2 = 0): it covers the zones just outside q
-        const int ri = b.nbr[1][o1 + 1][o2 + 1];
+        const int ri = xp ? b.pnbr[1][o2 + 1] : b.nbr[1][o1 + 1][o2 + 1];
         const Block& r = g.blocks[ri];
         const int n0 = b.n[0];
         // ranges of the padded indices that fall into q
@@ -227,8 +260,9 @@ static void exchange_refined(Grid& g, Block& b, Fields& dst, long long s_u) {
             for (int j = lo[1]; j <= hi[1]; j++)
               for (int k = lo[2]; k <= hi[2]; k++) {
                 int o2u;
-                const int lj = j - o1 * b.n[1];
-                const int mg = fd == 1 ? std::max(b.mrow[std::max(j - 1, -NG) + NG], b.mrow[j + NG]) : b.mrow[j + NG];
+                const int lj = xp ? pole_mirror(b, j, fd == 1) : j - o1 * b.n[1];
+                const int mg = xp ? pole_group(b, lj, fd == 1)
+                                  : (fd == 1 ? std::max(b.mrow[std::max(j - 1, -NG) + NG], b.mrow[j + NG]) : b.mrow[j + NG]);
                 const int lk = o2 != 0 ? deref_ghost_k(k, b.n[2], mg, fd == 2, o2u) : k;
                 const int nk = kind == 0 ? 5 : 1;
                 for (int c = 0; c < nk; c++) {
@@ -269,6 +303,7 @@ static void exchange_refined(Grid& g, Block& b, Fields& dst, long long s_u) {
                       v = 0.5 * (a3[1] + (high_half ? aR : aL));
                     }
                   }
+                  if (xp && (kd == 3 || fd == 1)) v = -v;   // ut^2, Bf^2 reverse across the pole
                   if (kind == 0) dst.P[c][b.idx(i, j, k)] = v;
                   else dst.Bf[fd][b.idx(i, j, k)] = v;
                 }
@@ -598,6 +633,10 @@ static void assign_levels(Grid& g) {
         int t = b.tau;
         for (int a = 0; a < 27; a++) {
           const int q = (&b.nbr[0][0][0])[a];
+          if (q >= 0) t = std::min(t, g.blocks[q].tau + 1);
+        }
+        for (int a = 0; a < 9; a++) {   // the blocks across a transmissive pole are neighbours too
+          const int q = (&b.pnbr[0][0])[a];
           if (q >= 0) t = std::min(t, g.blocks[q].tau + 1);
         }
         nt[i] = t;

@@ -133,7 +133,17 @@ static void fill_polar_transmit(const Block& b, std::vector<double>& a, bool do_
 
 void fill_physical_bc(const Params& par, Block& b, Fields& s) {
   for (int d = 0; d < 3; d++) {  // order x1, x2, x3 so that edge and corner ghosts are defined
-    const bool lo = b.phys_lo[d], hi = b.phys_hi[d];
+    bool lo = b.phys_lo[d], hi = b.phys_hi[d];
+    // a transmissive pole on blocks that cut x3 is closed by the block exchange (orc_blocks.cpp)
+    if (d == 1 && (b.xpole_lo || b.xpole_hi)) {
+      for (int i = -NG; i < b.n[0] + NG + 1; i++)
+        for (int k = -NG; k < b.n[2] + NG + 1; k++) {   // Bf^2 on the pole face is 0 (zero area)
+          if (lo && b.xpole_lo) s.Bf[1][b.idx(i, 0, k)] = 0.0;
+          if (hi && b.xpole_hi) s.Bf[1][b.idx(i, b.n[1], k)] = 0.0;
+        }
+      lo = lo && !b.xpole_lo;
+      hi = hi && !b.xpole_hi;
+    }
     if (!lo && !hi) continue;
     const int bl = par.bc_lo[d], bh = par.bc_hi[d];
     if (d == 1 && (bl == 3 || bh == 3)) {

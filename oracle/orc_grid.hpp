@@ -34,6 +34,10 @@ struct Block {
   // ---- block-structured grid (C-16, C-17; orc_blocks.cpp) ----
   int slot[3];                     // position in the block lattice (x1 slot, x2 block, x3 block)
   int nbr[3][3][3];                // neighbour block ids by offset (-1: outside the domain)
+  // NEXT-1 on blocks that cut x3: the ghost rows beyond a transmissive pole lie in the block row half a turn
+  // away; pnbr[o0 + 1][o2 + 1] is the block at (slot0 + o0, same slot1, slot2 + nslot2 / 2 + o2)
+  bool xpole_lo, xpole_hi;
+  int pnbr[3][3];
   long long tb_u, dt_u;            // LAT: time of sn and own step, in units of (finest dt)/2
   bool has_new;                    // snew holds the completed state at tb_u + dt_u
   std::vector<double> FA[3][5];    // flux register R1: dt_b * F of the latest corrector (C-17)
