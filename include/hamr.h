@@ -45,7 +45,8 @@ typedef enum {
 typedef enum { HAMR_METRIC_MINKOWSKI = 0, HAMR_METRIC_KERR_SCHILD = 1 } hamr_metric_t;
 /* HAMR_BC_POLAR_TRANSMIT (x2 only, both sides, "transmissive polar boundary"): the ghost zone beyond
  * the pole is the zone on the mirror row half a turn away in x3, with the x2 components (ut2, Bf2) changing sign;
- * needs an even N3, periodic x3 of extent 2 pi, and blocks that span x3. */
+ * needs an even N3, a periodic x3 of extent 2 pi, and blocks that span x3 or cut it into an EVEN number (the
+ * rows beyond the pole then come from the block half a turn away). */
 typedef enum { HAMR_BC_PERIODIC = 0, HAMR_BC_OUTFLOW = 1, HAMR_BC_POLAR_REFLECT = 2, HAMR_BC_POLAR_TRANSMIT = 3 } hamr_bc_t;
 typedef enum { HAMR_RECON_PPM = 0, HAMR_RECON_PLM_MC = 1 } hamr_recon_t;
 

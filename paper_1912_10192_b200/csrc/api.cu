@@ -38,8 +38,10 @@ bool params_ok(const hamr_params& p, std::string& why) {
     if (p.bc_lo[d] != HAMR_BC_PERIODIC && p.n[d] < NG) { why = "non-periodic dimension needs n >= 3"; return false; }
   }
   if (p.bc_lo[1] == HAMR_BC_POLAR_TRANSMIT || p.bc_hi[1] == HAMR_BC_POLAR_TRANSMIT) {
-    if (p.bc_lo[1] != p.bc_hi[1] || p.bc_lo[2] != HAMR_BC_PERIODIC || p.n[2] % 2 != 0 || (p.nb[2] != 0 && p.nb[2] != p.n[2])) {
-      why = "transmissive poles need both poles, a periodic even x3 and blocks that span x3";
+    // blocks that cut x3 come in an even number: half a turn is then a whole number of blocks
+    const bool cut_ok = p.nb[2] <= 0 || p.nb[2] == p.n[2] || (p.n[2] % p.nb[2] == 0 && (p.n[2] / p.nb[2]) % 2 == 0);
+    if (p.bc_lo[1] != p.bc_hi[1] || p.bc_lo[2] != HAMR_BC_PERIODIC || p.n[2] % 2 != 0 || !cut_ok) {
+      why = "transmissive poles need both poles, a periodic even x3 and blocks that span x3 or cut it into an even number";
       return false;
     }
   }

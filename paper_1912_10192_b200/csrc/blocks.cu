@@ -96,22 +96,39 @@ __device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, 
     const int mg = sd == 1 ? max(mj, __ldg(Dv.mrow + max(J - 1, -NG) + NG)) : mj;
     if (mg > 1) kz = deref_ghost_k(id[2], L.n[2], mg);
   }
-  // NEXT-1 transmissive pole: the mirror row's zone half a turn away in x3 (the block spans x3)
+  const int* nb = Dv.B.nbr + b * NNBR;
+  // NEXT-1 transmissive pole: the mirror row's zone half a turn away in x3: inside the block if
+  // it spans x3, else at the same local index of the block half the x3 block count further (xp: the nine
+  // such blocks replace the neighbour table)
+  bool xp = false;
   if (((s.negmask >> 1) & 1) && Dv.bc_lo[1] == HAMR_BC_POLAR_TRANSMIT) {
-    const int n3 = L.n[2];
-    kz = (kz % n3 + n3 / 2) % n3;
-    o[2] = 0;
+    xp = __ldg(nb + 27 + 4) >= 0;
+    if (xp) {
+      if (Dv.mrow && o[2] != 0) {   // C-15 group units follow the SOURCE row (face) m[1]
+        const int J = Dv.B.info[b].w + m[1];
+        const int mj = __ldg(Dv.mrow + J + NG);
+        const int mg = sd == 1 ? max(mj, __ldg(Dv.mrow + J - 1 + NG)) : mj;
+        kz = mg > 1 ? deref_ghost_k(id[2], L.n[2], mg) : m[2] - o[2] * L.n[2];
+      }
+    } else {
+      const int n3 = L.n[2];
+      kz = (kz % n3 + n3 / 2) % n3;
+      o[2] = 0;
+    }
   }
-  const int* nb = Dv.B.nbr + b * 27;
-  s.ghost = (o[0] | o[1] | o[2]) != 0;
-  s.q = s.ghost ? __ldg(nb + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1)) : b;
+  // neighbour by offset; across the pole the x2 offset is spent on the mirror
+  auto nbq = [&](int a0, int a1, int a2) {
+    return __ldg(xp ? nb + 27 + (a0 + 1) * 3 + (a2 + 1) : nb + (a0 + 1) * 9 + (a1 + 1) * 3 + (a2 + 1));
+  };
+  s.ghost = xp || (o[0] | o[1] | o[2]) != 0;
+  s.q = s.ghost ? nbq(o[0], o[1], o[2]) : b;
   int lq[3] = {m[0] - o[0] * L.n[0], m[1] - o[1] * L.n[1], kz};
   // C-17: a face on the plane between two blocks on different time levels has ONE value in every stage
   // source, that of the finer block
   if (!norule && sd >= 0 && (m[sd] == 0 || m[sd] == L.n[sd])) {
     int o2[3] = {o[0], o[1], o[2]};
     o2[sd] = m[sd] == 0 ? -1 : 1;
-    const int q2 = __ldg(nb + (o2[0] + 1) * 9 + (o2[1] + 1) * 3 + (o2[2] + 1));
+    const int q2 = (xp && sd == 1) ? -1 : nbq(o2[0], o2[1], o2[2]);
     if (q2 >= 0 && s.q >= 0 && Dv.B.tau[q2] < Dv.B.tau[s.q] && Dv.B.info[q2].y == Dv.B.info[s.q].y) {
       s.q = q2;
       lq[sd] = m[sd] == 0 ? L.n[sd] : 0;
@@ -124,7 +141,7 @@ __device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, 
   s.ref = false;
   if (!norule && o[0] != 0 && s.q >= 0 && Dv.B.info[s.q].y != Dv.B.info[b].y) {
     s.ref = true;
-    s.rq = __ldg(nb + 9 + (o[1] + 1) * 3 + (o[2] + 1));
+    s.rq = nbq(0, o[1], o[2]);
     s.side = o[0] > 0 ? 1 : 0;
     s.mi = m[0]; s.lj = lq[1]; s.lk = lq[2];
   }
@@ -271,7 +288,7 @@ __global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(Dev Dv, Buf
   const int cur = Dv.B.cur[b];
   const int own = role == 0 ? cur : 1;
   const long long z = (long long)b * Dv.B.blen + L.idx(id[0], id[1], id[2]);
-  const int* nb = Dv.B.nbr + b * 27;
+  const int* nb = Dv.B.nbr + b * NNBR;
 
   if ((flags & 1) && !all) {
     // ---- fast path: plain copies from same-level neighbours ------------------------------------------
@@ -506,7 +523,7 @@ __device__ __forceinline__ double blk_edge_ec(const Dev& Dv, int c, int tc, int 
       if (cand[t][0] == 0 && cand[t][1] == 0) continue;
       int o[3] = {0, 0, 0};
       o[d] = cand[t][0]; o[e] = cand[t][1];
-      const int q = __ldg(Dv.B.nbr + c * 27 + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
+      const int q = __ldg(Dv.B.nbr + c * NNBR + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
       if (q < 0 || Dv.B.tau[q] != tc - 1) continue;
       int lq[3] = {id[0], id[1], id[2]};
       lq[d] -= o[d] * L.n[d];
@@ -530,7 +547,7 @@ __device__ __forceinline__ bool blk_face_corr(const Dev& Dv, const Bufs& B, int 
   if (id[d] == 0 || id[d] == L.n[d]) {
     int o[3] = {0, 0, 0};
     o[d] = id[d] == 0 ? -1 : 1;
-    const int q = __ldg(Dv.B.nbr + c * 27 + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
+    const int q = __ldg(Dv.B.nbr + c * NNBR + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
     if (q >= 0 && Dv.B.tau[q] == tc - 1) {
       if (want_value) {
         int lq[3] = {id[0], id[1], id[2]};
@@ -623,7 +640,7 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
           if ((side == 0 && id[d] == 0) || (side == 1 && id[d] == L.n[d] - 1)) {
             int o[3] = {0, 0, 0};
             o[d] = side ? 1 : -1;
-            const int q = __ldg(Dv.B.nbr + c * 27 + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
+            const int q = __ldg(Dv.B.nbr + c * NNBR + (o[0] + 1) * 9 + (o[1] + 1) * 3 + (o[2] + 1));
             if (q >= 0 && Dv.B.tau[q] == tc - 1) {
               int lq[3] = {id[0], id[1], id[2]};
               lq[d] = side ? 0 : L.n[d];
@@ -847,7 +864,7 @@ __global__ void __launch_bounds__(128) k_blk_iface(Dev Dv) {
   const int side = (int)(t / (unsigned)(c1 * c2));
   t -= side * c1 * c2;
   const int j = (int)(t / (unsigned)c2), k = (int)(t - (t / (unsigned)c2) * c2);
-  const int q = __ldg(Dv.B.nbr + c * 27 + (side ? 2 : 0) * 9 + 4);
+  const int q = __ldg(Dv.B.nbr + c * NNBR + (side ? 2 : 0) * 9 + 4);
   if (q < 0 || Dv.B.info[q].y == 0 || Dv.B.tau[q] != Dv.B.tau[c]) return;
   const long long zc = (long long)c * Dv.B.blen + L.idx(side ? L.n[0] : 0, j, k);
   const long long zq = (long long)q * Dv.B.blen + L.idx(side ? 0 : L.n[0], j, k);
@@ -912,8 +929,8 @@ static cudaError_t blk_upload_flags(hamr_grid* g) {
   int* hf = H.h_ints + (size_t)9 * H.nblk;
   for (int b = 0; b < H.nblk; b++) {
     bool same = true, finer = false;
-    for (int a = 0; a < 27; a++) {
-      const int q = H.nbr[(size_t)b * 27 + a];
+    for (int a = 0; a < NNBR; a++) {
+      const int q = H.nbr[(size_t)b * NNBR + a];
       if (q < 0) continue;
       if (H.tau[q] != H.tau[b] || H.lev1[q] != H.lev1[b]) same = false;
       if (H.tau[q] < H.tau[b]) finer = true;
@@ -981,8 +998,8 @@ int blk_has_refinement(const hamr_params& p) {
 }
 
 size_t blk_table_bytes(int nblk) {
-  // info (int4), nbr (27), phys, K0, tau, cur, flags, 5 lists, 4 correction lists, ctopb (3 doubles)
-  return ((size_t)nblk * (16 + 4 * (27 + 5 + 5 + 4 + 5) + 24) + 1024 + 255) / 256 * 256;
+  // info (int4), nbr (NNBR), phys, K0, tau, cur, flags, 5 lists, 4 correction lists, ctopb (3 doubles)
+  return ((size_t)nblk * (16 + 4 * (NNBR + 5 + 5 + 4 + 5) + 24) + 1024 + 255) / 256 * 256;
 }
 
 // C-16: block lattice, neighbour table (periodic dimensions close through it), per-block table offsets
@@ -995,7 +1012,7 @@ int blk_setup(hamr_grid* g, void* tables) {
   H.on = true;
   H.nblk = nblk;
   H.tmax = p.lat_max_level > 0 ? p.lat_max_level : 0;
-  H.nbr.assign((size_t)nblk * 27, -1);
+  H.nbr.assign((size_t)nblk * NNBR, -1);
   H.lev1.assign(nblk, 0);
   H.tau.assign(nblk, 0);
   H.I0.assign((size_t)nblk * 3, 0);
@@ -1042,13 +1059,22 @@ int blk_setup(hamr_grid* g, void* tables) {
                   else inside = false;
                 }
               }
-              H.nbr[(size_t)b * 27 + (o0 + 1) * 9 + (o1 + 1) * 3 + (o2 + 1)] = inside ? id_of(q[0], q[1], q[2]) : -1;
+              H.nbr[(size_t)b * NNBR + (o0 + 1) * 9 + (o1 + 1) * 3 + (o2 + 1)] = inside ? id_of(q[0], q[1], q[2]) : -1;
             }
+        // NEXT-1 on blocks that cut x3: the rows beyond a transmissive pole lie in the block half a turn away
+        const bool xpole = H.nslot[2] > 1 && ((s1 == 0 && p.bc_lo[1] == HAMR_BC_POLAR_TRANSMIT) ||
+                                              (s1 == H.nslot[1] - 1 && p.bc_hi[1] == HAMR_BC_POLAR_TRANSMIT));
+        for (int o0 = -1; o0 <= 1; o0++)
+          for (int o2 = -1; o2 <= 1; o2++) {
+            const int q0 = s0 + o0, q2 = ((s2 + H.nslot[2] / 2 + o2) % H.nslot[2] + H.nslot[2]) % H.nslot[2];
+            H.nbr[(size_t)b * NNBR + 27 + (o0 + 1) * 3 + (o2 + 1)] =
+                (xpole && q0 >= 0 && q0 < H.nslot[0]) ? id_of(q0, s1, q2) : -1;
+          }
       }
   char* t = (char*)tables;
   auto take = [&](size_t bytes) { char* r = t; t += (bytes + 15) / 16 * 16; return r; };
   int4* d_info = (int4*)take((size_t)nblk * 16);
-  int* d_nbr = (int*)take((size_t)nblk * 27 * 4);
+  int* d_nbr = (int*)take((size_t)nblk * NNBR * 4);
   int* d_phys = (int*)take((size_t)nblk * 4);
   int* d_K0 = (int*)take((size_t)nblk * 4);
   B.tau = (int*)take((size_t)nblk * 4);
@@ -1074,7 +1100,7 @@ int blk_setup(hamr_grid* g, void* tables) {
     if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st);
   };
   up(d_info, info.data(), (size_t)nblk * 16);
-  up(d_nbr, H.nbr.data(), (size_t)nblk * 27 * 4);
+  up(d_nbr, H.nbr.data(), (size_t)nblk * NNBR * 4);
   up(d_phys, phys.data(), (size_t)nblk * 4);
   up(d_K0, K0.data(), (size_t)nblk * 4);
   up(H.d_lists, all.data(), (size_t)nblk * 4);                       // level 0 list (every block at tau = 0)
@@ -1292,8 +1318,8 @@ static int blk_assign(hamr_grid* g, bool after_step) {
     changed = false;
     for (int b = 0; b < nblk; b++) {
       int t = H.tau[b];
-      for (int a = 0; a < 27; a++) {
-        const int q = H.nbr[(size_t)b * 27 + a];
+      for (int a = 0; a < NNBR; a++) {
+        const int q = H.nbr[(size_t)b * NNBR + a];
         if (q >= 0) t = std::min(t, H.tau[q] + 1);
       }
       nt[b] = t;
@@ -1308,8 +1334,8 @@ static int blk_assign(hamr_grid* g, bool after_step) {
     const int t = H.tau[b];
     hl[(size_t)t * nblk + H.nlist[t]++] = b;
     bool any = false;
-    for (int a = 0; a < 27 && !any; a++) {
-      const int q = H.nbr[(size_t)b * 27 + a];
+    for (int a = 0; a < 27 && !any; a++) {   // (a block across the pole shares no face or edge)
+      const int q = H.nbr[(size_t)b * NNBR + a];
       any = q >= 0 && H.tau[q] == t - 1;
     }
     if (any) hl[(size_t)(4 + t) * nblk + H.nclist[t]++] = b;

@@ -172,7 +172,7 @@ __global__ void __launch_bounds__(128) k_deref_flux_layers(Dev Dv) {
   if (M == 1) return;
   int q = C.b;
   if (BLK) {
-    q = __ldg(Dv.B.nbr + C.b * 27 + 12 + (side ? 2 : 0));       // offset (0, 0, -1) / (0, 0, +1)
+    q = __ldg(Dv.B.nbr + C.b * NNBR + 12 + (side ? 2 : 0));       // offset (0, 0, -1) / (0, 0, +1)
     if (q < 0 || Dv.B.tau[q] != Dv.B.tau[C.b] || Dv.B.info[q].y != C.lev) return;
   }
   const long long zd = C.zoff + L.idx(i, j, side ? n3 : -1);

@@ -17,6 +17,7 @@
 namespace hamr {
 
 constexpr int NG = 3;     // ghost layers: a PPM face needs zones j-3 .. j+2 (C-5)
+constexpr int NNBR = 36;  // entries per block of the neighbour table (27 by offset + 9 across a transmissive pole)
 constexpr int LEAD = 13;  // leading pad so that active zone k = 0 sits on a 128-byte boundary
 
 // ---- array layout ------------------------------------------------------------------------------

@@ -35,7 +35,8 @@ struct BlkDev {
   const int* dlist;          // [ndact] those of them that hold phi-derefined rows (C-15 kernels); NULL: use list
   int ndact;
   const int4* info;          // [nblk] {table index of local zone (0,0), x1 level, I0, J0}
-  const int* nbr;            // [nblk][27] neighbour block by offset, -1 outside the domain
+  const int* nbr;            // [nblk][NNBR]: 27 neighbour blocks by offset (-1 outside the domain), then the 9 blocks
+                             // half a turn away across a transmissive pole, by (o0 + 1) * 3 + (o2 + 1) (NEXT-1; -1 if none)
   const int* phys;           // [nblk] bit d: low side of dim d is a physical boundary, bit 3+d: high side
   const int* K0;             // [nblk] global x3 index of local zone 0
   int* tau;                  // [nblk] LAT time level (C-17)
@@ -111,7 +112,7 @@ struct BlkHost {
   bool refined;              // some block columns carry the x1 refinement level (C-16)
   int nblk, tmax;            // blocks; highest LAT level (0: one global dt)
   int nslot[3];              // block lattice extents
-  std::vector<int> nbr;      // [nblk][27] host mirror of the neighbour table
+  std::vector<int> nbr;      // [nblk][NNBR] host mirror of the neighbour table
   std::vector<int> lev1;     // [nblk] x1 refinement level
   std::vector<int> tau;      // [nblk] current time level
   std::vector<int> I0;       // [nblk][3]

@@ -40,10 +40,11 @@ def _run_pair(H, orc, p, hyd, bf, fin=1):
     assert g.divb() <= TOL_DIVB and g.stats()[0] == 0 and o.stats()[0] == 0
 
 
-@pytest.mark.parametrize("extra", [dict(), dict(nb=(16, 8, 32))])
+@pytest.mark.parametrize("extra", [dict(), dict(nb=(16, 8, 32)), dict(nb=(16, 8, 8)), dict(nb=(32, 32, 16))])
 def test_tilted_disk_through_the_poles(H, orc, extra):
     # a thick (h/r = 0.1) version of the cfg 3 stand-in so that 64x32x32 resolves it: the inclined disk and its
-    # field cross both poles.  Monolithic ghost kernel, then the block ghost kernel.
+    # field cross both poles.  Monolithic ghost kernel, then the block ghost kernel on blocks that span x3 and
+    # on blocks that cut it (the rows beyond the pole come from the block half a turn away).
     p = I.tilted_disk_params(n=(64, 32, 32), **TRANSMIT, **extra)
     hyd, bf = I.tilted_disk(p, seed=3, hr=0.1)
     _run_pair(H, orc, p, hyd, bf)
@@ -56,6 +57,44 @@ def test_transmissive_poles_with_blocks_deref_and_lat(H, orc):
                        deref_factor=(2, 4), **TRANSMIT)
     hyd, bf = I.fm_torus(p, seed=4, pert=0.1)
     _run_pair(H, orc, p, hyd, bf, fin=2)
+
+
+def test_transmissive_poles_on_phi_cut_blocks_with_deref_refinement_and_lat(H, orc):
+    # everything at once on blocks that cut x3 (BASELINE cfg 4's block shape with the paper's pole): derefined
+    # polar rows (group-unit phi ghosts across the pole), one x1 refinement level (restriction / prolongation in
+    # the pole corner), two time levels
+    p = I.torus_params(n=(32, 16, 32), nb=(8, 4, 16), lat_max_level=1, deref_theta_deg=(30.0, 12.0),
+                       deref_factor=(2, 4), r_refine_max=4.0, **TRANSMIT)
+    g, o = H.Grid(p), orc.OrcGrid(p)
+    infos = []
+    for b in range(o.num_blocks()):
+        d = o.block_info(b)
+        infos.append((d["x_lo"], d["dx"], d["n"]))
+    assert any(o.block_info(b)["lev1"] for b in range(o.num_blocks()))
+    for b, (hyd, bf) in enumerate(I.fm_torus_blocks(p, infos, seed=4, pert=0.1)):
+        assert g.set_block_prims(b, hyd, bf) == 0 and o.set_block_prims(b, hyd, bf) == 0
+    assert g.commit() == 0 and o.commit() == 0
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt and g.levels() == list(o.levels())
+    assert len(set(g.levels())) == 2
+
+    def check(tol):
+        worst = {}
+        for b, (x_lo, dx, n) in enumerate(infos):
+            e = parity_errors(I.block_as_grid(p, x_lo, dx, n), o.get_block_prims(b), g.get_block_prims(b))
+            for k, v in e.items():
+                worst[k] = max(worst.get(k, 0.0), v)
+            for a, c in zip(o.get_block_bface(b), g.get_block_bface(b)):
+                assert np.abs(a - c).max() <= tol * max(np.abs(a).max(), 1e-300)
+        assert max(worst.values()) <= tol, worst
+
+    g.step(1)
+    o.step(1)
+    check(2 * TOL_1)
+    if g.levels() == list(o.levels()):
+        g.step(3)
+        o.step(3)
+        check(TOL_10)
+    assert g.divb() <= TOL_DIVB and g.stats()[0] == 0 and o.stats()[0] == 0
 
 
 def test_transmit_differs_from_reflect_and_torus_agrees(H):

@@ -107,12 +107,18 @@ def test_refined_torus(H, orc, extra):
         _check_blocks(p, infos, o, g, TOL_10)
 
 
-def test_cfg4_full_size_one_coarse_step(H, orc):
+@pytest.mark.parametrize("pole", ["reflect", "transmit"])
+def test_cfg4_full_size_one_coarse_step(H, orc, pole):
     """BASELINE cfg 4 at full size in the launch configuration bench.py --workload cfg4 times (1472 blocks of 16^3,
     6 029 312 zones, refinement r < 20, derefinement 2x / 4x, LAT levels 1 / 2 / 4): every zone of every block after one
-    coarse step (= 4 finest steps) against the oracle."""
+    coarse step (= 4 finest steps) against the oracle.  "transmit": the same grid with the paper's own polar
+    boundary (NEXT-1), the pole ghosts of every polar block coming from the block half a turn away."""
+    bc = {}
+    if pole == "transmit":
+        bc = dict(bc_lo=(I.BC_OUTFLOW, I.BC_POLAR_TRANSMIT, I.BC_PERIODIC),
+                  bc_hi=(I.BC_OUTFLOW, I.BC_POLAR_TRANSMIT, I.BC_PERIODIC))
     p = I.torus_params(n=(256, 128, 128), r_out=1000.0, nb=(16, 16, 16), lat_max_level=2, r_refine_max=20.0,
-                       deref_theta_deg=(15.0, 5.0), deref_factor=(2, 4))
+                       deref_theta_deg=(15.0, 5.0), deref_factor=(2, 4), **bc)
     g, o = H.Grid(p), orc.OrcGrid(p)
     assert g.num_blocks() == o.num_blocks() == 1472
     infos = _infos(o)
