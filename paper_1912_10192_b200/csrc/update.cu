@@ -35,10 +35,15 @@ __device__ __forceinline__ Fields pick_fields(const Fields& a, const Fields& b, 
 #ifndef HAMR_UPD_MINB
 #define HAMR_UPD_MINB 6  // 80 regs (72 B spilled); 4 / 5 measured 4 % / 7 % slower with the reload, 8 slower still
 #endif
+#ifndef HAMR_UPD_KFACE
+#define HAMR_UPD_KFACE 1
+#endif
 template <bool SAME, bool BLK>  // SAME: predictor, source state == base state
 __global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
   const Lay& L = Dv.L;
-  const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
+  // k runs over [0, n3): warps start on 128-byte lines when n3 is a multiple of 32; the thread at k = 0 also
+  // builds the x3-face at k = n3
+  const int c2 = L.n[2] + (HAMR_UPD_KFACE ? 0 : 1), c1 = L.n[1] + 1;
   // 32-bit index arithmetic throughout: 64-bit division is emulated (~100 instructions each)
   const unsigned per = (unsigned)(L.n[0] + 1) * c1 * c2;
   unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -69,6 +74,7 @@ __global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra,
       out.Bf[1][z] = lo[1];
     }
     if (in0 && in1) { lo[2] = bf_new<2>(Dv, base.Bf[2], z, dt, S, idx); out.Bf[2][z] = lo[2]; }
+    if (HAMR_UPD_KFACE && in0 && in1 && k == 0) out.Bf[2][z + L.n[2]] = bf_new<2>(Dv, base.Bf[2], z + L.n[2], dt, S, idx);
     if (in0 && in1 && in2) {
       const int q = C.q0 + i * (BLK ? Dv.B.ge2 : L.e2) + j;
       const double* grec = Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)q * NREC_C;
@@ -206,7 +212,7 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
   const Lay& L = Dv.L;
   const bool blk = Dv.B.nblk > 0;
   if (blk && Dv.B.nact == 0) return;
-  const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1) * (blk ? Dv.B.nact : 1);
+  const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + (HAMR_UPD_KFACE ? 0 : 1)) * (blk ? Dv.B.nact : 1);
   const unsigned nb = (unsigned)((tot + 127) / 128);
   Launch l_(g, same ? K_UPDATE_P : K_UPDATE_C);
   if (same && !blk) k_update<true, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
