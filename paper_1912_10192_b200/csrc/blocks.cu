@@ -37,6 +37,17 @@ __device__ __forceinline__ const double* buf_arr(const Bufs& B, int buf, int kin
   return buf == 0 ? a0 : (buf == 1 ? a1 : a2);
 }
 
+// k_blk_ghosts calls these from eleven places (370 KB of code).  Out of line the kernel is SLOWER (measured on
+// cfg 4: 0.396 -> 0.494 ms with both, 0.423 with blk_fetch_ref alone): the calls spill their arguments
+#ifndef HAMR_GHOST_SHELL
+#define HAMR_GHOST_SHELL 1
+#endif
+#ifndef HAMR_REF_INLINE
+#define HAMR_REF_INLINE __forceinline__
+#endif
+#ifndef HAMR_SRC_INLINE
+#define HAMR_SRC_INLINE __forceinline__
+#endif
 template <typename T>
 __device__ __forceinline__ T pick4(const T v[4], int i) {
   return i == 0 ? v[0] : (i == 1 ? v[1] : (i == 2 ? v[2] : v[3]));
@@ -62,7 +73,7 @@ struct GSrc {
 
 // sd: the array is staggered along sd (-1: zone-centred)
 // norule: every neighbour is on b's own time level, so no face is owned by a finer block
-__device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, const int id[3], bool norule) {
+__device__ HAMR_SRC_INLINE GSrc blk_src(const Dev& Dv, int b, int phys, int sd, const int id[3], bool norule) {
   const Lay& L = Dv.L;
   int m[3], o[3];
   GSrc s;
@@ -181,7 +192,7 @@ __device__ __forceinline__ double blk_at(const Dev& Dv, const Bufs& B, int kind,
 // coarse values (the coarse value beyond the interface is the restriction of the fine block rq), a quarter
 // of a coarse zone off the coarse centre; normal faces copy coincident coarse faces, in-between ones are
 // the mean of their two coarse neighbours.
-__device__ __forceinline__ double blk_fetch_ref(const Dev& Dv, const Bufs& B, const LevT& lt, int levb, int kind,
+__device__ HAMR_REF_INLINE double blk_fetch_ref(const Dev& Dv, const Bufs& B, const LevT& lt, int levb, int kind,
                                                 const GSrc& s, long long s_u) {
   if (s.zero) return 0.0;
   const int n0 = Dv.L.n[0];
@@ -254,7 +265,8 @@ __device__ __forceinline__ double blk_fetch(const Dev& Dv, const Bufs& B, int b,
 // Block flags (host, per level assignment): bit 0 "simple": no physical side and all 26 neighbours on
 // the block's own time level -> every ghost value (B_c included) is a plain copy of the neighbour's
 // stage source; bit 1: some neighbour is on a finer time level (only then can an ACTIVE face change).
-__global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(Dev Dv, Bufs B, LevT lt, int role, long long s_u, int all,
+__global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(const __grid_constant__ Dev Dv, const __grid_constant__ Bufs B,
+                                                    const __grid_constant__ LevT lt, int role, long long s_u, int all,
                                                     int zero_ctop) {
   // grid: x covers the padded locations of one block, y the blocks of the launch; 32-bit index arithmetic
   const Lay& L = Dv.L;
@@ -263,8 +275,41 @@ __global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(Dev Dv, Buf
   if (t >= (unsigned)(L.e1 * L.e2 * e3)) return;
   const int b = __ldg(Dv.B.list + blockIdx.y);
   if (zero_ctop && t == 0) Dv.B.ctopb[b * 3] = Dv.B.ctopb[b * 3 + 1] = Dv.B.ctopb[b * 3 + 2] = 0.0;
-  const unsigned tj = t / (unsigned)e3, ti = tj / (unsigned)L.e2;
-  const int id[3] = {(int)ti - NG, (int)(tj - ti * L.e2) - NG, (int)(t - tj * e3) - NG};
+  int i0, i1, i2;
+  if (HAMR_GHOST_SHELL && !all && !(Dv.B.flags[b] & 2)) {
+    // no finer neighbour: active storage is final, so only the ghost shell is enumerated (whole warps of ghost
+    // slots instead of warps that are two thirds active zones).  Part A: the (i, j) columns outside the active
+    // range, every k; part B: the active columns' 2 NG + 1 ghost slots in k.
+    const int n0 = L.n[0], n1 = L.n[1], gj = 2 * NG + 1;
+    const unsigned lo_rows = (unsigned)(NG * L.e2), mid_rows = (unsigned)(n0 * gj);
+    const unsigned nA = (lo_rows + mid_rows + (unsigned)((NG + 1) * L.e2)) * (unsigned)e3;
+    if (t < nA) {
+      unsigned row = t / (unsigned)e3;
+      i2 = (int)(t - row * e3) - NG;
+      if (row < lo_rows) {
+        i0 = (int)(row / (unsigned)L.e2) - NG; i1 = (int)(row % (unsigned)L.e2) - NG;
+      } else if (row < lo_rows + mid_rows) {
+        row -= lo_rows;
+        i0 = (int)(row / (unsigned)gj);
+        const int q = (int)(row - i0 * gj);
+        i1 = q < NG ? q - NG : n1 + q - NG;
+      } else {
+        row -= lo_rows + mid_rows;
+        i0 = n0 + (int)(row / (unsigned)L.e2); i1 = (int)(row % (unsigned)L.e2) - NG;
+      }
+    } else {
+      const unsigned u = t - nA;
+      const int q = (int)(u & 7);
+      if (q == 7 || u >= (unsigned)(n0 * n1 * 8)) return;
+      const unsigned col = u >> 3;
+      i0 = (int)(col / (unsigned)n1); i1 = (int)(col - i0 * n1);
+      i2 = q < NG ? q - NG : L.n[2] + q - NG;
+    }
+  } else {
+    const unsigned tj = t / (unsigned)e3, ti = tj / (unsigned)L.e2;
+    i0 = (int)ti - NG; i1 = (int)(tj - ti * L.e2) - NG; i2 = (int)(t - tj * e3) - NG;
+  }
+  const int id[3] = {i0, i1, i2};
   bool in_c[3], extra[3];
 #pragma unroll
   for (int d = 0; d < 3; d++) { in_c[d] = id[d] >= 0 && id[d] < L.n[d]; extra[d] = id[d] == L.n[d] + NG; }
