@@ -83,24 +83,17 @@ __global__ void __launch_bounds__(128) k_deref_fix_flux(Dev Dv) {
   const int m = __ldg(Dv.mrow + T.C.J0 + j + NG);
   const int M = max(m, __ldg(Dv.mrow + T.C.J0 + j - 1 + NG));   // x2-face j lies between rows j-1 and j
   const long long zrow = T.C.zoff + L.idx(i, j, 0);
+  // blockIdx.y: the quantity (five hydro fluxes, the two transverse face EMFs): seven independent threads per
+  // group instead of one thread walking 21 read-modify-write chains one after the other
+  const int c = blockIdx.y;
+  double* const a0 = c < 5 ? Dv.F[0][c] : (c == 5 ? Dv.EfA[0] : Dv.EfB[0]);
+  double* const a1 = c < 5 ? Dv.F[1][c] : (c == 5 ? Dv.EfA[1] : Dv.EfB[1]);
+  double* const a2 = c < 5 ? Dv.F[2][c] : (c == 5 ? Dv.EfA[2] : Dv.EfB[2]);
   if (m > 1 && k % m == 0) {
-    if (i >= 0) {                      // x1-faces of the row
-#pragma unroll
-      for (int c = 0; c < 5; c++) group_mean(Dv.F[0][c], zrow, k, m);
-      group_mean(Dv.EfA[0], zrow, k, m);
-      group_mean(Dv.EfB[0], zrow, k, m);
-    }
-#pragma unroll
-    for (int c = 0; c < 5; c++) group_interp(Dv.F[2][c], zrow, k, m);   // x3-faces inside the group
-    group_interp(Dv.EfA[2], zrow, k, m);
-    group_interp(Dv.EfB[2], zrow, k, m);
+    if (i >= 0) group_mean(a0, zrow, k, m);                 // x1-faces of the row
+    group_interp(a2, zrow, k, m);                           // x3-faces inside the group
   }
-  if (j >= 0 && M > 1 && k % M == 0) {  // x2-face on the low side of row j
-#pragma unroll
-    for (int c = 0; c < 5; c++) group_mean(Dv.F[1][c], zrow, k, M);
-    group_mean(Dv.EfA[1], zrow, k, M);
-    group_mean(Dv.EfB[1], zrow, k, M);
-  }
+  if (j >= 0 && M > 1 && k % M == 0) group_mean(a1, zrow, k, M);   // x2-face on the low side of row j
 }
 
 // C-15 (iv): after the edge-EMF kernel
@@ -223,8 +216,8 @@ void launch_deref_fix_flux(hamr_grid* g, const Dev& Dv0) {
   if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
   Launch l_(g, K_OTHER);
   const unsigned nb = nblocks_for(Dv, Dv.L.n[0] + 2, Dv.L.n[1] + 2);
-  if (Dv.B.nblk > 0) k_deref_fix_flux<true><<<nb, 128, 0, g->stream>>>(Dv);
-  else k_deref_fix_flux<false><<<nb, 128, 0, g->stream>>>(Dv);
+  if (Dv.B.nblk > 0) k_deref_fix_flux<true><<<dim3(nb, 7), 128, 0, g->stream>>>(Dv);
+  else k_deref_fix_flux<false><<<dim3(nb, 7), 128, 0, g->stream>>>(Dv);
 }
 
 void launch_deref_flux_layers(hamr_grid* g, const Dev& Dv0) {
