@@ -38,7 +38,9 @@ __device__ __forceinline__ const double* buf_arr(const Bufs& B, int buf, int kin
 }
 
 // k_blk_ghosts calls these from eleven places (370 KB of code).  Out of line the kernel is SLOWER (measured on
-// cfg 4: 0.396 -> 0.494 ms with both, 0.423 with blk_fetch_ref alone): the calls spill their arguments
+// cfg 4: 0.396 -> 0.494 ms with both, 0.423 with blk_fetch_ref alone): the calls spill their arguments.  A
+// single looped call site (10 k instructions instead of 23 k) was no faster either: each iteration consumes its
+// load at once, which serialises the DRAM round trips the unrolled form overlaps
 #ifndef HAMR_GHOST_SHELL
 #define HAMR_GHOST_SHELL 1
 #endif

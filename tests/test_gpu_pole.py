@@ -83,8 +83,10 @@ def test_transmissive_poles_on_phi_cut_blocks_with_deref_refinement_and_lat(H, o
             e = parity_errors(I.block_as_grid(p, x_lo, dx, n), o.get_block_prims(b), g.get_block_prims(b))
             for k, v in e.items():
                 worst[k] = max(worst.get(k, 0.0), v)
-            for a, c in zip(o.get_block_bface(b), g.get_block_bface(b)):
-                assert np.abs(a - c).max() <= tol * max(np.abs(a).max(), 1e-300)
+            ob = o.get_block_bface(b)
+            scale = max(np.abs(a).max() for a in ob)   # one scale per block: a component may be rounding noise only
+            for a, c in zip(ob, g.get_block_bface(b)):
+                assert np.abs(a - c).max() <= tol * max(scale, 1e-300)
         assert max(worst.values()) <= tol, worst
 
     g.step(1)
