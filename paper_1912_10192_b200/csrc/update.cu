@@ -35,11 +35,14 @@ __device__ __forceinline__ Fields pick_fields(const Fields& a, const Fields& b, 
 #ifndef HAMR_UPD_MINB
 #define HAMR_UPD_MINB 6  // 80 regs (72 B spilled); 4 / 5 measured 4 % / 7 % slower with the reload, 8 slower still
 #endif
+#ifndef HAMR_UPD_MINB_PRED
+#define HAMR_UPD_MINB_PRED 7  // the predictor (one state to load) gains from 72 regs: 0.445 -> 0.429 ms; the corrector loses
+#endif
 #ifndef HAMR_UPD_KFACE
 #define HAMR_UPD_KFACE 1
 #endif
 template <bool SAME, bool BLK>  // SAME: predictor, source state == base state
-__global__ void __launch_bounds__(128, HAMR_UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
+__global__ void __launch_bounds__(128, SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
   const Lay& L = Dv.L;
   // k runs over [0, n3): warps start on 128-byte lines when n3 is a multiple of 32; the thread at k = 0 also
   // builds the x3-face at k = n3
