@@ -145,10 +145,13 @@ ALG_DOUBLES = {"flux_x1": 16, "flux_x2": 16, "flux_x3": 16,   # 9 r (P5, 2 trans
 
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel class from the round's
-# `ncu --set full` capture of this same command on cfg 2 (profiles/r1e_ncu_full_cfg2.md)
-NCU_TRAFFIC_SOURCE = "profiles/r1e_ncu_full_cfg2.md"
-NCU_TRAFFIC = {"flux_x1": 611919756, "flux_x2": 595946828, "flux_x3": 542627352, "centre_emf": 318860700, "edge_emf": 535477916, "update_predictor": 1377812368, "update_corrector": 1669734608, "ghosts": 139722668}
+# `ncu --set full` capture of this same command on cfg 2 (profiles/r1g_ncu_full_cfg2.md)
+NCU_TRAFFIC_SOURCE = "profiles/r1g_ncu_full_cfg2.md"
+NCU_TRAFFIC = {"flux_x1": 612879812, "flux_x2": 596430160, "flux_x3": 542101620, "centre_emf": 324869584, "edge_emf": 536485500, "update_predictor": 1416654112, "update_corrector": 1665517104, "ghosts": 140757796}
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# fp64 FLOPs the flux kernels execute per face (dadd + dmul + 2 dfma, thread instructions counted by the same ncu
+# capture, divided by the faces of the launch): x1 / x2 sweeps 650, x3 sweep 661
+FLUX_FLOP_PER_FACE = {"flux_x1": 650.3, "flux_x2": 649.9, "flux_x3": 661.1}
 PAPER_V100_150CUBED = 0.85e8   # ~0.85e8 zone-cycles/s, 1 V100, one 150^3 block
 
 
@@ -391,13 +394,25 @@ def main():
         by = 0 if blocky else ALG_DOUBLES.get(k, 0) * 8 * units_per_launch(k, n)
         d["alg_bytes"] = by
         d["gbs"] = by / (d["ms_avg"] * 1e-3) / 1e9 if d["ms_avg"] > 0 else 0.0
-    dom = max(kern, key=lambda k: kern[k]["ms_total"])
+    # the dominant kernel: the longest single launch (k_update, corrector variant, on cfg 2).  The three flux
+    # kernels together are half of the step and are bound by the FP64 pipe, not by HBM: "flux_alu" below
+    dom = max(kern, key=lambda k: kern[k]["ms_avg"])
+    flux = [k for k in ("flux_x1", "flux_x2", "flux_x3") if k in kern and not blocky]
+    flux_alu = None
+    if flux:
+        fl = sum(FLUX_FLOP_PER_FACE[k] * units_per_launch(k, n) * kern[k]["launches"] for k in flux)
+        tf = fl / (sum(kern[k]["ms_total"] for k in flux) * 1e-3) / 1e12
+        flux_alu = {"bound": "alu", "kernels": "+".join(flux), "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": tf / FP64_PEAK_TFLOPS, "share_of_step": sum(kern[k]["share"] for k in flux),
+                    "flop_per_face": FLUX_FLOP_PER_FACE, "flop_source": NCU_TRAFFIC_SOURCE,
+                    "note": "executed fp64 FLOPs (FMA = 2); the same capture shows the FP64 pipe issuing on 57-64 % of cycles "
+                            "(a third of its instructions are FMAs)"}
     roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": hbm_peak, "unit": "GB/s",
             "frac": kern[dom]["gbs"] / hbm_peak, "traffic": NCU_TRAFFIC.get(dom) if args.workload == "cfg2" else None,
             "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": peak_src,
             "fp64_pipe": {"peak_tflops_derived": FP64_PEAK_TFLOPS, "note": "148 SMs x 64 DFMA lanes x 2 x 1.965 GHz; "
                           "per-kernel FP64 pipe utilisation from ncu is in profiles/ (DESIGN.md section 7)"},
-            "share_of_step": kern[dom]["share"],
+            "share_of_step": kern[dom]["share"], "flux_alu": flux_alu,
             "whole_step": {"alg_bytes_per_zone_cycle_floor": 440,
                            "frac_of_hbm_at_floor": 440.0 * value / world / 1e9 / hbm_peak,
                            "alg_bytes_per_zone_cycle_pipeline": sum(d["alg_bytes"] * d["launches"] for d in kern.values()) / (nz * fin * args.steps),
