@@ -58,13 +58,25 @@ __device__ __forceinline__ DIdx deref_idx(const Dev& Dv, int ilo, int ihi, int j
 // group mean in place (members z0 .. z0 + m - 1, m a power of two <= 16) by a pairwise (tree) sum: the mean of
 // m IDENTICAL values is then that value exactly, so quantities that are already uniform in the group are left
 // bit-for-bit alone and blocks that recompute a shared value from copies of each other's groups agree
+template <int M>
+__device__ __forceinline__ void group_mean_t(double* __restrict__ a) {
+  double v[M];   // registers: M is a compile-time constant
+#pragma unroll
+  for (int r = 0; r < M; r++) v[r] = a[r];
+#pragma unroll
+  for (int w = 1; w < M; w *= 2)
+#pragma unroll
+    for (int r = 0; r + w < M; r += 2 * w) v[r] = v[r] + v[r + w];
+  const double mean = v[0] / (double)M;
+#pragma unroll
+  for (int r = 0; r < M; r++) a[r] = mean;
+}
 __device__ __forceinline__ void group_mean(double* __restrict__ a, long long zrow, int k0, int m) {
-  double v[16];
-  for (int r = 0; r < m; r++) v[r] = a[zrow + k0 + r];
-  for (int w = 1; w < m; w *= 2)
-    for (int r = 0; r + w < m; r += 2 * w) v[r] = v[r] + v[r + w];
-  const double mean = v[0] / (double)m;
-  for (int r = 0; r < m; r++) a[zrow + k0 + r] = mean;
+  double* g = a + zrow + k0;
+  if (m == 2) group_mean_t<2>(g);
+  else if (m == 4) group_mean_t<4>(g);
+  else if (m == 8) group_mean_t<8>(g);
+  else group_mean_t<16>(g);
 }
 
 // members 1 .. m-1 become the linear interpolation of the values at k0 and k0 + m
