@@ -42,7 +42,7 @@ def _run_pair(H, orc, p, hyd, bf, fin=1):
     assert g.divb() <= TOL_DIVB and g.stats()[0] == 0 and o.stats()[0] == 0
 
 
-@pytest.mark.parametrize("extra", [dict(), dict(nb=(16, 8, 32)), dict(nb=(16, 8, 8)), dict(nb=(32, 32, 16))])
+@pytest.mark.parametrize("extra", [dict(), dict(nb=(16, 8, 32)), dict(nb=(16, 8, 8)), dict(nb=(32, 32, 16)), dict(nb=(16, 16, 4))])
 def test_tilted_disk_through_the_poles(H, orc, extra):
     # a thick (h/r = 0.1) version of the cfg 3 stand-in so that 64x32x32 resolves it: the inclined disk and its
     # field cross both poles.  Monolithic ghost kernel, then the block ghost kernel on blocks that span x3 and
