@@ -38,11 +38,14 @@ __device__ __forceinline__ Fields pick_fields(const Fields& a, const Fields& b, 
 #ifndef HAMR_UPD_MINB_PRED
 #define HAMR_UPD_MINB_PRED 7  // the predictor (one state to load) gains from 72 regs: 0.445 -> 0.429 ms; the corrector loses
 #endif
+#ifndef HAMR_UPD_T
+#define HAMR_UPD_T 128   // threads per CTA; 32 / 64 measured equal within noise, 256 is 4 % slower (cfg 2)
+#endif
 #ifndef HAMR_UPD_KFACE
 #define HAMR_UPD_KFACE 1
 #endif
 template <bool SAME, bool BLK>  // SAME: predictor, source state == base state
-__global__ void __launch_bounds__(128, SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
+__global__ void __launch_bounds__(HAMR_UPD_T, (SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB) * 128 / HAMR_UPD_T) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
   const Lay& L = Dv.L;
   // k runs over [0, n3): warps start on 128-byte lines when n3 is a multiple of 32; the thread at k = 0 also
   // builds the x3-face at k = n3
@@ -216,12 +219,12 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
   const bool blk = Dv.B.nblk > 0;
   if (blk && Dv.B.nact == 0) return;
   const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + (HAMR_UPD_KFACE ? 0 : 1)) * (blk ? Dv.B.nact : 1);
-  const unsigned nb = (unsigned)((tot + 127) / 128);
+  const unsigned nb = (unsigned)((tot + HAMR_UPD_T - 1) / HAMR_UPD_T);
   Launch l_(g, same ? K_UPDATE_P : K_UPDATE_C);
-  if (same && !blk) k_update<true, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
-  else if (same) k_update<true, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
-  else if (!blk) k_update<false, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
-  else k_update<false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+  if (same && !blk) k_update<true, false><<<nb, HAMR_UPD_T, 0, g->stream>>>(Dv, ra, rb, dtfac);
+  else if (same) k_update<true, true><<<nb, HAMR_UPD_T, 0, g->stream>>>(Dv, ra, rb, dtfac);
+  else if (!blk) k_update<false, false><<<nb, HAMR_UPD_T, 0, g->stream>>>(Dv, ra, rb, dtfac);
+  else k_update<false, true><<<nb, HAMR_UPD_T, 0, g->stream>>>(Dv, ra, rb, dtfac);
 }
 
 void launch_update(hamr_grid* g, const Fields& src, const Fields& base, const Fields& out, double dtfac,
