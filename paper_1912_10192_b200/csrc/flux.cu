@@ -226,6 +226,9 @@ __device__ __forceinline__ void ctop_commit(const Dev& Dv, int D, int b, double 
 #ifndef HAMR_MARCH_MINB
 #define HAMR_MARCH_MINB 4  // 128 regs/thread: measured best of 1/3/4 on cfg 2 (profiles/)
 #endif
+#ifndef HAMR_MARCH_T
+#define HAMR_MARCH_T 128  // threads per CTA; 32 / 64 / 256 measured within 0.5 % of each other (cfg 2)
+#endif
 #ifndef HAMR_MARCH_UNROLL
 #define HAMR_MARCH_UNROLL 1
 #endif
@@ -236,7 +239,7 @@ constexpr int MARCH_UNROLL = HAMR_MARCH_UNROLL;
 // BLK: the launch covers the blocks of Dv.B.list (block-structured grid, H7); s / s2 are the buffer sets
 // holding the stage source of blocks with cur == 0 / cur == 2.
 template <int D, int RECON, bool BLK>
-__global__ void __launch_bounds__(128, HAMR_MARCH_MINB) k_flux_march(Dev Dv, Fields s, Fields s2, int seg,
+__global__ void __launch_bounds__(HAMR_MARCH_T, HAMR_MARCH_MINB * 128 / HAMR_MARCH_T) k_flux_march(Dev Dv, Fields s, Fields s2, int seg,
                                                                       int want_ctop) {
   static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   const Lay& L = Dv.L;
@@ -478,7 +481,7 @@ static int pick_segment(const Lay& L, int nbx) {
   int dev = 0, sms = 148, per_sm = 2;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_flux_march<D, RECON, BLK>, 128, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_flux_march<D, RECON, BLK>, HAMR_MARCH_T, 0);
   if (per_sm < 1) per_sm = 1;
   const double slots = (double)sms * per_sm;
   double best = -1.0;
@@ -503,10 +506,10 @@ static void launch_march_t(hamr_grid* g, const Dev& Dv, const Fields& src, const
   const Lay& L = Dv.L;
   const int O = 1 - D;
   const long long ntr = (long long)(L.n[O] + 2) * (L.n[2] + 2) * (BLK ? Dv.B.nact : 1);
-  const int nbx = (int)((ntr + 127) / 128);
+  const int nbx = (int)((ntr + HAMR_MARCH_T - 1) / HAMR_MARCH_T);
   const int seg = pick_segment<D, RECON, BLK>(L, nbx);
   dim3 grid(nbx, (L.n[D] + 1 + seg - 1) / seg);
-  k_flux_march<D, RECON, BLK><<<grid, 128, 0, g->stream>>>(Dv, src, src2, seg, want_ctop ? 1 : 0);
+  k_flux_march<D, RECON, BLK><<<grid, HAMR_MARCH_T, 0, g->stream>>>(Dv, src, src2, seg, want_ctop ? 1 : 0);
 }
 
 template <int D>
