@@ -18,6 +18,9 @@
 namespace hamr {
 
 constexpr double SIXTH = 1.0 / 6.0;
+#ifndef HAMR_PPM_ONE_SIDED
+#define HAMR_PPM_ONE_SIDED 1
+#endif
 
 // ---- C-5 reconstruction, branch-free ----------------------------------------------------------------
 // van Leer / CW84 limited slope from dl = a_j - a_{j-1}, dr = a_{j+1} - a_j, dc = (a_{j+1} - a_{j-1})/2
@@ -32,7 +35,19 @@ __device__ __forceinline__ double ppm_iface(double aj, double d, double dm_j, do
 }
 
 // monotonised parabola edges of a zone with mean a and interface values l (low side), r (high side)
+// CW84 (1.10) in one-sided differences dl = a - l, dr = r - a: where the zone is not an extremum (dl dr > 0) the
+// overshoot tests (r - l)(a - (l + r)/2) > (r - l)^2 / 6 and < -(r - l)^2 / 6 divide through by (r - l) to
+// |dl| > 2 |dr| and |dr| > 2 |dl|, and the reset edges 3a - 2r, 3a - 2l are a - 2 dr, a + 2 dl: 10 fp64
+// instructions instead of 15; every switch is continuous, so the rounding of a test does not matter
 __device__ __forceinline__ void ppm_mono(double l, double a, double r, double& aL, double& aR) {
+#if HAMR_PPM_ONE_SIDED
+  const double dl = a - l, dr = r - a;
+  const bool flat = dl * dr <= 0.0;
+  const double adl = fabs(dl), adr = fabs(dr);
+  const bool over = adl > 2.0 * adr, under = adr > 2.0 * adl;
+  aL = flat ? a : (over ? a - 2.0 * dr : l);
+  aR = flat ? a : ((!over && under) ? a + 2.0 * dl : r);
+#else
   const bool flat = (r - a) * (a - l) <= 0.0;
   const double d = r - l;
   const double c = a - 0.5 * (l + r);
@@ -41,6 +56,7 @@ __device__ __forceinline__ void ppm_mono(double l, double a, double r, double& a
   const double nl = 3.0 * a - 2.0 * r, nr = 3.0 * a - 2.0 * l;
   aL = flat ? a : (over ? nl : l);
   aR = flat ? a : ((!over && under) ? nr : r);
+#endif
 }
 
 // parabola edges (aL at j-1/2, aR at j+1/2) of zone j from a0..a4 = a[j-2..j+2]
