@@ -146,13 +146,13 @@ ALG_DOUBLES = {"flux_x1": 16, "flux_x2": 16, "flux_x3": 16,   # 9 r (P5, 2 trans
 
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel class from the round's
-# `ncu --set full` capture of this same command on cfg 2 (profiles/r1g_ncu_full_cfg2.md)
-NCU_TRAFFIC_SOURCE = "profiles/r1g_ncu_full_cfg2.md"
-NCU_TRAFFIC = {"flux_x1": 612879812, "flux_x2": 596430160, "flux_x3": 542101620, "centre_emf": 324869584, "edge_emf": 536485500, "update_predictor": 1416654112, "update_corrector": 1665517104, "ghosts": 140757796}
+# `ncu --set full` capture of this same command on cfg 2 (profiles/r1h_ncu_full_cfg2.md)
+NCU_TRAFFIC_SOURCE = "profiles/r1h_ncu_full_cfg2.md"
+NCU_TRAFFIC = {"flux_x1": 613177160, "flux_x2": 598131024, "flux_x3": 542374640, "centre_emf": 325253308, "edge_emf": 534960992, "update_predictor": 1414139888, "update_corrector": 1667606816, "ghosts": 140912088}
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # fp64 FLOPs the flux kernels execute per face (dadd + dmul + 2 dfma, thread instructions counted by the same ncu
-# capture, divided by the faces of the launch): x1 / x2 sweeps 650, x3 sweep 661
-FLUX_FLOP_PER_FACE = {"flux_x1": 650.3, "flux_x2": 649.9, "flux_x3": 661.1}
+# capture, divided by the faces of the launch): x1 / x2 sweeps 598-599, x3 sweep 606
+FLUX_FLOP_PER_FACE = {"flux_x1": 599.2, "flux_x2": 598.0, "flux_x3": 605.8}
 PAPER_V100_150CUBED = 0.85e8   # ~0.85e8 zone-cycles/s, 1 V100, one 150^3 block
 
 
@@ -422,7 +422,7 @@ def main():
         flux_alu = {"bound": "alu", "kernels": "+".join(flux), "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "frac": tf / FP64_PEAK_TFLOPS, "share_of_step": sum(kern[k]["share"] for k in flux),
                     "flop_per_face": FLUX_FLOP_PER_FACE, "flop_source": NCU_TRAFFIC_SOURCE,
-                    "note": "executed fp64 FLOPs (FMA = 2); the same capture shows the FP64 pipe issuing on 57-64 % of cycles "
+                    "note": "executed fp64 FLOPs (FMA = 2); the same capture shows the FP64 pipe issuing on 53-62 % of cycles "
                             "(a third of its instructions are FMAs)"}
     roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": hbm_peak, "unit": "GB/s",
             "frac": kern[dom]["gbs"] / hbm_peak, "traffic": NCU_TRAFFIC.get(dom) if args.workload == "cfg2" else None,
