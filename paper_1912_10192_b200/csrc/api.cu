@@ -117,7 +117,7 @@ ArenaPlan plan_arena(const hamr_params& p, const Lay& L, const GridShape& G) {
   size_t off = 0;
   a.arr = off; off += (size_t)G.narr * L.len * 8;
   a.tabs = off; off += align_up((size_t)G.nlev * (((size_t)3 * NGEO + 2 * NDG) * L.n2d * 8 + (size_t)2 * G.te1 * 8), 256);
-  a.recs = off; off += align_up((size_t)G.nlev * (NREC_C + 2 * NREC_F) * L.n2d * 8, 256);   // array-of-records copies
+  a.recs = off; off += align_up((size_t)G.nlev * (NREC_C + 3 * NREC_F) * L.n2d * 8, 256);   // array-of-records copies
   a.scal = off; off += 256;
   a.cnt = off; off += 256;
   a.stage_doubles = (size_t)8 * (p.n[0] + 1) * (p.n[1] + 1) * (p.n[2] + 1);
@@ -249,8 +249,9 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   double* gcA = (double*)(base + ap.recs);
   double* gf1A = gcA + (size_t)NREC_C * D.L.n2d;
   double* gf2A = gf1A + (size_t)NREC_F * D.L.n2d;
-  D.gcA = gcA; D.gf1A = gf1A; D.gf2A = gf2A;
-  D.B.tlevA = (NREC_C + 2 * NREC_F) * D.L.n2d;
+  double* gf3A = gf2A + (size_t)NREC_F * D.L.n2d;
+  D.gcA = gcA; D.gf1A = gf1A; D.gf2A = gf2A; D.gf3A = gf3A;
+  D.B.tlevA = (NREC_C + 3 * NREC_F) * D.L.n2d;
   D.scal = (double*)(base + ap.scal);
   D.cnt = (unsigned long long*)(base + ap.cnt);
   g->stage = (double*)(base + ap.stage);
@@ -258,11 +259,11 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
 
   e = cudaMemsetAsync(g->arena, 0, ap.total, g->stream);
   if (e == cudaSuccess) {
-    launch_geometry_tab(g, gs.te1, gs.te2, D.L.n2d, D.dx[0], p->n[1], gc, gf1, gf2, dgc, rfl, ufl, gcA, gf1A, gf2A);
+    launch_geometry_tab(g, gs.te1, gs.te2, D.L.n2d, D.dx[0], p->n[1], gc, gf1, gf2, dgc, rfl, ufl, gcA, gf1A, gf2A, gf3A);
     if (gs.nlev > 1)   // C-16: the refined level's tables, dx1 / 2
       launch_geometry_tab(g, gs.te1, gs.te2, D.L.n2d, 0.5 * D.dx[0], p->n[1], gc + D.B.tlev, gf1 + D.B.tlev,
                           gf2 + D.B.tlev, dgc + D.B.tlev, rfl + D.B.flev, ufl + D.B.flev, gcA + D.B.tlevA,
-                          gf1A + D.B.tlevA, gf2A + D.B.tlevA);
+                          gf1A + D.B.tlevA, gf2A + D.B.tlevA, gf3A + D.B.tlevA);
     e = cudaGetLastError();
   }
   if (e == cudaSuccess && gs.nblk > 0 && blk_setup(g, base + ap.blk) != HAMR_OK) e = cudaErrorUnknown;

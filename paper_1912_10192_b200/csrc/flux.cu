@@ -18,15 +18,16 @@
 namespace hamr {
 
 constexpr double SIXTH = 1.0 / 6.0;
-#ifndef HAMR_PPM_ONE_SIDED
-#define HAMR_PPM_ONE_SIDED 1
-#endif
 
 // ---- C-5 reconstruction, branch-free ----------------------------------------------------------------
+// "dl and dr have the same sign" read off the sign bits (integer pipe; the FP64 pipe is the one these kernels
+// saturate).  A zero on either side makes the limited quantity zero by itself, so no product is needed.
+__device__ __forceinline__ bool same_sign(double a, double b) { return (__double2hiint(a) ^ __double2hiint(b)) >= 0; }
+
 // van Leer / CW84 limited slope from dl = a_j - a_{j-1}, dr = a_{j+1} - a_j, dc = (a_{j+1} - a_{j-1})/2
 __device__ __forceinline__ double lim_slope(double dl, double dr, double dc) {
   const double lim = dmin(fabs(dc), 2.0 * dmin(fabs(dl), fabs(dr)));
-  return (dl * dr > 0.0) ? copysign(lim, dc) : 0.0;
+  return same_sign(dl, dr) ? copysign(lim, dl) : 0.0;   // sign(dc) = sign(dl) where the slope survives
 }
 
 // interface value a_{j+1/2} from a_j, d = a_{j+1} - a_j and the limited slopes of zones j and j+1
@@ -37,26 +38,16 @@ __device__ __forceinline__ double ppm_iface(double aj, double d, double dm_j, do
 // monotonised parabola edges of a zone with mean a and interface values l (low side), r (high side)
 // CW84 (1.10) in one-sided differences dl = a - l, dr = r - a: where the zone is not an extremum (dl dr > 0) the
 // overshoot tests (r - l)(a - (l + r)/2) > (r - l)^2 / 6 and < -(r - l)^2 / 6 divide through by (r - l) to
-// |dl| > 2 |dr| and |dr| > 2 |dl|, and the reset edges 3a - 2r, 3a - 2l are a - 2 dr, a + 2 dl: 10 fp64
-// instructions instead of 15; every switch is continuous, so the rounding of a test does not matter
+// |dl| > 2 |dr| and |dr| > 2 |dl|, and the reset edges 3a - 2r, 3a - 2l are a - 2 dr, a + 2 dl; every switch is
+// continuous, so the rounding of a test does not matter.  dl = 0 or dr = 0 needs no case of its own: the
+// overshoot tests then reset the other edge to a as well.
 __device__ __forceinline__ void ppm_mono(double l, double a, double r, double& aL, double& aR) {
-#if HAMR_PPM_ONE_SIDED
   const double dl = a - l, dr = r - a;
-  const bool flat = dl * dr <= 0.0;
+  const bool flat = !same_sign(dl, dr);
   const double adl = fabs(dl), adr = fabs(dr);
   const bool over = adl > 2.0 * adr, under = adr > 2.0 * adl;
   aL = flat ? a : (over ? a - 2.0 * dr : l);
   aR = flat ? a : ((!over && under) ? a + 2.0 * dl : r);
-#else
-  const bool flat = (r - a) * (a - l) <= 0.0;
-  const double d = r - l;
-  const double c = a - 0.5 * (l + r);
-  const double dc = d * c, dd6 = d * d * SIXTH;
-  const bool over = dc > dd6, under = dc < -dd6;
-  const double nl = 3.0 * a - 2.0 * r, nr = 3.0 * a - 2.0 * l;
-  aL = flat ? a : (over ? nl : l);
-  aR = flat ? a : ((!over && under) ? nr : r);
-#endif
 }
 
 // parabola edges (aL at j-1/2, aR at j+1/2) of zone j from a0..a4 = a[j-2..j+2]
@@ -83,127 +74,135 @@ __device__ __forceinline__ void zone_edges(const double* __restrict__ a, int sd,
 }
 
 // ---- C-2..C-7 on one face ------------------------------------------------------------------------------
-// the subset of the face geometry the flux needs
+// The face record (hamr_dev.cuh FREC_*): the 3+1 split of the face metric.  With u^mu = ut^mu + gamma n^mu and
+// n_i = 0 the spatial covariant components need the spatial metric only, u_i = g_ij ut^j, and
+// u_t = -alpha gamma + beta^i u_i; likewise b_i = g_ij (b^j + beta^j b^t), b_t = -alpha^2 b^t + beta^i b_i.
+// Both metrics have beta^2 = beta^3 = 0 and g_12 = g_23 = 0.
 struct FGeo {
-  double c00, c01, c03, c11, c13, c22, c33;  // g_{mu nu}
+  double c11, c13, c22, c33;                 // g_ij
+  double alpha, ialpha, boa, beta1, nalpha2; // lapse, 1/lapse, beta^1/lapse, beta^1, -lapse^2
   double k00, kdd, k0d;                      // g^{tt}, g^{dd}, g^{td}
-  double gdet, igdet, alpha, ialpha, boa;
+  double gdet, igdet;
 };
 
-// from the array-of-records tables (hamr_dev.cuh): one 128-byte line per face record (x1-, x2-faces); the x3 sweep
-// reads the centre record (two lines)
-template <int D>
 __device__ __forceinline__ FGeo load_fgeo(const double* __restrict__ rec) {
+  double v[NREC_F];
+  load_rec(rec, NREC_F - 2, v);
   FGeo G;
-  if (D < 2) {
-    double v[NREC_F];
-    load_rec(rec, NREC_F, v);
-    G.c00 = v[0]; G.c01 = v[1]; G.c03 = v[2]; G.c11 = v[3]; G.c13 = v[4]; G.c22 = v[5]; G.c33 = v[6];
-    G.k00 = v[7]; G.kdd = v[8]; G.k0d = v[9];
-    G.gdet = v[10]; G.igdet = v[11]; G.alpha = v[12]; G.ialpha = v[13]; G.boa = v[14];
-  } else {
-    double v[18];
-    load_rec(rec, 18, v);
-    G.c00 = v[0]; G.c01 = v[1]; G.c03 = v[2]; G.c11 = v[3]; G.c13 = v[4]; G.c22 = v[5]; G.c33 = v[6];
-    G.k00 = v[7]; G.kdd = v[12]; G.k0d = 0.0;   // g^{33}; g^{t3} = 0 for both metrics
-    G.gdet = v[13]; G.alpha = v[14]; G.ialpha = v[15]; G.boa = v[16]; G.igdet = v[17];
-  }
+  G.c11 = v[FREC_C11]; G.c13 = v[FREC_C13]; G.c22 = v[FREC_C22]; G.c33 = v[FREC_C33];
+  G.alpha = v[FREC_ALPHA]; G.ialpha = v[FREC_IALPHA]; G.boa = v[FREC_BOA]; G.beta1 = v[FREC_BETA1];
+  G.nalpha2 = v[FREC_NALPHA2]; G.k00 = v[FREC_K00]; G.kdd = v[FREC_KDD]; G.k0d = v[FREC_K0D];
+  G.gdet = v[FREC_GDET]; G.igdet = v[FREC_IGDET];
   return G;
 }
 
-// one side of the face: U and F rows (without the sqrt(-g) factor, applied after HLL) and speed bounds
+// What the HLL combination needs from one side of the face.  The rows of U and F are never formed: with
+// T^mu_nu = eta u^mu u_nu + ptot delta^mu_nu - b^mu b_nu (eta = w + b^2, ptot = p + b^2/2) a weighted sum
+// wF F_nu + wU U_nu of the flux and conserved rows is (eta X) u_nu - Y b_nu + wF ptot delta^d_nu with the two scalars
+// X = wF u^d + wU u^t, Y = wF b^d + wU b^t: two FMAs per row and side instead of six.
+struct Side {
+  double rho, ut, ud, eta, ptot, b0, bd;
+  double ul[4], bl[4];   // u_mu, b_mu
+  double Be, Bf, Fe, Ff; // transverse field components and their flux rows b^e u^d - b^d u^e (C-4)
+  double a2, vp, vm;     // C-6: the speed bounds are vp / a2 and -vm / a2, a2 > 0
+};
+
 template <int D>
-__device__ __forceinline__ void side_state(const double P[8], const FGeo& G, double gam_ad, double U[7],
-                                           double F[7], double& vmin, double& vmax) {
+__device__ __forceinline__ void side_state(const double P[8], const FGeo& G, double gam_ad, Side& S) {
   constexpr int dir = D + 1, e = (D + 1) % 3, f = (D + 2) % 3;
   // C-2
-  const double q = G.c11 * P[2] * P[2] + G.c22 * P[3] * P[3] + G.c33 * P[4] * P[4] + 2.0 * (G.c13 * P[2] * P[4]);
-  const double q1 = 1.0 + q;
+  S.ul[1] = G.c11 * P[2] + G.c13 * P[4];
+  S.ul[2] = G.c22 * P[3];
+  S.ul[3] = G.c13 * P[2] + G.c33 * P[4];
+  const double q1 = 1.0 + (P[2] * S.ul[1] + P[3] * S.ul[2] + P[4] * S.ul[3]);
   const double rg = rsqrt(q1);  // gamma = q1 rg and 1/u^t = alpha/gamma = alpha rg share one special-function call
   const double gam = q1 * rg;
-  double u[4], ul[4], b[4], bl[4];
+  double u[4], b[4];
   u[0] = gam * G.ialpha;
   u[1] = P[2] - gam * G.boa;
   u[2] = P[3];
   u[3] = P[4];
-  ul[0] = G.c00 * u[0] + G.c01 * u[1] + G.c03 * u[3];
-  ul[1] = G.c01 * u[0] + G.c11 * u[1] + G.c13 * u[3];
-  ul[2] = G.c22 * u[2];
-  ul[3] = G.c03 * u[0] + G.c13 * u[1] + G.c33 * u[3];
+  S.ul[0] = G.beta1 * S.ul[1] - G.alpha * gam;
   // C-3
-  b[0] = P[5] * ul[1] + P[6] * ul[2] + P[7] * ul[3];
+  b[0] = P[5] * S.ul[1] + P[6] * S.ul[2] + P[7] * S.ul[3];
   const double iut = G.alpha * rg;
   b[1] = (P[5] + b[0] * u[1]) * iut;
   b[2] = (P[6] + b[0] * u[2]) * iut;
   b[3] = (P[7] + b[0] * u[3]) * iut;
-  bl[0] = G.c00 * b[0] + G.c01 * b[1] + G.c03 * b[3];
-  bl[1] = G.c01 * b[0] + G.c11 * b[1] + G.c13 * b[3];
-  bl[2] = G.c22 * b[2];
-  bl[3] = G.c03 * b[0] + G.c13 * b[1] + G.c33 * b[3];
-  const double bsq = b[0] * bl[0] + b[1] * bl[1] + b[2] * bl[2] + b[3] * bl[3];
+  const double bt1 = b[1] + b[0] * G.beta1;
+  S.bl[1] = G.c11 * bt1 + G.c13 * b[3];
+  S.bl[2] = G.c22 * b[2];
+  S.bl[3] = G.c13 * bt1 + G.c33 * b[3];
+  S.bl[0] = G.nalpha2 * b[0] + G.beta1 * S.bl[1];
+  const double bsq = b[0] * S.bl[0] + b[1] * S.bl[1] + b[2] * S.bl[2] + b[3] * S.bl[3];
   // C-4
   const double p = (gam_ad - 1.0) * P[1];
-  const double w = P[0] + P[1] + p;
-  const double eta = w + bsq;
-  const double ptot = p + 0.5 * bsq;
-  const double eu0 = eta * u[0], eud = eta * u[dir];
-  const double Dn = P[0] * u[0], m = P[0] * u[dir];
-  U[0] = Dn;
-  U[1] = eu0 * ul[0] + ptot - b[0] * bl[0] + Dn;
-  F[0] = m;
-  F[1] = eud * ul[0] - b[dir] * bl[0] + m;
-#pragma unroll
-  for (int c = 1; c < 4; c++) {
-    U[1 + c] = eu0 * ul[c] - b[0] * bl[c];
-    F[1 + c] = eud * ul[c] + (c == dir ? ptot : 0.0) - b[dir] * bl[c];
-  }
-  U[5] = P[5 + e];
-  U[6] = P[5 + f];
-  F[5] = b[1 + e] * u[dir] - b[dir] * u[1 + e];
-  F[6] = b[1 + f] * u[dir] - b[dir] * u[1 + f];
+  const double w = P[0] + gam_ad * P[1];
+  S.rho = P[0];
+  S.ut = u[0];
+  S.ud = u[dir];
+  S.b0 = b[0];
+  S.bd = b[dir];
+  S.eta = w + bsq;
+  S.ptot = p + 0.5 * bsq;
+  S.Be = P[5 + e];
+  S.Bf = P[5 + f];
+  S.Fe = b[1 + e] * u[dir] - b[dir] * u[1 + e];
+  S.Ff = b[1 + f] * u[dir] - b[dir] * u[1 + f];
   // C-6: c_m^2 = c_s^2 + v_A^2 - c_s^2 v_A^2 with c_s^2 = gamma p / w, v_A^2 = b^2 / (b^2 + w)
-  // = N / Dq with Dq = w (w + b^2) > 0; the quadratic is multiplied through by Dq (same roots, no division)
+  // = N / Dq with Dq = w (w + b^2) > 0; the quadratic a2 v^2 - 2 h v + a0 = 0 is multiplied through by Dq (same
+  // roots, no division).  With M = Dq - N >= 0: a2 = (u^t)^2 M - g^tt N > 0 (g^tt < 0), so the larger root is
+  // (h + sqrt(h^2 - a2 a0)) / a2 and the smaller one (h - sqrt(..)) / a2
   const double gp = gam_ad * p;
-  const double Dq = w * eta;
-  const double N = dmin(dmax(gp * eta + bsq * (w - gp), 0.0), Dq);  // clamp c_m^2 to [0, 1]
-  const double ut2 = u[0] * u[0], udt = u[dir] * u[0], ud2 = u[dir] * u[dir];
-  const double a2 = ut2 * Dq - (G.k00 + ut2) * N;
-  const double a1 = 2.0 * (udt * Dq - (G.k0d + udt) * N);
-  const double a0 = ud2 * Dq - (G.kdd + ud2) * N;
-  const double disc = sqrt(dmax(a1 * a1 - 4.0 * a2 * a0, 0.0));
-  const double i2 = 1.0 / (2.0 * a2);
-  const double v1 = (a1 + disc) * i2, v2 = (a1 - disc) * i2;
-  vmax = dmax(v1, v2);
-  vmin = dmin(v1, v2);
+  const double Dq = w * S.eta;
+  const double N = dmin(dmax(gp * S.eta + bsq * (w - gp), 0.0), Dq);  // clamp c_m^2 to [0, 1]
+  const double M = Dq - N;
+  S.a2 = (u[0] * u[0]) * M - G.k00 * N;
+  const double h = (u[dir] * u[0]) * M - G.k0d * N;
+  const double a0 = (u[dir] * u[dir]) * M - G.kdd * N;
+  const double disc = sqrt(dmax(h * h - S.a2 * a0, 0.0));
+  S.vp = h + disc;
+  S.vm = disc - h;
 }
 
 // HLL (C-7) from the two states; writes the 7 outputs of the face; returns ctop
 template <int D>
 __device__ __forceinline__ double face_flux(const double PL[8], const double PR[8], const FGeo& G, double gam_ad,
                                             const Dev& Dv, int z) {
-  double UL[7], UR[7], FL[7], FR[7], vminL, vmaxL, vminR, vmaxR;
-  side_state<D>(PL, G, gam_ad, UL, FL, vminL, vmaxL);
-  side_state<D>(PR, G, gam_ad, UR, FR, vminR, vmaxR);
-  const double cmax = dmax(0.0, dmax(vmaxL, vmaxR));
-  const double cmin = dmax(0.0, dmax(-vminL, -vminR));
+  constexpr int dir = D + 1;
+  Side L, R;
+  side_state<D>(PL, G, gam_ad, L);
+  side_state<D>(PR, G, gam_ad, R);
+  const double ia = 1.0 / (L.a2 * R.a2);   // one reciprocal for both sides
+  const double iL = R.a2 * ia, iR = L.a2 * ia;
+  const double cmax = dmax(0.0, dmax(L.vp * iL, R.vp * iR));
+  const double cmin = dmax(0.0, dmax(L.vm * iL, R.vm * iR));
   const double sum = cmax + cmin;
   const bool avg = sum < 1e-300;
-  const double isum = avg ? 0.0 : 1.0 / sum;
+  const double isg = avg ? 0.0 : G.gdet / sum;
   // F = g [cmax FL + cmin FR - cmax cmin (UR - UL)] / (cmax + cmin);  average if both speeds vanish
-  const double wl = avg ? 0.5 * G.gdet : cmax * isum * G.gdet;
-  const double wr = avg ? 0.5 * G.gdet : cmin * isum * G.gdet;
-  const double wc = avg ? 0.0 : cmax * cmin * isum * G.gdet;
-  double Fh[7];
-#pragma unroll
-  for (int c = 0; c < 7; c++) Fh[c] = wl * FL[c] + wr * FR[c] - wc * (UR[c] - UL[c]);
+  const double wl = avg ? 0.5 * G.gdet : cmax * isg;
+  const double wr = avg ? 0.5 * G.gdet : cmin * isg;
+  const double wc = wl * cmin;              // avg: cmin = 0
+  const double XL = wl * L.ud + wc * L.ut, XR = wr * R.ud - wc * R.ut;
+  double Fh0 = L.rho * XL + R.rho * XR;
   // C-7a: a mass flux below 1e-12 of the magnitude of its own HLL terms is rounding noise and is
   // flushed to exactly 0, so that the upwind selector of C-9 sees a tie
-  const double mag = wl * fabs(FL[0]) + wr * fabs(FR[0]) + wc * (fabs(UR[0]) + fabs(UL[0]));
-  if (!avg && fabs(Fh[0]) <= 1e-12 * mag) Fh[0] = 0.0;
+  const double mag = L.rho * (wl * fabs(L.ud) + wc * L.ut) + R.rho * (wr * fabs(R.ud) + wc * R.ut);
+  if (!avg && fabs(Fh0) <= 1e-12 * mag) Fh0 = 0.0;
+  const double AL = L.eta * XL, AR = R.eta * XR;
+  const double YL = wl * L.bd + wc * L.b0, YR = wr * R.bd - wc * R.b0;
+  double Fh[4];
 #pragma unroll
-  for (int c = 0; c < 5; c++) Dv.F[D][c][z] = Fh[c];
-  Dv.EfB[D][z] = -Fh[5];  // C-8: on a d-face, E_f = -F^d(B^e)
-  Dv.EfA[D][z] = Fh[6];   //                    E_e = +F^d(B^f)
+  for (int c = 0; c < 4; c++) Fh[c] = (AL * L.ul[c] - YL * L.bl[c]) + (AR * R.ul[c] - YR * R.bl[c]);
+  Fh[dir] += wl * L.ptot + wr * R.ptot;   // delta^d_nu of the flux rows
+  Fh[0] += wc * (L.ptot - R.ptot);        // delta^t_nu of the conserved rows
+  Dv.F[D][0][z] = Fh0;
+  Dv.F[D][1][z] = Fh[0] + Fh0;   // the energy row carries T^d_t + rho u^d (C-4)
+#pragma unroll
+  for (int c = 1; c < 4; c++) Dv.F[D][1 + c][z] = Fh[c];
+  Dv.EfB[D][z] = -(wl * L.Fe + wr * R.Fe - wc * (R.Be - L.Be));  // C-8: on a d-face, E_f = -F^d(B^e)
+  Dv.EfA[D][z] = wl * L.Ff + wr * R.Ff - wc * (R.Bf - L.Bf);     //                    E_e = +F^d(B^f)
   return dmax(cmax, cmin);
 }
 
@@ -333,7 +332,7 @@ __global__ void __launch_bounds__(HAMR_MARCH_T, HAMR_MARCH_MINB * 128 / HAMR_MAR
         zero_face(Dv, D, z);
       } else {
         const int q = C.q0 + ((D == 0) ? fc * ge2 + o : o * ge2 + fc);
-        const FGeo G = load_fgeo<D>(gtab + (size_t)q * NREC_F);
+        const FGeo G = load_fgeo(gtab + (size_t)q * NREC_F);
         PL[5 + D] = PR[5 + D] = bfn[z] * G.igdet;  // C-5: the normal field is single-valued at the face
         const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
         if (act) ctop = dmax(ctop, ct);
@@ -402,7 +401,7 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
   const bool fine_row = Dv.mrow == nullptr || __ldg(Dv.mrow + C.J0 + j + NG) == 1;
   if (valid && fine_row && lane >= HLO && lane < 32 - HHI && k >= 0 && k <= L.n[2]) {
     const int ge2 = BLK ? Dv.B.ge2 : L.e2;
-    const FGeo G = load_fgeo<D>(Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * ge2 + j) * NREC_C);
+    const FGeo G = load_fgeo(Dv.gf3A + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * ge2 + j) * NREC_F);
     PL[7] = PR[7] = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z] * G.igdet;
     const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
     if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct;
@@ -459,7 +458,7 @@ __global__ void __launch_bounds__(128) k_deref_x3(Dev Dv, Fields s, Fields s2, i
       }
     }
     const int ge2 = BLK ? Dv.B.ge2 : L.e2;
-    const FGeo G = load_fgeo<D>(Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * ge2 + j) * NREC_C);
+    const FGeo G = load_fgeo(Dv.gf3A + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * ge2 + j) * NREC_F);
     const int z = zrow + k;
     PL[7] = PR[7] = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z] * G.igdet;
     const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);

@@ -82,14 +82,17 @@ __device__ static void store_geo(double* tab, int n2d, int q, const Geo& G) {
 // domain's low corner in zones of spacing dx1 (the table of one x1 refinement level), n2glob zones in x2
 // face record of the array-of-records tables (hamr_dev.cuh); kdd / k0d: g^{dd}, g^{td} of the face's direction
 __device__ static void store_face_rec(double* rec, const Geo& G, double kdd, double k0d) {
-  const double v[NREC_F] = {G.c00, G.c01, G.c03, G.c11, G.c13, G.c22, G.c33, G.k00, kdd, k0d, G.gdet,
-                            G.gdet > 0.0 ? 1.0 / G.gdet : 0.0, G.alpha, G.ialpha, G.boa, 0.0};
+  double v[NREC_F] = {};
+  v[FREC_C11] = G.c11; v[FREC_C13] = G.c13; v[FREC_C22] = G.c22; v[FREC_C33] = G.c33;
+  v[FREC_ALPHA] = G.alpha; v[FREC_IALPHA] = G.ialpha; v[FREC_BOA] = G.boa; v[FREC_BETA1] = G.boa * G.alpha;
+  v[FREC_NALPHA2] = -(G.alpha * G.alpha); v[FREC_K00] = G.k00; v[FREC_KDD] = kdd; v[FREC_K0D] = k0d;
+  v[FREC_GDET] = G.gdet; v[FREC_IGDET] = G.gdet > 0.0 ? 1.0 / G.gdet : 0.0;
   for (int c = 0; c < NREC_F; c++) rec[c] = v[c];
 }
 
 __global__ void k_geometry(Dev D, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
                            double* gf2, double* dgc, double* rho_fl, double* u_fl, double* gcA, double* gf1A,
-                           double* gf2A) {
+                           double* gf2A, double* gf3A) {
   const int q = blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= e1 * e2) return;
   const int i = q / e2 - NG, j = q % e2 - NG;
@@ -108,6 +111,7 @@ __global__ void k_geometry(Dev D, int e1, int e2, int n2d, double dx1, int n2glo
     for (int c = 0; c < NGEO; c++) rec[c] = gc[c * n2d + q];
     for (int c = 0; c < NDG; c++) { rec[NGEO + c] = d1[c]; rec[NGEO + NDG + c] = d2[c]; }
   }
+  store_face_rec(gf3A + (size_t)q * NREC_F, G, G.k33, 0.0);   // g^{t3} = 0 for both metrics
   metric_at(D.metric, D.a, xf1, xc2, G, d1, d2);
   store_geo(gf1, n2d, q, G);
   store_face_rec(gf1A + (size_t)q * NREC_F, G, G.k11, G.k01);
@@ -124,10 +128,10 @@ __global__ void k_geometry(Dev D, int e1, int e2, int n2d, double dx1, int n2glo
 
 void launch_geometry_tab(hamr_grid* g, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
                          double* gf2, double* dgc, double* rho_fl, double* u_fl, double* gcA, double* gf1A,
-                         double* gf2A) {
+                         double* gf2A, double* gf3A) {
   Launch l_(g, K_OTHER);
   k_geometry<<<(e1 * e2 + 127) / 128, 128, 0, g->stream>>>(g->D, e1, e2, n2d, dx1, n2glob, gc, gf1, gf2, dgc,
-                                                         rho_fl, u_fl, gcA, gf1A, gf2A);
+                                                         rho_fl, u_fl, gcA, gf1A, gf2A, gf3A);
 }
 
 }  // namespace hamr

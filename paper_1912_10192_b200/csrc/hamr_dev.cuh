@@ -74,8 +74,15 @@ __device__ __forceinline__ Geo load_geo(const double* __restrict__ tab, int n2d,
 // cache line (one L2 round trip when it misses L1) per COMPONENT, 15-50 per face or zone.  They therefore read
 // array-of-records copies: a centre record is 32 doubles (the 18 components of Geo in GeoComp order, then the 7 x1-
 // and the 7 x2-derivatives of the covariant metric) = two 128-byte lines; a face record is 16 doubles = one line.
+// Face records exist for the x1-faces, the x2-faces and the x3-faces (the latter at the zone centre's (x1, x2)) and
+// hold the 3+1 split of the face metric that the flux kernels work with (flux.cu):
 constexpr int NREC_C = 32, NREC_F = 16;
-// face record: c00 c01 c03 c11 c13 c22 c33 | k00 kdd k0d | gdet igdet alpha ialpha boa | pad
+enum FaceRec {
+  FREC_C11 = 0, FREC_C13, FREC_C22, FREC_C33,              // spatial metric g_ij
+  FREC_ALPHA, FREC_IALPHA, FREC_BOA, FREC_BETA1,           // lapse, 1/lapse, beta^1/lapse, beta^1
+  FREC_NALPHA2, FREC_K00, FREC_KDD, FREC_K0D,              // -lapse^2, g^{tt}, g^{dd}, g^{td} of the face's direction d
+  FREC_GDET, FREC_IGDET                                    // sqrt(-g), 1/sqrt(-g) (0 on the polar axis); 2 pad
+};
 __device__ __forceinline__ void load_rec(const double* __restrict__ rec, int n, double* v) {
   const double2* r2 = reinterpret_cast<const double2*>(rec);
 #pragma unroll

@@ -61,7 +61,8 @@ struct Dev {                 // everything a kernel may need, passed by value
   const double* dgc;         // [2][NDG][n2d]: d_1 g, d_2 g at centres
   const double* gcA;         // array-of-records copies for the hot kernels (hamr_dev.cuh): centres [n2d][32],
   const double* gf1A;        // x1-faces [n2d][16],
-  const double* gf2A;        // x2-faces [n2d][16]
+  const double* gf2A;        // x2-faces [n2d][16],
+  const double* gf3A;        // x3-faces [n2d][16] (centre (x1, x2))
   const double* rho_fl;      // [e1] floor per x1 index
   const double* u_fl;
   double* F[3][5];           // hydro fluxes on d-faces
@@ -211,7 +212,7 @@ void launch_deref_project(hamr_grid* g, const Dev& Dv, const Fields& s, const Fi
 int deref_row_factor(const hamr_params& p, long long J);
 void launch_geometry_tab(hamr_grid* g, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
                          double* gf2, double* dgc, double* rho_fl, double* u_fl, double* gcA, double* gf1A,
-                         double* gf2A);
+                         double* gf2A, double* gf3A);
 
 // blocks.cu: block-structured grid (H7)
 int blk_count(const hamr_params& p, int nslot[3], int bn[3]);       // number of blocks (0 if invalid)
