@@ -19,14 +19,41 @@ namespace hamr {
 
 constexpr double SIXTH = 1.0 / 6.0;
 
+// ---- reciprocal, reciprocal square root, square root for arguments known to be positive, finite and normal ----
+// The hardware seed (MUFU.RCP64H / MUFU.RSQ64H, ~20 bits) refined by fused multiply-adds, without the
+// range checks and slow-path calls of the library routines (six branches and convergence barriers per face
+// otherwise).  Results are within 2 ulp; nothing here decides a branch.
+__device__ __forceinline__ double rcp_pos(double a) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+  double e = fma(-a, y, 1.0);
+  y = fma(y, e, y);          // relative error e^2 ~ 2^-40
+  e = fma(-a, y, 1.0);
+  return fma(y, e, y);
+}
+__device__ __forceinline__ double rsqrt_pos(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x, y * y, 1.0);
+  return fma(fma(e, 0.375, 0.5), y * e, y);   // y (1 + e/2 + 3 e^2/8): relative error ~ e^3 ~ 2^-60
+}
+__device__ __forceinline__ double sqrt_pos(double x) {
+  const double y = rsqrt_pos(x), s = x * y;
+  return fma(fma(-s, s, x), 0.5 * y, s);      // one Heron correction of s = x y
+}
+
 // ---- C-5 reconstruction, branch-free ----------------------------------------------------------------
 // "dl and dr have the same sign" read off the sign bits (integer pipe; the FP64 pipe is the one these kernels
 // saturate).  A zero on either side makes the limited quantity zero by itself, so no product is needed.
 __device__ __forceinline__ bool same_sign(double a, double b) { return (__double2hiint(a) ^ __double2hiint(b)) >= 0; }
 
-// van Leer / CW84 limited slope from dl = a_j - a_{j-1}, dr = a_{j+1} - a_j, dc = (a_{j+1} - a_{j-1})/2
+// van Leer / CW84 limited slope from dl = a_j - a_{j-1}, dr = a_{j+1} - a_j, dc = (a_{j+1} - a_{j-1})/2:
+// sign(dc) min(|dc|, 2 |dl|, 2 |dr|) where dl, dr agree in sign, else 0.  The minimum is taken over the SIGNED
+// values by magnitude (the compares take |.| as operand modifiers, the selects move the raw words) and the sign
+// is imposed once at the end, so no absolute value is ever materialised on the FP64 pipe.
 __device__ __forceinline__ double lim_slope(double dl, double dr, double dc) {
-  const double lim = dmin(fabs(dc), 2.0 * dmin(fabs(dl), fabs(dr)));
+  const double m = 2.0 * (fabs(dl) < fabs(dr) ? dl : dr);
+  const double lim = fabs(dc) < fabs(m) ? dc : m;
   return same_sign(dl, dr) ? copysign(lim, dl) : 0.0;   // sign(dc) = sign(dl) where the slope survives
 }
 
@@ -96,6 +123,20 @@ __device__ __forceinline__ FGeo load_fgeo(const double* __restrict__ rec) {
   return G;
 }
 
+// the same record from shared memory (every thread of the CTA reads the same words: a broadcast)
+__device__ __forceinline__ FGeo load_fgeo_shared(const double* rec) {
+  const double2* r2 = reinterpret_cast<const double2*>(rec);
+  double v[NREC_F];
+#pragma unroll
+  for (int q = 0; q < (NREC_F - 2) / 2; q++) { const double2 w = r2[q]; v[2 * q] = w.x; v[2 * q + 1] = w.y; }
+  FGeo G;
+  G.c11 = v[FREC_C11]; G.c13 = v[FREC_C13]; G.c22 = v[FREC_C22]; G.c33 = v[FREC_C33];
+  G.alpha = v[FREC_ALPHA]; G.ialpha = v[FREC_IALPHA]; G.boa = v[FREC_BOA]; G.beta1 = v[FREC_BETA1];
+  G.nalpha2 = v[FREC_NALPHA2]; G.k00 = v[FREC_K00]; G.kdd = v[FREC_KDD]; G.k0d = v[FREC_K0D];
+  G.gdet = v[FREC_GDET]; G.igdet = v[FREC_IGDET];
+  return G;
+}
+
 // What the HLL combination needs from one side of the face.  The rows of U and F are never formed: with
 // T^mu_nu = eta u^mu u_nu + ptot delta^mu_nu - b^mu b_nu (eta = w + b^2, ptot = p + b^2/2) a weighted sum
 // wF F_nu + wU U_nu of the flux and conserved rows is (eta X) u_nu - Y b_nu + wF ptot delta^d_nu with the two scalars
@@ -115,7 +156,7 @@ __device__ __forceinline__ void side_state(const double P[8], const FGeo& G, dou
   S.ul[2] = G.c22 * P[3];
   S.ul[3] = G.c13 * P[2] + G.c33 * P[4];
   const double q1 = 1.0 + (P[2] * S.ul[1] + P[3] * S.ul[2] + P[4] * S.ul[3]);
-  const double rg = rsqrt(q1);  // gamma = q1 rg and 1/u^t = alpha/gamma = alpha rg share one special-function call
+  const double rg = rsqrt_pos(q1);   // q1 >= 1  // gamma = q1 rg and 1/u^t = alpha/gamma = alpha rg share one special-function call
   const double gam = q1 * rg;
   double u[4], b[4];
   u[0] = gam * G.ialpha;
@@ -160,26 +201,26 @@ __device__ __forceinline__ void side_state(const double P[8], const FGeo& G, dou
   S.a2 = (u[0] * u[0]) * M - G.k00 * N;
   const double h = (u[dir] * u[0]) * M - G.k0d * N;
   const double a0 = (u[dir] * u[dir]) * M - G.kdd * N;
-  const double disc = sqrt(dmax(h * h - S.a2 * a0, 0.0));
+  const double disc = sqrt_pos(dmax(h * h - S.a2 * a0, 1e-300));   // the floor is ~1e-130 of the scale of h
   S.vp = h + disc;
   S.vm = disc - h;
 }
 
-// HLL (C-7) from the two states; writes the 7 outputs of the face; returns ctop
+// HLL (C-7) from the two states: the 7 outputs of the face (5 hydro fluxes, E_f, E_e); returns ctop
 template <int D>
 __device__ __forceinline__ double face_flux(const double PL[8], const double PR[8], const FGeo& G, double gam_ad,
-                                            const Dev& Dv, int z) {
+                                            double out[7]) {
   constexpr int dir = D + 1;
   Side L, R;
   side_state<D>(PL, G, gam_ad, L);
   side_state<D>(PR, G, gam_ad, R);
-  const double ia = 1.0 / (L.a2 * R.a2);   // one reciprocal for both sides
+  const double ia = rcp_pos(L.a2 * R.a2);   // one reciprocal for both sides
   const double iL = R.a2 * ia, iR = L.a2 * ia;
   const double cmax = dmax(0.0, dmax(L.vp * iL, R.vp * iR));
   const double cmin = dmax(0.0, dmax(L.vm * iL, R.vm * iR));
   const double sum = cmax + cmin;
   const bool avg = sum < 1e-300;
-  const double isg = avg ? 0.0 : G.gdet / sum;
+  const double isg = avg ? 0.0 : G.gdet * rcp_pos(sum);
   // F = g [cmax FL + cmin FR - cmax cmin (UR - UL)] / (cmax + cmin);  average if both speeds vanish
   const double wl = avg ? 0.5 * G.gdet : cmax * isg;
   const double wr = avg ? 0.5 * G.gdet : cmin * isg;
@@ -197,13 +238,30 @@ __device__ __forceinline__ double face_flux(const double PL[8], const double PR[
   for (int c = 0; c < 4; c++) Fh[c] = (AL * L.ul[c] - YL * L.bl[c]) + (AR * R.ul[c] - YR * R.bl[c]);
   Fh[dir] += wl * L.ptot + wr * R.ptot;   // delta^d_nu of the flux rows
   Fh[0] += wc * (L.ptot - R.ptot);        // delta^t_nu of the conserved rows
-  Dv.F[D][0][z] = Fh0;
-  Dv.F[D][1][z] = Fh[0] + Fh0;   // the energy row carries T^d_t + rho u^d (C-4)
+  out[0] = Fh0;
+  out[1] = Fh[0] + Fh0;   // the energy row carries T^d_t + rho u^d (C-4)
 #pragma unroll
-  for (int c = 1; c < 4; c++) Dv.F[D][1 + c][z] = Fh[c];
-  Dv.EfB[D][z] = -(wl * L.Fe + wr * R.Fe - wc * (R.Be - L.Be));  // C-8: on a d-face, E_f = -F^d(B^e)
-  Dv.EfA[D][z] = wl * L.Ff + wr * R.Ff - wc * (R.Bf - L.Bf);     //                    E_e = +F^d(B^f)
+  for (int c = 1; c < 4; c++) out[1 + c] = Fh[c];
+  out[5] = -(wl * L.Fe + wr * R.Fe - wc * (R.Be - L.Be));  // C-8: on a d-face, E_f = -F^d(B^e)
+  out[6] = wl * L.Ff + wr * R.Ff - wc * (R.Bf - L.Bf);     //                    E_e = +F^d(B^f)
   return dmax(cmax, cmin);
+}
+
+__device__ __forceinline__ void store_face(const Dev& Dv, int D, int z, const double out[7]) {
+#pragma unroll
+  for (int c = 0; c < 5; c++) Dv.F[D][c][z] = out[c];
+  Dv.EfB[D][z] = out[5];
+  Dv.EfA[D][z] = out[6];
+}
+
+// all three kinds of call sites: HLL on one face, results to the face arrays at z
+template <int D>
+__device__ __forceinline__ double face_flux(const double PL[8], const double PR[8], const FGeo& G, double gam_ad,
+                                            const Dev& Dv, int z) {
+  double out[7];
+  const double ct = face_flux<D>(PL, PR, G, gam_ad, out);
+  store_face(Dv, D, z, out);
+  return ct;
 }
 
 __device__ __forceinline__ void zero_face(const Dev& Dv, int D, int z) {
@@ -342,6 +400,154 @@ __global__ void __launch_bounds__(HAMR_MARCH_T, HAMR_MARCH_MINB * 128 / HAMR_MAR
     }
   }
   if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
+}
+
+// ---- sweeps along x1 / x2 through a shared-memory ring filled by bulk asynchronous copies (TMA) -----------
+// north_star: "per-direction fused reconstruct+HLL kernels that stage stencil tiles through shared memory or TMA".
+// Monolithic grids with PPM whose x3 extent is a multiple of the CTA width KT and periodic.  A CTA owns KT
+// consecutive x3 positions of ONE transverse row o and marches over a segment of faces; every row of the sweep it
+// needs (7 variables and the normal face field, KT doubles each, plus the 128-byte geometry record of the row's
+// face: all threads of the CTA are on the same (x1, x2)) is brought into a ring of RING slots by 9 bulk copies
+// (cp.async.bulk, completion on an mbarrier) issued three rows ahead by one thread.  The marching loop reads shared
+// memory only: no load of the loop can miss a cache, no address arithmetic per variable, and the rows in flight
+// hold no registers.  The x3-faces of the transverse ghost columns k = -1 and k = n3, which C-9 reads, are the
+// periodic images of columns n3 - 1 and 0: their threads store twice.
+namespace ring {
+constexpr int RING = 6;   // 3 live rows (zones fc, fc + 1, fc + 2) + 3 in flight
+__device__ __forceinline__ unsigned su32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(su32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect(unsigned long long* b, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(su32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(su32(dst)),
+               "l"(src), "r"(bytes), "r"(su32(b))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "HAMR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra HAMR_DONE;\n"
+      "bra HAMR_WAIT;\n"
+      "HAMR_DONE:\n"
+      "}" ::"r"(su32(b)),
+      "r"(parity)
+      : "memory");
+}
+}  // namespace ring
+
+#ifndef HAMR_RING_MINB
+#define HAMR_RING_MINB 4
+#endif
+template <int D, int KT>
+__global__ void __launch_bounds__(KT, HAMR_RING_MINB * 128 / KT) k_flux_ring(Dev Dv, Fields s, int seg, int want_ctop) {
+  static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
+  using namespace ring;
+  constexpr int O = 1 - D;
+  constexpr int e = (D + 1) % 3, f = (D + 2) % 3;
+  constexpr int SLOTD = 8 * KT + NREC_F;   // doubles per ring slot: 7 variables, the face field, the face record
+  extern __shared__ __align__(128) double ring_mem[];
+  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(ring_mem + RING * SLOTD);
+  const Lay& L = Dv.L;
+  const int t = threadIdx.x;
+  const int k0 = blockIdx.x * KT, k = k0 + t;
+  const int o = (int)blockIdx.y - 1;
+  const int f0 = blockIdx.z * seg, f1 = min(f0 + seg, L.n[D] + 1);
+  const int sd = (D == 0) ? L.S1 : L.S2;
+  const int rbase = f0 - 3, rlast = f1 + 1;   // rows (zones along the sweep) this CTA reads
+  const double* gtab = (D == 0 ? Dv.gf1A : Dv.gf2A);
+  // thread 0 is the producer: row r of every array, and the record of face r, into slot (r - rbase) % RING
+  auto issue = [&](int r) {
+    const int n = r - rbase, sl = n % RING;
+    double* dst = ring_mem + sl * SLOTD;
+    const long long zr = L.idx(D == 0 ? r : o, D == 0 ? o : r, k0);
+    const bool face = r >= f0 && r < f1;   // rows that are also faces of this segment carry field and record
+    mbar_expect(mbar + sl, (unsigned)((face ? 8 * KT + NREC_F : 7 * KT) * sizeof(double)));
+    const double* src[7] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[e], s.Bc[f]};
+#pragma unroll
+    for (int v = 0; v < 7; v++) bulk_g2s(dst + v * KT, src[v] + zr, KT * sizeof(double), mbar + sl);
+    if (face) {
+      bulk_g2s(dst + 7 * KT, s.Bf[D] + zr, KT * sizeof(double), mbar + sl);
+      const int q = (NG * L.e2 + NG) + ((D == 0) ? r * L.e2 + o : o * L.e2 + r);
+      bulk_g2s(dst + 8 * KT, gtab + (size_t)q * NREC_F, NREC_F * sizeof(double), mbar + sl);
+    }
+  };
+  if (t == 0) {
+    for (int c = 0; c < RING; c++) mbar_init(mbar + c, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    for (int r = rbase; r < rbase + RING && r <= rlast; r++) issue(r);
+  }
+  __syncthreads();
+  const bool act = o >= 0 && o < L.n[O];  // C-14: faces of ACTIVE zones (every k of the launch is active)
+  const bool ks = Dv.metric == HAMR_METRIC_KERR_SCHILD;
+  constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
+  int z = (int)L.idx(D == 0 ? f0 - 1 : o, D == 0 ? o : f0 - 1, k);
+  // the periodic images: column n3 - 1 also is column -1, column 0 also is column n3
+  const int dup = (k == L.n[2] - 1) ? -L.n[2] : (k == 0 ? L.n[2] : 0);
+  double PL[8], PR[8], dm[7], il[7];
+  double ctop = 0.0;
+  // prologue: the parabola of zone f0 - 1 from rows f0 - 3 .. f0 + 1 (slots 0 .. 4 of the first revolution)
+#pragma unroll
+  for (int c = 0; c < 5; c++) mbar_wait(mbar + c, 0);
+  {
+    const double* a = ring_mem + t;
+#pragma unroll
+    for (int v = 0; v < 7; v++) {
+      const double m2 = a[0 * SLOTD + v * KT], m1 = a[1 * SLOTD + v * KT], c0 = a[2 * SLOTD + v * KT],
+                   p1 = a[3 * SLOTD + v * KT], p2 = a[4 * SLOTD + v * KT];
+      const double d10 = m1 - m2, d21 = c0 - m1, d32 = p1 - c0, d43 = p2 - p1;
+      const double dm_m = lim_slope(d10, d21, 0.5 * (c0 - m2));
+      const double dm_0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
+      const double dm_p = lim_slope(d32, d43, 0.5 * (p2 - c0));
+      const double r = ppm_iface(c0, d32, dm_0, dm_p);
+      double aL;
+      ppm_mono(ppm_iface(m1, d21, dm_m, dm_0), c0, r, aL, PL[slot[v]]);
+      dm[v] = dm_p; il[v] = r;
+    }
+  }
+  for (int fc = f0; fc < f1; fc++) {
+    z += sd;
+    __syncthreads();   // every thread is done with the rows below fc: their slots can be refilled
+    if (t == 0) {
+      for (int r = (fc == f0 ? rbase : fc - 1) + RING; r <= fc - 1 + RING; r++)
+        if (r <= rlast) issue(r);
+    }
+    const int n0 = fc - rbase;   // ring position of row fc; rows fc + 1, fc + 2 follow
+    const int s0 = n0 % RING, s1 = (n0 + 1) % RING, s2 = (n0 + 2) % RING;
+    mbar_wait(mbar + s2, (unsigned)(((n0 + 2) / RING) & 1));
+    const double* r0 = ring_mem + s0 * SLOTD + t;
+    const double* r1 = ring_mem + s1 * SLOTD + t;
+    const double* r2 = ring_mem + s2 * SLOTD + t;
+    double carry[7];
+#pragma unroll
+    for (int v = 0; v < 7; v++) {
+      const double c0 = r0[v * KT], c1 = r1[v * KT], a2 = r2[v * KT];
+      const double d21 = c1 - c0, d32 = a2 - c1;
+      const double dmp = lim_slope(d21, d32, 0.5 * (a2 - c0));
+      const double r = ppm_iface(c0, d21, dm[v], dmp);
+      ppm_mono(il[v], c0, r, PR[slot[v]], carry[v]);
+      dm[v] = dmp; il[v] = r;
+    }
+    const bool pole = (D == 1) && ks && (fc == 0 || fc == L.n[1]);
+    double out[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // C-7: pole faces carry no flux and no state is evaluated there
+    if (!pole) {
+      const FGeo G = load_fgeo_shared(ring_mem + s0 * SLOTD + 8 * KT);
+      PL[5 + D] = PR[5 + D] = r0[7 * KT] * G.igdet;  // C-5: the normal field is single-valued at the face
+      const double ct = face_flux<D>(PL, PR, G, Dv.gam, out);
+      if (act) ctop = dmax(ctop, ct);
+    }
+    store_face(Dv, D, z, out);
+    if (dup != 0) store_face(Dv, D, z + dup, out);
+#pragma unroll
+    for (int v = 0; v < 7; v++) PL[slot[v]] = carry[v];
+  }
+  if (want_ctop) ctop_commit<false>(Dv, D, 0, ctop);
 }
 
 // ---- sweep along x3: one lane per zone, neighbouring lanes exchange slopes and edges -------------------
@@ -527,10 +733,55 @@ static void launch_march_t(hamr_grid* g, const Dev& Dv, const Fields& src, const
   k_flux_march<D, RECON, BLK><<<grid, HAMR_MARCH_T, 0, g->stream>>>(Dv, src, src2, seg, want_ctop ? 1 : 0);
 }
 
+// the ring kernel: segment length such that the grid fills whole waves of resident CTAs
+template <int D, int KT>
+static void launch_ring_t(hamr_grid* g, const Dev& Dv, const Fields& src, bool want_ctop) {
+  const Lay& L = Dv.L;
+  const int O = 1 - D;
+  const size_t smem = (size_t)ring::RING * ((8 * KT + NREC_F) * sizeof(double)) + ring::RING * sizeof(unsigned long long);
+  static int per_sm = 0;   // set once per instantiation (the attribute and the occupancy are per function)
+  if (per_sm == 0) {
+    cudaFuncSetAttribute(k_flux_ring<D, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    int v = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_flux_ring<D, KT>, KT, smem);
+    per_sm = v < 1 ? 1 : v;
+  }
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int nf = L.n[D] + 1, nrow = (L.n[2] / KT) * (L.n[O] + 2);
+  const double slots = (double)sms * per_sm;
+  double best = -1.0;
+  int best_seg = nf;
+  for (int nseg = 1; nseg <= nf && nseg <= 64; nseg++) {
+    const int seg = (nf + nseg - 1) / nseg;
+    if (seg < 8 && nseg > 1) break;
+    const int ns = (nf + seg - 1) / seg;
+    const double blocks = (double)nrow * ns, waves = ceil(blocks / slots);
+    // useful work / occupied slot-time: wave fill x (faces / (faces + one prologue zone per segment))
+    const double eff = blocks / (waves * slots) * ((double)nf / ((double)ns * (seg + 1)));
+    if (eff > best) { best = eff; best_seg = seg; }
+  }
+  dim3 grid(L.n[2] / KT, L.n[O] + 2, (nf + best_seg - 1) / best_seg);
+  k_flux_ring<D, KT><<<grid, KT, smem, g->stream>>>(Dv, src, best_seg, want_ctop ? 1 : 0);
+}
+
+// the shared-memory ring serves monolithic PPM grids whose x3 extent is periodic, not derefined, and a multiple of 32
+static int ring_width(const Dev& Dv) {
+  const int n3 = Dv.L.n[2];
+  if (Dv.B.nblk > 0 || Dv.recon != HAMR_RECON_PPM || Dv.mrow || Dv.bc_lo[2] != HAMR_BC_PERIODIC) return 0;
+  if (Dv.L.n[0] + 2 > 65535 || Dv.L.n[1] + 2 > 65535) return 0;
+  return n3 % 128 == 0 ? 128 : (n3 % 64 == 0 ? 64 : (n3 % 32 == 0 ? 32 : 0));
+}
+
 template <int D>
 static void launch_march(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
   Launch l_(g, K_FLUX1 + D);
   const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
+  const int kt = ring_width(Dv);
+  if (kt == 128) return launch_ring_t<D, 128>(g, Dv, src, want_ctop);
+  if (kt == 64) return launch_ring_t<D, 64>(g, Dv, src, want_ctop);
+  if (kt == 32) return launch_ring_t<D, 32>(g, Dv, src, want_ctop);
   if (ppm && !blk) launch_march_t<D, HAMR_RECON_PPM, false>(g, Dv, src, src2, want_ctop);
   else if (ppm) launch_march_t<D, HAMR_RECON_PPM, true>(g, Dv, src, src2, want_ctop);
   else if (!blk) launch_march_t<D, HAMR_RECON_PLM_MC, false>(g, Dv, src, src2, want_ctop);
