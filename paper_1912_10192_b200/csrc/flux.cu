@@ -413,7 +413,11 @@ __global__ void __launch_bounds__(HAMR_MARCH_T, HAMR_MARCH_MINB * 128 / HAMR_MAR
 // hold no registers.  The x3-faces of the transverse ghost columns k = -1 and k = n3, which C-9 reads, are the
 // periodic images of columns n3 - 1 and 0: their threads store twice.
 namespace ring {
-constexpr int RING = 6;   // 3 live rows (zones fc, fc + 1, fc + 2) + 3 in flight
+#ifndef HAMR_RING_SLOTS
+#define HAMR_RING_SLOTS 6
+#endif
+constexpr int RING = HAMR_RING_SLOTS;   // 3 live rows (zones fc, fc + 1, fc + 2) + the rows in flight
+static_assert(RING >= 6, "the prologue holds the six rows of two adjacent PPM stencils");
 __device__ __forceinline__ unsigned su32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(su32(b)), "r"(count) : "memory");
@@ -425,6 +429,12 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(su32(dst)),
                "l"(src), "r"(bytes), "r"(su32(b))
                : "memory");
+}
+// one lane of a converged warp
+__device__ __forceinline__ bool elect_one() {
+  unsigned p;
+  asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}" : "=r"(p));
+  return p != 0;
 }
 __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
   asm volatile(
@@ -442,7 +452,13 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity
 }  // namespace ring
 
 #ifndef HAMR_RING_MINB
-#define HAMR_RING_MINB 4
+#define HAMR_RING_MINB 3
+#endif
+#ifndef HAMR_RING_PIPE
+#define HAMR_RING_PIPE 0
+#endif
+#ifndef HAMR_RING_UNROLL2
+#define HAMR_RING_UNROLL2 1
 #endif
 template <int D, int KT>
 __global__ void __launch_bounds__(KT, HAMR_RING_MINB * 128 / KT) k_flux_ring(Dev Dv, Fields s, int seg, int want_ctop) {
@@ -459,31 +475,47 @@ __global__ void __launch_bounds__(KT, HAMR_RING_MINB * 128 / KT) k_flux_ring(Dev
   const int o = (int)blockIdx.y - 1;
   const int f0 = blockIdx.z * seg, f1 = min(f0 + seg, L.n[D] + 1);
   const int sd = (D == 0) ? L.S1 : L.S2;
-  const int rbase = f0 - 3, rlast = f1 + 1;   // rows (zones along the sweep) this CTA reads
+  const int rbase = f0 - 3, rlast = f1 + 1 + HAMR_RING_PIPE;   // rows (zones along the sweep) this CTA reads
   const double* gtab = (D == 0 ? Dv.gf1A : Dv.gf2A);
-  // thread 0 is the producer: row r of every array, and the record of face r, into slot (r - rbase) % RING
-  auto issue = [&](int r) {
-    const int n = r - rbase, sl = n % RING;
-    double* dst = ring_mem + sl * SLOTD;
-    const long long zr = L.idx(D == 0 ? r : o, D == 0 ? o : r, k0);
-    const bool face = r >= f0 && r < f1;   // rows that are also faces of this segment carry field and record
-    mbar_expect(mbar + sl, (unsigned)((face ? 8 * KT + NREC_F : 7 * KT) * sizeof(double)));
-    const double* src[7] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[e], s.Bc[f]};
-#pragma unroll
-    for (int v = 0; v < 7; v++) bulk_g2s(dst + v * KT, src[v] + zr, KT * sizeof(double), mbar + sl);
-    if (face) {
-      bulk_g2s(dst + 7 * KT, s.Bf[D] + zr, KT * sizeof(double), mbar + sl);
-      const int q = (NG * L.e2 + NG) + ((D == 0) ? r * L.e2 + o : o * L.e2 + r);
-      bulk_g2s(dst + 8 * KT, gtab + (size_t)q * NREC_F, NREC_F * sizeof(double), mbar + sl);
+  // The producer is one elected lane of warp 0: the next row of every array, and the record of its face, into the
+  // next slot.  Its state (row, slot, padded offset of the row, record index) is the same in every thread and
+  // advances by constants, so it lives in uniform registers.
+  int prow = rbase, pslot = 0;
+  int pz = (int)L.idx(D == 0 ? rbase : o, D == 0 ? o : rbase, k0);
+  int pq = (NG * L.e2 + NG) + ((D == 0) ? rbase * L.e2 + o : o * L.e2 + rbase);
+  const bool warp0 = t < 32;
+  auto issue_next = [&]() {
+    if (warp0 && elect_one()) {
+      double* dst = ring_mem + pslot * SLOTD;
+      unsigned long long* mb = mbar + pslot;
+      const bool face = prow >= f0 && prow < f1;   // rows that are also faces of this segment carry field and record
+      mbar_expect(mb, (unsigned)((face ? 8 * KT + NREC_F : 7 * KT) * sizeof(double)));
+      bulk_g2s(dst + 0 * KT, s.P[0] + pz, KT * sizeof(double), mb);
+      bulk_g2s(dst + 1 * KT, s.P[1] + pz, KT * sizeof(double), mb);
+      bulk_g2s(dst + 2 * KT, s.P[2] + pz, KT * sizeof(double), mb);
+      bulk_g2s(dst + 3 * KT, s.P[3] + pz, KT * sizeof(double), mb);
+      bulk_g2s(dst + 4 * KT, s.P[4] + pz, KT * sizeof(double), mb);
+      bulk_g2s(dst + 5 * KT, s.Bc[e] + pz, KT * sizeof(double), mb);
+      bulk_g2s(dst + 6 * KT, s.Bc[f] + pz, KT * sizeof(double), mb);
+      if (face) {
+        bulk_g2s(dst + 7 * KT, s.Bf[D] + pz, KT * sizeof(double), mb);
+        bulk_g2s(dst + 8 * KT, gtab + (size_t)pq * NREC_F, NREC_F * sizeof(double), mb);
+      }
     }
+    prow++;
+    pslot = (pslot + 1 == RING) ? 0 : pslot + 1;
+    pz += sd;
+    pq += (D == 0) ? L.e2 : 1;
   };
   if (t == 0) {
     for (int c = 0; c < RING; c++) mbar_init(mbar + c, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    for (int r = rbase; r < rbase + RING && r <= rlast; r++) issue(r);
   }
   __syncthreads();
+#pragma unroll 1
+  for (int c = 0; c < RING; c++)
+    if (prow <= rlast) issue_next();
   const bool act = o >= 0 && o < L.n[O];  // C-14: faces of ACTIVE zones (every k of the launch is active)
   const bool ks = Dv.metric == HAMR_METRIC_KERR_SCHILD;
   constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
@@ -492,6 +524,77 @@ __global__ void __launch_bounds__(KT, HAMR_RING_MINB * 128 / KT) k_flux_ring(Dev
   const int dup = (k == L.n[2] - 1) ? -L.n[2] : (k == 0 ? L.n[2] : 0);
   double PL[8], PR[8], dm[7], il[7];
   double ctop = 0.0;
+#if HAMR_RING_PIPE
+  // Software pipeline: step fc solves the Riemann problem of face fc (states built one step earlier) next to the
+  // parabola of zone fc + 1 (rows fc + 1 .. fc + 3).  The two are independent instruction streams in one basic
+  // block: the seven short limiter chains fill the issue slots that the long dependent chain of a side state
+  // (square root, reciprocal, quadratic) leaves empty.
+  double carry[7];
+  // prologue: the parabolas of zones f0 - 1 and f0 from rows f0 - 3 .. f0 + 2 (all slots of the first revolution)
+#pragma unroll
+  for (int c = 0; c < 6; c++) mbar_wait(mbar + c, 0);
+  {
+    const double* a = ring_mem + t;
+#pragma unroll
+    for (int v = 0; v < 7; v++) {
+      const double m2 = a[0 * SLOTD + v * KT], m1 = a[1 * SLOTD + v * KT], c0 = a[2 * SLOTD + v * KT],
+                   p1 = a[3 * SLOTD + v * KT], p2 = a[4 * SLOTD + v * KT], p3 = a[5 * SLOTD + v * KT];
+      const double d10 = m1 - m2, d21 = c0 - m1, d32 = p1 - c0, d43 = p2 - p1, d54 = p3 - p2;
+      const double dm_m = lim_slope(d10, d21, 0.5 * (c0 - m2));
+      const double dm_0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
+      const double dm_p = lim_slope(d32, d43, 0.5 * (p2 - c0));
+      const double dm_q = lim_slope(d43, d54, 0.5 * (p3 - p1));
+      const double r = ppm_iface(c0, d32, dm_0, dm_p), r2 = ppm_iface(p1, d43, dm_p, dm_q);
+      double aL;
+      ppm_mono(ppm_iface(m1, d21, dm_m, dm_0), c0, r, aL, PL[slot[v]]);
+      ppm_mono(r, p1, r2, PR[slot[v]], carry[v]);
+      dm[v] = dm_q; il[v] = r2;
+    }
+  }
+#if HAMR_RING_UNROLL2
+#pragma unroll 2
+#endif
+  for (int fc = f0; fc < f1; fc++) {
+    z += sd;
+    __syncthreads();   // every thread is done with the rows below fc: their slots can be refilled
+#pragma unroll 1
+    while (prow <= rlast && prow <= fc - 1 + RING) issue_next();
+    const int n0 = fc - rbase;   // ring position of row fc; rows fc + 1 .. fc + 3 follow
+    const int s0 = n0 % RING, s1 = (n0 + 1) % RING, s2 = (n0 + 2) % RING, s3 = (n0 + 3) % RING;
+    mbar_wait(mbar + s3, (unsigned)(((n0 + 3) / RING) & 1));
+    const double* r1 = ring_mem + s1 * SLOTD + t;
+    const double* r2 = ring_mem + s2 * SLOTD + t;
+    const double* r3 = ring_mem + s3 * SLOTD + t;
+    // stream A: HLL on face fc.  A pole face (C-7: no flux, no state) is computed on its record (gdet = 0) and
+    // discarded, so that the step stays one basic block
+    const FGeo G = load_fgeo_shared(ring_mem + s0 * SLOTD + 8 * KT);
+    PL[5 + D] = PR[5 + D] = ring_mem[s0 * SLOTD + 7 * KT + t] * G.igdet;  // C-5: the normal field is single-valued
+    double out[7];
+    const double ct = face_flux<D>(PL, PR, G, Dv.gam, out);
+    // stream B: the parabola of zone fc + 1 gives the right state of face fc + 1 and the left state of face fc + 2
+    double PRn[7], carryn[7];
+#pragma unroll
+    for (int v = 0; v < 7; v++) {
+      const double c0 = r1[v * KT], c1 = r2[v * KT], a2 = r3[v * KT];
+      const double d21 = c1 - c0, d32 = a2 - c1;
+      const double dmp = lim_slope(d21, d32, 0.5 * (a2 - c0));
+      const double r = ppm_iface(c0, d21, dm[v], dmp);
+      ppm_mono(il[v], c0, r, PRn[v], carryn[v]);
+      dm[v] = dmp; il[v] = r;
+    }
+    const bool pole = (D == 1) && ks && (fc == 0 || fc == L.n[1]);
+    if (pole) {
+#pragma unroll
+      for (int c = 0; c < 7; c++) out[c] = 0.0;
+    } else if (act) {
+      ctop = dmax(ctop, ct);
+    }
+    store_face(Dv, D, z, out);
+    if (dup != 0) store_face(Dv, D, z + dup, out);
+#pragma unroll
+    for (int v = 0; v < 7; v++) { PL[slot[v]] = carry[v]; PR[slot[v]] = PRn[v]; carry[v] = carryn[v]; }
+  }
+#else
   // prologue: the parabola of zone f0 - 1 from rows f0 - 3 .. f0 + 1 (slots 0 .. 4 of the first revolution)
 #pragma unroll
   for (int c = 0; c < 5; c++) mbar_wait(mbar + c, 0);
@@ -511,13 +614,15 @@ __global__ void __launch_bounds__(KT, HAMR_RING_MINB * 128 / KT) k_flux_ring(Dev
       dm[v] = dm_p; il[v] = r;
     }
   }
+#if HAMR_RING_UNROLL2
+#pragma unroll 2
+#endif
   for (int fc = f0; fc < f1; fc++) {
     z += sd;
     __syncthreads();   // every thread is done with the rows below fc: their slots can be refilled
-    if (t == 0) {
-      for (int r = (fc == f0 ? rbase : fc - 1) + RING; r <= fc - 1 + RING; r++)
-        if (r <= rlast) issue(r);
-    }
+    // rows below fc are dead: three after the prologue, one per step afterwards
+#pragma unroll 1
+    while (prow <= rlast && prow <= fc - 1 + RING) issue_next();
     const int n0 = fc - rbase;   // ring position of row fc; rows fc + 1, fc + 2 follow
     const int s0 = n0 % RING, s1 = (n0 + 1) % RING, s2 = (n0 + 2) % RING;
     mbar_wait(mbar + s2, (unsigned)(((n0 + 2) / RING) & 1));
@@ -547,6 +652,7 @@ __global__ void __launch_bounds__(KT, HAMR_RING_MINB * 128 / KT) k_flux_ring(Dev
 #pragma unroll
     for (int v = 0; v < 7; v++) PL[slot[v]] = carry[v];
   }
+#endif
   if (want_ctop) ctop_commit<false>(Dv, D, 0, ctop);
 }
 
@@ -584,6 +690,10 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
                           selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),
                           selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[0], s2.Bc[0], C.cur),
                           selp<BLK>(s.Bc[1], s2.Bc[1], C.cur)};
+  // the face's record and normal field are requested together with the stencil: one round trip to memory, not two
+  // (helper lanes read the record and field of the real zone they are clamped to)
+  const FGeo G = load_fgeo(Dv.gf3A + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * (BLK ? Dv.B.ge2 : L.e2) + j) * NREC_F);
+  const double bf3 = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z];
   double PL[8], PR[8];
 #pragma unroll
   for (int v = 0; v < 7; v++) {
@@ -606,9 +716,7 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
   // C-15: the x3-faces of a phi-derefined row are computed by k_deref_x3 with a strided stencil
   const bool fine_row = Dv.mrow == nullptr || __ldg(Dv.mrow + C.J0 + j + NG) == 1;
   if (valid && fine_row && lane >= HLO && lane < 32 - HHI && k >= 0 && k <= L.n[2]) {
-    const int ge2 = BLK ? Dv.B.ge2 : L.e2;
-    const FGeo G = load_fgeo(Dv.gf3A + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * ge2 + j) * NREC_F);
-    PL[7] = PR[7] = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z] * G.igdet;
+    PL[7] = PR[7] = bf3 * G.igdet;
     const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
     if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct;
   }
@@ -771,7 +879,10 @@ static int ring_width(const Dev& Dv) {
   const int n3 = Dv.L.n[2];
   if (Dv.B.nblk > 0 || Dv.recon != HAMR_RECON_PPM || Dv.mrow || Dv.bc_lo[2] != HAMR_BC_PERIODIC) return 0;
   if (Dv.L.n[0] + 2 > 65535 || Dv.L.n[1] + 2 > 65535) return 0;
-  return n3 % 128 == 0 ? 128 : (n3 % 64 == 0 ? 64 : (n3 % 32 == 0 ? 32 : 0));
+#ifndef HAMR_RING_KTMAX
+#define HAMR_RING_KTMAX 32
+#endif
+  return (n3 % 128 == 0 && HAMR_RING_KTMAX >= 128) ? 128 : ((n3 % 64 == 0 && HAMR_RING_KTMAX >= 64) ? 64 : (n3 % 32 == 0 ? 32 : 0));
 }
 
 template <int D>
