@@ -116,8 +116,8 @@ ArenaPlan plan_arena(const hamr_params& p, const Lay& L, const GridShape& G) {
   ArenaPlan a;
   size_t off = 0;
   a.arr = off; off += (size_t)G.narr * L.len * 8;
-  a.tabs = off; off += align_up((size_t)G.nlev * (((size_t)3 * NGEO + 2 * NDG) * L.n2d * 8 + (size_t)2 * G.te1 * 8), 256);
-  a.recs = off; off += align_up((size_t)G.nlev * (NREC_C + 3 * NREC_F) * L.n2d * 8, 256);   // array-of-records copies
+  a.tabs = off; off += align_up((size_t)G.nlev * ((size_t)2 * G.te1 * 8), 256);   // floor tables
+  a.recs = off; off += align_up((size_t)G.nlev * (NREC_C + 3 * NREC_F) * L.n2d * 8, 256);   // geometry records
   a.scal = off; off += 256;
   a.cnt = off; off += 256;
   a.stage_doubles = (size_t)8 * (p.n[0] + 1) * (p.n[1] + 1) * (p.n[2] + 1);
@@ -235,17 +235,11 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   D.B.blen = gs.blen;
   D.B.ge2 = gs.te2;
   D.B.n2g = p->n[1];
-  // geometry tables: [level][gc | gf1 | gf2 | dgc], then the floor tables [level][rho | u]
-  D.B.tlev = (int)(((size_t)3 * NGEO + 2 * NDG) * D.L.n2d);
+  // floor tables [level][rho | u], geometry records [level][centres | x1-faces | x2-faces | x3-faces]
   D.B.flev = 2 * gs.te1;
-  double* tabs = (double*)(base + ap.tabs);
-  double* gc = tabs;
-  double* gf1 = gc + (size_t)NGEO * D.L.n2d;
-  double* gf2 = gf1 + (size_t)NGEO * D.L.n2d;
-  double* dgc = gf2 + (size_t)NGEO * D.L.n2d;
-  double* rfl = tabs + (size_t)gs.nlev * D.B.tlev;
+  double* rfl = (double*)(base + ap.tabs);
   double* ufl = rfl + gs.te1;
-  D.gc = gc; D.gf1 = gf1; D.gf2 = gf2; D.dgc = dgc; D.rho_fl = rfl; D.u_fl = ufl;
+  D.rho_fl = rfl; D.u_fl = ufl;
   double* gcA = (double*)(base + ap.recs);
   double* gf1A = gcA + (size_t)NREC_C * D.L.n2d;
   double* gf2A = gf1A + (size_t)NREC_F * D.L.n2d;
@@ -259,10 +253,9 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
 
   e = cudaMemsetAsync(g->arena, 0, ap.total, g->stream);
   if (e == cudaSuccess) {
-    launch_geometry_tab(g, gs.te1, gs.te2, D.L.n2d, D.dx[0], p->n[1], gc, gf1, gf2, dgc, rfl, ufl, gcA, gf1A, gf2A, gf3A);
+    launch_geometry_tab(g, gs.te1, gs.te2, D.dx[0], p->n[1], rfl, ufl, gcA, gf1A, gf2A, gf3A);
     if (gs.nlev > 1)   // C-16: the refined level's tables, dx1 / 2
-      launch_geometry_tab(g, gs.te1, gs.te2, D.L.n2d, 0.5 * D.dx[0], p->n[1], gc + D.B.tlev, gf1 + D.B.tlev,
-                          gf2 + D.B.tlev, dgc + D.B.tlev, rfl + D.B.flev, ufl + D.B.flev, gcA + D.B.tlevA,
+      launch_geometry_tab(g, gs.te1, gs.te2, 0.5 * D.dx[0], p->n[1], rfl + D.B.flev, ufl + D.B.flev, gcA + D.B.tlevA,
                           gf1A + D.B.tlevA, gf2A + D.B.tlevA, gf3A + D.B.tlevA);
     e = cudaGetLastError();
   }

@@ -98,7 +98,7 @@ __device__ __forceinline__ void ghost_cell(const Dev& D, const Fields& s, int al
     if (!extra[d]) hi[d] = ghost_value(D, s.Bf[d], d, d, i + (d == 0), j + (d == 1), k + (d == 2));
   }
   if (zone_slot) {
-    const double g = __ldg(D.gc + GDET * L.n2d + L.idx2(i, j));
+    const double g = __ldg(D.gcA + (size_t)L.idx2(i, j) * NREC_C + CREC_GDET);
     if (D.mrow) {
       const int m = __ldg(D.mrow + j + NG), n3 = L.n[2];
       if (k >= 0 && k < n3) {
@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(256) k_ghosts_shell(Dev D, Fields s, int nj, l
   s.Bf[0][z] = lo0;
   s.Bf[1][z] = lo1;
   if (k != n3) s.Bf[2][z] = lo2;
-  const double g2 = 2.0 * __ldg(D.gc + GDET * L.n2d + L.idx2(i, j));
+  const double g2 = 2.0 * __ldg(D.gcA + (size_t)L.idx2(i, j) * NREC_C + CREC_GDET);
   s.Bc[0][z] = (lo0 + hi0) / g2;
   s.Bc[1][z] = (lo1 + hi1) / g2;
   s.Bc[2][z] = (lo2 + hi2) / g2;

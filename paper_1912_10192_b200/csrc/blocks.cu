@@ -233,9 +233,15 @@ __device__ HAMR_REF_INLINE double blk_fetch_ref(const Dev& Dv, const Bufs& B, co
           a3[w + 1] = 0.5 * (blk_at(Dv, B, kind, s.rq, tr, i0, j, k) + blk_at(Dv, B, kind, s.rq, tr, i0 + 1, j, k));
         }
       }
-      double aL, aR;
-      plm_zone(a3[0], a3[1], a3[2], aL, aR);
-      v = 0.5 * (a3[1] + (high_half ? aR : aL));
+      // C-16: piecewise linear in x1 with the MC-limited slope of the three coarse values, a quarter of a coarse
+      // zone off the coarse centre
+      const double dl = a3[1] - a3[0], dr = a3[2] - a3[1];
+      double sl = 0.0;
+      if (dl * dr > 0.0) {
+        sl = fmin(0.5 * fabs(a3[2] - a3[0]), 2.0 * fmin(fabs(dl), fabs(dr)));
+        if (dl < 0.0) sl = -sl;
+      }
+      v = 0.5 * (a3[1] + (high_half ? a3[1] + 0.5 * sl : a3[1] - 0.5 * sl));
     }
   }
   const int vc = kind >= 5 ? kind - 5 : (kind >= 2 ? kind - 2 : -1);
@@ -475,7 +481,7 @@ __global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(const __gri
     }
   } else if (zone_slot && (!zone_active || all || anymod)) {
     const int4 inf = __ldg(Dv.B.info + b);
-    const double g = __ldg(Dv.gc + inf.y * Dv.B.tlev + GDET * L.n2d + inf.x + id[0] * Dv.B.ge2 + id[1]);
+    const double g = __ldg(Dv.gcA + inf.y * Dv.B.tlevA + (size_t)(inf.x + id[0] * Dv.B.ge2 + id[1]) * NREC_C + CREC_GDET);
     if (Dv.mrow) {
       const int J = inf.w + id[1], n3 = L.n[2];
       const int m = __ldg(Dv.mrow + J + NG);
@@ -706,7 +712,7 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
       }
       if (touched) {
         const int q2 = inf.x + id[0] * Dv.B.ge2 + id[1];
-        const Geo G = load_geo(Dv.gc + inf.y * Dv.B.tlev, L.n2d, q2);
+        const CGeo G = load_cgeo(Dv.gcA + inf.y * Dv.B.tlevA + (size_t)q2 * NREC_C);
         double P[8], U[5], Bn[3], Pn[5];
         const int nw = 2 - curc;
 #pragma unroll
@@ -862,7 +868,7 @@ __global__ void __launch_bounds__(256) k_blk_diag(Dev Dv, Bufs B, int what) {
       if (what == 0) val = den;
       else if (den > 1e-12 * Dv.scal[S_DENMAX]) val = fabs(div) / den;
     } else if (what == 2) {
-      const Geo G = load_geo(Dv.gc + inf.y * Dv.B.tlev, L.n2d, inf.x + i * Dv.B.ge2 + j);
+      const CGeo G = load_cgeo(Dv.gcA + inf.y * Dv.B.tlevA + (size_t)(inf.x + i * Dv.B.ge2 + j) * NREC_C);
       double P[8];
       for (int c = 0; c < 5; c++) P[c] = s.P[c][z];
       for (int c = 0; c < 3; c++) P[5 + c] = s.Bc[c][z];

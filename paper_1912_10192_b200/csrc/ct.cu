@@ -29,8 +29,9 @@ __global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s0, Fields s2
   for (int c = 0; c < 3; c++) s.Bc[c] = selp<BLK>(s0.Bc[c], s2.Bc[c], C.cur);
   // the zone's geometry record (array-of-records table: two cache lines instead of seven, hamr_dev.cuh)
   const double* rec = Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)q * NREC_C;
-  const double c11 = __ldg(rec + C11), c13 = __ldg(rec + C13), c22 = __ldg(rec + C22), c33 = __ldg(rec + C33),
-               gdet = __ldg(rec + GDET), ialpha = __ldg(rec + IALPHA), boa = __ldg(rec + BOA);
+  const double c11 = __ldg(rec + CREC_C11), c13 = __ldg(rec + CREC_C13), c22 = __ldg(rec + CREC_C22),
+               c33 = __ldg(rec + CREC_C33), gdet = __ldg(rec + CREC_GDET), ialpha = __ldg(rec + CREC_IALPHA),
+               boa = __ldg(rec + CREC_BOA);
   const double v1 = s.P[2][z], v2 = s.P[3][z], v3 = s.P[4][z];
   const double gam = sqrt(1.0 + (c11 * v1 * v1 + c22 * v2 * v2 + c33 * v3 * v3 + 2.0 * (c13 * v1 * v3)));
   const double iut = 1.0 / (gam * ialpha);

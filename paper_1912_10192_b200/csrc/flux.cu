@@ -19,29 +19,6 @@ namespace hamr {
 
 constexpr double SIXTH = 1.0 / 6.0;
 
-// ---- reciprocal, reciprocal square root, square root for arguments known to be positive, finite and normal ----
-// The hardware seed (MUFU.RCP64H / MUFU.RSQ64H, ~20 bits) refined by fused multiply-adds, without the
-// range checks and slow-path calls of the library routines (six branches and convergence barriers per face
-// otherwise).  Results are within 2 ulp; nothing here decides a branch.
-__device__ __forceinline__ double rcp_pos(double a) {
-  double y;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
-  double e = fma(-a, y, 1.0);
-  y = fma(y, e, y);          // relative error e^2 ~ 2^-40
-  e = fma(-a, y, 1.0);
-  return fma(y, e, y);
-}
-__device__ __forceinline__ double rsqrt_pos(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  const double e = fma(-x, y * y, 1.0);
-  return fma(fma(e, 0.375, 0.5), y * e, y);   // y (1 + e/2 + 3 e^2/8): relative error ~ e^3 ~ 2^-60
-}
-__device__ __forceinline__ double sqrt_pos(double x) {
-  const double y = rsqrt_pos(x), s = x * y;
-  return fma(fma(-s, s, x), 0.5 * y, s);      // one Heron correction of s = x y
-}
-
 // ---- C-5 reconstruction, branch-free ----------------------------------------------------------------
 // "dl and dr have the same sign" read off the sign bits (integer pipe; the FP64 pipe is the one these kernels
 // saturate).  A zero on either side makes the limited quantity zero by itself, so no product is needed.
@@ -151,31 +128,13 @@ struct Side {
 template <int D>
 __device__ __forceinline__ void side_state(const double P[8], const FGeo& G, double gam_ad, Side& S) {
   constexpr int dir = D + 1, e = (D + 1) % 3, f = (D + 2) % 3;
-  // C-2
-  S.ul[1] = G.c11 * P[2] + G.c13 * P[4];
-  S.ul[2] = G.c22 * P[3];
-  S.ul[3] = G.c13 * P[2] + G.c33 * P[4];
-  const double q1 = 1.0 + (P[2] * S.ul[1] + P[3] * S.ul[2] + P[4] * S.ul[3]);
-  const double rg = rsqrt_pos(q1);   // q1 >= 1  // gamma = q1 rg and 1/u^t = alpha/gamma = alpha rg share one special-function call
-  const double gam = q1 * rg;
-  double u[4], b[4];
-  u[0] = gam * G.ialpha;
-  u[1] = P[2] - gam * G.boa;
-  u[2] = P[3];
-  u[3] = P[4];
-  S.ul[0] = G.beta1 * S.ul[1] - G.alpha * gam;
-  // C-3
-  b[0] = P[5] * S.ul[1] + P[6] * S.ul[2] + P[7] * S.ul[3];
-  const double iut = G.alpha * rg;
-  b[1] = (P[5] + b[0] * u[1]) * iut;
-  b[2] = (P[6] + b[0] * u[2]) * iut;
-  b[3] = (P[7] + b[0] * u[3]) * iut;
-  const double bt1 = b[1] + b[0] * G.beta1;
-  S.bl[1] = G.c11 * bt1 + G.c13 * b[3];
-  S.bl[2] = G.c22 * b[2];
-  S.bl[3] = G.c13 * bt1 + G.c33 * b[3];
-  S.bl[0] = G.nalpha2 * b[0] + G.beta1 * S.bl[1];
-  const double bsq = b[0] * S.bl[0] + b[1] * S.bl[1] + b[2] * S.bl[2] + b[3] * S.bl[3];
+  // C-2, C-3
+  St T;
+  state_3p1(P, G.c11, G.c13, G.c22, G.c33, G.alpha, G.ialpha, G.boa, G.beta1, G.nalpha2, T);
+  const double u[4] = {T.ut, T.u1, T.u2, T.u3}, b[4] = {T.b0, T.b1, T.b2, T.b3};
+  const double bsq = T.bsq;
+  S.ul[0] = T.ul0; S.ul[1] = T.ul1; S.ul[2] = T.ul2; S.ul[3] = T.ul3;
+  S.bl[0] = T.bl0; S.bl[1] = T.bl1; S.bl[2] = T.bl2; S.bl[3] = T.bl3;
   // C-4
   const double p = (gam_ad - 1.0) * P[1];
   const double w = P[0] + gam_ad * P[1];
@@ -214,13 +173,13 @@ __device__ __forceinline__ double face_flux(const double PL[8], const double PR[
   Side L, R;
   side_state<D>(PL, G, gam_ad, L);
   side_state<D>(PR, G, gam_ad, R);
-  const double ia = rcp_pos(L.a2 * R.a2);   // one reciprocal for both sides
+  const double ia = rcp_nr(L.a2 * R.a2);   // one reciprocal for both sides
   const double iL = R.a2 * ia, iR = L.a2 * ia;
   const double cmax = dmax(0.0, dmax(L.vp * iL, R.vp * iR));
   const double cmin = dmax(0.0, dmax(L.vm * iL, R.vm * iR));
   const double sum = cmax + cmin;
   const bool avg = sum < 1e-300;
-  const double isg = avg ? 0.0 : G.gdet * rcp_pos(sum);
+  const double isg = avg ? 0.0 : G.gdet * rcp_nr(sum);
   // F = g [cmax FL + cmin FR - cmax cmin (UR - UL)] / (cmax + cmin);  average if both speeds vanish
   const double wl = avg ? 0.5 * G.gdet : cmax * isg;
   const double wr = avg ? 0.5 * G.gdet : cmin * isg;

@@ -38,44 +38,12 @@ struct Lay {
   __host__ __device__ __forceinline__ int str(int d) const { return d == 0 ? S1 : (d == 1 ? S2 : 1); }
 };
 
-// ---- geometry tables (2-D over (i,j) incl. ghosts, SoA by component) ------------------------------
-enum GeoComp {
-  C00 = 0, C01, C03, C11, C13, C22, C33,  // covariant metric
-  K00, K01, K11, K13, K22, K33,           // contravariant metric
-  GDET, ALPHA, IALPHA, BOA,               // sqrt(-g), lapse, 1/lapse, beta^1/lapse
-  IGDET,                                  // 1/sqrt(-g) (0 on the polar axis)
-  NGEO
-};
-// centre-only extras: x1- and x2-derivatives of the 7 covariant components (for the source, C-12)
-enum DgComp { D00 = 0, D01, D03, D11, D13, D22, D33, NDG };
-
-struct Geo {
-  double c00, c01, c03, c11, c13, c22, c33;
-  double k00, k01, k11, k13, k22, k33;
-  double gdet, alpha, ialpha, boa, igdet;
-};
-
-__device__ __forceinline__ Geo load_geo(const double* __restrict__ tab, int n2d, int q) {
-  Geo G;
-  G.c00 = __ldg(tab + C00 * n2d + q); G.c01 = __ldg(tab + C01 * n2d + q);
-  G.c03 = __ldg(tab + C03 * n2d + q); G.c11 = __ldg(tab + C11 * n2d + q);
-  G.c13 = __ldg(tab + C13 * n2d + q); G.c22 = __ldg(tab + C22 * n2d + q);
-  G.c33 = __ldg(tab + C33 * n2d + q);
-  G.k00 = __ldg(tab + K00 * n2d + q); G.k01 = __ldg(tab + K01 * n2d + q);
-  G.k11 = __ldg(tab + K11 * n2d + q); G.k13 = __ldg(tab + K13 * n2d + q);
-  G.k22 = __ldg(tab + K22 * n2d + q); G.k33 = __ldg(tab + K33 * n2d + q);
-  G.gdet = __ldg(tab + GDET * n2d + q); G.alpha = __ldg(tab + ALPHA * n2d + q);
-  G.ialpha = __ldg(tab + IALPHA * n2d + q); G.boa = __ldg(tab + BOA * n2d + q);
-  G.igdet = __ldg(tab + IGDET * n2d + q);
-  return G;
-}
-
-// The hot kernels read a geometry RECORD with all lanes of a warp on the same (i, j): with the SoA tables that is one
-// cache line (one L2 round trip when it misses L1) per COMPONENT, 15-50 per face or zone.  They therefore read
-// array-of-records copies: a centre record is 32 doubles (the 18 components of Geo in GeoComp order, then the 7 x1-
-// and the 7 x2-derivatives of the covariant metric) = two 128-byte lines; a face record is 16 doubles = one line.
-// Face records exist for the x1-faces, the x2-faces and the x3-faces (the latter at the zone centre's (x1, x2)) and
-// hold the 3+1 split of the face metric that the flux kernels work with (flux.cu):
+// ---- geometry tables: one record per (i, j) of a 2-D table incl. ghosts ------------------------------
+// The kernels read a geometry RECORD with all lanes of a warp on the same (i, j): a record is one (faces) or two
+// (centres) 128-byte lines, so a warp's geometry costs one or two L1 / L2 round trips.  Records hold the 3+1 split
+// of the metric, which is what the per-zone physics below works with: spatial metric g_ij (the only non-zero
+// off-diagonal spatial component of either metric is g_13), lapse alpha, shift beta^1 (beta^2 = beta^3 = 0),
+// sqrt(-g).  Face records exist for x1-faces, x2-faces and x3-faces (the latter at the centre's (x1, x2)).
 constexpr int NREC_C = 32, NREC_F = 16;
 enum FaceRec {
   FREC_C11 = 0, FREC_C13, FREC_C22, FREC_C33,              // spatial metric g_ij
@@ -83,6 +51,25 @@ enum FaceRec {
   FREC_NALPHA2, FREC_K00, FREC_KDD, FREC_K0D,              // -lapse^2, g^{tt}, g^{dd}, g^{td} of the face's direction d
   FREC_GDET, FREC_IGDET                                    // sqrt(-g), 1/sqrt(-g) (0 on the polar axis); 2 pad
 };
+// centre record: the first 16 doubles are CGeo below; then the metric derivatives the source term contracts
+// (C-12): H1[7], H2[7] = the x1- and x2-derivatives of (g_00, g_01, g_03, g_11, g_13, g_22, g_33) with the
+// diagonal ones halved, so that (1/2) v^k v^l d_nu g_kl = sum_c H[c] (v v)_c over the 7 distinct products
+enum CentreRec {
+  CREC_C11 = 0, CREC_C13, CREC_C22, CREC_C33,              // spatial metric g_ij
+  CREC_I11, CREC_I13, CREC_I22, CREC_I33,                  // its inverse gamma^ij
+  CREC_ALPHA, CREC_IALPHA, CREC_BOA, CREC_BETA1,           // lapse, 1/lapse, beta^1/lapse, beta^1
+  CREC_GDET, CREC_IGDET, CREC_DLG1, CREC_DLG2,             // sqrt(-g), its reciprocal, d_1 and d_2 of ln sqrt(-g)
+  CREC_H1 = 16, CREC_H2 = 23, CREC_END = 30
+};
+enum HComp { H00 = 0, H01, H03, H11, H13, H22, H33, NH };
+
+struct CGeo {
+  double c11, c13, c22, c33;
+  double i11, i13, i22, i33;
+  double alpha, ialpha, boa, beta1;
+  double gdet, igdet, dlg1, dlg2;
+};
+
 __device__ __forceinline__ void load_rec(const double* __restrict__ rec, int n, double* v) {
   const double2* r2 = reinterpret_cast<const double2*>(rec);
 #pragma unroll
@@ -92,126 +79,203 @@ __device__ __forceinline__ void load_rec(const double* __restrict__ rec, int n, 
     v[2 * q + 1] = t.y;
   }
 }
-__device__ __forceinline__ Geo load_geo_rec(const double* __restrict__ rec) {
-  double v[18];
-  load_rec(rec, 18, v);
-  Geo G;
-  G.c00 = v[0]; G.c01 = v[1]; G.c03 = v[2]; G.c11 = v[3]; G.c13 = v[4]; G.c22 = v[5]; G.c33 = v[6];
-  G.k00 = v[7]; G.k01 = v[8]; G.k11 = v[9]; G.k13 = v[10]; G.k22 = v[11]; G.k33 = v[12];
-  G.gdet = v[13]; G.alpha = v[14]; G.ialpha = v[15]; G.boa = v[16]; G.igdet = v[17];
+__device__ __forceinline__ CGeo load_cgeo(const double* __restrict__ rec) {
+  double v[16];
+  load_rec(rec, 16, v);
+  CGeo G;
+  G.c11 = v[CREC_C11]; G.c13 = v[CREC_C13]; G.c22 = v[CREC_C22]; G.c33 = v[CREC_C33];
+  G.i11 = v[CREC_I11]; G.i13 = v[CREC_I13]; G.i22 = v[CREC_I22]; G.i33 = v[CREC_I33];
+  G.alpha = v[CREC_ALPHA]; G.ialpha = v[CREC_IALPHA]; G.boa = v[CREC_BOA]; G.beta1 = v[CREC_BETA1];
+  G.gdet = v[CREC_GDET]; G.igdet = v[CREC_IGDET]; G.dlg1 = v[CREC_DLG1]; G.dlg2 = v[CREC_DLG2];
   return G;
 }
 
-// ---- C-2, C-3: four-velocity and magnetic four-vector -----------------------------------------------
+// ---- reciprocal, reciprocal square root, square root for finite, normal, non-zero arguments ----------------
+// The hardware seed (MUFU.RCP64H / MUFU.RSQ64H, ~20 bits) refined by fused multiply-adds, without the range
+// checks and slow-path calls of the library routines.  Results are within 2 ulp; nothing here decides a branch.
+__device__ __forceinline__ double rcp_nr(double a) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+  double e = fma(-a, y, 1.0);
+  y = fma(y, e, y);          // relative error e^2 ~ 2^-40
+  e = fma(-a, y, 1.0);
+  return fma(y, e, y);
+}
+__device__ __forceinline__ double rsqrt_pos(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x, y * y, 1.0);
+  return fma(fma(e, 0.375, 0.5), y * e, y);   // y (1 + e/2 + 3 e^2/8): relative error ~ e^3 ~ 2^-60
+}
+__device__ __forceinline__ double sqrt_pos(double x) {
+  const double y = rsqrt_pos(x), s = x * y;
+  return fma(fma(-s, s, x), 0.5 * y, s);      // one Heron correction of s = x y
+}
+
+// plain compare-select min / max (no NaN special-casing, unlike fmin / fmax)
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+
+// ---- C-2, C-3: four-velocity and magnetic four-vector in the 3+1 split --------------------------------
+// With u^mu = ut^mu + gamma n^mu and n_i = 0: u_i = g_ij ut^j, gamma^2 = 1 + ut^i u_i, u^t = gamma / alpha,
+// u^i = ut^i - gamma beta^i / alpha, u_t = -alpha gamma + beta^i u_i.  With b^t = B^i u_i,
+// b^i = (B^i + b^t u^i) / u^t: b_i = g_ij (b^j + beta^j b^t), b_t = -alpha^2 b^t + beta^i b_i.
 struct St {
-  double ucon[4], ucov[4], bcon[4], bcov[4], bsq;
+  double ut, u1, u2, u3;        // u^mu
+  double ul0, ul1, ul2, ul3;    // u_mu
+  double b0, b1, b2, b3;        // b^mu
+  double bl0, bl1, bl2, bl3;    // b_mu
+  double bsq, gam, iut;         // b^2, Lorentz factor, 1/u^t
 };
 
-// q = g_ij ut^i ut^j
-__device__ __forceinline__ double vsq_tilde(const Geo& G, double v1, double v2, double v3) {
-  return G.c11 * v1 * v1 + G.c22 * v2 * v2 + G.c33 * v3 * v3 + 2.0 * (G.c13 * v1 * v3);
+// P = (rho, u, ut1, ut2, ut3, B1, B2, B3); nalpha2 = -alpha^2
+__device__ __forceinline__ void state_3p1(const double P[8], double c11, double c13, double c22, double c33,
+                                          double alpha, double ialpha, double boa, double beta1, double nalpha2,
+                                          St& S) {
+  S.ul1 = c11 * P[2] + c13 * P[4];
+  S.ul2 = c22 * P[3];
+  S.ul3 = c13 * P[2] + c33 * P[4];
+  const double q1 = 1.0 + (P[2] * S.ul1 + P[3] * S.ul2 + P[4] * S.ul3);
+  const double rg = rsqrt_pos(q1);   // q1 >= 1; gamma = q1 rg and 1/u^t = alpha rg share one special-function call
+  S.gam = q1 * rg;
+  S.iut = alpha * rg;
+  S.ut = S.gam * ialpha;
+  S.u1 = P[2] - S.gam * boa;
+  S.u2 = P[3];
+  S.u3 = P[4];
+  S.ul0 = beta1 * S.ul1 - alpha * S.gam;
+  S.b0 = P[5] * S.ul1 + P[6] * S.ul2 + P[7] * S.ul3;
+  S.b1 = (P[5] + S.b0 * S.u1) * S.iut;
+  S.b2 = (P[6] + S.b0 * S.u2) * S.iut;
+  S.b3 = (P[7] + S.b0 * S.u3) * S.iut;
+  const double bt1 = S.b1 + S.b0 * beta1;
+  S.bl1 = c11 * bt1 + c13 * S.b3;
+  S.bl2 = c22 * S.b2;
+  S.bl3 = c13 * bt1 + c33 * S.b3;
+  S.bl0 = nalpha2 * S.b0 + beta1 * S.bl1;
+  S.bsq = S.b0 * S.bl0 + S.b1 * S.bl1 + S.b2 * S.bl2 + S.b3 * S.bl3;
+}
+__device__ __forceinline__ void get_state(const double P[8], const CGeo& G, St& S) {
+  state_3p1(P, G.c11, G.c13, G.c22, G.c33, G.alpha, G.ialpha, G.boa, G.beta1, -(G.alpha * G.alpha), S);
 }
 
-__device__ __forceinline__ void lower(const Geo& G, const double v[4], double w[4]) {
-  w[0] = G.c00 * v[0] + G.c01 * v[1] + G.c03 * v[3];
-  w[1] = G.c01 * v[0] + G.c11 * v[1] + G.c13 * v[3];
-  w[2] = G.c22 * v[2];
-  w[3] = G.c03 * v[0] + G.c13 * v[1] + G.c33 * v[3];
-}
-
-// P = (rho, u, ut1, ut2, ut3, B1, B2, B3)
-__device__ __forceinline__ void get_state(const double P[8], const Geo& G, St& S) {
-  const double gam = sqrt(1.0 + vsq_tilde(G, P[2], P[3], P[4]));
-  S.ucon[0] = gam * G.ialpha;
-  S.ucon[1] = P[2] - gam * G.boa;   // beta^2 = beta^3 = 0 for both metrics
-  S.ucon[2] = P[3];
-  S.ucon[3] = P[4];
-  lower(G, S.ucon, S.ucov);
-  S.bcon[0] = P[5] * S.ucov[1] + P[6] * S.ucov[2] + P[7] * S.ucov[3];
-  const double iut = 1.0 / S.ucon[0];
-  S.bcon[1] = (P[5] + S.bcon[0] * S.ucon[1]) * iut;
-  S.bcon[2] = (P[6] + S.bcon[0] * S.ucon[2]) * iut;
-  S.bcon[3] = (P[7] + S.bcon[0] * S.ucon[3]) * iut;
-  lower(G, S.bcon, S.bcov);
-  S.bsq = S.bcon[0] * S.bcov[0] + S.bcon[1] * S.bcov[1] + S.bcon[2] * S.bcov[2] + S.bcon[3] * S.bcov[3];
-}
-
-// ---- C-4: conserved vector and flux -----------------------------------------------------------------
-// T^mu_nu = (w + b^2) u^mu u_nu + (p + b^2/2) delta^mu_nu - b^mu b_nu for fixed mu
-// hydro rows only: U = g (rho u^t, T^t_t + rho u^t, T^t_1, T^t_2, T^t_3)
+// ---- C-4: the hydro rows of the conserved vector -----------------------------------------------------------
+// U = g (rho u^t, T^t_t + rho u^t, T^t_1, T^t_2, T^t_3), T^t_nu = eta u^t u_nu + ptot delta^t_nu - b^t b_nu
 __device__ __forceinline__ void prim_to_U5(const double P[8], const St& S, double gdet, double gam_ad,
                                            double U[5]) {
   const double p = (gam_ad - 1.0) * P[1];
-  const double eta = P[0] + P[1] + p + S.bsq;
+  const double eta = P[0] + gam_ad * P[1] + S.bsq;
   const double ptot = p + 0.5 * S.bsq;
-  const double eu = eta * S.ucon[0], b0 = S.bcon[0];
-  const double D = P[0] * S.ucon[0];
+  const double eu = eta * S.ut;
+  const double D = P[0] * S.ut;
   U[0] = gdet * D;
-  U[1] = gdet * (eu * S.ucov[0] + ptot - b0 * S.bcov[0] + D);
-  U[2] = gdet * (eu * S.ucov[1] - b0 * S.bcov[1]);
-  U[3] = gdet * (eu * S.ucov[2] - b0 * S.bcov[2]);
-  U[4] = gdet * (eu * S.ucov[3] - b0 * S.bcov[3]);
+  U[1] = gdet * (eu * S.ul0 + ptot - S.b0 * S.bl0 + D);
+  U[2] = gdet * (eu * S.ul1 - S.b0 * S.bl1);
+  U[3] = gdet * (eu * S.ul2 - S.b0 * S.bl2);
+  U[4] = gdet * (eu * S.ul3 - S.b0 * S.bl3);
 }
 
-// ---- C-6: bounds on the fast-wave coordinate speeds along direction index dir = 1..3 ----------------
-// A = g^{dd}, Bq = g^{tt}, Cq = g^{td}
-__device__ __forceinline__ void wavespeeds(const double P[8], const St& S, double gam_ad, double A,
-                                           double Bq, double Cq, int dir, double& vmin, double& vmax) {
-  const double p = (gam_ad - 1.0) * P[1];
-  const double w = P[0] + P[1] + p;
-  const double cs2 = gam_ad * p / w;
-  const double va2 = S.bsq / (S.bsq + w);
-  double cm2 = cs2 + va2 - cs2 * va2;
-  cm2 = fmin(fmax(cm2, 0.0), 1.0);
-  const double ut = S.ucon[0], ud = S.ucon[dir];
-  const double a2 = ut * ut - (Bq + ut * ut) * cm2;
-  const double a1 = 2.0 * (ud * ut - (Cq + ud * ut) * cm2);
-  const double a0 = ud * ud - (A + ud * ud) * cm2;
-  const double disc = sqrt(fmax(a1 * a1 - 4.0 * a2 * a0, 0.0));
-  const double i2 = 1.0 / (2.0 * a2);
-  const double v1 = (a1 + disc) * i2;
-  const double v2 = (a1 - disc) * i2;
-  vmax = fmax(v1, v2);
-  vmin = fmin(v1, v2);
+// ---- C-12: geometric source ----------------------------------------------------------------------------
+// S_nu = g T^kappa_lambda Gamma^lambda_{nu kappa} = (g/2) T^{kappa lambda} d_nu g_{kappa lambda}; both metrics are
+// stationary and independent of x3, so S_t = S_3 = 0 identically.  With T^{kl} = eta u^k u^l + ptot g^{kl} - b^k b^l
+// and g^{kl} d_nu g_kl = 2 d_nu ln sqrt(-g):  S_nu = g [ sum_c H_nu[c] (eta (u u)_c - (b b)_c) + ptot d_nu ln sqrt(-g) ]
+// over the 7 distinct products (00, 01, 03, 11, 13, 22, 33); rec: the zone's centre record
+__device__ __forceinline__ void source_12(const double P[8], const St& S, const CGeo& G, double gam_ad,
+                                          const double* __restrict__ rec, double& S1, double& S2) {
+  const double eta = P[0] + gam_ad * P[1] + S.bsq;
+  const double ptot = (gam_ad - 1.0) * P[1] + 0.5 * S.bsq;
+  double w[NH];
+  w[H00] = eta * S.ut * S.ut - S.b0 * S.b0;
+  w[H01] = eta * S.ut * S.u1 - S.b0 * S.b1;
+  w[H03] = eta * S.ut * S.u3 - S.b0 * S.b3;
+  w[H11] = eta * S.u1 * S.u1 - S.b1 * S.b1;
+  w[H13] = eta * S.u1 * S.u3 - S.b1 * S.b3;
+  w[H22] = eta * S.u2 * S.u2 - S.b2 * S.b2;
+  w[H33] = eta * S.u3 * S.u3 - S.b3 * S.b3;
+  double h[2 * NH];
+  load_rec(rec + CREC_H1, 2 * NH, h);
+  double a1 = ptot * G.dlg1, a2 = ptot * G.dlg2;
+#pragma unroll
+  for (int c = 0; c < NH; c++) { a1 += h[c] * w[c]; a2 += h[NH + c] * w[c]; }
+  S1 = G.gdet * a1;
+  S2 = G.gdet * a2;
 }
 
-// ---- C-5: reconstruction -----------------------------------------------------------------------------
-__device__ __forceinline__ double ppm_slope(double am, double a0, double ap) {
-  const double dl = a0 - am, dr = ap - a0;
-  if (dl * dr <= 0.0) return 0.0;
-  const double dc = 0.5 * (ap - am);
-  const double lim = fmin(fabs(dc), fmin(2.0 * fabs(dl), 2.0 * fabs(dr)));
-  return dc > 0.0 ? lim : -lim;
-}
-
-// parabola edges of the zone with value a2 from a0..a4 = a[j-2..j+2] (Colella & Woodward 1984)
-__device__ __forceinline__ void ppm_zone(double a0, double a1, double a2, double a3, double a4,
-                                         double& aL, double& aR) {
-  const double dm_m = ppm_slope(a0, a1, a2);
-  const double dm_0 = ppm_slope(a1, a2, a3);
-  const double dm_p = ppm_slope(a2, a3, a4);
-  aL = a1 + 0.5 * (a2 - a1) - (dm_0 - dm_m) / 6.0;
-  aR = a2 + 0.5 * (a3 - a2) - (dm_p - dm_0) / 6.0;
-  if ((aR - a2) * (a2 - aL) <= 0.0) {
-    aL = aR = a2;
-  } else {
-    const double d = aR - aL;
-    const double c = a2 - 0.5 * (aL + aR);
-    if (d * c > d * d / 6.0) aL = 3.0 * a2 - 2.0 * aR;
-    else if (d * c < -d * d / 6.0) aR = 3.0 * a2 - 2.0 * aL;
+// ---- C-13: conserved -> primitive, 2-unknown (W = w gamma^2, v^2) Newton-Raphson (Noble et al. 2006) -------
+// In the 3+1 split the scheme's inputs are what the normal observer measures: D = alpha rho u^t = rho gamma,
+// Q_i = alpha T^t_i, the energy -Q.n = -(T^t_t - beta^i T^t_i) (rest mass removed from the energy row, C-4),
+// curlyB^i = alpha B^i, and all contractions use the spatial metric and its inverse.
+// U: densitised hydro rows; Bc: NEW cell-centred field; Pg: guess.  Returns 0 ok, 1 no convergence / non-finite.
+__device__ __forceinline__ int con2prim(const double U[5], const double Bc[3], const CGeo& G, double gam_ad,
+                                        const double Pg[5], double Pout[5]) {
+  const double D = G.alpha * (U[0] * G.igdet);
+  const double m1 = U[2] * G.igdet, m2 = U[3] * G.igdet, m3 = U[4] * G.igdet;   // T^t_i
+  const double Qdotn = (U[1] - U[0]) * G.igdet - G.beta1 * m1;                  // Q.n = T^t_t - beta^1 T^t_1
+  const double Q1 = G.alpha * m1, Q2 = G.alpha * m2, Q3 = G.alpha * m3;
+  const double Qu1 = G.i11 * Q1 + G.i13 * Q3, Qu2 = G.i22 * Q2, Qu3 = G.i13 * Q1 + G.i33 * Q3;   // Q~^i
+  const double Qtsq = Q1 * Qu1 + Q2 * Qu2 + Q3 * Qu3;
+  const double B1 = G.alpha * Bc[0], B2 = G.alpha * Bc[1], B3 = G.alpha * Bc[2];
+  const double Bsq = B1 * (G.c11 * B1 + G.c13 * B3) + B2 * (G.c22 * B2) + B3 * (G.c13 * B1 + G.c33 * B3);
+  const double QdB = Q1 * B1 + Q2 * B2 + Q3 * B3;
+  const double QdB2 = QdB * QdB;
+  const double cg = (gam_ad - 1.0) / gam_ad;
+  // guess from Pg: W = (rho + gamma_ad u) gamma^2, v^2 = 1 - 1/gamma^2
+  const double g2 = 1.0 + (Pg[2] * (G.c11 * Pg[2] + G.c13 * Pg[4]) + Pg[3] * (G.c22 * Pg[3]) +
+                           Pg[4] * (G.c13 * Pg[2] + G.c33 * Pg[4]));
+  double W = (Pg[0] + gam_ad * Pg[1]) * g2;
+  double v2 = dmin(dmax(1.0 - rcp_nr(g2), 0.0), 1.0 - 1e-15);
+  int extra = -1;
+  bool conv = false;
+  for (int it = 0; it < 30; it++) {
+    const double omv = 1.0 - v2;                   // in [1e-15, 1]
+    const double rs = rsqrt_pos(omv), sq = omv * rs;
+    const double iW = rcp_nr(W);
+    const double t = QdB2 * iW * iW;               // (Q.B)^2 / W^2
+    const double BW = Bsq + W;
+    const double f1 = Qtsq - v2 * BW * BW + t * (BW + W);
+    const double f2 = (cg * (W * omv - D * sq) - W) - Qdotn - 0.5 * (Bsq * (1.0 + v2) - t);
+    const double j11 = -2.0 * BW * (v2 + t * iW);
+    const double j12 = -BW * BW;
+    const double j21 = cg * omv - 1.0 - t * iW;
+    const double j22 = cg * (0.5 * D * rs - W) - 0.5 * Bsq;
+    const double idet = rcp_nr(j11 * j22 - j12 * j21);
+    const double dW = (j12 * f2 - j22 * f1) * idet;
+    const double dv = (j21 * f1 - j11 * f2) * idet;
+    W = fabs(W + dW);
+    v2 = dmin(dmax(v2 + dv, 0.0), 1.0 - 1e-15);
+    if (extra >= 0) {
+      if (++extra >= 2) { conv = true; break; }
+    } else if (fabs(dW) <= 1e-12 * W && fabs(dv) <= 1e-12) {
+      extra = 0;  // converged: take 2 more iterations so the result does not depend on the guess
+    }
   }
+  // a non-finite iterate never passes the convergence test (comparisons with NaN are false)
+  if (!conv) return 1;
+  const double rs = rsqrt_pos(1.0 - v2);           // gamma
+  const double rho = D * rcp_nr(rs);
+  const double iW = rcp_nr(W);
+  const double u = (W * (1.0 - v2) - rho) * rcp_nr(gam_ad);
+  if (!(fabs(rho) <= 1.79e308) || !(fabs(u) <= 1.79e308) || !(W <= 1.79e308)) return 1;
+  Pout[0] = rho;
+  Pout[1] = u;
+  const double fac = rs * rcp_nr(W + Bsq), qw = QdB * iW;
+  Pout[2] = fac * (Qu1 + qw * B1);
+  Pout[3] = fac * (Qu2 + qw * B2);
+  Pout[4] = fac * (Qu3 + qw * B3);
+  return 0;
 }
 
-// PLM with the MC limiter: minmod(2(a1-a0), (a2-a0)/2, 2(a2-a1))
-__device__ __forceinline__ void plm_zone(double a0, double a1, double a2, double& aL, double& aR) {
-  const double dl = 2.0 * (a1 - a0), dr = 2.0 * (a2 - a1), dc = 0.5 * (a2 - a0);
-  double s = 0.0;
-  if (dl * dr > 0.0) {
-    s = fmin(fabs(dc), fmin(fabs(dl), fabs(dr)));
-    if (dc < 0.0) s = -s;
+// floors and Lorentz-factor ceiling on primitives (C-13; PAPER.md:59)
+__device__ __forceinline__ void floors_ceiling(const CGeo& G, double rfl, double ufl, double gamma_max, double Pn[5],
+                                               int& nrf, int& nuf, int& ngc) {
+  if (Pn[0] < rfl) { Pn[0] = rfl; nrf = 1; }
+  if (Pn[1] < ufl) { Pn[1] = ufl; nuf = 1; }
+  const double q = Pn[2] * (G.c11 * Pn[2] + G.c13 * Pn[4]) + Pn[3] * (G.c22 * Pn[3]) + Pn[4] * (G.c13 * Pn[2] + G.c33 * Pn[4]);
+  if (q > gamma_max * gamma_max - 1.0) {   // gamma^2 = 1 + q > gamma_max^2
+    const double fac = sqrt((gamma_max * gamma_max - 1.0) / q);
+    Pn[2] *= fac; Pn[3] *= fac; Pn[4] *= fac;
+    ngc = 1;
   }
-  aL = a1 - 0.5 * s;
-  aR = a1 + 0.5 * s;
 }
 
 // positive doubles order like their bit patterns: max-reduce through an unsigned 64-bit atomic
@@ -219,100 +283,10 @@ __device__ __forceinline__ void atomic_max_pos(double* addr, double v) {
   atomicMax(reinterpret_cast<unsigned long long*>(addr), (unsigned long long)__double_as_longlong(v));
 }
 
-// plain compare-select min / max (no NaN special-casing, unlike fmin / fmax)
-__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
-__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
-
 __device__ __forceinline__ double warp_max(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
   return v;
-}
-
-// C-13: 2-unknown (W = w gamma^2, v^2) Newton-Raphson.  U: densitised hydro rows; Bc: NEW cell-centred
-// field; Pg: guess (the stage's source state).  Returns 0 ok, 1 no convergence, 2 non-finite.
-__device__ __forceinline__ int con2prim(const double U[5], const double Bc[3], const Geo& G, double gam_ad,
-                                        const double Pg[5], double Pout[5]) {
-  const double ig = 1.0 / G.gdet;
-  const double alpha = G.alpha;
-  const double rhout = U[0] * ig;
-  const double D = alpha * rhout;
-  // Q_mu = alpha T^t_mu with rho u^t removed from the energy row (C-4)
-  const double Q0 = alpha * (U[1] * ig - rhout), Q1 = alpha * (U[2] * ig), Q2 = alpha * (U[3] * ig),
-               Q3 = alpha * (U[4] * ig);
-  const double B1 = alpha * Bc[0], B2 = alpha * Bc[1], B3 = alpha * Bc[2];
-  const double Qc0 = G.k00 * Q0 + G.k01 * Q1;
-  const double Qc1 = G.k01 * Q0 + G.k11 * Q1 + G.k13 * Q3;
-  const double Qc2 = G.k22 * Q2;
-  const double Qc3 = G.k13 * Q1 + G.k33 * Q3;
-  const double n0 = -alpha * G.k00, n1 = -alpha * G.k01;  // n^mu = -alpha g^{mu t}; n^2 = n^3 = 0
-  const double Qdotn = Q0 * n0 + Q1 * n1;
-  const double QQ = Q0 * Qc0 + Q1 * Qc1 + Q2 * Qc2 + Q3 * Qc3;
-  const double Qtsq = QQ + Qdotn * Qdotn;
-  const double QdB = Q1 * B1 + Q2 * B2 + Q3 * B3;
-  const double Bsq = vsq_tilde(G, B1, B2, B3);
-  const double QdB2 = QdB * QdB;
-  const double cg = (gam_ad - 1.0) / gam_ad;
-
-  const double g2 = 1.0 + vsq_tilde(G, Pg[2], Pg[3], Pg[4]);
-  double W = (Pg[0] + gam_ad * Pg[1]) * g2;
-  double v2 = 1.0 - 1.0 / g2;
-  v2 = fmin(fmax(v2, 0.0), 1.0 - 1e-15);
-
-  int extra = -1;
-  bool conv = false;
-  for (int it = 0; it < 30; it++) {
-    const double omv = 1.0 - v2;
-    const double sq = sqrt(omv);
-    const double p = cg * (W * omv - D * sq);
-    const double dpdW = cg * omv;
-    const double dpdv = cg * (-W + D / (2.0 * sq));
-    const double BW = Bsq + W;
-    const double iW = 1.0 / W;
-    const double iW2 = iW * iW, iW3 = iW2 * iW;
-    const double f1 = Qtsq - v2 * BW * BW + QdB2 * (Bsq + 2.0 * W) * iW2;
-    const double f2 = -Qdotn - 0.5 * Bsq * (1.0 + v2) + 0.5 * QdB2 * iW2 - W + p;
-    const double j11 = -2.0 * v2 * BW - 2.0 * QdB2 * BW * iW3;
-    const double j12 = -BW * BW;
-    const double j21 = -QdB2 * iW3 - 1.0 + dpdW;
-    const double j22 = -0.5 * Bsq + dpdv;
-    const double idet = 1.0 / (j11 * j22 - j12 * j21);
-    const double dW = -(j22 * f1 - j12 * f2) * idet;
-    const double dv = -(-j21 * f1 + j11 * f2) * idet;
-    if (!isfinite(dW) || !isfinite(dv)) return 2;
-    W = fabs(W + dW);
-    v2 = fmin(fmax(v2 + dv, 0.0), 1.0 - 1e-15);
-    if (extra >= 0) {
-      if (++extra >= 2) { conv = true; break; }
-    } else if (fabs(dW) <= 1e-12 * fabs(W) && fabs(dv) <= 1e-12) {
-      extra = 0;  // converged: take 2 more iterations so the result does not depend on the guess
-    }
-  }
-  if (!conv) return 1;
-  const double gamma = 1.0 / sqrt(1.0 - v2);
-  const double rho = D / gamma;
-  const double u = (W / (gamma * gamma) - rho) / gam_ad;
-  if (!isfinite(rho) || !isfinite(u) || !isfinite(W)) return 2;
-  Pout[0] = rho;
-  Pout[1] = u;
-  const double fac = gamma / (W + Bsq), qw = QdB / W;
-  Pout[2] = fac * (Qc1 + Qdotn * n1 + qw * B1);
-  Pout[3] = fac * (Qc2 + qw * B2);
-  Pout[4] = fac * (Qc3 + qw * B3);
-  return 0;
-}
-
-// floors and Lorentz-factor ceiling on primitives (C-13; PAPER.md:59)
-__device__ __forceinline__ void floors_ceiling(const Geo& G, double rfl, double ufl, double gamma_max, double Pn[5],
-                                               int& nrf, int& nuf, int& ngc) {
-  if (Pn[0] < rfl) { Pn[0] = rfl; nrf = 1; }
-  if (Pn[1] < ufl) { Pn[1] = ufl; nuf = 1; }
-  const double gamma = sqrt(1.0 + vsq_tilde(G, Pn[2], Pn[3], Pn[4]));
-  if (gamma > gamma_max) {
-    const double fac = sqrt((gamma_max * gamma_max - 1.0) / (gamma * gamma - 1.0));
-    Pn[2] *= fac; Pn[3] *= fac; Pn[4] *= fac;
-    ngc = 1;
-  }
 }
 
 // ---- C-15: phi-ghost slots of derefined rows are in GROUP units -------------------------------------------

@@ -29,8 +29,8 @@ struct BlkDev {
   int blen;                  // doubles per block per array
   int ge2;                   // row pitch of the (global, per x1-level) geometry tables
   int n2g;                   // global N2 (pole faces: J == 0 or J == n2g)
-  int tlev, flev;            // offset in doubles of the level-1 geometry / floor tables
-  int tlevA;                 // the same for the array-of-records copies
+  int flev;                  // offset in doubles of the level-1 floor tables
+  int tlevA;                 // offset in doubles of the level-1 geometry records
   const int* list;           // [nact] block ids of this launch
   const int* dlist;          // [ndact] those of them that hold phi-derefined rows (C-15 kernels); NULL: use list
   int ndact;
@@ -55,13 +55,9 @@ struct Dev {                 // everything a kernel may need, passed by value
   double dx[3], x0[3];       // internal-coordinate spacing and origin
   double a, gam, cour, gamma_max;
   double rho_fl_coef, rho_fl_pow, u_fl_coef, u_fl_pow;
-  const double* gc;          // geometry at centres  [NGEO][n2d]
-  const double* gf1;         // at x1-faces
-  const double* gf2;         // at x2-faces (pole rows: gdet = 0)
-  const double* dgc;         // [2][NDG][n2d]: d_1 g, d_2 g at centres
-  const double* gcA;         // array-of-records copies for the hot kernels (hamr_dev.cuh): centres [n2d][32],
+  const double* gcA;         // geometry records (hamr_dev.cuh): centres [n2d][32],
   const double* gf1A;        // x1-faces [n2d][16],
-  const double* gf2A;        // x2-faces [n2d][16],
+  const double* gf2A;        // x2-faces [n2d][16] (pole rows: gdet = 0),
   const double* gf3A;        // x3-faces [n2d][16] (centre (x1, x2))
   const double* rho_fl;      // [e1] floor per x1 index
   const double* u_fl;
@@ -210,9 +206,8 @@ void launch_deref_fix_edges(hamr_grid* g, const Dev& Dv);
 void launch_deref_sync(hamr_grid* g, const Dev& Dv, const Fields& out, const Fields& out2);
 void launch_deref_project(hamr_grid* g, const Dev& Dv, const Fields& s, const Fields& s2);
 int deref_row_factor(const hamr_params& p, long long J);
-void launch_geometry_tab(hamr_grid* g, int e1, int e2, int n2d, double dx1, int n2glob, double* gc, double* gf1,
-                         double* gf2, double* dgc, double* rho_fl, double* u_fl, double* gcA, double* gf1A,
-                         double* gf2A, double* gf3A);
+void launch_geometry_tab(hamr_grid* g, int e1, int e2, double dx1, int n2glob, double* rho_fl, double* u_fl,
+                         double* gcA, double* gf1A, double* gf2A, double* gf3A);
 
 // blocks.cu: block-structured grid (H7)
 int blk_count(const hamr_params& p, int nslot[3], int bn[3]);       // number of blocks (0 if invalid)

@@ -112,7 +112,7 @@ __global__ void k_totals(Dev Dv, Fields s) {
   if (t < tot) {
     const int k = (int)(t % L.n[2]), j = (int)((t / L.n[2]) % L.n[1]), i = (int)(t / ((long long)L.n[2] * L.n[1]));
     const long long z = L.idx(i, j, k);
-    const Geo G = load_geo(Dv.gc, L.n2d, L.idx2(i, j));
+    const CGeo G = load_cgeo(Dv.gcA + (size_t)L.idx2(i, j) * NREC_C);
     double P[8];
     for (int c = 0; c < 5; c++) P[c] = s.P[c][z];
     for (int c = 0; c < 3; c++) P[5 + c] = s.Bc[c][z];

@@ -10,9 +10,10 @@ namespace hamr {
 
 // face-B update of the d-face on the low side of z (C-10):
 // Bf^d -= dt [ (E_f(e+) - E_f(e-))/dx^e - (E_e(f+) - E_e(f-))/dx^f ], (d,e,f) cyclic
+// All index arithmetic is 32-bit (an array holds fewer than 2^31 doubles, checked at creation).
 template <int d>
-__device__ __forceinline__ double bf_new(const Dev& Dv, const double* __restrict__ base, long long z, double dt,
-                                         const long long S[3], const double idx[3]) {
+__device__ __forceinline__ double bf_new(const Dev& Dv, const double* __restrict__ base, int z, double dt,
+                                         const int S[3], const double idx[3]) {
   constexpr int e = (d + 1) % 3, f = (d + 2) % 3;
   const double curl = (__ldg(Dv.Ee[f] + z + S[e]) - __ldg(Dv.Ee[f] + z)) * idx[e] -
                       (__ldg(Dv.Ee[e] + z + S[f]) - __ldg(Dv.Ee[e] + z)) * idx[f];
@@ -29,28 +30,21 @@ __device__ __forceinline__ Fields pick_fields(const Fields& a, const Fields& b, 
   return f;
 }
 
-#ifndef HAMR_UPD_RELOAD
-#define HAMR_UPD_RELOAD 1  // measured on cfg 2: 0.561 -> 0.516 ms (predictor) together with HAMR_UPD_MINB 6
-#endif
 #ifndef HAMR_UPD_MINB
-#define HAMR_UPD_MINB 6  // 80 regs (72 B spilled); 4 / 5 measured 4 % / 7 % slower with the reload, 8 slower still
+#define HAMR_UPD_MINB 6
 #endif
 #ifndef HAMR_UPD_MINB_PRED
-#define HAMR_UPD_MINB_PRED 7  // the predictor (one state to load) gains from 72 regs: 0.445 -> 0.429 ms; the corrector loses
+#define HAMR_UPD_MINB_PRED 7
 #endif
-#ifndef HAMR_UPD_T
-#define HAMR_UPD_T 128   // threads per CTA; 32 / 64 measured equal within noise, 256 is 4 % slower (cfg 2)
-#endif
-#ifndef HAMR_UPD_KFACE
-#define HAMR_UPD_KFACE 1
+#ifndef HAMR_UPD_RELOAD
+#define HAMR_UPD_RELOAD 1
 #endif
 template <bool SAME, bool BLK>  // SAME: predictor, source state == base state
-__global__ void __launch_bounds__(HAMR_UPD_T, (SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB) * 128 / HAMR_UPD_T) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
+__global__ void __launch_bounds__(128, SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
   const Lay& L = Dv.L;
   // k runs over [0, n3): warps start on 128-byte lines when n3 is a multiple of 32; the thread at k = 0 also
   // builds the x3-face at k = n3
-  const int c2 = L.n[2] + (HAMR_UPD_KFACE ? 0 : 1), c1 = L.n[1] + 1;
-  // 32-bit index arithmetic throughout: 64-bit division is emulated (~100 instructions each)
+  const int c2 = L.n[2], c1 = L.n[1] + 1;
   const unsigned per = (unsigned)(L.n[0] + 1) * c1 * c2;
   unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = t < (BLK ? per * Dv.B.nact : per);
@@ -65,26 +59,25 @@ __global__ void __launch_bounds__(HAMR_UPD_T, (SAME ? HAMR_UPD_MINB_PRED : HAMR_
     const int k = (int)(t - tj * c2);
     const int i = (int)(tj / (unsigned)c1);
     const int j = (int)(tj - i * c1);
-    const long long z = C.zoff + L.idx(i, j, k);
+    const int z = C.zoff + (int)L.idx(i, j, k);
     const double dt = dtfac * Dv.scal[S_DT];
-    const long long S[3] = {L.S1, L.S2, 1};
+    const int S[3] = {L.S1, L.S2, 1};
     const double idx[3] = {1.0 / ((BLK && C.lev) ? 0.5 * Dv.dx[0] : Dv.dx[0]), 1.0 / Dv.dx[1], 1.0 / Dv.dx[2]};
-    const bool in0 = i < L.n[0], in1 = j < L.n[1], in2 = k < L.n[2];
+    const bool in0 = i < L.n[0], in1 = j < L.n[1];
     const bool ks = Dv.metric == HAMR_METRIC_KERR_SCHILD;
     const int Jg = C.J0 + j, n2g = BLK ? Dv.B.n2g : L.n[1];
-    const int tl = BLK ? C.lev * Dv.B.tlev : 0;
     double lo[3] = {0.0, 0.0, 0.0};
-    if (in1 && in2) { lo[0] = bf_new<0>(Dv, base.Bf[0], z, dt, S, idx); out.Bf[0][z] = lo[0]; }
-    if (in0 && in2) {
+    if (in1) { lo[0] = bf_new<0>(Dv, base.Bf[0], z, dt, S, idx); out.Bf[0][z] = lo[0]; }
+    if (in0) {
       lo[1] = (ks && (Jg == 0 || Jg == n2g)) ? 0.0 : bf_new<1>(Dv, base.Bf[1], z, dt, S, idx);
       out.Bf[1][z] = lo[1];
     }
-    if (in0 && in1) { lo[2] = bf_new<2>(Dv, base.Bf[2], z, dt, S, idx); out.Bf[2][z] = lo[2]; }
-    if (HAMR_UPD_KFACE && in0 && in1 && k == 0) out.Bf[2][z + L.n[2]] = bf_new<2>(Dv, base.Bf[2], z + L.n[2], dt, S, idx);
-    if (in0 && in1 && in2) {
-      const int q = C.q0 + i * (BLK ? Dv.B.ge2 : L.e2) + j;
-      const double* grec = Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)q * NREC_C;
-      const Geo G = load_geo_rec(grec);
+    if (in0 && in1) {
+      lo[2] = bf_new<2>(Dv, base.Bf[2], z, dt, S, idx);
+      out.Bf[2][z] = lo[2];
+      if (k == 0) out.Bf[2][z + L.n[2]] = bf_new<2>(Dv, base.Bf[2], z + L.n[2], dt, S, idx);
+      const double* grec = Dv.gcA + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * (BLK ? Dv.B.ge2 : L.e2) + j) * NREC_C;
+      const CGeo G = load_cgeo(grec);
       // new cell-centred field from the new faces (the high faces are recomputed, bit-identically)
       double Bn[3];
       {
@@ -95,12 +88,12 @@ __global__ void __launch_bounds__(HAMR_UPD_T, (SAME ? HAMR_UPD_MINB_PRED : HAMR_
           // C-15: in a phi-derefined row B_c^3 is the GROUP's value, from the group's two outer x3-faces
           const int m = __ldg(Dv.mrow + Jg + NG);
           if (m > 1) {
-            const long long zg = z - (k % m);
+            const int zg = z - (k % m);
             l2 = bf_new<2>(Dv, base.Bf[2], zg, dt, S, idx);
             h2 = bf_new<2>(Dv, base.Bf[2], zg + m, dt, S, idx);
           }
         }
-        const double i2g = 1.0 / (2.0 * G.gdet);
+        const double i2g = 0.5 * G.igdet;
         Bn[0] = (lo[0] + h0) * i2g;
         Bn[1] = (lo[1] + h1) * i2g;
         Bn[2] = (l2 + h2) * i2g;
@@ -114,30 +107,7 @@ __global__ void __launch_bounds__(HAMR_UPD_T, (SAME ? HAMR_UPD_MINB_PRED : HAMR_
         St Ss;
         get_state(Ps, G, Ss);
         if (SAME) prim_to_U5(Ps, Ss, G.gdet, Dv.gam, U);
-        // C-12 source: S_nu = g T^kappa_lambda Gamma^lambda_{nu kappa} = (g/2) T^{kappa lambda} d_nu g_{kappa lambda};
-        // both metrics are stationary and independent of x3, so S_t = S_3 = 0 identically
-        const double p = (Dv.gam - 1.0) * Ps[1];
-        const double eta = Ps[0] + Ps[1] + p + Ss.bsq;
-        const double ptot = p + 0.5 * Ss.bsq;
-        const double* u = Ss.ucon;
-        const double* b = Ss.bcon;
-        const double T00 = eta * u[0] * u[0] + ptot * G.k00 - b[0] * b[0];
-        const double T01 = eta * u[0] * u[1] + ptot * G.k01 - b[0] * b[1];
-        const double T03 = eta * u[0] * u[3] - b[0] * b[3];
-        const double T11 = eta * u[1] * u[1] + ptot * G.k11 - b[1] * b[1];
-        const double T13 = eta * u[1] * u[3] + ptot * G.k13 - b[1] * b[3];
-        const double T22 = eta * u[2] * u[2] + ptot * G.k22 - b[2] * b[2];
-        const double T33 = eta * u[3] * u[3] + ptot * G.k33 - b[3] * b[3];
-        double dg[2 * NDG];   // d_1 g and d_2 g, in DgComp order, from the zone's record
-        load_rec(grec + NGEO, 2 * NDG, dg);
-        const double* d1 = dg;
-        double a1 = 0.5 * (T00 * d1[D00] + T11 * d1[D11] + T22 * d1[D22] + T33 * d1[D33]) + T01 * d1[D01] +
-                    T03 * d1[D03] + T13 * d1[D13];
-        const double* d2 = dg + NDG;
-        double a2 = 0.5 * (T00 * d2[D00] + T11 * d2[D11] + T22 * d2[D22] + T33 * d2[D33]) + T01 * d2[D01] +
-                    T03 * d2[D03] + T13 * d2[D13];
-        Ssrc1 = G.gdet * a1;
-        Ssrc2 = G.gdet * a2;
+        source_12(Ps, Ss, G, Dv.gam, grec, Ssrc1, Ssrc2);   // C-12: on the stage's source state
       }
       if (!SAME) {
         double Pb[8];
@@ -158,43 +128,33 @@ __global__ void __launch_bounds__(HAMR_UPD_T, (SAME ? HAMR_UPD_MINB_PRED : HAMR_
         const double sc = (c == 2) ? Ssrc1 : (c == 3 ? Ssrc2 : 0.0);
         U[c] = U[c] - dt * div + dt * sc;
       }
-      double Pn[5];
+      double Pn[5], Pg[5];
 #if HAMR_UPD_RELOAD
       // the geometry record and the guess are re-read (L1 / L2 hits) instead of being kept in registers
       // across the flux divergence: lower register pressure, more resident warps
       const double* gtab = grec;
       asm volatile("" : "+l"(gtab));
-      const Geo G2 = load_geo_rec(gtab);
+      const CGeo G2 = load_cgeo(gtab);
       const double* sp[5] = {src.P[0], src.P[1], src.P[2], src.P[3], src.P[4]};
-      double Pg[5];
 #pragma unroll
       for (int c = 0; c < 5; c++) { const double* a = sp[c]; asm volatile("" : "+l"(a)); Pg[c] = a[z]; }
-      const int rc = con2prim(U, Bn, G2, Dv.gam, Pg, Pn);
-      if (rc != 0) {
+#else
+      const CGeo& G2 = G;
+#pragma unroll
+      for (int c = 0; c < 5; c++) Pg[c] = Ps[c];
+#endif
+      if (con2prim(U, Bn, G2, Dv.gam, Pg, Pn) != 0) {  // C-13: keep the source state's hydro primitives, count the failure
         nfail = 1;
 #pragma unroll
         for (int c = 0; c < 5; c++) Pn[c] = Pg[c];
       }
-#define G G2
-#else
-      const int rc = con2prim(U, Bn, G, Dv.gam, Ps, Pn);
-      if (rc != 0) {  // C-13: keep the source state's hydro primitives, count the failure
-        nfail = 1;
-#pragma unroll
-        for (int c = 0; c < 5; c++) Pn[c] = Ps[c];
-      }
-#endif
       // floors and Lorentz-factor ceiling (C-13)
       const int fi = C.I0 + i + NG + (BLK ? C.lev * Dv.B.flev : 0);
-      const double rfl = __ldg(Dv.rho_fl + fi), ufl = __ldg(Dv.u_fl + fi);
-      floors_ceiling(G, rfl, ufl, Dv.gamma_max, Pn, nrf, nuf, ngc);
-#if HAMR_UPD_RELOAD
-#undef G
-#endif
+      floors_ceiling(G2, __ldg(Dv.rho_fl + fi), __ldg(Dv.u_fl + fi), Dv.gamma_max, Pn, nrf, nuf, ngc);
 #pragma unroll
       for (int c = 0; c < 5; c++) {
         out.P[c][z] = Pn[c];
-        if (!isfinite(Pn[c])) bad = 1;
+        if (!(fabs(Pn[c]) <= 1.79e308)) bad = 1;
       }
 #pragma unroll
       for (int c = 0; c < 3; c++) out.Bc[c][z] = Bn[c];
@@ -218,13 +178,13 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
   const Lay& L = Dv.L;
   const bool blk = Dv.B.nblk > 0;
   if (blk && Dv.B.nact == 0) return;
-  const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + (HAMR_UPD_KFACE ? 0 : 1)) * (blk ? Dv.B.nact : 1);
-  const unsigned nb = (unsigned)((tot + HAMR_UPD_T - 1) / HAMR_UPD_T);
+  const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * L.n[2] * (blk ? Dv.B.nact : 1);
+  const unsigned nb = (unsigned)((tot + 127) / 128);
   Launch l_(g, same ? K_UPDATE_P : K_UPDATE_C);
-  if (same && !blk) k_update<true, false><<<nb, HAMR_UPD_T, 0, g->stream>>>(Dv, ra, rb, dtfac);
-  else if (same) k_update<true, true><<<nb, HAMR_UPD_T, 0, g->stream>>>(Dv, ra, rb, dtfac);
-  else if (!blk) k_update<false, false><<<nb, HAMR_UPD_T, 0, g->stream>>>(Dv, ra, rb, dtfac);
-  else k_update<false, true><<<nb, HAMR_UPD_T, 0, g->stream>>>(Dv, ra, rb, dtfac);
+  if (same && !blk) k_update<true, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+  else if (same) k_update<true, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+  else if (!blk) k_update<false, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+  else k_update<false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
 }
 
 void launch_update(hamr_grid* g, const Fields& src, const Fields& base, const Fields& out, double dtfac,
