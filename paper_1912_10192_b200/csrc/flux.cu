@@ -377,37 +377,6 @@ namespace ring {
 #endif
 constexpr int RING = HAMR_RING_SLOTS;   // 3 live rows (zones fc, fc + 1, fc + 2) + the rows in flight
 static_assert(RING >= 6, "the prologue holds the six rows of two adjacent PPM stencils");
-__device__ __forceinline__ unsigned su32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(su32(b)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect(unsigned long long* b, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(su32(b)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(su32(dst)),
-               "l"(src), "r"(bytes), "r"(su32(b))
-               : "memory");
-}
-// one lane of a converged warp
-__device__ __forceinline__ bool elect_one() {
-  unsigned p;
-  asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}" : "=r"(p));
-  return p != 0;
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "HAMR_WAIT:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra HAMR_DONE;\n"
-      "bra HAMR_WAIT;\n"
-      "HAMR_DONE:\n"
-      "}" ::"r"(su32(b)),
-      "r"(parity)
-      : "memory");
-}
 }  // namespace ring
 
 #ifndef HAMR_RING_MINB
@@ -423,6 +392,7 @@ template <int D, int KT>
 __global__ void __launch_bounds__(KT, HAMR_RING_MINB * 128 / KT) k_flux_ring(Dev Dv, Fields s, int seg, int want_ctop) {
   static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   using namespace ring;
+  using namespace tma;
   constexpr int O = 1 - D;
   constexpr int e = (D + 1) % 3, f = (D + 2) % 3;
   constexpr int SLOTD = 8 * KT + NREC_F;   // doubles per ring slot: 7 variables, the face field, the face record

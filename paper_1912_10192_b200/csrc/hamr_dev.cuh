@@ -289,6 +289,41 @@ __device__ __forceinline__ double warp_max(double v) {
   return v;
 }
 
+// ---- bulk asynchronous copies global -> shared (TMA) with mbarrier completion --------------------------------
+namespace tma {
+__device__ __forceinline__ unsigned su32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(su32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect(unsigned long long* b, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(su32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(su32(dst)),
+               "l"(src), "r"(bytes), "r"(su32(b))
+               : "memory");
+}
+// one lane of a converged warp
+__device__ __forceinline__ bool elect_one() {
+  unsigned p;
+  asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}" : "=r"(p));
+  return p != 0;
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "HAMR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra HAMR_DONE;\n"
+      "bra HAMR_WAIT;\n"
+      "HAMR_DONE:\n"
+      "}" ::"r"(su32(b)),
+      "r"(parity)
+      : "memory");
+}
+}  // namespace tma
+
 // ---- C-15: phi-ghost slots of derefined rows are in GROUP units -------------------------------------------
 // x3 index inside the periodic neighbour that ghost slot k of an array whose row (or x2-face) has grouping mg
 // holds: ghost zone -g is group -g (the neighbour's zone n3 - g mg), ghost zone n3 - 1 + g is group g - 1 beyond the

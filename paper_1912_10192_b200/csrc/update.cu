@@ -34,10 +34,13 @@ __device__ __forceinline__ Fields pick_fields(const Fields& a, const Fields& b, 
 #define HAMR_UPD_MINB 6
 #endif
 #ifndef HAMR_UPD_MINB_PRED
-#define HAMR_UPD_MINB_PRED 7
+#define HAMR_UPD_MINB_PRED 5
 #endif
 #ifndef HAMR_UPD_RELOAD
 #define HAMR_UPD_RELOAD 1
+#endif
+#ifndef HAMR_UPD_TILE
+#define HAMR_UPD_TILE 1
 #endif
 template <bool SAME, bool BLK>  // SAME: predictor, source state == base state
 __global__ void __launch_bounds__(128, SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
@@ -173,6 +176,224 @@ __global__ void __launch_bounds__(128, SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB
   }
 }
 
+// ---- the same update on monolithic grids, staged through shared memory by bulk asynchronous copies (TMA) --------
+// A CTA owns TJ consecutive x2 rows over the whole x3 extent and marches along x1.  Every array with reuse between
+// zones (15 flux arrays: each value feeds two zones; 3 edge EMFs: eight uses; 3 base face fields: two uses) is brought
+// in as ONE contiguous chunk per plane (rows j0 .. j0 + TJ, whole x3 pitch: the k + 1 and j + 1 neighbours come with
+// it).  Arrays read at planes i and i + 1 (F^1, E_2, E_3, Bf^1) keep two planes (the march reuses plane i + 1 as the
+// next step's plane i), the others one.  A step first consumes everything staged (new faces, new B_c, flux
+// divergence), the CTA synchronises, one thread requests the next plane into the SAME buffers, and the long
+// dependent part (states, source, Newton inversion, floors) runs while those copies land.  Zone-centred arrays
+// without reuse (source / base state in, new state out) are read and written directly, requested at the top of the step.
+namespace tile {
+constexpr int TJ = 2;
+constexpr int NA = 8, NB = 13;   // arrays keeping two planes / one plane
+}
+
+template <bool SAME, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, double dtfac, int seg) {
+  using namespace tile;
+  using namespace tma;
+  extern __shared__ __align__(128) double tile_mem[];
+  const Lay& L = Dv.L;
+  const int AS = (TJ + 1) * L.p3;                  // doubles per staged array and plane
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(tile_mem + (2 * NA + NB) * AS);
+  const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+  const int wpr = (L.n[2] + 31) >> 5;              // warps per x3 row
+  const int jj = w / wpr, k = (w - jj * wpr) * 32 + lane;
+  const int j0 = blockIdx.x * TJ, j = j0 + jj;
+  const int i0 = blockIdx.y * seg, i1 = min(i0 + seg, L.n[0] + 1);
+  const bool live = jj < TJ && j <= L.n[1] && k < L.n[2];
+  const bool in1 = j < L.n[1];
+  const bool ks = Dv.metric == HAMR_METRIC_KERR_SCHILD;
+  const double dt = dtfac * Dv.scal[S_DT];
+  const double ix0 = 1.0 / Dv.dx[0], ix1 = 1.0 / Dv.dx[1], ix2 = 1.0 / Dv.dx[2];
+  // class A: F^1[0..4], Ee[1], Ee[2], Bf^1 ; class B: F^2[0..4], F^3[0..4], Ee[0], Bf^2, Bf^3
+  const double* srcA[NA] = {Dv.F[0][0], Dv.F[0][1], Dv.F[0][2], Dv.F[0][3], Dv.F[0][4], Dv.Ee[1], Dv.Ee[2], r.base.Bf[0]};
+  const double* srcB[NB] = {Dv.F[1][0], Dv.F[1][1], Dv.F[1][2], Dv.F[1][3], Dv.F[1][4], Dv.F[2][0], Dv.F[2][1],
+                            Dv.F[2][2], Dv.F[2][3], Dv.F[2][4], Dv.Ee[0], r.base.Bf[1], r.base.Bf[2]};
+  const unsigned bytes = (unsigned)(AS * sizeof(double));
+  const bool warp0 = t < 32;
+  // request plane pa of the class A arrays (into the buffer of its parity) and / or plane pb of the class B arrays
+  auto request = [&](int pa0, int pa1, int pb) {
+    if (warp0 && elect_one()) {
+      const int na = pa1 - pa0 + 1;
+      mbar_expect(full, (unsigned)((na * NA + (pb >= 0 ? NB : 0)) * bytes));
+      for (int pa = pa0; pa <= pa1; pa++) {
+        const int zc = (int)L.idx(pa, j0, 0);
+#pragma unroll
+        for (int a = 0; a < NA; a++) bulk_g2s(tile_mem + (2 * a + (pa & 1)) * AS, srcA[a] + zc, bytes, full);
+      }
+      if (pb >= 0) {
+        const int zc = (int)L.idx(pb, j0, 0);
+#pragma unroll
+        for (int b = 0; b < NB; b++) bulk_g2s(tile_mem + (2 * NA + b) * AS, srcB[b] + zc, bytes, full);
+      }
+    }
+  };
+  if (t == 0) {
+    mbar_init(full, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  request(i0, i0 + 1, i0);
+  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0;
+  const int sk = jj * L.p3 + k;                    // this thread's element inside a staged chunk
+  for (int i = i0; i < i1; i++) {
+    const bool in0 = i < L.n[0];
+    const bool zone = live && in0 && in1;
+    const int z = (int)L.idx(i, j, k);
+    // zone-centred inputs without reuse: requested now, used after the staged part
+    double Ps[8], Pb[8];
+    if (zone) {
+#pragma unroll
+      for (int c = 0; c < 5; c++) Ps[c] = __ldg(r.src.P[c] + z);
+#pragma unroll
+      for (int c = 0; c < 3; c++) Ps[5 + c] = __ldg(r.src.Bc[c] + z);
+      if (!SAME) {
+#pragma unroll
+        for (int c = 0; c < 5; c++) Pb[c] = __ldg(r.base.P[c] + z);
+#pragma unroll
+        for (int c = 0; c < 3; c++) Pb[5 + c] = __ldg(r.base.Bc[c] + z);
+      }
+    }
+    mbar_wait(full, (unsigned)((i - i0) & 1));
+    const double* A0 = tile_mem + (i & 1) * AS + sk;          // class A, plane i     (array a at + 2 a AS)
+    const double* A1 = tile_mem + ((i + 1) & 1) * AS + sk;    // class A, plane i + 1
+    const double* B0 = tile_mem + 2 * NA * AS + sk;           // class B, plane i     (array b at + b AS)
+    const int p3 = L.p3;
+    double Bn[3] = {0.0, 0.0, 0.0}, div[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    if (live) {
+      // C-10: Bf^d -= dt [ (E_f(e+) - E_f(e-))/dx^e - (E_e(f+) - E_e(f-))/dx^f ], (d,e,f) cyclic; the low faces of the
+      // zone are stored, the high faces are the neighbours' low faces recomputed from the same expression
+      const double* E1a = A0 + 10 * AS;  const double* E1b = A1 + 10 * AS;   // Ee[1] at planes i, i + 1
+      const double* E2a = A0 + 12 * AS;  const double* E2b = A1 + 12 * AS;   // Ee[2]
+      const double* E0 = B0 + 10 * AS;                                        // Ee[0]
+      const double* F0a = A0 + 14 * AS;  const double* F0b = A1 + 14 * AS;   // base Bf^1
+      const double* Bf1 = B0 + 11 * AS;  const double* Bf2 = B0 + 12 * AS;
+      const int Jg = j, n2g = L.n[1];
+      const double lo0 = F0a[0] - dt * ((E2a[p3] - E2a[0]) * ix1 - (E1a[1] - E1a[0]) * ix2);
+      const double hi0 = F0b[0] - dt * ((E2b[p3] - E2b[0]) * ix1 - (E1b[1] - E1b[0]) * ix2);
+      double lo1 = Bf1[0] - dt * ((E0[1] - E0[0]) * ix2 - (E2b[0] - E2a[0]) * ix0);
+      double hi1 = Bf1[p3] - dt * ((E0[p3 + 1] - E0[p3]) * ix2 - (E2b[p3] - E2a[p3]) * ix0);
+      const double lo2 = Bf2[0] - dt * ((E1b[0] - E1a[0]) * ix0 - (E0[p3] - E0[0]) * ix1);
+      const double hi2 = Bf2[1] - dt * ((E1b[1] - E1a[1]) * ix0 - (E0[p3 + 1] - E0[1]) * ix1);
+      if (ks && (Jg == 0 || Jg == n2g)) lo1 = 0.0;     // C-12: no field through the polar axis
+      if (ks && Jg + 1 == n2g) hi1 = 0.0;
+      if (in1) r.out.Bf[0][z] = lo0;
+      if (in0) r.out.Bf[1][z] = lo1;
+      if (in0 && in1) {
+        r.out.Bf[2][z] = lo2;
+        if (k == 0) {   // the x3-face at k = n3 of this row
+          const int q = L.n[2];
+          r.out.Bf[2][z + q] = Bf2[q] - dt * ((E1b[q] - E1a[q]) * ix0 - (E0[p3 + q] - E0[q]) * ix1);
+        }
+        Bn[0] = lo0 + hi0; Bn[1] = lo1 + hi1; Bn[2] = lo2 + hi2;   // times 1 / (2 sqrt(-g)) below
+#pragma unroll
+        for (int c = 0; c < 5; c++)
+          div[c] = (A1[2 * c * AS] - A0[2 * c * AS]) * ix0 + (B0[c * AS + p3] - B0[c * AS]) * ix1 +
+                   (B0[(5 + c) * AS + 1] - B0[(5 + c) * AS]) * ix2;
+      }
+    }
+    __syncthreads();   // everything staged for this plane has been read
+    if (i + 1 < i1) request(i + 2, i + 2, i + 1);
+    if (zone) {
+      const double* grec = Dv.gcA + (size_t)((NG + i) * L.e2 + NG + j) * NREC_C;
+      const CGeo G = load_cgeo(grec);
+      const double i2g = 0.5 * G.igdet;
+      Bn[0] *= i2g; Bn[1] *= i2g; Bn[2] *= i2g;
+      double U[5], S1, S2;
+      {
+        St Ss;
+        get_state(Ps, G, Ss);
+        if (SAME) prim_to_U5(Ps, Ss, G.gdet, Dv.gam, U);
+        source_12(Ps, Ss, G, Dv.gam, grec, S1, S2);   // C-12: on the stage's source state
+      }
+      if (!SAME) {
+        St Sb;
+        get_state(Pb, G, Sb);
+        prim_to_U5(Pb, Sb, G.gdet, Dv.gam, U);
+      }
+      // U_new = U_base - dt sum_d (F^d_+ - F^d_-)/dx^d + dt S
+#pragma unroll
+      for (int c = 0; c < 5; c++) {
+        const double sc = (c == 2) ? S1 : (c == 3 ? S2 : 0.0);
+        U[c] = U[c] - dt * div[c] + dt * sc;
+      }
+      double Pn[5];
+      if (con2prim(U, Bn, G, Dv.gam, Ps, Pn) != 0) {  // C-13: keep the source state's hydro primitives, count the failure
+        nfail = 1;
+#pragma unroll
+        for (int c = 0; c < 5; c++) Pn[c] = Ps[c];
+      }
+      floors_ceiling(G, __ldg(Dv.rho_fl + i + NG), __ldg(Dv.u_fl + i + NG), Dv.gamma_max, Pn, nrf, nuf, ngc);
+#pragma unroll
+      for (int c = 0; c < 5; c++) {
+        r.out.P[c][z] = Pn[c];
+        if (!(fabs(Pn[c]) <= 1.79e308)) bad = 1;
+      }
+#pragma unroll
+      for (int c = 0; c < 3; c++) r.out.Bc[c][z] = Bn[c];
+    }
+  }
+  // warp-aggregated event counters
+  const unsigned m_f = __ballot_sync(0xffffffffu, nfail), m_r = __ballot_sync(0xffffffffu, nrf),
+                 m_u = __ballot_sync(0xffffffffu, nuf), m_g = __ballot_sync(0xffffffffu, ngc),
+                 m_b = __ballot_sync(0xffffffffu, bad);
+  if (lane == 0) {
+    if (m_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)__popc(m_f));
+    if (m_r) atomicAdd(Dv.cnt + N_RHOFL, (unsigned long long)__popc(m_r));
+    if (m_u) atomicAdd(Dv.cnt + N_UFL, (unsigned long long)__popc(m_u));
+    if (m_g) atomicAdd(Dv.cnt + N_GCEIL, (unsigned long long)__popc(m_g));
+    if (m_b) atomicAdd(Dv.cnt + N_NONFINITE, (unsigned long long)__popc(m_b));
+  }
+}
+
+template <bool SAME, int NT>
+static void launch_tile_t(hamr_grid* g, const Dev& Dv, const Roles& r, double dtfac) {
+  using namespace tile;
+  const Lay& L = Dv.L;
+  const size_t smem = (size_t)(2 * NA + NB) * (TJ + 1) * L.p3 * sizeof(double) + 16;
+  static size_t attr_set = 0;
+  static int per_sm = 1;
+  if (attr_set != smem) {   // per function instantiation; smem depends on the x3 pitch only
+    cudaFuncSetAttribute(k_update_tile<SAME, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    int v = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_update_tile<SAME, NT>, NT, smem);
+    per_sm = v < 1 ? 1 : v;
+    attr_set = smem;
+  }
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int np = L.n[0] + 1, ntile = (L.n[1] + 1 + TJ - 1) / TJ;
+  const double slots = (double)sms * per_sm;
+  double best = -1.0;
+  int best_seg = np;
+  for (int nseg = 1; nseg <= np && nseg <= 64; nseg++) {
+    const int sg = (np + nseg - 1) / nseg;
+    if (sg < 8 && nseg > 1) break;
+    const int ns = (np + sg - 1) / sg;
+    const double blocks = (double)ntile * ns, waves = ceil(blocks / slots);
+    // wave fill x (planes / (planes + one exposed load latency per segment, about half a plane of work))
+    const double eff = blocks / (waves * slots) * ((double)np / ((double)ns * (sg + 0.5)));
+    if (eff > best) { best = eff; best_seg = sg; }
+  }
+  dim3 grid(ntile, (np + best_seg - 1) / best_seg);
+  k_update_tile<SAME, NT><<<grid, NT, smem, g->stream>>>(Dv, r, dtfac, best_seg);
+}
+
+// the tiled kernel serves monolithic grids without derefinement whose staged planes fit shared memory
+static int tile_threads(const Dev& Dv) {
+  using namespace tile;
+  if (Dv.B.nblk > 0 || Dv.mrow) return 0;
+  const int nt = 32 * ((Dv.L.n[2] + 31) / 32) * TJ;
+  const size_t smem = (size_t)(2 * NA + NB) * (TJ + 1) * Dv.L.p3 * sizeof(double) + 16;
+  if (nt > 512 || smem > 227 * 1024) return 0;
+  return nt <= 64 ? 64 : (nt <= 128 ? 128 : (nt <= 256 ? 256 : 512));
+}
+
 // ra / rb: the stage's roles in the buffer sets of blocks with cur == 0 / 2 (monolithic: rb unused)
 void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles& rb, double dtfac, bool same) {
   const Lay& L = Dv.L;
@@ -181,6 +402,15 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
   const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * L.n[2] * (blk ? Dv.B.nact : 1);
   const unsigned nb = (unsigned)((tot + 127) / 128);
   Launch l_(g, same ? K_UPDATE_P : K_UPDATE_C);
+#if HAMR_UPD_TILE
+  switch (tile_threads(Dv)) {
+    case 64: return same ? launch_tile_t<true, 64>(g, Dv, ra, dtfac) : launch_tile_t<false, 64>(g, Dv, ra, dtfac);
+    case 128: return same ? launch_tile_t<true, 128>(g, Dv, ra, dtfac) : launch_tile_t<false, 128>(g, Dv, ra, dtfac);
+    case 256: return same ? launch_tile_t<true, 256>(g, Dv, ra, dtfac) : launch_tile_t<false, 256>(g, Dv, ra, dtfac);
+    case 512: return same ? launch_tile_t<true, 512>(g, Dv, ra, dtfac) : launch_tile_t<false, 512>(g, Dv, ra, dtfac);
+    default: break;
+  }
+#endif
   if (same && !blk) k_update<true, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
   else if (same) k_update<true, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
   else if (!blk) k_update<false, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
