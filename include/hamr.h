@@ -49,9 +49,13 @@ typedef enum { HAMR_METRIC_MINKOWSKI = 0, HAMR_METRIC_KERR_SCHILD = 1 } hamr_met
  * rows beyond the pole then come from the block half a turn away). */
 typedef enum { HAMR_BC_PERIODIC = 0, HAMR_BC_OUTFLOW = 1, HAMR_BC_POLAR_REFLECT = 2, HAMR_BC_POLAR_TRANSMIT = 3 } hamr_bc_t;
 typedef enum { HAMR_RECON_PPM = 0, HAMR_RECON_PLM_MC = 1 } hamr_recon_t;
+/* Coordinate map of the internal coordinates ("any self-consistent coordinate system (and metric) can be
+ * chosen"): the Cartesian box (x^i linear) or x1 = ln r, x2 = theta, x3 = phi.  Two pairs are built: Minkowski on the
+ * Cartesian box and Kerr-Schild on the logarithmic spherical-polar map; HAMR_MAP_DEFAULT picks the metric's own map,
+ * any other pair is rejected with HAMR_EINVAL. */
+typedef enum { HAMR_MAP_DEFAULT = 0, HAMR_MAP_CARTESIAN = 1, HAMR_MAP_LOGR_SPHERICAL = 2 } hamr_map_t;
 
-/* Parameter block (plain data).  The coordinate map follows the metric: Minkowski = Cartesian box
- * (x^i linear), Kerr-Schild = (ln r, theta, phi). */
+/* Parameter block (plain data). */
 typedef struct {
   int metric;            /* hamr_metric_t                                                        */
   int recon;             /* hamr_recon_t (PPM; PLM+MC is the allowed alternative)   */
@@ -61,9 +65,11 @@ typedef struct {
   int n_deref;           /* number of phi-derefinement thresholds, 0 = none       */
   int deref_factor[4];   /* derefinement factor per threshold (see "phi-derefinement" below)            */
   int lat_max_level;     /* local adaptive time-stepping levels; 0 = global dt    */
-  int pad_;
+  int map;               /* hamr_map_t                                                           */
   double a;              /* black-hole spin (ignored for Minkowski)                              */
-  double xmin[3], xmax[3]; /* PHYSICAL extents: (r_in, r_out), (0, pi), (0, 2pi), or the box     */
+  double xmin[3], xmax[3]; /* PHYSICAL extents: (r_in, r_out), (0, pi), (0, 2pi), or the box.  On the spherical
+                            map x2 must span exactly (0, pi) with a polar boundary kind on both sides: the faces
+                            at theta = 0, pi are treated as the polar axis (no flux, no normal field, C-7 / C-9) */
   double gamma_ad;       /* adiabatic index, p = (gamma_ad - 1) u                                */
   double cour;           /* Courant factor C of dt_d = C dx^d / max ctop_d (PAPER.md:93 fn. 2)   */
   double rho_fl_coef, rho_fl_pow, u_fl_coef, u_fl_pow; /* floor = coef * r^pow (r = 1 Cartesian) */
@@ -164,32 +170,8 @@ int hamr_get_block_prims(hamr_grid* g, int b, double* const prims[8]);   /* 5 hy
 int hamr_set_all_blocks(hamr_grid* g, const double* const hydro[5], const double* const bface[3]);
 int hamr_get_all_blocks(hamr_grid* g, double* const prims[8]);
 int hamr_get_block_bface(hamr_grid* g, int b, double* const bface[3]);
-/* Test hook: prescribes the LAT level of every block (tau[hamr_num_blocks], clamped to
- * 0..lat_max_level, then lowered until neighbours differ by at most one); NULL restores the
- * Courant-based choice.  Takes effect at the next hamr_set_prims / coarse step.  The caller keeps tau. */
-int hamr_set_levels(hamr_grid* g, const int* tau);
-
-/* ---- diagnostics used by the parity tests (not part of the hot path) -------------------------- */
-/* Runs ghost fill + flux pass + CT EMFs on the current state (no update). */
-int hamr_debug_emf(hamr_grid* g);
-/* which 0..4: hydro flux F^d[c] of the last flux pass; 5, 6: the two face EMFs E_e, E_f with
- * (d, e, f) cyclic (C-8).  out: d-face array, extent n[d]+1 along d. */
-int hamr_get_face(hamr_grid* g, int d, int which, double* out);
-/* edge EMF E_f (extent n+1 along the two directions != f). */
-int hamr_get_edge(hamr_grid* g, int f, double* out);
-int hamr_get_ctop(hamr_grid* g, double ctop[3]); /* per-direction max signal speed of the last corrector pass */
-/* conserved totals sum_zones U[c] dV, c = 0..4, of the current state */
-int hamr_totals(hamr_grid* g, double tot[5]);
-/* Per-kernel device timers.  Between hamr_profile_begin and hamr_profile_end every kernel launch on
- * the grid's stream is bracketed by a CUDA event pair; _end synchronises and returns, per kernel
- * class c < HAMR_NKCLASS, the summed device time ms[c] and the number of launches count[c].
- * nclass must be >= HAMR_NKCLASS. */
-#define HAMR_NKCLASS 10
-int hamr_profile_begin(hamr_grid* g);
-int hamr_profile_end(hamr_grid* g, int nclass, double ms[], long long count[]);
-const char* hamr_profile_class_name(int c); /* "" if out of range */
-/* kernel launches issued on this grid's stream since creation */
-int hamr_launch_count(const hamr_grid* g, long long* n);
+/* Test hooks and diagnostics (flux / EMF getters, per-kernel timers, geometry tables, zone-level physics
+ * entry points, the FP64 peak measurement) are declared in hamr_debug.h. */
 
 #ifdef __cplusplus
 }

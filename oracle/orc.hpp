@@ -34,7 +34,7 @@ struct Params {
   int32_t n_deref;       // number of phi-derefinement thresholds (C-15)
   int32_t deref_factor[4];
   int32_t lat_max_level; // C-17; 0 -> global dt
-  int32_t pad_;
+  int32_t map;
   double a;              // spin
   double xmin[3], xmax[3];   // PHYSICAL extents ((r_in,r_out),(0,pi),(0,2pi)) or box
   double gamma_ad, cour;

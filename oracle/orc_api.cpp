@@ -443,6 +443,12 @@ int orc_con2prim(const double* U5, const double* Bc, const Geom* G, double gam, 
                  double* Pout, int* iters) {
   return con2prim(U5, Bc, *G, gam, Pguess, Pout, iters);
 }
+// floors and Lorentz-factor ceiling of C-13 on one zone at radius r; counts3: rho-floor, u-floor, ceiling hits
+void orc_floors(const Params* par, const Geom* G, double r, double* P5, long long* counts3) {
+  Stats st = {0, 0, 0, 0};
+  floors_and_ceiling(*par, *G, r, P5, st);
+  counts3[0] = st.rho_floor; counts3[1] = st.u_floor; counts3[2] = st.gam_ceil;
+}
 void orc_ppm_zone(const double* a5, double* aL, double* aR) { ppm_zone(a5, *aL, *aR); }
 void orc_plm_zone(const double* a3, double* aL, double* aR) { plm_zone(a3, *aL, *aR); }
 void orc_hll(const double* UL, const double* UR, const double* FL, const double* FR, double cmin,
@@ -490,9 +496,6 @@ void orc_get_ctop(void* h, double* c3) {
 }
 
 // failure-code histogram of con2prim since creation (debug): codes 1..4
-extern "C" void orc_get_fail_hist(long long h4[4]) {
-  for (int c = 0; c < 4; c++) h4[c] = orc::g_fail_hist[c];
-}
 
 // number of OpenMP threads the oracle's loops use (reported by bench.py's cpu_baseline leg)
 #include <omp.h>

@@ -6,7 +6,6 @@
 
 namespace orc {
 
-long long g_fail_hist[4] = {0, 0, 0, 0};  // debug: con2prim failure codes seen
 
 static const int CYC[3][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}};  // (d, e, f) cyclic
 
@@ -548,10 +547,6 @@ void update(const Params& par, Block& b, const Fields& src, const Fields& base, 
         const double Bn[3] = {out.Bc[0][z], out.Bc[1][z], out.Bc[2][z]};
         double Pn[5];
         int rc = con2prim(U, Bn, G, par.gamma_ad, Ps, Pn, nullptr);
-        if (rc != 0) {
-#pragma omp atomic
-          g_fail_hist[rc - 1]++;
-        }
         if (rc != 0) {  // C-13: keep the source state's hydro primitives, count the failure
           nfail++;
           for (int c = 0; c < 5; c++) Pn[c] = Ps[c];

@@ -60,7 +60,6 @@ struct Block {
   double xf(int d, int i) const { return x0[d] + (double)(I0[d] + i) * dx[d]; }
 };
 
-extern long long g_fail_hist[4];
 struct Stats { long long c2p_fail, rho_floor, u_floor, gam_ceil; };
 
 struct Grid {

@@ -11,8 +11,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libhamr.so")
-SOURCES = ["geom.cu", "bc.cu", "flux.cu", "ct.cu", "update.cu", "misc.cu", "blocks.cu", "deref.cu", "api.cu"]
-HEADERS = ["hamr_dev.cuh", "hamr_host.h", os.path.join("..", "..", "include", "hamr.h")]
+SOURCES = ["geom.cu", "bc.cu", "flux.cu", "ct.cu", "update.cu", "misc.cu", "blocks.cu", "deref.cu", "api.cu", "debug.cu"]
+HEADERS = ["hamr_dev.cuh", "hamr_host.h", os.path.join("..", "..", "include", "hamr.h"),
+           os.path.join("..", "..", "include", "hamr_debug.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -33,7 +34,6 @@ def _stale(target: str, deps) -> bool:
 
 def build_lib(verbose: bool = False, force: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
-    extra = os.environ.get("HAMR_EXTRA_NVCC_FLAGS", "").split()   # tuning experiments (-DHAMR_...=n)
     nvcc = _nvcc()
     hdrs = [os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
     jobs = []
@@ -45,7 +45,7 @@ def build_lib(verbose: bool = False, force: bool = False) -> str:
 
     def compile_one(job):
         src, obj = job
-        r = subprocess.run([nvcc] + NVCC_FLAGS + extra + ["-c", src, "-o", obj], capture_output=True, text=True)
+        r = subprocess.run([nvcc] + NVCC_FLAGS + ["-c", src, "-o", obj], capture_output=True, text=True)
         log = r.stdout + r.stderr
         with open(obj + ".log", "w") as f:
             f.write(log)

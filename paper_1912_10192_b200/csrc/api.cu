@@ -8,6 +8,7 @@
 #include <cstring>
 #include <new>
 #include <vector>
+#include "../../include/hamr_debug.h"
 #include "hamr_host.h"
 
 using namespace hamr;
@@ -46,6 +47,22 @@ bool params_ok(const hamr_params& p, std::string& why) {
     }
   }
   if (p.metric != HAMR_METRIC_MINKOWSKI && p.metric != HAMR_METRIC_KERR_SCHILD) { why = "bad metric"; return false; }
+  if (p.map != HAMR_MAP_DEFAULT &&
+      p.map != (p.metric == HAMR_METRIC_KERR_SCHILD ? HAMR_MAP_LOGR_SPHERICAL : HAMR_MAP_CARTESIAN)) {
+    why = "coordinate map and metric do not go together (Minkowski: Cartesian, Kerr-Schild: log-r spherical)";
+    return false;
+  }
+  if (p.metric == HAMR_METRIC_KERR_SCHILD) {
+    // the x2-faces J = 0 and J = N2 are treated as the polar axis (no flux, no normal field, pole-edge EMFs 0):
+    // x2 must span exactly (0, pi) with a polar boundary on both sides
+    const double pi = 3.14159265358979323846;
+    const bool polar_lo = p.bc_lo[1] == HAMR_BC_POLAR_REFLECT || p.bc_lo[1] == HAMR_BC_POLAR_TRANSMIT;
+    const bool polar_hi = p.bc_hi[1] == HAMR_BC_POLAR_REFLECT || p.bc_hi[1] == HAMR_BC_POLAR_TRANSMIT;
+    if (std::fabs(p.xmin[1]) > 1e-12 || std::fabs(p.xmax[1] - pi) > 1e-12 * pi || !polar_lo || !polar_hi) {
+      why = "the spherical map needs x2 = (0, pi) with a polar boundary kind on both sides";
+      return false;
+    }
+  }
   if (p.recon != HAMR_RECON_PPM && p.recon != HAMR_RECON_PLM_MC) { why = "bad recon"; return false; }
   if (p.metric == HAMR_METRIC_KERR_SCHILD && !(p.xmin[0] > 0.0)) { why = "r_in <= 0"; return false; }
   if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0) || !(p.gamma_max > 1.0)) { why = "gamma_ad / cour / gamma_max"; return false; }
@@ -494,8 +511,11 @@ int hamr_get_prims_dev(hamr_grid* g, double* const prims[8]) {
   if (!g || !prims) return HAMR_EINVAL;
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
   const Fields& sn = g->s[g->isn];
-  for (int c = 0; c < 8; c++)
-    if (prims[c]) get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], prims[c], -1, true, 0, c);
+  for (int c = 0; c < 8; c++) {
+    if (!prims[c]) continue;
+    const int rc = get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], prims[c], -1, true, 0, c);
+    if (rc != HAMR_OK) return rc;
+  }
   CK(cudaGetLastError());
   return HAMR_OK;
 }

@@ -1,0 +1,187 @@
+// debug.cu — entry points of include/hamr_debug.h that are not part of the step driver: the geometry tables, the
+// per-zone physics on caller-supplied states, and the FP64 pipe measurement.  Product code; the kernels here call
+// the same device functions (hamr_dev.cuh) as the hot kernels.
+#include <vector>
+#include "../../include/hamr_debug.h"
+#include "hamr_host.h"
+
+using namespace hamr;
+
+namespace {
+
+// one thread per state: what (0 prim -> U, 1 U -> prim, 2 floors / ceiling) on the centre record of entry q[s]
+__global__ void k_zone_physics(Dev Dv, int what, int n, const int* __restrict__ q, const int* __restrict__ ti,
+                               const double* __restrict__ in, const double* __restrict__ in2,
+                               const double* __restrict__ in3, double* __restrict__ out, int* __restrict__ iout) {
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const CGeo G = load_cgeo(Dv.gcA + (size_t)q[s] * NREC_C);
+  if (what == 0) {
+    double P[8], U[5];
+    for (int c = 0; c < 8; c++) P[c] = in[(size_t)s * 8 + c];
+    St S;
+    get_state(P, G, S);
+    prim_to_U5(P, S, G.gdet, Dv.gam, U);
+    for (int c = 0; c < 5; c++) out[(size_t)s * 5 + c] = U[c];
+  } else if (what == 1) {
+    double U[5], Bc[3], Pg[5], Pn[5];
+    for (int c = 0; c < 5; c++) { U[c] = in[(size_t)s * 5 + c]; Pg[c] = in3[(size_t)s * 5 + c]; }
+    for (int c = 0; c < 3; c++) Bc[c] = in2[(size_t)s * 3 + c];
+    const int rc = con2prim(U, Bc, G, Dv.gam, Pg, Pn);
+    for (int c = 0; c < 5; c++) out[(size_t)s * 5 + c] = rc == 0 ? Pn[c] : Pg[c];   // C-13: a failed zone keeps its guess
+    iout[s] = rc;
+  } else {
+    double P[5];
+    for (int c = 0; c < 5; c++) P[c] = out[(size_t)s * 5 + c];
+    int nrf = 0, nuf = 0, ngc = 0;
+    floors_ceiling(G, Dv.rho_fl[ti[s]], Dv.u_fl[ti[s]], Dv.gamma_max, P, nrf, nuf, ngc);
+    for (int c = 0; c < 5; c++) out[(size_t)s * 5 + c] = P[c];
+    iout[s] = nrf | (nuf << 1) | (ngc << 2);
+  }
+}
+
+// 8 independent chains per thread; mix 0: DFMA only; mix 1: DFMA, DADD, DMUL in turn
+template <int MIX>
+__global__ void __launch_bounds__(256) k_fp64_chains(int iters, double seed, double* sink) {
+  double a[8];
+#pragma unroll
+  for (int c = 0; c < 8; c++) a[c] = seed + 1e-3 * (threadIdx.x + 8 * c);
+  const double m = 1.0 - 1e-9, b = 1e-9;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int r = 0; r < 4; r++) {   // 4 rounds of 3 instructions on each of the 8 chains: 96 per iteration
+#pragma unroll
+      for (int c = 0; c < 8; c++) {
+        if (MIX == 0) {
+          a[c] = fma(a[c], m, b);
+          a[c] = fma(a[c], m, b);
+          a[c] = fma(a[c], m, b);
+        } else {
+          a[c] = fma(a[c], m, b);
+          a[c] = a[c] + b;
+          a[c] = a[c] * m;
+        }
+      }
+    }
+  }
+  double t = 0.0;
+#pragma unroll
+  for (int c = 0; c < 8; c++) t += a[c];
+  if (t == 123.456) sink[0] = t;   // never true: keeps the chains alive
+}
+
+int zone_call(hamr_grid* g, int what, int n, const int* ti, const int* tj, const double* in, int nin,
+              const double* in2, int nin2, const double* in3, int nin3, double* out, bool out_is_input, int* iout) {
+  if (!g || n < 0 || !ti || !tj || !out) return HAMR_EINVAL;
+  if (n == 0) return HAMR_OK;
+  const Lay& L = g->D.L;
+  const int te1 = (int)(L.n2d / g->D.B.ge2), te2 = g->D.B.ge2;
+  std::vector<int> q(n);
+  for (int s = 0; s < n; s++) {
+    if (ti[s] < 0 || ti[s] >= te1 || tj[s] < 0 || tj[s] >= te2) return HAMR_EINVAL;
+    q[s] = ti[s] * te2 + tj[s];
+  }
+  double *d_in = nullptr, *d_in2 = nullptr, *d_in3 = nullptr, *d_out = nullptr;
+  int *d_q = nullptr, *d_ti = nullptr, *d_i = nullptr;
+  cudaError_t e = cudaSuccess;
+  auto up = [&](const void* h, size_t bytes, void** d) {
+    if (e != cudaSuccess || !h || bytes == 0) return;
+    e = cudaMalloc(d, bytes);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(*d, h, bytes, cudaMemcpyHostToDevice, g->stream);
+  };
+  up(q.data(), n * sizeof(int), (void**)&d_q);
+  up(ti, n * sizeof(int), (void**)&d_ti);
+  up(in, (size_t)n * nin * 8, (void**)&d_in);
+  up(in2, (size_t)n * nin2 * 8, (void**)&d_in2);
+  up(in3, (size_t)n * nin3 * 8, (void**)&d_in3);
+  if (e == cudaSuccess) {
+    if (out_is_input) up(out, (size_t)n * 5 * 8, (void**)&d_out);
+    else e = cudaMalloc((void**)&d_out, (size_t)n * 5 * 8);
+  }
+  if (e == cudaSuccess) e = cudaMalloc((void**)&d_i, n * sizeof(int));
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_i, 0, n * sizeof(int), g->stream);
+  if (e == cudaSuccess) {
+    g->launches++;
+    k_zone_physics<<<(n + 127) / 128, 128, 0, g->stream>>>(g->D, what, n, d_q, d_ti, d_in, d_in2, d_in3, d_out, d_i);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, (size_t)n * 5 * 8, cudaMemcpyDeviceToHost, g->stream);
+  if (e == cudaSuccess && iout) e = cudaMemcpyAsync(iout, d_i, n * sizeof(int), cudaMemcpyDeviceToHost, g->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
+  cudaFree(d_q); cudaFree(d_ti); cudaFree(d_in); cudaFree(d_in2); cudaFree(d_in3); cudaFree(d_out); cudaFree(d_i);
+  if (e != cudaSuccess) { g->err = cudaGetErrorString(e); return HAMR_ECUDA; }
+  return HAMR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int hamr_debug_geometry(hamr_grid* g, int kind, int level, double* out, int* e1, int* e2, int* nrec) {
+  if (!g || kind < 0 || kind > 3 || level < 0) return HAMR_EINVAL;
+  const Lay& L = g->D.L;
+  const int te2 = g->D.B.ge2, te1 = (int)(L.n2d / te2);
+  const int nlev = (g->bh.on && g->bh.refined) ? 2 : 1;
+  if (level >= nlev) return HAMR_EINVAL;
+  const int nr = kind == 0 ? NREC_C : NREC_F;
+  if (e1) *e1 = te1;
+  if (e2) *e2 = te2;
+  if (nrec) *nrec = nr;
+  if (!out) return HAMR_OK;
+  const double* tab = kind == 0 ? g->D.gcA : (kind == 1 ? g->D.gf1A : (kind == 2 ? g->D.gf2A : g->D.gf3A));
+  tab += (size_t)level * g->D.B.tlevA;
+  cudaError_t e = cudaMemcpyAsync(out, tab, (size_t)L.n2d * nr * sizeof(double), cudaMemcpyDeviceToHost, g->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
+  if (e != cudaSuccess) { g->err = cudaGetErrorString(e); return HAMR_ECUDA; }
+  return HAMR_OK;
+}
+
+int hamr_debug_prim2cons(hamr_grid* g, int n, const int* ti, const int* tj, const double* prims, double* U) {
+  if (!prims) return HAMR_EINVAL;
+  return zone_call(g, 0, n, ti, tj, prims, 8, nullptr, 0, nullptr, 0, U, false, nullptr);
+}
+
+int hamr_debug_con2prim(hamr_grid* g, int n, const int* ti, const int* tj, const double* U, const double* Bc,
+                        const double* guess, double* out, int* rc) {
+  if (!U || !Bc || !guess || !rc) return HAMR_EINVAL;
+  return zone_call(g, 1, n, ti, tj, U, 5, Bc, 3, guess, 5, out, false, rc);
+}
+
+int hamr_debug_floors(hamr_grid* g, int n, const int* ti, const int* tj, double* P, int* flags) {
+  if (!flags) return HAMR_EINVAL;
+  return zone_call(g, 2, n, ti, tj, nullptr, 0, nullptr, 0, nullptr, 0, P, true, flags);
+}
+
+int hamr_bench_fp64(void* cuda_stream, int mix, int iters, double* seconds, double* thread_instructions) {
+  if (!seconds || !thread_instructions || iters < 1 || (mix != 0 && mix != 1)) return HAMR_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return HAMR_ECUDA;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return HAMR_ECUDA;
+  double* sink = nullptr;
+  if (cudaMalloc((void**)&sink, 8) != cudaSuccess) return HAMR_ENOMEM;
+  cudaEvent_t a, b;
+  cudaEventCreate(&a);
+  cudaEventCreate(&b);
+  const int blocks = sms * 8, threads = 256;   // 64 warps per SM: every scheduler has 16 warps of 8 chains
+  auto run = [&](int it) {
+    if (mix == 0) k_fp64_chains<0><<<blocks, threads, 0, st>>>(it, 1.0, sink);
+    else k_fp64_chains<1><<<blocks, threads, 0, st>>>(it, 1.0, sink);
+  };
+  run(iters / 10 + 1);   // warm-up
+  cudaEventRecord(a, st);
+  run(iters);
+  cudaEventRecord(b, st);
+  cudaError_t e = cudaEventSynchronize(b);
+  float ms = 0.f;
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  cudaFree(sink);
+  if (e != cudaSuccess) return HAMR_ECUDA;
+  *seconds = 1e-3 * ms;
+  *thread_instructions = 96.0 * iters * (double)blocks * threads;
+  return HAMR_OK;
+}
+
+}  // extern "C"

@@ -333,11 +333,13 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
       }
       double Pn[5];
       if (con2prim(U, Bn, G, Dv.gam, Ps, Pn) != 0) {  // C-13: keep the source state's hydro primitives, count the failure
-        nfail = 1;
+        nfail++;
 #pragma unroll
         for (int c = 0; c < 5; c++) Pn[c] = Ps[c];
       }
-      floors_ceiling(G, __ldg(Dv.rho_fl + i + NG), __ldg(Dv.u_fl + i + NG), Dv.gamma_max, Pn, nrf, nuf, ngc);
+      int frf = 0, fuf = 0, fgc = 0;
+      floors_ceiling(G, __ldg(Dv.rho_fl + i + NG), __ldg(Dv.u_fl + i + NG), Dv.gamma_max, Pn, frf, fuf, fgc);
+      nrf += frf; nuf += fuf; ngc += fgc;
 #pragma unroll
       for (int c = 0; c < 5; c++) {
         r.out.P[c][z] = Pn[c];
@@ -347,16 +349,16 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
       for (int c = 0; c < 3; c++) r.out.Bc[c][z] = Bn[c];
     }
   }
-  // warp-aggregated event counters
-  const unsigned m_f = __ballot_sync(0xffffffffu, nfail), m_r = __ballot_sync(0xffffffffu, nrf),
-                 m_u = __ballot_sync(0xffffffffu, nuf), m_g = __ballot_sync(0xffffffffu, ngc),
-                 m_b = __ballot_sync(0xffffffffu, bad);
+  // warp-aggregated event counters (a thread has seen many zones: sums, not flags)
+  const int s_f = __reduce_add_sync(0xffffffffu, nfail), s_r = __reduce_add_sync(0xffffffffu, nrf),
+            s_u = __reduce_add_sync(0xffffffffu, nuf), s_g = __reduce_add_sync(0xffffffffu, ngc),
+            s_b = __reduce_add_sync(0xffffffffu, bad);
   if (lane == 0) {
-    if (m_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)__popc(m_f));
-    if (m_r) atomicAdd(Dv.cnt + N_RHOFL, (unsigned long long)__popc(m_r));
-    if (m_u) atomicAdd(Dv.cnt + N_UFL, (unsigned long long)__popc(m_u));
-    if (m_g) atomicAdd(Dv.cnt + N_GCEIL, (unsigned long long)__popc(m_g));
-    if (m_b) atomicAdd(Dv.cnt + N_NONFINITE, (unsigned long long)__popc(m_b));
+    if (s_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)s_f);
+    if (s_r) atomicAdd(Dv.cnt + N_RHOFL, (unsigned long long)s_r);
+    if (s_u) atomicAdd(Dv.cnt + N_UFL, (unsigned long long)s_u);
+    if (s_g) atomicAdd(Dv.cnt + N_GCEIL, (unsigned long long)s_g);
+    if (s_b) atomicAdd(Dv.cnt + N_NONFINITE, (unsigned long long)s_b);
   }
 }
 

@@ -1,4 +1,4 @@
-"""Thin ctypes binding of libhamr.so (include/hamr.h).  Argument marshalling only: every step of the
+"""Thin ctypes binding of libhamr.so (include/hamr.h, include/hamr_debug.h).  Argument marshalling only: every step of the
 hot path runs in the CUDA kernels behind the C-ABI.  There is no CPU fallback: if the library is
 missing or fails to load, importing the binding's entry points raises.
 
@@ -29,10 +29,13 @@ SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "h
            "hamr_set_prims", "hamr_set_prims_dev", "hamr_step", "hamr_step_async", "hamr_sync",
            "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
            "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
-           "hamr_set_levels", "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
-           "hamr_get_block_bface", "hamr_set_all_blocks", "hamr_get_all_blocks",
-           "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
-           "hamr_profile_begin", "hamr_profile_end", "hamr_profile_class_name", "hamr_launch_count"]
+           "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
+           "hamr_get_block_bface", "hamr_set_all_blocks", "hamr_get_all_blocks"]
+# ... and include/hamr_debug.h (test hooks and diagnostics)
+DEBUG_SYMBOLS = ["hamr_set_levels", "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
+                 "hamr_profile_begin", "hamr_profile_end", "hamr_profile_class_name", "hamr_launch_count",
+                 "hamr_debug_geometry", "hamr_debug_prim2cons", "hamr_debug_con2prim", "hamr_debug_floors",
+                 "hamr_bench_fp64"]
 NKCLASS = 10
 
 
@@ -47,7 +50,7 @@ class Params(C.Structure):
     _fields_ = [("metric", C.c_int), ("recon", C.c_int), ("n", C.c_int * 3),
                 ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3), ("nb", C.c_int * 3),
                 ("n_deref", C.c_int), ("deref_factor", C.c_int * 4),
-                ("lat_max_level", C.c_int), ("pad_", C.c_int),
+                ("lat_max_level", C.c_int), ("map", C.c_int),
                 ("a", C.c_double), ("xmin", C.c_double * 3), ("xmax", C.c_double * 3),
                 ("gamma_ad", C.c_double), ("cour", C.c_double),
                 ("rho_fl_coef", C.c_double), ("rho_fl_pow", C.c_double),
@@ -101,7 +104,13 @@ def lib():
         L.hamr_profile_end.argtypes = [vp, C.c_int, c_double_p, C.POINTER(C.c_longlong)]
         L.hamr_profile_class_name.argtypes = [C.c_int]
         L.hamr_profile_class_name.restype = C.c_char_p
-        for s in SYMBOLS:
+        ip = C.POINTER(C.c_int)
+        L.hamr_debug_geometry.argtypes = [vp, C.c_int, C.c_int, c_double_p, ip, ip, ip]
+        L.hamr_debug_prim2cons.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p]
+        L.hamr_debug_con2prim.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p, c_double_p, c_double_p, ip]
+        L.hamr_debug_floors.argtypes = [vp, C.c_int, ip, ip, c_double_p, ip]
+        L.hamr_bench_fp64.argtypes = [vp, C.c_int, C.c_int, c_double_p, c_double_p]
+        for s in SYMBOLS + DEBUG_SYMBOLS:
             if s not in ("hamr_last_error", "hamr_profile_class_name"):
                 getattr(L, s).restype = C.c_int
         _LIB = L
@@ -120,6 +129,7 @@ def pack_params(p: dict) -> Params:
     for i, (t, f) in enumerate(zip(p["deref_theta_deg"], p["deref_factor"])):
         q.deref_theta_deg[i], q.deref_factor[i] = float(t), int(f)
     q.lat_max_level = int(p["lat_max_level"])
+    q.map = int(p.get("map", 0))
     q.a = float(p["a"])
     q.gamma_ad, q.cour = float(p["gamma_ad"]), float(p["cour"])
     q.rho_fl_coef, q.rho_fl_pow = float(p["rho_fl_coef"]), float(p["rho_fl_pow"])
@@ -357,7 +367,56 @@ class Grid:
         self._ck(self.L.hamr_profile_end(self.h, NKCLASS, ms, cnt))
         return {self.L.hamr_profile_class_name(c).decode(): (ms[c], cnt[c]) for c in range(NKCLASS)}
 
+    def geometry(self, kind, level=0):
+        """record table `kind` (0 centres, 1..3 faces) as an array (e1, e2, nrec); entry (ti, tj) = index (ti-3, tj-3)"""
+        e1, e2, nr = C.c_int(0), C.c_int(0), C.c_int(0)
+        self._ck(self.L.hamr_debug_geometry(self.h, kind, level, None, C.byref(e1), C.byref(e2), C.byref(nr)))
+        out = np.empty((e1.value, e2.value, nr.value))
+        self._ck(self.L.hamr_debug_geometry(self.h, kind, level, _dp(out), None, None, None))
+        return out
+
+    @staticmethod
+    def _ij(ti, tj):
+        a, b = np.ascontiguousarray(ti, dtype=np.int32), np.ascontiguousarray(tj, dtype=np.int32)
+        ip = C.POINTER(C.c_int)
+        return a, b, a.ctypes.data_as(ip), b.ctypes.data_as(ip)
+
+    def prim2cons(self, ti, tj, prims):
+        """prims (n, 8) at table entries (ti, tj) -> densitised hydro rows U (n, 5)"""
+        P = _arr(prims)
+        a, b, pa, pb = self._ij(ti, tj)
+        U = np.empty((len(a), 5))
+        self._ck(self.L.hamr_debug_prim2cons(self.h, len(a), pa, pb, _dp(P), _dp(U)))
+        return U
+
+    def con2prim(self, ti, tj, U, Bc, guess):
+        """U (n, 5), Bc (n, 3), guess (n, 5) -> hydro primitives (n, 5), rc (n)"""
+        U, Bc, gs = _arr(U), _arr(Bc), _arr(guess)
+        a, b, pa, pb = self._ij(ti, tj)
+        out = np.empty((len(a), 5))
+        rc = np.zeros(len(a), dtype=np.int32)
+        self._ck(self.L.hamr_debug_con2prim(self.h, len(a), pa, pb, _dp(U), _dp(Bc), _dp(gs), _dp(out),
+                                            rc.ctypes.data_as(C.POINTER(C.c_int))))
+        return out, rc
+
+    def floors(self, ti, tj, P):
+        """floors and ceiling on P (n, 5) -> new P, flags (bit 0 rho floor, 1 u floor, 2 ceiling)"""
+        Q = _arr(P).copy()
+        a, b, pa, pb = self._ij(ti, tj)
+        fl = np.zeros(len(a), dtype=np.int32)
+        self._ck(self.L.hamr_debug_floors(self.h, len(a), pa, pb, _dp(Q), fl.ctypes.data_as(C.POINTER(C.c_int))))
+        return Q, fl
+
     def launch_count(self):
         n = C.c_longlong(0)
         self._ck(self.L.hamr_launch_count(self.h, C.byref(n)))
         return n.value
+
+
+def bench_fp64(mix=0, iters=20000, stream=None):
+    """hamr_bench_fp64: (seconds, thread-level FP64 instructions) of the timed launch on the current device"""
+    sec, ins = C.c_double(0), C.c_double(0)
+    rc = lib().hamr_bench_fp64(C.c_void_p(stream), int(mix), int(iters), C.byref(sec), C.byref(ins))
+    if rc != OK:
+        raise HamrError(rc, "hamr_bench_fp64")
+    return sec.value, ins.value

@@ -18,7 +18,7 @@ class Params(C.Structure):
     _fields_ = [("metric", C.c_int32), ("recon", C.c_int32), ("n", C.c_int32 * 3),
                 ("bc_lo", C.c_int32 * 3), ("bc_hi", C.c_int32 * 3), ("nb", C.c_int32 * 3),
                 ("n_deref", C.c_int32), ("deref_factor", C.c_int32 * 4),
-                ("lat_max_level", C.c_int32), ("pad_", C.c_int32),
+                ("lat_max_level", C.c_int32), ("map", C.c_int32),
                 ("a", C.c_double), ("xmin", C.c_double * 3), ("xmax", C.c_double * 3),
                 ("gamma_ad", C.c_double), ("cour", C.c_double),
                 ("rho_fl_coef", C.c_double), ("rho_fl_pow", C.c_double),
@@ -72,6 +72,7 @@ def lib():
         L.orc_source.argtypes = [c_double_p, C.POINTER(Geom), c_double_p, C.c_double, c_double_p]
         L.orc_con2prim.argtypes = [c_double_p, c_double_p, C.POINTER(Geom), C.c_double, c_double_p,
                                    c_double_p, C.POINTER(C.c_int)]
+        L.orc_floors.argtypes = [C.POINTER(Params), C.POINTER(Geom), C.c_double, c_double_p, C.POINTER(C.c_longlong)]
         L.orc_ppm_zone.argtypes = [c_double_p] * 3
         L.orc_plm_zone.argtypes = [c_double_p] * 3
         L.orc_hll.argtypes = [c_double_p] * 4 + [C.c_double, C.c_double, c_double_p]
@@ -334,6 +335,15 @@ def con2prim(U5, Bc, G, gam, Pguess):
     it = C.c_int(0)
     rc = lib().orc_con2prim(_dp(U5), _dp(Bc), C.byref(G), gam, _dp(Pg), _dp(out), C.byref(it))
     return rc, out, it.value
+
+
+def floors(p, G, r, P5):
+    """floors and Lorentz-factor ceiling (C-13) on one zone: new P5, (rho-floor, u-floor, ceiling) hits"""
+    par = pack_params(p)
+    P = _arr(P5).copy()
+    c = (C.c_longlong * 3)()
+    lib().orc_floors(C.byref(par), C.byref(G), float(r), _dp(P), c)
+    return P, tuple(c[:])
 
 
 def ppm_zone(a5):

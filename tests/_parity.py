@@ -47,6 +47,16 @@ def parity_errors(p, ref, got):
     return out
 
 
+def raw_velocity_error(p, ref, got):
+    """the S-21 velocity norm WITHOUT the rounding floor S-21a (printed beside the bounded one so that what the floor
+    waives can be seen): max |d ut^i| sqrt(g_ii) / max(||ut||, 1e-3 max ||ut||)"""
+    sg, nrm = centre_gcov_diag_and_norm(p, ref[2:5])
+    if nrm.max() == 0.0:
+        return float(max(np.max(np.abs(got[2 + i] - ref[2 + i])) for i in range(3)))
+    scale = np.maximum(nrm, 1e-3 * nrm.max())
+    return float(max(np.max(np.abs(got[2 + i] - ref[2 + i]) * sg[i] / scale) for i in range(3)))
+
+
 def rel_max(ref, got):
     s = np.abs(ref).max()
     return float(np.abs(got - ref).max() / (s if s > 0 else 1.0))

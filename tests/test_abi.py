@@ -9,8 +9,8 @@ from paper_1912_10192_b200 import build, hamr
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared():
-    txt = open(os.path.join(ROOT, "include", "hamr.h")).read()
+def _declared(header="hamr.h"):
+    txt = open(os.path.join(ROOT, "include", header)).read()
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
     return sorted(set(re.findall(r"\b(hamr_[a-z_0-9]+)\s*\(", txt)))
 
@@ -23,6 +23,12 @@ def test_library_builds_and_exports_every_declared_symbol():
     for s in names:
         assert hasattr(L, s), s
     assert sorted(hamr.SYMBOLS) == names
+    dbg = _declared("hamr_debug.h")
+    assert "hamr_debug_geometry" in dbg and "hamr_bench_fp64" in dbg
+    for s in dbg:
+        assert hasattr(L, s), s
+    assert sorted(hamr.DEBUG_SYMBOLS) == dbg
+    assert not set(dbg) & set(names)
 
 
 def test_binding_params_layout_matches_header_order():
@@ -49,4 +55,12 @@ def test_bad_arguments_are_rejected_without_a_gpu():
     assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.OK and n.value > 0
     par.n[0] = 0
     assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.EINVAL
+    # the spherical map needs x2 = (0, pi) with polar boundaries: a wedge or an outflow x2 is refused, as is a map
+    # that does not go with the metric
+    for change in (dict(xmin=(1.2, 0.1, 0.0)), dict(xmax=(50.0, 3.0, 2.0 * 3.141592653589793)),
+                   dict(bc_lo=(I.BC_OUTFLOW, I.BC_OUTFLOW, I.BC_PERIODIC)), dict(map=1)):
+        par = hamr.pack_params(dict(I.torus_params(), **change))
+        assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.EINVAL, change
+    par = hamr.pack_params(dict(I.torus_params(), map=2))
+    assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.OK
     assert L.hamr_step(None, 1, None, None) == hamr.EINVAL

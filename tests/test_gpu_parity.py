@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 from paper_1912_10192_b200 import inputs as I
-from tests._parity import parity_errors, rel_max
+from tests._parity import parity_errors, raw_velocity_error, rel_max
 
 pytestmark = pytest.mark.gpu
 
@@ -105,7 +105,12 @@ def test_parity_after_1_and_10_steps(H, orc, name):
     assert g.divb() <= TOL_DIVB and o.divb() <= TOL_DIVB
     sg, so = g.stats(), o.stats()
     assert sg[0] == 0 and so[0] == 0                 # parity runs must report zero inversion failures
-    print(name, "1 step", e1, "10 steps", e10, "floors gpu/orc", sg, so)
+    # failures and ceiling hits agree; the two floor counters are printed only: the atmosphere of the torus sits AT
+    # the floors, where a last-bit difference of the inversion decides whether a zone counts as a hit (the counters
+    # are compared exactly in tests/test_gpu_zone.py on states well clear of the thresholds)
+    assert sg[3] == so[3]
+    print(name, "1 step", e1, "10 steps", e10, "velocity error without the S-21a rounding floor (10 steps):",
+          raw_velocity_error(p, o.get_prims(), g.get_prims()), "event counters", sg)
 
 
 def test_divb_and_conservation_minkowski(H):
@@ -134,14 +139,14 @@ def test_edge_cases(H, orc):
     g.step(3)
     o.step(3)
     e = parity_errors(p, o.get_prims(), g.get_prims())
-    assert max(e.values()) <= 1e-9, e
+    assert max(e.values()) <= 3 * TOL_1, e           # 3 steps
     # smallest non-periodic extents
     q = I.torus_params(n=(3, 3, 3))
     hyd, bf = I.fm_torus(q, seed=7)
     g, o = _pair(H, orc, q, hyd, bf)
     g.step(2)
     o.step(2)
-    assert max(parity_errors(q, o.get_prims(), g.get_prims()).values()) <= 1e-9
+    assert max(parity_errors(q, o.get_prims(), g.get_prims()).values()) <= 2 * TOL_1   # 2 steps
     # call order and bad input
     g2 = H.Grid(q)
     with pytest.raises(H.HamrError) as ei:
@@ -193,10 +198,15 @@ def test_full_size_headline_config_one_step(H, orc):
     e1 = parity_errors(p, o.get_prims(), g.get_prims())
     print("cfg2 1 step", e1)
     assert max(e1.values()) <= TOL_1, e1
-    o.close()
     g.step(9)
-    assert g.divb() <= TOL_DIVB
-    assert g.stats()[0] == 0
+    o.step(9)                                        # ~12 s of oracle: north_star's 1e-7 after 10 steps at full size
+    e10 = parity_errors(p, o.get_prims(), g.get_prims())
+    print("cfg2 10 steps", e10, "velocity error without the S-21a rounding floor:",
+          raw_velocity_error(p, o.get_prims(), g.get_prims()))
+    assert max(e10.values()) <= TOL_10, e10
+    assert g.divb() <= TOL_DIVB and o.divb() <= TOL_DIVB
+    sg, so = g.stats(), o.stats()
+    assert sg[0] == so[0] == 0 and sg[3] == so[3]
 
 
 def _cold_gas_errors(p, ref, got):
@@ -228,3 +238,20 @@ def test_cfg3_tilted_disk_stand_in(H, orc):
     e = _cold_gas_errors(p, o.get_prims(), g.get_prims())
     assert max(e.values()) <= TOL_10, e
     assert g.divb() <= TOL_DIVB and g.stats()[0] == 0 and o.stats()[0] == 0
+
+
+def test_cfg3_full_size_one_step(H, orc):
+    """BASELINE cfg 3 at the size bench.py --workload cfg3 times (512x256x256, 33.5 M zones): every zone against the
+    oracle after one step (norm S-21b for the cold gas, as in the stand-in test above)."""
+    p = I.tilted_disk_params()
+    assert tuple(p["n"]) == (512, 256, 256)
+    hyd, bf = I.tilted_disk(p, seed=3)
+    g, o = _pair(H, orc, p, hyd, bf)
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt
+    g.step(1)
+    o.step(1)
+    e = _cold_gas_errors(p, o.get_prims(), g.get_prims())
+    print("cfg3 full size, 1 step", e)
+    assert max(e.values()) <= TOL_1, e
+    sg, so = g.stats(), o.stats()
+    assert g.divb() <= TOL_DIVB and sg[0] == so[0] == 0 and sg[3] == so[3]

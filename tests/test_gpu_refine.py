@@ -104,10 +104,10 @@ def test_refined_torus(H, orc, extra):
     o.step(1)
     fin = 2 ** extra.get("lat_max_level", 0)
     _check_blocks(p, infos, o, g, TOL_1 * fin)
-    if g.levels() == list(o.levels()):
-        g.step(3)
-        o.step(3)
-        _check_blocks(p, infos, o, g, TOL_10)
+    assert g.levels() == list(o.levels())   # never skip the continuation: a diverging level assignment is a failure
+    g.step(3)
+    o.step(3)
+    _check_blocks(p, infos, o, g, TOL_10)
 
 
 @pytest.mark.parametrize("pole", ["reflect", "transmit"])
@@ -133,6 +133,15 @@ def test_cfg4_full_size_one_coarse_step(H, orc, pole):
     to, _ = o.step(1)
     assert abs(tg - to) <= 1e-13 * to
     _check_blocks(p, infos, o, g, 4 * TOL_1)
+    if pole == "reflect":
+        # two more coarse steps (12 finest steps in all), the level assignment compared after every coarse step
+        for _ in range(2):
+            assert g.levels() == list(o.levels())
+            tg, _ = g.step(1)
+            to, _ = o.step(1)
+            assert abs(tg - to) <= 1e-13 * to
+        assert g.levels() == list(o.levels())
+        _check_blocks(p, infos, o, g, TOL_10)
 
 
 def test_all_blocks_calls_equal_block_by_block(H):
