@@ -138,22 +138,35 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-# algorithmic doubles per unit of each kernel class: (reads + writes) per face / zone
-ALG_DOUBLES = {"flux_x1": 16, "flux_x2": 16, "flux_x3": 16,   # 9 r (P5, 2 transverse Bc, Bf^d) + 7 w (F5, 2 EMFs)
-               # update: r src P5+Bc3 (+ base P5+Bc3 in the corrector), base Bf3, Ee3, F15; w P5, Bc3, Bf3
-               "update_predictor": 8 + 3 + 3 + 15 + 11, "update_corrector": 8 + 8 + 3 + 3 + 15 + 11,
-               "centre_emf": 6 + 3, "edge_emf": 6 + 3 + 3 + 3, "ghosts": 0, "dt": 0, "other": 0}
+# algorithmic doubles per unit of each kernel class: (reads, writes) per face / zone
+ALG_RW = {"flux_x1": (9, 7), "flux_x2": (9, 7), "flux_x3": (9, 7),   # r: P5, 2 transverse Bc, Bf^d; w: F5, 2 EMFs
+          # update: r src P5+Bc3 (+ base P5+Bc3 in the corrector), base Bf3, Ee3, F15; w P5, Bc3, Bf3
+          "update_predictor": (8 + 3 + 3 + 15, 11), "update_corrector": (8 + 8 + 3 + 3 + 15, 11),
+          "centre_emf": (6, 3), "edge_emf": (6 + 3 + 3, 3), "ghosts": (0, 0), "dt": (0, 0), "other": (0, 0)}
 
-
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel class from the round's
-# `ncu --set full` capture of this same command on cfg 2 (profiles/r1h_ncu_full_cfg2.md)
-NCU_TRAFFIC_SOURCE = "profiles/r1h_ncu_full_cfg2.md"
-NCU_TRAFFIC = {"flux_x1": 613177160, "flux_x2": 598131024, "flux_x3": 542374640, "centre_emf": 325253308, "edge_emf": 534960992, "update_predictor": 1414139888, "update_corrector": 1667606816, "ghosts": 140912088}
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# fp64 FLOPs the flux kernels execute per face (dadd + dmul + 2 dfma, thread instructions counted by the same ncu
-# capture, divided by the faces of the launch): x1 / x2 sweeps 598-599, x3 sweep 606
-FLUX_FLOP_PER_FACE = {"flux_x1": 599.2, "flux_x2": 598.0, "flux_x3": 605.8}
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel class and the FP64 thread
+# instructions (dadd + dmul + dfma) the flux kernels execute per face, from the round's `ncu --set full` capture of
+# this same command on cfg 2
+NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_full_cfg2.md"
+NCU_TRAFFIC = {"flux_x1": 535800000, "flux_x2": 521100000, "flux_x3": 538700000}
+FLUX_FP64_INST_PER_FACE = {"flux_x1": 335.0, "flux_x2": 335.0, "flux_x3": 341.0}
+FLUX_FMA_FRACTION = 1.0 / 3.0      # a third of those are DFMA (2 FLOP), the rest DADD / DMUL (1 FLOP)
+FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
 PAPER_V100_150CUBED = 0.85e8   # ~0.85e8 zone-cycles/s, 1 V100, one 150^3 block
+
+
+def alg_bytes(cls, n):
+    """algorithmic bytes of one launch of kernel class `cls` on a monolithic n1 x n2 x n3 grid.  The flux kernels
+    evaluate one row of faces per transverse zone row incl. one ghost row on either side (C-9 reads them); along a
+    periodic x3 the two ghost columns are stored twice, not computed: reads count the computed faces,
+    writes the stored ones."""
+    n1, n2, n3 = n
+    r, w = ALG_RW.get(cls, (0, 0))
+    if cls == "flux_x1":
+        return 8 * (n1 + 1) * (n2 + 2) * (r * n3 + w * (n3 + 2))
+    if cls == "flux_x2":
+        return 8 * (n1 + 2) * (n2 + 1) * (r * n3 + w * (n3 + 2))
+    return 8 * (r + w) * units_per_launch(cls, n)
 
 
 def units_per_launch(cls, n):
@@ -200,9 +213,11 @@ def oracle_set(o, p, gen):
     return int(np.prod(p["n"]))
 
 
-def cpu_oracle_time(p, gen, steps):
-    """times the oracle as it stands on the host cores: `steps` full steps of the workload"""
+def cpu_oracle_time(p, gen, steps, threads=0):
+    """times the oracle as it stands on the host cores: `steps` full steps of the workload (threads = 0: all cores)"""
     from tests import _orc
+    _orc.lib().orc_set_threads.argtypes = [__import__("ctypes").c_int]
+    _orc.lib().orc_set_threads(int(threads))
     o = _orc.OrcGrid(p)
     nz = oracle_set(o, p, gen)
     t0 = time.perf_counter()
@@ -210,6 +225,7 @@ def cpu_oracle_time(p, gen, steps):
     dt = time.perf_counter() - t0
     cores = int(_orc.lib().orc_omp_threads())
     o.close()
+    _orc.lib().orc_set_threads(0)
     nz = nz * 2 ** int(p["lat_max_level"])   # effective zone-cycles per (coarse) step
     return nz * steps / dt, dt, cores
 
@@ -250,6 +266,8 @@ def run_reference(args):
     if shrunk:
         sample = (f"{args.steps} oracle steps of the workload on {shrunk[0]}x{shrunk[1]}x{shrunk[2]} zones (x1 zone count reduced, "
                   f"same r range) so that the run ends within minutes")
+    if shrunk:   # the label names the grid that actually ran
+        desc = desc.replace("256x128x128", f"{shrunk[0]}x{shrunk[1]}x{shrunk[2]} (x1 zone count reduced from 256, same r range)")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -323,13 +341,15 @@ def main():
         torch.cuda.synchronize()
 
     # ---- device-resident throughput ---------------------------------------------------------------
+    # three passes under one clock sampler: (1) the headline, EXACTLY --steps steps with no instrumentation; (2) the
+    # same steps with a CUDA event pair around every launch, for the per-kernel shares only; (3) a sustained pass of
+    # >= 0.7 s so that the sampler (100 ms period) sees the load and the power cap, reported beside the headline
     for _ in range(args.warmup):
         g.step_async(1)
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
     l0 = g.launch_count()
-    g.profile_begin()                          # per-kernel CUDA event pairs on the launching stream
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
@@ -338,12 +358,35 @@ def main():
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
-    prof = g.profile_end()
-    clocks = sampler.stop()
     launches = g.launch_count() - l0
+    g.profile_begin()                          # per-kernel CUDA event pairs on the launching stream
+    for _ in range(args.steps):
+        g.step_async(1)
+    barrier()
+    prof = g.profile_end()
+    ms_prof = sum(v[0] for v in prof.values())
+    sus_steps = max(args.steps, int(0.7e3 / max(ms / args.steps, 1e-3)) + 1)
+    barrier()
+    ev0.record()
+    for _ in range(sus_steps):
+        g.step_async(1)
+    ev1.record()
+    barrier()
+    ms_sus = ev0.elapsed_time(ev1)
+    # FP64 pipe peak, measured: all-DFMA chains and the flux kernels' DFMA / DADD / DMUL blend
+    fp64 = None
+    if rank == 0:
+        sec0, ins0 = hamr.bench_fp64(0, 20000, torch.cuda.current_stream().cuda_stream)
+        sec1, ins1 = hamr.bench_fp64(1, 20000, torch.cuda.current_stream().cuda_stream)
+        fp64 = {"tflops_measured_dfma": 2.0 * ins0 / sec0 / 1e12, "ginstr_per_s_dfma": ins0 / sec0 / 1e9,
+                "ginstr_per_s_flux_mix": ins1 / sec1 / 1e9, "tflops_flux_mix": (4.0 / 3.0) * ins1 / sec1 / 1e12,
+                "tflops_derived": FP64_PEAK_TFLOPS_DERIVED,
+                "how": "hamr_bench_fp64: 8 independent chains per thread, 64 warps per SM, 96 x 20000 instructions per thread"}
+    clocks = sampler.stop()
     g.sync()
     # LAT: "effective" zone-cycles (zones x finest-level steps, the paper's convention)
     value, ms_max = replica_throughput(ms, nz * fin * args.steps, world, "cuda")
+    sustained, _ = replica_throughput(ms_sus, nz * fin * sus_steps, world, "cuda")
     performed = None
     if blocky:
         lv = np.array(g.levels())
@@ -402,40 +445,51 @@ def main():
     nb_ws = C.c_size_t(0)
     L.hamr_workspace_bytes(C.byref(g._par), C.byref(nb_ws))
     ws_gb = nb_ws.value / 1e9
-    # ---- roofline of the dominant kernel ------------------------------------------------------------
+    # ---- roofline -----------------------------------------------------------------------------------------------
+    # per kernel class from the instrumented pass; the object leads with the class that takes the largest share of the
+    # step (the three fused reconstruct + HLL kernels count as one class: same code, one per direction)
     hbm_peak, peak_src = peaks()
     kern = {k: {"ms_total": v[0], "launches": v[1], "ms_avg": v[0] / v[1] if v[1] else 0.0,
-                "share": v[0] / ms if ms else 0.0} for k, v in prof.items() if v[1]}
+                "share": v[0] / ms_prof if ms_prof else 0.0} for k, v in prof.items() if v[1]}
     for k, d in kern.items():
         # per-launch algorithmic bytes are defined for the monolithic launch shape only
-        by = 0 if blocky else ALG_DOUBLES.get(k, 0) * 8 * units_per_launch(k, n)
+        by = 0 if blocky else alg_bytes(k, n)
         d["alg_bytes"] = by
         d["gbs"] = by / (d["ms_avg"] * 1e-3) / 1e9 if d["ms_avg"] > 0 else 0.0
-    # the dominant kernel: the longest single launch (k_update, corrector variant, on cfg 2).  The three flux
-    # kernels together are half of the step and are bound by the FP64 pipe, not by HBM: "flux_alu" below
-    dom = max(kern, key=lambda k: kern[k]["ms_avg"])
-    flux = [k for k in ("flux_x1", "flux_x2", "flux_x3") if k in kern and not blocky]
+    classes = {"flux": [k for k in ("flux_x1", "flux_x2", "flux_x3") if k in kern],
+               "update": [k for k in ("update_predictor", "update_corrector") if k in kern],
+               "ct": [k for k in ("centre_emf", "edge_emf") if k in kern], "ghosts": [k for k in ("ghosts",) if k in kern]}
+    cshare = {c: sum(kern[k]["share"] for k in ks) for c, ks in classes.items() if ks}
+    dom = max(cshare, key=cshare.get)
+    dk = classes[dom]
+    dom_bytes = sum(kern[k]["alg_bytes"] * kern[k]["launches"] for k in dk)
+    dom_ms = sum(kern[k]["ms_total"] for k in dk)
+    dom_gbs = dom_bytes / (dom_ms * 1e-3) / 1e9 if dom_ms else 0.0
+    traffic = None
+    if args.workload == "cfg2" and all(k in NCU_TRAFFIC for k in dk):
+        traffic = sum(NCU_TRAFFIC[k] for k in dk)          # the class's launches of one stage, like `achieved`
     flux_alu = None
-    if flux:
-        fl = sum(FLUX_FLOP_PER_FACE[k] * units_per_launch(k, n) * kern[k]["launches"] for k in flux)
-        tf = fl / (sum(kern[k]["ms_total"] for k in flux) * 1e-3) / 1e12
-        flux_alu = {"bound": "alu", "kernels": "+".join(flux), "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                    "frac": tf / FP64_PEAK_TFLOPS, "share_of_step": sum(kern[k]["share"] for k in flux),
-                    "flop_per_face": FLUX_FLOP_PER_FACE, "flop_source": NCU_TRAFFIC_SOURCE,
-                    "note": "executed fp64 FLOPs (FMA = 2); the same capture shows the FP64 pipe issuing on 53-62 % of cycles "
-                            "(a third of its instructions are FMAs)"}
-    roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": hbm_peak, "unit": "GB/s",
-            "frac": kern[dom]["gbs"] / hbm_peak, "traffic": NCU_TRAFFIC.get(dom) if args.workload == "cfg2" else None,
-            "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": peak_src,
-            "fp64_pipe": {"peak_tflops_derived": FP64_PEAK_TFLOPS, "note": "148 SMs x 64 DFMA lanes x 2 x 1.965 GHz; "
-                          "per-kernel FP64 pipe utilisation from ncu is in profiles/ (DESIGN.md section 7)"},
-            "share_of_step": kern[dom]["share"], "flux_alu": flux_alu,
+    if classes["flux"] and not blocky and fp64:
+        ins = sum(FLUX_FP64_INST_PER_FACE[k] * units_per_launch(k, n) * kern[k]["launches"] for k in classes["flux"])
+        sec = sum(kern[k]["ms_total"] for k in classes["flux"]) * 1e-3
+        flux_alu = {"bound": "alu", "kernels": "+".join(classes["flux"]), "achieved": ins / sec / 1e9,
+                    "peak": fp64["ginstr_per_s_flux_mix"], "unit": "G thread-instructions/s (FP64 pipe)",
+                    "frac": ins / sec / 1e9 / fp64["ginstr_per_s_flux_mix"],
+                    "tflops": (1.0 + FLUX_FMA_FRACTION) * ins / sec / 1e12,
+                    "fp64_inst_per_face": FLUX_FP64_INST_PER_FACE, "inst_source": NCU_TRAFFIC_SOURCE,
+                    "note": "executed dadd + dmul + dfma thread instructions per face (ncu) x faces / CUDA-event time, "
+                            "against the MEASURED issue rate of the same instruction blend (hamr_bench_fp64 mix 1)"}
+    roof = {"bound": "hbm", "kernel": "+".join(dk), "achieved": dom_gbs, "peak": hbm_peak, "unit": "GB/s",
+            "frac": dom_gbs / hbm_peak, "traffic": traffic, "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": peak_src,
+            "share_of_step": cshare[dom], "class_shares": {c: round(v, 4) for c, v in cshare.items()},
+            "fp64": fp64, "flux_alu": flux_alu,
             "whole_step": {"alg_bytes_per_zone_cycle_floor": 440,
                            "frac_of_hbm_at_floor": 440.0 * value / world / 1e9 / hbm_peak,
                            "alg_bytes_per_zone_cycle_pipeline": sum(d["alg_bytes"] * d["launches"] for d in kern.values()) / (nz * fin * args.steps),
-                           "frac_of_hbm_pipeline": sum(d["alg_bytes"] * d["launches"] for d in kern.values()) / (ms * 1e-3) / 1e9 / hbm_peak},
+                           "frac_of_hbm_pipeline": sum(d["alg_bytes"] * d["launches"] for d in kern.values()) / args.steps / (ms / args.steps * 1e-3) / 1e9 / hbm_peak},
             "kernels": {k: {"ms_avg": round(d["ms_avg"], 4), "share": round(d["share"], 4),
-                            "gbs": round(d["gbs"], 1), "launches": d["launches"]} for k, d in kern.items()}}
+                            "gbs": round(d["gbs"], 1), "frac_of_hbm": round(d["gbs"] / hbm_peak, 4),
+                            "launches": d["launches"]} for k, d in kern.items()}}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -444,6 +498,13 @@ def main():
         v, secs, cores = cpu_oracle_time(p, gen, steps_cpu)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"{steps_cpu} full {'coarse ' if fin > 1 else ''}steps of the same workload, all {nz} zones ({secs:.1f} s)"}
+        if args.workload == "cfg2":
+            # the oracle on ONE core as well, on the same torus at 64 x 32 x 32 zones (one core needs
+            # about a minute for a step of the full grid)
+            p1, gen1, _ = workload("cfg2", n_override=(64, 32, 32))
+            v1, secs1, c1 = cpu_oracle_time(p1, gen1, 3, threads=1)
+            cpu["single_thread"] = {"value": v1, "unit": UNIT, "cores": c1,
+                                    "sample": f"3 steps of the same torus on 64x32x32 zones ({secs1:.1f} s)"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
@@ -453,8 +514,11 @@ def main():
                        "performed_zone_updates_per_sec": performed,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": f"state arrays ({ws_gb:.1f} GB workspace) far larger than the 126 MB L2; no flush needed",
-                       "timing": "CUDA events on the launching (torch current) stream"},
+                       "timing": "CUDA events on the launching (torch current) stream; the headline pass carries no "
+                                 "per-kernel instrumentation (the kernel table comes from a second pass of the same steps)"},
             "clocks": clocks,
+            "sustained": {"value": sustained, "unit": UNIT, "steps": sus_steps, "ms_per_step": ms_sus / sus_steps,
+                          "what": "the same step repeated for >= 0.7 s right after the headline pass (power-capped clocks)"},
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": args.e2e_steps, "what": ("hamr_set_all_blocks + hamr_step(1) + hamr_get_all_blocks"
                              if refined else "hamr_set_prims(host) + hamr_step(1) + hamr_get_prims(host)") + ", pinned buffers"},

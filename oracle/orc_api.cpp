@@ -500,6 +500,8 @@ void orc_get_ctop(void* h, double* c3) {
 // number of OpenMP threads the oracle's loops use (reported by bench.py's cpu_baseline leg)
 #include <omp.h>
 extern "C" int orc_omp_threads() { return omp_get_max_threads(); }
+// the timing harness runs the oracle on one core and on all of them
+extern "C" void orc_set_threads(int n) { omp_set_num_threads(n > 0 ? n : omp_get_num_procs()); }
 
 // debug access for the boundary pins: fills the ghosts of the single block's current state and returns one
 // full padded array (kind 0..4 hydro, 5..7 Bc, 8..10 Bf), extents n + 2 NG + 1 per dimension, x3 fastest
