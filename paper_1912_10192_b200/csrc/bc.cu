@@ -131,12 +131,14 @@ __global__ void __launch_bounds__(256) k_ghosts(Dev D, Fields s, int all) {
 // The ghost shell only (the per-stage fill; ~12 % of the padded grid for cfg 2):
 //  part A: (i,j) columns with i or j outside the active range (plus the j = 0 wall row of a reflecting
 //          axis): every k;   part B: active (i,j) columns: the 2 NG + 1 ghost slots in k.
-__global__ void __launch_bounds__(256) k_ghosts_shell(Dev D, Fields s, int nj, long long nA) {
+// nox3: the stage kernels of this grid never read x3 ghost zones (x3_ghosts_unused, flux.cu): part A covers
+// k in [0, n3) only and there is no part B.
+__global__ void __launch_bounds__(256) k_ghosts_shell(Dev D, Fields s, int nj, long long nA, int nox3) {
   const Lay& L = D.L;
-  const int e3 = L.n[2] + 2 * NG + 1;
+  const int e3 = nox3 ? L.n[2] : L.n[2] + 2 * NG + 1;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t < nA) {
-    const int k = (int)(t % e3) - NG;
+    const int k = (int)(t % e3) - (nox3 ? 0 : NG);
     long long row = t / e3;
     int i, j;
     const long long lo_rows = (long long)NG * L.e2, mid_rows = (long long)L.n[0] * nj;
@@ -154,6 +156,7 @@ __global__ void __launch_bounds__(256) k_ghosts_shell(Dev D, Fields s, int nj, l
     ghost_cell(D, s, 0, i, j, k);
     return;
   }
+  if (nox3) return;
   const long long u = t - nA;
   const long long nB = (long long)L.n[0] * L.n[1] * 8;
   if (u >= nB) return;
@@ -200,9 +203,10 @@ void launch_ghosts(hamr_grid* g, const Fields& s, bool all) {
   }
   const int nj = 2 * NG + 1 + (g->D.bc_lo[1] >= HAMR_BC_POLAR_REFLECT ? 1 : 0);
   const long long rows = (long long)(2 * NG + 1) * L.e2 + (long long)L.n[0] * nj;
-  const long long nA = rows * e3;
-  const long long tot = nA + (long long)L.n[0] * L.n[1] * 8;
-  k_ghosts_shell<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s, nj, nA);
+    const bool nox3 = x3_ghosts_unused(g->D);
+  const long long nA = rows * (nox3 ? L.n[2] : e3);
+  const long long tot = nA + (nox3 ? 0 : (long long)L.n[0] * L.n[1] * 8);
+  k_ghosts_shell<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s, nj, nA, nox3 ? 1 : 0);
 }
 
 }  // namespace hamr

@@ -7,11 +7,12 @@
 
 namespace hamr {
 
-// centre EMFs on active zones plus one ghost layer
-template <bool BLK>
+// centre EMFs on active zones plus one ghost layer.  WRAP (x3_ghosts_unused): k runs over [0, n3) and the two x3
+// ghost columns are stored as the periodic images of columns n3 - 1 and 0 (their zones are not read)
+template <bool BLK, bool WRAP>
 __global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s0, Fields s2) {
   const Lay& L = Dv.L;
-  const int c2 = L.n[2] + 2, c1 = L.n[1] + 2;
+  const int c2 = L.n[2] + (WRAP ? 0 : 2), c1 = L.n[1] + 2;
   const unsigned per = (unsigned)(L.n[0] + 2) * c1 * c2;
   unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= (BLK ? per * Dv.B.nact : per)) return;
@@ -19,7 +20,7 @@ __global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s0, Fields s2
   if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
   const BCtx C = blk_ctx<BLK>(Dv, bslot);
   const unsigned tj = t / (unsigned)c2, ti = tj / (unsigned)c1;
-  const int k = (int)(t - tj * c2) - 1;
+  const int k = (int)(t - tj * c2) - (WRAP ? 0 : 1);
   const int j = (int)(tj - ti * c1) - 1;
   const int i = (int)ti - 1;
   const long long z = C.zoff + L.idx(i, j, k);
@@ -37,9 +38,15 @@ __global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s0, Fields s2
   const double iut = 1.0 / (gam * ialpha);
   const double w1 = (v1 - gam * boa) * iut, w2 = v2 * iut, w3 = v3 * iut;  // v^i = u^i / u^t
   const double B1 = gdet * s.Bc[0][z], B2 = gdet * s.Bc[1][z], B3 = gdet * s.Bc[2][z];
-  Dv.Cc[0][z] = -(w2 * B3 - w3 * B2);
-  Dv.Cc[1][z] = -(w3 * B1 - w1 * B3);
-  Dv.Cc[2][z] = -(w1 * B2 - w2 * B1);
+  const double e0 = -(w2 * B3 - w3 * B2), e1 = -(w3 * B1 - w1 * B3), e2 = -(w1 * B2 - w2 * B1);
+  Dv.Cc[0][z] = e0;
+  Dv.Cc[1][z] = e1;
+  Dv.Cc[2][z] = e2;
+  if (WRAP) {
+    const int n3 = L.n[2];
+    const long long zd = (k == n3 - 1) ? z - n3 : (k == 0 ? z + n3 : -1);
+    if (zd >= 0) { Dv.Cc[0][zd] = e0; Dv.Cc[1][zd] = e1; Dv.Cc[2][zd] = e2; }
+  }
 }
 
 __device__ __forceinline__ double up(double m, double lo, double hi) {
@@ -95,11 +102,13 @@ void launch_ct_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& 
   const bool blk = Dv.B.nblk > 0;
   if (blk && Dv.B.nact == 0) return;
   const long long mult = blk ? Dv.B.nact : 1;
-  long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 2) * mult;
+  const bool wrap = x3_ghosts_unused(Dv);
+  long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + (wrap ? 0 : 2)) * mult;
   {
     Launch l_(g, K_CEMF);
-    if (blk) k_centre_emf<true><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
-    else k_centre_emf<false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
+    if (blk) k_centre_emf<true, false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
+    else if (wrap) k_centre_emf<false, true><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
+    else k_centre_emf<false, false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
   }
   tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1) * mult;
   Launch l_(g, K_EDGE);

@@ -388,8 +388,11 @@ static_assert(RING >= 6, "the prologue holds the six rows of two adjacent PPM st
 #ifndef HAMR_RING_UNROLL2
 #define HAMR_RING_UNROLL2 1
 #endif
+#ifndef HAMR_RING_WARPS
+#define HAMR_RING_WARPS (HAMR_RING_MINB * 4)   // resident warps per SM the register budget is set for
+#endif
 template <int D, int KT>
-__global__ void __launch_bounds__(KT, HAMR_RING_MINB * 128 / KT) k_flux_ring(Dev Dv, Fields s, int seg, int want_ctop) {
+__global__ void __launch_bounds__(KT, HAMR_RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, Fields s, int seg, int want_ctop) {
   static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   using namespace ring;
   using namespace tma;
@@ -590,14 +593,17 @@ __global__ void __launch_bounds__(KT, HAMR_RING_MINB * 128 / KT) k_flux_ring(Dev
 // owns 32 consecutive zones of which the first HLO and the last HHI only help.
 // PPM (HLO = 2, HHI = 1): every lane builds the limited slope of ITS zone once; slopes, interface
 // values and right edges travel between lanes by warp shuffle.  PLM (HLO = 1, HHI = 0).
-template <int RECON, bool BLK>
+// WRAP (monolithic grids with a periodic x3, the grids the ring kernels serve): the stencil wraps inside the row and
+// the face at k = n3 is stored as the periodic image of the face at k = 0, so the x3 ghost zones are never read and the
+// per-stage ghost fill skips them (x3_ghosts_unused; bc.cu)
+template <int RECON, bool BLK, bool WRAP>
 __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s, Fields s2, int want_ctop) {
   constexpr int D = 2;
   constexpr int HLO = (RECON == HAMR_RECON_PPM) ? 2 : 1, HHI = (RECON == HAMR_RECON_PPM) ? 1 : 0;
   constexpr int OWN = 32 - HLO - HHI;
   constexpr unsigned FULL = 0xffffffffu;
   const Lay& L = Dv.L;
-  const int ck = L.n[2] + 1 + HLO + HHI, cj = L.n[1] + 2;
+  const int ck = L.n[2] + (WRAP ? 0 : 1) + HLO + HHI, cj = L.n[1] + 2;
   // 32-bit index arithmetic (the launcher guarantees tot < 2^31): 64-bit division is emulated
   const int per = (L.n[0] + 2) * cj * ck;
   const int tot = BLK ? per * Dv.B.nact : per;
@@ -615,6 +621,13 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
   const int j = (int)(tj - ti * cj) - 1;
   const int i = (int)ti - 1;
   const int z = C.zoff + (int)L.idx(i, j, k);
+  // offsets of zones k - 1, k, k + 1 relative to z (WRAP: their periodic images inside the row)
+  int om = -1, o0 = 0, op = 1;
+  if (WRAP) {
+    const int n3 = L.n[2];
+    auto wr = [n3](int q) { return q < 0 ? q + n3 : (q >= n3 ? q - n3 : q); };
+    om = wr(k - 1) - k; o0 = wr(k) - k; op = wr(k + 1) - k;
+  }
   const double* var[7] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
                           selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),
                           selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[0], s2.Bc[0], C.cur),
@@ -629,7 +642,7 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
     const double* a = var[v] + z;
     double aR;
     if (RECON == HAMR_RECON_PPM) {
-      const double m1 = a[-1], c0 = a[0], p1 = a[1];
+      const double m1 = a[om], c0 = a[o0], p1 = a[op];
       const double d21 = c0 - m1, d32 = p1 - c0;
       const double dm0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
       const double dmp = __shfl_down_sync(FULL, dm0, 1);         // slope of zone k+1
@@ -637,16 +650,19 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
       const double l = __shfl_up_sync(FULL, r, 1);               // a_{k-1/2}, built by lane-1 from the same expression
       ppm_mono(l, c0, r, PR[v], aR);
     } else {
-      plm_edges(a[-1], a[0], a[1], PR[v], aR);
+      plm_edges(a[om], a[o0], a[op], PR[v], aR);
     }
     PL[v] = __shfl_up_sync(FULL, aR, 1);  // right edge of zone k-1 = left state of face k-1/2
   }
   double ctop = 0.0;
   // C-15: the x3-faces of a phi-derefined row are computed by k_deref_x3 with a strided stencil
   const bool fine_row = Dv.mrow == nullptr || __ldg(Dv.mrow + C.J0 + j + NG) == 1;
-  if (valid && fine_row && lane >= HLO && lane < 32 - HHI && k >= 0 && k <= L.n[2]) {
+  if (valid && fine_row && lane >= HLO && lane < 32 - HHI && k >= 0 && k < L.n[2] + (WRAP ? 0 : 1)) {
     PL[7] = PR[7] = bf3 * G.igdet;
-    const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
+    double out[7];
+    const double ct = face_flux<D>(PL, PR, G, Dv.gam, out);
+    store_face(Dv, D, z, out);
+    if (WRAP && k == 0) store_face(Dv, D, z + L.n[2], out);
     if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct;
   }
   if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
@@ -814,6 +830,11 @@ static int ring_width(const Dev& Dv) {
   return (n3 % 128 == 0 && HAMR_RING_KTMAX >= 128) ? 128 : ((n3 % 64 == 0 && HAMR_RING_KTMAX >= 64) ? 64 : (n3 % 32 == 0 ? 32 : 0));
 }
 
+// On those grids no kernel of a stage reads a zone beyond the x3 range: the ring kernels and the wrapping x3 sweep
+// work on k in [0, n3) and store the periodic images, the centre-EMF kernel does the same (ct.cu), and the ghost
+// fill leaves the x3 ghost slots alone (bc.cu).
+bool x3_ghosts_unused(const Dev& Dv) { return ring_width(Dv) != 0; }
+
 template <int D>
 static void launch_march(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
   Launch l_(g, K_FLUX1 + D);
@@ -836,16 +857,18 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
   const Lay& L = Dv.L;
   const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
   const int own = ppm ? 29 : 31, halo = ppm ? 3 : 1;
-  const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + 1 + halo) * (blk ? Dv.B.nact : 1);
+  const bool x3wrap = x3_ghosts_unused(Dv);
+  const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + (x3wrap ? 0 : 1) + halo) * (blk ? Dv.B.nact : 1);
   const long long warps = (tot + own - 1) / own + 1;
   const unsigned nb = (unsigned)((warps + 3) / 4);
   const int wc = want_ctop ? 1 : 0;
   {
     Launch l_(g, K_FLUX3);
-    if (ppm && !blk) k_flux_x3<HAMR_RECON_PPM, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
-    else if (ppm) k_flux_x3<HAMR_RECON_PPM, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
-    else if (!blk) k_flux_x3<HAMR_RECON_PLM_MC, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
-    else k_flux_x3<HAMR_RECON_PLM_MC, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    if (x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (ppm && !blk) k_flux_x3<HAMR_RECON_PPM, false, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (ppm) k_flux_x3<HAMR_RECON_PPM, true, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (!blk) k_flux_x3<HAMR_RECON_PLM_MC, false, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else k_flux_x3<HAMR_RECON_PLM_MC, true, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
   }
   if (Dv.mrow) {  // C-15: strided x3 fluxes of the derefined rows, then the group structure on all face values
     launch_deref_x3(g, Dv, src, src2, want_ctop);

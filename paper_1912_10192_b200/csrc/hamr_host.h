@@ -186,6 +186,7 @@ namespace hamr {
 void launch_ghosts(hamr_grid* g, const Fields& s, bool bc_active_too);
 void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop);
 void launch_ct(hamr_grid* g, const Fields& src);
+bool x3_ghosts_unused(const Dev& Dv);   // flux.cu: the stage kernels of this grid never read x3 ghost zones
 void launch_update(hamr_grid* g, const Fields& src, const Fields& base, const Fields& out, double dtfac,
                    bool src_is_base);
 void launch_dt(hamr_grid* g, int mode);  // 0 set dt, 1 advance t + set dt, 2 latch ctop only
