@@ -304,6 +304,9 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     torch.cuda.set_device(local)
+    # everything below runs on one non-default stream (torch's current stream from here on): the library captures its
+    # step sequence as a CUDA graph, which the legacy default stream does not allow
+    torch.cuda.set_stream(torch.cuda.Stream())
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 

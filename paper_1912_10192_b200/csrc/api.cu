@@ -192,6 +192,9 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   g->launches = 0;
   g->prof = false;
   g->ev_used = 0;
+  g->step_graph[0] = g->step_graph[1] = nullptr;
+  g->graph_launches = 0;
+  g->plain_steps = 0;
   g->isn = 0; g->ish = 1; g->inew = 2;
   cudaError_t e;
   if (own) {
@@ -340,6 +343,38 @@ void enqueue_step(hamr_grid* g) {
   launch_dt(g, 1);  // C-14: the corrector's ctop of step n sets dt of step n+1
 }
 
+// One step of a monolithic grid.  The 15 launches of a step are captured once per buffer parity into a CUDA graph and
+// replayed (every kernel argument is fixed for a grid: dt and the Courant maxima live on the device); the first step
+// runs launch by launch (it also sets the per-kernel attributes and occupancy caches, which must not happen under
+// capture), and so does every step while the per-kernel timers are on.
+int step_once(hamr_grid* g) {
+  // (the legacy default stream cannot be captured: a grid created on it keeps launching kernel by kernel)
+  if (g->prof || g->plain_steps < 1 || g->stream == nullptr || g->stream == cudaStreamLegacy) {
+    enqueue_step(g);
+    g->plain_steps++;
+    return HAMR_OK;
+  }
+  const int par = g->isn == 0 ? 0 : 1;
+  if (!g->step_graph[par]) {
+    const int isn = g->isn, ish = g->ish, inew = g->inew;
+    const long long l0 = g->launches;
+    cudaGraph_t graph = nullptr;
+    CK(cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal));
+    enqueue_step(g);
+    cudaError_t e = cudaStreamEndCapture(g->stream, &graph);
+    g->isn = isn; g->ish = ish; g->inew = inew;      // the capture enqueued nothing: the state has not moved
+    g->graph_launches = g->launches - l0;
+    g->launches = l0;
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&g->step_graph[par], graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return fail(g, HAMR_ECUDA, "capturing the step as a CUDA graph", e);
+  }
+  CK(cudaGraphLaunch(g->step_graph[par], g->stream));
+  g->launches += g->graph_launches;
+  const int tmp = g->isn; g->isn = g->inew; g->inew = tmp;
+  return HAMR_OK;
+}
+
 int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* const bface[3], bool dev) {
   if (!g) return HAMR_EINVAL;
   if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
@@ -450,6 +485,8 @@ int hamr_grid_destroy(hamr_grid* g) {
   if (g->bh.h_ctop) cudaFreeHost(g->bh.h_ctop);
   if (g->bh.h_ints) cudaFreeHost(g->bh.h_ints);
   for (cudaEvent_t e : g->ev) cudaEventDestroy(e);
+  for (int c = 0; c < 2; c++)
+    if (g->step_graph[c]) cudaGraphExecDestroy(g->step_graph[c]);
   if (g->own_arena) cudaFree(g->arena);
   if (g->own_stream) cudaStreamDestroy(g->stream);
   delete g;
@@ -471,7 +508,10 @@ int hamr_step_async(hamr_grid* g, int nsteps) {
     const int rc = blk_step(g, nsteps);
     if (rc != HAMR_OK) return fail(g, rc, "block grid step failed");
   } else {
-    for (int s = 0; s < nsteps; s++) enqueue_step(g);
+    for (int s = 0; s < nsteps; s++) {
+      const int rc = step_once(g);
+      if (rc != HAMR_OK) return rc;
+    }
   }
   CK(cudaGetLastError());
   return HAMR_OK;

@@ -388,6 +388,9 @@ static_assert(RING >= 6, "the prologue holds the six rows of two adjacent PPM st
 #ifndef HAMR_RING_UNROLL2
 #define HAMR_RING_UNROLL2 1
 #endif
+#ifndef HAMR_X3_WARP
+#define HAMR_X3_WARP 1
+#endif
 #ifndef HAMR_RING_WARPS
 #define HAMR_RING_WARPS (HAMR_RING_MINB * 4)   // resident warps per SM the register budget is set for
 #endif
@@ -668,6 +671,124 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
   if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
 }
 
+// ---- sweep along x3, one warp per periodic row (monolithic grids the ring kernels serve, n3 = 32 M) ---------------
+// A lane owns M CONSECUTIVE zones of the row, so the parabolas of a row are built with the minimum of work: one
+// limited slope, one interface value and one monotonisation per zone, three shuffles per lane and variable (the
+// neighbours' edge quantities; lane 31 wraps to lane 0: the row is periodic, no lane is spent on halo zones and
+// no ghost zone is read).  The left / right states of the row's n3 faces go through shared memory (14 doubles per
+// face), because the Riemann problems are then solved with lanes on CONSECUTIVE faces (coalesced stores).
+// A warp walks over a contiguous range of rows; each row's stencil lines are prefetched into L2 one row ahead.
+template <int M>
+__global__ void __launch_bounds__(32, HAMR_RING_WARPS) k_flux_x3_warp(Dev Dv, Fields s, int seg, int want_ctop) {
+  constexpr int D = 2;
+  constexpr unsigned FULL = 0xffffffffu;
+  constexpr int QS = (M == 1) ? 32 : 32 + 16 / M;   // slot stride between a lane's zones: conflict-free both ways
+  constexpr int NV = M * QS;                         // doubles per variable and side
+  __shared__ double lr[14 * NV];
+  const Lay& L = Dv.L;
+  const int lane = threadIdx.x;
+  const int n3 = 32 * M, cj = L.n[1] + 2;
+  const int nrow = (L.n[0] + 2) * cj;
+  const int r0 = blockIdx.x * seg, r1 = min(r0 + seg, nrow);
+  const double* var[7] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[0], s.Bc[1]};
+  const int up = (lane + 31) & 31, dn = (lane + 1) & 31;   // the lanes owning the zones before / after this lane's
+  double ctop = 0.0;
+  for (int row = r0; row < r1; row++) {
+    const int i = row / cj - 1, j = row - (i + 1) * cj - 1;
+    const int zr = (int)L.idx(i, j, 0);
+    if (row + 1 < r1 && lane < n3 / 16) {   // next row's lines (7 variables + face field) into L2
+      const int i2 = (row + 1) / cj - 1, j2 = (row + 1) - (i2 + 1) * cj - 1;
+      const int zn = (int)L.idx(i2, j2, 0) + 16 * lane;
+#pragma unroll
+      for (int v = 0; v < 7; v++) asm volatile("prefetch.global.L2 [%0];" ::"l"(var[v] + zn));
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(s.Bf[2] + zn));
+    }
+    // ---- phase 1: parabolas of the lane's M zones, states of their low faces to shared memory ----
+#pragma unroll
+    for (int v = 0; v < 7; v++) {
+      double a[M + 2];   // zones M l - 1 .. M l + M
+      if (M >= 2) {
+        const double2* a2 = reinterpret_cast<const double2*>(var[v] + zr + M * lane);
+#pragma unroll
+        for (int q = 0; q < M / 2; q++) { const double2 t = __ldg(a2 + q); a[1 + 2 * q] = t.x; a[2 + 2 * q] = t.y; }
+      } else {
+        a[1] = __ldg(var[v] + zr + lane);
+      }
+      a[0] = __shfl_sync(FULL, a[M], up);
+      a[M + 1] = __shfl_sync(FULL, a[1], dn);
+      double dm[M + 1], r[M];
+#pragma unroll
+      for (int q = 0; q < M; q++) dm[q] = lim_slope(a[q + 1] - a[q], a[q + 2] - a[q + 1], 0.5 * (a[q + 2] - a[q]));
+      dm[M] = __shfl_sync(FULL, dm[0], dn);
+#pragma unroll
+      for (int q = 0; q < M; q++) r[q] = ppm_iface(a[q + 1], a[q + 2] - a[q + 1], dm[q], dm[q + 1]);
+      double l = __shfl_sync(FULL, r[M - 1], up), aRlast = 0.0;
+#pragma unroll
+      for (int q = 0; q < M; q++) {
+        double aL, aR;
+        ppm_mono(l, a[q + 1], r[q], aL, aR);
+        lr[(7 + v) * NV + q * QS + lane] = aL;                  // right state of the zone's low face
+        if (q + 1 < M) lr[v * NV + (q + 1) * QS + lane] = aR;   // left state of the next zone's low face
+        else aRlast = aR;
+        l = r[q];
+      }
+      lr[v * NV + lane] = __shfl_sync(FULL, aRlast, up);        // left state of this lane's first face
+    }
+    __syncwarp();
+    // ---- phase 2: Riemann problems, lanes on consecutive faces ----
+    const FGeo G = load_fgeo(Dv.gf3A + (size_t)((NG + i) * L.e2 + NG + j) * NREC_F);
+    const bool act = i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1];
+#pragma unroll 1
+    for (int q2 = 0; q2 < M; q2++) {
+      const int f = lane + 32 * q2;                  // face = zone index
+      const int sl = (f % M) * QS + f / M;
+      double PL[8], PR[8];
+#pragma unroll
+      for (int v = 0; v < 7; v++) { PL[v] = lr[v * NV + sl]; PR[v] = lr[(7 + v) * NV + sl]; }
+      const int z = zr + f;
+      PL[7] = PR[7] = __ldg(s.Bf[2] + z) * G.igdet;
+      double out[7];
+      const double ct = face_flux<D>(PL, PR, G, Dv.gam, out);
+      if (act) ctop = dmax(ctop, ct);
+      store_face(Dv, D, z, out);
+      if (f == 0) store_face(Dv, D, z + n3, out);   // the face at k = n3 is the periodic image of the face at k = 0
+    }
+    __syncwarp();
+  }
+  if (want_ctop) ctop_commit<false>(Dv, D, 0, ctop);
+}
+
+template <int M>
+static void launch_x3_warp_t(hamr_grid* g, const Dev& Dv, const Fields& src, bool want_ctop) {
+  const Lay& L = Dv.L;
+  static int per_sm = 0;
+  if (per_sm == 0) {
+    int v = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_flux_x3_warp<M>, 32, 0);
+    per_sm = v < 1 ? 1 : v;
+  }
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int nrow = (L.n[0] + 2) * (L.n[1] + 2);
+  // a whole number of waves of resident warps, at least 8 rows per warp
+  const int slots = sms * per_sm;
+  int waves = (nrow + 8 * slots - 1) / (8 * slots);
+  if (waves < 1) waves = 1;
+  int nw = waves * slots;
+  if (nw > nrow) nw = nrow;
+  const int seg = (nrow + nw - 1) / nw;
+  k_flux_x3_warp<M><<<(nrow + seg - 1) / seg, 32, 0, g->stream>>>(Dv, src, seg, want_ctop ? 1 : 0);
+}
+
+static int ring_width(const Dev& Dv);
+// M = n3 / 32 of the warp-per-row x3 sweep (0: not served)
+static int x3_warp_m(const Dev& Dv) {
+  if (ring_width(Dv) == 0) return 0;
+  const int n3 = Dv.L.n[2];
+  return (n3 == 32 || n3 == 64 || n3 == 128 || n3 == 256) ? n3 / 32 : 0;
+}
+
 // ---- C-15 (ii): x3-faces of phi-derefined rows -----------------------------------------------------------
 // "PPM ... modified for the increased cell spacing".  In a row with factor m the flux exists on
 // group-boundary faces only (k a multiple of m); its stencil takes one value per group, zones k + t m,
@@ -864,6 +985,15 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
   const int wc = want_ctop ? 1 : 0;
   {
     Launch l_(g, K_FLUX3);
+#if HAMR_X3_WARP
+    switch (x3_warp_m(Dv)) {
+      case 1: launch_x3_warp_t<1>(g, Dv, src, want_ctop); return;
+      case 2: launch_x3_warp_t<2>(g, Dv, src, want_ctop); return;
+      case 4: launch_x3_warp_t<4>(g, Dv, src, want_ctop); return;
+      case 8: launch_x3_warp_t<8>(g, Dv, src, want_ctop); return;
+      default: break;
+    }
+#endif
     if (x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (ppm && !blk) k_flux_x3<HAMR_RECON_PPM, false, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (ppm) k_flux_x3<HAMR_RECON_PPM, true, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);

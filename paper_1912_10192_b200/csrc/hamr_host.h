@@ -151,6 +151,11 @@ struct hamr_grid {
   std::vector<cudaEvent_t> ev;   // pairs: start, stop
   std::vector<int> ev_cls;
   size_t ev_used;
+  // the step sequence of a monolithic grid as a CUDA graph: one executable graph per parity of
+  // the rotating state buffers, captured on first use after one plain step has run
+  cudaGraphExec_t step_graph[2];
+  long long graph_launches;      // kernel launches one replay stands for
+  int plain_steps;               // steps enqueued launch by launch so far
 };
 
 namespace hamr {
