@@ -703,6 +703,12 @@ __global__ void __launch_bounds__(32, HAMR_RING_WARPS) k_flux_x3_warp(Dev Dv, Fi
       for (int v = 0; v < 7; v++) asm volatile("prefetch.global.L2 [%0];" ::"l"(var[v] + zn));
       asm volatile("prefetch.global.L2 [%0];" ::"l"(s.Bf[2] + zn));
     }
+    // the row's face record and the normal field of this lane's faces are requested with the stencil: they are
+    // used in phase 2, after the parabolas
+    const FGeo G = load_fgeo(Dv.gf3A + (size_t)((NG + i) * L.e2 + NG + j) * NREC_F);
+    double bf3[M];
+#pragma unroll
+    for (int q2 = 0; q2 < M; q2++) bf3[q2] = __ldg(s.Bf[2] + zr + lane + 32 * q2);
     // ---- phase 1: parabolas of the lane's M zones, states of their low faces to shared memory ----
 #pragma unroll
     for (int v = 0; v < 7; v++) {
@@ -736,9 +742,8 @@ __global__ void __launch_bounds__(32, HAMR_RING_WARPS) k_flux_x3_warp(Dev Dv, Fi
     }
     __syncwarp();
     // ---- phase 2: Riemann problems, lanes on consecutive faces ----
-    const FGeo G = load_fgeo(Dv.gf3A + (size_t)((NG + i) * L.e2 + NG + j) * NREC_F);
     const bool act = i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1];
-#pragma unroll 1
+#pragma unroll
     for (int q2 = 0; q2 < M; q2++) {
       const int f = lane + 32 * q2;                  // face = zone index
       const int sl = (f % M) * QS + f / M;
@@ -746,7 +751,7 @@ __global__ void __launch_bounds__(32, HAMR_RING_WARPS) k_flux_x3_warp(Dev Dv, Fi
 #pragma unroll
       for (int v = 0; v < 7; v++) { PL[v] = lr[v * NV + sl]; PR[v] = lr[(7 + v) * NV + sl]; }
       const int z = zr + f;
-      PL[7] = PR[7] = __ldg(s.Bf[2] + z) * G.igdet;
+      PL[7] = PR[7] = bf3[q2] * G.igdet;
       double out[7];
       const double ct = face_flux<D>(PL, PR, G, Dv.gam, out);
       if (act) ctop = dmax(ctop, ct);
@@ -786,7 +791,9 @@ static int ring_width(const Dev& Dv);
 static int x3_warp_m(const Dev& Dv) {
   if (ring_width(Dv) == 0) return 0;
   const int n3 = Dv.L.n[2];
-  return (n3 == 32 || n3 == 64 || n3 == 128 || n3 == 256) ? n3 / 32 : 0;
+  // n3 = 256 (M = 8) needs 30 KB of shared memory per warp (7 resident warps per SM): measured slower than the
+  // shuffle kernel on cfg 3 (1.86 vs 1.66 ms)
+  return (n3 == 32 || n3 == 64 || n3 == 128) ? n3 / 32 : 0;
 }
 
 // ---- C-15 (ii): x3-faces of phi-derefined rows -----------------------------------------------------------
@@ -990,7 +997,6 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
       case 1: launch_x3_warp_t<1>(g, Dv, src, want_ctop); return;
       case 2: launch_x3_warp_t<2>(g, Dv, src, want_ctop); return;
       case 4: launch_x3_warp_t<4>(g, Dv, src, want_ctop); return;
-      case 8: launch_x3_warp_t<8>(g, Dv, src, want_ctop); return;
       default: break;
     }
 #endif
