@@ -147,10 +147,11 @@ ALG_RW = {"flux_x1": (9, 7), "flux_x2": (9, 7), "flux_x3": (9, 7),   # r: P5, 2 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel class and the FP64 thread
 # instructions (dadd + dmul + dfma) the flux kernels execute per face, from the round's `ncu --set full` capture of
 # this same command on cfg 2
-NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_full_cfg2.md"
-NCU_TRAFFIC = {"flux_x1": 535800000, "flux_x2": 521100000, "flux_x3": 538700000}
-FLUX_FP64_INST_PER_FACE = {"flux_x1": 335.0, "flux_x2": 335.0, "flux_x3": 341.0}
-FLUX_FMA_FRACTION = 1.0 / 3.0      # a third of those are DFMA (2 FLOP), the rest DADD / DMUL (1 FLOP)
+NCU_TRAFFIC_SOURCE = "profiles/r2a_ncu_full_cfg2.md"
+NCU_TRAFFIC = {"flux_x1": 539500000, "flux_x2": 523200000, "flux_x3": 498500000, "centre_emf": 294900000,
+               "edge_emf": 534900000, "update_predictor": 1462600000, "update_corrector": 1736800000, "ghosts": 15600000}
+FLUX_FP64_INST_PER_FACE = {"flux_x1": 340.5, "flux_x2": 337.0, "flux_x3": 328.0}
+FLUX_FMA_FRACTION = 0.36           # the DFMA share of those (2 FLOP each), the rest DADD / DMUL (1 FLOP)
 FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
 PAPER_V100_150CUBED = 0.85e8   # ~0.85e8 zone-cycles/s, 1 V100, one 150^3 block
 
@@ -473,7 +474,10 @@ def main():
         traffic = sum(NCU_TRAFFIC[k] for k in dk)          # the class's launches of one stage, like `achieved`
     flux_alu = None
     if classes["flux"] and not blocky and fp64:
-        ins = sum(FLUX_FP64_INST_PER_FACE[k] * units_per_launch(k, n) * kern[k]["launches"] for k in classes["flux"])
+        # faces the kernels COMPUTE on cfg 2 (the x3 ghost columns and the face at k = n3 are stored periodic images)
+        nface = {"flux_x1": (n[0] + 1) * (n[1] + 2) * n[2], "flux_x2": (n[0] + 2) * (n[1] + 1) * n[2],
+                 "flux_x3": (n[0] + 2) * (n[1] + 2) * n[2]}
+        ins = sum(FLUX_FP64_INST_PER_FACE[k] * nface[k] * kern[k]["launches"] for k in classes["flux"])
         sec = sum(kern[k]["ms_total"] for k in classes["flux"]) * 1e-3
         flux_alu = {"bound": "alu", "kernels": "+".join(classes["flux"]), "achieved": ins / sec / 1e9,
                     "peak": fp64["ginstr_per_s_flux_mix"], "unit": "G thread-instructions/s (FP64 pipe)",

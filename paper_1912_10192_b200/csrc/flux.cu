@@ -376,17 +376,11 @@ namespace ring {
 #define HAMR_RING_SLOTS 6
 #endif
 constexpr int RING = HAMR_RING_SLOTS;   // 3 live rows (zones fc, fc + 1, fc + 2) + the rows in flight
-static_assert(RING >= 6, "the prologue holds the six rows of two adjacent PPM stencils");
+static_assert(RING >= 6, "three live rows, one dying, two in flight");
 }  // namespace ring
 
 #ifndef HAMR_RING_MINB
 #define HAMR_RING_MINB 3
-#endif
-#ifndef HAMR_RING_PIPE
-#define HAMR_RING_PIPE 0
-#endif
-#ifndef HAMR_RING_UNROLL2
-#define HAMR_RING_UNROLL2 1
 #endif
 #ifndef HAMR_X3_WARP
 #define HAMR_X3_WARP 1
@@ -401,40 +395,47 @@ __global__ void __launch_bounds__(KT, HAMR_RING_WARPS * 32 / KT) k_flux_ring(Dev
   using namespace tma;
   constexpr int O = 1 - D;
   constexpr int e = (D + 1) % 3, f = (D + 2) % 3;
+  constexpr int NW = KT / 32;              // warps of the CTA; warp 0 also is the producer
   constexpr int SLOTD = 8 * KT + NREC_F;   // doubles per ring slot: 7 variables, the face field, the face record
   extern __shared__ __align__(128) double ring_mem[];
-  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(ring_mem + RING * SLOTD);
+  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(ring_mem + RING * SLOTD);   // slot filled
+  unsigned long long* mbe = mbar + RING;                                                         // slot released
   const Lay& L = Dv.L;
   const int t = threadIdx.x;
   const int k0 = blockIdx.x * KT, k = k0 + t;
   const int o = (int)blockIdx.y - 1;
   const int f0 = blockIdx.z * seg, f1 = min(f0 + seg, L.n[D] + 1);
   const int sd = (D == 0) ? L.S1 : L.S2;
-  const int rbase = f0 - 3, rlast = f1 + 1 + HAMR_RING_PIPE;   // rows (zones along the sweep) this CTA reads
+  const int rbase = f0 - 3, rlast = f1 + 1;   // rows (zones along the sweep) this CTA reads
   const double* gtab = (D == 0 ? Dv.gf1A : Dv.gf2A);
   // The producer is one elected lane of warp 0: the next row of every array, and the record of its face, into the
   // next slot.  Its state (row, slot, padded offset of the row, record index) is the same in every thread and
-  // advances by constants, so it lives in uniform registers.
+  // advances by constants, so it lives in uniform registers.  A slot is refilled one step after the row in it died:
+  // the other warps have announced on the slot's second barrier that they are done with it, and warp 0 waits on that
+  // barrier only if one of them lags by more than a step (no CTA-wide barrier inside the loop).
   int prow = rbase, pslot = 0;
   int pz = (int)L.idx(D == 0 ? rbase : o, D == 0 ? o : rbase, k0);
   int pq = (NG * L.e2 + NG) + ((D == 0) ? rbase * L.e2 + o : o * L.e2 + rbase);
   const bool warp0 = t < 32;
   auto issue_next = [&]() {
-    if (warp0 && elect_one()) {
-      double* dst = ring_mem + pslot * SLOTD;
-      unsigned long long* mb = mbar + pslot;
-      const bool face = prow >= f0 && prow < f1;   // rows that are also faces of this segment carry field and record
-      mbar_expect(mb, (unsigned)((face ? 8 * KT + NREC_F : 7 * KT) * sizeof(double)));
-      bulk_g2s(dst + 0 * KT, s.P[0] + pz, KT * sizeof(double), mb);
-      bulk_g2s(dst + 1 * KT, s.P[1] + pz, KT * sizeof(double), mb);
-      bulk_g2s(dst + 2 * KT, s.P[2] + pz, KT * sizeof(double), mb);
-      bulk_g2s(dst + 3 * KT, s.P[3] + pz, KT * sizeof(double), mb);
-      bulk_g2s(dst + 4 * KT, s.P[4] + pz, KT * sizeof(double), mb);
-      bulk_g2s(dst + 5 * KT, s.Bc[e] + pz, KT * sizeof(double), mb);
-      bulk_g2s(dst + 6 * KT, s.Bc[f] + pz, KT * sizeof(double), mb);
-      if (face) {
-        bulk_g2s(dst + 7 * KT, s.Bf[D] + pz, KT * sizeof(double), mb);
-        bulk_g2s(dst + 8 * KT, gtab + (size_t)pq * NREC_F, NREC_F * sizeof(double), mb);
+    if (warp0) {
+      if (NW > 1 && prow >= rbase + RING) mbar_wait(mbe + pslot, (unsigned)(((prow - rbase) / RING - 1) & 1));
+      if (elect_one()) {
+        double* dst = ring_mem + pslot * SLOTD;
+        unsigned long long* mb = mbar + pslot;
+        const bool face = prow >= f0 && prow < f1;   // rows that are also faces of this segment carry field and record
+        mbar_expect(mb, (unsigned)((face ? 8 * KT + NREC_F : 7 * KT) * sizeof(double)));
+        bulk_g2s(dst + 0 * KT, s.P[0] + pz, KT * sizeof(double), mb);
+        bulk_g2s(dst + 1 * KT, s.P[1] + pz, KT * sizeof(double), mb);
+        bulk_g2s(dst + 2 * KT, s.P[2] + pz, KT * sizeof(double), mb);
+        bulk_g2s(dst + 3 * KT, s.P[3] + pz, KT * sizeof(double), mb);
+        bulk_g2s(dst + 4 * KT, s.P[4] + pz, KT * sizeof(double), mb);
+        bulk_g2s(dst + 5 * KT, s.Bc[e] + pz, KT * sizeof(double), mb);
+        bulk_g2s(dst + 6 * KT, s.Bc[f] + pz, KT * sizeof(double), mb);
+        if (face) {
+          bulk_g2s(dst + 7 * KT, s.Bf[D] + pz, KT * sizeof(double), mb);
+          bulk_g2s(dst + 8 * KT, gtab + (size_t)pq * NREC_F, NREC_F * sizeof(double), mb);
+        }
       }
     }
     prow++;
@@ -443,7 +444,7 @@ __global__ void __launch_bounds__(KT, HAMR_RING_WARPS * 32 / KT) k_flux_ring(Dev
     pq += (D == 0) ? L.e2 : 1;
   };
   if (t == 0) {
-    for (int c = 0; c < RING; c++) mbar_init(mbar + c, 1);
+    for (int c = 0; c < RING; c++) { mbar_init(mbar + c, 1); mbar_init(mbe + c, NW > 1 ? NW - 1 : 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -459,77 +460,6 @@ __global__ void __launch_bounds__(KT, HAMR_RING_WARPS * 32 / KT) k_flux_ring(Dev
   const int dup = (k == L.n[2] - 1) ? -L.n[2] : (k == 0 ? L.n[2] : 0);
   double PL[8], PR[8], dm[7], il[7];
   double ctop = 0.0;
-#if HAMR_RING_PIPE
-  // Software pipeline: step fc solves the Riemann problem of face fc (states built one step earlier) next to the
-  // parabola of zone fc + 1 (rows fc + 1 .. fc + 3).  The two are independent instruction streams in one basic
-  // block: the seven short limiter chains fill the issue slots that the long dependent chain of a side state
-  // (square root, reciprocal, quadratic) leaves empty.
-  double carry[7];
-  // prologue: the parabolas of zones f0 - 1 and f0 from rows f0 - 3 .. f0 + 2 (all slots of the first revolution)
-#pragma unroll
-  for (int c = 0; c < 6; c++) mbar_wait(mbar + c, 0);
-  {
-    const double* a = ring_mem + t;
-#pragma unroll
-    for (int v = 0; v < 7; v++) {
-      const double m2 = a[0 * SLOTD + v * KT], m1 = a[1 * SLOTD + v * KT], c0 = a[2 * SLOTD + v * KT],
-                   p1 = a[3 * SLOTD + v * KT], p2 = a[4 * SLOTD + v * KT], p3 = a[5 * SLOTD + v * KT];
-      const double d10 = m1 - m2, d21 = c0 - m1, d32 = p1 - c0, d43 = p2 - p1, d54 = p3 - p2;
-      const double dm_m = lim_slope(d10, d21, 0.5 * (c0 - m2));
-      const double dm_0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
-      const double dm_p = lim_slope(d32, d43, 0.5 * (p2 - c0));
-      const double dm_q = lim_slope(d43, d54, 0.5 * (p3 - p1));
-      const double r = ppm_iface(c0, d32, dm_0, dm_p), r2 = ppm_iface(p1, d43, dm_p, dm_q);
-      double aL;
-      ppm_mono(ppm_iface(m1, d21, dm_m, dm_0), c0, r, aL, PL[slot[v]]);
-      ppm_mono(r, p1, r2, PR[slot[v]], carry[v]);
-      dm[v] = dm_q; il[v] = r2;
-    }
-  }
-#if HAMR_RING_UNROLL2
-#pragma unroll 2
-#endif
-  for (int fc = f0; fc < f1; fc++) {
-    z += sd;
-    __syncthreads();   // every thread is done with the rows below fc: their slots can be refilled
-#pragma unroll 1
-    while (prow <= rlast && prow <= fc - 1 + RING) issue_next();
-    const int n0 = fc - rbase;   // ring position of row fc; rows fc + 1 .. fc + 3 follow
-    const int s0 = n0 % RING, s1 = (n0 + 1) % RING, s2 = (n0 + 2) % RING, s3 = (n0 + 3) % RING;
-    mbar_wait(mbar + s3, (unsigned)(((n0 + 3) / RING) & 1));
-    const double* r1 = ring_mem + s1 * SLOTD + t;
-    const double* r2 = ring_mem + s2 * SLOTD + t;
-    const double* r3 = ring_mem + s3 * SLOTD + t;
-    // stream A: HLL on face fc.  A pole face (C-7: no flux, no state) is computed on its record (gdet = 0) and
-    // discarded, so that the step stays one basic block
-    const FGeo G = load_fgeo_shared(ring_mem + s0 * SLOTD + 8 * KT);
-    PL[5 + D] = PR[5 + D] = ring_mem[s0 * SLOTD + 7 * KT + t] * G.igdet;  // C-5: the normal field is single-valued
-    double out[7];
-    const double ct = face_flux<D>(PL, PR, G, Dv.gam, out);
-    // stream B: the parabola of zone fc + 1 gives the right state of face fc + 1 and the left state of face fc + 2
-    double PRn[7], carryn[7];
-#pragma unroll
-    for (int v = 0; v < 7; v++) {
-      const double c0 = r1[v * KT], c1 = r2[v * KT], a2 = r3[v * KT];
-      const double d21 = c1 - c0, d32 = a2 - c1;
-      const double dmp = lim_slope(d21, d32, 0.5 * (a2 - c0));
-      const double r = ppm_iface(c0, d21, dm[v], dmp);
-      ppm_mono(il[v], c0, r, PRn[v], carryn[v]);
-      dm[v] = dmp; il[v] = r;
-    }
-    const bool pole = (D == 1) && ks && (fc == 0 || fc == L.n[1]);
-    if (pole) {
-#pragma unroll
-      for (int c = 0; c < 7; c++) out[c] = 0.0;
-    } else if (act) {
-      ctop = dmax(ctop, ct);
-    }
-    store_face(Dv, D, z, out);
-    if (dup != 0) store_face(Dv, D, z + dup, out);
-#pragma unroll
-    for (int v = 0; v < 7; v++) { PL[slot[v]] = carry[v]; PR[slot[v]] = PRn[v]; carry[v] = carryn[v]; }
-  }
-#else
   // prologue: the parabola of zone f0 - 1 from rows f0 - 3 .. f0 + 1 (slots 0 .. 4 of the first revolution)
 #pragma unroll
   for (int c = 0; c < 5; c++) mbar_wait(mbar + c, 0);
@@ -549,17 +479,20 @@ __global__ void __launch_bounds__(KT, HAMR_RING_WARPS * 32 / KT) k_flux_ring(Dev
       dm[v] = dm_p; il[v] = r;
     }
   }
-#if HAMR_RING_UNROLL2
+  // unrolled by two: the marching state alternates between two register sets instead of being moved at the loop end
 #pragma unroll 2
-#endif
   for (int fc = f0; fc < f1; fc++) {
     z += sd;
-    __syncthreads();   // every thread is done with the rows below fc: their slots can be refilled
-    // rows below fc are dead: three after the prologue, one per step afterwards
-#pragma unroll 1
-    while (prow <= rlast && prow <= fc - 1 + RING) issue_next();
+    __syncwarp();
     const int n0 = fc - rbase;   // ring position of row fc; rows fc + 1, fc + 2 follow
     const int s0 = n0 % RING, s1 = (n0 + 1) % RING, s2 = (n0 + 2) % RING;
+    if (NW > 1 && !warp0 && (t & 31) == 0) {   // this warp is done with the rows below fc
+      if (fc == f0) { mbar_arrive(mbe + 0); mbar_arrive(mbe + 1); mbar_arrive(mbe + 2); }
+      else mbar_arrive(mbe + (n0 + RING - 1) % RING);
+    }
+    // the rows that died a step ago are replaced (after the prologue: the first two of its three dead rows)
+#pragma unroll 1
+    while (prow <= rlast && prow <= fc - 2 + RING) issue_next();
     mbar_wait(mbar + s2, (unsigned)(((n0 + 2) / RING) & 1));
     const double* r0 = ring_mem + s0 * SLOTD + t;
     const double* r1 = ring_mem + s1 * SLOTD + t;
@@ -587,7 +520,6 @@ __global__ void __launch_bounds__(KT, HAMR_RING_WARPS * 32 / KT) k_flux_ring(Dev
 #pragma unroll
     for (int v = 0; v < 7; v++) PL[slot[v]] = carry[v];
   }
-#endif
   if (want_ctop) ctop_commit<false>(Dv, D, 0, ctop);
 }
 
@@ -919,7 +851,7 @@ template <int D, int KT>
 static void launch_ring_t(hamr_grid* g, const Dev& Dv, const Fields& src, bool want_ctop) {
   const Lay& L = Dv.L;
   const int O = 1 - D;
-  const size_t smem = (size_t)ring::RING * ((8 * KT + NREC_F) * sizeof(double)) + ring::RING * sizeof(unsigned long long);
+  const size_t smem = (size_t)ring::RING * ((8 * KT + NREC_F) * sizeof(double)) + 2 * ring::RING * sizeof(unsigned long long);
   static int per_sm = 0;   // set once per instantiation (the attribute and the occupancy are per function)
   if (per_sm == 0) {
     cudaFuncSetAttribute(k_flux_ring<D, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -953,7 +885,7 @@ static int ring_width(const Dev& Dv) {
   if (Dv.B.nblk > 0 || Dv.recon != HAMR_RECON_PPM || Dv.mrow || Dv.bc_lo[2] != HAMR_BC_PERIODIC) return 0;
   if (Dv.L.n[0] + 2 > 65535 || Dv.L.n[1] + 2 > 65535) return 0;
 #ifndef HAMR_RING_KTMAX
-#define HAMR_RING_KTMAX 32
+#define HAMR_RING_KTMAX 32   // 64 / 128 (two / four warps per CTA, slots released through a second mbarrier) measured 3-7 % slower
 #endif
   return (n3 % 128 == 0 && HAMR_RING_KTMAX >= 128) ? 128 : ((n3 % 64 == 0 && HAMR_RING_KTMAX >= 64) ? 64 : (n3 % 32 == 0 ? 32 : 0));
 }
