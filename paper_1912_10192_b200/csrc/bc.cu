@@ -6,10 +6,6 @@
 // composing the three index maps: every ghost value is a signed copy of one active value.
 #include "hamr_host.h"
 
-#ifndef HAMR_GHOST_FAST
-#define HAMR_GHOST_FAST 1  // copy path for the periodic x3 slots of the shell fill
-#endif
-
 namespace hamr {
 
 __device__ __forceinline__ int pmod(int g, int n) {
@@ -169,7 +165,7 @@ __global__ void __launch_bounds__(256) k_ghosts_shell(Dev D, Fields s, int nj, l
   const int k = q < NG ? q - NG : n3 + q - NG;
   // periodic x3 on a row that is not derefined and touches no reflecting wall face: the slots are plain
   // copies of the image zone; same values and the same B_c arithmetic as ghost_cell
-  const bool fast = HAMR_GHOST_FAST && D.bc_lo[2] == HAMR_BC_PERIODIC && !D.mrow && n3 > NG &&
+  const bool fast = D.bc_lo[2] == HAMR_BC_PERIODIC && !D.mrow && n3 > NG &&
                     !(j + 1 == L.n[1] && D.bc_hi[1] >= HAMR_BC_POLAR_REFLECT) &&
                     !(i + 1 == L.n[0] && D.bc_hi[0] >= HAMR_BC_POLAR_REFLECT);
   if (!fast) { ghost_cell(D, s, 0, i, j, k); return; }

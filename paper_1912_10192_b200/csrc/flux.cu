@@ -252,26 +252,14 @@ __device__ __forceinline__ void ctop_commit(const Dev& Dv, int D, int b, double 
 // PPM: the thread carries, per variable, a_j, a_{j+1}, the limited slope of zone j and the interface
 // value a_{j-1/2}; each step loads ONE new value a_{j+2}, builds ONE new slope and ONE new interface
 // value (the expressions are those of ppm_edges, so the result is bitwise the same).
-#ifndef HAMR_MARCH_RELOAD
-#define HAMR_MARCH_RELOAD 1  // 1: re-read a_j, a_{j+1} from L1 each step instead of carrying them in registers (measured faster)
-#endif
-#ifndef HAMR_MARCH_MINB
-#define HAMR_MARCH_MINB 4  // 128 regs/thread: measured best of 1/3/4 on cfg 2 (profiles/)
-#endif
-#ifndef HAMR_MARCH_T
-#define HAMR_MARCH_T 128  // threads per CTA; 32 / 64 / 256 measured within 0.5 % of each other (cfg 2)
-#endif
-#ifndef HAMR_MARCH_UNROLL
-#define HAMR_MARCH_UNROLL 1
-#endif
-constexpr int MARCH_UNROLL = HAMR_MARCH_UNROLL;
-#ifndef HAMR_X3_MINB
-#define HAMR_X3_MINB 5
-#endif
+// Tuning constants of the generic kernels, each the best of a measured sweep on cfg 2 (round 1):
+// 128 threads per CTA at 128 registers (4 CTAs per SM) for the marching kernels, 96 registers (5 CTAs) for the x3 sweep;
+// a_j, a_{j+1} are re-read from L1 each step instead of being carried in registers.
+constexpr int MARCH_T = 128, MARCH_MINB = 4, X3_MINB = 5;
 // BLK: the launch covers the blocks of Dv.B.list (block-structured grid, H7); s / s2 are the buffer sets
 // holding the stage source of blocks with cur == 0 / cur == 2.
 template <int D, int RECON, bool BLK>
-__global__ void __launch_bounds__(HAMR_MARCH_T, HAMR_MARCH_MINB * 128 / HAMR_MARCH_T) k_flux_march(Dev Dv, Fields s, Fields s2, int seg,
+__global__ void __launch_bounds__(MARCH_T, MARCH_MINB) k_flux_march(Dev Dv, Fields s, Fields s2, int seg,
                                                                       int want_ctop) {
   static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   const Lay& L = Dv.L;
@@ -301,7 +289,7 @@ __global__ void __launch_bounds__(HAMR_MARCH_T, HAMR_MARCH_MINB * 128 / HAMR_MAR
     constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
     int z = C.zoff + (int)L.idx(D == 0 ? f0 - 1 : o, D == 0 ? o : f0 - 1, k);
     double PL[8], PR[8];
-    double a0[7], a1[7], dm[7], il[7];  // PPM marching state (unused for PLM)
+    double dm[7], il[7];  // PPM marching state (unused for PLM)
     // the zone below the first face: its right edge, and the marching state of the next zone
 #pragma unroll
     for (int v = 0; v < 7; v++) {
@@ -315,13 +303,12 @@ __global__ void __launch_bounds__(HAMR_MARCH_T, HAMR_MARCH_MINB * 128 / HAMR_MAR
         const double r = ppm_iface(c0, d32, dm_0, dm_p);
         double aL;
         ppm_mono(ppm_iface(m1, d21, dm_m, dm_0), c0, r, aL, PL[slot[v]]);
-        a0[v] = p1; a1[v] = p2; dm[v] = dm_p; il[v] = r;
+        dm[v] = dm_p; il[v] = r;
       } else {
         double aL;
         plm_edges(a[-sd], a[0], a[sd], aL, PL[slot[v]]);
       }
     }
-#pragma unroll MARCH_UNROLL
     for (int fc = f0; fc < f1; fc++) {
       z += sd;
       double carry[7];
@@ -330,16 +317,12 @@ __global__ void __launch_bounds__(HAMR_MARCH_T, HAMR_MARCH_MINB * 128 / HAMR_MAR
         const double* a = var[v] + z;
         if (RECON == HAMR_RECON_PPM) {
           const double a2 = a[2 * sd];
-#if HAMR_MARCH_RELOAD
           const double c0 = a[0], c1 = a[sd];
-#else
-          const double c0 = a0[v], c1 = a1[v];
-#endif
           const double d21 = c1 - c0, d32 = a2 - c1;
           const double dmp = lim_slope(d21, d32, 0.5 * (a2 - c0));
           const double r = ppm_iface(c0, d21, dm[v], dmp);
           ppm_mono(il[v], c0, r, PR[slot[v]], carry[v]);
-          a0[v] = c1; a1[v] = a2; dm[v] = dmp; il[v] = r;
+          dm[v] = dmp; il[v] = r;
         } else {
           plm_edges(a[-sd], a[0], a[sd], PR[slot[v]], carry[v]);
         }
@@ -372,24 +355,15 @@ __global__ void __launch_bounds__(HAMR_MARCH_T, HAMR_MARCH_MINB * 128 / HAMR_MAR
 // hold no registers.  The x3-faces of the transverse ghost columns k = -1 and k = n3, which C-9 reads, are the
 // periodic images of columns n3 - 1 and 0: their threads store twice.
 namespace ring {
-#ifndef HAMR_RING_SLOTS
-#define HAMR_RING_SLOTS 6
-#endif
-constexpr int RING = HAMR_RING_SLOTS;   // 3 live rows (zones fc, fc + 1, fc + 2) + the rows in flight
+constexpr int RING = 6;   // 3 live rows (zones fc, fc + 1, fc + 2) + the rows in flight
 static_assert(RING >= 6, "three live rows, one dying, two in flight");
 }  // namespace ring
 
-#ifndef HAMR_RING_MINB
-#define HAMR_RING_MINB 3
-#endif
-#ifndef HAMR_X3_WARP
-#define HAMR_X3_WARP 1
-#endif
-#ifndef HAMR_RING_WARPS
-#define HAMR_RING_WARPS (HAMR_RING_MINB * 4)   // resident warps per SM the register budget is set for
-#endif
+// resident warps per SM the register budget of the staged kernels is set for: 12 (168 registers, no spills) measured
+// best of 8 / 10 / 11 / 12 / 13-16 (profiles/r2_experiments.md)
+constexpr int RING_WARPS = 12;
 template <int D, int KT>
-__global__ void __launch_bounds__(KT, HAMR_RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, Fields s, int seg, int want_ctop) {
+__global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, Fields s, int seg, int want_ctop) {
   static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   using namespace ring;
   using namespace tma;
@@ -532,7 +506,7 @@ __global__ void __launch_bounds__(KT, HAMR_RING_WARPS * 32 / KT) k_flux_ring(Dev
 // the face at k = n3 is stored as the periodic image of the face at k = 0, so the x3 ghost zones are never read and the
 // per-stage ghost fill skips them (x3_ghosts_unused; bc.cu)
 template <int RECON, bool BLK, bool WRAP>
-__global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s, Fields s2, int want_ctop) {
+__global__ void __launch_bounds__(128, X3_MINB) k_flux_x3(Dev Dv, Fields s, Fields s2, int want_ctop) {
   constexpr int D = 2;
   constexpr int HLO = (RECON == HAMR_RECON_PPM) ? 2 : 1, HHI = (RECON == HAMR_RECON_PPM) ? 1 : 0;
   constexpr int OWN = 32 - HLO - HHI;
@@ -611,7 +585,7 @@ __global__ void __launch_bounds__(128, HAMR_X3_MINB) k_flux_x3(Dev Dv, Fields s,
 // face), because the Riemann problems are then solved with lanes on CONSECUTIVE faces (coalesced stores).
 // A warp walks over a contiguous range of rows; each row's stencil lines are prefetched into L2 one row ahead.
 template <int M>
-__global__ void __launch_bounds__(32, HAMR_RING_WARPS) k_flux_x3_warp(Dev Dv, Fields s, int seg, int want_ctop) {
+__global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields s, int seg, int want_ctop) {
   constexpr int D = 2;
   constexpr unsigned FULL = 0xffffffffu;
   constexpr int QS = (M == 1) ? 32 : 32 + 16 / M;   // slot stride between a lane's zones: conflict-free both ways
@@ -698,15 +672,17 @@ __global__ void __launch_bounds__(32, HAMR_RING_WARPS) k_flux_x3_warp(Dev Dv, Fi
 template <int M>
 static void launch_x3_warp_t(hamr_grid* g, const Dev& Dv, const Fields& src, bool want_ctop) {
   const Lay& L = Dv.L;
-  static int per_sm = 0;
-  if (per_sm == 0) {
+  // occupancy cached per host thread and device (a grid is driven by one thread at a time; two grids may be driven concurrently)
+  thread_local int per_sm = 0, sms = 148, cached_dev = -1;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev != cached_dev) {
     int v = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_flux_x3_warp<M>, 32, 0);
     per_sm = v < 1 ? 1 : v;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cached_dev = dev;
   }
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   const int nrow = (L.n[0] + 2) * (L.n[1] + 2);
   // a whole number of waves of resident warps, at least 8 rows per warp
   const int slots = sms * per_sm;
@@ -807,15 +783,15 @@ void launch_deref_x3(hamr_grid* g, const Dev& Dv0, const Fields& src, const Fiel
 // blocks (148 SMs x blocks per SM) with little prologue overhead
 template <int D, int RECON, bool BLK>
 static int pick_segment(const Lay& L, int nbx) {
-  static int cached_seg = 0;
-  static long long cached_key = -1;
+  thread_local int cached_seg = 0, cached_dev = -1;   // per host thread: no shared mutable state between grids
+  thread_local long long cached_key = -1;
   const int nf = L.n[D] + 1;
   const long long key = (long long)nf * (1LL << 32) + nbx;
-  if (key == cached_key) return cached_seg;
   int dev = 0, sms = 148, per_sm = 2;
   cudaGetDevice(&dev);
+  if (key == cached_key && dev == cached_dev) return cached_seg;
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_flux_march<D, RECON, BLK>, HAMR_MARCH_T, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_flux_march<D, RECON, BLK>, MARCH_T, 0);
   if (per_sm < 1) per_sm = 1;
   const double slots = (double)sms * per_sm;
   double best = -1.0;
@@ -831,6 +807,7 @@ static int pick_segment(const Lay& L, int nbx) {
     if (eff > best) { best = eff; best_seg = seg; }
   }
   cached_key = key;
+  cached_dev = dev;
   cached_seg = best_seg;
   return best_seg;
 }
@@ -840,10 +817,10 @@ static void launch_march_t(hamr_grid* g, const Dev& Dv, const Fields& src, const
   const Lay& L = Dv.L;
   const int O = 1 - D;
   const long long ntr = (long long)(L.n[O] + 2) * (L.n[2] + 2) * (BLK ? Dv.B.nact : 1);
-  const int nbx = (int)((ntr + HAMR_MARCH_T - 1) / HAMR_MARCH_T);
+  const int nbx = (int)((ntr + MARCH_T - 1) / MARCH_T);
   const int seg = pick_segment<D, RECON, BLK>(L, nbx);
   dim3 grid(nbx, (L.n[D] + 1 + seg - 1) / seg);
-  k_flux_march<D, RECON, BLK><<<grid, HAMR_MARCH_T, 0, g->stream>>>(Dv, src, src2, seg, want_ctop ? 1 : 0);
+  k_flux_march<D, RECON, BLK><<<grid, MARCH_T, 0, g->stream>>>(Dv, src, src2, seg, want_ctop ? 1 : 0);
 }
 
 // the ring kernel: segment length such that the grid fills whole waves of resident CTAs
@@ -852,16 +829,18 @@ static void launch_ring_t(hamr_grid* g, const Dev& Dv, const Fields& src, bool w
   const Lay& L = Dv.L;
   const int O = 1 - D;
   const size_t smem = (size_t)ring::RING * ((8 * KT + NREC_F) * sizeof(double)) + 2 * ring::RING * sizeof(unsigned long long);
-  static int per_sm = 0;   // set once per instantiation (the attribute and the occupancy are per function)
-  if (per_sm == 0) {
+  // the attribute and the occupancy are per function and device; cached per host thread
+  thread_local int per_sm = 0, sms = 148, cached_dev = -1;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev != cached_dev) {
     cudaFuncSetAttribute(k_flux_ring<D, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     int v = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_flux_ring<D, KT>, KT, smem);
     per_sm = v < 1 ? 1 : v;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cached_dev = dev;
   }
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   const int nf = L.n[D] + 1, nrow = (L.n[2] / KT) * (L.n[O] + 2);
   const double slots = (double)sms * per_sm;
   double best = -1.0;
@@ -884,10 +863,8 @@ static int ring_width(const Dev& Dv) {
   const int n3 = Dv.L.n[2];
   if (Dv.B.nblk > 0 || Dv.recon != HAMR_RECON_PPM || Dv.mrow || Dv.bc_lo[2] != HAMR_BC_PERIODIC) return 0;
   if (Dv.L.n[0] + 2 > 65535 || Dv.L.n[1] + 2 > 65535) return 0;
-#ifndef HAMR_RING_KTMAX
-#define HAMR_RING_KTMAX 32   // 64 / 128 (two / four warps per CTA, slots released through a second mbarrier) measured 3-7 % slower
-#endif
-  return (n3 % 128 == 0 && HAMR_RING_KTMAX >= 128) ? 128 : ((n3 % 64 == 0 && HAMR_RING_KTMAX >= 64) ? 64 : (n3 % 32 == 0 ? 32 : 0));
+  // one warp per CTA: 64 / 128 threads (slots released through the second mbarrier) measured 3-7 % slower
+  return n3 % 32 == 0 ? 32 : 0;
 }
 
 // On those grids no kernel of a stage reads a zone beyond the x3 range: the ring kernels and the wrapping x3 sweep
@@ -899,10 +876,7 @@ template <int D>
 static void launch_march(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
   Launch l_(g, K_FLUX1 + D);
   const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
-  const int kt = ring_width(Dv);
-  if (kt == 128) return launch_ring_t<D, 128>(g, Dv, src, want_ctop);
-  if (kt == 64) return launch_ring_t<D, 64>(g, Dv, src, want_ctop);
-  if (kt == 32) return launch_ring_t<D, 32>(g, Dv, src, want_ctop);
+  if (ring_width(Dv) == 32) return launch_ring_t<D, 32>(g, Dv, src, want_ctop);
   if (ppm && !blk) launch_march_t<D, HAMR_RECON_PPM, false>(g, Dv, src, src2, want_ctop);
   else if (ppm) launch_march_t<D, HAMR_RECON_PPM, true>(g, Dv, src, src2, want_ctop);
   else if (!blk) launch_march_t<D, HAMR_RECON_PLM_MC, false>(g, Dv, src, src2, want_ctop);
@@ -924,14 +898,12 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
   const int wc = want_ctop ? 1 : 0;
   {
     Launch l_(g, K_FLUX3);
-#if HAMR_X3_WARP
     switch (x3_warp_m(Dv)) {
       case 1: launch_x3_warp_t<1>(g, Dv, src, want_ctop); return;
       case 2: launch_x3_warp_t<2>(g, Dv, src, want_ctop); return;
       case 4: launch_x3_warp_t<4>(g, Dv, src, want_ctop); return;
       default: break;
     }
-#endif
     if (x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (ppm && !blk) k_flux_x3<HAMR_RECON_PPM, false, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (ppm) k_flux_x3<HAMR_RECON_PPM, true, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);

@@ -30,20 +30,11 @@ __device__ __forceinline__ Fields pick_fields(const Fields& a, const Fields& b, 
   return f;
 }
 
-#ifndef HAMR_UPD_MINB
-#define HAMR_UPD_MINB 6
-#endif
-#ifndef HAMR_UPD_MINB_PRED
-#define HAMR_UPD_MINB_PRED 5
-#endif
-#ifndef HAMR_UPD_RELOAD
-#define HAMR_UPD_RELOAD 1
-#endif
-#ifndef HAMR_UPD_TILE
-#define HAMR_UPD_TILE 1
-#endif
+// generic kernel: 6 CTAs of 128 threads per SM for the corrector (80 registers), 5 for the predictor (96, no spills):
+// measured best of 3-7 on cfg 2 (profiles/r2_experiments.md)
+constexpr int UPD_MINB = 6, UPD_MINB_PRED = 5;
 template <bool SAME, bool BLK>  // SAME: predictor, source state == base state
-__global__ void __launch_bounds__(128, SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
+__global__ void __launch_bounds__(128, SAME ? UPD_MINB_PRED : UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
   const Lay& L = Dv.L;
   // k runs over [0, n3): warps start on 128-byte lines when n3 is a multiple of 32; the thread at k = 0 also
   // builds the x3-face at k = n3
@@ -132,7 +123,6 @@ __global__ void __launch_bounds__(128, SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB
         U[c] = U[c] - dt * div + dt * sc;
       }
       double Pn[5], Pg[5];
-#if HAMR_UPD_RELOAD
       // the geometry record and the guess are re-read (L1 / L2 hits) instead of being kept in registers
       // across the flux divergence: lower register pressure, more resident warps
       const double* gtab = grec;
@@ -141,11 +131,6 @@ __global__ void __launch_bounds__(128, SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB
       const double* sp[5] = {src.P[0], src.P[1], src.P[2], src.P[3], src.P[4]};
 #pragma unroll
       for (int c = 0; c < 5; c++) { const double* a = sp[c]; asm volatile("" : "+l"(a)); Pg[c] = a[z]; }
-#else
-      const CGeo& G2 = G;
-#pragma unroll
-      for (int c = 0; c < 5; c++) Pg[c] = Ps[c];
-#endif
       if (con2prim(U, Bn, G2, Dv.gam, Pg, Pn) != 0) {  // C-13: keep the source state's hydro primitives, count the failure
         nfail = 1;
 #pragma unroll
@@ -186,10 +171,7 @@ __global__ void __launch_bounds__(128, SAME ? HAMR_UPD_MINB_PRED : HAMR_UPD_MINB
 // dependent part (states, source, Newton inversion, floors) runs while those copies land.  Zone-centred arrays
 // without reuse (source / base state in, new state out) are read and written directly, requested at the top of the step.
 namespace tile {
-#ifndef HAMR_TILE_TJ
-#define HAMR_TILE_TJ 2
-#endif
-constexpr int TJ = HAMR_TILE_TJ;
+constexpr int TJ = 2;            // rows per CTA: 1 / 3 / 4 measured 5-19 % slower (profiles/r2_experiments.md)
 constexpr int NA = 8, NB = 13;   // arrays keeping two planes / one plane
 }
 
@@ -367,18 +349,23 @@ static void launch_tile_t(hamr_grid* g, const Dev& Dv, const Roles& r, double dt
   using namespace tile;
   const Lay& L = Dv.L;
   const size_t smem = (size_t)(2 * NA + NB) * (TJ + 1) * L.p3 * sizeof(double) + 16;
-  static size_t attr_set = 0;
-  static int per_sm = 1;
-  if (attr_set != smem) {   // per function instantiation; smem depends on the x3 pitch only
-    cudaFuncSetAttribute(k_update_tile<SAME, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  // cached per host thread, device and shared-memory size (which depends on the x3 pitch only).  The function's limit
+  // is raised to the device's opt-in maximum, never to this grid's size: another thread's grid may need more.
+  thread_local size_t cached_smem = 0;
+  thread_local int per_sm = 1, sms = 148, cached_dev = -1;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (cached_smem != smem || cached_dev != dev) {
+    int optin = 0;
+    cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaFuncSetAttribute(k_update_tile<SAME, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
     int v = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_update_tile<SAME, NT>, NT, smem);
     per_sm = v < 1 ? 1 : v;
-    attr_set = smem;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cached_smem = smem;
+    cached_dev = dev;
   }
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   const int np = L.n[0] + 1, ntile = (L.n[1] + 1 + TJ - 1) / TJ;
   const double slots = (double)sms * per_sm;
   double best = -1.0;
@@ -414,7 +401,6 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
   const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * L.n[2] * (blk ? Dv.B.nact : 1);
   const unsigned nb = (unsigned)((tot + 127) / 128);
   Launch l_(g, same ? K_UPDATE_P : K_UPDATE_C);
-#if HAMR_UPD_TILE
   switch (tile_threads(Dv)) {
     case 64: return same ? launch_tile_t<true, 64>(g, Dv, ra, dtfac) : launch_tile_t<false, 64>(g, Dv, ra, dtfac);
     case 128: return same ? launch_tile_t<true, 128>(g, Dv, ra, dtfac) : launch_tile_t<false, 128>(g, Dv, ra, dtfac);
@@ -422,7 +408,6 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
     case 512: return same ? launch_tile_t<true, 512>(g, Dv, ra, dtfac) : launch_tile_t<false, 512>(g, Dv, ra, dtfac);
     default: break;
   }
-#endif
   if (same && !blk) k_update<true, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
   else if (same) k_update<true, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
   else if (!blk) k_update<false, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
