@@ -35,6 +35,8 @@ struct Params {
   int32_t deref_factor[4];
   int32_t lat_max_level; // C-17; 0 -> global dt
   int32_t map;
+  int32_t entropy_backup;  // C-18 (NEXT-2): advect the entropy, invert with it where the energy inversion fails
+  int32_t drift_floors;    // C-19 (NEXT-2): floors inject mass / energy in the drift frame instead of the fluid frame
   double a;              // spin
   double xmin[3], xmax[3];   // PHYSICAL extents ((r_in,r_out),(0,pi),(0,2pi)) or box
   double gamma_ad, cour;
@@ -77,6 +79,16 @@ void source(const double P[8], const State& S, const Geom& G, const double conn[
 // returns 0 ok, >0 failure code; P_out[0..4] hydro primitives (B untouched = input Bc)
 int con2prim(const double U[5], const double Bc[3], const Geom& G, double gam,
              const double Pguess[5], double Pout[5], int* iters);
+
+// ---- C-18 entropy as a backup for the energy equation (Noble et al. 2009) ------------------------
+// kappa = p / rho^gamma_ad = (gamma_ad - 1) u / rho^gamma_ad: constant along smooth flow lines
+double entropy_kappa(double rho, double u, double gam);
+// conserved entropy and its flux along dir (1..3): gdet rho kappa u^t, gdet rho kappa u^dir
+void entropy_UF(const double P[8], const State& S, const Geom& G, double gam, int dir, double& US, double& FS);
+// inversion with the entropy row US in place of the energy row U[1] (which is not read): a 1-unknown root find.
+// returns 0 ok, 1 no convergence / no bracket, 2 non-finite or non-positive D or US
+int con2prim_entropy(const double U[5], double US, const double Bc[3], const Geom& G, double gam,
+                     const double Pguess[5], double Pout[5], int* iters);
 
 // ---- reconstruction (C-5) ------------------------------------------------------------------------
 // zone j's parabola edges from a[j-2..j+2] given as a[0..4]

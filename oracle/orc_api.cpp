@@ -27,6 +27,14 @@ static bool params_ok(const Params& p, std::string& why) {
     }
   }
   if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0)) { why = "gamma_ad/cour"; return false; }
+  if (p.entropy_backup || p.drift_floors) {  // C-18, C-19: built for the single-block grid
+    if ((p.entropy_backup & ~1) || (p.drift_floors & ~1)) { why = "entropy_backup / drift_floors are 0 or 1"; return false; }
+    if (p.nb[0] > 0 || p.nb[1] > 0 || p.nb[2] > 0 || p.n_deref > 0 || p.lat_max_level > 0 || p.r_refine_max > 0.0) {
+      why = "entropy_backup / drift_floors need a grid of one block without derefinement";
+      return false;
+    }
+    if (p.entropy_backup && !(p.gamma_ad < 2.0)) { why = "the entropy inversion needs gamma_ad < 2"; return false; }
+  }
   return true;
 }
 
@@ -42,7 +50,7 @@ static Grid* grid_new(const Params& par) {
   g->t = 0.0;
   g->dt = 0.0;
   g->have_state = false;
-  g->stats = Stats{0, 0, 0, 0};
+  g->stats = Stats{0, 0, 0, 0, 0};
   if (!params_ok(par, g->err)) { delete g; return nullptr; }
   g->multi = par.nb[0] > 0 || par.nb[1] > 0 || par.nb[2] > 0 || par.n_deref > 0 ||
              par.lat_max_level > 0 || par.r_refine_max > 0.0;
@@ -165,7 +173,7 @@ int orc_set_prims(void* h, const double* const hydro[5], const double* const bfa
     blocks_initial_dt(g);
     g.t = 0.0;
     g.have_state = true;
-    g.stats = Stats{0, 0, 0, 0};
+    g.stats = Stats{0, 0, 0, 0, 0};
     return state_finite(g) ? 0 : 5;
   }
   Block& b = g.blocks[0];
@@ -193,7 +201,7 @@ int orc_set_prims(void* h, const double* const hydro[5], const double* const bfa
   g.dt = dt_from_ctop(g.par, b);
   g.t = 0.0;
   g.have_state = true;
-  g.stats = Stats{0, 0, 0, 0};
+  g.stats = Stats{0, 0, 0, 0, 0};
   return state_finite(g) ? 0 : 5;
 }
 
@@ -286,17 +294,35 @@ int orc_get_stats(void* h, long long counts[4]) {
   Grid& g = *(Grid*)h;
   counts[0] = g.stats.c2p_fail; counts[1] = g.stats.rho_floor;
   counts[2] = g.stats.u_floor;  counts[3] = g.stats.gam_ceil;
-  g.stats = Stats{0, 0, 0, 0};
+  g.stats.c2p_fail = g.stats.rho_floor = g.stats.u_floor = g.stats.gam_ceil = 0;
+  return 0;
+}
+// zones, since the last call, whose primitives came from the entropy inversion (C-18)
+int orc_get_backup_count(void* h, long long* n) {
+  Grid& g = *(Grid*)h;
+  *n = g.stats.c2p_entropy;
+  g.stats.c2p_entropy = 0;
+  return 0;
+}
+// kappa = (entropy row) / (density row) of the latest update, before it is reset from the primitives; active zones
+int orc_get_kadv(void* h, double* out) {
+  Grid& g = *(Grid*)h;
+  Block& b = g.blocks[0];
+  if (!g.par.entropy_backup || b.Kadv.empty()) return 1;
+  for (int i = 0; i < b.n[0]; i++)
+    for (int j = 0; j < b.n[1]; j++)
+      for (int k = 0; k < b.n[2]; k++) out[((size_t)i * b.n[1] + j) * b.n[2] + k] = b.Kadv[b.idx(i, j, k)];
   return 0;
 }
 
 // Face fluxes / EMFs of the most recent flux pass, for face-by-face parity (debug access).
-// which: 0..4 hydro flux F^d[c]; 5,6 the two face EMFs E_e, E_f with (d,e,f) cyclic.
+// which: 0..4 hydro flux F^d[c]; 5,6 the two face EMFs E_e, E_f with (d,e,f) cyclic; 7 the entropy flux (C-18).
 int orc_get_face(void* h, int d, int which, double* out) {
   Grid& g = *(Grid*)h;
   Block& b = g.blocks[0];
   static const int CY[3][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}};
-  const std::vector<double>& a = (which < 5) ? b.F[d][which] : b.Ef[d][CY[d][which - 4]];
+  if (which == 7 && !g.par.entropy_backup) return 1;
+  const std::vector<double>& a = (which == 7) ? b.FK[d] : (which < 5) ? b.F[d][which] : b.Ef[d][CY[d][which - 4]];
   int m[3] = {b.n[0], b.n[1], b.n[2]};
   m[d] += 1;
   for (int i = 0; i < m[0]; i++)
@@ -367,7 +393,7 @@ int orc_blocks_commit(void* h) {
   blocks_initial_dt(g);
   g.t = 0.0;
   g.have_state = true;
-  g.stats = Stats{0, 0, 0, 0};
+  g.stats = Stats{0, 0, 0, 0, 0};
   return state_finite(g) ? 0 : 5;
 }
 int orc_get_block_prims(void* h, int bi, double* const prims[8]) {
@@ -444,10 +470,20 @@ int orc_con2prim(const double* U5, const double* Bc, const Geom* G, double gam, 
   return con2prim(U5, Bc, *G, gam, Pguess, Pout, iters);
 }
 // floors and Lorentz-factor ceiling of C-13 on one zone at radius r; counts3: rho-floor, u-floor, ceiling hits
-void orc_floors(const Params* par, const Geom* G, double r, double* P5, long long* counts3) {
-  Stats st = {0, 0, 0, 0};
-  floors_and_ceiling(*par, *G, r, P5, st);
+// Bc3: the zone's field (read with par->drift_floors; may be NULL)
+void orc_floors(const Params* par, const Geom* G, double r, double* P5, const double* Bc3, long long* counts3) {
+  Stats st = {0, 0, 0, 0, 0};
+  floors_and_ceiling(*par, *G, r, P5, Bc3, st);
   counts3[0] = st.rho_floor; counts3[1] = st.u_floor; counts3[2] = st.gam_ceil;
+}
+int orc_con2prim_entropy(const double* U5, double US, const double* Bc, const Geom* G, double gam,
+                         const double* Pguess, double* Pout, int* iters) {
+  return con2prim_entropy(U5, US, Bc, *G, gam, Pguess, Pout, iters);
+}
+void orc_entropy_UF(const double* P, const Geom* G, double gam, int dir, double* US, double* FS) {
+  State S;
+  get_state(P, *G, S);
+  entropy_UF(P, S, *G, gam, dir, *US, *FS);
 }
 void orc_ppm_zone(const double* a5, double* aL, double* aR) { ppm_zone(a5, *aL, *aR); }
 void orc_plm_zone(const double* a3, double* aL, double* aR) { plm_zone(a3, *aL, *aR); }

@@ -557,7 +557,7 @@ static void correct_level(Grid& g, int tau) {
             g.stats.c2p_fail++;
             for (int cc = 0; cc < 5; cc++) Pn[cc] = P[cc];
           }
-          floors_and_ceiling(par, G, r, Pn, g.stats);
+          floors_and_ceiling(par, G, r, Pn, nullptr, g.stats);
           for (int cc = 0; cc < 5; cc++) c.snew.P[cc][z] = Pn[cc];
         }
       }

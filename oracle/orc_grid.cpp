@@ -58,6 +58,7 @@ void block_init(const Params& par, Block& b) {
   b.snew.alloc(n);
   for (int d = 0; d < 3; d++) {
     for (int c = 0; c < 5; c++) b.F[d][c].assign(n, 0.0);
+    if (par.entropy_backup) b.FK[d].assign(n, 0.0);
     for (int c = 0; c < 3; c++) b.Ef[d][c].assign(n, 0.0);
     b.Ee[d].assign(n, 0.0);
     b.Cc[d].assign(n, 0.0);
@@ -194,18 +195,21 @@ void compute_Bc(const Block& b, Fields& s, bool active_only) {
 // ---- reconstruct + HLL on one face (C-5, C-6, C-7) -------------------------------------------------
 // face on the low side of zone z along d.  st6[v][0..5]: the six zone values a[j-3 .. j+2] of the
 // seven reconstructed variables around the face (j = the zone on the high side).
+// C-18: with par.entropy_backup an eighth variable, kappa = (gamma_ad - 1) u / rho^gamma_ad of the zones (b.K, filled
+// by flux_pass), is reconstructed like the others and the HLL flux of the entropy row goes to b.FK.
 static void face_flux_core(const Params& par, Block& b, const Fields& s, int d, int i, int j, size_t z,
-                           const double st6[7][6], double* ctop) {
+                           const double st6[8][6], double* ctop) {
   const int e = CYC[d][1], f = CYC[d][2];
   const Geom& G = (d == 0) ? b.gf1[b.idx2(i, j)] : (d == 1) ? b.gf2[b.idx2(i, j)] : b.gc[b.idx2(i, j)];
   if (d == 1 && b.pole2[j + NG]) {  // C-7: pole faces carry no flux; no state is evaluated
     for (int c = 0; c < 5; c++) b.F[d][c][z] = 0.0;
     b.Ef[d][e][z] = b.Ef[d][f][z] = 0.0;
+    if (par.entropy_backup) b.FK[d][z] = 0.0;
     return;
   }
-  double PL[8], PR[8];
+  double PL[8], PR[8], kL = 0.0, kR = 0.0;
   const int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
-  for (int v = 0; v < 7; v++) {
+  for (int v = 0; v < (par.entropy_backup ? 8 : 7); v++) {
     const double* a = st6[v];
     double aL, aR, dummy;
     if (par.recon == 0) {
@@ -215,6 +219,7 @@ static void face_flux_core(const Params& par, Block& b, const Fields& s, int d, 
       plm_zone(a + 1, dummy, aR);  // a[j-2 .. j]
       plm_zone(a + 2, aL, dummy);  // a[j-1 .. j+1]
     }
+    if (v == 7) { kL = aR; kR = aL; continue; }
     PL[slot[v]] = aR;
     PR[slot[v]] = aL;
   }
@@ -237,6 +242,14 @@ static void face_flux_core(const Params& par, Block& b, const Fields& s, int d, 
   // C-8: on a d-face, E_f = -F^d(B^e), E_e = +F^d(B^f)
   b.Ef[d][f][z] = -Fh[5 + e];
   b.Ef[d][e][z] = Fh[5 + f];
+  if (par.entropy_backup) {
+    // the entropy row (C-18) through the same HLL formula: U_S = gdet rho kappa u^t, F_S = gdet rho kappa u^d with the
+    // reconstructed kappa; gdet rho u^t and gdet rho u^d are row 0 of U and F
+    const double USL = UL[0] * kL, USR = UR[0] * kR, FSL = FL[0] * kL, FSR = FR[0] * kR;
+    double U2L[8] = {USL}, U2R[8] = {USR}, F2L[8] = {FSL}, F2R[8] = {FSR}, F2[8];
+    hll(U2L, U2R, F2L, F2R, cmin, cmax, F2);
+    b.FK[d][z] = F2[0];
+  }
   if (ctop) *ctop = std::max(cmax, cmin);
 }
 
@@ -248,9 +261,11 @@ static void face_flux(const Params& par, Block& b, const Fields& s, int d, int i
   const int e = CYC[d][1], f = CYC[d][2];
   const double* var[7] = {s.P[0].data(), s.P[1].data(), s.P[2].data(), s.P[3].data(),
                           s.P[4].data(), s.Bc[e].data(), s.Bc[f].data()};
-  double st6[7][6];
+  double st6[8][6];
   for (int v = 0; v < 7; v++)
     for (int t = 0; t < 6; t++) st6[v][t] = var[v][(ptrdiff_t)z + (t - 3) * sd];
+  if (par.entropy_backup)
+    for (int t = 0; t < 6; t++) st6[7][t] = b.K[(ptrdiff_t)z + (t - 3) * sd];
   face_flux_core(par, b, s, d, i, j, z, st6, ctop);
 }
 
@@ -262,7 +277,7 @@ static void face_flux_x3_deref(const Params& par, Block& b, const Fields& s, int
   const int n3 = b.n[2];
   const double* var[7] = {s.P[0].data(), s.P[1].data(), s.P[2].data(), s.P[3].data(),
                           s.P[4].data(), s.Bc[0].data(), s.Bc[1].data()};
-  double st6[7][6];
+  double st6[8][6];
   for (int v = 0; v < 7; v++)
     for (int t = 0; t < 6; t++) {
       int kk = k + (t - 3) * m;                      // first zone of the group, in fine zones
@@ -274,6 +289,10 @@ static void face_flux_x3_deref(const Params& par, Block& b, const Fields& s, int
 }
 
 void flux_pass(const Params& par, Block& b, const Fields& src) {
+  if (par.entropy_backup) {  // C-18: kappa of every zone of the source state, ghosts included
+    b.K.resize(b.size());
+    for (size_t z = 0; z < b.size(); z++) b.K[z] = entropy_kappa(src.P[0][z], src.P[1][z], par.gamma_ad);
+  }
   for (int d = 0; d < 3; d++) {
     int lo[3] = {-1, -1, -1}, hi[3] = {b.n[0], b.n[1], b.n[2]};  // one transverse ghost layer (CT)
     lo[d] = 0;
@@ -485,11 +504,50 @@ void ct_edges(const Params& par, Block& b, const Fields& s) {
 }
 
 // ---- floors and ceiling (C-13; PAPER.md:59 says only "below a certain threshold") -----------------
-void floors_and_ceiling(const Params& par, const Geom& G, double r, double P[5], Stats& st) {
+// C-19 (par.drift_floors; "injects mass and internal energy in the drift frame of the jet ... (Ressler et
+// al. 2017)"): the mass and energy added to reach the floors are added in the frame that moves with the part of the
+// velocity perpendicular to the magnetic field.  In the normal observer's frame, with v^i = ut^i / gamma and
+// curly-B^i = alpha B^i:   v^i = v_perp^i + v_par Bhat^i,   v_par = (v . B) / |B|.
+//   * v_perp (the E x B drift: E = -v x B does not see v_par) is left unchanged: no drag on the field lines;
+//   * the momentum along the field, m_par = w gamma^2 v_par (w = rho + gamma_ad u; the electromagnetic momentum
+//     is perpendicular to B), is conserved: the added matter carries none, so v_par drops and cannot run away.
+// With w' the enthalpy after the floors:  w' v_par' / (1 - v_perp^2 - v_par'^2) = m_par, whose root of the sign of
+// m_par is  v_par' = 2 m_par s / (w' + sqrt(w'^2 + 4 m_par^2 s)),  s = 1 - v_perp^2.   B = 0: the fluid frame.
+void floors_and_ceiling(const Params& par, const Geom& G, double r, double P[5], const double* Bc, Stats& st) {
   const double rfl = par.rho_fl_coef * std::pow(r, par.rho_fl_pow);
   const double ufl = par.u_fl_coef * std::pow(r, par.u_fl_pow);
-  if (P[0] < rfl) { P[0] = rfl; st.rho_floor++; }
-  if (P[1] < ufl) { P[1] = ufl; st.u_floor++; }
+  const bool lowr = P[0] < rfl, lowu = P[1] < ufl;
+  double Bsq = 0.0;
+  if (par.drift_floors && Bc && (lowr || lowu))
+    for (int i = 1; i < 4; i++)
+      for (int j = 1; j < 4; j++) Bsq += G.gcov[i][j] * (G.alpha * Bc[i - 1]) * (G.alpha * Bc[j - 1]);
+  if (Bsq > 0.0) {
+    double q = 0.0;
+    for (int i = 1; i < 4; i++)
+      for (int j = 1; j < 4; j++) q += G.gcov[i][j] * P[1 + i] * P[1 + j];
+    const double gamma = std::sqrt(1.0 + q);
+    double v[3], vB = 0.0;
+    for (int i = 0; i < 3; i++) v[i] = P[2 + i] / gamma;
+    for (int i = 1; i < 4; i++)
+      for (int j = 1; j < 4; j++) vB += G.gcov[i][j] * v[i - 1] * (G.alpha * Bc[j - 1]);
+    const double Bn = std::sqrt(Bsq);
+    const double vpar = vB / Bn;
+    double vperp[3], vperp2 = 0.0;
+    for (int i = 0; i < 3; i++) vperp[i] = v[i] - vpar * (G.alpha * Bc[i]) / Bn;
+    for (int i = 1; i < 4; i++)
+      for (int j = 1; j < 4; j++) vperp2 += G.gcov[i][j] * vperp[i - 1] * vperp[j - 1];
+    const double mpar = (P[0] + par.gamma_ad * P[1]) * gamma * gamma * vpar;
+    if (lowr) { P[0] = rfl; st.rho_floor++; }
+    if (lowu) { P[1] = ufl; st.u_floor++; }
+    const double wn = P[0] + par.gamma_ad * P[1];
+    const double s = 1.0 - vperp2;
+    const double vparn = 2.0 * mpar * s / (wn + std::sqrt(wn * wn + 4.0 * mpar * mpar * s));
+    const double gn = 1.0 / std::sqrt(s - vparn * vparn);
+    for (int i = 0; i < 3; i++) P[2 + i] = gn * (vperp[i] + vparn * (G.alpha * Bc[i]) / Bn);
+  } else {
+    if (lowr) { P[0] = rfl; st.rho_floor++; }
+    if (lowu) { P[1] = ufl; st.u_floor++; }
+  }
   double q = 0.0;
   for (int i = 1; i < 4; i++)
     for (int j = 1; j < 4; j++) q += G.gcov[i][j] * P[1 + i] * P[1 + j];
@@ -522,8 +580,9 @@ void update(const Params& par, Block& b, const Fields& src, const Fields& base, 
         }
   }
   compute_Bc(b, out, true);
-  long long nfail = 0, nrf = 0, nuf = 0, ngc = 0;
-#pragma omp parallel for collapse(2) reduction(+ : nfail, nrf, nuf, ngc)
+  long long nfail = 0, nrf = 0, nuf = 0, ngc = 0, nent = 0;
+  if (par.entropy_backup) b.Kadv.assign(b.size(), 0.0);
+#pragma omp parallel for collapse(2) reduction(+ : nfail, nrf, nuf, ngc, nent)
   for (int i = 0; i < b.n[0]; i++)
     for (int j = 0; j < b.n[1]; j++) {
       const Geom& G = b.gc[b.idx2(i, j)];
@@ -547,17 +606,37 @@ void update(const Params& par, Block& b, const Fields& src, const Fields& base, 
         const double Bn[3] = {out.Bc[0][z], out.Bc[1][z], out.Bc[2][z]};
         double Pn[5];
         int rc = con2prim(U, Bn, G, par.gamma_ad, Ps, Pn, nullptr);
+        if (par.entropy_backup) {
+          // C-18: the entropy row, advanced like the others (no source term), and the backup inversion wherever
+          // the energy inversion failed or returned a state without positive density and non-negative energy
+          double USb, Fdummy;
+          entropy_UF(Pb, Sb, G, par.gamma_ad, 1, USb, Fdummy);
+          double div = 0.0;
+          for (int d = 0; d < 3; d++) div += (b.FK[d][z + str[d]] - b.FK[d][z]) / b.dx[d];
+          const double US = USb - dt * div;
+          b.Kadv[z] = US / U[0];
+          if (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) {
+            double Pe[5];
+            // an entropy row that went negative (kappa < 0) or has no root leaves what the energy inversion gave:
+            // its converged state for the floors to repair, or its failure
+            if (con2prim_entropy(U, US, Bn, G, par.gamma_ad, Ps, Pe, nullptr) == 0) {
+              for (int c = 0; c < 5; c++) Pn[c] = Pe[c];
+              rc = 0;
+              nent++;
+            }
+          }
+        }
         if (rc != 0) {  // C-13: keep the source state's hydro primitives, count the failure
           nfail++;
           for (int c = 0; c < 5; c++) Pn[c] = Ps[c];
         }
-        Stats loc = {0, 0, 0, 0};
-        floors_and_ceiling(par, G, r, Pn, loc);
+        Stats loc = {0, 0, 0, 0, 0};
+        floors_and_ceiling(par, G, r, Pn, Bn, loc);
         nrf += loc.rho_floor; nuf += loc.u_floor; ngc += loc.gam_ceil;
         for (int c = 0; c < 5; c++) out.P[c][z] = Pn[c];
       }
     }
-  st.c2p_fail += nfail; st.rho_floor += nrf; st.u_floor += nuf; st.gam_ceil += ngc;
+  st.c2p_entropy += nent; st.c2p_fail += nfail; st.rho_floor += nrf; st.u_floor += nuf; st.gam_ceil += ngc;
   deref_sync_groups(par, b, out);
 }
 

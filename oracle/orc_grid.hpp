@@ -45,6 +45,9 @@ struct Block {
   std::vector<double> FA2[3][5];   // R2: R1 summed over the two steps inside one step of the next
   std::vector<double> EA2[3];      //     coarser time level
   double ctop_last[3];             // ctop of this block's most recent corrector (or initial) pass
+  std::vector<double> K;           // C-18: kappa of the flux pass's source state, every zone incl. ghosts
+  std::vector<double> FK[3];       // C-18: entropy fluxes on d-faces
+  std::vector<double> Kadv;        // C-18: kappa the entropy row gives after the latest update (before it is reset)
   std::vector<double> F[3][5];     // hydro fluxes on d-faces
   std::vector<double> Ef[3][3];    // Ef[d][c]: E_c on d-faces, c != d (C-8)
   std::vector<double> Ee[3];       // edge EMFs (C-9)
@@ -60,7 +63,7 @@ struct Block {
   double xf(int d, int i) const { return x0[d] + (double)(I0[d] + i) * dx[d]; }
 };
 
-struct Stats { long long c2p_fail, rho_floor, u_floor, gam_ceil; };
+struct Stats { long long c2p_fail, rho_floor, u_floor, gam_ceil, c2p_entropy; };
 
 struct Grid {
   Params par;
@@ -116,6 +119,7 @@ void deref_fix_fluxes(const Params& par, Block& b);
 void deref_fix_edges(const Params& par, Block& b);
 void deref_sync_groups(const Params& par, Block& b, Fields& s);
 void deref_project(const Params& par, Block& b, Fields& s);
-void floors_and_ceiling(const Params& par, const Geom& G, double r, double P[5], Stats& st);
+// Bc: the zone's cell-centred field (read only with par.drift_floors; may be NULL)
+void floors_and_ceiling(const Params& par, const Geom& G, double r, double P[5], const double* Bc, Stats& st);
 
 }  // namespace orc

@@ -210,6 +210,111 @@ int con2prim(const double U[5], const double Bc[3], const Geom& G, double gam,
   return 0;
 }
 
+// ---- C-18: entropy advection and the backup inversion ("H-AMR also advects the entropy (Noble et al.
+// 2009), which is then used in place of the energy equation to recover the primitive variables") -----------------
+// For an ideal gas p = (gamma_ad - 1) u the quantity kappa = p / rho^gamma_ad is a function of the specific entropy
+// only, so along smooth adiabatic flow  d(kappa)/d(tau) = 0, which with mass conservation is the conservation law
+//   d_t (gdet rho kappa u^t) + d_i (gdet rho kappa u^i) = 0            (no source term).
+double entropy_kappa(double rho, double u, double gam) { return (gam - 1.0) * u / std::pow(rho, gam); }
+
+void entropy_UF(const double P[8], const State& S, const Geom& G, double gam, int dir, double& US, double& FS) {
+  const double k = entropy_kappa(P[0], P[1], gam);
+  US = G.gdet * P[0] * k * S.ucon[0];
+  FS = G.gdet * P[0] * k * S.ucon[dir];
+}
+
+// The inversion.  In the normal observer's frame (n_mu = (-alpha, 0, 0, 0)) the conserved rows give
+//   D = gamma rho,  Q_mu = alpha T^t_mu,  curly-B^i = alpha B^i,  and  alpha (rho kappa u^t) = D kappa,
+// so kappa = US / U[0] is known at once.  With  q = ut^2 = gamma^2 - 1  as the one unknown:
+//   rho = D / gamma,  p = kappa rho^gamma_ad,  w = rho + gamma_ad/(gamma_ad - 1) p,
+//   W(q) = w gamma^2 = D gamma + c kappa D^gamma_ad gamma^(2 - gamma_ad),   c = gamma_ad / (gamma_ad - 1),
+// and the squared momentum equation of Noble et al. 2006 (their Eq. 27, the f1 of con2prim above) closes it:
+//   f(q) = v^2 (Bsq + W)^2 - (Q.B)^2 (Bsq + 2 W) / W^2 - Qt^2 = 0,   v^2 = q / (1 + q).
+// W grows with q for gamma_ad < 2, each term of f grows with W and with v^2, f(0) <= 0 and f -> infinity: the
+// root exists and is unique.  It is found by Newton's method kept inside a bracket [lo, hi] (a step that leaves the
+// bracket is replaced by its midpoint), from the guess q of P_guess, until |dq| <= 1e-14 (1 + q); cap 100.
+int con2prim_entropy(const double U[5], double US, const double Bc[3], const Geom& G, double gam,
+                     const double Pguess[5], double Pout[5], int* iters) {
+  if (iters) *iters = 0;
+  const double ig = 1.0 / G.gdet;
+  const double alpha = G.alpha;
+  const double rhout = U[0] * ig;
+  const double D = alpha * rhout;
+  const double kappa = US / U[0];
+  if (!(D > 0.0) || !(kappa >= 0.0) || !std::isfinite(D) || !std::isfinite(kappa)) return 2;
+  // momentum rows exactly as in con2prim (the energy row U[1] is NOT read: Q_t follows from Q.n below only through
+  // the spatial rows, see Qtsq)
+  double Qcov[4] = {0.0, alpha * U[2] * ig, alpha * U[3] * ig, alpha * U[4] * ig};
+  double Bs[4] = {0.0, alpha * Bc[0], alpha * Bc[1], alpha * Bc[2]};
+  // Qt^2 = Qt_i Qt^i with Qt_mu = Q_mu + (Q.n) n_mu: its spatial covariant part is Q_i itself (n_i = 0), and for a
+  // vector orthogonal to n the square is the 3-metric's inverse applied to the spatial part:
+  //   Qt^2 = gamma^ij Q_i Q_j,  gamma^ij = g^ij + beta^i beta^j / alpha^2   (so Q_t is never needed)
+  double Qtsq = 0.0, Qtcon[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int i = 1; i < 4; i++) {
+    double acc = 0.0;
+    for (int j = 1; j < 4; j++)
+      acc += (G.gcon[i][j] + G.beta[i - 1] * G.beta[j - 1] / (alpha * alpha)) * Qcov[j];
+    Qtcon[i] = acc;
+    Qtsq += Qcov[i] * acc;
+  }
+  double QdB = 0.0, Bsq = 0.0;
+  for (int i = 1; i < 4; i++) {
+    QdB += Qcov[i] * Bs[i];
+    for (int j = 1; j < 4; j++) Bsq += G.gcov[i][j] * Bs[i] * Bs[j];
+  }
+  const double QdB2 = QdB * QdB;
+  const double c = gam / (gam - 1.0);
+  const double A = c * kappa * std::pow(D, gam);  // W = D g + A g^(2 - gamma_ad)
+  if (!std::isfinite(Qtsq) || !std::isfinite(Bsq) || !std::isfinite(A)) return 2;
+
+  auto feval = [&](double q, double& W, double& df) {
+    const double g = std::sqrt(1.0 + q);
+    const double gp = std::pow(g, -gam);            // g^(-gamma_ad)
+    W = D * g + A * gp * (1.0 + q);                 // g^(2 - gamma_ad) = g^(-gamma_ad) (1 + q)
+    const double dW = D / (2.0 * g) + A * 0.5 * (2.0 - gam) * gp;
+    const double v2 = q / (1.0 + q), BW = Bsq + W;
+    const double W2 = W * W, W3 = W2 * W;
+    df = BW * BW / ((1.0 + q) * (1.0 + q)) + 2.0 * BW * dW * (v2 + QdB2 / W3);
+    return v2 * BW * BW - QdB2 * (Bsq + 2.0 * W) / W2 - Qtsq;
+  };
+  double W, df;
+  // bracket: f(0) <= 0; hi grows by factors of 4 from 1 until f(hi) >= 0
+  double lo = 0.0, hi = 1.0;
+  int nb = 0;
+  while (feval(hi, W, df) < 0.0) {
+    lo = hi;
+    hi *= 4.0;
+    if (++nb > 60) return 1;
+  }
+  double q = 0.0;
+  for (int i = 1; i < 4; i++)
+    for (int j = 1; j < 4; j++) q += G.gcov[i][j] * Pguess[1 + i] * Pguess[1 + j];
+  if (!(q > lo && q < hi)) q = 0.5 * (lo + hi);
+  bool conv = false;
+  int it;
+  for (it = 0; it < 100; it++) {
+    const double f = feval(q, W, df);
+    if (!std::isfinite(f) || !std::isfinite(df)) { if (iters) *iters = it; return 2; }
+    if (f < 0.0) lo = q; else hi = q;
+    double qn = q - f / df;
+    if (!(qn > lo && qn < hi)) qn = 0.5 * (lo + hi);
+    const double dq = qn - q;
+    q = qn;
+    if (std::fabs(dq) <= 1e-14 * (1.0 + q)) { conv = true; it++; break; }
+  }
+  if (iters) *iters = it;
+  if (!conv) return 1;
+  feval(q, W, df);
+  const double gamma = std::sqrt(1.0 + q);
+  const double rho = D / gamma;
+  const double u = kappa * std::pow(rho, gam) / (gam - 1.0);
+  if (!std::isfinite(rho) || !std::isfinite(u) || !std::isfinite(W)) return 2;
+  Pout[0] = rho;
+  Pout[1] = u;
+  for (int i = 1; i < 4; i++) Pout[1 + i] = gamma / (W + Bsq) * (Qtcon[i] + QdB * Bs[i] / W);
+  return 0;
+}
+
 // C-5 PPM (Colella & Woodward 1984) on a uniform grid, zone j = a[2]
 static double ppm_slope(double am, double a0, double ap) {
   const double dl = a0 - am, dr = ap - a0;

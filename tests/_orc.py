@@ -19,6 +19,7 @@ class Params(C.Structure):
                 ("bc_lo", C.c_int32 * 3), ("bc_hi", C.c_int32 * 3), ("nb", C.c_int32 * 3),
                 ("n_deref", C.c_int32), ("deref_factor", C.c_int32 * 4),
                 ("lat_max_level", C.c_int32), ("map", C.c_int32),
+                ("entropy_backup", C.c_int32), ("drift_floors", C.c_int32),
                 ("a", C.c_double), ("xmin", C.c_double * 3), ("xmax", C.c_double * 3),
                 ("gamma_ad", C.c_double), ("cour", C.c_double),
                 ("rho_fl_coef", C.c_double), ("rho_fl_pow", C.c_double),
@@ -72,7 +73,13 @@ def lib():
         L.orc_source.argtypes = [c_double_p, C.POINTER(Geom), c_double_p, C.c_double, c_double_p]
         L.orc_con2prim.argtypes = [c_double_p, c_double_p, C.POINTER(Geom), C.c_double, c_double_p,
                                    c_double_p, C.POINTER(C.c_int)]
-        L.orc_floors.argtypes = [C.POINTER(Params), C.POINTER(Geom), C.c_double, c_double_p, C.POINTER(C.c_longlong)]
+        L.orc_floors.argtypes = [C.POINTER(Params), C.POINTER(Geom), C.c_double, c_double_p, c_double_p,
+                                 C.POINTER(C.c_longlong)]
+        L.orc_con2prim_entropy.argtypes = [c_double_p, C.c_double, c_double_p, C.POINTER(Geom), C.c_double,
+                                           c_double_p, c_double_p, C.POINTER(C.c_int)]
+        L.orc_entropy_UF.argtypes = [c_double_p, C.POINTER(Geom), C.c_double, C.c_int, c_double_p, c_double_p]
+        L.orc_get_backup_count.argtypes = [C.c_void_p, C.POINTER(C.c_longlong)]
+        L.orc_get_kadv.argtypes = [C.c_void_p, c_double_p]
         L.orc_ppm_zone.argtypes = [c_double_p] * 3
         L.orc_plm_zone.argtypes = [c_double_p] * 3
         L.orc_hll.argtypes = [c_double_p] * 4 + [C.c_double, C.c_double, c_double_p]
@@ -107,6 +114,8 @@ def pack_params(p: dict) -> Params:
     q.u_fl_coef, q.u_fl_pow = float(p["u_fl_coef"]), float(p["u_fl_pow"])
     q.gamma_max = float(p["gamma_max"])
     q.r_refine_max = float(p["r_refine_max"])
+    q.entropy_backup = int(p.get("entropy_backup", 0))
+    q.drift_floors = int(p.get("drift_floors", 0))
     return q
 
 
@@ -186,6 +195,17 @@ class OrcGrid:
         c = (C.c_longlong * 4)()
         self.L.orc_get_stats(self.h, c)
         return tuple(c[:])
+
+    def backup_count(self):
+        v = C.c_longlong(0)
+        self.L.orc_get_backup_count(self.h, C.byref(v))
+        return v.value
+
+    def kadv(self):
+        out = np.empty(self.n)
+        rc = self.L.orc_get_kadv(self.h, _dp(out))
+        assert rc == 0
+        return out
 
     def totals(self):
         t = np.zeros(5)
@@ -337,13 +357,31 @@ def con2prim(U5, Bc, G, gam, Pguess):
     return rc, out, it.value
 
 
-def floors(p, G, r, P5):
-    """floors and Lorentz-factor ceiling (C-13) on one zone: new P5, (rho-floor, u-floor, ceiling) hits"""
+def floors(p, G, r, P5, Bc=None):
+    """floors and Lorentz-factor ceiling (C-13; C-19 with p["drift_floors"] and a field Bc) on one zone: new P5,
+    (rho-floor, u-floor, ceiling) hits"""
     par = pack_params(p)
     P = _arr(P5).copy()
     c = (C.c_longlong * 3)()
-    lib().orc_floors(C.byref(par), C.byref(G), float(r), _dp(P), c)
+    B = _arr(Bc) if Bc is not None else None
+    lib().orc_floors(C.byref(par), C.byref(G), float(r), _dp(P), _dp(B) if B is not None else None, c)
     return P, tuple(c[:])
+
+
+def con2prim_entropy(U5, US, Bc, G, gam, Pguess):
+    """C-18: inversion with the entropy row US in place of the energy row"""
+    U5, Bc, Pg = _arr(U5), _arr(Bc), _arr(Pguess)
+    out = np.zeros(5)
+    it = C.c_int(0)
+    rc = lib().orc_con2prim_entropy(_dp(U5), float(US), _dp(Bc), C.byref(G), gam, _dp(Pg), _dp(out), C.byref(it))
+    return rc, out, it.value
+
+
+def entropy_UF(P, G, gam, direction):
+    P = _arr(P)
+    a, b = np.zeros(1), np.zeros(1)
+    lib().orc_entropy_UF(_dp(P), C.byref(G), gam, direction, _dp(a), _dp(b))
+    return a[0], b[0]
 
 
 def ppm_zone(a5):
