@@ -3,7 +3,7 @@
 fraction of the dominant kernel, the end-to-end number through the C-ABI with host buffers, and the
 CPU oracle timed beside it.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg1|cfg0|cfg3|cfg4b|cfg4|cfg4t|paper150]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg2r|cfg1|cfg0|cfg3|cfg4b|cfg4|cfg4t|paper150]
 
 A "step" is one full pass of the hot path over the whole grid: hamr_step(1) = predictor + corrector
 = one zone-cycle per zone.  Default workload: BASELINE.json configs[2], the 256x128x128
@@ -37,6 +37,12 @@ def workload(name, n_override=None):
         # n_override: the reference arm's bounded sample (run_reference) only
         p = I.torus_params(n=n_override or (256, 128, 128), r_out=1000.0)
         return p, (lambda: I.fm_torus(p, seed=2)), "BASELINE cfg2: Kerr FM torus 256x128x128 fp64, a=0.9375, PPM+HLL+CT"
+    if name == "cfg2r":
+        # cfg 2 with the robust inversion path on: ninth conserved row, entropy inversion where
+        # the energy inversion fails, drift-frame floors; runs on the generic kernels
+        p = I.torus_params(n=n_override or (256, 128, 128), r_out=1000.0, entropy_backup=1, drift_floors=1)
+        return p, (lambda: I.fm_torus(p, seed=2)), ("cfg2 with entropy advection + backup inversion and drift-frame floors "
+                                                    "(NEXT-2): Kerr FM torus 256x128x128 fp64")
     if name == "cfg0":
         p = I.torus_params()
         return p, (lambda: I.fm_torus(p, seed=0)), "BASELINE cfg0: tiny Kerr FM torus 32x16x16"
@@ -296,7 +302,7 @@ def main():
         return run_reference(args)
     if args.steps is None:
         # BASELINE cfg 2 runs 200 steps (0.6 s on a B200: long enough for the clock sampler to see the load)
-        args.steps = 200 if args.workload in ("cfg2", "cfg1", "cfg0", "paper150") else 20
+        args.steps = 200 if args.workload in ("cfg2", "cfg2r", "cfg1", "cfg0", "paper150") else 20
     args.warmup = max(args.warmup, 3)
 
     import torch

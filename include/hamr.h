@@ -66,6 +66,8 @@ typedef struct {
   int deref_factor[4];   /* derefinement factor per threshold (see "phi-derefinement" below)            */
   int lat_max_level;     /* local adaptive time-stepping levels; 0 = global dt    */
   int map;               /* hamr_map_t                                                           */
+  int entropy_backup;    /* 1: advect the entropy and invert with it where the energy inversion fails */
+  int drift_floors;      /* 1: floors inject mass / energy in the drift frame; 0: fluid frame        */
   double a;              /* black-hole spin (ignored for Minkowski)                              */
   double xmin[3], xmax[3]; /* PHYSICAL extents: (r_in, r_out), (0, pi), (0, 2pi), or the box.  On the spherical
                             map x2 must span exactly (0, pi) with a polar boundary kind on both sides: the faces
@@ -123,9 +125,27 @@ int hamr_get_bface(hamr_grid* g, double* const bface[3]);
 int hamr_divb(hamr_grid* g, double* max_norm_divb);
 /* counts since the last call: con2prim failures, rho-floor, u-floor, gamma-ceiling hits */
 int hamr_get_stats(hamr_grid* g, long long counts[4]);
+/* zones, since the last call, whose primitives came from the entropy inversion (entropy_backup; see below) */
+int hamr_get_backup_count(hamr_grid* g, long long* n);
 int hamr_get_time(hamr_grid* g, double* t, double* dt_next);
 int hamr_set_dt(hamr_grid* g, double dt_next); /* overrides the next step's dt (run-to-time) */
 const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the next call on g */
+
+/* ---- robust inversion path (C-18, C-19) ------------------------ */
+/* entropy_backup = 1 ("H-AMR also advects the entropy (Noble et al. 2009), which is then used in place of
+ * the energy equation to recover the primitive variables"): a ninth conserved row, sqrt(-g) rho u^t kappa with
+ * kappa = p / rho^gamma_ad, is advanced in every stage beside the others (HLL flux of the reconstructed kappa, no
+ * source term) and, wherever the 2-unknown energy inversion does not converge or returns rho <= 0 or u < 0, the zone
+ * is inverted from the density, momentum and entropy rows instead (one unknown, bracketed Newton).  kappa is reset
+ * from the new primitives after every update, so the state handed in and out stays the eight primitives.  A zone
+ * whose entropy row has no admissible root (kappa < 0) keeps what the energy inversion gave it: its converged state,
+ * for the floors to repair, or the failure path of hamr_get_stats counts[0].  Needs gamma_ad < 2.
+ * drift_floors = 1 ("injects mass and internal energy in the drift frame of the jet ... (Ressler et al.
+ * 2017)"): a zone below a floor is raised to it with the velocity perpendicular to the magnetic field unchanged and
+ * the momentum along the field, (rho + gamma_ad u) gamma^2 v_par, conserved; zones without field get the fluid-frame
+ * floors.  The Lorentz-factor ceiling follows as before.
+ * Both options need a grid of one block (nb = 0, no LAT, no derefinement, no refinement), else HAMR_EINVAL; such a
+ * grid then runs on the generic kernels (the shared-memory staged ones carry eight variables). */
 
 /* ---- block-structured grid (BASELINE.json cfg 4) ------------------ */
 /* A grid with nb != {0,0,0} or lat_max_level > 0 is cut into blocks of nb zones (nb[d] = 0: the whole

@@ -22,7 +22,8 @@ int hamr_set_levels(hamr_grid* g, const int* tau);
 /* Runs ghost fill + flux pass + CT EMFs on the current state (no update). */
 int hamr_debug_emf(hamr_grid* g);
 /* which 0..4: hydro flux F^d[c] of the last flux pass; 5, 6: the two face EMFs E_e, E_f with
- * (d, e, f) cyclic (C-8).  out: d-face array, extent n[d]+1 along d. */
+ * (d, e, f) cyclic (C-8); 7: the flux of the entropy row (entropy_backup grids, C-18).
+ * out: d-face array, extent n[d]+1 along d. */
 int hamr_get_face(hamr_grid* g, int d, int which, double* out);
 /* edge EMF E_f (extent n+1 along the two directions != f). */
 int hamr_get_edge(hamr_grid* g, int f, double* out);
@@ -63,6 +64,17 @@ int hamr_debug_con2prim(hamr_grid* g, int n, const int* ti, const int* tj, const
 /* Floors and Lorentz-factor ceiling applied to P (n x 5, in place); flags[s] bit 0: rho floor, 1: u floor,
  * 2: ceiling.  The floor of state s is that of x1 table index ti[s]. */
 int hamr_debug_floors(hamr_grid* g, int n, const int* ti, const int* tj, double* P, int* flags);
+
+/* ---- robust inversion path (C-18, C-19) ------------------------------------------------------------------ */
+/* kappa = (entropy row) / (density row) that the latest update stage advected, on the active zones (N1*N2*N3), before
+ * it was reset from the new primitives.  entropy_backup grids only. */
+int hamr_debug_kappa(hamr_grid* g, double* out);
+/* The entropy inversion as the update kernel runs it: U (n x 5; the energy row U[.][1] is not read), entropy row US (n),
+ * new field Bc (n x 3), guess (n x 5) -> out (n x 5), rc (n): 0 ok, 1 no admissible root (out then holds the guess). */
+int hamr_debug_con2prim_entropy(hamr_grid* g, int n, const int* ti, const int* tj, const double* U, const double* US,
+                                const double* Bc, const double* guess, double* out, int* rc);
+/* hamr_debug_floors with the zone's field Bc (n x 3): drift-frame floors (C-19) when the grid has drift_floors = 1 */
+int hamr_debug_floors_drift(hamr_grid* g, int n, const int* ti, const int* tj, double* P, const double* Bc, int* flags);
 
 /* ---- FP64 pipe peak ("measure it with an FMA-chain microbenchmark") ---------------------------------- */
 /* Runs `iters` rounds of 8 independent dependent-chains of FP64 instructions per thread on every SM of the current

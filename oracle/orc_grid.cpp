@@ -246,9 +246,10 @@ static void face_flux_core(const Params& par, Block& b, const Fields& s, int d, 
     // the entropy row (C-18) through the same HLL formula: U_S = gdet rho kappa u^t, F_S = gdet rho kappa u^d with the
     // reconstructed kappa; gdet rho u^t and gdet rho u^d are row 0 of U and F
     const double USL = UL[0] * kL, USR = UR[0] * kR, FSL = FL[0] * kL, FSR = FR[0] * kR;
-    double U2L[8] = {USL}, U2R[8] = {USR}, F2L[8] = {FSL}, F2R[8] = {FSR}, F2[8];
+    // (slot 1: slot 0 of hll is the mass row with its C-7a flush, which does not apply here)
+    double U2L[8] = {0.0, USL}, U2R[8] = {0.0, USR}, F2L[8] = {0.0, FSL}, F2R[8] = {0.0, FSR}, F2[8];
     hll(U2L, U2R, F2L, F2R, cmin, cmax, F2);
-    b.FK[d][z] = F2[0];
+    b.FK[d][z] = F2[1];
   }
   if (ctop) *ctop = std::max(cmax, cmin);
 }

@@ -82,6 +82,14 @@ bool params_ok(const hamr_params& p, std::string& why) {
     }
   }
   if (p.lat_max_level < 0 || p.lat_max_level > 3) { why = "lat_max_level must be 0..3"; return false; }
+  if ((p.entropy_backup & ~1) || (p.drift_floors & ~1)) { why = "entropy_backup / drift_floors are 0 or 1"; return false; }
+  if (p.entropy_backup || p.drift_floors) {   // NEXT-2 (C-18, C-19) is built for the monolithic grid
+    if (is_block_grid(p) || p.n_deref > 0 || p.r_refine_max > 0.0) {
+      why = "entropy_backup / drift_floors need a grid of one block without derefinement";
+      return false;
+    }
+    if (p.entropy_backup && !(p.gamma_ad < 2.0)) { why = "the entropy inversion needs gamma_ad < 2"; return false; }
+  }
   if (is_block_grid(p)) {
     int ns[3], bn[3];
     if (p.nb[0] < 0 || p.nb[1] < 0 || p.nb[2] < 0 || blk_count(p, ns, bn) <= 0) {
@@ -120,7 +128,7 @@ bool make_layout(const hamr_params& p, Lay& L, GridShape& G) {
   G.te1 = G.nlev * p.n[0] + 2 * NG + 1;   // the level-1 table is indexed in fine zones
   G.te2 = p.n[1] + 2 * NG + 1;
   L.n2d = G.te1 * G.te2;
-  G.narr = N_ARR + ((G.nblk > 0 && p.lat_max_level > 0) ? N_REG_ARR : 0);
+  G.narr = N_ARR + ((G.nblk > 0 && p.lat_max_level > 0) ? N_REG_ARR : 0) + (p.entropy_backup ? 4 : 0);
   return true;
 }
 
@@ -247,9 +255,15 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   for (int d = 0; d < 3; d++) D.EfB[d] = next();
   for (int d = 0; d < 3; d++) D.Ee[d] = next();
   for (int d = 0; d < 3; d++) D.Cc[d] = next();
-  if (gs.narr > N_ARR) {
+  if (gs.nblk > 0 && p->lat_max_level > 0) {
     for (int d = 0; d < 3; d++) for (int c = 0; c < 5; c++) D.B.FA2[d][c] = next();
     for (int d = 0; d < 3; d++) D.B.EA2[d] = next();
+  }
+  D.entropy = p->entropy_backup;
+  D.drift = p->drift_floors;
+  if (D.entropy) {   // C-18: kappa of the stage source and the entropy flux per direction
+    D.K = next();
+    for (int d = 0; d < 3; d++) D.FK[d] = next();
   }
   D.B.nblk = gs.nblk;
   D.B.blen = gs.blen;
@@ -594,6 +608,16 @@ int hamr_get_stats(hamr_grid* g, long long counts[4]) {
   return HAMR_OK;
 }
 
+int hamr_get_backup_count(hamr_grid* g, long long* n) {
+  if (!g || !n) return HAMR_EINVAL;
+  unsigned long long* h = (unsigned long long*)(g->h_pinned + 32);
+  CK(cudaMemcpyAsync(h, g->D.cnt + N_ENTROPY, sizeof(unsigned long long), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaMemsetAsync(g->D.cnt + N_ENTROPY, 0, sizeof(unsigned long long), g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  *n = (long long)h[0];
+  return HAMR_OK;
+}
+
 int hamr_get_time(hamr_grid* g, double* t, double* dt_next) {
   if (!g) return HAMR_EINVAL;
   double v[2];
@@ -774,9 +798,18 @@ int hamr_debug_emf(hamr_grid* g) {
 }
 
 int hamr_get_face(hamr_grid* g, int d, int which, double* out) {
-  if (!g || !out || d < 0 || d > 2 || which < 0 || which > 6) return HAMR_EINVAL;
-  const double* a = which < 5 ? g->D.F[d][which] : (which == 5 ? g->D.EfA[d] : g->D.EfB[d]);
+  if (!g || !out || d < 0 || d > 2 || which < 0 || which > 7 || (which == 7 && !g->D.entropy)) return HAMR_EINVAL;
+  const double* a = which == 7 ? g->D.FK[d] : (which < 5 ? g->D.F[d][which] : (which == 5 ? g->D.EfA[d] : g->D.EfB[d]));
   int rc = get_dense(g, a, out, d, false, 0);
+  if (rc != HAMR_OK) return rc;
+  CK(cudaStreamSynchronize(g->stream));
+  return HAMR_OK;
+}
+
+int hamr_debug_kappa(hamr_grid* g, double* out) {
+  if (!g || !out || !g->D.entropy) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  int rc = get_dense(g, g->D.K, out, -1, false, 0);
   if (rc != HAMR_OK) return rc;
   CK(cudaStreamSynchronize(g->stream));
   return HAMR_OK;

@@ -9,7 +9,8 @@ using namespace hamr;
 
 namespace {
 
-// one thread per state: what (0 prim -> U, 1 U -> prim, 2 floors / ceiling) on the centre record of entry q[s]
+// one thread per state: what (0 prim -> U, 1 U -> prim, 2 floors / ceiling, 3 entropy inversion, 4 floors with the
+// zone's field) on the centre record of entry q[s]
 __global__ void k_zone_physics(Dev Dv, int what, int n, const int* __restrict__ q, const int* __restrict__ ti,
                                const double* __restrict__ in, const double* __restrict__ in2,
                                const double* __restrict__ in3, double* __restrict__ out, int* __restrict__ iout) {
@@ -30,11 +31,27 @@ __global__ void k_zone_physics(Dev Dv, int what, int n, const int* __restrict__ 
     const int rc = con2prim(U, Bc, G, Dv.gam, Pg, Pn);
     for (int c = 0; c < 5; c++) out[(size_t)s * 5 + c] = rc == 0 ? Pn[c] : Pg[c];   // C-13: a failed zone keeps its guess
     iout[s] = rc;
+  } else if (what == 3) {   // C-18: in = (U[5], US) per state
+    double U[5], Bc[3], Pg[5], Pn[5];
+    for (int c = 0; c < 5; c++) { U[c] = in[(size_t)s * 6 + c]; Pg[c] = in3[(size_t)s * 5 + c]; }
+    for (int c = 0; c < 3; c++) Bc[c] = in2[(size_t)s * 3 + c];
+    const int rc = con2prim_entropy(U, in[(size_t)s * 6 + 5], Bc, &G, Dv.gam, Pg, Pn);
+    for (int c = 0; c < 5; c++) out[(size_t)s * 5 + c] = rc == 0 ? Pn[c] : Pg[c];
+    iout[s] = rc;
   } else {
     double P[5];
     for (int c = 0; c < 5; c++) P[c] = out[(size_t)s * 5 + c];
     int nrf = 0, nuf = 0, ngc = 0;
-    floors_ceiling(G, Dv.rho_fl[ti[s]], Dv.u_fl[ti[s]], Dv.gamma_max, P, nrf, nuf, ngc);
+    const double rfl = Dv.rho_fl[ti[s]], ufl = Dv.u_fl[ti[s]];
+    if (what == 4 && Dv.drift) {   // C-19, as k_update applies it
+      double Bc[3];
+      for (int c = 0; c < 3; c++) Bc[c] = in2[(size_t)s * 3 + c];
+      nrf = P[0] < rfl;
+      nuf = P[1] < ufl;
+      if (nrf | nuf) floors_drift(&G, Bc, Dv.gam, nrf ? rfl : P[0], nuf ? ufl : P[1], P);
+      ceiling_only(G, Dv.gamma_max, P, ngc);
+    } else
+    floors_ceiling(G, rfl, ufl, Dv.gamma_max, P, nrf, nuf, ngc);
     for (int c = 0; c < 5; c++) out[(size_t)s * 5 + c] = P[c];
     iout[s] = nrf | (nuf << 1) | (ngc << 2);
   }
@@ -150,6 +167,22 @@ int hamr_debug_con2prim(hamr_grid* g, int n, const int* ti, const int* tj, const
 int hamr_debug_floors(hamr_grid* g, int n, const int* ti, const int* tj, double* P, int* flags) {
   if (!flags) return HAMR_EINVAL;
   return zone_call(g, 2, n, ti, tj, nullptr, 0, nullptr, 0, nullptr, 0, P, true, flags);
+}
+
+int hamr_debug_con2prim_entropy(hamr_grid* g, int n, const int* ti, const int* tj, const double* U, const double* US,
+                                const double* Bc, const double* guess, double* out, int* rc) {
+  if (!U || !US || !Bc || !guess || !rc || n < 0) return HAMR_EINVAL;
+  std::vector<double> u6((size_t)n * 6);
+  for (int s = 0; s < n; s++) {
+    for (int c = 0; c < 5; c++) u6[(size_t)s * 6 + c] = U[(size_t)s * 5 + c];
+    u6[(size_t)s * 6 + 5] = US[s];
+  }
+  return zone_call(g, 3, n, ti, tj, u6.data(), 6, Bc, 3, guess, 5, out, false, rc);
+}
+
+int hamr_debug_floors_drift(hamr_grid* g, int n, const int* ti, const int* tj, double* P, const double* Bc, int* flags) {
+  if (!flags || !Bc) return HAMR_EINVAL;
+  return zone_call(g, 4, n, ti, tj, nullptr, 0, Bc, 3, nullptr, 0, P, true, flags);
 }
 
 int hamr_bench_fp64(void* cuda_stream, int mix, int iters, double* seconds, double* thread_instructions) {

@@ -165,10 +165,12 @@ __device__ __forceinline__ void side_state(const double P[8], const FGeo& G, dou
   S.vm = disc - h;
 }
 
-// HLL (C-7) from the two states: the 7 outputs of the face (5 hydro fluxes, E_f, E_e); returns ctop
-template <int D>
-__device__ __forceinline__ double face_flux(const double PL[8], const double PR[8], const FGeo& G, double gam_ad,
-                                            double out[7]) {
+// HLL (C-7) from the two states: the 7 outputs of the face (5 hydro fluxes, E_f, E_e); returns ctop.
+// ENT (C-18): PL[8], PR[8] hold the reconstructed kappa and out[7] receives the flux of the entropy row, which is
+// carried by the two parts of the mass flux: kappa_L (rho X)_L + kappa_R (rho X)_R (no flush: C-7a is about CT)
+template <int D, bool ENT = false>
+__device__ __forceinline__ double face_flux(const double* __restrict__ PL, const double* __restrict__ PR, const FGeo& G,
+                                            double gam_ad, double* __restrict__ out) {
   constexpr int dir = D + 1;
   Side L, R;
   side_state<D>(PL, G, gam_ad, L);
@@ -186,6 +188,7 @@ __device__ __forceinline__ double face_flux(const double PL[8], const double PR[
   const double wc = wl * cmin;              // avg: cmin = 0
   const double XL = wl * L.ud + wc * L.ut, XR = wr * R.ud - wc * R.ut;
   double Fh0 = L.rho * XL + R.rho * XR;
+  if (ENT) out[7] = PL[8] * (L.rho * XL) + PR[8] * (R.rho * XR);
   // C-7a: a mass flux below 1e-12 of the magnitude of its own HLL terms is rounding noise and is
   // flushed to exactly 0, so that the upwind selector of C-9 sees a tie
   const double mag = L.rho * (wl * fabs(L.ud) + wc * L.ut) + R.rho * (wr * fabs(R.ud) + wc * R.ut);
@@ -214,12 +217,13 @@ __device__ __forceinline__ void store_face(const Dev& Dv, int D, int z, const do
 }
 
 // all three kinds of call sites: HLL on one face, results to the face arrays at z
-template <int D>
-__device__ __forceinline__ double face_flux(const double PL[8], const double PR[8], const FGeo& G, double gam_ad,
-                                            const Dev& Dv, int z) {
-  double out[7];
-  const double ct = face_flux<D>(PL, PR, G, gam_ad, out);
+template <int D, bool ENT = false>
+__device__ __forceinline__ double face_flux(const double* __restrict__ PL, const double* __restrict__ PR, const FGeo& G,
+                                            double gam_ad, const Dev& Dv, int z) {
+  double out[8];
+  const double ct = face_flux<D, ENT>(PL, PR, G, gam_ad, out);
   store_face(Dv, D, z, out);
+  if (ENT) Dv.FK[D][z] = out[7];
   return ct;
 }
 
@@ -227,6 +231,7 @@ __device__ __forceinline__ void zero_face(const Dev& Dv, int D, int z) {
   for (int c = 0; c < 5; c++) Dv.F[D][c][z] = 0.0;
   Dv.EfA[D][z] = 0.0;
   Dv.EfB[D][z] = 0.0;
+  if (Dv.entropy) Dv.FK[D][z] = 0.0;
 }
 
 // C-14 / H5: per-direction maximum signal speed: warp-shuffle max, then one atomic max per warp on the
@@ -258,9 +263,10 @@ __device__ __forceinline__ void ctop_commit(const Dev& Dv, int D, int b, double 
 constexpr int MARCH_T = 128, MARCH_MINB = 4, X3_MINB = 5;
 // BLK: the launch covers the blocks of Dv.B.list (block-structured grid, H7); s / s2 are the buffer sets
 // holding the stage source of blocks with cur == 0 / cur == 2.
-template <int D, int RECON, bool BLK>
-__global__ void __launch_bounds__(MARCH_T, MARCH_MINB) k_flux_march(Dev Dv, Fields s, Fields s2, int seg,
-                                                                      int want_ctop) {
+// ENT (C-18, monolithic grids): kappa of the zones (Dv.K) is reconstructed as an eighth variable for the entropy flux.
+template <int D, int RECON, bool BLK, bool ENT = false>
+__global__ void __launch_bounds__(MARCH_T, ENT ? 3 : MARCH_MINB) k_flux_march(Dev Dv, Fields s, Fields s2, int seg,
+                                                                                int want_ctop) {
   static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   const Lay& L = Dv.L;
   constexpr int O = 1 - D;          // the other non-x3 dimension
@@ -280,19 +286,20 @@ __global__ void __launch_bounds__(MARCH_T, MARCH_MINB) k_flux_march(Dev Dv, Fiel
     const int sd = (D == 0) ? L.S1 : L.S2;
     const bool act = o >= 0 && o < L.n[O] && k >= 0 && k < L.n[2];  // C-14: faces of ACTIVE zones
     const bool ks = Dv.metric == HAMR_METRIC_KERR_SCHILD;
-    const double* var[7] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
+    constexpr int NVR = ENT ? 8 : 7;   // reconstructed variables
+    const double* var[8] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
                             selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),
                             selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[e], s2.Bc[e], C.cur),
-                            selp<BLK>(s.Bc[f], s2.Bc[f], C.cur)};
+                            selp<BLK>(s.Bc[f], s2.Bc[f], C.cur), Dv.K};
     const double* bfn = selp<BLK>(s.Bf[D], s2.Bf[D], C.cur);
     const double* gtab = (D == 0 ? Dv.gf1A : Dv.gf2A) + (BLK ? C.lev * Dv.B.tlevA : 0);
-    constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
+    constexpr int slot[8] = {0, 1, 2, 3, 4, 5 + e, 5 + f, 8};
     int z = C.zoff + (int)L.idx(D == 0 ? f0 - 1 : o, D == 0 ? o : f0 - 1, k);
-    double PL[8], PR[8];
-    double dm[7], il[7];  // PPM marching state (unused for PLM)
+    double PL[9], PR[9];
+    double dm[8], il[8];  // PPM marching state (unused for PLM)
     // the zone below the first face: its right edge, and the marching state of the next zone
 #pragma unroll
-    for (int v = 0; v < 7; v++) {
+    for (int v = 0; v < NVR; v++) {
       const double* a = var[v] + z;
       if (RECON == HAMR_RECON_PPM) {
         const double m2 = a[-2 * sd], m1 = a[-sd], c0 = a[0], p1 = a[sd], p2 = a[2 * sd];
@@ -311,9 +318,9 @@ __global__ void __launch_bounds__(MARCH_T, MARCH_MINB) k_flux_march(Dev Dv, Fiel
     }
     for (int fc = f0; fc < f1; fc++) {
       z += sd;
-      double carry[7];
+      double carry[8];
 #pragma unroll
-      for (int v = 0; v < 7; v++) {
+      for (int v = 0; v < NVR; v++) {
         const double* a = var[v] + z;
         if (RECON == HAMR_RECON_PPM) {
           const double a2 = a[2 * sd];
@@ -334,11 +341,11 @@ __global__ void __launch_bounds__(MARCH_T, MARCH_MINB) k_flux_march(Dev Dv, Fiel
         const int q = C.q0 + ((D == 0) ? fc * ge2 + o : o * ge2 + fc);
         const FGeo G = load_fgeo(gtab + (size_t)q * NREC_F);
         PL[5 + D] = PR[5 + D] = bfn[z] * G.igdet;  // C-5: the normal field is single-valued at the face
-        const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
+        const double ct = face_flux<D, ENT>(PL, PR, G, Dv.gam, Dv, z);
         if (act) ctop = dmax(ctop, ct);
       }
 #pragma unroll
-      for (int v = 0; v < 7; v++) PL[slot[v]] = carry[v];
+      for (int v = 0; v < NVR; v++) PL[slot[v]] = carry[v];
     }
   }
   if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
@@ -505,8 +512,8 @@ __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, 
 // WRAP (monolithic grids with a periodic x3, the grids the ring kernels serve): the stencil wraps inside the row and
 // the face at k = n3 is stored as the periodic image of the face at k = 0, so the x3 ghost zones are never read and the
 // per-stage ghost fill skips them (x3_ghosts_unused; bc.cu)
-template <int RECON, bool BLK, bool WRAP>
-__global__ void __launch_bounds__(128, X3_MINB) k_flux_x3(Dev Dv, Fields s, Fields s2, int want_ctop) {
+template <int RECON, bool BLK, bool WRAP, bool ENT = false>
+__global__ void __launch_bounds__(128, ENT ? 4 : X3_MINB) k_flux_x3(Dev Dv, Fields s, Fields s2, int want_ctop) {
   constexpr int D = 2;
   constexpr int HLO = (RECON == HAMR_RECON_PPM) ? 2 : 1, HHI = (RECON == HAMR_RECON_PPM) ? 1 : 0;
   constexpr int OWN = 32 - HLO - HHI;
@@ -537,17 +544,19 @@ __global__ void __launch_bounds__(128, X3_MINB) k_flux_x3(Dev Dv, Fields s, Fiel
     auto wr = [n3](int q) { return q < 0 ? q + n3 : (q >= n3 ? q - n3 : q); };
     om = wr(k - 1) - k; o0 = wr(k) - k; op = wr(k + 1) - k;
   }
-  const double* var[7] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
+  constexpr int NVR = ENT ? 8 : 7;   // reconstructed variables; C-18: kappa goes to slot 8 of the states
+  const double* var[8] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
                           selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),
                           selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[0], s2.Bc[0], C.cur),
-                          selp<BLK>(s.Bc[1], s2.Bc[1], C.cur)};
+                          selp<BLK>(s.Bc[1], s2.Bc[1], C.cur), Dv.K};
+  constexpr int slot[8] = {0, 1, 2, 3, 4, 5, 6, 8};
   // the face's record and normal field are requested together with the stencil: one round trip to memory, not two
   // (helper lanes read the record and field of the real zone they are clamped to)
   const FGeo G = load_fgeo(Dv.gf3A + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * (BLK ? Dv.B.ge2 : L.e2) + j) * NREC_F);
   const double bf3 = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z];
-  double PL[8], PR[8];
+  double PL[9], PR[9];
 #pragma unroll
-  for (int v = 0; v < 7; v++) {
+  for (int v = 0; v < NVR; v++) {
     const double* a = var[v] + z;
     double aR;
     if (RECON == HAMR_RECON_PPM) {
@@ -557,20 +566,21 @@ __global__ void __launch_bounds__(128, X3_MINB) k_flux_x3(Dev Dv, Fields s, Fiel
       const double dmp = __shfl_down_sync(FULL, dm0, 1);         // slope of zone k+1
       const double r = ppm_iface(c0, d32, dm0, dmp);             // a_{k+1/2}
       const double l = __shfl_up_sync(FULL, r, 1);               // a_{k-1/2}, built by lane-1 from the same expression
-      ppm_mono(l, c0, r, PR[v], aR);
+      ppm_mono(l, c0, r, PR[slot[v]], aR);
     } else {
-      plm_edges(a[om], a[o0], a[op], PR[v], aR);
+      plm_edges(a[om], a[o0], a[op], PR[slot[v]], aR);
     }
-    PL[v] = __shfl_up_sync(FULL, aR, 1);  // right edge of zone k-1 = left state of face k-1/2
+    PL[slot[v]] = __shfl_up_sync(FULL, aR, 1);  // right edge of zone k-1 = left state of face k-1/2
   }
   double ctop = 0.0;
   // C-15: the x3-faces of a phi-derefined row are computed by k_deref_x3 with a strided stencil
   const bool fine_row = Dv.mrow == nullptr || __ldg(Dv.mrow + C.J0 + j + NG) == 1;
   if (valid && fine_row && lane >= HLO && lane < 32 - HHI && k >= 0 && k < L.n[2] + (WRAP ? 0 : 1)) {
     PL[7] = PR[7] = bf3 * G.igdet;
-    double out[7];
-    const double ct = face_flux<D>(PL, PR, G, Dv.gam, out);
+    double out[8];
+    const double ct = face_flux<D, ENT>(PL, PR, G, Dv.gam, out);
     store_face(Dv, D, z, out);
+    if (ENT) Dv.FK[D][z] = out[7];
     if (WRAP && k == 0) store_face(Dv, D, z + L.n[2], out);
     if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct;
   }
@@ -781,7 +791,7 @@ void launch_deref_x3(hamr_grid* g, const Dev& Dv0, const Fields& src, const Fiel
 
 // picks the number of faces per marching segment so that the grid fills whole waves of resident
 // blocks (148 SMs x blocks per SM) with little prologue overhead
-template <int D, int RECON, bool BLK>
+template <int D, int RECON, bool BLK, bool ENT>
 static int pick_segment(const Lay& L, int nbx) {
   thread_local int cached_seg = 0, cached_dev = -1;   // per host thread: no shared mutable state between grids
   thread_local long long cached_key = -1;
@@ -791,7 +801,7 @@ static int pick_segment(const Lay& L, int nbx) {
   cudaGetDevice(&dev);
   if (key == cached_key && dev == cached_dev) return cached_seg;
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_flux_march<D, RECON, BLK>, MARCH_T, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_flux_march<D, RECON, BLK, ENT>, MARCH_T, 0);
   if (per_sm < 1) per_sm = 1;
   const double slots = (double)sms * per_sm;
   double best = -1.0;
@@ -812,15 +822,15 @@ static int pick_segment(const Lay& L, int nbx) {
   return best_seg;
 }
 
-template <int D, int RECON, bool BLK>
+template <int D, int RECON, bool BLK, bool ENT = false>
 static void launch_march_t(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
   const Lay& L = Dv.L;
   const int O = 1 - D;
   const long long ntr = (long long)(L.n[O] + 2) * (L.n[2] + 2) * (BLK ? Dv.B.nact : 1);
   const int nbx = (int)((ntr + MARCH_T - 1) / MARCH_T);
-  const int seg = pick_segment<D, RECON, BLK>(L, nbx);
+  const int seg = pick_segment<D, RECON, BLK, ENT>(L, nbx);
   dim3 grid(nbx, (L.n[D] + 1 + seg - 1) / seg);
-  k_flux_march<D, RECON, BLK><<<grid, MARCH_T, 0, g->stream>>>(Dv, src, src2, seg, want_ctop ? 1 : 0);
+  k_flux_march<D, RECON, BLK, ENT><<<grid, MARCH_T, 0, g->stream>>>(Dv, src, src2, seg, want_ctop ? 1 : 0);
 }
 
 // the ring kernel: segment length such that the grid fills whole waves of resident CTAs
@@ -862,6 +872,7 @@ static void launch_ring_t(hamr_grid* g, const Dev& Dv, const Fields& src, bool w
 static int ring_width(const Dev& Dv) {
   const int n3 = Dv.L.n[2];
   if (Dv.B.nblk > 0 || Dv.recon != HAMR_RECON_PPM || Dv.mrow || Dv.bc_lo[2] != HAMR_BC_PERIODIC) return 0;
+  if (Dv.entropy) return 0;   // C-18: the entropy row is carried by the generic kernels
   if (Dv.L.n[0] + 2 > 65535 || Dv.L.n[1] + 2 > 65535) return 0;
   // one warp per CTA: 64 / 128 threads (slots released through the second mbarrier) measured 3-7 % slower
   return n3 % 32 == 0 ? 32 : 0;
@@ -877,6 +888,11 @@ static void launch_march(hamr_grid* g, const Dev& Dv, const Fields& src, const F
   Launch l_(g, K_FLUX1 + D);
   const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
   if (ring_width(Dv) == 32) return launch_ring_t<D, 32>(g, Dv, src, want_ctop);
+  if (Dv.entropy) {   // C-18 (monolithic grids only: checked at creation)
+    if (ppm) launch_march_t<D, HAMR_RECON_PPM, false, true>(g, Dv, src, src2, want_ctop);
+    else launch_march_t<D, HAMR_RECON_PLM_MC, false, true>(g, Dv, src, src2, want_ctop);
+    return;
+  }
   if (ppm && !blk) launch_march_t<D, HAMR_RECON_PPM, false>(g, Dv, src, src2, want_ctop);
   else if (ppm) launch_march_t<D, HAMR_RECON_PPM, true>(g, Dv, src, src2, want_ctop);
   else if (!blk) launch_march_t<D, HAMR_RECON_PLM_MC, false>(g, Dv, src, src2, want_ctop);
@@ -904,7 +920,9 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
       case 4: launch_x3_warp_t<4>(g, Dv, src, want_ctop); return;
       default: break;
     }
-    if (x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    if (Dv.entropy && ppm) k_flux_x3<HAMR_RECON_PPM, false, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (Dv.entropy) k_flux_x3<HAMR_RECON_PLM_MC, false, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (ppm && !blk) k_flux_x3<HAMR_RECON_PPM, false, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (ppm) k_flux_x3<HAMR_RECON_PPM, true, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (!blk) k_flux_x3<HAMR_RECON_PLM_MC, false, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
@@ -917,6 +935,9 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
   }
 }
 
-void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop) { launch_flux_on(g, g->D, src, src, want_ctop); }
+void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop) {
+  if (g->D.entropy) launch_kappa(g, src);   // C-18: kappa of the (ghost-filled) source state for the entropy flux
+  launch_flux_on(g, g->D, src, src, want_ctop);
+}
 
 }  // namespace hamr

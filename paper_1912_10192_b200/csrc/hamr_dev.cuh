@@ -266,16 +266,117 @@ __device__ __forceinline__ int con2prim(const double U[5], const double Bc[3], c
 }
 
 // floors and Lorentz-factor ceiling on primitives (C-13)
-__device__ __forceinline__ void floors_ceiling(const CGeo& G, double rfl, double ufl, double gamma_max, double Pn[5],
-                                               int& nrf, int& nuf, int& ngc) {
-  if (Pn[0] < rfl) { Pn[0] = rfl; nrf = 1; }
-  if (Pn[1] < ufl) { Pn[1] = ufl; nuf = 1; }
+__device__ __forceinline__ void ceiling_only(const CGeo& G, double gamma_max, double Pn[5], int& ngc) {
   const double q = Pn[2] * (G.c11 * Pn[2] + G.c13 * Pn[4]) + Pn[3] * (G.c22 * Pn[3]) + Pn[4] * (G.c13 * Pn[2] + G.c33 * Pn[4]);
   if (q > gamma_max * gamma_max - 1.0) {   // gamma^2 = 1 + q > gamma_max^2
     const double fac = sqrt((gamma_max * gamma_max - 1.0) / q);
     Pn[2] *= fac; Pn[3] *= fac; Pn[4] *= fac;
     ngc = 1;
   }
+}
+__device__ __forceinline__ void floors_ceiling(const CGeo& G, double rfl, double ufl, double gamma_max, double Pn[5],
+                                               int& nrf, int& nuf, int& ngc) {
+  if (Pn[0] < rfl) { Pn[0] = rfl; nrf = 1; }
+  if (Pn[1] < ufl) { Pn[1] = ufl; nuf = 1; }
+  ceiling_only(G, gamma_max, Pn, ngc);
+}
+
+// ---- C-18: the entropy row and the inversion that uses it ------------------------
+// kappa = p / rho^gamma_ad is carried by the mass: the row is gdet rho u^t kappa with flux gdet rho u^d kappa and no
+// source.  Where the energy inversion fails (or returns rho <= 0 or u < 0) the zone is inverted from the density,
+// momentum and ENTROPY rows instead.  The normal observer sees D = gamma rho and D kappa, so kappa = US / U[0] is
+// known and one unknown is left, q = gamma^2 - 1:
+//   W(q) = w gamma^2 = D gamma + A gamma^(2 - gamma_ad),   A = gamma_ad / (gamma_ad - 1) kappa D^gamma_ad,
+//   f(q) = q / (1 + q) (Bsq + W)^2 - (Q.B)^2 (Bsq + 2 W) / W^2 - Qt^2 = 0        (momentum equation of Noble et al. 2006)
+// f grows monotonically from f(0) <= 0 (gamma_ad < 2): Newton steps kept inside a bracket that is first grown by
+// factors of 4.  The energy row U[1] is not read.  Returns 0 ok, 1 no root found / input without one.
+static __device__ __noinline__ int con2prim_entropy(const double* __restrict__ U, double US, const double* __restrict__ Bc,
+                                             const CGeo* __restrict__ Gp, double gam_ad,
+                                             const double* __restrict__ Pg, double* __restrict__ Pout) {
+  const CGeo& G = *Gp;
+  const double D = G.alpha * (U[0] * G.igdet);
+  const double kap = US / U[0];
+  if (!(D > 0.0) || !(kap >= 0.0) || !(D <= 1.79e308) || !(kap <= 1.79e308)) return 1;
+  const double Q1 = G.alpha * (U[2] * G.igdet), Q2 = G.alpha * (U[3] * G.igdet), Q3 = G.alpha * (U[4] * G.igdet);
+  const double Qu1 = G.i11 * Q1 + G.i13 * Q3, Qu2 = G.i22 * Q2, Qu3 = G.i13 * Q1 + G.i33 * Q3;
+  const double Qtsq = Q1 * Qu1 + Q2 * Qu2 + Q3 * Qu3;
+  const double B1 = G.alpha * Bc[0], B2 = G.alpha * Bc[1], B3 = G.alpha * Bc[2];
+  const double Bsq = B1 * (G.c11 * B1 + G.c13 * B3) + B2 * (G.c22 * B2) + B3 * (G.c13 * B1 + G.c33 * B3);
+  const double QdB = Q1 * B1 + Q2 * B2 + Q3 * B3, QdB2 = QdB * QdB;
+  const double A = gam_ad / (gam_ad - 1.0) * kap * pow(D, gam_ad);
+  if (!(Qtsq <= 1.79e308) || !(Bsq <= 1.79e308) || !(A <= 1.79e308)) return 1;
+  double W = 0.0, df = 0.0;
+  auto feval = [&](double q) {
+    const double q1 = 1.0 + q, g = sqrt(q1);
+    const double gp = pow(q1, -0.5 * gam_ad);              // gamma^(-gamma_ad)
+    W = D * g + A * gp * q1;
+    const double dW = 0.5 * (D / g + A * (2.0 - gam_ad) * gp);
+    const double v2 = q / q1, BW = Bsq + W, iW = 1.0 / W, t = QdB2 * iW * iW;
+    df = BW * BW / (q1 * q1) + 2.0 * BW * dW * (v2 + t * iW);
+    return v2 * BW * BW - t * (BW + W) - Qtsq;
+  };
+  double lo = 0.0, hi = 1.0;
+  for (int nb = 0; feval(hi) < 0.0; nb++) {
+    if (nb >= 60) return 1;
+    lo = hi;
+    hi *= 4.0;
+  }
+  double q = Pg[2] * (G.c11 * Pg[2] + G.c13 * Pg[4]) + Pg[3] * (G.c22 * Pg[3]) + Pg[4] * (G.c13 * Pg[2] + G.c33 * Pg[4]);
+  if (!(q > lo && q < hi)) q = 0.5 * (lo + hi);
+  bool conv = false;
+  for (int it = 0; it < 100 && !conv; it++) {
+    const double f = feval(q);
+    if (!(fabs(f) <= 1.79e308) || !(fabs(df) <= 1.79e308)) return 1;
+    if (f < 0.0) lo = q; else hi = q;
+    double qn = q - f / df;
+    if (!(qn > lo && qn < hi)) qn = 0.5 * (lo + hi);
+    conv = fabs(qn - q) <= 1e-14 * (1.0 + qn);
+    q = qn;
+  }
+  if (!conv) return 1;
+  feval(q);
+  const double gamma = sqrt(1.0 + q);
+  const double rho = D / gamma;
+  const double u = kap * pow(rho, gam_ad) / (gam_ad - 1.0);
+  if (!(rho <= 1.79e308) || !(u <= 1.79e308) || !(W <= 1.79e308)) return 1;
+  Pout[0] = rho;
+  Pout[1] = u;
+  const double fac = gamma / (W + Bsq), qw = QdB / W;
+  Pout[2] = fac * (Qu1 + qw * B1);
+  Pout[3] = fac * (Qu2 + qw * B2);
+  Pout[4] = fac * (Qu3 + qw * B3);
+  return 0;
+}
+
+// ---- C-19 (Ressler et al. 2017): floors applied in the drift frame ---------------
+// The matter added to reach the floors carries no momentum along the field and does not change the velocity across
+// it: with v = ut / gamma = v_perp + v_par Bhat in the normal observer's frame, v_perp is kept and v_par follows
+// from the conserved field-aligned momentum  m = w gamma^2 v_par  (w = rho + gamma_ad u):
+//   v_par' = 2 m s / (w' + sqrt(w'^2 + 4 m^2 s)),  s = 1 - v_perp^2.     Called only for a zone below a floor.
+static __device__ __noinline__ void floors_drift(const CGeo* __restrict__ Gp, const double* __restrict__ Bc, double gam_ad,
+                                          double rho_new, double u_new, double* __restrict__ Pn) {
+  const CGeo& G = *Gp;
+  const double B1 = G.alpha * Bc[0], B2 = G.alpha * Bc[1], B3 = G.alpha * Bc[2];
+  const double Bl1 = G.c11 * B1 + G.c13 * B3, Bl2 = G.c22 * B2, Bl3 = G.c13 * B1 + G.c33 * B3;
+  const double Bsq = B1 * Bl1 + B2 * Bl2 + B3 * Bl3;
+  if (!(Bsq > 0.0)) { Pn[0] = rho_new; Pn[1] = u_new; return; }   // no field: the fluid frame
+  const double q = Pn[2] * (G.c11 * Pn[2] + G.c13 * Pn[4]) + Pn[3] * (G.c22 * Pn[3]) + Pn[4] * (G.c13 * Pn[2] + G.c33 * Pn[4]);
+  const double gamma = sqrt(1.0 + q), ig = 1.0 / gamma;
+  const double v1 = Pn[2] * ig, v2 = Pn[3] * ig, v3 = Pn[4] * ig;
+  const double iB = 1.0 / sqrt(Bsq);
+  const double vpar = (v1 * Bl1 + v2 * Bl2 + v3 * Bl3) * iB;
+  const double h1 = B1 * iB, h2 = B2 * iB, h3 = B3 * iB;           // unit vector along the field
+  const double p1 = v1 - vpar * h1, p2 = v2 - vpar * h2, p3 = v3 - vpar * h3;
+  const double vperp2 = p1 * (G.c11 * p1 + G.c13 * p3) + p2 * (G.c22 * p2) + p3 * (G.c13 * p1 + G.c33 * p3);
+  const double m = (Pn[0] + gam_ad * Pn[1]) * (1.0 + q) * vpar;
+  const double wn = rho_new + gam_ad * u_new, s = 1.0 - vperp2;
+  const double vpn = 2.0 * m * s / (wn + sqrt(wn * wn + 4.0 * m * m * s));
+  const double gn = 1.0 / sqrt(s - vpn * vpn);
+  Pn[0] = rho_new;
+  Pn[1] = u_new;
+  Pn[2] = gn * (p1 + vpn * h1);
+  Pn[3] = gn * (p2 + vpn * h2);
+  Pn[4] = gn * (p3 + vpn * h3);
 }
 
 // positive doubles order like their bit patterns: max-reduce through an unsigned 64-bit atomic

@@ -18,7 +18,7 @@ struct Fields {
 enum Scal { S_T = 0, S_DT, S_CTOP0, S_CTOP1, S_CTOP2, S_DTLAST, S_DENMAX, S_DIVB, S_TOT0 /* ..+4 */,
             S_CTOPL0 = 13 /* ..+2: ctop of the last finished pass */, NSCAL = 16 };
 // device counters
-enum Cnt { N_C2PFAIL = 0, N_RHOFL, N_UFL, N_GCEIL, N_NONFINITE, NCNT = 8 };
+enum Cnt { N_C2PFAIL = 0, N_RHOFL, N_UFL, N_GCEIL, N_NONFINITE, N_ENTROPY /* zones inverted from the entropy row (C-18) */, NCNT = 8 };
 
 // Block-structured grid: every per-variable array holds nblk
 // padded blocks back to back (block b at doubles [b*blen, (b+1)*blen)); a launch works on the blocks
@@ -61,6 +61,10 @@ struct Dev {                 // everything a kernel may need, passed by value
   const double* gf3A;        // x3-faces [n2d][16] (centre (x1, x2))
   const double* rho_fl;      // [e1] floor per x1 index
   const double* u_fl;
+  int entropy, drift;        // C-18 entropy row + backup inversion, C-19 drift-frame floors (hamr_params; monolithic grids)
+  double* K;                 // C-18: kappa = (gamma_ad - 1) u / rho^gamma_ad of the stage's source state, every zone
+                             // incl. ghosts (k_kappa); the update kernel leaves the advected kappa of the active zones in it
+  double* FK[3];             // C-18: flux of the entropy row on d-faces
   double* F[3][5];           // hydro fluxes on d-faces
   double* EfA[3];            // on d-faces: E_e, (d,e,f) cyclic  (C-8)
   double* EfB[3];            // on d-faces: E_f
@@ -191,6 +195,7 @@ namespace hamr {
 void launch_ghosts(hamr_grid* g, const Fields& s, bool bc_active_too);
 void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop);
 void launch_ct(hamr_grid* g, const Fields& src);
+void launch_kappa(hamr_grid* g, const Fields& src);   // misc.cu: C-18, fills Dv.K from the source state (after its ghost fill)
 bool x3_ghosts_unused(const Dev& Dv);   // flux.cu: the stage kernels of this grid never read x3 ghost zones
 void launch_update(hamr_grid* g, const Fields& src, const Fields& base, const Fields& out, double dtfac,
                    bool src_is_base);

@@ -160,6 +160,20 @@ void launch_check_finite(hamr_grid* g, const Fields& s) {
   k_check_finite<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(g->D, s);
 }
 
+// C-18: kappa = p / rho^gamma_ad of every zone of the stage's source state, ghosts included (run after
+// the ghost fill), for the entropy flux of the generic flux kernels.  Slots no kernel reads (rho = 0) get 0.
+__global__ void k_kappa(Dev Dv, Fields s) {
+  const long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (z >= Dv.L.len) return;
+  const double rho = s.P[0][z], u = s.P[1][z];
+  Dv.K[z] = rho > 0.0 ? (Dv.gam - 1.0) * u * pow(rho, -Dv.gam) : 0.0;
+}
+
+void launch_kappa(hamr_grid* g, const Fields& s) {
+  Launch l_(g, K_OTHER);
+  k_kappa<<<(unsigned)((g->D.L.len + 255) / 256), 256, 0, g->stream>>>(g->D, s);
+}
+
 void launch_zero_ctop(hamr_grid* g) {
   Launch l_(g, K_OTHER);
   k_zero_ctop<<<1, 1, 0, g->stream>>>(g->D);

@@ -33,8 +33,11 @@ __device__ __forceinline__ Fields pick_fields(const Fields& a, const Fields& b, 
 // generic kernel: 6 CTAs of 128 threads per SM for the corrector (80 registers), 5 for the predictor (96, no spills):
 // measured best of 3-7 on cfg 2 (profiles/r2_experiments.md)
 constexpr int UPD_MINB = 6, UPD_MINB_PRED = 5;
-template <bool SAME, bool BLK>  // SAME: predictor, source state == base state
-__global__ void __launch_bounds__(128, SAME ? UPD_MINB_PRED : UPD_MINB) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
+// ROB (monolithic grids): the robust path.  With Dv.entropy the entropy row is advanced beside the
+// others and inverts the zones whose energy inversion failed or came back with rho <= 0 or u < 0 (C-18); with Dv.drift
+// the floors add mass and energy in the drift frame (C-19).
+template <bool SAME, bool BLK, bool ROB = false>  // SAME: predictor, source state == base state
+__global__ void __launch_bounds__(128, ROB ? 3 : (SAME ? UPD_MINB_PRED : UPD_MINB)) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
   const Lay& L = Dv.L;
   // k runs over [0, n3): warps start on 128-byte lines when n3 is a multiple of 32; the thread at k = 0 also
   // builds the x3-face at k = n3
@@ -42,7 +45,7 @@ __global__ void __launch_bounds__(128, SAME ? UPD_MINB_PRED : UPD_MINB) k_update
   const unsigned per = (unsigned)(L.n[0] + 1) * c1 * c2;
   unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = t < (BLK ? per * Dv.B.nact : per);
-  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0;
+  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0, nent = 0;
   if (valid) {
     int bslot = 0;
     if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
@@ -103,6 +106,7 @@ __global__ void __launch_bounds__(128, SAME ? UPD_MINB_PRED : UPD_MINB) k_update
         if (SAME) prim_to_U5(Ps, Ss, G.gdet, Dv.gam, U);
         source_12(Ps, Ss, G, Dv.gam, grec, Ssrc1, Ssrc2);   // C-12: on the stage's source state
       }
+      double rho_b = Ps[0], u_b = Ps[1];   // ROB: the base state's density and energy (C-18)
       if (!SAME) {
         double Pb[8];
 #pragma unroll
@@ -112,6 +116,15 @@ __global__ void __launch_bounds__(128, SAME ? UPD_MINB_PRED : UPD_MINB) k_update
         St Sb;
         get_state(Pb, G, Sb);
         prim_to_U5(Pb, Sb, G.gdet, Dv.gam, U);
+        rho_b = Pb[0]; u_b = Pb[1];
+      }
+      double US = 0.0;
+      if (ROB && Dv.entropy) {
+        // C-18: the entropy row of the base state is its density row times kappa; no source term
+        double div = 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; d++) div += (__ldg(Dv.FK[d] + z + S[d]) - __ldg(Dv.FK[d] + z)) * idx[d];
+        US = U[0] * ((Dv.gam - 1.0) * u_b * pow(rho_b, -Dv.gam)) - dt * div;
       }
       // U_new = U_base - dt sum_d (F^d_+ - F^d_-)/dx^d + dt S
 #pragma unroll
@@ -131,14 +144,37 @@ __global__ void __launch_bounds__(128, SAME ? UPD_MINB_PRED : UPD_MINB) k_update
       const double* sp[5] = {src.P[0], src.P[1], src.P[2], src.P[3], src.P[4]};
 #pragma unroll
       for (int c = 0; c < 5; c++) { const double* a = sp[c]; asm volatile("" : "+l"(a)); Pg[c] = a[z]; }
-      if (con2prim(U, Bn, G2, Dv.gam, Pg, Pn) != 0) {  // C-13: keep the source state's hydro primitives, count the failure
+      int rc = con2prim(U, Bn, G2, Dv.gam, Pg, Pn);
+      if (ROB && Dv.entropy) {
+        Dv.K[z] = US / U[0];   // the advected kappa (diagnostic: k_kappa overwrites it before the next flux pass)
+        if (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) {
+          // an entropy row that went negative or has no root leaves what the energy inversion gave: its converged
+          // state for the floors to repair, or its failure
+          double Pe[5];
+          if (con2prim_entropy(U, US, Bn, &G2, Dv.gam, Pg, Pe) == 0) {
+#pragma unroll
+            for (int c = 0; c < 5; c++) Pn[c] = Pe[c];
+            rc = 0;
+            nent = 1;
+          }
+        }
+      }
+      if (rc != 0) {  // C-13: keep the source state's hydro primitives, count the failure
         nfail = 1;
 #pragma unroll
         for (int c = 0; c < 5; c++) Pn[c] = Pg[c];
       }
       // floors and Lorentz-factor ceiling (C-13)
       const int fi = C.I0 + i + NG + (BLK ? C.lev * Dv.B.flev : 0);
-      floors_ceiling(G2, __ldg(Dv.rho_fl + fi), __ldg(Dv.u_fl + fi), Dv.gamma_max, Pn, nrf, nuf, ngc);
+      const double rfl = __ldg(Dv.rho_fl + fi), ufl = __ldg(Dv.u_fl + fi);
+      if (ROB && Dv.drift) {
+        nrf = Pn[0] < rfl;
+        nuf = Pn[1] < ufl;
+        if (nrf | nuf) floors_drift(&G2, Bn, Dv.gam, nrf ? rfl : Pn[0], nuf ? ufl : Pn[1], Pn);
+        ceiling_only(G2, Dv.gamma_max, Pn, ngc);
+      } else {
+        floors_ceiling(G2, rfl, ufl, Dv.gamma_max, Pn, nrf, nuf, ngc);
+      }
 #pragma unroll
       for (int c = 0; c < 5; c++) {
         out.P[c][z] = Pn[c];
@@ -152,6 +188,10 @@ __global__ void __launch_bounds__(128, SAME ? UPD_MINB_PRED : UPD_MINB) k_update
   const unsigned m_f = __ballot_sync(0xffffffffu, nfail), m_r = __ballot_sync(0xffffffffu, nrf),
                  m_u = __ballot_sync(0xffffffffu, nuf), m_g = __ballot_sync(0xffffffffu, ngc),
                  m_b = __ballot_sync(0xffffffffu, bad);
+  if (ROB) {
+    const unsigned m_e = __ballot_sync(0xffffffffu, nent);
+    if ((threadIdx.x & 31) == 0 && m_e) atomicAdd(Dv.cnt + N_ENTROPY, (unsigned long long)__popc(m_e));
+  }
   if ((threadIdx.x & 31) == 0) {
     if (m_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)__popc(m_f));
     if (m_r) atomicAdd(Dv.cnt + N_RHOFL, (unsigned long long)__popc(m_r));
@@ -386,7 +426,7 @@ static void launch_tile_t(hamr_grid* g, const Dev& Dv, const Roles& r, double dt
 // the tiled kernel serves monolithic grids without derefinement whose staged planes fit shared memory
 static int tile_threads(const Dev& Dv) {
   using namespace tile;
-  if (Dv.B.nblk > 0 || Dv.mrow) return 0;
+  if (Dv.B.nblk > 0 || Dv.mrow || Dv.entropy || Dv.drift) return 0;   // NEXT-2 runs on the generic kernel
   const int nt = 32 * ((Dv.L.n[2] + 31) / 32) * TJ;
   const size_t smem = (size_t)(2 * NA + NB) * (TJ + 1) * Dv.L.p3 * sizeof(double) + 16;
   if (nt > 512 || smem > 227 * 1024) return 0;
@@ -407,6 +447,11 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
     case 256: return same ? launch_tile_t<true, 256>(g, Dv, ra, dtfac) : launch_tile_t<false, 256>(g, Dv, ra, dtfac);
     case 512: return same ? launch_tile_t<true, 512>(g, Dv, ra, dtfac) : launch_tile_t<false, 512>(g, Dv, ra, dtfac);
     default: break;
+  }
+  if (Dv.entropy || Dv.drift) {   // monolithic grids only (checked at creation)
+    if (same) k_update<true, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+    else k_update<false, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+    return;
   }
   if (same && !blk) k_update<true, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
   else if (same) k_update<true, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);

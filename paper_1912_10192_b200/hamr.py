@@ -28,14 +28,14 @@ _STATUS = {0: "HAMR_OK", 1: "HAMR_EINVAL", 2: "HAMR_ENOMEM", 3: "HAMR_ECUDA", 4:
 SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "hamr_grid_destroy",
            "hamr_set_prims", "hamr_set_prims_dev", "hamr_step", "hamr_step_async", "hamr_sync",
            "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
-           "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
+           "hamr_get_backup_count", "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
            "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
            "hamr_get_block_bface", "hamr_set_all_blocks", "hamr_get_all_blocks"]
 # ... and include/hamr_debug.h (test hooks and diagnostics)
 DEBUG_SYMBOLS = ["hamr_set_levels", "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
                  "hamr_profile_begin", "hamr_profile_end", "hamr_profile_class_name", "hamr_launch_count",
                  "hamr_debug_geometry", "hamr_debug_prim2cons", "hamr_debug_con2prim", "hamr_debug_floors",
-                 "hamr_bench_fp64"]
+                 "hamr_debug_kappa", "hamr_debug_con2prim_entropy", "hamr_debug_floors_drift", "hamr_bench_fp64"]
 NKCLASS = 10
 
 
@@ -51,6 +51,7 @@ class Params(C.Structure):
                 ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3), ("nb", C.c_int * 3),
                 ("n_deref", C.c_int), ("deref_factor", C.c_int * 4),
                 ("lat_max_level", C.c_int), ("map", C.c_int),
+                ("entropy_backup", C.c_int), ("drift_floors", C.c_int),
                 ("a", C.c_double), ("xmin", C.c_double * 3), ("xmax", C.c_double * 3),
                 ("gamma_ad", C.c_double), ("cour", C.c_double),
                 ("rho_fl_coef", C.c_double), ("rho_fl_pow", C.c_double),
@@ -81,6 +82,7 @@ def lib():
         L.hamr_get_bface.argtypes = [vp, C.POINTER(c_double_p)]
         L.hamr_divb.argtypes = [vp, c_double_p]
         L.hamr_get_stats.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.hamr_get_backup_count.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.hamr_get_time.argtypes = [vp, c_double_p, c_double_p]
         L.hamr_set_dt.argtypes = [vp, C.c_double]
         L.hamr_last_error.argtypes = [vp]
@@ -109,6 +111,10 @@ def lib():
         L.hamr_debug_prim2cons.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p]
         L.hamr_debug_con2prim.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p, c_double_p, c_double_p, ip]
         L.hamr_debug_floors.argtypes = [vp, C.c_int, ip, ip, c_double_p, ip]
+        L.hamr_debug_kappa.argtypes = [vp, c_double_p]
+        L.hamr_debug_con2prim_entropy.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p, c_double_p, c_double_p,
+                                                  c_double_p, ip]
+        L.hamr_debug_floors_drift.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p, ip]
         L.hamr_bench_fp64.argtypes = [vp, C.c_int, C.c_int, c_double_p, c_double_p]
         for s in SYMBOLS + DEBUG_SYMBOLS:
             if s not in ("hamr_last_error", "hamr_profile_class_name"):
@@ -130,6 +136,8 @@ def pack_params(p: dict) -> Params:
         q.deref_theta_deg[i], q.deref_factor[i] = float(t), int(f)
     q.lat_max_level = int(p["lat_max_level"])
     q.map = int(p.get("map", 0))
+    q.entropy_backup = int(p.get("entropy_backup", 0))
+    q.drift_floors = int(p.get("drift_floors", 0))
     q.a = float(p["a"])
     q.gamma_ad, q.cour = float(p["gamma_ad"]), float(p["cour"])
     q.rho_fl_coef, q.rho_fl_pow = float(p["rho_fl_coef"]), float(p["rho_fl_pow"])
@@ -254,6 +262,12 @@ class Grid:
         c = (C.c_longlong * 4)()
         self._ck(self.L.hamr_get_stats(self.h, c))
         return tuple(c[:])
+
+    def backup_count(self):
+        """zones, since the last call, inverted from the entropy row (entropy_backup grids)"""
+        n = C.c_longlong(0)
+        self._ck(self.L.hamr_get_backup_count(self.h, C.byref(n)))
+        return n.value
 
     @property
     def t(self):
@@ -405,6 +419,31 @@ class Grid:
         a, b, pa, pb = self._ij(ti, tj)
         fl = np.zeros(len(a), dtype=np.int32)
         self._ck(self.L.hamr_debug_floors(self.h, len(a), pa, pb, _dp(Q), fl.ctypes.data_as(C.POINTER(C.c_int))))
+        return Q, fl
+
+    def kadv(self):
+        """kappa the entropy row gave in the latest update stage, active zones (entropy_backup grids)"""
+        out = np.empty(self.n)
+        self._ck(self.L.hamr_debug_kappa(self.h, _dp(out)))
+        return out
+
+    def con2prim_entropy(self, ti, tj, U, US, Bc, guess):
+        """U (n, 5), entropy row US (n), Bc (n, 3), guess (n, 5) -> hydro primitives (n, 5), rc (n)"""
+        U, US, Bc, gs = _arr(U), _arr(US), _arr(Bc), _arr(guess)
+        a, b, pa, pb = self._ij(ti, tj)
+        out = np.empty((len(a), 5))
+        rc = np.zeros(len(a), dtype=np.int32)
+        self._ck(self.L.hamr_debug_con2prim_entropy(self.h, len(a), pa, pb, _dp(U), _dp(US), _dp(Bc), _dp(gs), _dp(out),
+                                                    rc.ctypes.data_as(C.POINTER(C.c_int))))
+        return out, rc
+
+    def floors_drift(self, ti, tj, P, Bc):
+        """floors (in the drift frame on a drift_floors grid) and ceiling on P (n, 5) with field Bc (n, 3)"""
+        Q, Bc = _arr(P).copy(), _arr(Bc)
+        a, b, pa, pb = self._ij(ti, tj)
+        fl = np.zeros(len(a), dtype=np.int32)
+        self._ck(self.L.hamr_debug_floors_drift(self.h, len(a), pa, pb, _dp(Q), _dp(Bc),
+                                                fl.ctypes.data_as(C.POINTER(C.c_int))))
         return Q, fl
 
     def launch_count(self):
