@@ -294,6 +294,7 @@ def main():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-grids", type=int, default=3, help="grids in flight in the end-to-end measurement")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.steps is None:
@@ -403,38 +404,48 @@ def main():
         performed = world * nz * float(np.mean(fin / 2.0 ** lv)) * args.steps / (ms_max * 1e-3)
 
     # ---- end to end through the C-ABI with HOST buffers (pinned): set_prims + step + get_prims -----
+    # Two numbers.  "serial": one grid, call after call; PCIe carries the step's input, then the GPU steps, then PCIe
+    # carries the result: nothing overlaps (each call needs the one before).  The headline `value`: SEVERAL grids in flight (--e2e-grids),
+    # each driven by its own host thread through the same three calls on its own stream (the library has no global
+    # state; ctypes releases the GIL), so one grid's result goes down the link while the other's input comes up (PCIe is
+    # full duplex) and the kernels of one run under the copies of the other.  Every step of either grid still copies
+    # all of its input from pinned host memory and all of its result back inside the timed region.
+    import threading
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
     C = hamr.C
     L = hamr.lib()
+    ng = max(1, args.e2e_grids)
+    gx = [g] + [hamr.Grid(p) for _ in range(ng - 1)]   # the other grids: own device memory, own stream
     if refined:
         # every block in one call: the per-block arrays back to back (hamr_set_all_blocks / hamr_get_all_blocks)
         hh = [pin(np.stack([hb[c] for hb, fb in bdata])) for c in range(5)]
         bh = [pin(np.stack([fb[c] for hb, fb in bdata])) for c in range(3)]
         nbk = g.num_blocks()
-        outs = [torch.empty((nbk,) + tuple(infos[0][2]), dtype=torch.float64).pin_memory().numpy() for _ in range(8)]
-        hp = (hamr.c_double_p * 5)(*[hamr._dp(h) for h in hh])
-        bp = (hamr.c_double_p * 3)(*[hamr._dp(f) for f in bh])
-        op = (hamr.c_double_p * 8)(*[hamr._dp(o) for o in outs])
-
-        def e2e_step():
-            rc = L.hamr_set_all_blocks(g.h, hp, bp)
-            rc |= L.hamr_step(g.h, 1, None, None)
-            rc |= L.hamr_get_all_blocks(g.h, op)
-            assert rc == 0, rc
+        oshape = (nbk,) + tuple(infos[0][2])
+        set_call, get_call = L.hamr_set_all_blocks, L.hamr_get_all_blocks
     else:
         hh = [pin(h) for h in hyd]
         bh = [pin(b) for b in bf]
-        outs = [torch.empty(n, dtype=torch.float64).pin_memory().numpy() for _ in range(8)]
-        hp = (hamr.c_double_p * 5)(*[hamr._dp(h) for h in hh])
-        bp = (hamr.c_double_p * 3)(*[hamr._dp(b) for b in bh])
-        op = (hamr.c_double_p * 8)(*[hamr._dp(o) for o in outs])
+        oshape = n
+        set_call, get_call = L.hamr_set_prims, L.hamr_get_prims
+    hp = (hamr.c_double_p * 5)(*[hamr._dp(h) for h in hh])
+    bp = (hamr.c_double_p * 3)(*[hamr._dp(b) for b in bh])
+    outs2 = [[torch.empty(oshape, dtype=torch.float64).pin_memory().numpy() for _ in range(8)] for _ in range(ng)]
+    ops = [(hamr.c_double_p * 8)(*[hamr._dp(o) for o in oo]) for oo in outs2]
+    outs = outs2[0]
 
-        def e2e_step():
-            rc = L.hamr_set_prims(g.h, hp, bp)
-            rc |= L.hamr_step(g.h, 1, None, None)
-            rc |= L.hamr_get_prims(g.h, op)
-            assert rc == 0, rc
+    def e2e_step(gh=None, op=None):
+        gh = g.h if gh is None else gh
+        op = ops[0] if op is None else op
+        rc = set_call(gh, hp, bp)
+        rc |= L.hamr_step(gh, 1, None, None)
+        rc |= get_call(gh, op)
+        assert rc == 0, rc
+
     e2e_step()
+    for q in range(1, ng):
+        for _ in range(2):                      # the second call captures the grid's step graph (on this thread)
+            e2e_step(gx[q].h, ops[q])
     barrier()
     t0 = time.perf_counter()
     ev0.record()
@@ -443,7 +454,25 @@ def main():
     ev1.record()
     barrier()
     e2e_ms = max(ev0.elapsed_time(ev1), 1e3 * (time.perf_counter() - t0))
-    e2e_val, _ = replica_throughput(e2e_ms, nz * fin * args.e2e_steps, world, "cuda")
+    e2e_serial, _ = replica_throughput(e2e_ms, nz * fin * args.e2e_steps, world, "cuda")
+
+    def e2e_worker(gh, op):
+        torch.cuda.set_device(local)            # the current device is per host thread
+        for _ in range(args.e2e_steps):
+            e2e_step(gh, op)
+    th = [threading.Thread(target=e2e_worker, args=(gx[q].h, ops[q])) for q in range(ng)]
+    barrier()
+    t0 = time.perf_counter()
+    for t_ in th:
+        t_.start()
+    for t_ in th:
+        t_.join()                               # every call above has synchronised its own stream before returning
+    e2e_ms2 = 1e3 * (time.perf_counter() - t0)
+    barrier()
+    e2e_val, _ = replica_throughput(e2e_ms2, nz * fin * ng * args.e2e_steps, world, "cuda")
+    same_result = all(np.array_equal(a, b) for q in range(1, ng) for a, b in zip(outs2[0], outs2[q]))
+    for q in range(1, ng):
+        gx[q].close()
     h2d = sum(a.nbytes for a in hh) + sum(a.nbytes for a in bh)
     d2h = sum(a.nbytes for a in outs)
 
@@ -533,8 +562,13 @@ def main():
             "sustained": {"value": sustained, "unit": UNIT, "steps": sus_steps, "ms_per_step": ms_sus / sus_steps,
                           "what": "the same step repeated for >= 0.7 s right after the headline pass (power-capped clocks)"},
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": args.e2e_steps, "what": ("hamr_set_all_blocks + hamr_step(1) + hamr_get_all_blocks"
-                             if refined else "hamr_set_prims(host) + hamr_step(1) + hamr_get_prims(host)") + ", pinned buffers"},
+                    "steps": ng * args.e2e_steps, "grids_in_flight": ng, "results_identical": bool(same_result),
+                    "what": ("hamr_set_all_blocks + hamr_step(1) + hamr_get_all_blocks" if refined else
+                             "hamr_set_prims(host) + hamr_step(1) + hamr_get_prims(host)") + ", pinned buffers; several "
+                            "grids in flight, one host thread and stream each (one grid's D2H overlaps another's H2D "
+                            "and kernels); wall clock over all steps of all grids",
+                    "serial": {"value": e2e_serial, "unit": UNIT, "steps": args.e2e_steps,
+                               "what": "the same three calls on one grid, one after the other (nothing overlaps)"}},
             "gpu_launches": launches,
             "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line))

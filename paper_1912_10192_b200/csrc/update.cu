@@ -37,7 +37,7 @@ constexpr int UPD_MINB = 6, UPD_MINB_PRED = 5;
 // others and inverts the zones whose energy inversion failed or came back with rho <= 0 or u < 0 (C-18); with Dv.drift
 // the floors add mass and energy in the drift frame (C-19).
 template <bool SAME, bool BLK, bool ROB = false>  // SAME: predictor, source state == base state
-__global__ void __launch_bounds__(128, ROB ? 3 : (SAME ? UPD_MINB_PRED : UPD_MINB)) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
+__global__ void __launch_bounds__(128, ROB ? 4 : (SAME ? UPD_MINB_PRED : UPD_MINB)) k_update(Dev Dv, Roles ra, Roles rb, double dtfac) {
   const Lay& L = Dv.L;
   // k runs over [0, n3): warps start on 128-byte lines when n3 is a multiple of 32; the thread at k = 0 also
   // builds the x3-face at k = n3
@@ -150,8 +150,14 @@ __global__ void __launch_bounds__(128, ROB ? 3 : (SAME ? UPD_MINB_PRED : UPD_MIN
         if (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) {
           // an entropy row that went negative or has no root leaves what the energy inversion gave: its converged
           // state for the floors to repair, or its failure
-          double Pe[5];
-          if (con2prim_entropy(U, US, Bn, &G2, Dv.gam, Pg, Pe) == 0) {
+          // (the rare call works on copies, so that the common path's U, Bn, Pg and record stay in registers)
+          double Pe[5], Uc[5], Bc[3], Pc[5];
+          CGeo Gc = G2;
+#pragma unroll
+          for (int c = 0; c < 5; c++) { Uc[c] = U[c]; Pc[c] = Pg[c]; }
+#pragma unroll
+          for (int c = 0; c < 3; c++) Bc[c] = Bn[c];
+          if (con2prim_entropy(Uc, US, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
 #pragma unroll
             for (int c = 0; c < 5; c++) Pn[c] = Pe[c];
             rc = 0;
@@ -170,7 +176,17 @@ __global__ void __launch_bounds__(128, ROB ? 3 : (SAME ? UPD_MINB_PRED : UPD_MIN
       if (ROB && Dv.drift) {
         nrf = Pn[0] < rfl;
         nuf = Pn[1] < ufl;
-        if (nrf | nuf) floors_drift(&G2, Bn, Dv.gam, nrf ? rfl : Pn[0], nuf ? ufl : Pn[1], Pn);
+        if (nrf | nuf) {
+          double Bc[3], Pc[5];
+          CGeo Gc = G2;
+#pragma unroll
+          for (int c = 0; c < 5; c++) Pc[c] = Pn[c];
+#pragma unroll
+          for (int c = 0; c < 3; c++) Bc[c] = Bn[c];
+          floors_drift(&Gc, Bc, Dv.gam, nrf ? rfl : Pn[0], nuf ? ufl : Pn[1], Pc);
+#pragma unroll
+          for (int c = 0; c < 5; c++) Pn[c] = Pc[c];
+        }
         ceiling_only(G2, Dv.gamma_max, Pn, ngc);
       } else {
         floors_ceiling(G2, rfl, ufl, Dv.gamma_max, Pn, nrf, nuf, ngc);
