@@ -151,7 +151,7 @@ ArenaPlan plan_arena(const hamr_params& p, const Lay& L, const GridShape& G) {
   if (G.nblk > 0)
     a.stage_doubles = std::max(a.stage_doubles, (size_t)G.nblk * 8 * (L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1));
   a.stage = off; off += align_up(a.stage_doubles * 8, 256);
-  a.blk = off; off += G.nblk > 0 ? blk_table_bytes(G.nblk) : 0;
+  a.blk = off; off += G.nblk > 0 ? blk_table_bytes(G.nblk, (long long)L.e1 * L.e2 * (L.n[2] + 2 * NG + 1)) : 0;
   a.mrow = off; off += p.n_deref > 0 ? align_up((size_t)G.te2 * sizeof(int), 256) : 0;
   a.total = off;
   return a;

@@ -37,19 +37,9 @@ __device__ __forceinline__ const double* buf_arr(const Bufs& B, int buf, int kin
   return buf == 0 ? a0 : (buf == 1 ? a1 : a2);
 }
 
-// k_blk_ghosts calls these from eleven places (370 KB of code).  Out of line the kernel is SLOWER (measured on
-// cfg 4: 0.396 -> 0.494 ms with both, 0.423 with blk_fetch_ref alone): the calls spill their arguments.  A
-// single looped call site (10 k instructions instead of 23 k) was no faster either: each iteration consumes its
-// load at once, which serialises the DRAM round trips the unrolled form overlaps
-#ifndef HAMR_GHOST_SHELL
-#define HAMR_GHOST_SHELL 1
-#endif
-#ifndef HAMR_REF_INLINE
-#define HAMR_REF_INLINE __forceinline__
-#endif
-#ifndef HAMR_SRC_INLINE
-#define HAMR_SRC_INLINE __forceinline__
-#endif
+// k_blk_ghosts calls blk_fetch_ref from eleven places.  Out of line the kernel is slower (measured on cfg 4: 0.260 ->
+// 0.286 ms): the calls spill their arguments.  A single looped call site was no faster either: each iteration consumes
+// its load at once, which serialises the DRAM round trips the unrolled form overlaps.
 template <typename T>
 __device__ __forceinline__ T pick4(const T v[4], int i) {
   return i == 0 ? v[0] : (i == 1 ? v[1] : (i == 2 ? v[2] : v[3]));
@@ -75,7 +65,7 @@ struct GSrc {
 
 // sd: the array is staggered along sd (-1: zone-centred)
 // norule: every neighbour is on b's own time level, so no face is owned by a finer block
-__device__ HAMR_SRC_INLINE GSrc blk_src(const Dev& Dv, int b, int phys, int sd, const int id[3], bool norule) {
+__device__ __forceinline__ GSrc blk_src(const Dev& Dv, int b, int phys, int sd, const int id[3], bool norule) {
   const Lay& L = Dv.L;
   int m[3], o[3];
   GSrc s;
@@ -161,6 +151,67 @@ __device__ HAMR_SRC_INLINE GSrc blk_src(const Dev& Dv, int b, int phys, int sd, 
   return s;
 }
 
+// ---- the ghost-source table -------------------------------------------------------------------------------------------
+// blk_src is a pure function of (block, array kind, padded location) once the time levels are fixed, and it is most of
+// the ghost kernel's instructions (neighbour look-ups, boundary maps, the finer-face rule).  k_blk_src_table evaluates
+// it once per level assignment for every location; the ghost kernel then reads 8 bytes instead.  Packed: bits 0..31 the
+// offset zl, 32..53 q + 1, 54..56 negmask, 57 ghost, 58 zero, 59 mod, 60 moved, 63 "not in the table" (the value is a
+// restriction / prolongation across the x1 refinement interface, whose five extra fields are computed on the fly).
+__device__ __forceinline__ unsigned long long gsrc_pack(const GSrc& s) {
+  if (s.ref) return 1ull << 63;
+  return (unsigned long long)(unsigned)s.zl | ((unsigned long long)(unsigned)(s.q + 1) << 32) |
+         ((unsigned long long)(s.negmask & 7) << 54) | ((unsigned long long)s.ghost << 57) |
+         ((unsigned long long)s.zero << 58) | ((unsigned long long)s.mod << 59) | ((unsigned long long)s.moved << 60);
+}
+
+__device__ __noinline__ void blk_src_slow(const Dev* Dv, int b, int phys, int sd, int i0, int i1, int i2, int norule, GSrc* out) {
+  const int id[3] = {i0, i1, i2};
+  *out = blk_src(*Dv, b, phys, sd, id, norule != 0);
+}
+
+__device__ __forceinline__ GSrc blk_src_tab(const Dev& Dv, int b, int phys, int sd, const int id[3], bool norule) {
+  const Lay& L = Dv.L;
+  const int e3 = L.n[2] + 2 * NG + 1;
+  const bool inside = id[0] >= -NG && id[0] <= L.n[0] + NG && id[1] >= -NG && id[1] <= L.n[1] + NG && id[2] >= -NG &&
+                      id[2] <= L.n[2] + NG;
+  if (Dv.B.gsrc && inside) {
+    const int loc = ((id[0] + NG) * L.e2 + id[1] + NG) * e3 + id[2] + NG;
+    const unsigned long long w = __ldg(Dv.B.gsrc + ((size_t)b * 4 + (sd + 1)) * Dv.B.gloc + loc);
+    if (!(w >> 63)) {
+      GSrc s;
+      s.zl = (int)(unsigned)(w & 0xffffffffull);
+      s.q = (int)((w >> 32) & 0x3fffffull) - 1;
+      s.negmask = (int)((w >> 54) & 7);
+      s.ghost = (w >> 57) & 1;
+      s.zero = (w >> 58) & 1;
+      s.mod = (w >> 59) & 1;
+      s.moved = (w >> 60) & 1;
+      s.ref = false;
+      s.rq = -1; s.side = 0; s.mi = 0; s.lj = 0; s.lk = 0;
+      return s;
+    }
+  }
+  GSrc s;
+  blk_src_slow(&Dv, b, phys, sd, id[0], id[1], id[2], norule ? 1 : 0, &s);
+  return s;
+}
+
+// one thread per padded location of every block: the four sources of the location
+__global__ void __launch_bounds__(256) k_blk_src_table(const __grid_constant__ Dev Dv, unsigned long long* __restrict__ tab) {
+  const Lay& L = Dv.L;
+  const int e3 = L.n[2] + 2 * NG + 1;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (unsigned)Dv.B.gloc) return;
+  const int b = blockIdx.y;
+  const unsigned tj = t / (unsigned)e3, ti = tj / (unsigned)L.e2;
+  const int id[3] = {(int)ti - NG, (int)(tj - ti * L.e2) - NG, (int)(t - tj * e3) - NG};
+  const int phys = __ldg(Dv.B.phys + b);
+  const bool same = (Dv.B.flags[b] & 4) != 0;
+#pragma unroll 1
+  for (int sd = -1; sd < 3; sd++)
+    tab[((size_t)b * 4 + (sd + 1)) * Dv.B.gloc + t] = gsrc_pack(blk_src(Dv, b, phys, sd, id, same));
+}
+
 // C-17 time sampling of block q at time s_u: which buffers and with what weight
 struct QTime { int b0, b1; double w; };  // value = (1 - w) a[b0] + w a[b1]; b1 < 0: a plain copy of a[b0]
 __device__ __forceinline__ QTime blk_qtime(const Dev& Dv, const LevT& lt, int q, long long s_u) {
@@ -194,7 +245,7 @@ __device__ __forceinline__ double blk_at(const Dev& Dv, const Bufs& B, int kind,
 // coarse values (the coarse value beyond the interface is the restriction of the fine block rq), a quarter
 // of a coarse zone off the coarse centre; normal faces copy coincident coarse faces, in-between ones are
 // the mean of their two coarse neighbours.
-__device__ HAMR_REF_INLINE double blk_fetch_ref(const Dev& Dv, const Bufs& B, const LevT& lt, int levb, int kind,
+__device__ __forceinline__ double blk_fetch_ref(const Dev& Dv, const Bufs& B, const LevT& lt, int levb, int kind,
                                                 const GSrc& s, long long s_u) {
   if (s.zero) return 0.0;
   const int n0 = Dv.L.n[0];
@@ -263,9 +314,9 @@ __device__ __forceinline__ double blk_fetch(const Dev& Dv, const Bufs& B, int b,
   return (vc >= 0 && ((s.negmask >> vc) & 1)) ? -v : v;
 }
 
-#ifndef HAMR_GHOST_MINB
-#define HAMR_GHOST_MINB 5  // 48 registers; 2 / 3 (104 / 80 registers, no spills) measured 12 % / 3 % slower on cfg 4: occupancy wins
-#endif
+// 4 CTAs of 256 threads per SM (64 registers): with the sources read from the table 3 / 4 / 5 / 6 / 8 CTAs measured
+// 0.299 / 0.260 / 0.285 / 0.306 / 0.303 ms per launch on cfg 4 (0.317 before the table, at 5)
+constexpr int GHOST_MINB = 4;
 // Ghost fill of the stage source of every listed block: neighbour exchange with time interpolation
 // (C-16, C-17), physical boundaries (C-12), cell-centred B wherever a face changed (C-10).
 // role: 0 the source is the block's time-n state, 1 its predictor state.  all: also derive B_c on the
@@ -273,7 +324,7 @@ __device__ __forceinline__ double blk_fetch(const Dev& Dv, const Bufs& B, int b,
 // Block flags (host, per level assignment): bit 0 "simple": no physical side and all 26 neighbours on
 // the block's own time level -> every ghost value (B_c included) is a plain copy of the neighbour's
 // stage source; bit 1: some neighbour is on a finer time level (only then can an ACTIVE face change).
-__global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(const __grid_constant__ Dev Dv, const __grid_constant__ Bufs B,
+__global__ void __launch_bounds__(256, GHOST_MINB) k_blk_ghosts(const __grid_constant__ Dev Dv, const __grid_constant__ Bufs B,
                                                     const __grid_constant__ LevT lt, int role, long long s_u, int all,
                                                     int zero_ctop) {
   // grid: x covers the padded locations of one block, y the blocks of the launch; 32-bit index arithmetic
@@ -284,7 +335,7 @@ __global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(const __gri
   const int b = __ldg(Dv.B.list + blockIdx.y);
   if (zero_ctop && t == 0) Dv.B.ctopb[b * 3] = Dv.B.ctopb[b * 3 + 1] = Dv.B.ctopb[b * 3 + 2] = 0.0;
   int i0, i1, i2;
-  if (HAMR_GHOST_SHELL && !all && !(Dv.B.flags[b] & 2)) {
+  if (!all && !(Dv.B.flags[b] & 2)) {
     // no finer neighbour: active storage is final, so only the ghost shell is enumerated (whole warps of ghost
     // slots instead of warps that are two thirds active zones).  Part A: the (i, j) columns outside the active
     // range, every k; part B: the active columns' 2 NG + 1 ghost slots in k.
@@ -431,7 +482,7 @@ __global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(const __gri
   // here is a neighbour of b on b's own level, so none of them rewrites those zones in this launch.
   bool pure = false;
   if (wP) {
-    const GSrc s = blk_src(Dv, b, phys, -1, id, same);
+    const GSrc s = blk_src_tab(Dv, b, phys, -1, id, same);
     if (s.ghost) { qt = qtime(s.q); lastq = s.q; }
 #pragma unroll
     for (int c = 0; c < 5; c++) vP[c] = fetch(c, s);
@@ -452,7 +503,7 @@ __global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(const __gri
     if (extra[o1] || extra[o2]) { lo[d] = hi[d] = 0.0; continue; }
     const bool face_read = shell1[o1] && shell1[o2] && id[d] >= 0 && id[d] <= L.n[d];   // a flux kernel reads this face
     if (pure && !face_read) { lo[d] = hi[d] = 0.0; continue; }
-    GSrc s = blk_src(Dv, b, phys, d, id, same);
+    GSrc s = blk_src_tab(Dv, b, phys, d, id, same);
     if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
     lo[d] = fetch(5 + d, s);
     if (s.mod) { wF[d] = face_read; anymod = true; }
@@ -460,7 +511,7 @@ __global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(const __gri
     if (!extra[d] && !pure) {
       int idp[3] = {id[0], id[1], id[2]};
       idp[d] += 1;
-      s = blk_src(Dv, b, phys, d, idp, same);
+      s = blk_src_tab(Dv, b, phys, d, idp, same);
       if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
       hi[d] = fetch(5 + d, s);
       anymod = anymod || s.mod;
@@ -489,11 +540,11 @@ __global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(const __gri
         if (m > 1) {   // C-15: B_c^3 of a phi-derefined row is the group's value, from the group's two outer x3-faces
           const int k0 = id[2] - id[2] % m;
           int ig[3] = {id[0], id[1], k0};
-          GSrc s = blk_src(Dv, b, phys, 2, ig, same);
+          GSrc s = blk_src_tab(Dv, b, phys, 2, ig, same);
           if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
           lo[2] = fetch(7, s);
           ig[2] = k0 + m;
-          s = blk_src(Dv, b, phys, 2, ig, same);
+          s = blk_src_tab(Dv, b, phys, 2, ig, same);
           if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
           hi[2] = fetch(7, s);
         }
@@ -503,13 +554,13 @@ __global__ void __launch_bounds__(256, HAMR_GHOST_MINB) k_blk_ghosts(const __gri
         const int Mhi = max(m, __ldg(Dv.mrow + min(J + 1, Dv.B.n2g + NG) + NG));
         if (Mlo != m) {
           int ig[3] = {id[0], id[1], deref_face2_slot(id[2], n3, m, Mlo)};
-          const GSrc s = blk_src(Dv, b, phys, 1, ig, same);
+          const GSrc s = blk_src_tab(Dv, b, phys, 1, ig, same);
           if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
           lo[1] = fetch(6, s);
         }
         if (Mhi != m) {
           int ig[3] = {id[0], id[1] + 1, deref_face2_slot(id[2], n3, m, Mhi)};
-          const GSrc s = blk_src(Dv, b, phys, 1, ig, same);
+          const GSrc s = blk_src_tab(Dv, b, phys, 1, ig, same);
           if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
           hi[1] = fetch(6, s);
         }
@@ -993,6 +1044,17 @@ static cudaError_t blk_upload_flags(hamr_grid* g) {
   return cudaMemcpyAsync(g->D.B.flags, hf, (size_t)H.nblk * 4, cudaMemcpyHostToDevice, g->stream);
 }
 
+// (re)builds the ghost-source table if the time levels differ from those it was built for; the flags and levels must
+// have been uploaded on the stream before
+static void blk_build_gsrc(hamr_grid* g) {
+  BlkHost& H = g->bh;
+  if (!H.d_gsrc || H.gsrc_tau == H.tau) return;
+  const Dev D = dev_list(g, 4);
+  Launch l_(g, K_OTHER);
+  k_blk_src_table<<<dim3((D.B.gloc + 255) / 256, H.nblk), 256, 0, g->stream>>>(D, H.d_gsrc);
+  H.gsrc_tau = H.tau;
+}
+
 // C-16 x1 slots: a base block column whose x1-centre has r < r_refine_max (x1 itself on the Cartesian map)
 // is replaced by two children with dx1 / 2 (per-dimension splitting).  Returns the number of
 // refined columns (they must be contiguous from the low x1 side), -1 if they are not.
@@ -1050,9 +1112,16 @@ int blk_has_refinement(const hamr_params& p) {
   return blk_refined_columns(p, p.n[0] / bn[0], bn[0]) > 0 ? 1 : 0;
 }
 
-size_t blk_table_bytes(int nblk) {
-  // info (int4), nbr (NNBR), phys, K0, tau, cur, flags, 5 lists, 4 correction lists, ctopb (3 doubles)
-  return ((size_t)nblk * (16 + 4 * (NNBR + 5 + 5 + 4 + 5) + 24) + 1024 + 255) / 256 * 256;
+// the ghost-source table is kept when it stays below 4 GB (cfg 4: 1472 blocks x 12167 locations x 32 B = 0.57 GB; a grid
+// of a few huge blocks has few ghost zones per zone and computes the sources on the fly)
+static size_t blk_gsrc_bytes(int nblk, long long nloc) {
+  const unsigned long long bytes = (unsigned long long)nblk * 4ull * (unsigned long long)nloc * 8ull;
+  return (bytes <= (4ull << 30) && nloc < (1ll << 31) && nblk <= 65535) ? (size_t)bytes : 0;   // grid.y carries the block id
+}
+
+size_t blk_table_bytes(int nblk, long long nloc) {
+  // info (int4), nbr (NNBR), phys, K0, tau, cur, flags, 5 lists, 4 correction lists, ctopb (3 doubles), source table
+  return ((size_t)nblk * (16 + 4 * (NNBR + 5 + 5 + 4 + 5) + 24) + 1024 + 255) / 256 * 256 + blk_gsrc_bytes(nblk, nloc) + 256;
 }
 
 // C-16: block lattice, neighbour table (periodic dimensions close through it), per-block table offsets
@@ -1141,6 +1210,15 @@ int blk_setup(hamr_grid* g, void* tables) {
       if (deref_row_factor(p, J) > 1) H.hasderef[b] = 1;
   B.flags = (int*)take((size_t)nblk * 4);
   B.ctopb = (double*)take((size_t)nblk * 24);
+  {
+    const Lay& L = g->D.L;
+    const long long nloc = (long long)L.e1 * L.e2 * (L.n[2] + 2 * NG + 1);
+    const size_t gb = blk_gsrc_bytes(nblk, nloc);
+    H.d_gsrc = gb ? (unsigned long long*)take(gb) : nullptr;
+    H.gsrc_tau.clear();
+    B.gsrc = H.d_gsrc;
+    B.gloc = (int)nloc;
+  }
   B.info = d_info; B.nbr = d_nbr; B.phys = d_phys; B.K0 = d_K0;
   B.list = H.d_lists; B.nact = 0;
   if (cudaMallocHost((void**)&H.h_ctop, (size_t)nblk * 3 * sizeof(double)) != cudaSuccess) return HAMR_ECUDA;
@@ -1399,6 +1477,7 @@ static int blk_assign(hamr_grid* g, bool after_step) {
   if (e == cudaSuccess) e = cudaMemcpyAsync(g->D.B.tau, hl + (size_t)8 * nblk, (size_t)nblk * 4, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = blk_upload_flags(g);
   if (e == cudaSuccess) e = blk_upload_dlists(g);
+  if (e == cudaSuccess) blk_build_gsrc(g);
   H.dt0 = dt0;
   g->h_pinned[56] = dt0;
   if (e == cudaSuccess) e = cudaMemcpyAsync(g->D.scal + S_DT, g->h_pinned + 56, sizeof(double), cudaMemcpyHostToDevice, st);
@@ -1425,6 +1504,7 @@ int blk_initial(hamr_grid* g) {
   if (cudaStreamSynchronize(st) != cudaSuccess) return HAMR_ECUDA;   // the pinned staging area is reused
   if (blk_upload_flags(g) != cudaSuccess) return HAMR_ECUDA;
   if (blk_upload_dlists(g) != cudaSuccess) return HAMR_ECUDA;
+  blk_build_gsrc(g);
   // level-0 list = every block
   if (cudaMemcpyAsync(H.d_lists, H.d_lists + (size_t)4 * H.nblk, (size_t)H.nblk * 4, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
     return HAMR_ECUDA;

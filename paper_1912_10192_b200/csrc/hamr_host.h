@@ -41,6 +41,11 @@ struct BlkDev {
   const int* K0;             // [nblk] global x3 index of local zone 0
   int* tau;                  // [nblk] LAT time level (C-17)
   int* cur;                  // [nblk] which of the 3 buffers holds the block's time-n state (0 or 2)
+  // ghost-source table (blocks.cu): for every padded location of every block and each of the four array kinds
+  // (zone-centred, x1-, x2-, x3-faces) WHERE the ghost fill takes the value from, packed in 64 bits; a pure function of
+  // the block tables and the time levels, rebuilt when the levels change.  [nblk][4][gloc]; NULL: computed on the fly
+  const unsigned long long* gsrc;
+  int gloc;                  // padded locations per block: e1 * e2 * (n3 + 2 NG + 1)
   int* flags;                // [nblk] bit 0: ghost fill is a plain copy; bit 1: has a finer-level neighbour
   double* ctopb;             // [nblk][3] max signal speed of the block's last corrector pass (C-14)
   double* FA2[3][5];         // flux registers: dt_b F summed over the steps inside one coarser step (C-17)
@@ -130,6 +135,8 @@ struct BlkHost {
   double* h_ctop;            // pinned [nblk][3]
   int* h_ints;               // pinned [16][nblk]
   double dt0;                // host copy of the finest step (LAT)
+  unsigned long long* d_gsrc;  // device ghost-source table (NULL: none)
+  std::vector<int> gsrc_tau;   // the time levels the table was built for (empty: not built)
 };
 }
 
@@ -225,7 +232,7 @@ int blk_count(const hamr_params& p, int nslot[3], int bn[3]);       // number of
 int blk_has_refinement(const hamr_params& p);
 void blk_pack_one(hamr_grid* g, int b, const double* dense, int kind, int stag, bool zero_pole);
 void blk_unpack_one(hamr_grid* g, int b, int kind, double* dense);
-size_t blk_table_bytes(int nblk);                                   // device bytes of the block tables
+size_t blk_table_bytes(int nblk, long long nloc);                   // device bytes of the block tables; nloc: padded locations per block
 int blk_setup(hamr_grid* g, void* tables);                          // lattice, neighbour tables, lists
 void blk_pack(hamr_grid* g, const double* dense, int kind, int stag, bool zero_pole);  // kind: 0..4 P, 5..7 Bf
 void blk_unpack(hamr_grid* g, int kind, double* dense);             // kind: 0..4 P, 5..7 Bc, 8..10 Bf
