@@ -158,6 +158,11 @@ NCU_TRAFFIC = {"flux_x1": 539500000, "flux_x2": 523200000, "flux_x3": 498500000,
                "edge_emf": 534900000, "update_predictor": 1462600000, "update_corrector": 1736800000, "ghosts": 15600000}
 FLUX_FP64_INST_PER_FACE = {"flux_x1": 340.5, "flux_x2": 337.0, "flux_x3": 328.0}
 FLUX_FMA_FRACTION = 0.36           # the DFMA share of those (2 FLOP each), the rest DADD / DMUL (1 FLOP)
+# every instruction the flux kernels send down the FP64 pipe per face (the arithmetic above plus the compares behind
+# min / max / limiter switches), from the same capture: sm__pipe_fp64_cycles_active x cycles / 2 cycles per warp
+# instruction x 592 schedulers x 32 threads / faces; and all warp-level instructions per face-warp
+FLUX_FP64PIPE_INST_PER_FACE = {"flux_x1": 405.0, "flux_x2": 403.0, "flux_x3": 416.0}
+FLUX_INST_PER_FACE = {"flux_x1": 806.0, "flux_x2": 812.0, "flux_x3": 704.0}
 FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
 PAPER_V100_150CUBED = 0.85e8   # ~0.85e8 zone-cycles/s, 1 V100, one 150^3 block
 
@@ -389,8 +394,12 @@ def main():
     if rank == 0:
         sec0, ins0 = hamr.bench_fp64(0, 20000, torch.cuda.current_stream().cuda_stream)
         sec1, ins1 = hamr.bench_fp64(1, 20000, torch.cuda.current_stream().cuda_stream)
+        sec2, ins2 = hamr.bench_fp64(2, 20000, torch.cuda.current_stream().cuda_stream)
         fp64 = {"tflops_measured_dfma": 2.0 * ins0 / sec0 / 1e12, "ginstr_per_s_dfma": ins0 / sec0 / 1e9,
                 "ginstr_per_s_flux_mix": ins1 / sec1 / 1e9, "tflops_flux_mix": (4.0 / 3.0) * ins1 / sec1 / 1e12,
+                # FP64-pipe instruction rate when every 4 of them come with 5 select / integer instructions, as in
+                # the flux kernels (376 : 400 per face): what the machine sustains on THAT blend
+                "ginstr_per_s_flux_blend": ins2 / sec2 / 1e9,
                 "tflops_derived": FP64_PEAK_TFLOPS_DERIVED,
                 "how": "hamr_bench_fp64: 8 independent chains per thread, 64 warps per SM, 96 x 20000 instructions per thread"}
     clocks = sampler.stop()
@@ -521,6 +530,21 @@ def main():
                     "fp64_inst_per_face": FLUX_FP64_INST_PER_FACE, "inst_source": NCU_TRAFFIC_SOURCE,
                     "note": "executed dadd + dmul + dfma thread instructions per face (ncu) x faces / CUDA-event time, "
                             "against the MEASURED issue rate of the same instruction blend (hamr_bench_fp64 mix 1)"}
+        # The bound that holds for these kernels: of their ~800 instructions per face only half go down the FP64 pipe,
+        # and the others (selects, integer, shared-memory loads) take issue slots from it.  hamr_bench_fp64 mix 2 runs
+        # dependency-free chains with that blend (4 FP64-pipe : 5 other) on every scheduler; the flux kernels' FP64-pipe
+        # instruction rate is measured against the rate that microbenchmark sustains
+        pins = sum(FLUX_FP64PIPE_INST_PER_FACE[k] * nface[k] * kern[k]["launches"] for k in classes["flux"])
+        flux_alu["blend"] = {"achieved": pins / sec / 1e9, "peak": fp64["ginstr_per_s_flux_blend"],
+                             "unit": "G thread-instructions/s on the FP64 pipe (arithmetic + compares)",
+                             "frac": pins / sec / 1e9 / fp64["ginstr_per_s_flux_blend"],
+                             "fp64pipe_inst_per_face": FLUX_FP64PIPE_INST_PER_FACE, "inst_per_face": FLUX_INST_PER_FACE,
+                             "per_kernel_frac": {k: FLUX_FP64PIPE_INST_PER_FACE[k] * nface[k] * kern[k]["launches"] /
+                                                 (kern[k]["ms_total"] * 1e-3) / 1e9 / fp64["ginstr_per_s_flux_blend"]
+                                                 for k in classes["flux"]},
+                             "note": "FP64-pipe instruction rate of the flux kernels against the rate the same blend of "
+                                     "FP64-pipe and other instructions sustains without dependencies (hamr_bench_fp64 "
+                                     "mix 2: 4 FP64-pipe to 5 select / integer instructions; the kernels: 405 to ~400)"}
     roof = {"bound": "hbm", "kernel": "+".join(dk), "achieved": dom_gbs, "peak": hbm_peak, "unit": "GB/s",
             "frac": dom_gbs / hbm_peak, "traffic": traffic, "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": peak_src,
             "share_of_step": cshare[dom], "class_shares": {c: round(v, 4) for c, v in cshare.items()},

@@ -57,16 +57,21 @@ __global__ void k_zone_physics(Dev Dv, int what, int n, const int* __restrict__ 
   }
 }
 
-// 8 independent chains per thread; mix 0: DFMA only; mix 1: DFMA, DADD, DMUL in turn
+// 8 independent chains per thread; mix 0: DFMA only; mix 1: DFMA, DADD, DMUL in turn; mix 2: the flux kernels' whole
+// instruction blend: per chain and round the three FP64 arithmetic instructions, one double compare-and-select (DSETP
+// + 2 FSEL: how min / max / limiter switches compile, there is no FP64 min / max instruction) and two 32-bit integer
+// instructions on a chain of their own: 4 FP64-pipe : 4 other, against 376 : 400 per face in k_flux_ring
 template <int MIX>
 __global__ void __launch_bounds__(256) k_fp64_chains(int iters, double seed, double* sink) {
   double a[8];
+  unsigned h[8];
 #pragma unroll
-  for (int c = 0; c < 8; c++) a[c] = seed + 1e-3 * (threadIdx.x + 8 * c);
+  for (int c = 0; c < 8; c++) { a[c] = seed + 1e-3 * (threadIdx.x + 8 * c); h[c] = threadIdx.x * 2654435761u + c; }
   const double m = 1.0 - 1e-9, b = 1e-9;
+  const double cap = seed + 0.5, back = seed + 0.25;
   for (int it = 0; it < iters; it++) {
 #pragma unroll
-    for (int r = 0; r < 4; r++) {   // 4 rounds of 3 instructions on each of the 8 chains: 96 per iteration
+    for (int r = 0; r < 4; r++) {   // 4 rounds of 3 arithmetic instructions on each of the 8 chains: 96 per iteration
 #pragma unroll
       for (int c = 0; c < 8; c++) {
         if (MIX == 0) {
@@ -77,14 +82,19 @@ __global__ void __launch_bounds__(256) k_fp64_chains(int iters, double seed, dou
           a[c] = fma(a[c], m, b);
           a[c] = a[c] + b;
           a[c] = a[c] * m;
+          if (MIX == 2) {
+            a[c] = a[c] < cap ? a[c] : back;                 // DSETP + 2 FSEL
+            h[c] = (h[c] ^ (h[c] >> 15)) + 0x9e3779b9u;      // LOP3 (with the shift folded or a SHF) + IADD3
+          }
         }
       }
     }
   }
   double t = 0.0;
+  unsigned hs = 0;
 #pragma unroll
-  for (int c = 0; c < 8; c++) t += a[c];
-  if (t == 123.456) sink[0] = t;   // never true: keeps the chains alive
+  for (int c = 0; c < 8; c++) { t += a[c]; hs ^= h[c]; }
+  if (t == 123.456 || (MIX == 2 && hs == 0x12345u)) sink[0] = t;   // never true: keeps the chains alive
 }
 
 int zone_call(hamr_grid* g, int what, int n, const int* ti, const int* tj, const double* in, int nin,
@@ -186,7 +196,7 @@ int hamr_debug_floors_drift(hamr_grid* g, int n, const int* ti, const int* tj, d
 }
 
 int hamr_bench_fp64(void* cuda_stream, int mix, int iters, double* seconds, double* thread_instructions) {
-  if (!seconds || !thread_instructions || iters < 1 || (mix != 0 && mix != 1)) return HAMR_EINVAL;
+  if (!seconds || !thread_instructions || iters < 1 || mix < 0 || mix > 2) return HAMR_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int dev = 0, sms = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return HAMR_ECUDA;
@@ -199,7 +209,8 @@ int hamr_bench_fp64(void* cuda_stream, int mix, int iters, double* seconds, doub
   const int blocks = sms * 8, threads = 256;   // 64 warps per SM: every scheduler has 16 warps of 8 chains
   auto run = [&](int it) {
     if (mix == 0) k_fp64_chains<0><<<blocks, threads, 0, st>>>(it, 1.0, sink);
-    else k_fp64_chains<1><<<blocks, threads, 0, st>>>(it, 1.0, sink);
+    else if (mix == 1) k_fp64_chains<1><<<blocks, threads, 0, st>>>(it, 1.0, sink);
+    else k_fp64_chains<2><<<blocks, threads, 0, st>>>(it, 1.0, sink);
   };
   run(iters / 10 + 1);   // warm-up
   cudaEventRecord(a, st);
@@ -213,7 +224,8 @@ int hamr_bench_fp64(void* cuda_stream, int mix, int iters, double* seconds, doub
   cudaFree(sink);
   if (e != cudaSuccess) return HAMR_ECUDA;
   *seconds = 1e-3 * ms;
-  *thread_instructions = 96.0 * iters * (double)blocks * threads;
+  // FP64-pipe instructions: 96 arithmetic ones per iteration, plus 32 compares in the blend
+  *thread_instructions = (mix == 2 ? 128.0 : 96.0) * iters * (double)blocks * threads;
   return HAMR_OK;
 }
 
