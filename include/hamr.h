@@ -144,8 +144,8 @@ const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the 
  * 2017)"): a zone below a floor is raised to it with the velocity perpendicular to the magnetic field unchanged and
  * the momentum along the field, (rho + gamma_ad u) gamma^2 v_par, conserved; zones without field get the fluid-frame
  * floors.  The Lorentz-factor ceiling follows as before.
- * Both options need a grid of one block (nb = 0, no LAT, no derefinement, no refinement), else HAMR_EINVAL; such a
- * grid then runs on the generic kernels (the shared-memory staged ones carry eight variables). */
+ * Both options need a grid of one block (nb = 0, no LAT, no derefinement, no refinement), else HAMR_EINVAL.  The
+ * staged kernels carry the ninth row where they serve the grid (cfg 2 with both options: 80 % of its plain rate). */
 
 /* ---- block-structured grid (BASELINE.json cfg 4) ------------------ */
 /* A grid with nb != {0,0,0} or lat_max_level > 0 is cut into blocks of nb zones (nb[d] = 0: the whole

@@ -48,7 +48,7 @@ __global__ void k_zone_physics(Dev Dv, int what, int n, const int* __restrict__ 
       for (int c = 0; c < 3; c++) Bc[c] = in2[(size_t)s * 3 + c];
       nrf = P[0] < rfl;
       nuf = P[1] < ufl;
-      if (nrf | nuf) floors_drift(&G, Bc, Dv.gam, nrf ? rfl : P[0], nuf ? ufl : P[1], P);
+      if (nrf | nuf) floors_drift(G, Bc, Dv.gam, nrf ? rfl : P[0], nuf ? ufl : P[1], P);
       ceiling_only(G, Dv.gamma_max, P, ngc);
     } else
     floors_ceiling(G, rfl, ufl, Dv.gamma_max, P, nrf, nuf, ngc);

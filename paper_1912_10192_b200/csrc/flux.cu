@@ -369,7 +369,9 @@ static_assert(RING >= 6, "three live rows, one dying, two in flight");
 // resident warps per SM the register budget of the staged kernels is set for: 12 (168 registers, no spills) measured
 // best of 8 / 10 / 11 / 12 / 13-16 (profiles/r2_experiments.md)
 constexpr int RING_WARPS = 12;
-template <int D, int KT>
+// ENT (C-18): kappa of the zones (Dv.K) is a ninth staged array and an eighth reconstructed variable; the flux of the
+// entropy row goes to Dv.FK[D] (still 168 registers without spills).
+template <int D, int KT, bool ENT = false>
 __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, Fields s, int seg, int want_ctop) {
   static_assert(D == 0 || D == 1, "marching kernels sweep x1 or x2");
   using namespace ring;
@@ -377,7 +379,10 @@ __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, 
   constexpr int O = 1 - D;
   constexpr int e = (D + 1) % 3, f = (D + 2) % 3;
   constexpr int NW = KT / 32;              // warps of the CTA; warp 0 also is the producer
-  constexpr int SLOTD = 8 * KT + NREC_F;   // doubles per ring slot: 7 variables, the face field, the face record
+  constexpr int NVR = ENT ? 8 : 7;         // reconstructed variables
+  constexpr int KOFF = 8 * KT + NREC_F;    // where kappa sits in a slot (ENT)
+  constexpr int SLOTD = (ENT ? 9 : 8) * KT + NREC_F;   // doubles per ring slot: 7 variables, the face field, the face record (, kappa)
+  constexpr int voff[8] = {0, KT, 2 * KT, 3 * KT, 4 * KT, 5 * KT, 6 * KT, KOFF};
   extern __shared__ __align__(128) double ring_mem[];
   unsigned long long* mbar = reinterpret_cast<unsigned long long*>(ring_mem + RING * SLOTD);   // slot filled
   unsigned long long* mbe = mbar + RING;                                                         // slot released
@@ -405,7 +410,8 @@ __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, 
         double* dst = ring_mem + pslot * SLOTD;
         unsigned long long* mb = mbar + pslot;
         const bool face = prow >= f0 && prow < f1;   // rows that are also faces of this segment carry field and record
-        mbar_expect(mb, (unsigned)((face ? 8 * KT + NREC_F : 7 * KT) * sizeof(double)));
+        mbar_expect(mb, (unsigned)(((face ? 8 * KT + NREC_F : 7 * KT) + (ENT ? KT : 0)) * sizeof(double)));
+        if (ENT) bulk_g2s(dst + KOFF, Dv.K + pz, KT * sizeof(double), mb);
         bulk_g2s(dst + 0 * KT, s.P[0] + pz, KT * sizeof(double), mb);
         bulk_g2s(dst + 1 * KT, s.P[1] + pz, KT * sizeof(double), mb);
         bulk_g2s(dst + 2 * KT, s.P[2] + pz, KT * sizeof(double), mb);
@@ -435,11 +441,11 @@ __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, 
     if (prow <= rlast) issue_next();
   const bool act = o >= 0 && o < L.n[O];  // C-14: faces of ACTIVE zones (every k of the launch is active)
   const bool ks = Dv.metric == HAMR_METRIC_KERR_SCHILD;
-  constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + e, 5 + f};
+  constexpr int slot[8] = {0, 1, 2, 3, 4, 5 + e, 5 + f, 8};
   int z = (int)L.idx(D == 0 ? f0 - 1 : o, D == 0 ? o : f0 - 1, k);
   // the periodic images: column n3 - 1 also is column -1, column 0 also is column n3
   const int dup = (k == L.n[2] - 1) ? -L.n[2] : (k == 0 ? L.n[2] : 0);
-  double PL[8], PR[8], dm[7], il[7];
+  double PL[9], PR[9], dm[8], il[8];
   double ctop = 0.0;
   // prologue: the parabola of zone f0 - 1 from rows f0 - 3 .. f0 + 1 (slots 0 .. 4 of the first revolution)
 #pragma unroll
@@ -447,9 +453,9 @@ __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, 
   {
     const double* a = ring_mem + t;
 #pragma unroll
-    for (int v = 0; v < 7; v++) {
-      const double m2 = a[0 * SLOTD + v * KT], m1 = a[1 * SLOTD + v * KT], c0 = a[2 * SLOTD + v * KT],
-                   p1 = a[3 * SLOTD + v * KT], p2 = a[4 * SLOTD + v * KT];
+    for (int v = 0; v < NVR; v++) {
+      const double m2 = a[0 * SLOTD + voff[v]], m1 = a[1 * SLOTD + voff[v]], c0 = a[2 * SLOTD + voff[v]],
+                   p1 = a[3 * SLOTD + voff[v]], p2 = a[4 * SLOTD + voff[v]];
       const double d10 = m1 - m2, d21 = c0 - m1, d32 = p1 - c0, d43 = p2 - p1;
       const double dm_m = lim_slope(d10, d21, 0.5 * (c0 - m2));
       const double dm_0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
@@ -478,10 +484,10 @@ __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, 
     const double* r0 = ring_mem + s0 * SLOTD + t;
     const double* r1 = ring_mem + s1 * SLOTD + t;
     const double* r2 = ring_mem + s2 * SLOTD + t;
-    double carry[7];
+    double carry[8];
 #pragma unroll
-    for (int v = 0; v < 7; v++) {
-      const double c0 = r0[v * KT], c1 = r1[v * KT], a2 = r2[v * KT];
+    for (int v = 0; v < NVR; v++) {
+      const double c0 = r0[voff[v]], c1 = r1[voff[v]], a2 = r2[voff[v]];
       const double d21 = c1 - c0, d32 = a2 - c1;
       const double dmp = lim_slope(d21, d32, 0.5 * (a2 - c0));
       const double r = ppm_iface(c0, d21, dm[v], dmp);
@@ -489,17 +495,21 @@ __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, 
       dm[v] = dmp; il[v] = r;
     }
     const bool pole = (D == 1) && ks && (fc == 0 || fc == L.n[1]);
-    double out[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // C-7: pole faces carry no flux and no state is evaluated there
+    double out[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // C-7: pole faces carry no flux and no state is evaluated there
     if (!pole) {
       const FGeo G = load_fgeo_shared(ring_mem + s0 * SLOTD + 8 * KT);
       PL[5 + D] = PR[5 + D] = r0[7 * KT] * G.igdet;  // C-5: the normal field is single-valued at the face
-      const double ct = face_flux<D>(PL, PR, G, Dv.gam, out);
+      const double ct = face_flux<D, ENT>(PL, PR, G, Dv.gam, out);
       if (act) ctop = dmax(ctop, ct);
     }
     store_face(Dv, D, z, out);
-    if (dup != 0) store_face(Dv, D, z + dup, out);
+    if (ENT) Dv.FK[D][z] = out[7];
+    if (dup != 0) {
+      store_face(Dv, D, z + dup, out);
+      if (ENT) Dv.FK[D][z + dup] = out[7];
+    }
 #pragma unroll
-    for (int v = 0; v < 7; v++) PL[slot[v]] = carry[v];
+    for (int v = 0; v < NVR; v++) PL[slot[v]] = carry[v];
   }
   if (want_ctop) ctop_commit<false>(Dv, D, 0, ctop);
 }
@@ -581,7 +591,10 @@ __global__ void __launch_bounds__(128, ENT ? 4 : X3_MINB) k_flux_x3(Dev Dv, Fiel
     const double ct = face_flux<D, ENT>(PL, PR, G, Dv.gam, out);
     store_face(Dv, D, z, out);
     if (ENT) Dv.FK[D][z] = out[7];
-    if (WRAP && k == 0) store_face(Dv, D, z + L.n[2], out);
+    if (WRAP && k == 0) {
+      store_face(Dv, D, z + L.n[2], out);
+      if (ENT) Dv.FK[D][z + L.n[2]] = out[7];
+    }
     if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct;
   }
   if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
@@ -594,19 +607,20 @@ __global__ void __launch_bounds__(128, ENT ? 4 : X3_MINB) k_flux_x3(Dev Dv, Fiel
 // no ghost zone is read).  The left / right states of the row's n3 faces go through shared memory (14 doubles per
 // face), because the Riemann problems are then solved with lanes on CONSECUTIVE faces (coalesced stores).
 // A warp walks over a contiguous range of rows; each row's stencil lines are prefetched into L2 one row ahead.
-template <int M>
+template <int M, bool ENT = false>
 __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields s, int seg, int want_ctop) {
   constexpr int D = 2;
   constexpr unsigned FULL = 0xffffffffu;
   constexpr int QS = (M == 1) ? 32 : 32 + 16 / M;   // slot stride between a lane's zones: conflict-free both ways
   constexpr int NV = M * QS;                         // doubles per variable and side
-  __shared__ double lr[14 * NV];
+  constexpr int NVR = ENT ? 8 : 7;                   // reconstructed variables (C-18: kappa is the eighth)
+  __shared__ double lr[2 * NVR * NV];
   const Lay& L = Dv.L;
   const int lane = threadIdx.x;
   const int n3 = 32 * M, cj = L.n[1] + 2;
   const int nrow = (L.n[0] + 2) * cj;
   const int r0 = blockIdx.x * seg, r1 = min(r0 + seg, nrow);
-  const double* var[7] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[0], s.Bc[1]};
+  const double* var[8] = {s.P[0], s.P[1], s.P[2], s.P[3], s.P[4], s.Bc[0], s.Bc[1], Dv.K};
   const int up = (lane + 31) & 31, dn = (lane + 1) & 31;   // the lanes owning the zones before / after this lane's
   double ctop = 0.0;
   for (int row = r0; row < r1; row++) {
@@ -616,7 +630,7 @@ __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields 
       const int i2 = (row + 1) / cj - 1, j2 = (row + 1) - (i2 + 1) * cj - 1;
       const int zn = (int)L.idx(i2, j2, 0) + 16 * lane;
 #pragma unroll
-      for (int v = 0; v < 7; v++) asm volatile("prefetch.global.L2 [%0];" ::"l"(var[v] + zn));
+      for (int v = 0; v < NVR; v++) asm volatile("prefetch.global.L2 [%0];" ::"l"(var[v] + zn));
       asm volatile("prefetch.global.L2 [%0];" ::"l"(s.Bf[2] + zn));
     }
     // the row's face record and the normal field of this lane's faces are requested with the stencil: they are
@@ -627,7 +641,7 @@ __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields 
     for (int q2 = 0; q2 < M; q2++) bf3[q2] = __ldg(s.Bf[2] + zr + lane + 32 * q2);
     // ---- phase 1: parabolas of the lane's M zones, states of their low faces to shared memory ----
 #pragma unroll
-    for (int v = 0; v < 7; v++) {
+    for (int v = 0; v < NVR; v++) {
       double a[M + 2];   // zones M l - 1 .. M l + M
       if (M >= 2) {
         const double2* a2 = reinterpret_cast<const double2*>(var[v] + zr + M * lane);
@@ -649,7 +663,7 @@ __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields 
       for (int q = 0; q < M; q++) {
         double aL, aR;
         ppm_mono(l, a[q + 1], r[q], aL, aR);
-        lr[(7 + v) * NV + q * QS + lane] = aL;                  // right state of the zone's low face
+        lr[(NVR + v) * NV + q * QS + lane] = aL;                  // right state of the zone's low face
         if (q + 1 < M) lr[v * NV + (q + 1) * QS + lane] = aR;   // left state of the next zone's low face
         else aRlast = aR;
         l = r[q];
@@ -663,23 +677,28 @@ __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields 
     for (int q2 = 0; q2 < M; q2++) {
       const int f = lane + 32 * q2;                  // face = zone index
       const int sl = (f % M) * QS + f / M;
-      double PL[8], PR[8];
+      double PL[9], PR[9];
 #pragma unroll
-      for (int v = 0; v < 7; v++) { PL[v] = lr[v * NV + sl]; PR[v] = lr[(7 + v) * NV + sl]; }
+      for (int v = 0; v < 7; v++) { PL[v] = lr[v * NV + sl]; PR[v] = lr[(NVR + v) * NV + sl]; }
+      if (ENT) { PL[8] = lr[7 * NV + sl]; PR[8] = lr[(NVR + 7) * NV + sl]; }
       const int z = zr + f;
       PL[7] = PR[7] = bf3[q2] * G.igdet;
-      double out[7];
-      const double ct = face_flux<D>(PL, PR, G, Dv.gam, out);
+      double out[8];
+      const double ct = face_flux<D, ENT>(PL, PR, G, Dv.gam, out);
       if (act) ctop = dmax(ctop, ct);
       store_face(Dv, D, z, out);
-      if (f == 0) store_face(Dv, D, z + n3, out);   // the face at k = n3 is the periodic image of the face at k = 0
+      if (ENT) Dv.FK[D][z] = out[7];
+      if (f == 0) {   // the face at k = n3 is the periodic image of the face at k = 0
+        store_face(Dv, D, z + n3, out);
+        if (ENT) Dv.FK[D][z + n3] = out[7];
+      }
     }
     __syncwarp();
   }
   if (want_ctop) ctop_commit<false>(Dv, D, 0, ctop);
 }
 
-template <int M>
+template <int M, bool ENT = false>
 static void launch_x3_warp_t(hamr_grid* g, const Dev& Dv, const Fields& src, bool want_ctop) {
   const Lay& L = Dv.L;
   // occupancy cached per host thread and device (a grid is driven by one thread at a time; two grids may be driven concurrently)
@@ -688,7 +707,7 @@ static void launch_x3_warp_t(hamr_grid* g, const Dev& Dv, const Fields& src, boo
   cudaGetDevice(&dev);
   if (dev != cached_dev) {
     int v = 1;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_flux_x3_warp<M>, 32, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_flux_x3_warp<M, ENT>, 32, 0);
     per_sm = v < 1 ? 1 : v;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cached_dev = dev;
@@ -701,7 +720,7 @@ static void launch_x3_warp_t(hamr_grid* g, const Dev& Dv, const Fields& src, boo
   int nw = waves * slots;
   if (nw > nrow) nw = nrow;
   const int seg = (nrow + nw - 1) / nw;
-  k_flux_x3_warp<M><<<(nrow + seg - 1) / seg, 32, 0, g->stream>>>(Dv, src, seg, want_ctop ? 1 : 0);
+  k_flux_x3_warp<M, ENT><<<(nrow + seg - 1) / seg, 32, 0, g->stream>>>(Dv, src, seg, want_ctop ? 1 : 0);
 }
 
 static int ring_width(const Dev& Dv);
@@ -834,19 +853,19 @@ static void launch_march_t(hamr_grid* g, const Dev& Dv, const Fields& src, const
 }
 
 // the ring kernel: segment length such that the grid fills whole waves of resident CTAs
-template <int D, int KT>
+template <int D, int KT, bool ENT = false>
 static void launch_ring_t(hamr_grid* g, const Dev& Dv, const Fields& src, bool want_ctop) {
   const Lay& L = Dv.L;
   const int O = 1 - D;
-  const size_t smem = (size_t)ring::RING * ((8 * KT + NREC_F) * sizeof(double)) + 2 * ring::RING * sizeof(unsigned long long);
+  const size_t smem = (size_t)ring::RING * (((ENT ? 9 : 8) * KT + NREC_F) * sizeof(double)) + 2 * ring::RING * sizeof(unsigned long long);
   // the attribute and the occupancy are per function and device; cached per host thread
   thread_local int per_sm = 0, sms = 148, cached_dev = -1;
   int dev = 0;
   cudaGetDevice(&dev);
   if (dev != cached_dev) {
-    cudaFuncSetAttribute(k_flux_ring<D, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_flux_ring<D, KT, ENT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     int v = 1;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_flux_ring<D, KT>, KT, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_flux_ring<D, KT, ENT>, KT, smem);
     per_sm = v < 1 ? 1 : v;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cached_dev = dev;
@@ -865,14 +884,13 @@ static void launch_ring_t(hamr_grid* g, const Dev& Dv, const Fields& src, bool w
     if (eff > best) { best = eff; best_seg = seg; }
   }
   dim3 grid(L.n[2] / KT, L.n[O] + 2, (nf + best_seg - 1) / best_seg);
-  k_flux_ring<D, KT><<<grid, KT, smem, g->stream>>>(Dv, src, best_seg, want_ctop ? 1 : 0);
+  k_flux_ring<D, KT, ENT><<<grid, KT, smem, g->stream>>>(Dv, src, best_seg, want_ctop ? 1 : 0);
 }
 
 // the shared-memory ring serves monolithic PPM grids whose x3 extent is periodic, not derefined, and a multiple of 32
 static int ring_width(const Dev& Dv) {
   const int n3 = Dv.L.n[2];
   if (Dv.B.nblk > 0 || Dv.recon != HAMR_RECON_PPM || Dv.mrow || Dv.bc_lo[2] != HAMR_BC_PERIODIC) return 0;
-  if (Dv.entropy) return 0;   // C-18: the entropy row is carried by the generic kernels
   if (Dv.L.n[0] + 2 > 65535 || Dv.L.n[1] + 2 > 65535) return 0;
   // one warp per CTA: 64 / 128 threads (slots released through the second mbarrier) measured 3-7 % slower
   return n3 % 32 == 0 ? 32 : 0;
@@ -887,7 +905,8 @@ template <int D>
 static void launch_march(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
   Launch l_(g, K_FLUX1 + D);
   const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
-  if (ring_width(Dv) == 32) return launch_ring_t<D, 32>(g, Dv, src, want_ctop);
+  if (ring_width(Dv) == 32)
+    return Dv.entropy ? launch_ring_t<D, 32, true>(g, Dv, src, want_ctop) : launch_ring_t<D, 32, false>(g, Dv, src, want_ctop);
   if (Dv.entropy) {   // C-18 (monolithic grids only: checked at creation)
     if (ppm) launch_march_t<D, HAMR_RECON_PPM, false, true>(g, Dv, src, src2, want_ctop);
     else launch_march_t<D, HAMR_RECON_PLM_MC, false, true>(g, Dv, src, src2, want_ctop);
@@ -914,13 +933,17 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
   const int wc = want_ctop ? 1 : 0;
   {
     Launch l_(g, K_FLUX3);
-    switch (x3_warp_m(Dv)) {
+    switch (x3_warp_m(Dv) * (Dv.entropy ? -1 : 1)) {
       case 1: launch_x3_warp_t<1>(g, Dv, src, want_ctop); return;
       case 2: launch_x3_warp_t<2>(g, Dv, src, want_ctop); return;
       case 4: launch_x3_warp_t<4>(g, Dv, src, want_ctop); return;
+      case -1: launch_x3_warp_t<1, true>(g, Dv, src, want_ctop); return;
+      case -2: launch_x3_warp_t<2, true>(g, Dv, src, want_ctop); return;
+      case -4: launch_x3_warp_t<4, true>(g, Dv, src, want_ctop); return;
       default: break;
     }
-    if (Dv.entropy && ppm) k_flux_x3<HAMR_RECON_PPM, false, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    if (Dv.entropy && x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (Dv.entropy && ppm) k_flux_x3<HAMR_RECON_PPM, false, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (Dv.entropy) k_flux_x3<HAMR_RECON_PLM_MC, false, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (ppm && !blk) k_flux_x3<HAMR_RECON_PPM, false, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);

@@ -281,6 +281,12 @@ __device__ __forceinline__ void floors_ceiling(const CGeo& G, double rfl, double
   ceiling_only(G, gamma_max, Pn, ngc);
 }
 
+// kappa = (gamma_ad - 1) u rho^-gamma_ad through exp / log (each good to an ulp; |gamma_ad ln rho| < 100 keeps the
+// result within 1e-14 of the correctly rounded power at a third of the cost of the library's pow)
+__device__ __forceinline__ double kappa_of(double rho, double u, double gam_ad) {
+  return (gam_ad - 1.0) * u * exp(-gam_ad * log(rho));
+}
+
 // ---- C-18: the entropy row and the inversion that uses it ------------------------
 // kappa = p / rho^gamma_ad is carried by the mass: the row is gdet rho u^t kappa with flux gdet rho u^d kappa and no
 // source.  Where the energy inversion fails (or returns rho <= 0 or u < 0) the zone is inverted from the density,
@@ -353,25 +359,26 @@ static __device__ __noinline__ int con2prim_entropy(const double* __restrict__ U
 // it: with v = ut / gamma = v_perp + v_par Bhat in the normal observer's frame, v_perp is kept and v_par follows
 // from the conserved field-aligned momentum  m = w gamma^2 v_par  (w = rho + gamma_ad u):
 //   v_par' = 2 m s / (w' + sqrt(w'^2 + 4 m^2 s)),  s = 1 - v_perp^2.     Called only for a zone below a floor.
-static __device__ __noinline__ void floors_drift(const CGeo* __restrict__ Gp, const double* __restrict__ Bc, double gam_ad,
-                                          double rho_new, double u_new, double* __restrict__ Pn) {
-  const CGeo& G = *Gp;
+// (inline: on a torus whose atmosphere sits at the floors this runs for almost half of the zone updates; reciprocals
+// and roots from the hardware seed as in the rest of the per-zone physics)
+__device__ __forceinline__ void floors_drift(const CGeo& G, const double Bc[3], double gam_ad, double rho_new, double u_new,
+                                             double Pn[5]) {
   const double B1 = G.alpha * Bc[0], B2 = G.alpha * Bc[1], B3 = G.alpha * Bc[2];
   const double Bl1 = G.c11 * B1 + G.c13 * B3, Bl2 = G.c22 * B2, Bl3 = G.c13 * B1 + G.c33 * B3;
   const double Bsq = B1 * Bl1 + B2 * Bl2 + B3 * Bl3;
-  if (!(Bsq > 0.0)) { Pn[0] = rho_new; Pn[1] = u_new; return; }   // no field: the fluid frame
-  const double q = Pn[2] * (G.c11 * Pn[2] + G.c13 * Pn[4]) + Pn[3] * (G.c22 * Pn[3]) + Pn[4] * (G.c13 * Pn[2] + G.c33 * Pn[4]);
-  const double gamma = sqrt(1.0 + q), ig = 1.0 / gamma;
+  if (!(Bsq > 1e-300)) { Pn[0] = rho_new; Pn[1] = u_new; return; }   // no field: the fluid frame
+  const double q1 = 1.0 + (Pn[2] * (G.c11 * Pn[2] + G.c13 * Pn[4]) + Pn[3] * (G.c22 * Pn[3]) + Pn[4] * (G.c13 * Pn[2] + G.c33 * Pn[4]));
+  const double ig = rsqrt_pos(q1);                                   // 1 / gamma
   const double v1 = Pn[2] * ig, v2 = Pn[3] * ig, v3 = Pn[4] * ig;
-  const double iB = 1.0 / sqrt(Bsq);
+  const double iB = rsqrt_pos(Bsq);
   const double vpar = (v1 * Bl1 + v2 * Bl2 + v3 * Bl3) * iB;
-  const double h1 = B1 * iB, h2 = B2 * iB, h3 = B3 * iB;           // unit vector along the field
+  const double h1 = B1 * iB, h2 = B2 * iB, h3 = B3 * iB;             // unit vector along the field
   const double p1 = v1 - vpar * h1, p2 = v2 - vpar * h2, p3 = v3 - vpar * h3;
   const double vperp2 = p1 * (G.c11 * p1 + G.c13 * p3) + p2 * (G.c22 * p2) + p3 * (G.c13 * p1 + G.c33 * p3);
-  const double m = (Pn[0] + gam_ad * Pn[1]) * (1.0 + q) * vpar;
+  const double m = (Pn[0] + gam_ad * Pn[1]) * q1 * vpar;
   const double wn = rho_new + gam_ad * u_new, s = 1.0 - vperp2;
-  const double vpn = 2.0 * m * s / (wn + sqrt(wn * wn + 4.0 * m * m * s));
-  const double gn = 1.0 / sqrt(s - vpn * vpn);
+  const double vpn = 2.0 * m * s * rcp_nr(wn + sqrt_pos(wn * wn + 4.0 * m * m * s));
+  const double gn = rsqrt_pos(s - vpn * vpn);
   Pn[0] = rho_new;
   Pn[1] = u_new;
   Pn[2] = gn * (p1 + vpn * h1);

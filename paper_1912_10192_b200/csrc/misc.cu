@@ -166,7 +166,7 @@ __global__ void k_kappa(Dev Dv, Fields s) {
   const long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (z >= Dv.L.len) return;
   const double rho = s.P[0][z], u = s.P[1][z];
-  Dv.K[z] = rho > 0.0 ? (Dv.gam - 1.0) * u * pow(rho, -Dv.gam) : 0.0;
+  Dv.K[z] = rho > 0.0 ? kappa_of(rho, u, Dv.gam) : 0.0;
 }
 
 void launch_kappa(hamr_grid* g, const Fields& s) {

@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(128, ROB ? 4 : (SAME ? UPD_MINB_PRED : UPD_MIN
         double div = 0.0;
 #pragma unroll
         for (int d = 0; d < 3; d++) div += (__ldg(Dv.FK[d] + z + S[d]) - __ldg(Dv.FK[d] + z)) * idx[d];
-        US = U[0] * ((Dv.gam - 1.0) * u_b * pow(rho_b, -Dv.gam)) - dt * div;
+        US = U[0] * kappa_of(rho_b, u_b, Dv.gam) - dt * div;
       }
       // U_new = U_base - dt sum_d (F^d_+ - F^d_-)/dx^d + dt S
 #pragma unroll
@@ -176,17 +176,7 @@ __global__ void __launch_bounds__(128, ROB ? 4 : (SAME ? UPD_MINB_PRED : UPD_MIN
       if (ROB && Dv.drift) {
         nrf = Pn[0] < rfl;
         nuf = Pn[1] < ufl;
-        if (nrf | nuf) {
-          double Bc[3], Pc[5];
-          CGeo Gc = G2;
-#pragma unroll
-          for (int c = 0; c < 5; c++) Pc[c] = Pn[c];
-#pragma unroll
-          for (int c = 0; c < 3; c++) Bc[c] = Bn[c];
-          floors_drift(&Gc, Bc, Dv.gam, nrf ? rfl : Pn[0], nuf ? ufl : Pn[1], Pc);
-#pragma unroll
-          for (int c = 0; c < 5; c++) Pn[c] = Pc[c];
-        }
+        if (nrf | nuf) floors_drift(G2, Bn, Dv.gam, nrf ? rfl : Pn[0], nuf ? ufl : Pn[1], Pn);
         ceiling_only(G2, Dv.gamma_max, Pn, ngc);
       } else {
         floors_ceiling(G2, rfl, ufl, Dv.gamma_max, Pn, nrf, nuf, ngc);
@@ -231,7 +221,10 @@ constexpr int TJ = 2;            // rows per CTA: 1 / 3 / 4 measured 5-19 % slow
 constexpr int NA = 8, NB = 13;   // arrays keeping two planes / one plane
 }
 
-template <bool SAME, int NT>
+// ROB: the robust path of k_update above (C-18 entropy row and backup inversion, C-19 drift-frame floors).  The three
+// entropy fluxes are not staged (a third CTA-plane set would halve the CTAs per SM): each zone reads its six values
+// directly, requested with the zone-centred inputs at the top of the step.
+template <bool SAME, int NT, bool ROB = false>
 __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, double dtfac, int seg) {
   using namespace tile;
   using namespace tma;
@@ -279,7 +272,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
   }
   __syncthreads();
   request(i0, i0 + 1, i0);
-  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0;
+  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0, nent = 0;
   const int sk = jj * L.p3 + k;                    // this thread's element inside a staged chunk
   for (int i = i0; i < i1; i++) {
     const bool in0 = i < L.n[0];
@@ -299,6 +292,10 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
         for (int c = 0; c < 3; c++) Pb[5 + c] = __ldg(r.base.Bc[c] + z);
       }
     }
+    double divK = 0.0;   // C-18: divergence of the entropy flux
+    if (ROB && zone && Dv.entropy)
+      divK = (__ldg(Dv.FK[0] + z + L.S1) - __ldg(Dv.FK[0] + z)) * ix0 + (__ldg(Dv.FK[1] + z + L.S2) - __ldg(Dv.FK[1] + z)) * ix1 +
+             (__ldg(Dv.FK[2] + z + 1) - __ldg(Dv.FK[2] + z)) * ix2;
     // The corrector evaluates its two input states BEFORE the staged part (16 doubles of input become 7 of result
     // while the copies land: measured 0.393 -> 0.369 ms); the predictor, with one input state, is faster the other
     // way round (0.274 vs 0.293 ms)
@@ -363,6 +360,11 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
         prim_to_U5(Ps, Ss, G.gdet, Dv.gam, U);
         source_12(Ps, Ss, G, Dv.gam, grec, S1, S2);   // C-12: on the stage's source state
       }
+      double US = 0.0;
+      if (ROB && Dv.entropy) {   // C-18: the base state's entropy row is its density row times kappa; no source term
+        const double rho_b = SAME ? Ps[0] : Pb[0], u_b = SAME ? Ps[1] : Pb[1];
+        US = U[0] * kappa_of(rho_b, u_b, Dv.gam) - dt * divK;
+      }
       // U_new = U_base - dt sum_d (F^d_+ - F^d_-)/dx^d + dt S
 #pragma unroll
       for (int c = 0; c < 5; c++) {
@@ -370,13 +372,40 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
         U[c] = U[c] - dt * div[c] + dt * sc;
       }
       double Pn[5];
-      if (con2prim(U, Bn, G, Dv.gam, Ps, Pn) != 0) {  // C-13: keep the source state's hydro primitives, count the failure
+      int rc = con2prim(U, Bn, G, Dv.gam, Ps, Pn);
+      if (ROB && Dv.entropy) {
+        Dv.K[z] = US / U[0];   // the advected kappa (diagnostic: k_kappa overwrites it before the next flux pass)
+        if (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) {
+          // the rare call works on copies, so that the common path's U, Bn, Ps and record stay in registers
+          double Pe[5], Uc[5], Bc[3], Pc[5];
+          CGeo Gc = G;
+#pragma unroll
+          for (int c = 0; c < 5; c++) { Uc[c] = U[c]; Pc[c] = Ps[c]; }
+#pragma unroll
+          for (int c = 0; c < 3; c++) Bc[c] = Bn[c];
+          if (con2prim_entropy(Uc, US, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
+#pragma unroll
+            for (int c = 0; c < 5; c++) Pn[c] = Pe[c];
+            rc = 0;
+            nent++;
+          }
+        }
+      }
+      if (rc != 0) {  // C-13: keep the source state's hydro primitives, count the failure
         nfail++;
 #pragma unroll
         for (int c = 0; c < 5; c++) Pn[c] = Ps[c];
       }
       int frf = 0, fuf = 0, fgc = 0;
-      floors_ceiling(G, __ldg(Dv.rho_fl + i + NG), __ldg(Dv.u_fl + i + NG), Dv.gamma_max, Pn, frf, fuf, fgc);
+      const double rfl = __ldg(Dv.rho_fl + i + NG), ufl = __ldg(Dv.u_fl + i + NG);
+      if (ROB && Dv.drift) {   // C-19
+        frf = Pn[0] < rfl;
+        fuf = Pn[1] < ufl;
+        if (frf | fuf) floors_drift(G, Bn, Dv.gam, frf ? rfl : Pn[0], fuf ? ufl : Pn[1], Pn);
+        ceiling_only(G, Dv.gamma_max, Pn, fgc);
+      } else {
+        floors_ceiling(G, rfl, ufl, Dv.gamma_max, Pn, frf, fuf, fgc);
+      }
       nrf += frf; nuf += fuf; ngc += fgc;
 #pragma unroll
       for (int c = 0; c < 5; c++) {
@@ -391,6 +420,10 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
   const int s_f = __reduce_add_sync(0xffffffffu, nfail), s_r = __reduce_add_sync(0xffffffffu, nrf),
             s_u = __reduce_add_sync(0xffffffffu, nuf), s_g = __reduce_add_sync(0xffffffffu, ngc),
             s_b = __reduce_add_sync(0xffffffffu, bad);
+  if (ROB) {
+    const int s_e = __reduce_add_sync(0xffffffffu, nent);
+    if (lane == 0 && s_e) atomicAdd(Dv.cnt + N_ENTROPY, (unsigned long long)s_e);
+  }
   if (lane == 0) {
     if (s_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)s_f);
     if (s_r) atomicAdd(Dv.cnt + N_RHOFL, (unsigned long long)s_r);
@@ -400,7 +433,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
   }
 }
 
-template <bool SAME, int NT>
+template <bool SAME, int NT, bool ROB = false>
 static void launch_tile_t(hamr_grid* g, const Dev& Dv, const Roles& r, double dtfac) {
   using namespace tile;
   const Lay& L = Dv.L;
@@ -414,9 +447,9 @@ static void launch_tile_t(hamr_grid* g, const Dev& Dv, const Roles& r, double dt
   if (cached_smem != smem || cached_dev != dev) {
     int optin = 0;
     cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    cudaFuncSetAttribute(k_update_tile<SAME, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_update_tile<SAME, NT, ROB>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
     int v = 1;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_update_tile<SAME, NT>, NT, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_update_tile<SAME, NT, ROB>, NT, smem);
     per_sm = v < 1 ? 1 : v;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cached_smem = smem;
@@ -436,13 +469,13 @@ static void launch_tile_t(hamr_grid* g, const Dev& Dv, const Roles& r, double dt
     if (eff > best) { best = eff; best_seg = sg; }
   }
   dim3 grid(ntile, (np + best_seg - 1) / best_seg);
-  k_update_tile<SAME, NT><<<grid, NT, smem, g->stream>>>(Dv, r, dtfac, best_seg);
+  k_update_tile<SAME, NT, ROB><<<grid, NT, smem, g->stream>>>(Dv, r, dtfac, best_seg);
 }
 
 // the tiled kernel serves monolithic grids without derefinement whose staged planes fit shared memory
 static int tile_threads(const Dev& Dv) {
   using namespace tile;
-  if (Dv.B.nblk > 0 || Dv.mrow || Dv.entropy || Dv.drift) return 0;   // NEXT-2 runs on the generic kernel
+  if (Dv.B.nblk > 0 || Dv.mrow) return 0;
   const int nt = 32 * ((Dv.L.n[2] + 31) / 32) * TJ;
   const size_t smem = (size_t)(2 * NA + NB) * (TJ + 1) * Dv.L.p3 * sizeof(double) + 16;
   if (nt > 512 || smem > 227 * 1024) return 0;
@@ -457,17 +490,25 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
   const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * L.n[2] * (blk ? Dv.B.nact : 1);
   const unsigned nb = (unsigned)((tot + 127) / 128);
   Launch l_(g, same ? K_UPDATE_P : K_UPDATE_C);
+  const bool rob = Dv.entropy || Dv.drift;   // NEXT-2 (monolithic grids only: checked at creation)
+  if (rob) {
+    switch (tile_threads(Dv)) {
+      case 64: return same ? launch_tile_t<true, 64, true>(g, Dv, ra, dtfac) : launch_tile_t<false, 64, true>(g, Dv, ra, dtfac);
+      case 128: return same ? launch_tile_t<true, 128, true>(g, Dv, ra, dtfac) : launch_tile_t<false, 128, true>(g, Dv, ra, dtfac);
+      case 256: return same ? launch_tile_t<true, 256, true>(g, Dv, ra, dtfac) : launch_tile_t<false, 256, true>(g, Dv, ra, dtfac);
+      case 512: return same ? launch_tile_t<true, 512, true>(g, Dv, ra, dtfac) : launch_tile_t<false, 512, true>(g, Dv, ra, dtfac);
+      default: break;
+    }
+    if (same) k_update<true, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+    else k_update<false, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+    return;
+  }
   switch (tile_threads(Dv)) {
     case 64: return same ? launch_tile_t<true, 64>(g, Dv, ra, dtfac) : launch_tile_t<false, 64>(g, Dv, ra, dtfac);
     case 128: return same ? launch_tile_t<true, 128>(g, Dv, ra, dtfac) : launch_tile_t<false, 128>(g, Dv, ra, dtfac);
     case 256: return same ? launch_tile_t<true, 256>(g, Dv, ra, dtfac) : launch_tile_t<false, 256>(g, Dv, ra, dtfac);
     case 512: return same ? launch_tile_t<true, 512>(g, Dv, ra, dtfac) : launch_tile_t<false, 512>(g, Dv, ra, dtfac);
     default: break;
-  }
-  if (Dv.entropy || Dv.drift) {   // monolithic grids only (checked at creation)
-    if (same) k_update<true, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
-    else k_update<false, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
-    return;
   }
   if (same && !blk) k_update<true, false><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
   else if (same) k_update<true, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);

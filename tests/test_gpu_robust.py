@@ -238,9 +238,9 @@ def test_torus_with_entropy_backup_and_drift_floors(H, orc):
     assert g.divb() <= 1e-12
 
 
-def test_entropy_row_is_passive_and_generic_kernels_agree_with_staged_ones(H):
-    """with no zone in need of the backup the option changes nothing but the kernels that run (the generic ones carry
-    the ninth row): same primitives as the TMA-staged kernels of the default grid to rounding"""
+def test_entropy_row_is_passive(H):
+    """with no zone in need of the backup the option changes nothing but the kernels that run (their variants that carry
+    the ninth row): same primitives as the default grid's to rounding"""
     p = I.minkowski_params(n=(32, 16, 32))
     hyd, bf = I.minkowski_waves(p, seed=2, amp=1e-2)[:2]
     out = []
