@@ -170,10 +170,13 @@ def _u_error(ref, got):
     return float((np.abs(got[1] - ref[1]) / np.maximum(ref[1], _e_scale(ref))).max())
 
 
-@pytest.mark.parametrize("drift", [0, 1])
-def test_funnel_parity_with_entropy_backup(H, orc, drift):
-    n = (24, 20, 32)
-    p = I.minkowski_params(n=n, cour=0.5, rho_fl_coef=1e-9, u_fl_coef=1e-13, entropy_backup=1, drift_floors=drift)
+@pytest.mark.parametrize("drift,n,recon", [(0, (24, 20, 32), I.RECON_PPM), (1, (24, 20, 32), I.RECON_PPM),
+                                           (1, (24, 20, 30), I.RECON_PPM), (0, (20, 24, 30), I.RECON_PLM)])
+def test_funnel_parity_with_entropy_backup(H, orc, drift, n, recon):
+    # n3 = 32: the staged kernels (ring sweeps, warp-per-row x3 sweep, tiled update) with the ninth row; n3 = 30: the
+    # generic ones, with PPM and with PLM
+    p = I.minkowski_params(n=n, recon=recon, cour=0.5, rho_fl_coef=1e-9, u_fl_coef=1e-13, entropy_backup=1,
+                           drift_floors=drift)
     hyd, bf = _funnel(p)
     g, o = _pair(H, orc, p, hyd, bf)
     assert abs(g.dt - o.dt) <= 1e-13 * o.dt
@@ -198,7 +201,7 @@ def test_funnel_parity_with_entropy_backup(H, orc, drift):
         # zones whose state came from the entropy row in the last stage: u sits on the advected adiabat
         resc_o = np.abs((gam - 1.0) * Po[1] / Po[0] ** gam - ko) <= 1e-9 * np.abs(ko)
         resc_g = np.abs((gam - 1.0) * Pg[1] / Pg[0] ** gam - kg) <= 1e-9 * np.abs(kg)
-        assert np.array_equal(resc_o, resc_g) and resc_o.sum() > nz // 10, (step, resc_o.sum(), resc_g.sum())
+        assert np.array_equal(resc_o, resc_g) and resc_o.sum() > nz // 20, (step, resc_o.sum(), resc_g.sum())
         e = parity_errors(p, Po, Pg)
         e["u"] = _u_error(Po, Pg)
         print(f"funnel drift={drift} step {step}: {e} kappa {ek:.2e} rescued {resc_o.sum()} of {nz}")
@@ -208,7 +211,7 @@ def test_funnel_parity_with_entropy_backup(H, orc, drift):
         assert sg[0] == 0
         tot_g += bg
         tot_o += bo
-    assert tot_o > nz                      # more than one rescue per zone over the three steps
+    assert tot_o > nz // 2                 # PPM: more than one rescue per zone over the three steps, PLM: 0.9
     assert g.divb() <= 1e-12
     for a, b in zip(o.get_bface(), g.get_bface()):
         assert rel_max(a, b) <= 1e-7
