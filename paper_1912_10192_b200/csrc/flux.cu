@@ -34,9 +34,19 @@ __device__ __forceinline__ double lim_slope(double dl, double dr, double dc) {
   return same_sign(dl, dr) ? copysign(lim, dl) : 0.0;   // sign(dc) = sign(dl) where the slope survives
 }
 
-// interface value a_{j+1/2} from a_j, d = a_{j+1} - a_j and the limited slopes of zones j and j+1
-__device__ __forceinline__ double ppm_iface(double aj, double d, double dm_j, double dm_jp) {
-  return aj + 0.5 * d - (dm_jp - dm_j) * SIXTH;
+// TWICE that slope from dl, dr and ds = a_{j+1} - a_{j-1} = 2 dc: sign min(|ds|, 4 |dl|, 4 |dr|).  Scaling by powers of
+// two is exact, so 2 lim_slope(dl, dr, ds / 2) == lim_slope2(dl, dr, ds) bit for bit; PPM only ever needs differences of
+// slopes times a constant (ppm_iface2), which saves the halving of every centred difference on the FP64 pipe.
+__device__ __forceinline__ double lim_slope2(double dl, double dr, double ds) {
+  const double m = 4.0 * (fabs(dl) < fabs(dr) ? dl : dr);
+  const double lim = fabs(ds) < fabs(m) ? ds : m;
+  return same_sign(dl, dr) ? copysign(lim, dl) : 0.0;
+}
+
+// interface value a_{j+1/2} from a_j, d = a_{j+1} - a_j and TWICE the limited slopes of zones j and j+1
+constexpr double TWELFTH = 1.0 / 12.0;   // exactly SIXTH / 2
+__device__ __forceinline__ double ppm_iface2(double aj, double d, double dm2_j, double dm2_jp) {
+  return aj + 0.5 * d - (dm2_jp - dm2_j) * TWELFTH;
 }
 
 // monotonised parabola edges of a zone with mean a and interface values l (low side), r (high side)
@@ -48,8 +58,10 @@ __device__ __forceinline__ double ppm_iface(double aj, double d, double dm_j, do
 __device__ __forceinline__ void ppm_mono(double l, double a, double r, double& aL, double& aR) {
   const double dl = a - l, dr = r - a;
   const bool flat = !same_sign(dl, dr);
-  const double adl = fabs(dl), adr = fabs(dr);
-  const bool over = adl > 2.0 * adr, under = adr > 2.0 * adl;
+  // |dl| > 2 |dr| and |dr| > 2 |dl| as the sign of ONE fused multiply-add each (the difference of two doubles is never
+  // rounded to zero, so the sign is exact), read off the high word: one FP64 instruction per test instead of two
+  const bool over = __double2hiint(fma(-2.0, fabs(dr), fabs(dl))) > 0;
+  const bool under = __double2hiint(fma(-2.0, fabs(dl), fabs(dr))) > 0;
   aL = flat ? a : (over ? a - 2.0 * dr : l);
   aR = flat ? a : ((!over && under) ? a + 2.0 * dl : r);
 }
@@ -58,10 +70,10 @@ __device__ __forceinline__ void ppm_mono(double l, double a, double r, double& a
 __device__ __forceinline__ void ppm_edges(double a0, double a1, double a2, double a3, double a4, double& aL,
                                           double& aR) {
   const double d10 = a1 - a0, d21 = a2 - a1, d32 = a3 - a2, d43 = a4 - a3;
-  const double dm_m = lim_slope(d10, d21, 0.5 * (a2 - a0));
-  const double dm_0 = lim_slope(d21, d32, 0.5 * (a3 - a1));
-  const double dm_p = lim_slope(d32, d43, 0.5 * (a4 - a2));
-  ppm_mono(ppm_iface(a1, d21, dm_m, dm_0), a2, ppm_iface(a2, d32, dm_0, dm_p), aL, aR);
+  const double dm_m = lim_slope2(d10, d21, a2 - a0);
+  const double dm_0 = lim_slope2(d21, d32, a3 - a1);
+  const double dm_p = lim_slope2(d32, d43, a4 - a2);
+  ppm_mono(ppm_iface2(a1, d21, dm_m, dm_0), a2, ppm_iface2(a2, d32, dm_0, dm_p), aL, aR);
 }
 
 // PLM with the MC limiter: minmod(2(a1-a0), (a2-a0)/2, 2(a2-a1))
@@ -304,12 +316,12 @@ __global__ void __launch_bounds__(MARCH_T, ENT ? 3 : MARCH_MINB) k_flux_march(De
       if (RECON == HAMR_RECON_PPM) {
         const double m2 = a[-2 * sd], m1 = a[-sd], c0 = a[0], p1 = a[sd], p2 = a[2 * sd];
         const double d10 = m1 - m2, d21 = c0 - m1, d32 = p1 - c0, d43 = p2 - p1;
-        const double dm_m = lim_slope(d10, d21, 0.5 * (c0 - m2));
-        const double dm_0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
-        const double dm_p = lim_slope(d32, d43, 0.5 * (p2 - c0));
-        const double r = ppm_iface(c0, d32, dm_0, dm_p);
+        const double dm_m = lim_slope2(d10, d21, c0 - m2);
+        const double dm_0 = lim_slope2(d21, d32, p1 - m1);
+        const double dm_p = lim_slope2(d32, d43, p2 - c0);
+        const double r = ppm_iface2(c0, d32, dm_0, dm_p);
         double aL;
-        ppm_mono(ppm_iface(m1, d21, dm_m, dm_0), c0, r, aL, PL[slot[v]]);
+        ppm_mono(ppm_iface2(m1, d21, dm_m, dm_0), c0, r, aL, PL[slot[v]]);
         dm[v] = dm_p; il[v] = r;
       } else {
         double aL;
@@ -326,8 +338,8 @@ __global__ void __launch_bounds__(MARCH_T, ENT ? 3 : MARCH_MINB) k_flux_march(De
           const double a2 = a[2 * sd];
           const double c0 = a[0], c1 = a[sd];
           const double d21 = c1 - c0, d32 = a2 - c1;
-          const double dmp = lim_slope(d21, d32, 0.5 * (a2 - c0));
-          const double r = ppm_iface(c0, d21, dm[v], dmp);
+          const double dmp = lim_slope2(d21, d32, a2 - c0);
+          const double r = ppm_iface2(c0, d21, dm[v], dmp);
           ppm_mono(il[v], c0, r, PR[slot[v]], carry[v]);
           dm[v] = dmp; il[v] = r;
         } else {
@@ -457,12 +469,12 @@ __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, 
       const double m2 = a[0 * SLOTD + voff[v]], m1 = a[1 * SLOTD + voff[v]], c0 = a[2 * SLOTD + voff[v]],
                    p1 = a[3 * SLOTD + voff[v]], p2 = a[4 * SLOTD + voff[v]];
       const double d10 = m1 - m2, d21 = c0 - m1, d32 = p1 - c0, d43 = p2 - p1;
-      const double dm_m = lim_slope(d10, d21, 0.5 * (c0 - m2));
-      const double dm_0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
-      const double dm_p = lim_slope(d32, d43, 0.5 * (p2 - c0));
-      const double r = ppm_iface(c0, d32, dm_0, dm_p);
+      const double dm_m = lim_slope2(d10, d21, c0 - m2);
+      const double dm_0 = lim_slope2(d21, d32, p1 - m1);
+      const double dm_p = lim_slope2(d32, d43, p2 - c0);
+      const double r = ppm_iface2(c0, d32, dm_0, dm_p);
       double aL;
-      ppm_mono(ppm_iface(m1, d21, dm_m, dm_0), c0, r, aL, PL[slot[v]]);
+      ppm_mono(ppm_iface2(m1, d21, dm_m, dm_0), c0, r, aL, PL[slot[v]]);
       dm[v] = dm_p; il[v] = r;
     }
   }
@@ -489,8 +501,8 @@ __global__ void __launch_bounds__(KT, RING_WARPS * 32 / KT) k_flux_ring(Dev Dv, 
     for (int v = 0; v < NVR; v++) {
       const double c0 = r0[voff[v]], c1 = r1[voff[v]], a2 = r2[voff[v]];
       const double d21 = c1 - c0, d32 = a2 - c1;
-      const double dmp = lim_slope(d21, d32, 0.5 * (a2 - c0));
-      const double r = ppm_iface(c0, d21, dm[v], dmp);
+      const double dmp = lim_slope2(d21, d32, a2 - c0);
+      const double r = ppm_iface2(c0, d21, dm[v], dmp);
       ppm_mono(il[v], c0, r, PR[slot[v]], carry[v]);
       dm[v] = dmp; il[v] = r;
     }
@@ -572,9 +584,9 @@ __global__ void __launch_bounds__(128, ENT ? 4 : X3_MINB) k_flux_x3(Dev Dv, Fiel
     if (RECON == HAMR_RECON_PPM) {
       const double m1 = a[om], c0 = a[o0], p1 = a[op];
       const double d21 = c0 - m1, d32 = p1 - c0;
-      const double dm0 = lim_slope(d21, d32, 0.5 * (p1 - m1));
+      const double dm0 = lim_slope2(d21, d32, p1 - m1);
       const double dmp = __shfl_down_sync(FULL, dm0, 1);         // slope of zone k+1
-      const double r = ppm_iface(c0, d32, dm0, dmp);             // a_{k+1/2}
+      const double r = ppm_iface2(c0, d32, dm0, dmp);             // a_{k+1/2}
       const double l = __shfl_up_sync(FULL, r, 1);               // a_{k-1/2}, built by lane-1 from the same expression
       ppm_mono(l, c0, r, PR[slot[v]], aR);
     } else {
@@ -654,10 +666,10 @@ __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields 
       a[M + 1] = __shfl_sync(FULL, a[1], dn);
       double dm[M + 1], r[M];
 #pragma unroll
-      for (int q = 0; q < M; q++) dm[q] = lim_slope(a[q + 1] - a[q], a[q + 2] - a[q + 1], 0.5 * (a[q + 2] - a[q]));
+      for (int q = 0; q < M; q++) dm[q] = lim_slope2(a[q + 1] - a[q], a[q + 2] - a[q + 1], a[q + 2] - a[q]);
       dm[M] = __shfl_sync(FULL, dm[0], dn);
 #pragma unroll
-      for (int q = 0; q < M; q++) r[q] = ppm_iface(a[q + 1], a[q + 2] - a[q + 1], dm[q], dm[q + 1]);
+      for (int q = 0; q < M; q++) r[q] = ppm_iface2(a[q + 1], a[q + 2] - a[q + 1], dm[q], dm[q + 1]);
       double l = __shfl_sync(FULL, r[M - 1], up), aRlast = 0.0;
 #pragma unroll
       for (int q = 0; q < M; q++) {
