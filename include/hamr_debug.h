@@ -83,8 +83,8 @@ int hamr_debug_floors_drift(hamr_grid* g, int n, const int* ti, const int* tj, d
  * mix 1: the flux kernels' blend, one third DFMA and two thirds DADD / DMUL (the pipe issues all three at the same
  * rate, so the instruction rate is the same and the FLOP rate is 4/3 x instructions / time);
  * mix 2: the flux kernels' whole instruction blend: per three FP64 arithmetic instructions one double compare-and-select
- * (DSETP + 2 FSEL) and two integer instructions, i.e. 4 FP64-pipe instructions to 4 others (k_flux_ring: 376 to 400
- * per face); thread_instructions then counts the FP64-pipe instructions (arithmetic + compares).  What this rate
+ * (DSETP + 2 FSEL) and two integer instructions (three in SASS), i.e. 4 FP64-pipe instructions to 5 others
+ * (k_flux_ring: about 380 to 430 per face); thread_instructions then counts the FP64-pipe instructions (arithmetic + compares).  What this rate
  * falls short of mix 1's is what the other instructions cost the FP64 pipe in issue slots. */
 int hamr_bench_fp64(void* cuda_stream, int mix, int iters, double* seconds, double* thread_instructions);
 

@@ -60,7 +60,8 @@ __global__ void k_zone_physics(Dev Dv, int what, int n, const int* __restrict__ 
 // 8 independent chains per thread; mix 0: DFMA only; mix 1: DFMA, DADD, DMUL in turn; mix 2: the flux kernels' whole
 // instruction blend: per chain and round the three FP64 arithmetic instructions, one double compare-and-select (DSETP
 // + 2 FSEL: how min / max / limiter switches compile, there is no FP64 min / max instruction) and two 32-bit integer
-// instructions on a chain of their own: 4 FP64-pipe : 4 other, against 376 : 400 per face in k_flux_ring
+// instructions on a chain of their own (three in SASS): 4 FP64-pipe : 5 other, against about 380 : 430 per face in
+// k_flux_ring
 template <int MIX>
 __global__ void __launch_bounds__(256) k_fp64_chains(int iters, double seed, double* sink) {
   double a[8];
