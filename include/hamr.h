@@ -147,6 +147,30 @@ const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the 
  * Both options need a grid of one block (nb = 0, no LAT, no derefinement, no refinement), else HAMR_EINVAL.  The
  * staged kernels carry the ninth row where they serve the grid (cfg 2 with both options: 80 % of its plain rate). */
 
+/* ---- one entry point that allocates nothing -------------------------------------------------------------------- */
+/* For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): the div B diagnostic of hamr_divb ("divergence-free evolution of the magnetic field"; C-11)
+ * on caller-owned DENSE device arrays, without a grid object.  The scratch memory of its two-pass reduction is a
+ * file-scope device array of fixed size inside the library (1 MB, held by every GPU that loads the library until the
+ * process exits); the call itself makes no cudaMalloc / cudaFree and calls no allocating library routine.
+ *   n[3]: zones; dx[3]: zone widths (both host); bface_dev[d]: DEVICE pointer to sqrt(-g) B^d on d-faces, extent
+ *   n[d] + 1 along d, x3 fastest (the layout hamr_set_prims takes); out_dev: DEVICE pointer to one double that
+ *   receives max over zones of |div| / sum_d (|Bf+| + |Bf-|) / (2 dx^d), zones whose denominator is below 1e-12 of its
+ *   maximum counting 0 (hamr_divb's definition); cuda_stream: a cudaStream_t cast to void* (NULL: the default stream).
+ * Four kernels are enqueued on the stream and the call returns without synchronising; the caller owns every array.
+ * Limit: n[0] n[1] n[2] <= HAMR_NOALLOC_MAX_ZONES, else HAMR_EINVAL and nothing is launched (hamr_noalloc_last_error
+ * says so); larger fields go through hamr_divb on a grid.  Every call on a device shares the one scratch array, which
+ * keeps the last call's contents (each call writes every slot before it reads it, so nothing needs clearing): calls
+ * that overlap on the GPU (streams without ordering between them, several host threads) race: serialise them.
+ * hamr_noalloc_setup resolves the scratch array's device address for the CURRENT device (once per device; no
+ * allocation); hamr_divb_noalloc does the same on first use, so calling it beforehand matters only where even that
+ * first look-up must happen outside a captured or timed region. */
+#define HAMR_NOALLOC_MAX_ZONES 16777216
+int hamr_noalloc_setup(void);
+int hamr_divb_noalloc(const int n[3], const double dx[3], const double* const bface_dev[3], double* out_dev,
+                      void* cuda_stream);
+const char* hamr_noalloc_last_error(void); /* never NULL; per host thread; "" after a successful call */
+
 /* ---- block-structured grid (BASELINE.json cfg 4) ------------------ */
 /* A grid with nb != {0,0,0} or lat_max_level > 0 is cut into blocks of nb zones (nb[d] = 0: the whole
  * extent; nb[d] must divide n[d] and be >= 3).  Blocks exchange ghost zones directly;

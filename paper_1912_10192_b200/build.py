@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libhamr.so")
-SOURCES = ["geom.cu", "bc.cu", "flux.cu", "ct.cu", "update.cu", "misc.cu", "blocks.cu", "deref.cu", "api.cu", "debug.cu"]
+SOURCES = ["geom.cu", "bc.cu", "flux.cu", "ct.cu", "update.cu", "misc.cu", "blocks.cu", "deref.cu", "api.cu", "debug.cu", "noalloc.cu"]
 HEADERS = ["hamr_dev.cuh", "hamr_host.h", os.path.join("..", "..", "include", "hamr.h"),
            os.path.join("..", "..", "include", "hamr_debug.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

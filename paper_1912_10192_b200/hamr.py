@@ -30,7 +30,9 @@ SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "h
            "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
            "hamr_get_backup_count", "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
            "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
-           "hamr_get_block_bface", "hamr_set_all_blocks", "hamr_get_all_blocks"]
+           "hamr_get_block_bface", "hamr_set_all_blocks", "hamr_get_all_blocks",
+           "hamr_noalloc_setup", "hamr_divb_noalloc", "hamr_noalloc_last_error"]
+NOALLOC_MAX_ZONES = 16777216
 # ... and include/hamr_debug.h (test hooks and diagnostics)
 DEBUG_SYMBOLS = ["hamr_set_levels", "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
                  "hamr_profile_begin", "hamr_profile_end", "hamr_profile_class_name", "hamr_launch_count",
@@ -116,8 +118,12 @@ def lib():
                                                   c_double_p, ip]
         L.hamr_debug_floors_drift.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p, ip]
         L.hamr_bench_fp64.argtypes = [vp, C.c_int, C.c_int, c_double_p, c_double_p]
+        L.hamr_noalloc_setup.argtypes = []
+        L.hamr_divb_noalloc.argtypes = [C.POINTER(C.c_int), c_double_p, C.POINTER(vp), vp, vp]
+        L.hamr_noalloc_last_error.argtypes = []
+        L.hamr_noalloc_last_error.restype = C.c_char_p
         for s in SYMBOLS + DEBUG_SYMBOLS:
-            if s not in ("hamr_last_error", "hamr_profile_class_name"):
+            if s not in ("hamr_last_error", "hamr_profile_class_name", "hamr_noalloc_last_error"):
                 getattr(L, s).restype = C.c_int
         _LIB = L
     return _LIB
@@ -450,6 +456,18 @@ class Grid:
         n = C.c_longlong(0)
         self._ck(self.L.hamr_launch_count(self.h, C.byref(n)))
         return n.value
+
+
+def divb_noalloc(n, dx, bface_dev_ptrs, out_dev_ptr, stream=None):
+    """hamr_divb_noalloc: n (3 ints), dx (3 floats), bface_dev_ptrs (3 device addresses as ints), out_dev_ptr (device
+    address of one double), stream (cudaStream_t as int or None).  Enqueues and returns; raises on a non-zero status."""
+    L = lib()
+    nn = (C.c_int * 3)(*[int(v) for v in n])
+    dd = (C.c_double * 3)(*[float(v) for v in dx])
+    bp = (C.c_void_p * 3)(*[C.c_void_p(int(a)) for a in bface_dev_ptrs])
+    rc = L.hamr_divb_noalloc(nn, dd, bp, C.c_void_p(int(out_dev_ptr)), C.c_void_p(stream))
+    if rc != OK:
+        raise HamrError(rc, L.hamr_noalloc_last_error().decode())
 
 
 def bench_fp64(mix=0, iters=20000, stream=None):
