@@ -157,6 +157,33 @@ void* orc_grid_create(const Params* p) {
 
 void orc_grid_destroy(void* h) { delete (Grid*)h; }
 
+// C-20: the refinement criterion (max density per block column >= rho_cut) as the r_refine_max it asks for
+int orc_refine_radius(void* h, double rho_cut, double* r_new) {
+  Grid& g = *(Grid*)h;
+  if (!g.multi || !g.have_state || !r_new) return 1;
+  *r_new = blocks_refine_radius(g, rho_cut);
+  return 0;
+}
+// C-20: a new grid with r_refine_max = r_new holding the state of h (which stays valid); NULL if the grid is not a
+// block grid between coarse steps, is phi-derefined, or the new lattice is not admissible
+void* orc_regrid(void* h, double r_new) {
+  Grid& go = *(Grid*)h;
+  if (!go.multi || !go.have_state || go.par.n_deref > 0) return nullptr;
+  Params p = go.par;
+  p.r_refine_max = r_new;
+  Grid* gn = nullptr;
+  try {
+    gn = grid_new(p);
+    if (!gn) return nullptr;
+    if (!gn->multi) { delete gn; return nullptr; }
+    blocks_regrid(go, *gn);
+  } catch (const std::exception&) {
+    delete gn;
+    return nullptr;
+  }
+  return gn;
+}
+
 // hydro[c]: N1*N2*N3 active zones, x3 fastest.  bface[d]: d-faces, extent n[d]+1 along d; NULL -> 0.
 int orc_set_prims(void* h, const double* const hydro[5], const double* const bface[3]) {
   Grid& g = *(Grid*)h;
@@ -220,6 +247,7 @@ int orc_step(void* h, int nsteps, double* t_out, double* dt_last) {
 }
 
 double orc_get_dt(void* h) { return ((Grid*)h)->dt; }
+double orc_get_t(void* h) { return ((Grid*)h)->t; }
 void orc_set_dt(void* h, double dt) { ((Grid*)h)->dt = dt; }
 
 int orc_get_prims(void* h, double* const prims[8]) {

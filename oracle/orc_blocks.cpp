@@ -675,4 +675,125 @@ void blocks_coarse_step(Grid& g) {
   assign_levels(g);
 }
 
+// ---- C-20 (the x1-only part): regridding ---------------------------------------------------------
+// PAPER.md:73 "H-AMR allows the user to implement an arbitrary refinement criterion ... a cutoff on the maximum density in
+// each block"; PAPER.md:71 blocks are split per dimension; "(de-)refinement ... including the divergence-free
+// prolongation and restriction of magnetic fields (Balsara 2001)".  This grid has ONE refinement level along x1 whose
+// block columns must be contiguous from the inner edge (C-16), so a regrid moves the outer edge of the refined region.
+//
+// Criterion: a block column wants refinement if any of its blocks holds a zone with rho >= rho_cut; the refined region
+// is every column up to the outermost such column (the nesting rule of PAPER.md:73 with one level: no resolution jump
+// greater than two exists).  Returned as the r_refine_max that selects exactly those columns; 0: none.
+double blocks_refine_radius(const Grid& g, double rho_cut) {
+  const Params& par = g.par;
+  const int nb0 = par.nb[0] > 0 ? par.nb[0] : par.n[0];
+  const int ncol = par.n[0] / nb0;
+  int cmax = -1;
+  for (const Block& b : g.blocks) {
+    const int col = b.lev1 ? (int)(b.I0[0] / nb0) / 2 : (int)(b.I0[0] / nb0);
+    double m = 0.0;
+    for (int i = 0; i < b.n[0]; i++)
+      for (int j = 0; j < b.n[1]; j++)
+        for (int k = 0; k < b.n[2]; k++) m = std::max(m, b.sn.P[0][b.idx(i, j, k)]);
+    if (m >= rho_cut) cmax = std::max(cmax, col);
+  }
+  if (cmax < 0) return 0.0;
+  double lo = par.xmin[0], hi = par.xmax[0];
+  if (par.metric == 1) { lo = std::log(lo); hi = std::log(hi); }
+  const double edge = lo + (hi - lo) * (double)(cmax + 1) / (double)ncol;   // high edge of column cmax
+  return par.metric == 1 ? std::exp(edge) : edge;
+}
+
+// Transfer of the state of `go` (all blocks at the same time: between coarse steps) onto the lattice of `gn`, which
+// differs in r_refine_max only.  Per new block: same level as before -> copy; newly refined -> prolongation of the old
+// coarse block; newly coarsened -> restriction of the two old fine blocks.
+//   prolongation: hydro primitives piecewise linear in x1 with the MC-limited slope of the coarse values, evaluated a
+//     quarter of a coarse zone off the coarse centre (the operator of the ghost fill, C-16); x1-faces: coincident ones
+//     copied, the new one in the middle of a coarse zone is the MEAN of that zone's two x1-faces; x2- and x3-faces: both
+//     children take the coarse zone's face value.  Each child then has the coarse zone's transverse divergence and, over
+//     half the width, half of its x1 difference: the coarse zone's divergence, i.e. zero if that was (the lowest-order
+//     member of Balsara 2001's divergence-free prolongation).
+//   restriction: hydro primitives and transverse faces are the mean of the two fine values, x1-faces the coincident
+//     fine faces: the coarse divergence is the mean of the two children's.
+void blocks_regrid(Grid& go, Grid& gn) {
+  const Params& par = go.par;
+  const int nb0 = par.nb[0] > 0 ? par.nb[0] : par.n[0];
+  const int ncol = par.n[0] / nb0;
+  const int nref_o = go.nslot[0] - ncol, nref_n = gn.nslot[0] - ncol;
+  if (nb0 % 2 != 0 && nref_o != nref_n) throw std::runtime_error("regrid needs an even nb[0]");
+  // ghosts of the old state (the slopes of the prolongation read one zone beyond the block)
+  for (Block& b : go.blocks) {
+    exchange_block(go, b, b.sn, b.tb_u);
+    exchange_refined(go, b, b.sn, b.tb_u);
+    fill_physical_bc(go.par, b, b.sn);
+  }
+  auto old_block = [&](int slot0, int bj, int bk) -> const Block& {
+    return go.blocks[go.lattice[((size_t)slot0 * go.nslot[1] + bj) * go.nslot[2] + bk]];
+  };
+  for (Block& b : gn.blocks) {
+    const int n0 = b.n[0], n1 = b.n[1], n2 = b.n[2];
+    const int col = b.lev1 ? (int)(b.I0[0] / nb0) / 2 : (int)(b.I0[0] / nb0);
+    const int child = b.lev1 ? (int)(b.I0[0] / nb0) % 2 : 0;
+    const bool old_fine = col < nref_o;
+    Fields& d = b.sn;
+    if ((b.lev1 != 0) == old_fine) {
+      // ---- same level: copy
+      const Block& q = old_block(old_fine ? 2 * col + child : col + nref_o, b.slot[1], b.slot[2]);
+      for (int i = 0; i <= n0; i++)
+        for (int j = 0; j <= n1; j++)
+          for (int k = 0; k <= n2; k++) {
+            const size_t z = b.idx(i, j, k);
+            if (i < n0 && j < n1 && k < n2)
+              for (int c = 0; c < 5; c++) d.P[c][z] = q.sn.P[c][z];
+            if (j < n1 && k < n2) d.Bf[0][z] = q.sn.Bf[0][z];
+            if (i < n0 && k < n2) d.Bf[1][z] = q.sn.Bf[1][z];
+            if (i < n0 && j < n1) d.Bf[2][z] = q.sn.Bf[2][z];
+          }
+    } else if (b.lev1) {
+      // ---- newly refined: prolongation of the old coarse block; this child covers its zones [h n0/2, (h+1) n0/2)
+      const Block& q = old_block(col + nref_o, b.slot[1], b.slot[2]);
+      const int c0 = child * (n0 / 2);
+      for (int i = 0; i <= n0; i++)
+        for (int j = 0; j <= n1; j++)
+          for (int k = 0; k <= n2; k++) {
+            const size_t z = b.idx(i, j, k);
+            const int ic = c0 + i / 2;
+            if (i < n0 && j < n1 && k < n2)
+              for (int c = 0; c < 5; c++) {
+                const double a3[3] = {q.sn.P[c][q.idx(ic - 1, j, k)], q.sn.P[c][q.idx(ic, j, k)], q.sn.P[c][q.idx(ic + 1, j, k)]};
+                double aL, aR;
+                plm_zone(a3, aL, aR);
+                d.P[c][z] = 0.5 * (a3[1] + ((i & 1) ? aR : aL));
+              }
+            if (j < n1 && k < n2) {
+              const int f2 = 2 * c0 + i;                 // the face's position in half coarse zones
+              d.Bf[0][z] = (f2 % 2 == 0) ? q.sn.Bf[0][q.idx(f2 / 2, j, k)]
+                                         : 0.5 * (q.sn.Bf[0][q.idx(f2 / 2, j, k)] + q.sn.Bf[0][q.idx(f2 / 2 + 1, j, k)]);
+            }
+            if (i < n0 && k < n2) d.Bf[1][z] = q.sn.Bf[1][q.idx(ic, j, k)];
+            if (i < n0 && j < n1) d.Bf[2][z] = q.sn.Bf[2][q.idx(ic, j, k)];
+          }
+    } else {
+      // ---- newly coarsened: restriction of the two old fine blocks
+      for (int i = 0; i <= n0; i++) {
+        const int hh = (i == n0) ? 1 : ((i < n0 / 2) ? 0 : 1);   // the child holding coarse zone i (coarse face n0: the second)
+        const Block& q = old_block(2 * col + hh, b.slot[1], b.slot[2]);
+        const int i0 = 2 * i - hh * n0;                   // first of the two fine zones / the coincident fine face
+        for (int j = 0; j <= n1; j++)
+          for (int k = 0; k <= n2; k++) {
+            const size_t z = b.idx(i, j, k);
+            if (i < n0 && j < n1 && k < n2)
+              for (int c = 0; c < 5; c++) d.P[c][z] = 0.5 * (q.sn.P[c][q.idx(i0, j, k)] + q.sn.P[c][q.idx(i0 + 1, j, k)]);
+            if (j < n1 && k < n2) d.Bf[0][z] = q.sn.Bf[0][q.idx(i0, j, k)];
+            if (i < n0 && k < n2) d.Bf[1][z] = 0.5 * (q.sn.Bf[1][q.idx(i0, j, k)] + q.sn.Bf[1][q.idx(i0 + 1, j, k)]);
+            if (i < n0 && j < n1) d.Bf[2][z] = 0.5 * (q.sn.Bf[2][q.idx(i0, j, k)] + q.sn.Bf[2][q.idx(i0 + 1, j, k)]);
+          }
+      }
+    }
+  }
+  gn.t = go.t;
+  gn.have_state = true;
+  blocks_initial_dt(gn);
+}
+
 }  // namespace orc

@@ -83,6 +83,8 @@ void blocks_build(Grid& g);                       // block lattice, neighbours, 
 void blocks_exchange(Grid& g, int level, int stage_half);  // ghost fill of the level's stage source
 void blocks_initial_dt(Grid& g);                  // flux pass on every block, first dt / levels
 void blocks_coarse_step(Grid& g);                 // one (coarse) step: advance(tau_max)
+double blocks_refine_radius(const Grid& g, double rho_cut);   // C-20: the refinement criterion as an r_refine_max
+void blocks_regrid(Grid& go, Grid& gn);           // C-20: state of go onto the lattice of gn (built, differing in r_refine_max)
 
 void block_init(const Params& par, Block& b);           // geometry tables, allocation
 void fill_physical_bc(const Params& par, Block& b, Fields& s);

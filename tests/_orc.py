@@ -79,6 +79,11 @@ def lib():
                                            c_double_p, c_double_p, C.POINTER(C.c_int)]
         L.orc_entropy_UF.argtypes = [c_double_p, C.POINTER(Geom), C.c_double, C.c_int, c_double_p, c_double_p]
         L.orc_get_backup_count.argtypes = [C.c_void_p, C.POINTER(C.c_longlong)]
+        L.orc_refine_radius.argtypes = [C.c_void_p, C.c_double, c_double_p]
+        L.orc_regrid.restype = C.c_void_p
+        L.orc_regrid.argtypes = [C.c_void_p, C.c_double]
+        L.orc_get_t.restype = C.c_double
+        L.orc_get_t.argtypes = [C.c_void_p]
         L.orc_get_kadv.argtypes = [C.c_void_p, c_double_p]
         L.orc_ppm_zone.argtypes = [c_double_p] * 3
         L.orc_plm_zone.argtypes = [c_double_p] * 3
@@ -122,15 +127,32 @@ def pack_params(p: dict) -> Params:
 class OrcGrid:
     """Thin wrapper: same call names as the product binding (create/set_prims/step/...)."""
 
-    def __init__(self, p: dict):
+    def __init__(self, p: dict, _handle=None):
         self.L = lib()
         self.p = p
         self.n = tuple(int(v) for v in p["n"])
         self._par = pack_params(p)
-        self.h = self.L.orc_grid_create(C.byref(self._par))
+        self.h = _handle if _handle is not None else self.L.orc_grid_create(C.byref(self._par))
         if not self.h:
             raise RuntimeError("orc_grid_create failed")
         self.h = C.c_void_p(self.h)
+
+    def refine_radius(self, rho_cut):
+        """C-20: the r_refine_max the density criterion asks for (0: no refined region)"""
+        r = np.zeros(1)
+        assert self.L.orc_refine_radius(self.h, float(rho_cut), _dp(r)) == 0
+        return float(r[0])
+
+    def regrid(self, r_refine_max):
+        """C-20: a new grid with that r_refine_max carrying this grid's state (this grid stays valid)"""
+        h = self.L.orc_regrid(self.h, float(r_refine_max))
+        if not h:
+            raise RuntimeError("orc_regrid failed")
+        return OrcGrid(dict(self.p, r_refine_max=float(r_refine_max)), _handle=h)
+
+    @property
+    def t(self):
+        return self.L.orc_get_t(self.h)
 
     def close(self):
         if self.h:
