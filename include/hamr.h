@@ -147,6 +147,26 @@ const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the 
  * Both options need a grid of one block (nb = 0, no LAT, no derefinement, no refinement), else HAMR_EINVAL.  The
  * staged kernels carry the ninth row where they serve the grid (cfg 2 with both options: 80 % of its plain rate). */
 
+/* ---- regridding of the x1 refinement level (the x1-only part; C-20) ------------------ */
+/* "H-AMR allows the user to implement an arbitrary refinement criterion.  For example ... a cutoff on the
+ * maximum density in each block"; "(de-)refinement ... including the divergence-free prolongation and
+ * restriction of magnetic fields (Balsara 2001)".  The grid carries ONE refinement level along x1 whose block columns are
+ * contiguous from the inner x1 edge (r < r_refine_max), so a regrid moves the outer edge of the refined region.
+ * hamr_refine_radius evaluates the density criterion on the current state: a block column wants refinement if one of its
+ * blocks holds a zone with rho >= rho_cut; *r_refine_max receives the radius (x1 on the Cartesian map) that refines every
+ * column up to the outermost such column, 0 if there is none.  Synchronises the stream.
+ * hamr_regrid creates a NEW grid (own device memory and stream, as hamr_grid_create) with g's parameters but for
+ * r_refine_max, transfers g's state onto it on the device and initialises it as hamr_blocks_commit does (ghosts, first
+ * step and time levels from a flux pass, C-14); the time is carried over.  g stays valid and unchanged; the caller
+ * destroys both.  Blocks that keep their level are copied bit for bit; newly refined blocks are the prolongation of their
+ * parent (hydro: piecewise linear in x1 with the MC-limited slope; x1-faces: coincident ones copied, the new one the mean
+ * of the parent zone's two; transverse faces: the parent's value), newly coarsened ones the restriction of their two
+ * children (means; coincident x1-faces copied): every new zone has the divergence of the zone(s) it came from, so
+ * div B stays at round-off.  Needs a block grid (nb) with an even nb[0], between steps, without phi-derefinement;
+ * HAMR_EINVAL otherwise (also if r_refine_max does not give an admissible lattice). */
+int hamr_refine_radius(hamr_grid* g, double rho_cut, double* r_refine_max);
+int hamr_regrid(hamr_grid* g, double r_refine_max, hamr_grid** out);
+
 /* ---- one entry point that allocates nothing -------------------------------------------------------------------- */
 /* For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
  * it): the div B diagnostic of hamr_divb ("divergence-free evolution of the magnetic field"; C-11)

@@ -753,6 +753,49 @@ int hamr_blocks_commit(hamr_grid* g) {
   return check_state(g);
 }
 
+// ---- C-20: regridding of the x1 refinement level (the x1-only part) ----------------------------------
+int hamr_refine_radius(hamr_grid* g, double rho_cut, double* r_refine_max) {
+  if (!g || !r_refine_max) return HAMR_EINVAL;
+  if (!g->bh.on) return fail(g, HAMR_EINVAL, "the refinement criterion needs a block grid (nb)");
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  const int rc = blk_refine_radius(g, rho_cut, r_refine_max);
+  return rc == HAMR_OK ? rc : fail(g, rc, "hamr_refine_radius");
+}
+
+int hamr_regrid(hamr_grid* g, double r_refine_max, hamr_grid** out) {
+  if (out) *out = nullptr;
+  if (!g || !out) return HAMR_EINVAL;
+  if (!g->bh.on) return fail(g, HAMR_EINVAL, "regridding needs a block grid (nb)");
+  if (g->par.n_deref > 0) return fail(g, HAMR_EINVAL, "regridding is not available on a phi-derefined grid");
+  if (!g->have_state || g->blocks_open) return fail(g, HAMR_ESTATE, "no committed state");
+  if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
+  hamr_params p = g->par;
+  p.r_refine_max = r_refine_max > 0.0 ? r_refine_max : 0.0;
+  hamr_grid* gn = nullptr;
+  int rc = hamr_grid_create(&p, &gn);
+  if (rc != HAMR_OK) return fail(g, rc, "regrid: the new lattice was refused (refined columns must leave a block grid)");
+  if (!gn->bh.on) { hamr_grid_destroy(gn); return fail(g, HAMR_EINVAL, "regrid: the new grid is not a block grid"); }
+  double tt[2];
+  rc = read_scal(g, S_T, 2, tt);
+  if (rc == HAMR_OK) rc = blk_regrid(g, gn);
+  if (rc != HAMR_OK) { hamr_grid_destroy(gn); return fail(g, rc, "regrid: state transfer failed"); }
+  // as hamr_blocks_commit: ghosts, B_c, one flux pass for the step and the time levels (C-14), then the clock
+  gn->isn = 0; gn->ish = 1; gn->inew = 2;
+  cudaError_t e = cudaMemsetAsync(gn->D.scal, 0, NSCAL * sizeof(double), gn->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(gn->D.cnt, 0, NCNT * sizeof(unsigned long long), gn->stream);
+  if (e == cudaSuccess) rc = blk_initial(gn);
+  gn->h_pinned[57] = tt[0];
+  if (e == cudaSuccess && rc == HAMR_OK)
+    e = cudaMemcpyAsync(gn->D.scal + S_T, gn->h_pinned + 57, sizeof(double), cudaMemcpyHostToDevice, gn->stream);
+  if (e != cudaSuccess || rc != HAMR_OK) { hamr_grid_destroy(gn); return fail(g, e != cudaSuccess ? HAMR_ECUDA : rc, "regrid: initialisation of the new grid failed"); }
+  blk_check_finite(gn);
+  gn->have_state = true;
+  rc = check_state(gn);
+  if (rc != HAMR_OK) { hamr_grid_destroy(gn); return fail(g, rc, "regrid: non-finite state after the transfer"); }
+  *out = gn;
+  return HAMR_OK;
+}
+
 static int get_block(hamr_grid* g, int b, int kind0, int nkind, double* const out[]) {
   if (!g || !g->bh.on || b < 0 || b >= g->bh.nblk || !out) return HAMR_EINVAL;
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");

@@ -1548,4 +1548,166 @@ void blk_totals(hamr_grid* g) {
 
 void blk_check_finite(hamr_grid* g) { blk_diag(g, 3); }
 
+// ---- C-20 (the x1-only part): regridding of the x1 refinement level --------------------------------
+// refinement criterion "a cutoff on the maximum density in each block"; "(de-)refinement ...
+// including the divergence-free prolongation and restriction of magnetic fields (Balsara 2001)".  The refined block
+// columns are contiguous from the inner x1 edge (C-16), so a regrid moves the outer edge of the refined region: a new
+// grid is created with another r_refine_max and the state is transferred on the device.
+
+// maximum density over the active zones of every block: one CTA per block, result to out[b]
+__global__ void __launch_bounds__(256) k_blk_max_rho(Dev Dv, Bufs B, double* __restrict__ out) {
+  const Lay& L = Dv.L;
+  const int b = blockIdx.x;
+  const double* rho = buf_arr(B, Dv.B.cur[b], 0) + (long long)b * Dv.B.blen;
+  const int tot = L.n[0] * L.n[1] * L.n[2];
+  double m = 0.0;
+  for (int t = threadIdx.x; t < tot; t += blockDim.x) {
+    const int k = t % L.n[2], j = (t / L.n[2]) % L.n[1], i = t / (L.n[2] * L.n[1]);
+    m = fmax(m, rho[L.idx(i, j, k)]);
+  }
+  __shared__ double wm[8];
+  m = warp_max(m);
+  if ((threadIdx.x & 31) == 0) wm[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; w++) m = fmax(m, wm[w]);
+    out[b] = m;
+  }
+}
+
+// State transfer between two lattices of the same blocks that differ in the refined columns.  map[bn] = {kind, q0, q1,
+// child}: kind 0 copy of old block q0; 1 prolongation of old coarse block q0, this block being its child `child`;
+// 2 restriction of the old fine blocks q0 (low half) and q1 (high half).  One thread per zone / face location
+// (i <= n0, j <= n1, k <= n2) of every new block; the old state must have its x1 ghost zones filled.
+//   prolongation: hydro piecewise linear in x1 with the MC-limited slope of the coarse values, a quarter of a coarse
+//   zone off the coarse centre (the operator of the ghost fill, C-16); x1-faces: coincident ones copied, the new face
+//   in the middle of a coarse zone the mean of that zone's two faces; transverse faces: the coarse zone's value for both
+//   children: every child keeps the coarse zone's divergence.  restriction: means of the two fine values; x1-faces the
+//   coincident fine faces.
+__global__ void __launch_bounds__(256) k_blk_regrid(Dev Do, Bufs Bo, Dev Dn, Fields sn, const int4* __restrict__ map) {
+  const Lay& L = Dn.L;
+  const int n0 = L.n[0], n1 = L.n[1], n2 = L.n[2];
+  const int c2 = n2 + 1, c1 = n1 + 1;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (unsigned)((n0 + 1) * c1 * c2)) return;
+  const int bn = blockIdx.y;
+  const int4 m = __ldg(map + bn);
+  const unsigned tj = t / (unsigned)c2;
+  const int k = (int)(t - tj * c2), i = (int)(tj / (unsigned)c1), j = (int)(tj - (unsigned)i * c1);
+  const bool zi = i < n0, zj = j < n1, zk = k < n2;
+  const long long zn = (long long)bn * Dn.B.blen + L.idx(i, j, k);
+  if (m.x == 0) {
+    const int cur = Do.B.cur[m.y];
+    const long long zo = (long long)m.y * Do.B.blen + L.idx(i, j, k);
+    if (zi && zj && zk)
+      for (int c = 0; c < 5; c++) sn.P[c][zn] = buf_arr(Bo, cur, c)[zo];
+    if (zj && zk) sn.Bf[0][zn] = buf_arr(Bo, cur, 5)[zo];
+    if (zi && zk) sn.Bf[1][zn] = buf_arr(Bo, cur, 6)[zo];
+    if (zi && zj) sn.Bf[2][zn] = buf_arr(Bo, cur, 7)[zo];
+  } else if (m.x == 1) {
+    const int cur = Do.B.cur[m.y];
+    const long long base = (long long)m.y * Do.B.blen;
+    const int c0 = m.w * (n0 / 2), ic = c0 + i / 2;
+    if (zi && zj && zk)
+      for (int c = 0; c < 5; c++) {
+        const double* a = buf_arr(Bo, cur, c) + base;
+        const double am = a[L.idx(ic - 1, j, k)], a0 = a[L.idx(ic, j, k)], ap = a[L.idx(ic + 1, j, k)];
+        const double dl = a0 - am, dr = ap - a0;
+        double sl = 0.0;
+        if (dl * dr > 0.0) {
+          sl = fmin(0.5 * fabs(ap - am), 2.0 * fmin(fabs(dl), fabs(dr)));
+          if (dl < 0.0) sl = -sl;
+        }
+        sn.P[c][zn] = 0.5 * (a0 + ((i & 1) ? a0 + 0.5 * sl : a0 - 0.5 * sl));
+      }
+    if (zj && zk) {
+      const double* a = buf_arr(Bo, cur, 5) + base;
+      const int f2 = 2 * c0 + i;
+      sn.Bf[0][zn] = (f2 & 1) ? 0.5 * (a[L.idx(f2 / 2, j, k)] + a[L.idx(f2 / 2 + 1, j, k)]) : a[L.idx(f2 / 2, j, k)];
+    }
+    if (zi && zk) sn.Bf[1][zn] = buf_arr(Bo, cur, 6)[base + L.idx(ic, j, k)];
+    if (zi && zj) sn.Bf[2][zn] = buf_arr(Bo, cur, 7)[base + L.idx(ic, j, k)];
+  } else {
+    const int hh = (i == n0) ? 1 : ((i < n0 / 2) ? 0 : 1);
+    const int q = hh ? m.z : m.y;
+    const int cur = Do.B.cur[q];
+    const long long base = (long long)q * Do.B.blen;
+    const int i0 = 2 * i - hh * n0;
+    const long long za = base + L.idx(i0, j, k), zb = base + L.idx(i0 + 1, j, k);
+    if (zi && zj && zk)
+      for (int c = 0; c < 5; c++) { const double* a = buf_arr(Bo, cur, c); sn.P[c][zn] = 0.5 * (a[za] + a[zb]); }
+    if (zj && zk) sn.Bf[0][zn] = buf_arr(Bo, cur, 5)[za];
+    if (zi && zk) { const double* a = buf_arr(Bo, cur, 6); sn.Bf[1][zn] = 0.5 * (a[za] + a[zb]); }
+    if (zi && zj) { const double* a = buf_arr(Bo, cur, 7); sn.Bf[2][zn] = 0.5 * (a[za] + a[zb]); }
+  }
+}
+
+// the refinement criterion as the r_refine_max it asks for: every block column up to the outermost one that holds a
+// zone with rho >= rho_cut (0: none).  Synchronises the stream (one read-back of a double per block).
+int blk_refine_radius(hamr_grid* g, double rho_cut, double* r_new) {
+  BlkHost& H = g->bh;
+  const hamr_params& p = g->par;
+  if (g->stage_doubles < (size_t)H.nblk) return HAMR_ENOMEM;
+  {
+    Launch l_(g, K_OTHER);
+    k_blk_max_rho<<<H.nblk, 256, 0, g->stream>>>(g->D, bufs_of(g), g->stage);
+  }
+  // h_ctop is pinned, [nblk][3] doubles, idle between steps
+  if (cudaMemcpyAsync(H.h_ctop, g->stage, (size_t)H.nblk * 8, cudaMemcpyDeviceToHost, g->stream) != cudaSuccess) return HAMR_ECUDA;
+  if (cudaStreamSynchronize(g->stream) != cudaSuccess) return HAMR_ECUDA;
+  const int nb0 = g->D.L.n[0], ncol = p.n[0] / nb0;
+  int cmax = -1;
+  for (int b = 0; b < H.nblk; b++) {
+    const int c = H.I0[(size_t)b * 3] / nb0, col = H.lev1[b] ? c / 2 : c;
+    if (H.h_ctop[b] >= rho_cut) cmax = std::max(cmax, col);
+  }
+  if (cmax < 0) { *r_new = 0.0; return HAMR_OK; }
+  const bool ks = p.metric == HAMR_METRIC_KERR_SCHILD;
+  const double lo = ks ? std::log(p.xmin[0]) : p.xmin[0], hi = ks ? std::log(p.xmax[0]) : p.xmax[0];
+  const double edge = lo + (hi - lo) * (double)(cmax + 1) / (double)ncol;
+  *r_new = ks ? std::exp(edge) : edge;
+  return HAMR_OK;
+}
+
+// state of go (between coarse steps) onto gn, created with the same parameters but for r_refine_max; gn's stream
+int blk_regrid(hamr_grid* go, hamr_grid* gn) {
+  BlkHost& Ho = go->bh;
+  BlkHost& Hn = gn->bh;
+  const Lay& L = go->D.L;
+  const int nb0 = L.n[0], ncol = go->par.n[0] / nb0;
+  const int nref_o = (Ho.nslot[0] - ncol), nref_n = (Hn.nslot[0] - ncol);
+  if (nref_o != nref_n && (nb0 & 1)) return HAMR_EINVAL;
+  // x1 ghost zones of the old state: the slopes of the prolongation read one zone beyond a block (all clocks are 0
+  // between coarse steps, so every sample is a plain copy of a time-n state)
+  blk_ghosts(go, dev_list(go, 4), 0, 0, false, false);
+  std::vector<int> map((size_t)Hn.nblk * 4);
+  auto old_id = [&](int s0, int s1, int s2) { return (s0 * Ho.nslot[1] + s1) * Ho.nslot[2] + s2; };
+  for (int s0 = 0; s0 < Hn.nslot[0]; s0++)
+    for (int s1 = 0; s1 < Hn.nslot[1]; s1++)
+      for (int s2 = 0; s2 < Hn.nslot[2]; s2++) {
+        const int bn = (s0 * Hn.nslot[1] + s1) * Hn.nslot[2] + s2;
+        const bool fine = s0 < 2 * nref_n;
+        const int col = fine ? s0 / 2 : s0 - nref_n, child = fine ? s0 & 1 : 0;
+        const bool old_fine = col < nref_o;
+        int* m = &map[(size_t)bn * 4];
+        if (fine == old_fine) { m[0] = 0; m[1] = old_id(old_fine ? 2 * col + child : col + nref_o, s1, s2); m[2] = -1; m[3] = 0; }
+        else if (fine) { m[0] = 1; m[1] = old_id(col + nref_o, s1, s2); m[2] = -1; m[3] = child; }
+        else { m[0] = 2; m[1] = old_id(2 * col, s1, s2); m[2] = old_id(2 * col + 1, s1, s2); m[3] = 0; }
+      }
+  // the map travels through the new grid's staging buffer (it is free until the state is committed)
+  if (gn->stage_doubles * 8 < map.size() * 4) return HAMR_ENOMEM;
+  int4* d_map = (int4*)gn->stage;
+  cudaError_t e = cudaMemcpyAsync(d_map, map.data(), map.size() * 4, cudaMemcpyHostToDevice, go->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(gn->D.B.cur, 0, (size_t)Hn.nblk * sizeof(int), go->stream);
+  if (e != cudaSuccess) return HAMR_ECUDA;
+  {
+    Launch l_(go, K_OTHER);
+    const int per = (L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);
+    k_blk_regrid<<<dim3((per + 255) / 256, Hn.nblk), 256, 0, go->stream>>>(go->D, bufs_of(go), gn->D, gn->s[0], d_map);
+  }
+  // the old grid's stream has written the new grid's arrays: finish before the new grid's stream goes on
+  if (cudaStreamSynchronize(go->stream) != cudaSuccess) return HAMR_ECUDA;
+  return cudaGetLastError() == cudaSuccess ? HAMR_OK : HAMR_ECUDA;
+}
+
 }  // namespace hamr

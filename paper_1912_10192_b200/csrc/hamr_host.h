@@ -239,6 +239,8 @@ void blk_unpack(hamr_grid* g, int kind, double* dense);             // kind: 0..
 int blk_initial(hamr_grid* g);                                      // ghosts, first flux pass, dt / levels
 int blk_step(hamr_grid* g, int nsteps);                             // nsteps coarse steps
 int blk_set_levels(hamr_grid* g, const int* tau);
+int blk_refine_radius(hamr_grid* g, double rho_cut, double* r_new);   // C-20: refinement criterion -> r_refine_max
+int blk_regrid(hamr_grid* go, hamr_grid* gn);                         // C-20: state of go onto the lattice of gn
 void blk_divb(hamr_grid* g);
 void blk_totals(hamr_grid* g);
 void blk_check_finite(hamr_grid* g);

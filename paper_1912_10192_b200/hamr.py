@@ -31,6 +31,7 @@ SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "h
            "hamr_get_backup_count", "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
            "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
            "hamr_get_block_bface", "hamr_set_all_blocks", "hamr_get_all_blocks",
+           "hamr_refine_radius", "hamr_regrid",
            "hamr_noalloc_setup", "hamr_divb_noalloc", "hamr_noalloc_last_error"]
 NOALLOC_MAX_ZONES = 16777216
 # ... and include/hamr_debug.h (test hooks and diagnostics)
@@ -118,6 +119,8 @@ def lib():
                                                   c_double_p, ip]
         L.hamr_debug_floors_drift.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p, ip]
         L.hamr_bench_fp64.argtypes = [vp, C.c_int, C.c_int, c_double_p, c_double_p]
+        L.hamr_refine_radius.argtypes = [vp, C.c_double, c_double_p]
+        L.hamr_regrid.argtypes = [vp, C.c_double, C.POINTER(vp)]
         L.hamr_noalloc_setup.argtypes = []
         L.hamr_divb_noalloc.argtypes = [C.POINTER(C.c_int), c_double_p, C.POINTER(vp), vp, vp]
         L.hamr_noalloc_last_error.argtypes = []
@@ -164,13 +167,16 @@ def _arr(x):
 class Grid:
     """hamr_grid handle.  p: parameter dict as produced by paper_1912_10192_b200.inputs.*_params."""
 
-    def __init__(self, p: dict, torch_arena: bool = False):
+    def __init__(self, p: dict, torch_arena: bool = False, _handle=None):
         self.L = lib()
         self.p = p
         self.n = tuple(int(v) for v in p["n"])
         self._par = pack_params(p)
         self._arena = None
         h = C.c_void_p(None)
+        if _handle is not None:          # a grid the library created itself (hamr_regrid)
+            self.h = _handle
+            return
         if torch_arena:
             import torch
             nbytes = C.c_size_t(0)
@@ -268,6 +274,18 @@ class Grid:
         c = (C.c_longlong * 4)()
         self._ck(self.L.hamr_get_stats(self.h, c))
         return tuple(c[:])
+
+    def refine_radius(self, rho_cut):
+        """hamr_refine_radius: the r_refine_max the density criterion asks for (0: no refined region)"""
+        r = C.c_double(0)
+        self._ck(self.L.hamr_refine_radius(self.h, float(rho_cut), C.byref(r)))
+        return r.value
+
+    def regrid(self, r_refine_max):
+        """hamr_regrid: a new Grid with that r_refine_max carrying this grid's state (this grid stays valid)"""
+        h = C.c_void_p(None)
+        self._ck(self.L.hamr_regrid(self.h, float(r_refine_max), C.byref(h)))
+        return Grid(dict(self.p, r_refine_max=float(r_refine_max)), _handle=h)
 
     def backup_count(self):
         """zones, since the last call, inverted from the entropy row (entropy_backup grids)"""
