@@ -157,6 +157,18 @@ ArenaPlan plan_arena(const hamr_params& p, const Lay& L, const GridShape& G) {
   return a;
 }
 
+void destroy_aux(hamr_grid* g) {
+  if (!g->aux[0]) return;
+  cudaStreamSynchronize(g->aux[0]);
+  cudaStreamSynchronize(g->aux[1]);
+  cudaStreamDestroy(g->aux[0]);
+  cudaStreamDestroy(g->aux[1]);
+  cudaEventDestroy(g->ev_fork);
+  cudaEventDestroy(g->ev_join[0]);
+  cudaEventDestroy(g->ev_join[1]);
+  g->aux[0] = g->aux[1] = nullptr;
+}
+
 int fail(hamr_grid* g, int code, const char* what, cudaError_t e = cudaSuccess) {
   if (g) {
     g->err = what;
@@ -193,6 +205,8 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   g->own_stream = own;
   g->arena = nullptr;
   g->stream = nullptr;
+  g->aux[0] = g->aux[1] = nullptr;
+  g->cemf_done = false;
   g->h_pinned = nullptr;
   g->have_state = false;
   g->blocks_open = false;
@@ -220,7 +234,17 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
     g->arena_bytes = arena_bytes;
     g->stream = (cudaStream_t)stream;
   }
+  // side streams and events of the fork / join in launch_flux_on; without them the sweeps run one after the other
+  if (cudaStreamCreateWithFlags(&g->aux[0], cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&g->aux[1], cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&g->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&g->ev_join[0], cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&g->ev_join[1], cudaEventDisableTiming) != cudaSuccess) {
+    g->aux[0] = g->aux[1] = nullptr;
+    cudaGetLastError();
+  }
   if ((e = cudaMallocHost((void**)&g->h_pinned, 64 * sizeof(double))) != cudaSuccess) {
+    destroy_aux(g);
     if (own) { cudaFree(g->arena); cudaStreamDestroy(g->stream); }
     delete g;
     return HAMR_ECUDA;
@@ -306,6 +330,7 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
   if (e != cudaSuccess) {
+    destroy_aux(g);
     cudaFreeHost(g->h_pinned);
     if (g->bh.h_ctop) cudaFreeHost(g->bh.h_ctop);
     if (g->bh.h_ints) cudaFreeHost(g->bh.h_ints);
@@ -340,7 +365,7 @@ int check_state(hamr_grid* g) {  // after a sync point: non-finite flag, sticky 
 void enqueue_stage(hamr_grid* g, const Fields& src, const Fields& base, const Fields& out, double dtfac,
                    bool same, bool want_ctop) {
   launch_ghosts(g, src, false);
-  launch_flux(g, src, want_ctop);
+  launch_flux(g, src, want_ctop, true);
   launch_ct(g, src);
   launch_deref_fix_edges(g, g->D);
   launch_update(g, src, base, out, dtfac, same);
@@ -501,6 +526,7 @@ int hamr_grid_destroy(hamr_grid* g) {
   for (cudaEvent_t e : g->ev) cudaEventDestroy(e);
   for (int c = 0; c < 2; c++)
     if (g->step_graph[c]) cudaGraphExecDestroy(g->step_graph[c]);
+  destroy_aux(g);
   if (g->own_arena) cudaFree(g->arena);
   if (g->own_stream) cudaStreamDestroy(g->stream);
   delete g;
@@ -831,7 +857,7 @@ int hamr_debug_emf(hamr_grid* g) {
   const Fields& sn = g->s[g->isn];
   launch_ghosts(g, sn, false);
   launch_zero_ctop(g);
-  launch_flux(g, sn, true);
+  launch_flux(g, sn, true, true);
   launch_ct(g, sn);
   launch_deref_fix_edges(g, g->D);
   launch_dt(g, 2);

@@ -1325,7 +1325,7 @@ static void blk_stage(hamr_grid* g, int tau, bool corrector) {
     const Fields& s0 = g->s[0];
     const Fields& s1 = g->s[1];
     const Fields& s2 = g->s[2];
-    launch_flux_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2, corrector);
+    launch_flux_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2, corrector, true);
     launch_ct_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2);
     launch_deref_fix_edges(g, D);
     if (H.refined) {   // C-16: same-time flux / EMF agreement on the refinement interface

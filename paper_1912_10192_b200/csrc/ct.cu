@@ -97,20 +97,28 @@ __global__ void __launch_bounds__(128) k_edge_emf(Dev Dv) {
   }
 }
 
-void launch_ct_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2) {
+// centre EMFs of the stage source (C-8); launch_flux_on may have issued this beside the flux sweeps (g->cemf_done)
+void launch_centre_emf_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2) {
   const Lay& L = Dv.L;
   const bool blk = Dv.B.nblk > 0;
   if (blk && Dv.B.nact == 0) return;
   const long long mult = blk ? Dv.B.nact : 1;
   const bool wrap = x3_ghosts_unused(Dv);
-  long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + (wrap ? 0 : 2)) * mult;
-  {
-    Launch l_(g, K_CEMF);
-    if (blk) k_centre_emf<true, false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
-    else if (wrap) k_centre_emf<false, true><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
-    else k_centre_emf<false, false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
-  }
-  tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1) * mult;
+  const long long tot = (long long)(L.n[0] + 2) * (L.n[1] + 2) * (L.n[2] + (wrap ? 0 : 2)) * mult;
+  Launch l_(g, K_CEMF);
+  if (blk) k_centre_emf<true, false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
+  else if (wrap) k_centre_emf<false, true><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
+  else k_centre_emf<false, false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv, src, src2);
+}
+
+void launch_ct_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2) {
+  const Lay& L = Dv.L;
+  const bool blk = Dv.B.nblk > 0;
+  if (blk && Dv.B.nact == 0) return;
+  const long long mult = blk ? Dv.B.nact : 1;
+  if (g->cemf_done) g->cemf_done = false;   // issued with the flux sweeps of the same source
+  else launch_centre_emf_on(g, Dv, src, src2);
+  const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1) * mult;
   Launch l_(g, K_EDGE);
   if (blk) k_edge_emf<true><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv);
   else k_edge_emf<false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(Dv);

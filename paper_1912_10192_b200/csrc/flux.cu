@@ -930,11 +930,7 @@ static void launch_march(hamr_grid* g, const Dev& Dv, const Fields& src, const F
   else launch_march_t<D, HAMR_RECON_PLM_MC, true>(g, Dv, src, src2, want_ctop);
 }
 
-// src / src2: the stage source in the buffer sets of blocks with cur == 0 / 2 (monolithic: src2 unused)
-void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
-  if (Dv.B.nblk > 0 && Dv.B.nact == 0) return;
-  launch_march<0>(g, Dv, src, src2, want_ctop);
-  launch_march<1>(g, Dv, src, src2, want_ctop);
+static void launch_x3(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop) {
   const Lay& L = Dv.L;
   const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
   const int own = ppm ? 29 : 31, halo = ppm ? 3 : 1;
@@ -963,16 +959,56 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
     else if (!blk) k_flux_x3<HAMR_RECON_PLM_MC, false, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else k_flux_x3<HAMR_RECON_PLM_MC, true, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
   }
-  if (Dv.mrow) {  // C-15: strided x3 fluxes of the derefined rows, then the group structure on all face values
-    launch_deref_x3(g, Dv, src, src2, want_ctop);
+  if (Dv.mrow) launch_deref_x3(g, Dv, src, src2, want_ctop);   // C-15: strided x3 fluxes of the derefined rows
+}
+
+// launches issued while this object lives go to `st` instead of the grid's stream
+struct OnStream {
+  hamr_grid* g;
+  cudaStream_t keep;
+  OnStream(hamr_grid* g_, cudaStream_t st) : g(g_), keep(g_->stream) { g->stream = st; }
+  ~OnStream() { g->stream = keep; }
+};
+
+// src / src2: the stage source in the buffer sets of blocks with cur == 0 / 2 (monolithic: src2 unused).
+// The three sweeps read the same source and write disjoint arrays (and disjoint Courant slots), so they are issued on
+// three streams between a fork and a join (inside a captured step: three parallel branches of the graph): the tail of
+// one sweep's last wave is filled by the next sweep's first, and the small launches of the upper LAT levels, which
+// leave most SMs idle, run side by side.  with_cemf: the caller's next call is launch_ct_on with the same source; its
+// centre-EMF kernel is then issued here, beside the sweeps.  Not while the per-kernel timers are on (they bracket launches on one stream).
+void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop, bool with_cemf) {
+  if (Dv.B.nblk > 0 && Dv.B.nact == 0) return;
+  const bool fork = g->aux[0] && g->aux[1] && !g->prof;
+  if (fork) {
+    cudaEventRecord(g->ev_fork, g->stream);
+    cudaStreamWaitEvent(g->aux[0], g->ev_fork, 0);
+    cudaStreamWaitEvent(g->aux[1], g->ev_fork, 0);
+    { OnStream os(g, g->aux[0]); launch_march<1>(g, Dv, src, src2, want_ctop); }
+    { OnStream os(g, g->aux[1]); launch_x3(g, Dv, src, src2, want_ctop); }
+    launch_march<0>(g, Dv, src, src2, want_ctop);
+    if (with_cemf) {
+      // the centre EMFs (C-8) need the source only: a memory-bound kernel beside the issue-bound sweeps
+      launch_centre_emf_on(g, Dv, src, src2);
+      g->cemf_done = true;
+    }
+    cudaEventRecord(g->ev_join[0], g->aux[0]);
+    cudaEventRecord(g->ev_join[1], g->aux[1]);
+    cudaStreamWaitEvent(g->stream, g->ev_join[0], 0);
+    cudaStreamWaitEvent(g->stream, g->ev_join[1], 0);
+  } else {
+    launch_march<0>(g, Dv, src, src2, want_ctop);
+    launch_march<1>(g, Dv, src, src2, want_ctop);
+    launch_x3(g, Dv, src, src2, want_ctop);
+  }
+  if (Dv.mrow) {  // C-15: the group structure on all face values
     launch_deref_fix_flux(g, Dv);
     launch_deref_flux_layers(g, Dv);
   }
 }
 
-void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop) {
+void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop, bool with_cemf) {
   if (g->D.entropy) launch_kappa(g, src);   // C-18: kappa of the (ghost-filled) source state for the entropy flux
-  launch_flux_on(g, g->D, src, src, want_ctop);
+  launch_flux_on(g, g->D, src, src, want_ctop, with_cemf);
 }
 
 }  // namespace hamr

@@ -150,6 +150,9 @@ struct hamr_grid {
   size_t arena_bytes;
   bool own_arena, own_stream;
   cudaStream_t stream;
+  cudaStream_t aux[2];       // side streams of the fork / join around independent launches of a stage (flux.cu); NULL: none
+  cudaEvent_t ev_fork, ev_join[2];
+  bool cemf_done;            // launch_flux_on has issued the centre-EMF kernel of the coming launch_ct_on
   double* stage;             // device staging buffer for dense <-> padded transfers
   size_t stage_doubles;
   double* h_pinned;          // small pinned host buffer for scalar read-back
@@ -200,7 +203,7 @@ namespace hamr {
 
 // kernel launchers (each returns after enqueueing on g->stream)
 void launch_ghosts(hamr_grid* g, const Fields& s, bool bc_active_too);
-void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop);
+void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop, bool with_cemf = false);
 void launch_ct(hamr_grid* g, const Fields& src);
 void launch_kappa(hamr_grid* g, const Fields& src);   // misc.cu: C-18, fills Dv.K from the source state (after its ghost fill)
 bool x3_ghosts_unused(const Dev& Dv);   // flux.cu: the stage kernels of this grid never read x3 ghost zones
@@ -213,7 +216,8 @@ void launch_divb(hamr_grid* g, const Fields& s);
 void launch_totals(hamr_grid* g, const Fields& s);
 void launch_check_finite(hamr_grid* g, const Fields& s);
 void launch_zero_ctop(hamr_grid* g);
-void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop);
+void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2, bool want_ctop, bool with_cemf = false);
+void launch_centre_emf_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2);
 void launch_ct_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2);
 void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles& rb, double dtfac, bool same);
 // deref.cu / flux.cu: phi-derefinement (C-15)
