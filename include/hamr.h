@@ -136,7 +136,9 @@ const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the 
  * the energy equation to recover the primitive variables"): a ninth conserved row, sqrt(-g) rho u^t kappa with
  * kappa = p / rho^gamma_ad, is advanced in every stage beside the others (HLL flux of the reconstructed kappa, no
  * source term) and, wherever the 2-unknown energy inversion does not converge or returns rho <= 0 or u < 0, the zone
- * is inverted from the density, momentum and entropy rows instead (one unknown, bracketed Newton).  kappa is reset
+ * is inverted from the density, momentum and entropy rows instead (one unknown, bracketed Newton).  Before that, where
+ * the Newton-Raphson inversion did not converge, the Aitken-accelerated fixed-point inversion the paper names beside it
+ * is tried: the chain is Newton-Raphson, Aitken, entropy, failure path (C-21).  kappa is reset
  * from the new primitives after every update, so the state handed in and out stays the eight primitives.  A zone
  * whose entropy row has no admissible root (kappa < 0) keeps what the energy inversion gave it: its converged state,
  * for the floors to repair, or the failure path of hamr_get_stats counts[0].  Needs gamma_ad < 2.

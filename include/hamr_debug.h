@@ -73,6 +73,12 @@ int hamr_debug_kappa(hamr_grid* g, double* out);
  * new field Bc (n x 3), guess (n x 5) -> out (n x 5), rc (n): 0 ok, 1 no admissible root (out then holds the guess). */
 int hamr_debug_con2prim_entropy(hamr_grid* g, int n, const int* ti, const int* tj, const double* U, const double* US,
                                 const double* Bc, const double* guess, double* out, int* rc);
+/* The Aitken-accelerated inversion (C-21) as the update kernels run it where the Newton-Raphson one did not
+ * converge: arguments and codes as hamr_debug_con2prim.  hamr_debug_aitken_count: zones, since the last call, whose
+ * primitives came from it (entropy_backup grids). */
+int hamr_debug_con2prim_aitken(hamr_grid* g, int n, const int* ti, const int* tj, const double* U, const double* Bc,
+                               const double* guess, double* out, int* rc);
+int hamr_debug_aitken_count(hamr_grid* g, long long* n);
 /* hamr_debug_floors with the zone's field Bc (n x 3): drift-frame floors (C-19) when the grid has drift_floors = 1 */
 int hamr_debug_floors_drift(hamr_grid* g, int n, const int* ti, const int* tj, double* P, const double* Bc, int* flags);
 

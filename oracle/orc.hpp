@@ -80,6 +80,10 @@ void source(const double P[8], const State& S, const Geom& G, const double conn[
 int con2prim(const double U[5], const double Bc[3], const Geom& G, double gam,
              const double Pguess[5], double Pout[5], int* iters);
 
+// C-21: the Aitken-accelerated fixed-point inversion, same arguments and codes as con2prim
+int con2prim_aitken(const double U[5], const double Bc[3], const Geom& G, double gam,
+                    const double Pguess[5], double Pout[5], int* iters);
+
 // ---- C-18 entropy as a backup for the energy equation (Noble et al. 2009) ------------------------
 // kappa = p / rho^gamma_ad = (gamma_ad - 1) u / rho^gamma_ad: constant along smooth flow lines
 double entropy_kappa(double rho, double u, double gam);

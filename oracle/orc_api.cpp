@@ -50,7 +50,7 @@ static Grid* grid_new(const Params& par) {
   g->t = 0.0;
   g->dt = 0.0;
   g->have_state = false;
-  g->stats = Stats{0, 0, 0, 0, 0};
+  g->stats = Stats{0, 0, 0, 0, 0, 0};
   if (!params_ok(par, g->err)) { delete g; return nullptr; }
   g->multi = par.nb[0] > 0 || par.nb[1] > 0 || par.nb[2] > 0 || par.n_deref > 0 ||
              par.lat_max_level > 0 || par.r_refine_max > 0.0;
@@ -200,7 +200,7 @@ int orc_set_prims(void* h, const double* const hydro[5], const double* const bfa
     blocks_initial_dt(g);
     g.t = 0.0;
     g.have_state = true;
-    g.stats = Stats{0, 0, 0, 0, 0};
+    g.stats = Stats{0, 0, 0, 0, 0, 0};
     return state_finite(g) ? 0 : 5;
   }
   Block& b = g.blocks[0];
@@ -228,7 +228,7 @@ int orc_set_prims(void* h, const double* const hydro[5], const double* const bfa
   g.dt = dt_from_ctop(g.par, b);
   g.t = 0.0;
   g.have_state = true;
-  g.stats = Stats{0, 0, 0, 0, 0};
+  g.stats = Stats{0, 0, 0, 0, 0, 0};
   return state_finite(g) ? 0 : 5;
 }
 
@@ -332,6 +332,13 @@ int orc_get_backup_count(void* h, long long* n) {
   g.stats.c2p_entropy = 0;
   return 0;
 }
+// zones, since the last call, whose primitives came from the Aitken-accelerated inversion (C-21)
+int orc_get_aitken_count(void* h, long long* n) {
+  Grid& g = *(Grid*)h;
+  *n = g.stats.c2p_aitken;
+  g.stats.c2p_aitken = 0;
+  return 0;
+}
 // kappa = (entropy row) / (density row) of the latest update, before it is reset from the primitives; active zones
 int orc_get_kadv(void* h, double* out) {
   Grid& g = *(Grid*)h;
@@ -421,7 +428,7 @@ int orc_blocks_commit(void* h) {
   blocks_initial_dt(g);
   g.t = 0.0;
   g.have_state = true;
-  g.stats = Stats{0, 0, 0, 0, 0};
+  g.stats = Stats{0, 0, 0, 0, 0, 0};
   return state_finite(g) ? 0 : 5;
 }
 int orc_get_block_prims(void* h, int bi, double* const prims[8]) {
@@ -500,9 +507,13 @@ int orc_con2prim(const double* U5, const double* Bc, const Geom* G, double gam, 
 // floors and Lorentz-factor ceiling of C-13 on one zone at radius r; counts3: rho-floor, u-floor, ceiling hits
 // Bc3: the zone's field (read with par->drift_floors; may be NULL)
 void orc_floors(const Params* par, const Geom* G, double r, double* P5, const double* Bc3, long long* counts3) {
-  Stats st = {0, 0, 0, 0, 0};
+  Stats st = {0, 0, 0, 0, 0, 0};
   floors_and_ceiling(*par, *G, r, P5, Bc3, st);
   counts3[0] = st.rho_floor; counts3[1] = st.u_floor; counts3[2] = st.gam_ceil;
+}
+int orc_con2prim_aitken(const double* U5, const double* Bc, const Geom* G, double gam, const double* Pguess,
+                        double* Pout, int* iters) {
+  return con2prim_aitken(U5, Bc, *G, gam, Pguess, Pout, iters);
 }
 int orc_con2prim_entropy(const double* U5, double US, const double* Bc, const Geom* G, double gam,
                          const double* Pguess, double* Pout, int* iters) {

@@ -581,9 +581,9 @@ void update(const Params& par, Block& b, const Fields& src, const Fields& base, 
         }
   }
   compute_Bc(b, out, true);
-  long long nfail = 0, nrf = 0, nuf = 0, ngc = 0, nent = 0;
+  long long nfail = 0, nrf = 0, nuf = 0, ngc = 0, nent = 0, nait = 0;
   if (par.entropy_backup) b.Kadv.assign(b.size(), 0.0);
-#pragma omp parallel for collapse(2) reduction(+ : nfail, nrf, nuf, ngc, nent)
+#pragma omp parallel for collapse(2) reduction(+ : nfail, nrf, nuf, ngc, nent, nait)
   for (int i = 0; i < b.n[0]; i++)
     for (int j = 0; j < b.n[1]; j++) {
       const Geom& G = b.gc[b.idx2(i, j)];
@@ -607,6 +607,15 @@ void update(const Params& par, Block& b, const Fields& src, const Fields& base, 
         const double Bn[3] = {out.Bc[0][z], out.Bc[1][z], out.Bc[2][z]};
         double Pn[5];
         int rc = con2prim(U, Bn, G, par.gamma_ad, Ps, Pn, nullptr);
+        if (par.entropy_backup && rc != 0) {
+          // C-21: the second primary inversion, where the Newton-Raphson one did not converge
+          double Pa[5];
+          if (con2prim_aitken(U, Bn, G, par.gamma_ad, Ps, Pa, nullptr) == 0) {
+            for (int c = 0; c < 5; c++) Pn[c] = Pa[c];
+            rc = 0;
+            nait++;
+          }
+        }
         if (par.entropy_backup) {
           // C-18: the entropy row, advanced like the others (no source term), and the backup inversion wherever
           // the energy inversion failed or returned a state without positive density and non-negative energy
@@ -631,13 +640,13 @@ void update(const Params& par, Block& b, const Fields& src, const Fields& base, 
           nfail++;
           for (int c = 0; c < 5; c++) Pn[c] = Ps[c];
         }
-        Stats loc = {0, 0, 0, 0, 0};
+        Stats loc = {0, 0, 0, 0, 0, 0};
         floors_and_ceiling(par, G, r, Pn, Bn, loc);
         nrf += loc.rho_floor; nuf += loc.u_floor; ngc += loc.gam_ceil;
         for (int c = 0; c < 5; c++) out.P[c][z] = Pn[c];
       }
     }
-  st.c2p_entropy += nent; st.c2p_fail += nfail; st.rho_floor += nrf; st.u_floor += nuf; st.gam_ceil += ngc;
+  st.c2p_entropy += nent; st.c2p_aitken += nait; st.c2p_fail += nfail; st.rho_floor += nrf; st.u_floor += nuf; st.gam_ceil += ngc;
   deref_sync_groups(par, b, out);
 }
 

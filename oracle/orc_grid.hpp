@@ -63,7 +63,7 @@ struct Block {
   double xf(int d, int i) const { return x0[d] + (double)(I0[d] + i) * dx[d]; }
 };
 
-struct Stats { long long c2p_fail, rho_floor, u_floor, gam_ceil, c2p_entropy; };
+struct Stats { long long c2p_fail, rho_floor, u_floor, gam_ceil, c2p_entropy, c2p_aitken; };
 
 struct Grid {
   Params par;

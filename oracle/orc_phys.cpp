@@ -315,6 +315,86 @@ int con2prim_entropy(const double U[5], double US, const double Bc[3], const Geo
   return 0;
 }
 
+// ---- C-21: the Aitken-accelerated inversion ("... or Aitken acceleration scheme (Hamlin & Newman 2013;
+// Newman & Hamlin 2014)"): the second primary inversion, tried where the Newton-Raphson one does not converge -------
+// A fixed-point iteration on the gas pressure.  With the normal observer's e = -Q.n (total energy density, rest mass
+// included), M^2 = Qt^2, T = Q.B, and  eps = W + Bsq  (W = w gamma^2), the energy equation
+//   e = W - p + Bsq/2 + (Bsq v^2 - T^2/W^2)/2   and the momentum equation   M^2 = eps^2 v^2 - T^2 (2W + Bsq)/W^2
+// combine (Bsq (2W + Bsq) - eps^2 = -W^2) into a cubic for eps at GIVEN pressure:
+//   eps^3 - a eps^2 + d = 0,   a = e + p + Bsq/2,   d = (M^2 Bsq - T^2)/2 >= 0,
+// whose largest root, for 0 <= d <= 4 a^3/27, is  eps = (a/3)(1 + 2 cos((2/3) asin sqrt(27 d/(4 a^3)))).
+// Then W = eps - Bsq, v^2 = (M^2 W^2 + T^2 (Bsq + 2W))/(W eps)^2, rho = D sqrt(1 - v^2), and the new pressure
+// p' = (gamma_ad - 1)/gamma_ad (W (1 - v^2) - rho).  Every third value of the sequence is replaced by Aitken's
+// extrapolation  p2 - (p2 - p1)^2/((p2 - p1) - (p1 - p0)).  Start: p of P_guess.  Stop when two successive plain
+// iterates differ by <= 1e-13 |p| + 1e-16 a; cap 60 double steps.  Returns 0 ok, 1 no convergence or a converged
+// pressure whose v^2 had to be clamped below 1 (no state carries that momentum), 2 no real root / non-finite.  A converged root with u < 0 is returned as such (as in con2prim).
+int con2prim_aitken(const double U[5], const double Bc[3], const Geom& G, double gam,
+                    const double Pguess[5], double Pout[5], int* iters) {
+  if (iters) *iters = 0;
+  const double ig = 1.0 / G.gdet, alpha = G.alpha;
+  const double rhout = U[0] * ig;
+  const double D = alpha * rhout;
+  double Qcov[4] = {alpha * (U[1] * ig - rhout), alpha * U[2] * ig, alpha * U[3] * ig, alpha * U[4] * ig};
+  double Qcon[4], ncon[4], Bs[4] = {0.0, alpha * Bc[0], alpha * Bc[1], alpha * Bc[2]};
+  for (int m = 0; m < 4; m++) {
+    double acc = 0.0;
+    for (int n = 0; n < 4; n++) acc += G.gcon[m][n] * Qcov[n];
+    Qcon[m] = acc;
+    ncon[m] = -alpha * G.gcon[m][0];
+  }
+  double Qdotn = 0.0, QQ = 0.0, T = 0.0, Bsq = 0.0;
+  for (int m = 0; m < 4; m++) { Qdotn += Qcov[m] * ncon[m]; QQ += Qcov[m] * Qcon[m]; }
+  for (int i = 1; i < 4; i++) {
+    T += Qcov[i] * Bs[i];
+    for (int j = 1; j < 4; j++) Bsq += G.gcov[i][j] * Bs[i] * Bs[j];
+  }
+  const double M2 = QQ + Qdotn * Qdotn, e = -Qdotn;
+  const double d = std::max(0.0, 0.5 * (M2 * Bsq - T * T));
+  const double cg = (gam - 1.0) / gam;
+  if (!std::isfinite(e) || !std::isfinite(M2) || !std::isfinite(Bsq) || !(D > 0.0)) return 2;
+  double W = 0.0, v2 = 0.0, a = 0.0;
+  int bad = 0;
+  bool clamped = false;
+  auto step = [&](double p) {
+    a = e + p + 0.5 * Bsq;
+    if (!(a > 0.0)) { bad = 2; return p; }
+    const double s2 = 27.0 * d / (4.0 * a * a * a);
+    if (!(s2 <= 1.0)) { bad = 2; return p; }
+    const double eps = (a / 3.0) * (1.0 + 2.0 * std::cos((2.0 / 3.0) * std::asin(std::sqrt(s2))));
+    W = eps - Bsq;
+    if (!(W > 0.0)) { bad = 2; return p; }
+    v2 = (M2 * W * W + T * T * (Bsq + 2.0 * W)) / ((W * eps) * (W * eps));
+    clamped = !(v2 <= 1.0 - 1e-15);   // more momentum than this energy can carry: iterated on, refused at the end
+    v2 = std::min(std::max(v2, 0.0), 1.0 - 1e-15);
+    return cg * (W * (1.0 - v2) - D * std::sqrt(1.0 - v2));
+  };
+  double p0 = (gam - 1.0) * Pguess[1];
+  bool conv = false;
+  int it;
+  for (it = 0; it < 60 && !conv; it++) {
+    const double p1 = step(p0);
+    const double p2 = step(p1);
+    if (bad || !std::isfinite(p2)) { if (iters) *iters = it; return 2; }
+    conv = std::fabs(p2 - p1) <= 1e-13 * std::fabs(p2) + 1e-16 * a;
+    const double den = (p2 - p1) - (p1 - p0);
+    const double pa = p2 - (p2 - p1) * (p2 - p1) / den;
+    p0 = (conv || den == 0.0 || !std::isfinite(pa)) ? p2 : pa;
+  }
+  if (iters) *iters = it;
+  if (!conv) return 1;
+  step(p0);   // W, v^2 of the converged pressure
+  if (bad) return 2;
+  if (clamped) return 1;
+  const double gamma = 1.0 / std::sqrt(1.0 - v2);
+  const double rho = D / gamma;
+  const double u = (W / (gamma * gamma) - rho) / gam;
+  if (!std::isfinite(rho) || !std::isfinite(u) || !std::isfinite(W)) return 2;
+  Pout[0] = rho;
+  Pout[1] = u;
+  for (int i = 1; i < 4; i++) Pout[1 + i] = gamma / (W + Bsq) * (Qcon[i] + Qdotn * ncon[i] + T * Bs[i] / W);
+  return 0;
+}
+
 // C-5 PPM (Colella & Woodward 1984) on a uniform grid, zone j = a[2]
 static double ppm_slope(double am, double a0, double ap) {
   const double dl = a0 - am, dr = ap - a0;

@@ -31,6 +31,13 @@ __global__ void k_zone_physics(Dev Dv, int what, int n, const int* __restrict__ 
     const int rc = con2prim(U, Bc, G, Dv.gam, Pg, Pn);
     for (int c = 0; c < 5; c++) out[(size_t)s * 5 + c] = rc == 0 ? Pn[c] : Pg[c];   // C-13: a failed zone keeps its guess
     iout[s] = rc;
+  } else if (what == 5) {   // C-21
+    double U[5], Bc[3], Pg[5], Pn[5];
+    for (int c = 0; c < 5; c++) { U[c] = in[(size_t)s * 5 + c]; Pg[c] = in3[(size_t)s * 5 + c]; }
+    for (int c = 0; c < 3; c++) Bc[c] = in2[(size_t)s * 3 + c];
+    const int rc = con2prim_aitken(U, Bc, &G, Dv.gam, Pg, Pn);
+    for (int c = 0; c < 5; c++) out[(size_t)s * 5 + c] = rc == 0 ? Pn[c] : Pg[c];
+    iout[s] = rc;
   } else if (what == 3) {   // C-18: in = (U[5], US) per state
     double U[5], Bc[3], Pg[5], Pn[5];
     for (int c = 0; c < 5; c++) { U[c] = in[(size_t)s * 6 + c]; Pg[c] = in3[(size_t)s * 5 + c]; }
@@ -189,6 +196,23 @@ int hamr_debug_con2prim_entropy(hamr_grid* g, int n, const int* ti, const int* t
     u6[(size_t)s * 6 + 5] = US[s];
   }
   return zone_call(g, 3, n, ti, tj, u6.data(), 6, Bc, 3, guess, 5, out, false, rc);
+}
+
+int hamr_debug_con2prim_aitken(hamr_grid* g, int n, const int* ti, const int* tj, const double* U, const double* Bc,
+                               const double* guess, double* out, int* rc) {
+  if (!U || !Bc || !guess || !rc) return HAMR_EINVAL;
+  return zone_call(g, 5, n, ti, tj, U, 5, Bc, 3, guess, 5, out, false, rc);
+}
+
+int hamr_debug_aitken_count(hamr_grid* g, long long* n) {
+  if (!g || !n) return HAMR_EINVAL;
+  unsigned long long h = 0;
+  cudaError_t e = cudaMemcpyAsync(&h, g->D.cnt + N_AITKEN, sizeof(h), cudaMemcpyDeviceToHost, g->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(g->D.cnt + N_AITKEN, 0, sizeof(h), g->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
+  if (e != cudaSuccess) { g->err = cudaGetErrorString(e); return HAMR_ECUDA; }
+  *n = (long long)h;
+  return HAMR_OK;
 }
 
 int hamr_debug_floors_drift(hamr_grid* g, int n, const int* ti, const int* tj, double* P, const double* Bc, int* flags) {

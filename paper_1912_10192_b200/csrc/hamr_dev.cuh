@@ -354,6 +354,73 @@ static __device__ __noinline__ int con2prim_entropy(const double* __restrict__ U
   return 0;
 }
 
+// ---- C-21 ("... or Aitken acceleration scheme (Hamlin & Newman 2013; Newman & Hamlin
+// 2014)"): the second primary inversion, tried where the Newton-Raphson one does not converge ----------------------------
+// Fixed-point iteration on the gas pressure p.  With the normal observer's e = -Q.n, M^2 = Qt^2, T = Q.B and
+// eps = W + Bsq, energy and momentum equations combine into a cubic for eps at given p,
+//   eps^3 - a eps^2 + d = 0,  a = e + p + Bsq/2,  d = (M^2 Bsq - T^2)/2 >= 0,
+// with largest root eps = (a/3)(1 + 2 cos((2/3) asin sqrt(27 d/(4 a^3)))); then W = eps - Bsq,
+// v^2 = (M^2 W^2 + T^2 (Bsq + 2W))/(W eps)^2, rho = D sqrt(1 - v^2), p' = (gamma_ad - 1)/gamma_ad (W (1 - v^2) - rho).
+// Every third value is Aitken's extrapolation p2 - (p2 - p1)^2 / ((p2 - p1) - (p1 - p0)).  The start is the guess's
+// pressure only.  Returns 0 ok, 1 no convergence / no real root / non-finite.
+static __device__ __noinline__ int con2prim_aitken(const double* __restrict__ U, const double* __restrict__ Bc,
+                                                   const CGeo* __restrict__ Gp, double gam_ad,
+                                                   const double* __restrict__ Pg, double* __restrict__ Pout) {
+  const CGeo& G = *Gp;
+  const double D = G.alpha * (U[0] * G.igdet);
+  const double m1 = U[2] * G.igdet, m2 = U[3] * G.igdet, m3 = U[4] * G.igdet;
+  const double e = -((U[1] - U[0]) * G.igdet - G.beta1 * m1);
+  const double Q1 = G.alpha * m1, Q2 = G.alpha * m2, Q3 = G.alpha * m3;
+  const double Qu1 = G.i11 * Q1 + G.i13 * Q3, Qu2 = G.i22 * Q2, Qu3 = G.i13 * Q1 + G.i33 * Q3;
+  const double M2 = Q1 * Qu1 + Q2 * Qu2 + Q3 * Qu3;
+  const double B1 = G.alpha * Bc[0], B2 = G.alpha * Bc[1], B3 = G.alpha * Bc[2];
+  const double Bsq = B1 * (G.c11 * B1 + G.c13 * B3) + B2 * (G.c22 * B2) + B3 * (G.c13 * B1 + G.c33 * B3);
+  const double T = Q1 * B1 + Q2 * B2 + Q3 * B3;
+  const double d = fmax(0.0, 0.5 * (M2 * Bsq - T * T));
+  const double cg = (gam_ad - 1.0) / gam_ad;
+  if (!(fabs(e) <= 1.79e308) || !(M2 <= 1.79e308) || !(Bsq <= 1.79e308) || !(D > 0.0)) return 1;
+  double W = 0.0, v2 = 0.0, a = 0.0;
+  bool bad = false, clamped = false;
+  auto step = [&](double p) {
+    a = e + p + 0.5 * Bsq;
+    if (!(a > 0.0)) { bad = true; return p; }
+    const double s2 = 27.0 * d / (4.0 * a * a * a);
+    if (!(s2 <= 1.0)) { bad = true; return p; }
+    const double eps = (a / 3.0) * (1.0 + 2.0 * cos((2.0 / 3.0) * asin(sqrt(s2))));
+    W = eps - Bsq;
+    if (!(W > 0.0)) { bad = true; return p; }
+    v2 = (M2 * W * W + T * T * (Bsq + 2.0 * W)) / ((W * eps) * (W * eps));
+    clamped = !(v2 <= 1.0 - 1e-15);   // more momentum than this energy can carry: refused at the end
+    v2 = dmin(dmax(v2, 0.0), 1.0 - 1e-15);
+    return cg * (W * (1.0 - v2) - D * sqrt(1.0 - v2));
+  };
+  double p0 = (gam_ad - 1.0) * Pg[1];
+  bool conv = false;
+  for (int it = 0; it < 60 && !conv; it++) {
+    const double p1 = step(p0);
+    const double p2 = step(p1);
+    if (bad || !(fabs(p2) <= 1.79e308)) return 1;
+    conv = fabs(p2 - p1) <= 1e-13 * fabs(p2) + 1e-16 * a;
+    const double den = (p2 - p1) - (p1 - p0);
+    const double pa = p2 - (p2 - p1) * (p2 - p1) / den;
+    p0 = (conv || den == 0.0 || !(fabs(pa) <= 1.79e308)) ? p2 : pa;
+  }
+  if (!conv) return 1;
+  step(p0);
+  if (bad || clamped) return 1;
+  const double gamma = 1.0 / sqrt(1.0 - v2);
+  const double rho = D / gamma;
+  const double u = (W / (gamma * gamma) - rho) / gam_ad;
+  if (!(fabs(rho) <= 1.79e308) || !(fabs(u) <= 1.79e308) || !(W <= 1.79e308)) return 1;
+  Pout[0] = rho;
+  Pout[1] = u;
+  const double fac = gamma / (W + Bsq), qw = T / W;
+  Pout[2] = fac * (Qu1 + qw * B1);
+  Pout[3] = fac * (Qu2 + qw * B2);
+  Pout[4] = fac * (Qu3 + qw * B3);
+  return 0;
+}
+
 // ---- C-19 (Ressler et al. 2017): floors applied in the drift frame ---------------
 // The matter added to reach the floors carries no momentum along the field and does not change the velocity across
 // it: with v = ut / gamma = v_perp + v_par Bhat in the normal observer's frame, v_perp is kept and v_par follows

@@ -18,7 +18,7 @@ struct Fields {
 enum Scal { S_T = 0, S_DT, S_CTOP0, S_CTOP1, S_CTOP2, S_DTLAST, S_DENMAX, S_DIVB, S_TOT0 /* ..+4 */,
             S_CTOPL0 = 13 /* ..+2: ctop of the last finished pass */, NSCAL = 16 };
 // device counters
-enum Cnt { N_C2PFAIL = 0, N_RHOFL, N_UFL, N_GCEIL, N_NONFINITE, N_ENTROPY /* zones inverted from the entropy row (C-18) */, NCNT = 8 };
+enum Cnt { N_C2PFAIL = 0, N_RHOFL, N_UFL, N_GCEIL, N_NONFINITE, N_ENTROPY /* zones inverted from the entropy row (C-18) */, N_AITKEN /* ... by the Aitken scheme (C-21) */, NCNT = 8 };
 
 // Block-structured grid: every per-variable array holds nblk
 // padded blocks back to back (block b at doubles [b*blen, (b+1)*blen)); a launch works on the blocks

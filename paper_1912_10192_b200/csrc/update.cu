@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(128, ROB ? 4 : (SAME ? UPD_MINB_PRED : UPD_MIN
   const unsigned per = (unsigned)(L.n[0] + 1) * c1 * c2;
   unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = t < (BLK ? per * Dv.B.nact : per);
-  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0, nent = 0;
+  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0, nent = 0, nait = 0;
   if (valid) {
     int bslot = 0;
     if (BLK) { bslot = (int)(t / per); t -= bslot * per; }
@@ -148,16 +148,23 @@ __global__ void __launch_bounds__(128, ROB ? 4 : (SAME ? UPD_MINB_PRED : UPD_MIN
       if (ROB && Dv.entropy) {
         Dv.K[z] = US / U[0];   // the advected kappa (diagnostic: k_kappa overwrites it before the next flux pass)
         if (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) {
-          // an entropy row that went negative or has no root leaves what the energy inversion gave: its converged
-          // state for the floors to repair, or its failure
-          // (the rare call works on copies, so that the common path's U, Bn, Pg and record stay in registers)
+          // the rare calls work on copies, so that the common path's U, Bn, Pg and record stay in registers
           double Pe[5], Uc[5], Bc[3], Pc[5];
           CGeo Gc = G2;
 #pragma unroll
           for (int c = 0; c < 5; c++) { Uc[c] = U[c]; Pc[c] = Pg[c]; }
 #pragma unroll
           for (int c = 0; c < 3; c++) Bc[c] = Bn[c];
-          if (con2prim_entropy(Uc, US, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
+          // C-21: the second primary inversion where Newton-Raphson did not converge
+          if (rc != 0 && con2prim_aitken(Uc, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
+#pragma unroll
+            for (int c = 0; c < 5; c++) Pn[c] = Pe[c];
+            rc = 0;
+            nait = 1;
+          }
+          // C-18: the entropy row where no energy inversion gave an admissible state.  An entropy row that went
+          // negative or has no root leaves what the energy inversion gave: its state for the floors, or its failure
+          if ((rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) && con2prim_entropy(Uc, US, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
 #pragma unroll
             for (int c = 0; c < 5; c++) Pn[c] = Pe[c];
             rc = 0;
@@ -195,8 +202,9 @@ __global__ void __launch_bounds__(128, ROB ? 4 : (SAME ? UPD_MINB_PRED : UPD_MIN
                  m_u = __ballot_sync(0xffffffffu, nuf), m_g = __ballot_sync(0xffffffffu, ngc),
                  m_b = __ballot_sync(0xffffffffu, bad);
   if (ROB) {
-    const unsigned m_e = __ballot_sync(0xffffffffu, nent);
+    const unsigned m_e = __ballot_sync(0xffffffffu, nent), m_a = __ballot_sync(0xffffffffu, nait);
     if ((threadIdx.x & 31) == 0 && m_e) atomicAdd(Dv.cnt + N_ENTROPY, (unsigned long long)__popc(m_e));
+    if ((threadIdx.x & 31) == 0 && m_a) atomicAdd(Dv.cnt + N_AITKEN, (unsigned long long)__popc(m_a));
   }
   if ((threadIdx.x & 31) == 0) {
     if (m_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)__popc(m_f));
@@ -272,7 +280,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
   }
   __syncthreads();
   request(i0, i0 + 1, i0);
-  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0, nent = 0;
+  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0, nent = 0, nait = 0;
   const int sk = jj * L.p3 + k;                    // this thread's element inside a staged chunk
   for (int i = i0; i < i1; i++) {
     const bool in0 = i < L.n[0];
@@ -376,14 +384,23 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
       if (ROB && Dv.entropy) {
         Dv.K[z] = US / U[0];   // the advected kappa (diagnostic: k_kappa overwrites it before the next flux pass)
         if (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) {
-          // the rare call works on copies, so that the common path's U, Bn, Ps and record stay in registers
+          // the rare calls work on copies, so that the common path's U, Bn, Ps and record stay in registers
           double Pe[5], Uc[5], Bc[3], Pc[5];
           CGeo Gc = G;
 #pragma unroll
           for (int c = 0; c < 5; c++) { Uc[c] = U[c]; Pc[c] = Ps[c]; }
 #pragma unroll
           for (int c = 0; c < 3; c++) Bc[c] = Bn[c];
-          if (con2prim_entropy(Uc, US, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
+          // C-21: the second primary inversion where Newton-Raphson did not converge
+          if (rc != 0 && con2prim_aitken(Uc, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
+#pragma unroll
+            for (int c = 0; c < 5; c++) Pn[c] = Pe[c];
+            rc = 0;
+            nait++;
+          }
+          // C-18: the entropy row where no energy inversion gave an admissible state.  An entropy row that went
+          // negative or has no root leaves what the energy inversion gave: its state for the floors, or its failure
+          if ((rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) && con2prim_entropy(Uc, US, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
 #pragma unroll
             for (int c = 0; c < 5; c++) Pn[c] = Pe[c];
             rc = 0;
@@ -421,8 +438,9 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
             s_u = __reduce_add_sync(0xffffffffu, nuf), s_g = __reduce_add_sync(0xffffffffu, ngc),
             s_b = __reduce_add_sync(0xffffffffu, bad);
   if (ROB) {
-    const int s_e = __reduce_add_sync(0xffffffffu, nent);
+    const int s_e = __reduce_add_sync(0xffffffffu, nent), s_a = __reduce_add_sync(0xffffffffu, nait);
     if (lane == 0 && s_e) atomicAdd(Dv.cnt + N_ENTROPY, (unsigned long long)s_e);
+    if (lane == 0 && s_a) atomicAdd(Dv.cnt + N_AITKEN, (unsigned long long)s_a);
   }
   if (lane == 0) {
     if (s_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)s_f);

@@ -38,7 +38,8 @@ NOALLOC_MAX_ZONES = 16777216
 DEBUG_SYMBOLS = ["hamr_set_levels", "hamr_debug_emf", "hamr_get_face", "hamr_get_edge", "hamr_get_ctop", "hamr_totals",
                  "hamr_profile_begin", "hamr_profile_end", "hamr_profile_class_name", "hamr_launch_count",
                  "hamr_debug_geometry", "hamr_debug_prim2cons", "hamr_debug_con2prim", "hamr_debug_floors",
-                 "hamr_debug_kappa", "hamr_debug_con2prim_entropy", "hamr_debug_floors_drift", "hamr_bench_fp64"]
+                 "hamr_debug_kappa", "hamr_debug_con2prim_entropy", "hamr_debug_floors_drift", "hamr_debug_con2prim_aitken",
+                 "hamr_debug_aitken_count", "hamr_bench_fp64"]
 NKCLASS = 10
 
 
@@ -117,6 +118,8 @@ def lib():
         L.hamr_debug_kappa.argtypes = [vp, c_double_p]
         L.hamr_debug_con2prim_entropy.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p, c_double_p, c_double_p,
                                                   c_double_p, ip]
+        L.hamr_debug_con2prim_aitken.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p, c_double_p, c_double_p, ip]
+        L.hamr_debug_aitken_count.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.hamr_debug_floors_drift.argtypes = [vp, C.c_int, ip, ip, c_double_p, c_double_p, ip]
         L.hamr_bench_fp64.argtypes = [vp, C.c_int, C.c_int, c_double_p, c_double_p]
         L.hamr_refine_radius.argtypes = [vp, C.c_double, c_double_p]
@@ -460,6 +463,21 @@ class Grid:
         self._ck(self.L.hamr_debug_con2prim_entropy(self.h, len(a), pa, pb, _dp(U), _dp(US), _dp(Bc), _dp(gs), _dp(out),
                                                     rc.ctypes.data_as(C.POINTER(C.c_int))))
         return out, rc
+
+    def con2prim_aitken(self, ti, tj, U, Bc, guess):
+        """U (n, 5), Bc (n, 3), guess (n, 5) -> hydro primitives (n, 5), rc (n): the Aitken-accelerated inversion"""
+        U, Bc, gs = _arr(U), _arr(Bc), _arr(guess)
+        a, b, pa, pb = self._ij(ti, tj)
+        out = np.empty((len(a), 5))
+        rc = np.zeros(len(a), dtype=np.int32)
+        self._ck(self.L.hamr_debug_con2prim_aitken(self.h, len(a), pa, pb, _dp(U), _dp(Bc), _dp(gs), _dp(out),
+                                                   rc.ctypes.data_as(C.POINTER(C.c_int))))
+        return out, rc
+
+    def aitken_count(self):
+        n = C.c_longlong(0)
+        self._ck(self.L.hamr_debug_aitken_count(self.h, C.byref(n)))
+        return n.value
 
     def floors_drift(self, ti, tj, P, Bc):
         """floors (in the drift frame on a drift_floors grid) and ceiling on P (n, 5) with field Bc (n, 3)"""

@@ -75,6 +75,8 @@ def lib():
                                    c_double_p, C.POINTER(C.c_int)]
         L.orc_floors.argtypes = [C.POINTER(Params), C.POINTER(Geom), C.c_double, c_double_p, c_double_p,
                                  C.POINTER(C.c_longlong)]
+        L.orc_con2prim_aitken.argtypes = [c_double_p, c_double_p, C.POINTER(Geom), C.c_double, c_double_p,
+                                          c_double_p, C.POINTER(C.c_int)]
         L.orc_con2prim_entropy.argtypes = [c_double_p, C.c_double, c_double_p, C.POINTER(Geom), C.c_double,
                                            c_double_p, c_double_p, C.POINTER(C.c_int)]
         L.orc_entropy_UF.argtypes = [c_double_p, C.POINTER(Geom), C.c_double, C.c_int, c_double_p, c_double_p]
@@ -85,6 +87,7 @@ def lib():
         L.orc_get_t.restype = C.c_double
         L.orc_get_t.argtypes = [C.c_void_p]
         L.orc_get_kadv.argtypes = [C.c_void_p, c_double_p]
+        L.orc_get_aitken_count.argtypes = [C.c_void_p, C.POINTER(C.c_longlong)]
         L.orc_ppm_zone.argtypes = [c_double_p] * 3
         L.orc_plm_zone.argtypes = [c_double_p] * 3
         L.orc_hll.argtypes = [c_double_p] * 4 + [C.c_double, C.c_double, c_double_p]
@@ -221,6 +224,11 @@ class OrcGrid:
     def backup_count(self):
         v = C.c_longlong(0)
         self.L.orc_get_backup_count(self.h, C.byref(v))
+        return v.value
+
+    def aitken_count(self):
+        v = C.c_longlong(0)
+        self.L.orc_get_aitken_count(self.h, C.byref(v))
         return v.value
 
     def kadv(self):
@@ -388,6 +396,15 @@ def floors(p, G, r, P5, Bc=None):
     B = _arr(Bc) if Bc is not None else None
     lib().orc_floors(C.byref(par), C.byref(G), float(r), _dp(P), _dp(B) if B is not None else None, c)
     return P, tuple(c[:])
+
+
+def con2prim_aitken(U5, Bc, G, gam, Pguess):
+    """C-21: the Aitken-accelerated fixed-point inversion"""
+    U5, Bc, Pg = _arr(U5), _arr(Bc), _arr(Pguess)
+    out = np.zeros(5)
+    it = C.c_int(0)
+    rc = lib().orc_con2prim_aitken(_dp(U5), _dp(Bc), C.byref(G), gam, _dp(Pg), _dp(out), C.byref(it))
+    return rc, out, it.value
 
 
 def con2prim_entropy(U5, US, Bc, G, gam, Pguess):

@@ -285,3 +285,78 @@ def test_cfg2_full_size_with_entropy_backup_and_drift_floors(H, orc):
     # floors act on ~45 % of the zone updates, the entropy inversion on none; it is driven by the other tests)
     assert abs(bg - bo) <= max(3, bo // 50) and abs(sg[2] - so[2]) <= so[2] // 1000 and sg[2] > 10 ** 7
     assert g.divb() <= 1e-12
+
+
+@pytest.mark.parametrize("regime,tol", [("mild", 1e-12), ("magnetised", 1e-9), ("relativistic", 1e-9)])
+def test_aitken_inversion_matches_oracle(H, orc, regime, tol):
+    """C-21: the Aitken-accelerated fixed-point inversion zone by zone: round trip, against the oracle's
+    from the same guess, from guesses wrong by 1e-6 .. 1e6 (where Newton-Raphson fails for a third), and refusals"""
+    p = I.torus_params(entropy_backup=1)
+    ns = 300
+    g, rng, ti, tj, x1, x2, C, sc = _zone_setup(H, p, ns, 41)
+    kw = dict(mild=(1.5, 1.0, 0.0), magnetised=(1.0, 30.0, 0.0), relativistic=(12.0, 3.0, 0.0))[regime]
+    P = _states(rng, ns, sc, C[ti, tj, 8], *kw)
+    gam = p["gamma_ad"]
+    U = g.prim2cons(ti, tj, P)
+    Gs = [orc.geom_at(p["metric"], p["a"], x1[s], x2[s]) for s in range(ns)]
+    guess = P[:, :5] * (1 + 0.3 * rng.uniform(-1, 1, (ns, 5)))
+    out, rc = g.con2prim_aitken(ti, tj, U, P[:, 5:8], guess)
+    assert np.all(rc == 0)
+    vn = np.sqrt(((P[:, 2:5] * sc) ** 2).sum(axis=1, keepdims=True))
+    assert (np.abs(out[:, :2] - P[:, :2]) / P[:, :2]).max() <= tol
+    assert (np.abs(out[:, 2:5] - P[:, 2:5]) * sc / np.maximum(vn, 1e-3)).max() <= tol
+    worst = 0.0
+    for s in range(ns):
+        rco, Po, _ = orc.con2prim_aitken(U[s], P[s, 5:8], Gs[s], gam, guess[s])
+        assert rco == 0
+        worst = max(worst, (np.abs(out[s, :2] - Po[:2]) / Po[:2]).max(),
+                    (np.abs(out[s, 2:5] - Po[2:5]) * sc[s]).max() / max(vn[s, 0], 1e-3))
+    assert worst <= tol, worst
+    # the start is the guess's pressure only
+    nfail_newton = 0
+    for f in (1e-6, 1e3, 1e6):
+        bad = np.zeros((ns, 5))
+        bad[:, 0], bad[:, 1] = P[:, 0] * f, P[:, 1] * f
+        out2, rc2 = g.con2prim_aitken(ti, tj, U, P[:, 5:8], bad)
+        assert np.all(rc2 == 0)
+        assert (np.abs(out2[:, :2] - out[:, :2]) / np.abs(out[:, :2])).max() <= 100 * tol
+        nfail_newton += int((g.con2prim(ti, tj, U, P[:, 5:8], bad)[1] != 0).sum())
+    assert nfail_newton > ns // 10
+    # refusals: negative density row, momentum without a real root, NaN: the guess is kept
+    Ub = U.copy()
+    Ub[0::3, 0] *= -1.0
+    Ub[1::3, 2] = 50.0 * C[ti[1::3], tj[1::3], 12] * (np.abs(U[1::3, 0]) + np.abs(U[1::3, 1]) + 1.0) * sc[1::3, 0]
+    Ub[2::3, 1] = np.nan
+    out3, rc3 = g.con2prim_aitken(ti, tj, Ub, P[:, 5:8], guess)
+    assert np.all(rc3 != 0) and np.array_equal(out3, guess)
+    for s in range(0, ns, 7):
+        assert orc.con2prim_aitken(Ub[s], P[s, 5:8], Gs[s], gam, guess[s])[0] != 0
+
+
+def test_blast_step_takes_the_whole_inversion_chain(H, orc):
+    """a strong blast stepped at 4 x and at 40 x the Courant limit with the robust path on: zones where Newton-Raphson
+    does not converge go to the Aitken scheme, what that cannot invert to the entropy row, the rest keeps its source
+    state; all three counts and the four event counters equal on both sides, primitives to 1e-10"""
+    n = (32, 8, 32)
+    p = I.minkowski_params(n=n, entropy_backup=1)
+    x = (np.arange(n[0]) + 0.5) / n[0]
+    y = (np.arange(n[1]) + 0.5) / n[1]
+    core = (np.abs(x - 0.5) < 0.13)[:, None, None] & np.ones(n, dtype=bool)
+    rho = np.where(core, 1.0, 1e-3) * (1.0 + 0.05 * np.cos(2 * np.pi * y))[None, :, None]
+    u = np.where(core, 1e3, 1e-3) * np.ones(n)
+    hyd = [rho, u, np.zeros(n), np.zeros(n), np.zeros(n)]
+    seen = np.zeros(3, dtype=int)
+    for fac in (4.0, 40.0):
+        g, o = _pair(H, orc, p, hyd, None)
+        g.dt = fac * g.dt
+        o.dt = fac * o.dt
+        g.step(1)
+        o.step(1)
+        cg = (g.stats(), g.aitken_count(), g.backup_count())
+        co = (o.stats(), o.aitken_count(), o.backup_count())
+        print("blast x", fac, "stats / aitken / entropy:", cg, co)
+        assert cg == co
+        seen += np.array([co[0][0], co[1], co[2]])
+        e = parity_errors(p, o.get_prims(), g.get_prims())
+        assert max(e.values()) <= 1e-10, e
+    assert seen[0] > 0 and seen[1] > 0 and seen[2] > 0, seen
