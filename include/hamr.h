@@ -193,6 +193,46 @@ int hamr_divb_noalloc(const int n[3], const double dx[3], const double* const bf
                       void* cuda_stream);
 const char* hamr_noalloc_last_error(void); /* never NULL; per host thread; "" after a successful call */
 
+/* ---- x1 slabs over peer memory: one grid on several GPUs ----------------------- */
+/* "H-AMR uses ... NVLINK for intra-node GPU-GPU ... communication" — blocks on different GPUs exchange
+ * their boundary zones every stage; PAPER.md:93 fn. 2: one Courant step for the whole grid.  Here the unit that is
+ * distributed is an x1 SLAB of a one-block grid: zones [i_lo, i_lo + n1) of the n[0] zones of `global` (global extents and
+ * boundary kinds; n1 >= 3).  One process per GPU holds one slab; a slab's geometry tables, floors and zone widths are those
+ * of the global grid bit for bit, and so is every zone it computes: slabs stepped in lockstep reproduce the one-grid
+ * result exactly.  There is NO exchange buffer and no pack / unpack step: the per-stage ghost fill of a slab reads the
+ * three x1 ghost layers of a side that has a neighbour straight from the neighbour's active zones through a device
+ * pointer to the neighbour's arena (the x2 / x3 boundary maps composed with it as with the physical x1 rules), i.e. over
+ * NVLink when that arena lives on a peer GPU (CUDA IPC / symmetric memory; the caller maps it) and through L2 / HBM when
+ * both slabs live on one GPU.  The interface face i_lo is held by both slabs, which advance it with bitwise equal EMFs.
+ * What the caller provides between the calls is ordering and one reduction (the Python binding's shard.py does it with
+ * torch.distributed: an all-reduce on the grid's stream is both):
+ *     every slab: hamr_set_prims(_dev)              | its part of the state (zones and faces i_lo .. i_lo + n1)
+ *     -- all slabs have been set --                 | barrier
+ *     every slab: hamr_shard_commit                 | ghosts from the neighbours, first flux pass
+ *     hamr_shard_ctop_get_dev -> MAX over slabs -> hamr_shard_ctop_set_dev      | first dt (C-14)
+ *     per step:   hamr_shard_stage(0)               | predictor: reads the neighbours' time-n state
+ *                 -- all slabs have finished stage 0 --
+ *                 hamr_shard_stage(1)               | corrector: reads the neighbours' predictor state
+ *                 hamr_shard_ctop_get_dev -> MAX over slabs -> hamr_shard_ctop_set_dev   | clock + next dt; also the barrier
+ * A slab never writes to a neighbour's memory; the buffer set a stage writes is never the one a neighbour reads in that
+ * stage, so the two ordering points per step are all the synchronisation there is.  hamr_step on a slab returns
+ * HAMR_ESTATE.  State out: the usual getters, per slab.  Needs a grid of one block without phi-derefinement; the robust
+ * inversion options (entropy_backup, drift_floors) are allowed.  A periodic x1 closes the ring (the last slab is the
+ * first one's low neighbour); with one slab covering the whole grid no neighbour is needed.
+ * hamr_shard_attach: `peer_arena` is the neighbour slab's arena (the pointer ITS hamr_shard_create_in was given, as
+ * seen from this process and device), (peer_i_lo, peer_n1) its extent; side 0 = low x1, 1 = high x1.  The library reads
+ * the neighbour's state arrays at the offsets its own arena plan gives for that extent; nothing is copied or owned.
+ * hamr_shard_ctop_get_dev / _set_dev take DEVICE pointers to three doubles (max signal speed per dimension, C-14) and
+ * enqueue on the grid's stream without synchronising. */
+int hamr_shard_workspace_bytes(const hamr_params* global, int i_lo, int n1, size_t* bytes);
+int hamr_shard_create_in(const hamr_params* global, int i_lo, int n1, void* arena, size_t arena_bytes,
+                         void* cuda_stream, hamr_grid** out);
+int hamr_shard_attach(hamr_grid* g, int side, const void* peer_arena, int peer_i_lo, int peer_n1);
+int hamr_shard_commit(hamr_grid* g);
+int hamr_shard_stage(hamr_grid* g, int stage);
+int hamr_shard_ctop_get_dev(hamr_grid* g, double* ctop3_dev);
+int hamr_shard_ctop_set_dev(hamr_grid* g, const double* ctop3_dev);
+
 /* ---- block-structured grid (BASELINE.json cfg 4) ------------------ */
 /* A grid with nb != {0,0,0} or lat_max_level > 0 is cut into blocks of nb zones (nb[d] = 0: the whole
  * extent; nb[d] must divide n[d] and be >= 3).  Blocks exchange ghost zones directly;

@@ -133,7 +133,7 @@ bool make_layout(const hamr_params& p, Lay& L, GridShape& G) {
 }
 
 struct ArenaPlan {
-  size_t arr, tabs, recs, scal, cnt, stage, blk, mrow, total;
+  size_t arr, tabs, recs, scal, cnt, peer, stage, blk, mrow, total;
   size_t stage_doubles;
 };
 
@@ -145,6 +145,7 @@ ArenaPlan plan_arena(const hamr_params& p, const Lay& L, const GridShape& G) {
   a.recs = off; off += align_up((size_t)G.nlev * (NREC_C + 3 * NREC_F) * L.n2d * 8, 256);   // geometry records
   a.scal = off; off += 256;
   a.cnt = off; off += 256;
+  a.peer = off; off += align_up(sizeof(PeerTab), 256);   // NEXT-4: neighbour-slab table (unused on other grids)
   a.stage_doubles = (size_t)8 * (p.n[0] + 1) * (p.n[1] + 1) * (p.n[2] + 1);
   // block-by-block state: every block has its own staging slot, so hamr_set_block_prims need not wait for the
   // previous block's copies (the stream is synchronised once, in hamr_blocks_commit)
@@ -183,8 +184,19 @@ int fail(hamr_grid* g, int code, const char* what, cudaError_t e = cudaSuccess) 
     if (e_ != cudaSuccess) return fail(g, HAMR_ECUDA, #call, e_);   \
   } while (0)
 
+// An x1 slab of a global grid (NEXT-4): zones [i_lo, i_lo + n1) of n1_global; p carries the slab's n[0] and the
+// GLOBAL extents and boundary kinds.
+struct SlabSpec { int i_lo, n1_global; };
+
+bool slab_ok(const hamr_params& gp, int i_lo, int n1, std::string& why) {
+  if (!params_ok(gp, why)) return false;
+  if (is_block_grid(gp) || gp.n_deref > 0 || gp.r_refine_max > 0.0) { why = "a slab is cut from a grid of one block without derefinement"; return false; }
+  if (i_lo < 0 || n1 < NG || i_lo + n1 > gp.n[0]) { why = "a slab needs 0 <= i_lo, n1 >= 3, i_lo + n1 <= n[0]"; return false; }
+  return true;
+}
+
 int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* stream, bool own,
-                  hamr_grid** out) {
+                  hamr_grid** out, const SlabSpec* slab = nullptr) {
   if (out) *out = nullptr;
   if (!p || !out) return HAMR_EINVAL;
   std::string why;
@@ -217,6 +229,11 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   g->step_graph[0] = g->step_graph[1] = nullptr;
   g->graph_launches = 0;
   g->plain_steps = 0;
+  g->sharded = slab != nullptr;
+  g->n1_global = slab ? slab->n1_global : p->n[0];
+  std::memset(&g->peers, 0, sizeof(g->peers));
+  g->shard_committed = false;
+  g->shard_stage = 0;
   g->isn = 0; g->ish = 1; g->inew = 2;
   cudaError_t e;
   if (own) {
@@ -258,9 +275,10 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   for (int d = 0; d < 3; d++) {
     D.bc_lo[d] = p->bc_lo[d];
     D.bc_hi[d] = p->bc_hi[d];
-    D.dx[d] = (hi[d] - lo[d]) / p->n[d];
+    D.dx[d] = (hi[d] - lo[d]) / (d == 0 ? g->n1_global : p->n[d]);
     D.x0[d] = lo[d];
   }
+  D.ioff = slab ? slab->i_lo : 0;
   D.a = p->a; D.gam = p->gamma_ad; D.cour = p->cour; D.gamma_max = p->gamma_max;
   D.rho_fl_coef = p->rho_fl_coef; D.rho_fl_pow = p->rho_fl_pow;
   D.u_fl_coef = p->u_fl_coef; D.u_fl_pow = p->u_fl_pow;
@@ -306,6 +324,7 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   D.B.tlevA = (NREC_C + 3 * NREC_F) * D.L.n2d;
   D.scal = (double*)(base + ap.scal);
   D.cnt = (unsigned long long*)(base + ap.cnt);
+  D.peer = slab ? (const PeerTab*)(base + ap.peer) : nullptr;
   g->stage = (double*)(base + ap.stage);
   g->stage_doubles = ap.stage_doubles;
 
@@ -456,6 +475,16 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
   }
   CK(cudaMemsetAsync(g->D.scal, 0, NSCAL * sizeof(double), g->stream));
   CK(cudaMemsetAsync(g->D.cnt, 0, NCNT * sizeof(unsigned long long), g->stream));
+  if (g->sharded) {
+    // NEXT-4: the ghost fill reads the neighbour slabs, which may not hold their state yet: hamr_shard_commit does the
+    // rest once every slab has been set
+    g->have_state = false;
+    g->shard_committed = false;
+    launch_check_finite(g, sn);
+    CK(cudaGetLastError());
+    if (dev) return HAMR_OK;
+    return check_state(g);
+  }
   if (blk) {
     const int rc = blk_initial(g);
     if (rc != HAMR_OK) return fail(g, rc, "block grid initialisation failed");
@@ -543,6 +572,7 @@ int hamr_set_prims_dev(hamr_grid* g, const double* const hydro[5], const double*
 int hamr_step_async(hamr_grid* g, int nsteps) {
   if (!g || nsteps < 0) return HAMR_EINVAL;
   if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
+  if (g->sharded) return fail(g, HAMR_ESTATE, "an x1 slab steps through hamr_shard_stage (its neighbours must keep pace)");
   if (!g->have_state) return fail(g, HAMR_ESTATE, "hamr_step before hamr_set_prims");
   if (g->bh.on) {
     const int rc = blk_step(g, nsteps);
@@ -670,7 +700,7 @@ int hamr_block_info(const hamr_grid* g, int b, double x_lo[3], double dx[3], int
   if (!g || b < 0 || b >= hamr_num_blocks(g)) return HAMR_EINVAL;
   for (int d = 0; d < 3; d++) {
     const double dxd = (d == 0 && g->bh.on && g->bh.lev1[b]) ? 0.5 * g->D.dx[0] : g->D.dx[d];
-    if (x_lo) x_lo[d] = g->D.x0[d] + (g->bh.on ? g->bh.I0[(size_t)b * 3 + d] * dxd : 0.0);
+    if (x_lo) x_lo[d] = g->D.x0[d] + (g->bh.on ? g->bh.I0[(size_t)b * 3 + d] * dxd : (d == 0 ? g->D.ioff * dxd : 0.0));
     if (dx) dx[d] = dxd;
     if (n) n[d] = g->D.L.n[d];
   }
@@ -844,6 +874,115 @@ static int get_block(hamr_grid* g, int b, int kind0, int nkind, double* const ou
 
 int hamr_get_block_prims(hamr_grid* g, int b, double* const prims[8]) { return get_block(g, b, 0, 8, prims); }
 int hamr_get_block_bface(hamr_grid* g, int b, double* const bface[3]) { return get_block(g, b, 8, 3, bface); }
+
+// ---- NEXT-4: x1 slabs with ghost layers read from peer memory ------------------
+static hamr_params slab_params(const hamr_params& gp, int n1) {
+  hamr_params p = gp;
+  p.n[0] = n1;
+  return p;
+}
+
+int hamr_shard_workspace_bytes(const hamr_params* gp, int i_lo, int n1, size_t* bytes) {
+  std::string why;
+  if (!gp || !bytes || !slab_ok(*gp, i_lo, n1, why)) return HAMR_EINVAL;
+  const hamr_params p = slab_params(*gp, n1);
+  return hamr_workspace_bytes(&p, bytes);
+}
+
+int hamr_shard_create_in(const hamr_params* gp, int i_lo, int n1, void* arena, size_t arena_bytes, void* cuda_stream,
+                         hamr_grid** out) {
+  if (out) *out = nullptr;
+  std::string why;
+  if (!gp || !out || !slab_ok(*gp, i_lo, n1, why)) return HAMR_EINVAL;
+  const hamr_params p = slab_params(*gp, n1);
+  const SlabSpec sp = {i_lo, gp->n[0]};
+  return create_common(&p, arena, arena_bytes, cuda_stream, false, out, &sp);
+}
+
+int hamr_shard_attach(hamr_grid* g, int side, const void* peer_arena, int peer_i_lo, int peer_n1) {
+  if (!g || !g->sharded || side < 0 || side > 1) return HAMR_EINVAL;
+  if (!peer_arena || ((uintptr_t)peer_arena & 255) != 0) return fail(g, HAMR_EINVAL, "peer arena is NULL or not 256-byte aligned");
+  const int i_lo = g->D.ioff, n1 = g->par.n[0], n1g = g->n1_global;
+  const bool periodic = g->par.bc_lo[0] == HAMR_BC_PERIODIC && n1 < n1g;
+  bool fits;
+  if (side == 0) fits = i_lo > 0 ? peer_i_lo + peer_n1 == i_lo : (periodic && peer_i_lo + peer_n1 == n1g);
+  else fits = i_lo + n1 < n1g ? peer_i_lo == i_lo + n1 : (periodic && peer_i_lo == 0);
+  if (peer_n1 < NG || peer_i_lo < 0 || !fits) return fail(g, HAMR_EINVAL, "the neighbour slab does not adjoin this side (or is thinner than 3 zones)");
+  // the neighbour's arena is laid out by the same plan: its 33 state arrays come first
+  const hamr_params pp = slab_params(g->par, peer_n1);
+  Lay PL;
+  GridShape pgs;
+  if (!make_layout(pp, PL, pgs)) return fail(g, HAMR_EINVAL, "neighbour layout");
+  if (PL.S1 != g->D.L.S1 || PL.S2 != g->D.L.S2) return fail(g, HAMR_EINVAL, "neighbour layout differs in x2 / x3");
+  const ArenaPlan pap = plan_arena(pp, PL, pgs);
+  const double* arr = (const double*)((const char*)peer_arena + pap.arr);
+  for (int q = 0; q < 3 * N_STATE_ARR; q++) g->peers.a[side][q] = arr + (size_t)q * PL.len;
+  g->peers.n1[side] = peer_n1;
+  g->peers.on[side] = 1;
+  CK(cudaMemcpyAsync((void*)g->D.peer, &g->peers, sizeof(PeerTab), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaStreamSynchronize(g->stream));   // g->peers may change before an asynchronous copy from pageable memory has read it
+  g->shard_committed = false;
+  return HAMR_OK;
+}
+
+static bool slab_sides_attached(const hamr_grid* g) {
+  const int i_lo = g->D.ioff, n1 = g->par.n[0], n1g = g->n1_global;
+  const bool periodic = g->par.bc_lo[0] == HAMR_BC_PERIODIC && n1 < n1g;
+  const bool need_lo = i_lo > 0 || periodic, need_hi = i_lo + n1 < n1g || periodic;
+  return (!need_lo || g->peers.on[0]) && (!need_hi || g->peers.on[1]);
+}
+
+int hamr_shard_commit(hamr_grid* g) {
+  if (!g || !g->sharded) return HAMR_EINVAL;
+  if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
+  if (!slab_sides_attached(g)) return fail(g, HAMR_ESTATE, "a side without a physical boundary has no neighbour slab (hamr_shard_attach)");
+  const Fields& sn = g->s[g->isn];
+  launch_ghosts(g, sn, true);
+  launch_flux(g, sn, true);   // C-14: one flux pass gives this slab's Courant maxima for the first step
+  g->have_state = true;
+  g->shard_committed = true;
+  g->shard_stage = 3;
+  CK(cudaGetLastError());
+  return HAMR_OK;
+}
+
+int hamr_shard_stage(hamr_grid* g, int stage) {
+  if (!g || !g->sharded || stage < 0 || stage > 1) return HAMR_EINVAL;
+  if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
+  if (!g->shard_committed) return fail(g, HAMR_ESTATE, "hamr_shard_stage before hamr_shard_commit");
+  if (g->shard_stage != stage) return fail(g, HAMR_ESTATE, "stages out of order: commit, ctop get / set, stage 0, stage 1, ctop get / set, ...");
+  const Fields& sn = g->s[g->isn];
+  const Fields& sh = g->s[g->ish];
+  const Fields& sw = g->s[g->inew];
+  if (stage == 0) {
+    enqueue_stage(g, sn, sn, sh, 0.5, true, false);
+    g->shard_stage = 1;
+  } else {
+    enqueue_stage(g, sh, sn, sw, 1.0, false, true);
+    const int tmp = g->isn; g->isn = g->inew; g->inew = tmp;
+    g->shard_stage = 2;
+  }
+  g->plain_steps++;
+  CK(cudaGetLastError());
+  return HAMR_OK;
+}
+
+int hamr_shard_ctop_get_dev(hamr_grid* g, double* ctop3_dev) {
+  if (!g || !g->sharded || !ctop3_dev) return HAMR_EINVAL;
+  if (!g->shard_committed || g->shard_stage < 2) return fail(g, HAMR_ESTATE, "the Courant maxima are complete after hamr_shard_commit or stage 1");
+  launch_ctop_out(g, ctop3_dev);
+  CK(cudaGetLastError());
+  return HAMR_OK;
+}
+
+int hamr_shard_ctop_set_dev(hamr_grid* g, const double* ctop3_dev) {
+  if (!g || !g->sharded || !ctop3_dev) return HAMR_EINVAL;
+  if (!g->shard_committed || g->shard_stage < 2) return fail(g, HAMR_ESTATE, "hamr_shard_ctop_set_dev follows hamr_shard_commit or stage 1");
+  launch_dt_slab(g, ctop3_dev, g->shard_stage == 2);   // after a step: advance the clock; after a commit: first dt only
+  g->shard_stage = 0;
+  CK(cudaGetLastError());
+  return HAMR_OK;
+}
 
 int hamr_set_levels(hamr_grid* g, const int* tau) {
   if (!g || !g->bh.on) return HAMR_EINVAL;

@@ -124,7 +124,9 @@ __global__ void k_geometry(Dev D, int e1, int e2, double dx1, int n2glob, double
   const int q = blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= e1 * e2) return;
   const int i = q / e2 - NG, j = q % e2 - NG;
-  const double xc1 = D.x0[0] + ((double)i + 0.5) * dx1, xf1 = D.x0[0] + (double)i * dx1;
+  // an x1 slab (NEXT-4) counts from the GLOBAL low corner, so that its tables equal the global grid's bit for bit
+  const int ig = i + D.ioff;
+  const double xc1 = D.x0[0] + ((double)ig + 0.5) * dx1, xf1 = D.x0[0] + (double)ig * dx1;
   const double xc2 = D.x0[1] + ((double)j + 0.5) * D.dx[1], xf2 = D.x0[1] + (double)j * D.dx[1];
   Metric4 M;
   metric_at(D.metric, D.a, xc1, xc2, M);

@@ -52,9 +52,20 @@ struct BlkDev {
   double* EA2[3];            // EMF registers
 };
 
+// x1-slab sharding: the state arrays of the neighbour slabs, as device pointers
+// valid on THIS device (peer memory over NVLink, or the same device).  Lives in device memory; the ghost fill reads the
+// x1 ghost layers of a side that has a neighbour straight from the neighbour's active zones.
+struct PeerTab {
+  const double* a[2][33];    // [side: 0 low x1, 1 high x1][buffer set * 11 + array: P 0..4, Bc 5..7, Bf 8..10]
+  int n1[2];                 // the neighbour's zone count along x1
+  int on[2];                 // side has a neighbour
+};
+
 struct Dev {                 // everything a kernel may need, passed by value
   Lay L;
   BlkDev B;
+  const PeerTab* peer;       // NEXT-4: neighbour slabs (NULL: the grid is not a slab)
+  int ioff;                  // NEXT-4: global x1 index of local zone 0 (geometry tables, floors)
   int metric, recon;
   int bc_lo[3], bc_hi[3];
   double dx[3], x0[3];       // internal-coordinate spacing and origin
@@ -170,6 +181,12 @@ struct hamr_grid {
   cudaGraphExec_t step_graph[2];
   long long graph_launches;      // kernel launches one replay stands for
   int plain_steps;               // steps enqueued launch by launch so far
+  // NEXT-4: the grid is an x1 slab [i_lo, i_lo + n[0]) of a global grid of n1_global zones
+  bool sharded;
+  int n1_global;
+  hamr::PeerTab peers;           // host copy of D.peer
+  bool shard_committed;          // hamr_shard_commit has run on the current state
+  int shard_stage;               // next stage hamr_shard_stage expects (0 / 1), 2: the step's hamr_shard_ctop_set_dev
 };
 
 namespace hamr {
@@ -210,6 +227,8 @@ bool x3_ghosts_unused(const Dev& Dv);   // flux.cu: the stage kernels of this gr
 void launch_update(hamr_grid* g, const Fields& src, const Fields& base, const Fields& out, double dtfac,
                    bool src_is_base);
 void launch_dt(hamr_grid* g, int mode);  // 0 set dt, 1 advance t + set dt, 2 latch ctop only
+void launch_ctop_out(hamr_grid* g, double* out3);                    // NEXT-4: this slab's Courant maxima -> out3 (device)
+void launch_dt_slab(hamr_grid* g, const double* in3, bool advance);  // NEXT-4: dt from the maxima over all slabs (device)
 void launch_pack(hamr_grid* g, const double* dense, double* padded, int stag, bool zero_pole);
 void launch_unpack(hamr_grid* g, const double* padded, double* dense, const int m[3]);
 void launch_divb(hamr_grid* g, const Fields& s);

@@ -22,6 +22,35 @@ __global__ void k_dt(Dev Dv, int mode) {
   if (mode != 2) s[S_DT] = Dv.cour / sum;
 }
 
+// NEXT-4 (x1 slabs): the Courant maxima leave the grid for the max over all slabs (one global step) ...
+__global__ void k_ctop_out(Dev Dv, double* __restrict__ out3) {
+  for (int d = 0; d < 3; d++) out3[d] = Dv.scal[S_CTOP0 + d];
+}
+// ... and come back reduced: the arithmetic of k_dt on them
+__global__ void k_dt_slab(Dev Dv, const double* __restrict__ in3, int advance) {
+  double* s = Dv.scal;
+  if (advance) {
+    s[S_T] += s[S_DT];
+    s[S_DTLAST] = s[S_DT];
+  }
+  double sum = 0.0;
+  for (int d = 0; d < 3; d++) {
+    sum += in3[d] / Dv.dx[d];
+    s[S_CTOPL0 + d] = in3[d];
+    s[S_CTOP0 + d] = 0.0;
+  }
+  s[S_DT] = Dv.cour / sum;
+}
+
+void launch_ctop_out(hamr_grid* g, double* out3) {
+  Launch l_(g, K_DT);
+  k_ctop_out<<<1, 1, 0, g->stream>>>(g->D, out3);
+}
+void launch_dt_slab(hamr_grid* g, const double* in3, bool advance) {
+  Launch l_(g, K_DT);
+  k_dt_slab<<<1, 1, 0, g->stream>>>(g->D, in3, advance ? 1 : 0);
+}
+
 __global__ void k_zero_ctop(Dev Dv) {
   Dv.scal[S_CTOP0] = Dv.scal[S_CTOP1] = Dv.scal[S_CTOP2] = 0.0;
 }

@@ -32,6 +32,8 @@ SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "h
            "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
            "hamr_get_block_bface", "hamr_set_all_blocks", "hamr_get_all_blocks",
            "hamr_refine_radius", "hamr_regrid",
+           "hamr_shard_workspace_bytes", "hamr_shard_create_in", "hamr_shard_attach", "hamr_shard_commit",
+           "hamr_shard_stage", "hamr_shard_ctop_get_dev", "hamr_shard_ctop_set_dev",
            "hamr_noalloc_setup", "hamr_divb_noalloc", "hamr_noalloc_last_error"]
 NOALLOC_MAX_ZONES = 16777216
 # ... and include/hamr_debug.h (test hooks and diagnostics)
@@ -124,6 +126,13 @@ def lib():
         L.hamr_bench_fp64.argtypes = [vp, C.c_int, C.c_int, c_double_p, c_double_p]
         L.hamr_refine_radius.argtypes = [vp, C.c_double, c_double_p]
         L.hamr_regrid.argtypes = [vp, C.c_double, C.POINTER(vp)]
+        L.hamr_shard_workspace_bytes.argtypes = [C.POINTER(Params), C.c_int, C.c_int, C.POINTER(C.c_size_t)]
+        L.hamr_shard_create_in.argtypes = [C.POINTER(Params), C.c_int, C.c_int, vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.hamr_shard_attach.argtypes = [vp, C.c_int, vp, C.c_int, C.c_int]
+        L.hamr_shard_commit.argtypes = [vp]
+        L.hamr_shard_stage.argtypes = [vp, C.c_int]
+        L.hamr_shard_ctop_get_dev.argtypes = [vp, vp]
+        L.hamr_shard_ctop_set_dev.argtypes = [vp, vp]
         L.hamr_noalloc_setup.argtypes = []
         L.hamr_divb_noalloc.argtypes = [C.POINTER(C.c_int), c_double_p, C.POINTER(vp), vp, vp]
         L.hamr_noalloc_last_error.argtypes = []
