@@ -4,12 +4,14 @@ fraction of the dominant kernel, the end-to-end number through the C-ABI with ho
 CPU oracle timed beside it.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg2r|cfg1|cfg0|cfg3|cfg4b|cfg4|cfg4t|paper150]
+                  [--shard S]
 
 A "step" is one full pass of the hot path over the whole grid: hamr_step(1) = predictor + corrector
 = one zone-cycle per zone.  Default workload: BASELINE.json configs[2], the 256x128x128
 Kerr Fishbone-Moncrief torus (the config the metric is quoted on).  Inputs are seeded and synthetic
 (paper_1912_10192_b200/inputs.py); the state (2.4 GB of fp64 arrays) is far larger than the 126 MB L2.
-N > 1: the path does not shard ("replicas only"): every rank runs an independent replica.
+N > 1: BASELINE's north_star runs everything on one GPU ("replicas only"): every rank runs an independent
+replica.  --shard runs ONE grid as x1 slabs instead: one slab per rank under torchrun.
 """
 from __future__ import annotations
 
@@ -290,6 +292,102 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_sharded(args):
+    """--shard: ONE grid as x1 slabs (paper_1912_10192_b200/shard.py).  Under torchrun every rank holds
+    one slab on its GPU and reads its neighbours' ghost layers over NVLink (strong scaling: the grid is fixed); on one GPU
+    (--shard S) the S slabs live in this process and the line carries the cost of slab stepping against the one-grid step."""
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local)
+    torch.cuda.set_stream(torch.cuda.Stream())
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import __graft_entry__ as ge
+    if rank == 0:
+        ge.build()
+    if world > 1:
+        dist.barrier()
+    from paper_1912_10192_b200 import hamr, shard
+    p, gen, desc = workload(args.workload)
+    if any(p["nb"]) or p["lat_max_level"] > 0:
+        raise SystemExit("--shard needs a one-block workload (cfg2, cfg2r, cfg3, cfg1, cfg0, paper150)")
+    nz = int(np.prod(p["n"]))
+    hyd, bf = gen()
+    steps = args.steps or 200
+    warm = max(args.warmup, 3)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(obj, k):
+        for _ in range(warm):
+            obj.step_async(1)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(k):
+            obj.step_async(1)
+        e1.record()
+        barrier()
+        return e0.elapsed_time(e1)
+
+    sampler = ClockSampler(local)
+    one_ms = None
+    if world > 1:
+        mem = "symm"
+        try:
+            ds = shard.DistSlab(p, peer_memory="symm")
+        except Exception as e:   # no symmetric-memory support on this box: CUDA IPC handles
+            mem = f"ipc (symmetric memory unavailable: {type(e).__name__})"
+            ds = shard.DistSlab(p, peer_memory="ipc")
+        assert ds.set_prims(hyd, bf) == 0
+        sampler.start()
+        l0 = ds.slab.launch_count()
+        ms = timed(ds, steps)
+        launches = round((ds.slab.launch_count() - l0) * steps / (steps + warm))   # the timed steps' share
+        clocks = sampler.stop()
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        parts, par = ds.ranges, f"{world} x1 slabs, one per GPU, ghost layers read over NVLink ({mem}); 2 all-reduces per step"
+        divb = ds.slab.divb()
+        ds.close()
+    else:
+        nslab = max(1, args.shard)
+        ring = shard.LocalRing(p, nslab)
+        assert ring.set_prims(hyd, bf) == 0
+        sampler.start()
+        l0 = ring.launch_count()
+        ms = timed(ring, steps)
+        launches = round((ring.launch_count() - l0) * steps / (steps + warm))      # the timed steps' share
+        one = hamr.Grid(p, torch_arena=True)
+        assert one.set_prims(hyd, bf) == 0
+        one_ms = timed(one, steps)
+        clocks = sampler.stop()
+        parts, par = ring.ranges, f"{nslab} x1 slabs on 1 GPU in one process (neighbour arenas on the same device)"
+        divb = ring.divb()
+        ring.close()
+        one.close()
+    if rank == 0:
+        line = {"metric": METRIC, "value": nz * steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": steps,
+                "warmup": warm, "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": desc, "zones": nz, "parallelism": par, "slabs": [list(q) for q in parts]},
+                "clocks": clocks, "gpu_launches": launches, "divb": divb}
+        if one_ms is not None:
+            line["one_grid"] = {"ms_per_step": one_ms / steps, "value": nz * steps / (one_ms * 1e-3),
+                                "slab_cost": ms / one_ms,
+                                "what": "the same workload as one grid (CUDA-graph replay of the step), timed right after"}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -300,7 +398,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--e2e-grids", type=int, default=3, help="grids in flight in the end-to-end measurement")
+    ap.add_argument("--shard", type=int, default=0,
+                    help="run ONE grid as x1 slabs (NEXT-4): under torchrun one slab per rank; on one GPU this many slabs")
     args = ap.parse_args()
+    if args.shard and args.impl != "reference":
+        return run_sharded(args)
     if args.impl == "reference":
         if args.steps is None:
             args.steps = 5
