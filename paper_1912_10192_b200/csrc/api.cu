@@ -234,6 +234,7 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   std::memset(&g->peers, 0, sizeof(g->peers));
   g->shard_committed = false;
   g->shard_stage = 0;
+  for (int a = 0; a < 2; a++) for (int b = 0; b < 2; b++) g->stage_graph[a][b] = nullptr;
   g->isn = 0; g->ish = 1; g->inew = 2;
   cudaError_t e;
   if (own) {
@@ -555,6 +556,9 @@ int hamr_grid_destroy(hamr_grid* g) {
   for (cudaEvent_t e : g->ev) cudaEventDestroy(e);
   for (int c = 0; c < 2; c++)
     if (g->step_graph[c]) cudaGraphExecDestroy(g->step_graph[c]);
+  for (int a = 0; a < 2; a++)
+    for (int b = 0; b < 2; b++)
+      if (g->stage_graph[a][b]) cudaGraphExecDestroy(g->stage_graph[a][b]);
   destroy_aux(g);
   if (g->own_arena) cudaFree(g->arena);
   if (g->own_stream) cudaStreamDestroy(g->stream);
@@ -954,15 +958,38 @@ int hamr_shard_stage(hamr_grid* g, int stage) {
   const Fields& sn = g->s[g->isn];
   const Fields& sh = g->s[g->ish];
   const Fields& sw = g->s[g->inew];
+  auto enqueue = [&]() {
+    if (stage == 0) enqueue_stage(g, sn, sn, sh, 0.5, true, false);
+    else enqueue_stage(g, sh, sn, sw, 1.0, false, true);
+  };
+  // as step_once: the stage's launches are captured once per buffer parity and replayed (every argument, the
+  // neighbour table included, is fixed for the grid); the first step, the legacy stream and the timers launch plainly
+  const int par = g->isn == 0 ? 0 : 1;
+  if (g->prof || g->plain_steps < 2 || g->stream == nullptr || g->stream == cudaStreamLegacy) {
+    enqueue();
+    g->plain_steps++;
+  } else {
+    if (!g->stage_graph[stage][par]) {
+      const long long l0 = g->launches;
+      cudaGraph_t graph = nullptr;
+      CK(cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal));
+      enqueue();
+      cudaError_t e = cudaStreamEndCapture(g->stream, &graph);
+      g->stage_launches[stage][par] = g->launches - l0;
+      g->launches = l0;
+      if (e == cudaSuccess) e = cudaGraphInstantiate(&g->stage_graph[stage][par], graph, 0);
+      if (graph) cudaGraphDestroy(graph);
+      if (e != cudaSuccess) return fail(g, HAMR_ECUDA, "capturing the stage as a CUDA graph", e);
+    }
+    CK(cudaGraphLaunch(g->stage_graph[stage][par], g->stream));
+    g->launches += g->stage_launches[stage][par];
+  }
   if (stage == 0) {
-    enqueue_stage(g, sn, sn, sh, 0.5, true, false);
     g->shard_stage = 1;
   } else {
-    enqueue_stage(g, sh, sn, sw, 1.0, false, true);
     const int tmp = g->isn; g->isn = g->inew; g->inew = tmp;
     g->shard_stage = 2;
   }
-  g->plain_steps++;
   CK(cudaGetLastError());
   return HAMR_OK;
 }

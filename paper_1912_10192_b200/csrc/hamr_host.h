@@ -187,6 +187,8 @@ struct hamr_grid {
   hamr::PeerTab peers;           // host copy of D.peer
   bool shard_committed;          // hamr_shard_commit has run on the current state
   int shard_stage;               // next stage hamr_shard_stage expects (0 / 1), 2: the step's hamr_shard_ctop_set_dev
+  cudaGraphExec_t stage_graph[2][2];   // [stage][parity of the rotating buffers]: a slab's stage as a CUDA graph
+  long long stage_launches[2][2];      // kernel launches one replay stands for
 };
 
 namespace hamr {
