@@ -396,7 +396,7 @@ def main():
     ap.add_argument("--impl", default="hamr", choices=["hamr", "reference"])
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--e2e-grids", type=int, default=3, help="grids in flight in the end-to-end measurement")
     ap.add_argument("--shard", type=int, default=0,
                     help="run ONE grid as x1 slabs (NEXT-4): under torchrun one slab per rank; on one GPU this many slabs")
@@ -545,12 +545,19 @@ def main():
     ops = [(hamr.c_double_p * 8)(*[hamr._dp(o) for o in oo]) for oo in outs2]
     outs = outs2[0]
 
+    # one grid at a time per direction of the link: a grid that shares the link with two others gets its input three
+    # times later, while one that has the link to itself starts stepping after a third of that time and frees the link
+    # for the next (the copies of concurrent calls would otherwise interleave array by array)
+    link_in, link_out = threading.Lock(), threading.Lock()
+
     def e2e_step(gh=None, op=None):
         gh = g.h if gh is None else gh
         op = ops[0] if op is None else op
-        rc = set_call(gh, hp, bp)
+        with link_in:
+            rc = set_call(gh, hp, bp)
         rc |= L.hamr_step(gh, 1, None, None)
-        rc |= get_call(gh, op)
+        with link_out:
+            rc |= get_call(gh, op)
         assert rc == 0, rc
 
     e2e_step()

@@ -216,8 +216,8 @@ const char* hamr_noalloc_last_error(void); /* never NULL; per host thread; "" af
  *                 hamr_shard_ctop_get_dev -> MAX over slabs -> hamr_shard_ctop_set_dev   | clock + next dt; also the barrier
  * A slab never writes to a neighbour's memory; the buffer set a stage writes is never the one a neighbour reads in that
  * stage, so the two ordering points per step are all the synchronisation there is.  hamr_step on a slab returns
- * HAMR_ESTATE.  State out: the usual getters, per slab.  Needs a grid of one block without phi-derefinement; the robust
- * inversion options (entropy_backup, drift_floors) are allowed.  A periodic x1 closes the ring (the last slab is the
+ * HAMR_ESTATE.  State out: the usual getters, per slab.  Needs a grid of one block (nb = 0, no LAT, no x1 refinement);
+ * phi-derefinement and the robust inversion options (entropy_backup, drift_floors) are allowed.  A periodic x1 closes the ring (the last slab is the
  * first one's low neighbour); with one slab covering the whole grid no neighbour is needed.
  * hamr_shard_attach: `peer_arena` is the neighbour slab's arena (the pointer ITS hamr_shard_create_in was given, as
  * seen from this process and device), (peer_i_lo, peer_n1) its extent; side 0 = low x1, 1 = high x1.  The library reads

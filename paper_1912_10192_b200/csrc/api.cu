@@ -190,7 +190,7 @@ struct SlabSpec { int i_lo, n1_global; };
 
 bool slab_ok(const hamr_params& gp, int i_lo, int n1, std::string& why) {
   if (!params_ok(gp, why)) return false;
-  if (is_block_grid(gp) || gp.n_deref > 0 || gp.r_refine_max > 0.0) { why = "a slab is cut from a grid of one block without derefinement"; return false; }
+  if (is_block_grid(gp) || gp.r_refine_max > 0.0) { why = "a slab is cut from a grid of one block"; return false; }
   if (i_lo < 0 || n1 < NG || i_lo + n1 > gp.n[0]) { why = "a slab needs 0 <= i_lo, n1 >= 3, i_lo + n1 <= n[0]"; return false; }
   return true;
 }
@@ -479,6 +479,8 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
   if (g->sharded) {
     // NEXT-4: the ghost fill reads the neighbour slabs, which may not hold their state yet: hamr_shard_commit does the
     // rest once every slab has been set
+    launch_deref_project(g, g->D, sn, sn);
+    launch_deref_sync(g, g->D, sn, sn);
     g->have_state = false;
     g->shard_committed = false;
     launch_check_finite(g, sn);

@@ -5,7 +5,7 @@ the neighbour reads of the multi-GPU job, the neighbour's arena being a pointer 
 What is checked: (1) the slabs reproduce the ONE-grid result of the same library bit for bit — same geometry tables,
 same per-face and per-zone arithmetic, interface faces advanced identically on both sides — for 2 and 3 slabs, ragged
 thicknesses, an outflow x1 (Kerr torus) and a periodic x1 that closes the ring (Minkowski waves), also with the robust
-inversion options; (2) parity of the slabs with the ORACLE at north_star's tolerances (the oracle knows nothing of
+inversion options and with phi-derefined polar rows; (2) parity of the slabs with the ORACLE at north_star's tolerances (the oracle knows nothing of
 slabs: it steps the whole grid); (3) div B, also across the interfaces; (4) the call-order and argument checks of the
 boundary; (5) cfg 2 at full size in two slabs, every zone, against the one-grid run."""
 import ctypes as C
@@ -48,6 +48,8 @@ def _cases():
     c["torus_plm_2"] = (r, lambda: I.fm_torus(r, seed=5), 2)
     e = dict(I.torus_params(n=(32, 16, 32)), entropy_backup=1, drift_floors=1)
     c["torus_robust_2"] = (e, lambda: I.fm_torus(e, seed=6), 2)
+    d = I.torus_params(n=(32, 16, 16), deref_theta_deg=(30.0, 12.0), deref_factor=(2, 4))   # phi-derefined polar rows
+    c["torus_deref_2"] = (d, lambda: I.fm_torus(d, seed=7), 2)
     return c
 
 
