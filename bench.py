@@ -554,7 +554,11 @@ def main():
         gh = g.h if gh is None else gh
         op = ops[0] if op is None else op
         with link_in:
-            rc = set_call(gh, hp, bp)
+            if refined:
+                rc = set_call(gh, hp, bp)
+            else:   # the link is released as soon as the input has left the host, not when the first flux pass is done
+                rc = L.hamr_set_prims_async(gh, hp, bp)
+                rc |= L.hamr_wait_input(gh)
         rc |= L.hamr_step(gh, 1, None, None)
         with link_out:
             rc |= get_call(gh, op)

@@ -102,6 +102,14 @@ int hamr_grid_destroy(hamr_grid* g);
  * Returns HAMR_ENONFINITE if the input contains NaN/Inf. */
 int hamr_set_prims(hamr_grid* g, const double* const hydro[5], const double* const bface[3]);
 int hamr_set_prims_dev(hamr_grid* g, const double* const hydro[5], const double* const bface[3]);
+/* hamr_set_prims with HOST arrays that does not wait: the eight host-to-device copies and the kernels behind them are
+ * enqueued on the grid's stream and the call returns.  The arrays should be page-locked (pinned; pageable memory makes
+ * every copy synchronous) and must stay UNCHANGED until hamr_wait_input has returned, which waits for the copies only
+ * (not for the kernels behind them): the host link is then free for another grid's input while this grid's first flux
+ * pass and step run.  NaN / Inf input is reported by the next full wait (hamr_sync, hamr_step: HAMR_ENONFINITE).  On a
+ * block-structured grid the call waits as hamr_set_prims does (the first time levels are assigned on the host). */
+int hamr_set_prims_async(hamr_grid* g, const double* const hydro[5], const double* const bface[3]);
+int hamr_wait_input(hamr_grid* g);
 
 /* ---- the hot path ---------------------------------------------------------------------------- */
 /* Advances nsteps full steps (predictor + corrector = one zone-cycle each): ghost

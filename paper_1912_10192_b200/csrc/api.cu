@@ -261,7 +261,13 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
     g->aux[0] = g->aux[1] = nullptr;
     cudaGetLastError();
   }
+  g->ev_input = nullptr;
+  if (cudaEventCreateWithFlags(&g->ev_input, cudaEventDisableTiming | cudaEventBlockingSync) != cudaSuccess) {
+    g->ev_input = nullptr;
+    cudaGetLastError();
+  }
   if ((e = cudaMallocHost((void**)&g->h_pinned, 64 * sizeof(double))) != cudaSuccess) {
+    if (g->ev_input) cudaEventDestroy(g->ev_input);
     destroy_aux(g);
     if (own) { cudaFree(g->arena); cudaStreamDestroy(g->stream); }
     delete g;
@@ -434,7 +440,9 @@ int step_once(hamr_grid* g) {
   return HAMR_OK;
 }
 
-int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* const bface[3], bool dev) {
+// dev: device pointers (no staging, no wait).  nowait (host pointers): the copies and kernels are enqueued and the call
+// returns; the caller's arrays must stay unchanged until hamr_wait_input (or any later wait on the stream) has returned
+int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* const bface[3], bool dev, bool nowait = false) {
   if (!g) return HAMR_EINVAL;
   if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
   if (!hydro) return fail(g, HAMR_EINVAL, "hydro is NULL");
@@ -448,31 +456,39 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
   }
   const Fields& sn = g->s[g->isn];
   const size_t nz = (size_t)N[0] * N[1] * N[2];
+  // host arrays: ALL copies first, then the pack kernels (a copy behind a kernel on the same stream would leave the
+  // host link idle while that kernel waits for SMs another grid is using)
+  const double* srcs[8];
+  size_t off = 5 * nz;
   for (int c = 0; c < 5; c++) {
-    const double* src = hydro[c];
+    srcs[c] = hydro[c];
     if (!dev) {
       double* st = g->stage + (size_t)c * nz;
       CK(cudaMemcpyAsync(st, hydro[c], nz * 8, cudaMemcpyHostToDevice, g->stream));
-      src = st;
+      srcs[c] = st;
     }
-    if (blk) blk_pack(g, src, c, -1, false);
-    else launch_pack(g, src, sn.P[c], -1, false);
   }
-  size_t off = 5 * nz;
   for (int d = 0; d < 3; d++) {
     int m[3] = {N[0], N[1], N[2]};
     m[d] += 1;
     const size_t nf = (size_t)m[0] * m[1] * m[2];
-    const double* src = (bface && bface[d]) ? bface[d] : nullptr;
-    if (src && !dev) {
+    srcs[5 + d] = (bface && bface[d]) ? bface[d] : nullptr;
+    if (srcs[5 + d] && !dev) {
       if (off + nf > g->stage_doubles) return fail(g, HAMR_ENOMEM, "staging buffer too small");
       double* st = g->stage + off;
-      CK(cudaMemcpyAsync(st, src, nf * 8, cudaMemcpyHostToDevice, g->stream));
-      src = st;
+      CK(cudaMemcpyAsync(st, srcs[5 + d], nf * 8, cudaMemcpyHostToDevice, g->stream));
+      srcs[5 + d] = st;
       off += nf;
     }
-    if (blk) blk_pack(g, src, 5 + d, d, d == 1);
-    else launch_pack(g, src, sn.Bf[d], d, d == 1);
+  }
+  if (nowait && g->ev_input) CK(cudaEventRecord(g->ev_input, g->stream));   // every input array has left the host
+  for (int c = 0; c < 5; c++) {
+    if (blk) blk_pack(g, srcs[c], c, -1, false);
+    else launch_pack(g, srcs[c], sn.P[c], -1, false);
+  }
+  for (int d = 0; d < 3; d++) {
+    if (blk) blk_pack(g, srcs[5 + d], 5 + d, d, d == 1);
+    else launch_pack(g, srcs[5 + d], sn.Bf[d], d, d == 1);
   }
   CK(cudaMemsetAsync(g->D.scal, 0, NSCAL * sizeof(double), g->stream));
   CK(cudaMemsetAsync(g->D.cnt, 0, NCNT * sizeof(unsigned long long), g->stream));
@@ -485,7 +501,7 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
     g->shard_committed = false;
     launch_check_finite(g, sn);
     CK(cudaGetLastError());
-    if (dev) return HAMR_OK;
+    if (dev || nowait) return HAMR_OK;
     return check_state(g);
   }
   if (blk) {
@@ -502,7 +518,7 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
   }
   g->have_state = true;
   CK(cudaGetLastError());
-  if (dev) return HAMR_OK;
+  if (dev || nowait) return HAMR_OK;
   return check_state(g);
 }
 
@@ -556,6 +572,7 @@ int hamr_grid_destroy(hamr_grid* g) {
   if (g->bh.h_ctop) cudaFreeHost(g->bh.h_ctop);
   if (g->bh.h_ints) cudaFreeHost(g->bh.h_ints);
   for (cudaEvent_t e : g->ev) cudaEventDestroy(e);
+  if (g->ev_input) cudaEventDestroy(g->ev_input);
   for (int c = 0; c < 2; c++)
     if (g->step_graph[c]) cudaGraphExecDestroy(g->step_graph[c]);
   for (int a = 0; a < 2; a++)
@@ -573,6 +590,17 @@ int hamr_set_prims(hamr_grid* g, const double* const hydro[5], const double* con
 }
 int hamr_set_prims_dev(hamr_grid* g, const double* const hydro[5], const double* const bface[3]) {
   return set_prims_common(g, hydro, bface, true);
+}
+
+int hamr_set_prims_async(hamr_grid* g, const double* const hydro[5], const double* const bface[3]) {
+  return set_prims_common(g, hydro, bface, false, true);
+}
+
+int hamr_wait_input(hamr_grid* g) {
+  if (!g) return HAMR_EINVAL;
+  if (!g->ev_input) { CK(cudaStreamSynchronize(g->stream)); return HAMR_OK; }
+  CK(cudaEventSynchronize(g->ev_input));
+  return HAMR_OK;
 }
 
 int hamr_step_async(hamr_grid* g, int nsteps) {
@@ -614,11 +642,15 @@ int hamr_get_prims(hamr_grid* g, double* const prims[8]) {
   if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
   const Fields& sn = g->s[g->isn];
   const size_t nz = (size_t)g->par.n[0] * g->par.n[1] * g->par.n[2];
+  // all unpack kernels first (into the staging area), then the eight copies back to back: the host link does not wait
+  // for a kernel between two copies
   for (int c = 0; c < 8; c++) {
     if (!prims[c]) continue;
-    int rc = get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], prims[c], -1, false, (size_t)c * nz, c);
+    int rc = get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], g->stage + (size_t)c * nz, -1, true, 0, c);
     if (rc != HAMR_OK) return rc;
   }
+  for (int c = 0; c < 8; c++)
+    if (prims[c]) CK(cudaMemcpyAsync(prims[c], g->stage + (size_t)c * nz, nz * 8, cudaMemcpyDeviceToHost, g->stream));
   CK(cudaStreamSynchronize(g->stream));
   return HAMR_OK;
 }

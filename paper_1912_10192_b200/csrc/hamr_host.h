@@ -163,6 +163,7 @@ struct hamr_grid {
   cudaStream_t stream;
   cudaStream_t aux[2];       // side streams of the fork / join around independent launches of a stage (flux.cu); NULL: none
   cudaEvent_t ev_fork, ev_join[2];
+  cudaEvent_t ev_input;      // recorded behind the last host-to-device copy of hamr_set_prims_async (hamr_wait_input); NULL: none
   bool cemf_done;            // launch_flux_on has issued the centre-EMF kernel of the coming launch_ct_on
   double* stage;             // device staging buffer for dense <-> padded transfers
   size_t stage_doubles;

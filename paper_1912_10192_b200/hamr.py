@@ -26,7 +26,7 @@ _STATUS = {0: "HAMR_OK", 1: "HAMR_EINVAL", 2: "HAMR_ENOMEM", 3: "HAMR_ECUDA", 4:
 
 # every symbol include/hamr.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "hamr_grid_destroy",
-           "hamr_set_prims", "hamr_set_prims_dev", "hamr_step", "hamr_step_async", "hamr_sync",
+           "hamr_set_prims", "hamr_set_prims_dev", "hamr_set_prims_async", "hamr_wait_input", "hamr_step", "hamr_step_async", "hamr_sync",
            "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
            "hamr_get_backup_count", "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
            "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
@@ -80,6 +80,8 @@ def lib():
         L.hamr_grid_destroy.argtypes = [vp]
         L.hamr_set_prims.argtypes = [vp, C.POINTER(c_double_p), C.POINTER(c_double_p)]
         L.hamr_set_prims_dev.argtypes = [vp, C.POINTER(c_double_p), C.POINTER(c_double_p)]
+        L.hamr_set_prims_async.argtypes = [vp, C.POINTER(c_double_p), C.POINTER(c_double_p)]
+        L.hamr_wait_input.argtypes = [vp]
         L.hamr_step.argtypes = [vp, C.c_int, c_double_p, c_double_p]
         L.hamr_step_async.argtypes = [vp, C.c_int]
         L.hamr_sync.argtypes = [vp]
@@ -241,6 +243,16 @@ class Grid:
             bp = (c_double_p * 3)(*[_dp(b) for b in bf])
             rc = self.L.hamr_set_prims(self.h, hp, bp)
         return rc
+
+    def set_prims_async(self, hydro, bface=None):
+        """hamr_set_prims_async: hydro / bface are C-contiguous float64 numpy arrays in PINNED memory that the caller
+        keeps alive and unchanged until wait_input() (or a later sync) has returned"""
+        hp = (c_double_p * 5)(*[_dp(h) for h in hydro])
+        bp = None if bface is None else (c_double_p * 3)(*[_dp(b) for b in bface])
+        return self.L.hamr_set_prims_async(self.h, hp, bp)
+
+    def wait_input(self):
+        self._ck(self.L.hamr_wait_input(self.h))
 
     def set_prims_dev(self, hydro, bface=None):
         """hydro / bface: torch CUDA float64 contiguous tensors (device pointers are passed through)."""

@@ -255,3 +255,31 @@ def test_cfg3_full_size_one_step(H, orc):
     assert max(e.values()) <= TOL_1, e
     sg, so = g.stats(), o.stats()
     assert g.divb() <= TOL_DIVB and sg[0] == so[0] == 0 and sg[3] == so[3]
+
+
+def test_set_prims_async_equals_set_prims(H):
+    """hamr_set_prims_async + hamr_wait_input (host arrays in pinned memory, no wait for the kernels behind the copies)
+    leaves the grid in the state hamr_set_prims does: same dt, same primitives after 3 steps, bit for bit; NaN input is
+    reported by the next full wait."""
+    import torch
+    p = I.torus_params()
+    hyd, bf = I.fm_torus(p, seed=0)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    hp, bp = [pin(h) for h in hyd], [pin(b) for b in bf]
+    a, b = H.Grid(p), H.Grid(p)
+    assert a.set_prims(hyd, bf) == 0
+    assert b.set_prims_async(hp, bp) == 0
+    b.wait_input()
+    for x in hp + bp:
+        x[...] = -7.0                      # the input has left the host: the arrays are the caller's again
+    assert a.dt == b.dt
+    a.step(3)
+    b.step(3)
+    assert all(np.array_equal(x, y) for x, y in zip(a.get_prims(), b.get_prims()))
+    hp2 = [pin(h) for h in hyd]
+    hp2[1][3, 4, 5] = np.nan
+    assert b.set_prims_async(hp2, None) == 0
+    b.wait_input()
+    assert H.lib().hamr_sync(b.h) == H.ENONFINITE
+    a.close()
+    b.close()
