@@ -40,7 +40,7 @@ __device__ __forceinline__ double lim_slope(double dl, double dr, double dc) {
 __device__ __forceinline__ double lim_slope2(double dl, double dr, double ds) {
   const double m = 4.0 * (fabs(dl) < fabs(dr) ? dl : dr);
   const double lim = fabs(ds) < fabs(m) ? ds : m;
-  return same_sign(dl, dr) ? copysign(lim, dl) : 0.0;
+  return same_sign(dl, dr) ? lim : 0.0;   // where dl and dr agree in sign, ds and m carry that sign already
 }
 
 // interface value a_{j+1/2} from a_j, d = a_{j+1} - a_j and TWICE the limited slopes of zones j and j+1
@@ -62,8 +62,15 @@ __device__ __forceinline__ void ppm_mono(double l, double a, double r, double& a
   // rounded to zero, so the sign is exact), read off the high word: one FP64 instruction per test instead of two
   const bool over = __double2hiint(fma(-2.0, fabs(dr), fabs(dl))) > 0;
   const bool under = __double2hiint(fma(-2.0, fabs(dl), fabs(dr))) > 0;
-  aL = flat ? a : (over ? a - 2.0 * dr : l);
-  aR = flat ? a : ((!over && under) ? a + 2.0 * dl : r);
+  // the resets as PREDICATED writes over l and r (one instruction each instead of the reset value plus two word selects)
+  aL = l;
+  aR = r;
+  asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %1, 0;\n\t@p fma.rn.f64 %0, %2, %3, %4;\n\t}"
+      : "+d"(aL) : "r"((int)over), "d"(-2.0), "d"(dr), "d"(a));
+  asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %1, 0;\n\t@p fma.rn.f64 %0, %2, %3, %4;\n\t}"
+      : "+d"(aR) : "r"((int)(!over && under)), "d"(2.0), "d"(dl), "d"(a));
+  asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %2, 0;\n\t@p mov.f64 %0, %3;\n\t@p mov.f64 %1, %3;\n\t}"
+      : "+d"(aL), "+d"(aR) : "r"((int)flat), "d"(a));
 }
 
 // parabola edges (aL at j-1/2, aR at j+1/2) of zone j from a0..a4 = a[j-2..j+2]
