@@ -155,16 +155,16 @@ ALG_RW = {"flux_x1": (9, 7), "flux_x2": (9, 7), "flux_x3": (9, 7),   # r: P5, 2 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel class and the FP64 thread
 # instructions (dadd + dmul + dfma) the flux kernels execute per face, from the round's `ncu --set full` capture of
 # this same command on cfg 2
-NCU_TRAFFIC_SOURCE = "profiles/r2b_ncu_full_cfg2.md"
-NCU_TRAFFIC = {"flux_x1": 539000000, "flux_x2": 523500000, "flux_x3": 497900000, "centre_emf": 295300000,
-               "edge_emf": 534800000, "update_predictor": 1462100000, "update_corrector": 1737200000, "ghosts": 15600000}
-FLUX_FP64_INST_PER_FACE = {"flux_x1": 330.7, "flux_x2": 326.9, "flux_x3": 317.7}
-FLUX_FMA_FRACTION = 0.41           # the DFMA share of those (2 FLOP each), the rest DADD / DMUL (1 FLOP)
+NCU_TRAFFIC_SOURCE = "profiles/r2d_ncu_full_cfg2.md"
+NCU_TRAFFIC = {"flux_x1": 539100000, "flux_x2": 523200000, "flux_x3": 497900000, "centre_emf": 295200000,
+               "edge_emf": 535100000, "update_predictor": 1462100000, "update_corrector": 1735700000, "ghosts": 15600000}
+FLUX_FP64_INST_PER_FACE = {"flux_x1": 324.7, "flux_x2": 321.2, "flux_x3": 313.7}
+FLUX_FMA_FRACTION = 0.445          # the DFMA share of those (2 FLOP each), the rest DADD / DMUL (1 FLOP)
 # every instruction the flux kernels send down the FP64 pipe per face (the arithmetic above plus the compares behind
 # min / max / limiter switches), from the same capture: sm__pipe_fp64_cycles_active x cycles / 2 cycles per warp
 # instruction x 592 schedulers x 32 threads / faces; and all warp-level instructions per face-warp
-FLUX_FP64PIPE_INST_PER_FACE = {"flux_x1": 380.0, "flux_x2": 376.0, "flux_x3": 388.0}
-FLUX_INST_PER_FACE = {"flux_x1": 812.0, "flux_x2": 817.0, "flux_x3": 701.0}
+FLUX_FP64PIPE_INST_PER_FACE = {"flux_x1": 355.0, "flux_x2": 352.0, "flux_x3": 343.0}
+FLUX_INST_PER_FACE = {"flux_x1": 777.0, "flux_x2": 786.0, "flux_x3": 679.0}
 FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
 PAPER_V100_150CUBED = 0.85e8   # ~0.85e8 zone-cycles/s, 1 V100, one 150^3 block
 
@@ -500,7 +500,7 @@ def main():
         fp64 = {"tflops_measured_dfma": 2.0 * ins0 / sec0 / 1e12, "ginstr_per_s_dfma": ins0 / sec0 / 1e9,
                 "ginstr_per_s_flux_mix": ins1 / sec1 / 1e9, "tflops_flux_mix": (4.0 / 3.0) * ins1 / sec1 / 1e12,
                 # FP64-pipe instruction rate when every 4 of them come with 5 select / integer instructions, as in
-                # the flux kernels (~380 : ~430 per face): what the machine sustains on THAT blend
+                # the flux kernels (~350 : ~420 per face): what the machine sustains on THAT blend
                 "ginstr_per_s_flux_blend": ins2 / sec2 / 1e9,
                 "tflops_derived": FP64_PEAK_TFLOPS_DERIVED,
                 "how": "hamr_bench_fp64: 8 independent chains per thread, 64 warps per SM, 96 x 20000 instructions per thread"}
@@ -657,7 +657,7 @@ def main():
                                                  for k in classes["flux"]},
                              "note": "FP64-pipe instruction rate of the flux kernels against the rate the same blend of "
                                      "FP64-pipe and other instructions sustains without dependencies (hamr_bench_fp64 "
-                                     "mix 2: 4 FP64-pipe to 5 select / integer instructions; the kernels: ~380 to ~430)"}
+                                     "mix 2: 4 FP64-pipe to 5 select / integer instructions; the kernels: ~350 to ~420)"}
     roof = {"bound": "hbm", "kernel": "+".join(dk), "achieved": dom_gbs, "peak": hbm_peak, "unit": "GB/s",
             "frac": dom_gbs / hbm_peak, "traffic": traffic, "traffic_source": NCU_TRAFFIC_SOURCE, "peak_source": peak_src,
             "share_of_step": cshare[dom], "class_shares": {c: round(v, 4) for c, v in cshare.items()},

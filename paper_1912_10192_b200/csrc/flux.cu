@@ -200,10 +200,10 @@ __device__ __forceinline__ double face_flux(const double* __restrict__ PL, const
   const double cmin = dmax(0.0, dmax(L.vm * iL, R.vm * iR));
   const double sum = cmax + cmin;
   const bool avg = sum < 1e-300;
-  const double isg = avg ? 0.0 : G.gdet * rcp_nr(sum);
+  const double isg = G.gdet * rcp_nr(sum);
   // F = g [cmax FL + cmin FR - cmax cmin (UR - UL)] / (cmax + cmin);  average if both speeds vanish
-  const double wl = avg ? 0.5 * G.gdet : cmax * isg;
-  const double wr = avg ? 0.5 * G.gdet : cmin * isg;
+  double wl = cmax * isg, wr = cmin * isg;
+  if (__builtin_expect(avg, 0)) wl = wr = 0.5 * G.gdet;   // (a branch no lane takes: no select on the common path)
   const double wc = wl * cmin;              // avg: cmin = 0
   const double XL = wl * L.ud + wc * L.ut, XR = wr * R.ud - wc * R.ut;
   double Fh0 = L.rho * XL + R.rho * XR;
