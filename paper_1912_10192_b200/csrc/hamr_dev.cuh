@@ -481,6 +481,10 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
                "l"(src), "r"(bytes), "r"(su32(b))
                : "memory");
 }
+// asks for [src, src + bytes) to be brought into L2 (no destination, no completion: a hint)
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
 // one lane of a converged warp
 __device__ __forceinline__ bool elect_one() {
   unsigned p;

@@ -232,6 +232,7 @@ constexpr int NA = 8, NB = 13;   // arrays keeping two planes / one plane
 // ROB: the robust path of k_update above (C-18 entropy row and backup inversion, C-19 drift-frame floors).  The three
 // entropy fluxes are not staged (a third CTA-plane set would halve the CTAs per SM): each zone reads its six values
 // directly, requested with the zone-centred inputs at the top of the step.
+constexpr bool PREFETCH_STATE = true;
 template <bool SAME, int NT, bool ROB = false>
 __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, double dtfac, int seg) {
   using namespace tile;
@@ -286,6 +287,24 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_update_tile(Dev Dv, Roles r, d
     const bool in0 = i < L.n[0];
     const bool zone = live && in0 && in1;
     const int z = (int)L.idx(i, j, k);
+    // corrector: the zone-centred inputs of the NEXT plane (two whole rows per array: one contiguous chunk) are asked into
+    // L2 now, so that the direct loads at the top of the next step, which its early state evaluation waits for, find them
+    // there: 0.374 -> 0.335 ms on cfg 2.  The predictor, which uses its inputs after the staged part, loses by it
+    // (0.276 -> 0.291 ms) and does without
+    if (PREFETCH_STATE && !SAME && warp0 && i + 1 < L.n[0] && i + 1 < i1 && elect_one()) {
+      const int zn = (int)L.idx(i + 1, j0, 0);
+      const unsigned pb = (unsigned)(2 * L.p3 * sizeof(double));
+#pragma unroll
+      for (int c = 0; c < 5; c++) bulk_prefetch_l2(r.src.P[c] + zn, pb);
+#pragma unroll
+      for (int c = 0; c < 3; c++) bulk_prefetch_l2(r.src.Bc[c] + zn, pb);
+      if (!SAME) {
+#pragma unroll
+        for (int c = 0; c < 5; c++) bulk_prefetch_l2(r.base.P[c] + zn, pb);
+#pragma unroll
+        for (int c = 0; c < 3; c++) bulk_prefetch_l2(r.base.Bc[c] + zn, pb);
+      }
+    }
     // zone-centred inputs without reuse: requested now, used after the staged part
     double Ps[8], Pb[8];
     if (zone) {
