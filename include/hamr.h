@@ -172,8 +172,10 @@ const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the 
  * parent (hydro: piecewise linear in x1 with the MC-limited slope; x1-faces: coincident ones copied, the new one the mean
  * of the parent zone's two; transverse faces: the parent's value), newly coarsened ones the restriction of their two
  * children (means; coincident x1-faces copied): every new zone has the divergence of the zone(s) it came from, so
- * div B stays at round-off.  Needs a block grid (nb) with an even nb[0], between steps, without phi-derefinement;
- * HAMR_EINVAL otherwise (also if r_refine_max does not give an admissible lattice). */
+ * div B stays at round-off.  On a phi-derefined grid the group structure of the polar rows (C-15) goes through the transfer
+ * (every member of a group sees the same arithmetic) and is imposed again on the new grid as after hamr_blocks_commit.
+ * Needs a block grid (nb) with an even nb[0], between steps; HAMR_EINVAL otherwise (also if r_refine_max does not give an
+ * admissible lattice). */
 int hamr_refine_radius(hamr_grid* g, double rho_cut, double* r_refine_max);
 int hamr_regrid(hamr_grid* g, double r_refine_max, hamr_grid** out);
 

@@ -165,10 +165,10 @@ int orc_refine_radius(void* h, double rho_cut, double* r_new) {
   return 0;
 }
 // C-20: a new grid with r_refine_max = r_new holding the state of h (which stays valid); NULL if the grid is not a
-// block grid between coarse steps, is phi-derefined, or the new lattice is not admissible
+// block grid between coarse steps or the new lattice is not admissible
 void* orc_regrid(void* h, double r_new) {
   Grid& go = *(Grid*)h;
-  if (!go.multi || !go.have_state || go.par.n_deref > 0) return nullptr;
+  if (!go.multi || !go.have_state) return nullptr;
   Params p = go.par;
   p.r_refine_max = r_new;
   Grid* gn = nullptr;

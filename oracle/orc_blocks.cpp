@@ -791,6 +791,10 @@ void blocks_regrid(Grid& go, Grid& gn) {
       }
     }
   }
+  // C-15: on a phi-derefined grid the transfer keeps the group structure (every member of a group goes through the same
+  // arithmetic on the same values) except for the last bit of the in-group x3-faces after a restriction (the mean of two
+  // interpolated values is not bitwise the interpolation of the means): the invariant is imposed as after set_prims
+  for (Block& b : gn.blocks) deref_project(gn.par, b, b.sn);
   gn.t = go.t;
   gn.have_state = true;
   blocks_initial_dt(gn);

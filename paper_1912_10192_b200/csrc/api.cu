@@ -860,7 +860,6 @@ int hamr_regrid(hamr_grid* g, double r_refine_max, hamr_grid** out) {
   if (out) *out = nullptr;
   if (!g || !out) return HAMR_EINVAL;
   if (!g->bh.on) return fail(g, HAMR_EINVAL, "regridding needs a block grid (nb)");
-  if (g->par.n_deref > 0) return fail(g, HAMR_EINVAL, "regridding is not available on a phi-derefined grid");
   if (!g->have_state || g->blocks_open) return fail(g, HAMR_ESTATE, "no committed state");
   if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
   hamr_params p = g->par;

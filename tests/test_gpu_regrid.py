@@ -1,6 +1,7 @@
 """GPU <-> oracle parity of the regridding of the x1 refinement level (the x1-only part;
 DESIGN.md C-20): the refinement criterion, the state transfer (copy / prolongation / restriction)
-block by block, and the steps that follow on the new lattice, with one global step and with LAT.  Needs a B200."""
+block by block, and the steps that follow on the new lattice, with one global step and with LAT, also on a grid with
+phi-derefined polar rows.  Needs a B200."""
 import numpy as np
 import pytest
 
@@ -126,11 +127,46 @@ def test_regrid_is_refused_where_it_does_not_apply(H):
     g = H.Grid(p)
     with pytest.raises(H.HamrError):          # no state yet
         g.regrid(4.0)
-    pd = I.torus_params(n=(32, 16, 16), nb=(8, 8, 16), deref_theta_deg=(15.0,), deref_factor=(2,))
-    gd = H.Grid(pd)
-    data = I.fm_torus_blocks(pd, [gd.block_info(b)[:3] for b in range(gd.num_blocks())], seed=4)
-    for b, (hy, bb) in enumerate(data):
-        assert gd.set_block_prims(b, hy, bb) == 0
-    assert gd.commit() == 0
-    with pytest.raises(H.HamrError):          # phi-derefined grid
-        gd.regrid(4.0)
+
+
+@pytest.mark.parametrize("lat,n3", [(0, 16), (1, 16), (1, 32)])
+def test_regrid_on_a_phi_derefined_grid(H, orc, lat, n3):
+    """cfg 4 carries derefined polar rows AND the x1 level: the regrid on such a grid (rows derefined by 4 / 2 / 2; blocks
+    that span x3, n3 = 16, or cut it in two, n3 = 32: phi-ghost zones in group units) against the oracle's: transferred
+    state, three steps on the refined lattice, back, two more steps"""
+    p = I.torus_params(n=(32, 16, n3), nb=(8, 4, 16), lat_max_level=lat, deref_theta_deg=(30.0, 12.0), deref_factor=(2, 4))
+    g, o = H.Grid(p), orc.OrcGrid(p)
+    _set_both(g, o, I.fm_torus_blocks(p, _infos(o), seed=4))
+    g.step(1)
+    o.step(1)
+    rg, ro = g.refine_radius(0.3), o.refine_radius(0.3)
+    assert ro > p["xmin"][0] and abs(rg - ro) <= 1e-12 * ro
+    g2, o2 = g.regrid(rg), o.regrid(ro)
+    assert g2.num_blocks() == o2.num_blocks() > g.num_blocks()
+    assert abs(g2.t - o2.t) <= 1e-13 * o2.t and abs(g2.dt - o2.dt) <= 1e-13 * o2.dt
+    if lat:
+        assert list(g2.levels()) == list(o2.levels())
+    p2 = dict(p, r_refine_max=ro)
+    print("after the transfer", _check_blocks(p2, o2, g2, TOL_1))
+    g2.step(3)
+    o2.step(3)
+    if lat:
+        assert list(g2.levels()) == list(o2.levels())
+    print("3 steps on the refined lattice", _check_blocks(p2, o2, g2, 4 * TOL_1 if not lat else TOL_10))
+    g3, o3 = g2.regrid(0.0), o2.regrid(0.0)
+    assert g3.num_blocks() == o3.num_blocks() == g.num_blocks()
+    _check_blocks(p, o3, g3, TOL_10)
+    g3.step(2)
+    o3.step(2)
+    print("coarse again + 2 steps", _check_blocks(p, o3, g3, TOL_10))
+    # the same-lattice regrid of a derefined grid is the identity, bit for bit, on what is evolved: hydro primitives and
+    # face field (the cell-centred field is rebuilt from the faces by the commit's division by 2 sqrt(-g), where the update
+    # kernel multiplies by the stored reciprocal: one ulp)
+    g4 = g3.regrid(0.0)
+    for b in range(g3.num_blocks()):
+        Pa, Pb = g3.get_block_prims(b), g4.get_block_prims(b)
+        assert all(np.array_equal(a, c) for a, c in zip(Pa[:5], Pb[:5]))
+        assert all(np.allclose(a, c, rtol=4e-16, atol=0) for a, c in zip(Pa[5:], Pb[5:]))
+        assert all(np.array_equal(a, c) for a, c in zip(g3.get_block_bface(b), g4.get_block_bface(b)))
+    for x in (g, g2, g3, g4):
+        x.close()

@@ -162,3 +162,48 @@ def test_r5_torus_runs_on_after_a_regrid(orc, lat):
     assert k.num_blocks() == g.num_blocks()
     k.step(1)
     assert k.stats()[0] == 0 and k.divb() <= 1e-12
+
+
+def _block_group_checks(g, mrow_global):
+    """the C-15 group structure of every block of a phi-derefined grid (blocks spanning x3): hydro exactly uniform in a
+    group, Bf1 / Bf2 uniform, Bf3 linear inside a group (to 1e-13 of the field)"""
+    from tests.test_oracle_deref import _group_checks
+    for b in range(g.num_blocks()):
+        d = g.block_info(b)
+        J0 = int(round(d["x_lo"][1] / d["dx"][1]))
+        n1 = d["n"][1]
+        _group_checks(g.get_block_prims(b), g.get_block_bface(b), mrow_global[J0:J0 + n1])
+
+
+@pytest.mark.parametrize("lat", [0, 1])
+def test_r6_regrid_on_a_phi_derefined_grid(orc, lat):
+    """C-20 with C-15 (cfg 4 carries both): the group structure of the derefined polar rows goes through copy, prolongation
+    and restriction; the same-lattice regrid stays the identity bit for bit; div B stays at round-off; the torus runs on"""
+    p = I.torus_params(n=(32, 16, 16), nb=(8, 4, 16), lat_max_level=lat, deref_theta_deg=(30.0, 12.0), deref_factor=(2, 4))
+    mrow = [4, 2, 2] + [1] * 10 + [2, 2, 4]
+    g = orc.OrcGrid(p)
+    data = I.fm_torus_blocks(p, _infos(g), seed=4)
+    for b, (hyd, bf) in enumerate(data):
+        assert g.set_block_prims(b, hyd, bf) == 0
+    assert g.commit() == 0
+    g.step(2)
+    _block_group_checks(g, mrow)
+    same = g.regrid(0.0)                                # same lattice: identity, bit for bit (the projection included)
+    for (Pa, Ba), (Pb, Bb) in zip(_state(g), _state(same)):
+        assert all(np.array_equal(a, b) for a, b in zip(Pa, Pb)) and all(np.array_equal(a, b) for a, b in zip(Ba, Bb))
+    r = g.refine_radius(0.3)
+    assert r > p["xmin"][0]
+    h = g.regrid(r)                                     # copy + prolongation
+    assert h.num_blocks() > g.num_blocks() and h.t == g.t and h.divb() <= 1e-12
+    _block_group_checks(h, mrow)
+    k = h.regrid(0.0)                                   # restriction: back on the first lattice
+    assert k.num_blocks() == g.num_blocks() and k.divb() <= 1e-12
+    _block_group_checks(k, mrow)
+    for (Pa, Ba), (Pb, Bb) in zip(_state(g), _state(k)):
+        for c in range(5):
+            assert np.allclose(Pa[c], Pb[c], rtol=4e-16, atol=1e-18)
+        for d in range(3):
+            assert np.array_equal(Ba[d], Bb[d])          # restriction inverts prolongation on the face field, bit for bit
+    h.step(2)
+    assert h.stats()[0] == 0 and h.divb() <= 1e-12
+    _block_group_checks(h, mrow)
