@@ -626,6 +626,10 @@ __global__ void __launch_bounds__(128, ENT ? 4 : X3_MINB) k_flux_x3(Dev Dv, Fiel
 // no ghost zone is read).  The left / right states of the row's n3 faces go through shared memory (14 doubles per
 // face), because the Riemann problems are then solved with lanes on CONSECUTIVE faces (coalesced stores).
 // A warp walks over a contiguous range of rows; each row's stencil lines are prefetched into L2 one row ahead.
+// Phase 2 (the row's Riemann problems, M per lane) is a ROLLED loop: unrolled by M = 4 the kernel is 2870 instructions
+// (46 KB) per row and waits for its own instructions (no_instruction 0.42 warps per issue); rolled it is 1820 and needs 156
+// registers.  Measured on cfg 2 (whole step, the three sweeps side by side): rolled 1.934 ms, by two 1.942, by four 1.963.
+constexpr int X3W_U = 1;
 template <int M, bool ENT = false>
 __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields s, int seg, int want_ctop) {
   constexpr int D = 2;
@@ -634,6 +638,7 @@ __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields 
   constexpr int NV = M * QS;                         // doubles per variable and side
   constexpr int NVR = ENT ? 8 : 7;                   // reconstructed variables (C-18: kappa is the eighth)
   __shared__ double lr[2 * NVR * NV];
+  __shared__ double sb[32 * M];                      // the normal field of the row's faces (phase 2 is a rolled loop)
   const Lay& L = Dv.L;
   const int lane = threadIdx.x;
   const int n3 = 32 * M, cj = L.n[1] + 2;
@@ -658,6 +663,8 @@ __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields 
     double bf3[M];
 #pragma unroll
     for (int q2 = 0; q2 < M; q2++) bf3[q2] = __ldg(s.Bf[2] + zr + lane + 32 * q2);
+#pragma unroll
+    for (int q2 = 0; q2 < M; q2++) sb[lane + 32 * q2] = bf3[q2];
     // ---- phase 1: parabolas of the lane's M zones, states of their low faces to shared memory ----
 #pragma unroll
     for (int v = 0; v < NVR; v++) {
@@ -692,7 +699,7 @@ __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields 
     __syncwarp();
     // ---- phase 2: Riemann problems, lanes on consecutive faces ----
     const bool act = i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1];
-#pragma unroll
+#pragma unroll X3W_U
     for (int q2 = 0; q2 < M; q2++) {
       const int f = lane + 32 * q2;                  // face = zone index
       const int sl = (f % M) * QS + f / M;
@@ -701,7 +708,7 @@ __global__ void __launch_bounds__(32, RING_WARPS) k_flux_x3_warp(Dev Dv, Fields 
       for (int v = 0; v < 7; v++) { PL[v] = lr[v * NV + sl]; PR[v] = lr[(NVR + v) * NV + sl]; }
       if (ENT) { PL[8] = lr[7 * NV + sl]; PR[8] = lr[(NVR + 7) * NV + sl]; }
       const int z = zr + f;
-      PL[7] = PR[7] = bf3[q2] * G.igdet;
+      PL[7] = PR[7] = sb[f] * G.igdet;
       double out[8];
       const double ct = face_flux<D, ENT>(PL, PR, G, Dv.gam, out);
       if (act) ctop = dmax(ctop, ct);
