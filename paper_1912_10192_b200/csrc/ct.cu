@@ -9,8 +9,10 @@ namespace hamr {
 
 // centre EMFs on active zones plus one ghost layer.  WRAP (x3_ghosts_unused): k runs over [0, n3) and the two x3
 // ghost columns are stored as the periodic images of columns n3 - 1 and 0 (their zones are not read)
+// 16 CTAs of 128 threads per SM (32 registers): 0.063 -> 0.058 ms on cfg 2 (it is bound by memory latency); the edge
+// kernel below gains nothing from the same cap (0.105 ms at 40 or 32 registers)
 template <bool BLK, bool WRAP>
-__global__ void __launch_bounds__(128) k_centre_emf(Dev Dv, Fields s0, Fields s2) {
+__global__ void __launch_bounds__(128, 16) k_centre_emf(Dev Dv, Fields s0, Fields s2) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + (WRAP ? 0 : 2), c1 = L.n[1] + 2;
   const unsigned per = (unsigned)(L.n[0] + 2) * c1 * c2;
