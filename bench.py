@@ -155,16 +155,16 @@ ALG_RW = {"flux_x1": (9, 7), "flux_x2": (9, 7), "flux_x3": (9, 7),   # r: P5, 2 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel class and the FP64 thread
 # instructions (dadd + dmul + dfma) the flux kernels execute per face, from the round's `ncu --set full` capture of
 # this same command on cfg 2
-NCU_TRAFFIC_SOURCE = "profiles/r2d_ncu_full_cfg2.md"
-NCU_TRAFFIC = {"flux_x1": 539100000, "flux_x2": 523200000, "flux_x3": 497900000, "centre_emf": 295200000,
-               "edge_emf": 535100000, "update_predictor": 1462100000, "update_corrector": 1735700000, "ghosts": 15600000}
+NCU_TRAFFIC_SOURCE = "profiles/r2e_ncu_full_cfg2.md"
+NCU_TRAFFIC = {"flux_x1": 539700000, "flux_x2": 523600000, "flux_x3": 499400000, "centre_emf": 294500000,
+               "edge_emf": 534800000, "update_predictor": 1459300000, "update_corrector": 1822900000, "ghosts": 15600000}
 FLUX_FP64_INST_PER_FACE = {"flux_x1": 324.7, "flux_x2": 321.2, "flux_x3": 313.7}
 FLUX_FMA_FRACTION = 0.445          # the DFMA share of those (2 FLOP each), the rest DADD / DMUL (1 FLOP)
 # every instruction the flux kernels send down the FP64 pipe per face (the arithmetic above plus the compares behind
 # min / max / limiter switches), from the same capture: sm__pipe_fp64_cycles_active x cycles / 2 cycles per warp
 # instruction x 592 schedulers x 32 threads / faces; and all warp-level instructions per face-warp
 FLUX_FP64PIPE_INST_PER_FACE = {"flux_x1": 355.0, "flux_x2": 352.0, "flux_x3": 343.0}
-FLUX_INST_PER_FACE = {"flux_x1": 777.0, "flux_x2": 786.0, "flux_x3": 679.0}
+FLUX_INST_PER_FACE = {"flux_x1": 777.0, "flux_x2": 786.0, "flux_x3": 709.0}
 FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
 PAPER_V100_150CUBED = 0.85e8   # ~0.85e8 zone-cycles/s, 1 V100, one 150^3 block
 
