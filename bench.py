@@ -559,7 +559,12 @@ def main():
             else:   # the link is released as soon as the input has left the host, not when the first flux pass is done
                 rc = L.hamr_set_prims_async(gh, hp, bp)
                 rc |= L.hamr_wait_input(gh)
-        rc |= L.hamr_step(gh, 1, None, None)
+        if refined:
+            rc |= L.hamr_step(gh, 1, None, None)
+        else:   # the outbound link is taken when the result is ready to leave (gathered into the staging area), not before
+            rc |= L.hamr_step_async(gh, 1)
+            rc |= L.hamr_stage_output(gh)
+            rc |= L.hamr_sync(gh)
         with link_out:
             rc |= get_call(gh, op)
         assert rc == 0, rc

@@ -109,7 +109,7 @@ int hamr_set_prims_dev(hamr_grid* g, const double* const hydro[5], const double*
  * pass and step run.  NaN / Inf input is reported by the next full wait (hamr_sync, hamr_step: HAMR_ENONFINITE).  On a
  * block-structured grid the call waits as hamr_set_prims does (the first time levels are assigned on the host). */
 int hamr_set_prims_async(hamr_grid* g, const double* const hydro[5], const double* const bface[3]);
-int hamr_wait_input(hamr_grid* g);
+int hamr_wait_input(hamr_grid* g);   /* spins on the event behind the last copy (no sleep: the wake-up would idle the link) */
 
 /* ---- the hot path ---------------------------------------------------------------------------- */
 /* Advances nsteps full steps (predictor + corrector = one zone-cycle each): ghost
@@ -126,6 +126,12 @@ int hamr_sync(hamr_grid* g); /* waits for the stream; reports HAMR_ENONFINITE / 
 
 /* ---- state out ------------------------------------------------------------------------------- */
 int hamr_get_prims(hamr_grid* g, double* const prims[8]); /* 5 hydro + cell-centred B^i */
+/* Enqueues, without waiting, the kernels that gather the eight dense arrays hamr_get_prims returns into the grid's staging
+ * area; a hamr_get_prims that follows (with no step, state change or other getter on the grid in between) then consists
+ * of its eight device-to-host copies only.  Lets a caller that shares the host link among several grids take the link
+ * when the data are ready to leave, not before (hamr_step_async, hamr_stage_output, hamr_sync, then hamr_get_prims).
+ * Not on grids with x1 refinement (HAMR_ESTATE: their state is read block by block). */
+int hamr_stage_output(hamr_grid* g);
 int hamr_get_prims_dev(hamr_grid* g, double* const prims[8]);
 int hamr_get_bface(hamr_grid* g, double* const bface[3]);
 /* max over zones of |div| / sum_d (|Bf+| + |Bf-|)/(2 dx^d), div = sum_d (Bf^d_+ - Bf^d_-)/dx^d;

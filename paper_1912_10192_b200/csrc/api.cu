@@ -221,6 +221,7 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   g->cemf_done = false;
   g->h_pinned = nullptr;
   g->have_state = false;
+  g->out_staged = false;
   g->blocks_open = false;
   g->dead = false;
   g->launches = 0;
@@ -262,7 +263,7 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
     cudaGetLastError();
   }
   g->ev_input = nullptr;
-  if (cudaEventCreateWithFlags(&g->ev_input, cudaEventDisableTiming | cudaEventBlockingSync) != cudaSuccess) {
+  if (cudaEventCreateWithFlags(&g->ev_input, cudaEventDisableTiming) != cudaSuccess) {
     g->ev_input = nullptr;
     cudaGetLastError();
   }
@@ -449,6 +450,7 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
   for (int c = 0; c < 5; c++) if (!hydro[c]) return fail(g, HAMR_EINVAL, "hydro[c] is NULL");
   const bool blk = g->bh.on;
   const int* N = g->par.n;
+  g->out_staged = false;
   if (blk && g->bh.refined) return fail(g, HAMR_ESTATE, "a grid with x1 refinement is set block by block (hamr_set_block_prims)");
   if (blk) {
     g->isn = 0; g->ish = 1; g->inew = 2;
@@ -463,7 +465,7 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
   for (int c = 0; c < 5; c++) {
     srcs[c] = hydro[c];
     if (!dev) {
-      double* st = g->stage + (size_t)c * nz;
+      double* st = stage_take(g) + (size_t)c * nz;
       CK(cudaMemcpyAsync(st, hydro[c], nz * 8, cudaMemcpyHostToDevice, g->stream));
       srcs[c] = st;
     }
@@ -475,7 +477,7 @@ int set_prims_common(hamr_grid* g, const double* const hydro[5], const double* c
     srcs[5 + d] = (bface && bface[d]) ? bface[d] : nullptr;
     if (srcs[5 + d] && !dev) {
       if (off + nf > g->stage_doubles) return fail(g, HAMR_ENOMEM, "staging buffer too small");
-      double* st = g->stage + off;
+      double* st = stage_take(g) + off;
       CK(cudaMemcpyAsync(st, srcs[5 + d], nf * 8, cudaMemcpyHostToDevice, g->stream));
       srcs[5 + d] = st;
       off += nf;
@@ -534,7 +536,7 @@ int get_dense(hamr_grid* g, const double* padded, double* out, int stag, bool de
     if (g->bh.on) blk_unpack(g, kind, out);
     else launch_unpack(g, padded, out, m);
   } else {
-    double* st = g->stage + stage_off;
+    double* st = stage_take(g) + stage_off;
     if (g->bh.on) blk_unpack(g, kind, st);
     else launch_unpack(g, padded, st, m);
     CK(cudaMemcpyAsync(out, st, nf * 8, cudaMemcpyDeviceToHost, g->stream));
@@ -605,6 +607,7 @@ int hamr_wait_input(hamr_grid* g) {
 
 int hamr_step_async(hamr_grid* g, int nsteps) {
   if (!g || nsteps < 0) return HAMR_EINVAL;
+  g->out_staged = false;
   if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
   if (g->sharded) return fail(g, HAMR_ESTATE, "an x1 slab steps through hamr_shard_stage (its neighbours must keep pace)");
   if (!g->have_state) return fail(g, HAMR_ESTATE, "hamr_step before hamr_set_prims");
@@ -643,15 +646,33 @@ int hamr_get_prims(hamr_grid* g, double* const prims[8]) {
   const Fields& sn = g->s[g->isn];
   const size_t nz = (size_t)g->par.n[0] * g->par.n[1] * g->par.n[2];
   // all unpack kernels first (into the staging area), then the eight copies back to back: the host link does not wait
-  // for a kernel between two copies
-  for (int c = 0; c < 8; c++) {
-    if (!prims[c]) continue;
-    int rc = get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], g->stage + (size_t)c * nz, -1, true, 0, c);
-    if (rc != HAMR_OK) return rc;
+  // for a kernel between two copies.  After hamr_stage_output the unpacked arrays are there already
+  if (!g->out_staged) {
+    double* st = stage_take(g);
+    for (int c = 0; c < 8; c++) {
+      if (!prims[c]) continue;
+      int rc = get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], st + (size_t)c * nz, -1, true, 0, c);
+      if (rc != HAMR_OK) return rc;
+    }
   }
   for (int c = 0; c < 8; c++)
     if (prims[c]) CK(cudaMemcpyAsync(prims[c], g->stage + (size_t)c * nz, nz * 8, cudaMemcpyDeviceToHost, g->stream));
   CK(cudaStreamSynchronize(g->stream));
+  return HAMR_OK;
+}
+
+int hamr_stage_output(hamr_grid* g) {
+  if (!g) return HAMR_EINVAL;
+  if (!g->have_state) return fail(g, HAMR_ESTATE, "no state");
+  const Fields& sn = g->s[g->isn];
+  const size_t nz = (size_t)g->par.n[0] * g->par.n[1] * g->par.n[2];
+  double* st = stage_take(g);
+  for (int c = 0; c < 8; c++) {
+    int rc = get_dense(g, c < 5 ? sn.P[c] : sn.Bc[c - 5], st + (size_t)c * nz, -1, true, 0, c);
+    if (rc != HAMR_OK) return rc;
+  }
+  CK(cudaGetLastError());
+  g->out_staged = true;
   return HAMR_OK;
 }
 
@@ -760,7 +781,7 @@ int hamr_set_block_prims(hamr_grid* g, int b, const double* const hydro[5], cons
   const size_t nz = (size_t)L.n[0] * L.n[1] * L.n[2];
   size_t off = (size_t)b * 8 * (L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1);   // the block's own staging slot
   for (int c = 0; c < 5; c++) {
-    double* st = g->stage + off;
+    double* st = stage_take(g) + off;
     CK(cudaMemcpyAsync(st, hydro[c], nz * 8, cudaMemcpyHostToDevice, g->stream));
     blk_pack_one(g, b, st, c, -1, false);
     off += nz;
@@ -771,7 +792,7 @@ int hamr_set_block_prims(hamr_grid* g, int b, const double* const hydro[5], cons
     const size_t nf = (size_t)m[0] * m[1] * m[2];
     const double* src = (bface && bface[d]) ? bface[d] : nullptr;
     if (src) {
-      double* st = g->stage + off;
+      double* st = stage_take(g) + off;
       CK(cudaMemcpyAsync(st, src, nf * 8, cudaMemcpyHostToDevice, g->stream));
       src = st;
       off += nf;
@@ -795,7 +816,7 @@ int hamr_set_all_blocks(hamr_grid* g, const double* const hydro[5], const double
   const size_t nz = (size_t)L.n[0] * L.n[1] * L.n[2] * nb;
   size_t off = 0;
   for (int c = 0; c < 5; c++) {
-    double* st = g->stage + off;
+    double* st = stage_take(g) + off;
     CK(cudaMemcpyAsync(st, hydro[c], nz * 8, cudaMemcpyHostToDevice, g->stream));
     blk_pack_one(g, -1, st, c, -1, false);
     off += nz;
@@ -806,7 +827,7 @@ int hamr_set_all_blocks(hamr_grid* g, const double* const hydro[5], const double
     const size_t nf = (size_t)m[0] * m[1] * m[2] * nb;
     const double* src = (bface && bface[d]) ? bface[d] : nullptr;
     if (src) {
-      double* st = g->stage + off;
+      double* st = stage_take(g) + off;
       CK(cudaMemcpyAsync(st, src, nf * 8, cudaMemcpyHostToDevice, g->stream));
       src = st;
       off += nf;
@@ -824,7 +845,7 @@ int hamr_get_all_blocks(hamr_grid* g, double* const prims[8]) {
   const size_t nz = (size_t)L.n[0] * L.n[1] * L.n[2] * g->bh.nblk;
   for (int c = 0; c < 8; c++) {
     if (!prims[c]) continue;
-    double* st = g->stage + (size_t)c * nz;
+    double* st = stage_take(g) + (size_t)c * nz;
     blk_unpack_one(g, -1, c, st);
     CK(cudaMemcpyAsync(prims[c], st, nz * 8, cudaMemcpyDeviceToHost, g->stream));
   }
@@ -834,6 +855,7 @@ int hamr_get_all_blocks(hamr_grid* g, double* const prims[8]) {
 
 int hamr_blocks_commit(hamr_grid* g) {
   if (!g || !g->bh.on) return HAMR_EINVAL;
+  g->out_staged = false;
   if (!g->blocks_open) return fail(g, HAMR_ESTATE, "hamr_blocks_commit without hamr_set_block_prims");
   g->blocks_open = false;
   g->isn = 0; g->ish = 1; g->inew = 2;
@@ -900,7 +922,7 @@ static int get_block(hamr_grid* g, int b, int kind0, int nkind, double* const ou
     int m[3] = {L.n[0], L.n[1], L.n[2]};
     if (stag >= 0) m[stag] += 1;
     const size_t nf = (size_t)m[0] * m[1] * m[2];
-    double* st = g->stage + off;
+    double* st = stage_take(g) + off;
     blk_unpack_one(g, b, kind, st);
     CK(cudaMemcpyAsync(out[c], st, nf * 8, cudaMemcpyDeviceToHost, g->stream));
     off += nf;
@@ -988,6 +1010,7 @@ int hamr_shard_stage(hamr_grid* g, int stage) {
   if (g->dead) return fail(g, HAMR_ESTATE, "grid unusable after a non-finite state");
   if (!g->shard_committed) return fail(g, HAMR_ESTATE, "hamr_shard_stage before hamr_shard_commit");
   if (g->shard_stage != stage) return fail(g, HAMR_ESTATE, "stages out of order: commit, ctop get / set, stage 0, stage 1, ctop get / set, ...");
+  g->out_staged = false;
   const Fields& sn = g->s[g->isn];
   const Fields& sh = g->s[g->ish];
   const Fields& sw = g->s[g->inew];
@@ -1089,8 +1112,9 @@ int hamr_get_edge(hamr_grid* g, int f, double* out) {
   const Lay& L = g->D.L;
   int m[3] = {L.n[0] + 1, L.n[1] + 1, L.n[2] + 1};
   m[f] -= 1;
-  launch_unpack(g, g->D.Ee[f], g->stage, m);
-  CK(cudaMemcpyAsync(out, g->stage, (size_t)m[0] * m[1] * m[2] * 8, cudaMemcpyDeviceToHost, g->stream));
+  double* st = stage_take(g);
+  launch_unpack(g, g->D.Ee[f], st, m);
+  CK(cudaMemcpyAsync(out, st, (size_t)m[0] * m[1] * m[2] * 8, cudaMemcpyDeviceToHost, g->stream));
   CK(cudaStreamSynchronize(g->stream));
   return HAMR_OK;
 }

@@ -1650,7 +1650,7 @@ int blk_refine_radius(hamr_grid* g, double rho_cut, double* r_new) {
   if (g->stage_doubles < (size_t)H.nblk) return HAMR_ENOMEM;
   {
     Launch l_(g, K_OTHER);
-    k_blk_max_rho<<<H.nblk, 256, 0, g->stream>>>(g->D, bufs_of(g), g->stage);
+    k_blk_max_rho<<<H.nblk, 256, 0, g->stream>>>(g->D, bufs_of(g), stage_take(g));
   }
   // h_ctop is pinned, [nblk][3] doubles, idle between steps
   if (cudaMemcpyAsync(H.h_ctop, g->stage, (size_t)H.nblk * 8, cudaMemcpyDeviceToHost, g->stream) != cudaSuccess) return HAMR_ECUDA;

@@ -169,6 +169,7 @@ struct hamr_grid {
   size_t stage_doubles;
   double* h_pinned;          // small pinned host buffer for scalar read-back
   bool have_state, dead;
+  bool out_staged;           // the staging area holds the dense primitives of the current state (hamr_stage_output)
   bool blocks_open;          // hamr_set_block_prims calls are being collected; hamr_blocks_commit closes
   long long launches;
   std::string err;
@@ -193,6 +194,8 @@ struct hamr_grid {
 };
 
 namespace hamr {
+// the staging area for a new use: whatever hamr_stage_output left there is gone
+inline double* stage_take(hamr_grid* g) { g->out_staged = false; return g->stage; }
 // brackets one kernel launch with an event pair when profiling is on; always counts the launch
 struct Launch {
   hamr_grid* g;

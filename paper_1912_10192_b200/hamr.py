@@ -26,7 +26,7 @@ _STATUS = {0: "HAMR_OK", 1: "HAMR_EINVAL", 2: "HAMR_ENOMEM", 3: "HAMR_ECUDA", 4:
 
 # every symbol include/hamr.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ["hamr_grid_create", "hamr_workspace_bytes", "hamr_grid_create_in", "hamr_grid_destroy",
-           "hamr_set_prims", "hamr_set_prims_dev", "hamr_set_prims_async", "hamr_wait_input", "hamr_step", "hamr_step_async", "hamr_sync",
+           "hamr_set_prims", "hamr_set_prims_dev", "hamr_set_prims_async", "hamr_wait_input", "hamr_stage_output", "hamr_step", "hamr_step_async", "hamr_sync",
            "hamr_get_prims", "hamr_get_prims_dev", "hamr_get_bface", "hamr_divb", "hamr_get_stats",
            "hamr_get_backup_count", "hamr_get_time", "hamr_set_dt", "hamr_last_error", "hamr_num_blocks", "hamr_block_info",
            "hamr_set_block_prims", "hamr_blocks_commit", "hamr_get_block_prims",
@@ -82,6 +82,7 @@ def lib():
         L.hamr_set_prims_dev.argtypes = [vp, C.POINTER(c_double_p), C.POINTER(c_double_p)]
         L.hamr_set_prims_async.argtypes = [vp, C.POINTER(c_double_p), C.POINTER(c_double_p)]
         L.hamr_wait_input.argtypes = [vp]
+        L.hamr_stage_output.argtypes = [vp]
         L.hamr_step.argtypes = [vp, C.c_int, c_double_p, c_double_p]
         L.hamr_step_async.argtypes = [vp, C.c_int]
         L.hamr_sync.argtypes = [vp]
@@ -250,6 +251,10 @@ class Grid:
         hp = (c_double_p * 5)(*[_dp(h) for h in hydro])
         bp = None if bface is None else (c_double_p * 3)(*[_dp(b) for b in bface])
         return self.L.hamr_set_prims_async(self.h, hp, bp)
+
+    def stage_output(self):
+        """hamr_stage_output: the next get_prims() is its eight copies only"""
+        self._ck(self.L.hamr_stage_output(self.h))
 
     def wait_input(self):
         self._ck(self.L.hamr_wait_input(self.h))

@@ -283,3 +283,31 @@ def test_set_prims_async_equals_set_prims(H):
     assert H.lib().hamr_sync(b.h) == H.ENONFINITE
     a.close()
     b.close()
+
+
+def test_stage_output_then_get_prims_equals_get_prims(H):
+    """hamr_stage_output gathers the dense output into the staging area ahead of hamr_get_prims: same arrays, bit for bit;
+    a step, a new state or another getter in between makes the next hamr_get_prims gather again"""
+    p = I.torus_params()
+    hyd, bf = I.fm_torus(p, seed=0)
+    a, b = H.Grid(p), H.Grid(p)
+    assert a.set_prims(hyd, bf) == 0 and b.set_prims(hyd, bf) == 0
+    a.step(2)
+    b.step_async(2)
+    b.stage_output()
+    b.sync()
+    assert all(np.array_equal(x, y) for x, y in zip(a.get_prims(), b.get_prims()))
+    b.stage_output()
+    b.get_bface()                        # another getter takes the staging area
+    assert all(np.array_equal(x, y) for x, y in zip(a.get_prims(), b.get_prims()))
+    b.stage_output()
+    a.step(1)
+    b.step(1)                            # the staged arrays are stale now
+    assert all(np.array_equal(x, y) for x, y in zip(a.get_prims(), b.get_prims()))
+    b.stage_output()
+    assert b.set_prims(hyd, bf) == 0     # ... and after a new state
+    assert all(np.array_equal(x, y) for x, y in zip(hyd, b.get_prims()[:5]))
+    r = H.Grid(I.torus_params(n=(32, 16, 16), nb=(8, 8, 8), r_refine_max=4.0))
+    assert H.lib().hamr_stage_output(r.h) == H.ESTATE
+    for g in (a, b, r):
+        g.close()
