@@ -231,3 +231,19 @@ def test_two_processes_with_ipc_neighbour_arenas_reproduce_the_one_grid_run(H, S
         for d in (1, 2):
             assert np.array_equal(z[f"B{d}"], B[d][lo:lo + n1])
     one.close()
+
+
+def test_bench_shard_line():
+    """`bench.py --shard 2` (the slab arm of the bench) prints one JSON line with the slab and the one-grid step"""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--shard", "2", "--workload", "cfg0", "--steps", "5"],
+                       capture_output=True, text=True, timeout=600, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = json.loads(r.stdout.strip().split("\n")[-1])
+    assert line["metric"] == "zone_cycles_per_sec" and line["scaling"] == "strong" and line["value"] > 0
+    assert line["config"]["slabs"] == [[0, 16], [16, 16]] and line["gpu_launches"] > 0
+    assert line["divb"] <= TOL_DIVB and line["one_grid"]["ms_per_step"] > 0
