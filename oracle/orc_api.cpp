@@ -27,10 +27,11 @@ static bool params_ok(const Params& p, std::string& why) {
     }
   }
   if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0)) { why = "gamma_ad/cour"; return false; }
-  if (p.entropy_backup || p.drift_floors) {  // C-18, C-19: built for the single-block grid
+  if (p.entropy_backup || p.drift_floors) {  // C-18, C-19: one block, or blocks that step together on one lattice level
     if ((p.entropy_backup & ~1) || (p.drift_floors & ~1)) { why = "entropy_backup / drift_floors are 0 or 1"; return false; }
-    if (p.nb[0] > 0 || p.nb[1] > 0 || p.nb[2] > 0 || p.n_deref > 0 || p.lat_max_level > 0 || p.r_refine_max > 0.0) {
-      why = "entropy_backup / drift_floors need a grid of one block without derefinement";
+    // (LAT's flux registers and correction, the refinement interface and the derefinement fix-ups do not carry the ninth row)
+    if (p.n_deref > 0 || p.lat_max_level > 0 || p.r_refine_max > 0.0) {
+      why = "entropy_backup / drift_floors need a grid without derefinement, refinement and LAT";
       return false;
     }
     if (p.entropy_backup && !(p.gamma_ad < 2.0)) { why = "the entropy inversion needs gamma_ad < 2"; return false; }

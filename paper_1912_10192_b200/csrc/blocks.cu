@@ -1325,6 +1325,7 @@ static void blk_stage(hamr_grid* g, int tau, bool corrector) {
     const Fields& s0 = g->s[0];
     const Fields& s1 = g->s[1];
     const Fields& s2 = g->s[2];
+    if (D.entropy) launch_kappa(g, D, corrector ? s1 : s0, corrector ? s1 : s2);   // C-18 (no LAT: every block is in this launch)
     launch_flux_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2, corrector, true);
     launch_ct_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2);
     launch_deref_fix_edges(g, D);
@@ -1512,6 +1513,7 @@ int blk_initial(hamr_grid* g) {
   launch_deref_project(g, D, g->s[0], g->s[2]);
   launch_deref_sync(g, D, g->s[0], g->s[2]);
   blk_ghosts(g, D, 0, 0, true, true);
+  if (D.entropy) launch_kappa(g, D, g->s[0], g->s[2]);
   launch_flux_on(g, D, g->s[0], g->s[2], true);
   return blk_assign(g, false);
 }

@@ -933,9 +933,11 @@ static void launch_march(hamr_grid* g, const Dev& Dv, const Fields& src, const F
   const bool ppm = Dv.recon == HAMR_RECON_PPM, blk = Dv.B.nblk > 0;
   if (ring_width(Dv) == 32)
     return Dv.entropy ? launch_ring_t<D, 32, true>(g, Dv, src, want_ctop) : launch_ring_t<D, 32, false>(g, Dv, src, want_ctop);
-  if (Dv.entropy) {   // C-18 (monolithic grids only: checked at creation)
-    if (ppm) launch_march_t<D, HAMR_RECON_PPM, false, true>(g, Dv, src, src2, want_ctop);
-    else launch_march_t<D, HAMR_RECON_PLM_MC, false, true>(g, Dv, src, src2, want_ctop);
+  if (Dv.entropy) {   // C-18
+    if (ppm && !blk) launch_march_t<D, HAMR_RECON_PPM, false, true>(g, Dv, src, src2, want_ctop);
+    else if (ppm) launch_march_t<D, HAMR_RECON_PPM, true, true>(g, Dv, src, src2, want_ctop);
+    else if (!blk) launch_march_t<D, HAMR_RECON_PLM_MC, false, true>(g, Dv, src, src2, want_ctop);
+    else launch_march_t<D, HAMR_RECON_PLM_MC, true, true>(g, Dv, src, src2, want_ctop);
     return;
   }
   if (ppm && !blk) launch_march_t<D, HAMR_RECON_PPM, false>(g, Dv, src, src2, want_ctop);
@@ -964,7 +966,9 @@ static void launch_x3(hamr_grid* g, const Dev& Dv, const Fields& src, const Fiel
       case -4: launch_x3_warp_t<4, true>(g, Dv, src, want_ctop); return;
       default: break;
     }
-    if (Dv.entropy && x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    if (Dv.entropy && blk && ppm) k_flux_x3<HAMR_RECON_PPM, true, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (Dv.entropy && blk) k_flux_x3<HAMR_RECON_PLM_MC, true, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (Dv.entropy && x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (Dv.entropy && ppm) k_flux_x3<HAMR_RECON_PPM, false, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (Dv.entropy) k_flux_x3<HAMR_RECON_PLM_MC, false, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
     else if (x3wrap) k_flux_x3<HAMR_RECON_PPM, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
@@ -1021,7 +1025,7 @@ void launch_flux_on(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields
 }
 
 void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop, bool with_cemf) {
-  if (g->D.entropy) launch_kappa(g, src);   // C-18: kappa of the (ghost-filled) source state for the entropy flux
+  if (g->D.entropy) launch_kappa(g, g->D, src, src);   // C-18: kappa of the (ghost-filled) source state for the entropy flux
   launch_flux_on(g, g->D, src, src, want_ctop, with_cemf);
 }
 

@@ -228,7 +228,7 @@ namespace hamr {
 void launch_ghosts(hamr_grid* g, const Fields& s, bool bc_active_too);
 void launch_flux(hamr_grid* g, const Fields& src, bool want_ctop, bool with_cemf = false);
 void launch_ct(hamr_grid* g, const Fields& src);
-void launch_kappa(hamr_grid* g, const Fields& src);   // misc.cu: C-18, fills Dv.K from the source state (after its ghost fill)
+void launch_kappa(hamr_grid* g, const Dev& Dv, const Fields& src, const Fields& src2);   // misc.cu: C-18, fills Dv.K from the source state (after its ghost fill)
 bool x3_ghosts_unused(const Dev& Dv);   // flux.cu: the stage kernels of this grid never read x3 ghost zones
 void launch_update(hamr_grid* g, const Fields& src, const Fields& base, const Fields& out, double dtfac,
                    bool src_is_base);

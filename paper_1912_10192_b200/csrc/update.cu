@@ -527,7 +527,7 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
   const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * L.n[2] * (blk ? Dv.B.nact : 1);
   const unsigned nb = (unsigned)((tot + 127) / 128);
   Launch l_(g, same ? K_UPDATE_P : K_UPDATE_C);
-  const bool rob = Dv.entropy || Dv.drift;   // NEXT-2 (monolithic grids only: checked at creation)
+  const bool rob = Dv.entropy || Dv.drift;   // NEXT-2
   if (rob) {
     switch (tile_threads(Dv)) {
       case 64: return same ? launch_tile_t<true, 64, true>(g, Dv, ra, dtfac) : launch_tile_t<false, 64, true>(g, Dv, ra, dtfac);
@@ -536,8 +536,10 @@ void launch_update_on(hamr_grid* g, const Dev& Dv, const Roles& ra, const Roles&
       case 512: return same ? launch_tile_t<true, 512, true>(g, Dv, ra, dtfac) : launch_tile_t<false, 512, true>(g, Dv, ra, dtfac);
       default: break;
     }
-    if (same) k_update<true, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
-    else k_update<false, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+    if (same && !blk) k_update<true, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+    else if (same) k_update<true, true, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+    else if (!blk) k_update<false, false, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
+    else k_update<false, true, true><<<nb, 128, 0, g->stream>>>(Dv, ra, rb, dtfac);
     return;
   }
   switch (tile_threads(Dv)) {

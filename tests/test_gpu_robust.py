@@ -360,3 +360,43 @@ def test_blast_step_takes_the_whole_inversion_chain(H, orc):
         e = parity_errors(p, o.get_prims(), g.get_prims())
         assert max(e.values()) <= 1e-10, e
     assert seen[0] > 0 and seen[1] > 0 and seen[2] > 0, seen
+
+
+@pytest.mark.parametrize("case", ["funnel", "torus"])
+def test_robust_path_on_a_block_grid(H, orc, case):
+    """the entropy row, the backup inversion and the drift-frame floors on a grid cut into blocks that step together (no
+    LAT: its registers and correction do not carry the ninth row): the generic block kernels with the ninth row against
+    the oracle, whose block-decomposed robust run equals its one-block run bit for bit (tests/test_oracle_entropy_drift.py)"""
+    if case == "funnel":
+        p = I.minkowski_params(n=(24, 16, 32), nb=(8, 8, 16), cour=0.5, rho_fl_coef=1e-9, u_fl_coef=1e-13, entropy_backup=1,
+                               drift_floors=1)
+        hyd, bf = _funnel(p)
+        steps, tols = 3, (1e-10, 1e-8, 1e-7)
+    else:
+        p = I.torus_params(n=(32, 16, 16), nb=(8, 8, 8), entropy_backup=1, drift_floors=1)
+        hyd, bf = I.fm_torus(p, seed=0)
+        steps, tols = 3, (1e-10, 4e-10, 1e-9)
+    g, o = _pair(H, orc, p, hyd, bf)
+    assert g.num_blocks() == o.num_blocks() > 1
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt
+    tot = 0
+    for step in range(steps):
+        g.step(1)
+        o.step(1)
+        Pg, Po = g.get_prims(), o.get_prims()
+        e = parity_errors(p, Po, Pg)
+        if case == "funnel":
+            e["u"] = _u_error(Po, Pg)
+        sg, so, bg, bo = g.stats(), o.stats(), g.backup_count(), o.backup_count()
+        print(f"{case} on blocks, step {step + 1}: {e} stats {sg} {so} entropy inversions {bg} {bo}")
+        assert max(e.values()) <= tols[step], (step, e)
+        assert sg[0] == so[0] == 0 and sg[3] == so[3]
+        if case == "funnel":
+            assert sg == so and bg == bo
+        else:       # at the floors a last-bit difference decides whether a zone counts (see test_gpu_parity)
+            assert abs(bg - bo) <= max(3, bo // 50)
+        tot += bo
+    assert tot > (np.prod(p["n"]) // 2 if case == "funnel" else 100)
+    assert g.divb() <= 1e-12
+    for a, b in zip(o.get_bface(), g.get_bface()):
+        assert rel_max(a, b) <= 1e-7

@@ -348,3 +348,22 @@ def test_d1_ceiling_follows_the_drift_floors(orc):
     Pn, c = orc.floors(p, G, 1.0, P, [1.0, 0.0, 0.0])
     assert c == (1, 1, 1) and np.isclose(np.sqrt(1 + Pn[2:5] @ Pn[2:5]), 5.0, rtol=1e-14)
     assert Pn[2] == 0.0 and Pn[4] == 0.0
+
+
+def test_robust_path_block_decomposition_is_the_one_block_run(orc):
+    """C-18 / C-19 on a grid cut into blocks that step together: the ninth row lives per block (kappa of the ghost-filled
+    source state, entropy flux on the block's own faces), so the decomposition changes nothing: every primitive bit for
+    bit, the same event counters and the same number of entropy inversions (the robust analogue of pin P15)"""
+    import numpy as np
+    from paper_1912_10192_b200 import inputs as I
+    for p, gen in ((dict(I.torus_params(n=(32, 16, 16)), entropy_backup=1, drift_floors=1), lambda q: I.fm_torus(q, seed=0)),):
+        hyd, bf = gen(p)
+        m = orc.OrcGrid(p)
+        b = orc.OrcGrid(dict(p, nb=(8, 8, 8)))
+        assert m.set_prims(hyd, bf) == 0 and b.set_prims(hyd, bf) == 0
+        m.step(3)
+        b.step(3)
+        assert b.num_blocks() == 16
+        assert all(np.array_equal(x, y) for x, y in zip(m.get_prims(), b.get_prims()))
+        assert m.stats() == b.stats() and m.backup_count() == b.backup_count() > 100
+        assert b.divb() <= 1e-12
