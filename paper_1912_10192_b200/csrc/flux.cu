@@ -754,9 +754,10 @@ static int ring_width(const Dev& Dv);
 static int x3_warp_m(const Dev& Dv) {
   if (ring_width(Dv) == 0) return 0;
   const int n3 = Dv.L.n[2];
-  // n3 = 256 (M = 8) needs 30 KB of shared memory per warp (7 resident warps per SM): measured slower than the
-  // shuffle kernel on cfg 3 (1.86 vs 1.66 ms)
-  return (n3 == 32 || n3 == 64 || n3 == 128) ? n3 / 32 : 0;
+  // n3 = 256 (M = 8) needs 32 KB of shared memory per warp (7 resident warps per SM).  With the Riemann problems unrolled it
+  // lost to the shuffle kernel on cfg 3 (1.86 vs 1.66 ms); rolled (156 registers) it wins: cfg 3 step 15.37 -> 14.87 ms.
+  // With the entropy row (36 KB per warp) the shuffle kernel stays
+  return (n3 == 32 || n3 == 64 || n3 == 128 || (n3 == 256 && !Dv.entropy)) ? n3 / 32 : 0;
 }
 
 // ---- C-15 (ii): x3-faces of phi-derefined rows -----------------------------------------------------------
@@ -961,6 +962,7 @@ static void launch_x3(hamr_grid* g, const Dev& Dv, const Fields& src, const Fiel
       case 1: launch_x3_warp_t<1>(g, Dv, src, want_ctop); return;
       case 2: launch_x3_warp_t<2>(g, Dv, src, want_ctop); return;
       case 4: launch_x3_warp_t<4>(g, Dv, src, want_ctop); return;
+      case 8: launch_x3_warp_t<8>(g, Dv, src, want_ctop); return;
       case -1: launch_x3_warp_t<1, true>(g, Dv, src, want_ctop); return;
       case -2: launch_x3_warp_t<2, true>(g, Dv, src, want_ctop); return;
       case -4: launch_x3_warp_t<4, true>(g, Dv, src, want_ctop); return;
