@@ -285,6 +285,7 @@ static void face_flux_x3_deref(const Params& par, Block& b, const Fields& s, int
       if (kk < 0) kk = kk / m;                       // groups beyond the low edge: ghost zones -1, -2, -3
       else if (kk >= n3) kk = n3 + (kk - n3) / m;    // beyond the high edge: ghost zones n3, n3 + 1, n3 + 2
       st6[v][t] = var[v][b.idx(i, j, kk)];
+      if (v == 0 && par.entropy_backup) st6[7][t] = b.K[b.idx(i, j, kk)];   // C-18: kappa of the same groups
     }
   face_flux_core(par, b, s, 2, i, j, z, st6, ctop);
 }
@@ -362,12 +363,15 @@ void deref_fix_fluxes(const Params& par, Block& b) {
   for (int i = -1; i <= b.n[0]; i++)
     for (int j = -1; j <= b.n[1]; j++) {
       const int m = b.mrow[j + NG];
+      const bool ent = par.entropy_backup != 0;   // C-18: the entropy flux is one more flux of the row
       if (m > 1 && i >= 0) {          // x1-faces of the row
+        if (ent) group_mean(b.FK[0], b, i, j, m);
         for (int c = 0; c < 5; c++) group_mean(b.F[0][c], b, i, j, m);
         group_mean(b.Ef[0][1], b, i, j, m);
         group_mean(b.Ef[0][2], b, i, j, m);
       }
       if (m > 1) {                    // x3-faces of the row: in-group faces
+        if (ent) group_interp(b.FK[2], b, i, j, m);
         for (int c = 0; c < 5; c++) group_interp(b.F[2][c], b, i, j, m);
         group_interp(b.Ef[2][0], b, i, j, m);
         group_interp(b.Ef[2][1], b, i, j, m);
@@ -375,6 +379,7 @@ void deref_fix_fluxes(const Params& par, Block& b) {
       if (j >= 0) {                   // x2-face between rows j-1 and j: the coarser of the two groupings
         const int M = face2_factor(b, j);
         if (M > 1) {
+          if (ent) group_mean(b.FK[1], b, i, j, M);
           for (int c = 0; c < 5; c++) group_mean(b.F[1][c], b, i, j, M);
           group_mean(b.Ef[1][2], b, i, j, M);
           group_mean(b.Ef[1][0], b, i, j, M);

@@ -97,10 +97,10 @@ __global__ void __launch_bounds__(128) k_deref_fix_flux(Dev Dv) {
   const long long zrow = T.C.zoff + L.idx(i, j, 0);
   // blockIdx.y: the quantity (five hydro fluxes, the two transverse face EMFs): seven independent threads per
   // group instead of one thread walking 21 read-modify-write chains one after the other
-  const int c = blockIdx.y;
-  double* const a0 = c < 5 ? Dv.F[0][c] : (c == 5 ? Dv.EfA[0] : Dv.EfB[0]);
-  double* const a1 = c < 5 ? Dv.F[1][c] : (c == 5 ? Dv.EfA[1] : Dv.EfB[1]);
-  double* const a2 = c < 5 ? Dv.F[2][c] : (c == 5 ? Dv.EfA[2] : Dv.EfB[2]);
+  const int c = blockIdx.y;   // 7 (C-18): the entropy flux, one more flux of the row
+  double* const a0 = c < 5 ? Dv.F[0][c] : (c == 5 ? Dv.EfA[0] : (c == 6 ? Dv.EfB[0] : Dv.FK[0]));
+  double* const a1 = c < 5 ? Dv.F[1][c] : (c == 5 ? Dv.EfA[1] : (c == 6 ? Dv.EfB[1] : Dv.FK[1]));
+  double* const a2 = c < 5 ? Dv.F[2][c] : (c == 5 ? Dv.EfA[2] : (c == 6 ? Dv.EfB[2] : Dv.FK[2]));
   if (m > 1 && k % m == 0) {
     if (i >= 0) group_mean(a0, zrow, k, m);                 // x1-faces of the row
     group_interp(a2, zrow, k, m);                           // x3-faces inside the group
@@ -228,8 +228,9 @@ void launch_deref_fix_flux(hamr_grid* g, const Dev& Dv0) {
   if (!Dv.mrow || (Dv.B.nblk > 0 && Dv.B.nact == 0)) return;
   Launch l_(g, K_OTHER);
   const unsigned nb = nblocks_for(Dv, Dv.L.n[0] + 2, Dv.L.n[1] + 2);
-  if (Dv.B.nblk > 0) k_deref_fix_flux<true><<<dim3(nb, 7), 128, 0, g->stream>>>(Dv);
-  else k_deref_fix_flux<false><<<dim3(nb, 7), 128, 0, g->stream>>>(Dv);
+  const unsigned nq = Dv.entropy ? 8 : 7;
+  if (Dv.B.nblk > 0) k_deref_fix_flux<true><<<dim3(nb, nq), 128, 0, g->stream>>>(Dv);
+  else k_deref_fix_flux<false><<<dim3(nb, nq), 128, 0, g->stream>>>(Dv);
 }
 
 void launch_deref_flux_layers(hamr_grid* g, const Dev& Dv0) {

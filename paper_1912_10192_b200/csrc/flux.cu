@@ -765,7 +765,8 @@ static int x3_warp_m(const Dev& Dv) {
 // group-boundary faces only (k a multiple of m); its stencil takes one value per group, zones k + t m,
 // t = -3..2 (beyond the block the phi-ghost zones hold groups, C-15); the Courant limit uses m dx3.
 // One thread per group-boundary face; rows with m = 1 return at once.
-template <int RECON, bool BLK>
+// ENT (C-18): kappa of the same groups is the eighth reconstructed variable, the entropy flux goes to FK
+template <int RECON, bool BLK, bool ENT = false>
 __global__ void __launch_bounds__(128) k_deref_x3(Dev Dv, Fields s, Fields s2, int want_ctop) {
   constexpr int D = 2;
   const Lay& L = Dv.L;
@@ -784,35 +785,36 @@ __global__ void __launch_bounds__(128) k_deref_x3(Dev Dv, Fields s, Fields s2, i
   if (valid && m > 1 && k % m == 0) {
     const int n3 = L.n[2];
     const int zrow = C.zoff + (int)L.idx(i, j, 0);
-    const double* var[7] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
+    const double* var[8] = {selp<BLK>(s.P[0], s2.P[0], C.cur), selp<BLK>(s.P[1], s2.P[1], C.cur),
                             selp<BLK>(s.P[2], s2.P[2], C.cur), selp<BLK>(s.P[3], s2.P[3], C.cur),
                             selp<BLK>(s.P[4], s2.P[4], C.cur), selp<BLK>(s.Bc[0], s2.Bc[0], C.cur),
-                            selp<BLK>(s.Bc[1], s2.Bc[1], C.cur)};
+                            selp<BLK>(s.Bc[1], s2.Bc[1], C.cur), Dv.K};
+    constexpr int slot[8] = {0, 1, 2, 3, 4, 5, 6, 8};   // kappa goes to slot 8 of the states (slot 7: the normal field)
     int kk[6];   // beyond the block the phi-ghost zones hold whole groups: -1, -2, -3 and n3, n3 + 1, n3 + 2
 #pragma unroll
     for (int q = 0; q < 6; q++) {
       const int w = k + (q - 3) * m;
       kk[q] = w < 0 ? w / m : (w >= n3 ? n3 + (w - n3) / m : w);
     }
-    double PL[8], PR[8];
+    double PL[9], PR[9];
 #pragma unroll
-    for (int v = 0; v < 7; v++) {
+    for (int v = 0; v < (ENT ? 8 : 7); v++) {
       const double* a = var[v] + zrow;
       const double a0 = a[kk[0]], a1 = a[kk[1]], a2 = a[kk[2]], a3 = a[kk[3]], a4 = a[kk[4]], a5 = a[kk[5]];
       double dum;
       if (RECON == HAMR_RECON_PPM) {
-        ppm_edges(a0, a1, a2, a3, a4, dum, PL[v]);   // left of the face: a_R of group k/m - 1
-        ppm_edges(a1, a2, a3, a4, a5, PR[v], dum);   // right of the face: a_L of group k/m
+        ppm_edges(a0, a1, a2, a3, a4, dum, PL[slot[v]]);   // left of the face: a_R of group k/m - 1
+        ppm_edges(a1, a2, a3, a4, a5, PR[slot[v]], dum);   // right of the face: a_L of group k/m
       } else {
-        plm_edges(a1, a2, a3, dum, PL[v]);
-        plm_edges(a2, a3, a4, PR[v], dum);
+        plm_edges(a1, a2, a3, dum, PL[slot[v]]);
+        plm_edges(a2, a3, a4, PR[slot[v]], dum);
       }
     }
     const int ge2 = BLK ? Dv.B.ge2 : L.e2;
     const FGeo G = load_fgeo(Dv.gf3A + (BLK ? C.lev * Dv.B.tlevA : 0) + (size_t)(C.q0 + i * ge2 + j) * NREC_F);
     const int z = zrow + k;
     PL[7] = PR[7] = selp<BLK>(s.Bf[2], s2.Bf[2], C.cur)[z] * G.igdet;
-    const double ct = face_flux<D>(PL, PR, G, Dv.gam, Dv, z);
+    const double ct = face_flux<D, ENT>(PL, PR, G, Dv.gam, Dv, z);
     if (i >= 0 && i < L.n[0] && j >= 0 && j < L.n[1]) ctop = ct / (double)m;
   }
   if (want_ctop) ctop_commit<BLK>(Dv, D, C.b, ctop);
@@ -829,6 +831,13 @@ void launch_deref_x3(hamr_grid* g, const Dev& Dv0, const Fields& src, const Fiel
   const unsigned nb = (unsigned)((tot + 127) / 128);
   const int wc = want_ctop ? 1 : 0;
   Launch l_(g, K_FLUX3);
+  if (Dv.entropy) {   // C-18
+    if (ppm && !blk) k_deref_x3<HAMR_RECON_PPM, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (ppm) k_deref_x3<HAMR_RECON_PPM, true, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else if (!blk) k_deref_x3<HAMR_RECON_PLM_MC, false, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    else k_deref_x3<HAMR_RECON_PLM_MC, true, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
+    return;
+  }
   if (ppm && !blk) k_deref_x3<HAMR_RECON_PPM, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
   else if (ppm) k_deref_x3<HAMR_RECON_PPM, true><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);
   else if (!blk) k_deref_x3<HAMR_RECON_PLM_MC, false><<<nb, 128, 0, g->stream>>>(Dv, src, src2, wc);

@@ -400,3 +400,27 @@ def test_robust_path_on_a_block_grid(H, orc, case):
     assert g.divb() <= 1e-12
     for a, b in zip(o.get_bface(), g.get_bface()):
         assert rel_max(a, b) <= 1e-7
+
+
+@pytest.mark.parametrize("nb", [(0, 0, 0), (8, 4, 16)])
+def test_robust_path_with_phi_derefined_rows(H, orc, nb):
+    """C-18 / C-19 on a torus whose polar rows are derefined by 4 / 2 / 2 (one block, and blocks stepping together): the
+    strided x3 sweep reconstructs kappa of the same groups, the entropy flux goes through the group fix-up"""
+    p = I.torus_params(n=(32, 16, 16), nb=nb, deref_theta_deg=(30.0, 12.0), deref_factor=(2, 4), entropy_backup=1, drift_floors=1)
+    hyd, bf = I.fm_torus(p, seed=4)
+    g, o = _pair(H, orc, p, hyd, bf)
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt
+    tot = 0
+    for step, tol in ((1, 1e-10), (2, 4e-10), (3, 1e-9)):
+        g.step(1)
+        o.step(1)
+        e = parity_errors(p, o.get_prims(), g.get_prims())
+        sg, so, bg, bo = g.stats(), o.stats(), g.backup_count(), o.backup_count()
+        print(f"deref + NEXT-2 nb={nb} step {step}: {e} stats {sg} {so} entropy inversions {bg} {bo}")
+        assert max(e.values()) <= tol, (step, e)
+        assert sg[0] == so[0] == 0 and sg[3] == so[3]
+        assert abs(bg - bo) <= max(3, bo // 50)      # at the floors a last-bit difference decides (see test_gpu_parity)
+        tot += bo
+    assert tot > 100 and g.divb() <= 1e-12
+    for a, b in zip(o.get_bface(), g.get_bface()):
+        assert rel_max(a, b) <= 1e-7

@@ -367,3 +367,35 @@ def test_robust_path_block_decomposition_is_the_one_block_run(orc):
         assert all(np.array_equal(x, y) for x, y in zip(m.get_prims(), b.get_prims()))
         assert m.stats() == b.stats() and m.backup_count() == b.backup_count() > 100
         assert b.divb() <= 1e-12
+
+
+@pytest.mark.parametrize("m", [2, 4])
+def test_robust_path_on_a_grid_derefined_everywhere_is_the_coarse_phi_grid(orc, m):
+    """C-18 / C-19 with C-15 (the robust analogue of pin P14): a grid derefined by m in EVERY row equals, zone for zone, the
+    plain grid with N3 / m zones — the strided x3 stencil reconstructs kappa of the same groups, the entropy flux is one
+    more flux of the row (group mean / interpolation) — and every event is counted m times (once per member)"""
+    import numpy as np
+    from paper_1912_10192_b200 import inputs as I
+    from tests.test_oracle_deref import _rep_state
+    opt = dict(entropy_backup=1, drift_floors=1)
+    pc = dict(I.torus_params(n=(16, 8, 8)), **opt)
+    pf = dict(I.torus_params(n=(16, 8, 8 * m), deref_theta_deg=(91.0,), deref_factor=(m,)), **opt)
+    hyd, bf = I.fm_torus(pc, seed=3)
+    c0 = orc.OrcGrid(pc)                       # a phi-dependent field as well: a few steps of evolution first
+    assert c0.set_prims(hyd, bf) == 0
+    c0.step(3)
+    hyd, bf = c0.get_prims()[:5], c0.get_bface()
+    c, f = orc.OrcGrid(pc), orc.OrcGrid(pf)
+    Hf, Bf = _rep_state(hyd, bf, m)
+    assert c.set_prims(hyd, bf) == 0 and f.set_prims(Hf, Bf) == 0
+    c.step(4)
+    f.step(4)
+    for a, b in zip(c.get_prims(), f.get_prims()):
+        s = max(np.abs(a).max(), 1e-300)
+        for r in range(m):
+            assert np.abs(b[:, :, r::m] - a).max() <= 1e-12 * s
+    sc, sf = c.stats(), f.stats()
+    assert sc[0] == sf[0] == 0 and sf[3] == m * sc[3]
+    bc, bf_ = c.backup_count(), f.backup_count()      # (the counter is read and reset)
+    assert bc > 100 and bf_ == m * bc
+    assert f.divb() <= 1e-12
