@@ -162,8 +162,9 @@ const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the 
  * floors.  The Lorentz-factor ceiling follows as before.
  * Both options work on a grid of one block and on a grid cut into blocks that step together (nb set, lat_max_level = 0),
  * with or without phi-derefined polar rows (the strided x3 sweep reconstructs kappa of the same groups, the entropy flux
- * goes through the group fix-up like the other fluxes); LAT and the x1 refinement level are refused with them (HAMR_EINVAL:
- * the flux / EMF registers, the correction pass and the refinement interface do not carry the ninth row).  The staged kernels
+ * goes through the group fix-up like the other fluxes) and with the x1 refinement level (the coarse block takes the fine
+ * block's entropy flux on the interface face); LAT is refused with them (HAMR_EINVAL: the flux registers and the
+ * correction pass do not carry the ninth row).  The staged kernels
  * carry the ninth row where they serve the grid (cfg 2 with both options: 80 % of its plain rate). */
 
 /* ---- regridding of the x1 refinement level (the x1-only part; C-20) ------------------ */

@@ -29,9 +29,9 @@ static bool params_ok(const Params& p, std::string& why) {
   if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0)) { why = "gamma_ad/cour"; return false; }
   if (p.entropy_backup || p.drift_floors) {  // C-18, C-19: one block, or blocks that step together on one lattice level
     if ((p.entropy_backup & ~1) || (p.drift_floors & ~1)) { why = "entropy_backup / drift_floors are 0 or 1"; return false; }
-    // (LAT's flux registers and correction and the refinement interface do not carry the ninth row)
-    if (p.lat_max_level > 0 || p.r_refine_max > 0.0) {
-      why = "entropy_backup / drift_floors need a grid without refinement and LAT";
+    // (LAT's flux registers and correction do not carry the ninth row)
+    if (p.lat_max_level > 0) {
+      why = "entropy_backup / drift_floors need a grid without LAT";
       return false;
     }
     if (p.entropy_backup && !(p.gamma_ad < 2.0)) { why = "the entropy inversion needs gamma_ad < 2"; return false; }
@@ -344,6 +344,18 @@ int orc_get_aitken_count(void* h, long long* n) {
 int orc_get_kadv(void* h, double* out) {
   Grid& g = *(Grid*)h;
   Block& b = g.blocks[0];
+  if (!g.par.entropy_backup || b.Kadv.empty()) return 1;
+  for (int i = 0; i < b.n[0]; i++)
+    for (int j = 0; j < b.n[1]; j++)
+      for (int k = 0; k < b.n[2]; k++) out[((size_t)i * b.n[1] + j) * b.n[2] + k] = b.Kadv[b.idx(i, j, k)];
+  return 0;
+}
+
+// the same for block bi of a block grid (block-local dense array)
+int orc_get_block_kadv(void* h, int bi, double* out) {
+  Grid& g = *(Grid*)h;
+  if (bi < 0 || bi >= (int)g.blocks.size()) return 1;
+  Block& b = g.blocks[bi];
   if (!g.par.entropy_backup || b.Kadv.empty()) return 1;
   for (int i = 0; i < b.n[0]; i++)
     for (int j = 0; j < b.n[1]; j++)

@@ -328,8 +328,10 @@ static void interface_agreement(Grid& g, int tau) {
       for (int j = 0; j <= c.n[1]; j++)
         for (int k = 0; k <= c.n[2]; k++) {
           const size_t zc = c.idx(ic, j, k), zq = q.idx(iq, j, k);
-          if (j < c.n[1] && k < c.n[2])
+          if (j < c.n[1] && k < c.n[2]) {
             for (int cc = 0; cc < 5; cc++) c.F[0][cc][zc] = q.F[0][cc][zq];
+            if (g.par.entropy_backup) c.FK[0][zc] = q.FK[0][zq];   // C-18: the entropy flux is one more flux of the face
+          }
           if (j < c.n[1]) c.Ee[1][zc] = q.Ee[1][zq];   // E2 on edges along x2 at (i-1/2, k-1/2)
           if (k < c.n[2]) c.Ee[2][zc] = q.Ee[2][zq];   // E3 on edges along x3 at (i-1/2, j-1/2)
         }

@@ -84,9 +84,9 @@ bool params_ok(const hamr_params& p, std::string& why) {
   if (p.lat_max_level < 0 || p.lat_max_level > 3) { why = "lat_max_level must be 0..3"; return false; }
   if ((p.entropy_backup & ~1) || (p.drift_floors & ~1)) { why = "entropy_backup / drift_floors are 0 or 1"; return false; }
   if (p.entropy_backup || p.drift_floors) {   // NEXT-2 (C-18, C-19): one block, or blocks that step together on one lattice level
-    // (LAT's flux registers and correction and the refinement interface do not carry the ninth row)
-    if (p.lat_max_level > 0 || p.r_refine_max > 0.0) {
-      why = "entropy_backup / drift_floors need a grid without LAT and x1 refinement";
+    // (LAT's flux registers and correction do not carry the ninth row)
+    if (p.lat_max_level > 0) {
+      why = "entropy_backup / drift_floors need a grid without LAT";
       return false;
     }
     if (p.entropy_backup && !(p.gamma_ad < 2.0)) { why = "the entropy inversion needs gamma_ad < 2"; return false; }

@@ -975,6 +975,7 @@ __global__ void __launch_bounds__(128) k_blk_iface(Dev Dv) {
   if (j < L.n[1] && k < L.n[2]) {
 #pragma unroll
     for (int cc = 0; cc < 5; cc++) Dv.F[0][cc][zc] = Dv.F[0][cc][zq];
+    if (Dv.entropy) Dv.FK[0][zc] = Dv.FK[0][zq];   // C-18: the entropy flux is one more flux of the face
   }
   if (j < L.n[1]) Dv.Ee[1][zc] = Dv.Ee[1][zq];
   if (k < L.n[2]) Dv.Ee[2][zc] = Dv.Ee[2][zq];

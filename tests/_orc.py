@@ -87,6 +87,7 @@ def lib():
         L.orc_get_t.restype = C.c_double
         L.orc_get_t.argtypes = [C.c_void_p]
         L.orc_get_kadv.argtypes = [C.c_void_p, c_double_p]
+        L.orc_get_block_kadv.argtypes = [C.c_void_p, C.c_int, c_double_p]
         L.orc_get_aitken_count.argtypes = [C.c_void_p, C.POINTER(C.c_longlong)]
         L.orc_ppm_zone.argtypes = [c_double_p] * 3
         L.orc_plm_zone.argtypes = [c_double_p] * 3
@@ -307,6 +308,12 @@ class OrcGrid:
 
     def commit(self):
         return self.L.orc_blocks_commit(self.h)
+
+    def get_block_kadv(self, b):
+        out = np.empty(self.block_info(b)["n"])
+        rc = self.L.orc_get_block_kadv(self.h, C.c_int(b), _dp(out))
+        assert rc == 0
+        return out
 
     def get_block_prims(self, b):
         n = self.block_info(b)["n"]

@@ -424,3 +424,34 @@ def test_robust_path_with_phi_derefined_rows(H, orc, nb):
     assert tot > 100 and g.divb() <= 1e-12
     for a, b in zip(o.get_bface(), g.get_bface()):
         assert rel_max(a, b) <= 1e-7
+
+
+def test_robust_path_on_a_refined_grid(H, orc):
+    """C-18 / C-19 across the x1 refinement interface (blocks stepping together): kappa of the restricted / prolonged ghost
+    zones, the fine block's entropy flux taken by the coarse block on the interface face"""
+    p = I.torus_params(n=(32, 16, 16), nb=(8, 8, 8), r_refine_max=6.0, entropy_backup=1, drift_floors=1)
+    g, o = H.Grid(p), orc.OrcGrid(p)
+    infos = []
+    for b in range(o.num_blocks()):
+        d = o.block_info(b)
+        infos.append((d["x_lo"], d["dx"], d["n"]))
+    assert len({round(i[1][0], 12) for i in infos}) == 2
+    for b, (hyd, bf) in enumerate(I.fm_torus_blocks(p, infos, seed=4)):
+        assert g.set_block_prims(b, hyd, bf) == 0 and o.set_block_prims(b, hyd, bf) == 0
+    assert g.commit() == 0 and o.commit() == 0
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt
+    tot = 0
+    for step, tol in ((1, 1e-10), (2, 4e-10), (3, 1e-9)):
+        g.step(1)
+        o.step(1)
+        worst = {}
+        for b, (x_lo, dx, n) in enumerate(infos):
+            e = parity_errors(I.block_as_grid(p, x_lo, dx, n), o.get_block_prims(b), g.get_block_prims(b))
+            for k, v in e.items():
+                worst[k] = max(worst.get(k, 0.0), v)
+        sg, so, bg, bo = g.stats(), o.stats(), g.backup_count(), o.backup_count()
+        print(f"refined + NEXT-2 step {step}: {worst} stats {sg} {so} entropy inversions {bg} {bo}")
+        assert max(worst.values()) <= tol, (step, worst)
+        assert sg[0] == so[0] == 0 and sg[3] == so[3] and abs(bg - bo) <= max(3, bo // 50)
+        tot += bo
+    assert tot > 100 and g.divb() <= 1e-12

@@ -399,3 +399,36 @@ def test_robust_path_on_a_grid_derefined_everywhere_is_the_coarse_phi_grid(orc, 
     bc, bf_ = c.backup_count(), f.backup_count()      # (the counter is read and reset)
     assert bc > 100 and bf_ == m * bc
     assert f.divb() <= 1e-12
+
+
+def test_entropy_row_telescopes_across_the_refinement_interface(orc):
+    """C-18 with C-16: the coarse block takes the fine block's entropy flux on the interface face (as it takes the other
+    fluxes), so the volume-weighted sum of the entropy row over a periodic box with a refined column is unchanged by a
+    step to round-off; with its OWN flux on that face the sum would move at truncation level (checked: the same sum
+    with the coarse side's flux differences is off by > 1e-9 on this data).  D = gamma rho in numpy on both sides."""
+    import numpy as np
+    from paper_1912_10192_b200 import inputs as I
+    gam = 4.0 / 3.0
+    p = I.minkowski_params(n=(32, 8, 8), nb=(8, 4, 4), r_refine_max=0.3, entropy_backup=1)
+    g = orc.OrcGrid(p)
+    infos = [g.block_info(b) for b in range(g.num_blocks())]
+    assert len({round(d["dx"][0], 12) for d in infos}) == 2          # both levels present
+    for b, d in enumerate(infos):
+        hyd, bf = I.minkowski_waves(I.block_as_grid(p, d["x_lo"], d["dx"], d["n"]), seed=3, amp=5e-2, noise=1e-3,
+                                    box=(1.0, 1.0, 1.0))[:2]
+        assert g.set_block_prims(b, hyd, bf) == 0
+    assert g.commit() == 0
+    g.step(2)
+
+    def dens(P):
+        return np.sqrt(1.0 + P[2] ** 2 + P[3] ** 2 + P[4] ** 2) * P[0]
+    base = [g.get_block_prims(b) for b in range(g.num_blocks())]
+    g.step(1)                                                        # kappa was reset from `base` before this step
+    assert g.stats()[0] == 0 and g.backup_count() == 0
+    s0 = s1 = 0.0
+    for b, d in enumerate(infos):
+        vol = d["dx"][0]                                             # x2, x3 widths are the same on both levels
+        P0, P1, ka = base[b], g.get_block_prims(b), g.get_block_kadv(b)
+        s0 += vol * (dens(P0) * (gam - 1.0) * P0[1] / P0[0] ** gam).sum()
+        s1 += vol * (dens(P1) * ka).sum()
+    assert abs(s1 - s0) <= 5e-13 * abs(s0), (s0, s1, (s1 - s0) / s0)
