@@ -160,11 +160,12 @@ const char* hamr_last_error(const hamr_grid* g); /* never NULL; valid until the 
  * 2017)"): a zone below a floor is raised to it with the velocity perpendicular to the magnetic field unchanged and
  * the momentum along the field, (rho + gamma_ad u) gamma^2 v_par, conserved; zones without field get the fluid-frame
  * floors.  The Lorentz-factor ceiling follows as before.
- * Both options work on a grid of one block and on a grid cut into blocks that step together (nb set, lat_max_level = 0),
- * with or without phi-derefined polar rows (the strided x3 sweep reconstructs kappa of the same groups, the entropy flux
- * goes through the group fix-up like the other fluxes) and with the x1 refinement level (the coarse block takes the fine
- * block's entropy flux on the interface face); LAT is refused with them (HAMR_EINVAL: the flux registers and the
- * correction pass do not carry the ninth row).  The staged kernels
+ * Both options work on every grid the library builds: one block, blocks, phi-derefined polar rows (the strided x3 sweep
+ * reconstructs kappa of the same groups, the entropy flux goes through the group fix-up like the other fluxes), the x1
+ * refinement level (the coarse block takes the fine block's entropy flux on the interface face) and LAT (the flux
+ * registers carry the entropy flux; the correction pass corrects the entropy row of the coarse block's boundary zones —
+ * kappa having been reset, their row before the correction is density row x kappa of the new primitives — and inverts
+ * them through the same chain, with the drift-frame floors if they are on).  The staged kernels
  * carry the ninth row where they serve the grid (cfg 2 with both options: 80 % of its plain rate). */
 
 /* ---- regridding of the x1 refinement level (the x1-only part; C-20) ------------------ */

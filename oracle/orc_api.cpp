@@ -29,11 +29,6 @@ static bool params_ok(const Params& p, std::string& why) {
   if (!(p.gamma_ad > 1.0) || !(p.cour > 0.0)) { why = "gamma_ad/cour"; return false; }
   if (p.entropy_backup || p.drift_floors) {  // C-18, C-19: one block, or blocks that step together on one lattice level
     if ((p.entropy_backup & ~1) || (p.drift_floors & ~1)) { why = "entropy_backup / drift_floors are 0 or 1"; return false; }
-    // (LAT's flux registers and correction do not carry the ninth row)
-    if (p.lat_max_level > 0) {
-      why = "entropy_backup / drift_floors need a grid without LAT";
-      return false;
-    }
     if (p.entropy_backup && !(p.gamma_ad < 2.0)) { why = "the entropy inversion needs gamma_ad < 2"; return false; }
   }
   return true;

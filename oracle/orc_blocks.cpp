@@ -119,6 +119,7 @@ void blocks_build(Grid& g) {
       for (int c = 0; c < 5; c++) { b.FA[d][c].assign(n, 0.0); b.FA2[d][c].assign(n, 0.0); }
       b.EA[d].assign(n, 0.0);
       b.EA2[d].assign(n, 0.0);
+      if (par.entropy_backup) { b.FKA[d].assign(n, 0.0); b.FKA2[d].assign(n, 0.0); }
       b.ctop_last[d] = 0.0;
     }
   }
@@ -418,6 +419,12 @@ static void stage_level(Grid& g, int tau, bool corrector) {
           b.EA[d][z] = v;
           b.EA2[d][z] = first ? v : b.EA2[d][z] + v;
         }
+        if (g.par.entropy_backup)   // C-18: the entropy flux is one more flux of the face
+          for (size_t z = 0; z < n; z++) {
+            const double v = dtb * b.FK[d][z];
+            b.FKA[d][z] = v;
+            b.FKA2[d][z] = first ? v : b.FKA2[d][z] + v;
+          }
         b.ctop_last[d] = b.ctop[d];
       }
     }
@@ -449,7 +456,7 @@ static void correct_level(Grid& g, int tau) {
     const size_t n = c.size();
     std::vector<double> EC[3];
     std::vector<char> erep[3], ftouch[3], zmask(n, 0);
-    std::vector<double> dU[5];
+    std::vector<double> dU[5], dUS(n, 0.0);
     for (int d = 0; d < 3; d++) { EC[d] = c.EA[d]; erep[d].assign(n, 0); ftouch[d].assign(n, 0); }
     for (int cc = 0; cc < 5; cc++) dU[cc].assign(n, 0.0);
     // (1) replace boundary edge EMFs by the finer sharer's accumulated value
@@ -524,6 +531,10 @@ static void correct_level(Grid& g, int tau) {
               // U_new = U - (dt F_hi - dt F_lo)/dx: the high face enters with -, the low face with +
               dU[cc][zz] += (side ? -dF : dF) / c.dx[d];
             }
+            if (par.entropy_backup) {
+              const double dF = q.FKA2[d][zq] - c.FKA[d][zf];
+              dUS[zz] += (side ? -dF : dF) / c.dx[d];
+            }
             zmask[zz] = 1;
           }
       }
@@ -555,11 +566,32 @@ static void correct_level(Grid& g, int tau) {
             c.snew.Bc[d][z] = Bn[d];
           }
           int rc = con2prim(U, Bn, G, par.gamma_ad, P, Pn, nullptr);
+          if (par.entropy_backup) {
+            // C-18 / C-21 under LAT: the corrected rows go through the same chain as in the update.  kappa was reset from
+            // the zone's new primitives, so its entropy row before the correction is its density row times kappa(P)
+            if (rc != 0) {
+              double Pa[5];
+              if (con2prim_aitken(U, Bn, G, par.gamma_ad, P, Pa, nullptr) == 0) {
+                for (int cc = 0; cc < 5; cc++) Pn[cc] = Pa[cc];
+                rc = 0;
+                g.stats.c2p_aitken++;
+              }
+            }
+            if (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) {
+              const double US = (U[0] - dU[0][z]) * entropy_kappa(P[0], P[1], par.gamma_ad) + dUS[z];
+              double Pe[5];
+              if (con2prim_entropy(U, US, Bn, G, par.gamma_ad, P, Pe, nullptr) == 0) {
+                for (int cc = 0; cc < 5; cc++) Pn[cc] = Pe[cc];
+                rc = 0;
+                g.stats.c2p_entropy++;
+              }
+            }
+          }
           if (rc != 0) {
             g.stats.c2p_fail++;
             for (int cc = 0; cc < 5; cc++) Pn[cc] = P[cc];
           }
-          floors_and_ceiling(par, G, r, Pn, nullptr, g.stats);
+          floors_and_ceiling(par, G, r, Pn, par.drift_floors ? Bn : nullptr, g.stats);
           for (int cc = 0; cc < 5; cc++) c.snew.P[cc][z] = Pn[cc];
         }
       }

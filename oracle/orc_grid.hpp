@@ -44,6 +44,7 @@ struct Block {
   std::vector<double> EA[3];       // EMF register R1: dt_b * E_edge of the latest corrector
   std::vector<double> FA2[3][5];   // R2: R1 summed over the two steps inside one step of the next
   std::vector<double> EA2[3];      //     coarser time level
+  std::vector<double> FKA[3], FKA2[3];   // C-18 under LAT: the same two registers for the entropy flux
   double ctop_last[3];             // ctop of this block's most recent corrector (or initial) pass
   std::vector<double> K;           // C-18: kappa of the flux pass's source state, every zone incl. ghosts
   std::vector<double> FK[3];       // C-18: entropy fluxes on d-faces

@@ -84,11 +84,6 @@ bool params_ok(const hamr_params& p, std::string& why) {
   if (p.lat_max_level < 0 || p.lat_max_level > 3) { why = "lat_max_level must be 0..3"; return false; }
   if ((p.entropy_backup & ~1) || (p.drift_floors & ~1)) { why = "entropy_backup / drift_floors are 0 or 1"; return false; }
   if (p.entropy_backup || p.drift_floors) {   // NEXT-2 (C-18, C-19): one block, or blocks that step together on one lattice level
-    // (LAT's flux registers and correction do not carry the ninth row)
-    if (p.lat_max_level > 0) {
-      why = "entropy_backup / drift_floors need a grid without LAT";
-      return false;
-    }
     if (p.entropy_backup && !(p.gamma_ad < 2.0)) { why = "the entropy inversion needs gamma_ad < 2"; return false; }
   }
   if (is_block_grid(p)) {
@@ -129,7 +124,7 @@ bool make_layout(const hamr_params& p, Lay& L, GridShape& G) {
   G.te1 = G.nlev * p.n[0] + 2 * NG + 1;   // the level-1 table is indexed in fine zones
   G.te2 = p.n[1] + 2 * NG + 1;
   L.n2d = G.te1 * G.te2;
-  G.narr = N_ARR + ((G.nblk > 0 && p.lat_max_level > 0) ? N_REG_ARR : 0) + (p.entropy_backup ? 4 : 0);
+  G.narr = N_ARR + ((G.nblk > 0 && p.lat_max_level > 0) ? N_REG_ARR + (p.entropy_backup ? 3 : 0) : 0) + (p.entropy_backup ? 4 : 0);
   return true;
 }
 
@@ -309,6 +304,7 @@ int create_common(const hamr_params* p, void* arena, size_t arena_bytes, void* s
   if (gs.nblk > 0 && p->lat_max_level > 0) {
     for (int d = 0; d < 3; d++) for (int c = 0; c < 5; c++) D.B.FA2[d][c] = next();
     for (int d = 0; d < 3; d++) D.B.EA2[d] = next();
+    if (p->entropy_backup) for (int d = 0; d < 3; d++) D.B.FKA2[d] = next();   // C-18 under LAT
   }
   D.entropy = p->entropy_backup;
   D.drift = p->drift_floors;

@@ -601,6 +601,10 @@ __global__ void __launch_bounds__(128) k_blk_registers(Dev Dv, int first, double
         const double v = dtb * Dv.F[d][c][z];
         Dv.B.FA2[d][c][z] = first ? v : Dv.B.FA2[d][c][z] + v;
       }
+      if (Dv.entropy) {   // C-18: the entropy flux is one more flux of the face
+        const double v = dtb * Dv.FK[d][z];
+        Dv.B.FKA2[d][z] = first ? v : Dv.B.FKA2[d][z] + v;
+      }
     }
     // edge along d lies on the boundary if either transverse index does
     if (id[d] < L.n[d] && (onb[e] || onb[f])) {
@@ -714,7 +718,7 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
   const Lay& L = Dv.L;
   const unsigned per = (unsigned)L.n[0] * L.n[1] * L.n[2];
   unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
-  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0;
+  int nfail = 0, nrf = 0, nuf = 0, ngc = 0, bad = 0, nent = 0, nait = 0;
   if (t < per * Dv.B.nact) {
     const int bslot = (int)(t / per);
     t -= bslot * per;
@@ -731,7 +735,7 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
       const long long S[3] = {L.S1, L.S2, 1};
       const long long z = (long long)c * Dv.B.blen + L.idx(id[0], id[1], id[2]);
       bool touched = false;
-      double dU[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      double dU[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, dUS = 0.0;
 #pragma unroll
       for (int d = 0; d < 3; d++) {
 #pragma unroll
@@ -756,6 +760,10 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
                 // U_new = U - (dt F_hi - dt F_lo)/dx: the high face enters with -, the low face with +
                 dU[cc] += (side ? -dF : dF) / dxd[d];
               }
+              if (Dv.entropy) {   // C-18: the entropy row is corrected like the others
+                const double dF = Dv.B.FKA2[d][zq] - dtc * Dv.FK[d][zf];
+                dUS += (side ? -dF : dF) / dxd[d];
+              }
               touched = true;
             }
           }
@@ -779,15 +787,47 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
         St Sx;
         get_state(P, G, Sx);
         prim_to_U5(P, Sx, G.gdet, Dv.gam, U);
+        // C-18 under LAT: kappa was reset from the zone's new primitives, so its entropy row before the correction is its
+        // density row times kappa(P)
+        const double US = Dv.entropy ? U[0] * kappa_of(P[0], P[1], Dv.gam) + dUS : 0.0;
 #pragma unroll
         for (int cc = 0; cc < 5; cc++) U[cc] += dU[cc];
-        if (con2prim(U, Bn, G, Dv.gam, P, Pn) != 0) {
+        int rc = con2prim(U, Bn, G, Dv.gam, P, Pn);
+        if (Dv.entropy && (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0))) {   // the chain of the update (C-21, C-18)
+          double Pe[5], Uc[5], Bc[3], Pc[5];
+          CGeo Gc = G;
+#pragma unroll
+          for (int cc = 0; cc < 5; cc++) { Uc[cc] = U[cc]; Pc[cc] = P[cc]; }
+#pragma unroll
+          for (int cc = 0; cc < 3; cc++) Bc[cc] = Bn[cc];
+          if (rc != 0 && con2prim_aitken(Uc, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
+#pragma unroll
+            for (int cc = 0; cc < 5; cc++) Pn[cc] = Pe[cc];
+            rc = 0;
+            nait = 1;
+          }
+          if ((rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0)) && con2prim_entropy(Uc, US, Bc, &Gc, Dv.gam, Pc, Pe) == 0) {
+#pragma unroll
+            for (int cc = 0; cc < 5; cc++) Pn[cc] = Pe[cc];
+            rc = 0;
+            nent = 1;
+          }
+        }
+        if (rc != 0) {
           nfail = 1;
 #pragma unroll
           for (int cc = 0; cc < 5; cc++) Pn[cc] = P[cc];
         }
         const int fi = inf.z + id[0] + NG + inf.y * Dv.B.flev;
-        floors_ceiling(G, __ldg(Dv.rho_fl + fi), __ldg(Dv.u_fl + fi), Dv.gamma_max, Pn, nrf, nuf, ngc);
+        const double rfl = __ldg(Dv.rho_fl + fi), ufl = __ldg(Dv.u_fl + fi);
+        if (Dv.drift) {   // C-19
+          nrf = Pn[0] < rfl;
+          nuf = Pn[1] < ufl;
+          if (nrf | nuf) floors_drift(G, Bn, Dv.gam, nrf ? rfl : Pn[0], nuf ? ufl : Pn[1], Pn);
+          ceiling_only(G, Dv.gamma_max, Pn, ngc);
+        } else {
+          floors_ceiling(G, rfl, ufl, Dv.gamma_max, Pn, nrf, nuf, ngc);
+        }
 #pragma unroll
         for (int cc = 0; cc < 5; cc++) {
           const_cast<double*>(buf_arr(B, nw, cc))[z] = Pn[cc];
@@ -799,12 +839,15 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
   const unsigned m_f = __ballot_sync(0xffffffffu, nfail), m_r = __ballot_sync(0xffffffffu, nrf),
                  m_u = __ballot_sync(0xffffffffu, nuf), m_g = __ballot_sync(0xffffffffu, ngc),
                  m_b = __ballot_sync(0xffffffffu, bad);
+  const unsigned m_e = __ballot_sync(0xffffffffu, nent), m_a = __ballot_sync(0xffffffffu, nait);
   if ((threadIdx.x & 31) == 0) {
     if (m_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)__popc(m_f));
     if (m_r) atomicAdd(Dv.cnt + N_RHOFL, (unsigned long long)__popc(m_r));
     if (m_u) atomicAdd(Dv.cnt + N_UFL, (unsigned long long)__popc(m_u));
     if (m_g) atomicAdd(Dv.cnt + N_GCEIL, (unsigned long long)__popc(m_g));
     if (m_b) atomicAdd(Dv.cnt + N_NONFINITE, (unsigned long long)__popc(m_b));
+    if (m_e) atomicAdd(Dv.cnt + N_ENTROPY, (unsigned long long)__popc(m_e));
+    if (m_a) atomicAdd(Dv.cnt + N_AITKEN, (unsigned long long)__popc(m_a));
   }
 }
 
@@ -1326,7 +1369,7 @@ static void blk_stage(hamr_grid* g, int tau, bool corrector) {
     const Fields& s0 = g->s[0];
     const Fields& s1 = g->s[1];
     const Fields& s2 = g->s[2];
-    if (D.entropy) launch_kappa(g, D, corrector ? s1 : s0, corrector ? s1 : s2);   // C-18 (no LAT: every block is in this launch)
+    if (D.entropy) launch_kappa(g, D, corrector ? s1 : s0, corrector ? s1 : s2);   // C-18: kappa of the level's stage sources
     launch_flux_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2, corrector, true);
     launch_ct_on(g, D, corrector ? s1 : s0, corrector ? s1 : s2);
     launch_deref_fix_edges(g, D);

@@ -50,6 +50,7 @@ struct BlkDev {
   double* ctopb;             // [nblk][3] max signal speed of the block's last corrector pass (C-14)
   double* FA2[3][5];         // flux registers: dt_b F summed over the steps inside one coarser step (C-17)
   double* EA2[3];            // EMF registers
+  double* FKA2[3];           // C-18 under LAT: the register of the entropy flux (NULL without the entropy row)
 };
 
 // x1-slab sharding: the state arrays of the neighbour slabs, as device pointers

@@ -191,19 +191,26 @@ void launch_check_finite(hamr_grid* g, const Fields& s) {
 
 // C-18: kappa = p / rho^gamma_ad of every zone of the stage's source state, ghosts included (run after
 // the ghost fill), for the entropy flux of the generic flux kernels.  Slots no kernel reads (rho = 0) get 0.
-// On a block grid the stage source of a block is in buffer set s (cur == 0) or s2 (cur == 2); every block is done (the
-// blocks of one lattice level step together: the robust path excludes LAT)
+// On a block grid the stage source of a block is in buffer set s (cur == 0) or s2 (cur == 2)
 __global__ void k_kappa(Dev Dv, Fields s, Fields s2) {
-  const long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (z >= Dv.L.len) return;
-  const bool second = Dv.B.nblk > 0 && Dv.B.cur[z / Dv.B.blen] != 0;
+  long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  bool second = false;
+  if (Dv.B.nblk > 0) {          // the blocks of the launch's list (under LAT: one time level)
+    const long long slot = z / Dv.B.blen;
+    if (slot >= Dv.B.nact) return;
+    const int b = __ldg(Dv.B.list + slot);
+    z = (long long)b * Dv.B.blen + (z - slot * Dv.B.blen);
+    second = Dv.B.cur[b] != 0;
+  } else if (z >= Dv.L.len) return;
   const double rho = (second ? s2.P[0] : s.P[0])[z], u = (second ? s2.P[1] : s.P[1])[z];
   Dv.K[z] = rho > 0.0 ? kappa_of(rho, u, Dv.gam) : 0.0;
 }
 
 void launch_kappa(hamr_grid* g, const Dev& Dv, const Fields& s, const Fields& s2) {
+  const long long tot = Dv.B.nblk > 0 ? (long long)Dv.B.nact * Dv.B.blen : Dv.L.len;
+  if (tot == 0) return;
   Launch l_(g, K_OTHER);
-  k_kappa<<<(unsigned)((Dv.L.len + 255) / 256), 256, 0, g->stream>>>(Dv, s, s2);
+  k_kappa<<<(unsigned)((tot + 255) / 256), 256, 0, g->stream>>>(Dv, s, s2);
 }
 
 void launch_zero_ctop(hamr_grid* g) {

@@ -63,7 +63,7 @@ def test_bad_arguments_are_rejected_without_a_gpu():
         assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.EINVAL, change
     par = hamr.pack_params(dict(I.torus_params(), map=2))
     assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.OK
-    # NEXT-2 (entropy backup, drift-frame floors): no LAT, flags 0 / 1, gamma_ad < 2; four more arrays
+    # NEXT-2 (entropy backup, drift-frame floors): flags 0 / 1, gamma_ad < 2; four more arrays
     base = n.value
     par = hamr.pack_params(dict(I.torus_params(), entropy_backup=1, drift_floors=1))
     assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.OK and n.value > base
@@ -71,8 +71,9 @@ def test_bad_arguments_are_rejected_without_a_gpu():
     assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.OK
     par = hamr.pack_params(dict(I.torus_params(), entropy_backup=1, deref_theta_deg=(15.0,), deref_factor=(2,)))   # derefined rows: fine
     assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.OK
-    for change in (dict(entropy_backup=1, nb=(8, 8, 8), lat_max_level=1), dict(drift_floors=1, nb=(8, 8, 8), lat_max_level=1),
-                   dict(entropy_backup=2),
+    par = hamr.pack_params(dict(I.torus_params(), entropy_backup=1, drift_floors=1, nb=(8, 8, 8), lat_max_level=1))   # LAT: fine
+    assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.OK
+    for change in (dict(entropy_backup=2),
                    dict(drift_floors=-1), dict(entropy_backup=1, gamma_ad=2.0)):
         par = hamr.pack_params(dict(I.torus_params(), **change))
         assert L.hamr_workspace_bytes(C.byref(par), C.byref(n)) == hamr.EINVAL, change

@@ -455,3 +455,67 @@ def test_robust_path_on_a_refined_grid(H, orc):
         assert sg[0] == so[0] == 0 and sg[3] == so[3] and abs(bg - bo) <= max(3, bo // 50)
         tot += bo
     assert tot > 100 and g.divb() <= 1e-12
+
+
+@pytest.mark.parametrize("case", ["funnel_forced", "torus_courant", "cfg4_features"])
+def test_robust_path_under_lat(H, orc, case):
+    """C-18 / C-19 / C-21 under local adaptive time-stepping: the registers carry the entropy flux, the correction pass
+    corrects the entropy row of the coarse block's boundary zones and inverts them through the same chain (kappa having
+    been reset, their entropy row before the correction is density row x kappa of the new primitives).  funnel_forced:
+    time levels prescribed in bands (0, 1, 0, 1) on the magnetised funnel, where a third of the zone updates is rescued
+    by the entropy row, corrected zones included; torus_courant: Courant-based levels on the torus; cfg4_features:
+    blocks + LAT + phi-derefined rows + the x1 refinement level + both options at once"""
+    lv = None
+    if case == "funnel_forced":
+        p = I.minkowski_params(n=(32, 16, 16), nb=(8, 8, 8), lat_max_level=1, cour=0.25, rho_fl_coef=1e-9, u_fl_coef=1e-13,
+                               entropy_backup=1, drift_floors=1)
+        hyd, bf = _funnel(p)
+        tols = (1e-10, 1e-8, 1e-7)
+    elif case == "torus_courant":
+        p = I.torus_params(n=(32, 16, 16), nb=(8, 8, 8), lat_max_level=1, entropy_backup=1, drift_floors=1)
+        hyd, bf = I.fm_torus(p, seed=0)
+        tols = (4e-10, 1e-9, 4e-9)
+    else:
+        p = I.torus_params(n=(32, 16, 16), nb=(8, 4, 16), lat_max_level=1, r_refine_max=4.0, deref_theta_deg=(30.0, 12.0),
+                           deref_factor=(2, 4), entropy_backup=1, drift_floors=1)
+        tols = (4e-10, 1e-9, 4e-9)
+    g, o = H.Grid(p), orc.OrcGrid(p)
+    infos = []
+    for b in range(o.num_blocks()):
+        d = o.block_info(b)
+        infos.append((d["x_lo"], d["dx"], d["n"]))
+    if case == "funnel_forced":
+        lv = [(0, 1, 0, 1)[int(round(x_lo[0] / (dx[0] * n[0]))) % 4] for x_lo, dx, n in infos]
+        o.force_levels(lv)
+        g.set_levels(lv)
+    if case == "cfg4_features":
+        for b, (hb, fb) in enumerate(I.fm_torus_blocks(p, infos, seed=4)):
+            assert g.set_block_prims(b, hb, fb) == 0 and o.set_block_prims(b, hb, fb) == 0
+        assert g.commit() == 0 and o.commit() == 0
+    else:
+        assert g.set_prims(hyd, bf) == 0 and o.set_prims(hyd, bf) == 0
+    assert g.levels() == list(o.levels())
+    assert abs(g.dt - o.dt) <= 1e-13 * o.dt
+    tot = 0
+    for step in range(3):
+        g.step(1)
+        o.step(1)
+        assert g.levels() == list(o.levels())
+        worst = {}
+        for b, (x_lo, dx, n) in enumerate(infos):
+            Po, Pg = o.get_block_prims(b), g.get_block_prims(b)
+            e = parity_errors(I.block_as_grid(p, x_lo, dx, n), Po, Pg)
+            if case == "funnel_forced":
+                e["u"] = _u_error(Po, Pg)
+            for k, v in e.items():
+                worst[k] = max(worst.get(k, 0.0), v)
+        sg, so, bg, bo = g.stats(), o.stats(), g.backup_count(), o.backup_count()
+        print(f"{case} step {step + 1}: levels {sorted(set(o.levels()))} {worst} stats {sg} {so} entropy inversions {bg} {bo}")
+        assert max(worst.values()) <= tols[step], (step, worst)
+        assert sg[0] == so[0] == 0 and sg[3] == so[3]
+        if case == "funnel_forced":
+            assert sg == so and bg == bo
+        else:
+            assert abs(bg - bo) <= max(3, bo // 50)
+        tot += bo
+    assert len(set(o.levels())) > 1 and tot > 100 and g.divb() <= 1e-12
