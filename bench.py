@@ -3,7 +3,7 @@
 fraction of the dominant kernel, the end-to-end number through the C-ABI with host buffers, and the
 CPU oracle timed beside it.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg2r|cfg1|cfg0|cfg3|cfg4b|cfg4|cfg4t|paper150]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg2|cfg2r|cfg1|cfg0|cfg3|cfg4b|cfg4|cfg4t|cfg4r|paper150]
                   [--shard S]
 
 A "step" is one full pass of the hot path over the whole grid: hamr_step(1) = predictor + corrector
@@ -66,7 +66,7 @@ def workload(name, n_override=None):
                            deref_theta_deg=(15.0, 5.0), deref_factor=(2, 4))
         return p, (lambda: I.fm_torus(p, seed=4)), ("BASELINE cfg4 without r-refinement: Kerr FM torus 256x128x128 in 16x16x128 "
                                                      "blocks, phi-derefinement 2x/4x, LAT levels 1/2/4")
-    if name in ("cfg4", "cfg4t"):
+    if name in ("cfg4", "cfg4t", "cfg4r"):
         # BASELINE cfg 4: base 256x128x128 in 16^3 blocks, phi-derefined 2x / 4x within 15 / 5
         # degrees of the poles, one x1 refinement level for r < 20 (1472 blocks, 6 029 312 zones), LAT levels 1, 2, 4;
         # torus data sampled per block, seed 4.  gen() returns the per-block data.
@@ -76,11 +76,14 @@ def workload(name, n_override=None):
         if name == "cfg4t":
             bc = dict(bc_lo=(I.BC_OUTFLOW, I.BC_POLAR_TRANSMIT, I.BC_PERIODIC),
                       bc_hi=(I.BC_OUTFLOW, I.BC_POLAR_TRANSMIT, I.BC_PERIODIC))
+        if name == "cfg4r":   # cfg 4 with the robust inversion path on (NEXT-2 on the whole feature set)
+            bc = dict(entropy_backup=1, drift_floors=1)
         p = I.torus_params(n=(256, 128, 128), r_out=1000.0, nb=(16, 16, 16), lat_max_level=2, r_refine_max=20.0,
                            deref_theta_deg=(15.0, 5.0), deref_factor=(2, 4), **bc)
         return p, (lambda infos: I.fm_torus_blocks(p, infos, seed=4)), ("BASELINE cfg4: Kerr FM torus, base 256x128x128 in "
                    "16^3 blocks (1472), one x1 refinement level r<20, phi-derefinement 2x/4x, LAT levels 1/2/4"
-                   + (", transmissive poles" if name == "cfg4t" else ""))
+                   + (", transmissive poles" if name == "cfg4t" else "")
+                   + (", entropy backup + drift-frame floors (NEXT-2)" if name == "cfg4r" else ""))
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -678,7 +681,7 @@ def main():
     cpu = None
     if not args.no_cpu_baseline:
         subprocess.check_call(["make", "-s", "-C", os.path.join(ROOT, "oracle")])
-        steps_cpu = 3 if args.workload == "cfg2" else (1 if args.workload in ("cfg4b", "cfg4", "cfg4t") else 2)
+        steps_cpu = 3 if args.workload == "cfg2" else (1 if args.workload in ("cfg4b", "cfg4", "cfg4t", "cfg4r") else 2)
         v, secs, cores = cpu_oracle_time(p, gen, steps_cpu)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"{steps_cpu} full {'coarse ' if fin > 1 else ''}steps of the same workload, all {nz} zones ({secs:.1f} s)"}

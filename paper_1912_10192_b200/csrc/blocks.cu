@@ -576,6 +576,7 @@ __global__ void __launch_bounds__(256, GHOST_MINB) k_blk_ghosts(const __grid_con
 
 // C-17 registers: R2 = sum over the steps inside one step of the next coarser level of dt_b F and
 // dt_b E of the corrector pass, on the faces and edges of the block boundary only.
+template <bool ENT>
 __global__ void __launch_bounds__(128) k_blk_registers(Dev Dv, int first, double dtfac) {
   const Lay& L = Dv.L;
   const int c2 = L.n[2] + 1, c1 = L.n[1] + 1;
@@ -601,7 +602,7 @@ __global__ void __launch_bounds__(128) k_blk_registers(Dev Dv, int first, double
         const double v = dtb * Dv.F[d][c][z];
         Dv.B.FA2[d][c][z] = first ? v : Dv.B.FA2[d][c][z] + v;
       }
-      if (Dv.entropy) {   // C-18: the entropy flux is one more flux of the face
+      if (ENT) {   // C-18: the entropy flux is one more flux of the face
         const double v = dtb * Dv.FK[d][z];
         Dv.B.FKA2[d][z] = first ? v : Dv.B.FKA2[d][z] + v;
       }
@@ -714,6 +715,8 @@ __global__ void __launch_bounds__(128) k_blk_correct_faces(Dev Dv, Bufs B, int t
 
 // correct(tau-1 -> tau), zone part: flux difference into the boundary zones, new cell-centred field,
 // re-inversion of every touched zone
+// ROB: the grid carries the entropy row and / or the drift-frame floors (C-18, C-19, C-21)
+template <bool ROB>
 __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int tc, double dtfac) {
   const Lay& L = Dv.L;
   const unsigned per = (unsigned)L.n[0] * L.n[1] * L.n[2];
@@ -760,7 +763,7 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
                 // U_new = U - (dt F_hi - dt F_lo)/dx: the high face enters with -, the low face with +
                 dU[cc] += (side ? -dF : dF) / dxd[d];
               }
-              if (Dv.entropy) {   // C-18: the entropy row is corrected like the others
+              if (ROB && Dv.entropy) {   // C-18: the entropy row is corrected like the others
                 const double dF = Dv.B.FKA2[d][zq] - dtc * Dv.FK[d][zf];
                 dUS += (side ? -dF : dF) / dxd[d];
               }
@@ -789,11 +792,11 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
         prim_to_U5(P, Sx, G.gdet, Dv.gam, U);
         // C-18 under LAT: kappa was reset from the zone's new primitives, so its entropy row before the correction is its
         // density row times kappa(P)
-        const double US = Dv.entropy ? U[0] * kappa_of(P[0], P[1], Dv.gam) + dUS : 0.0;
+        const double US = (ROB && Dv.entropy) ? U[0] * kappa_of(P[0], P[1], Dv.gam) + dUS : 0.0;
 #pragma unroll
         for (int cc = 0; cc < 5; cc++) U[cc] += dU[cc];
         int rc = con2prim(U, Bn, G, Dv.gam, P, Pn);
-        if (Dv.entropy && (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0))) {   // the chain of the update (C-21, C-18)
+        if (ROB && Dv.entropy && (rc != 0 || !(Pn[0] > 0.0) || !(Pn[1] >= 0.0))) {   // the chain of the update (C-21, C-18)
           double Pe[5], Uc[5], Bc[3], Pc[5];
           CGeo Gc = G;
 #pragma unroll
@@ -820,7 +823,7 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
         }
         const int fi = inf.z + id[0] + NG + inf.y * Dv.B.flev;
         const double rfl = __ldg(Dv.rho_fl + fi), ufl = __ldg(Dv.u_fl + fi);
-        if (Dv.drift) {   // C-19
+        if (ROB && Dv.drift) {   // C-19
           nrf = Pn[0] < rfl;
           nuf = Pn[1] < ufl;
           if (nrf | nuf) floors_drift(G, Bn, Dv.gam, nrf ? rfl : Pn[0], nuf ? ufl : Pn[1], Pn);
@@ -839,15 +842,17 @@ __global__ void __launch_bounds__(128) k_blk_correct_zones(Dev Dv, Bufs B, int t
   const unsigned m_f = __ballot_sync(0xffffffffu, nfail), m_r = __ballot_sync(0xffffffffu, nrf),
                  m_u = __ballot_sync(0xffffffffu, nuf), m_g = __ballot_sync(0xffffffffu, ngc),
                  m_b = __ballot_sync(0xffffffffu, bad);
-  const unsigned m_e = __ballot_sync(0xffffffffu, nent), m_a = __ballot_sync(0xffffffffu, nait);
+  if (ROB) {
+    const unsigned m_e = __ballot_sync(0xffffffffu, nent), m_a = __ballot_sync(0xffffffffu, nait);
+    if ((threadIdx.x & 31) == 0 && m_e) atomicAdd(Dv.cnt + N_ENTROPY, (unsigned long long)__popc(m_e));
+    if ((threadIdx.x & 31) == 0 && m_a) atomicAdd(Dv.cnt + N_AITKEN, (unsigned long long)__popc(m_a));
+  }
   if ((threadIdx.x & 31) == 0) {
     if (m_f) atomicAdd(Dv.cnt + N_C2PFAIL, (unsigned long long)__popc(m_f));
     if (m_r) atomicAdd(Dv.cnt + N_RHOFL, (unsigned long long)__popc(m_r));
     if (m_u) atomicAdd(Dv.cnt + N_UFL, (unsigned long long)__popc(m_u));
     if (m_g) atomicAdd(Dv.cnt + N_GCEIL, (unsigned long long)__popc(m_g));
     if (m_b) atomicAdd(Dv.cnt + N_NONFINITE, (unsigned long long)__popc(m_b));
-    if (m_e) atomicAdd(Dv.cnt + N_ENTROPY, (unsigned long long)__popc(m_e));
-    if (m_a) atomicAdd(Dv.cnt + N_AITKEN, (unsigned long long)__popc(m_a));
   }
 }
 
@@ -1385,7 +1390,8 @@ static void blk_stage(hamr_grid* g, int tau, bool corrector) {
       const Lay& L = D.L;
       const long long tot = (long long)(L.n[0] + 1) * (L.n[1] + 1) * (L.n[2] + 1) * D.B.nact;
       Launch l_(g, K_OTHER);
-      k_blk_registers<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, first, lev_fac);
+      if (D.entropy) k_blk_registers<true><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, first, lev_fac);
+      else k_blk_registers<false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, first, lev_fac);
     }
     if (!corrector) {
       const Roles ra = {s0, s0, s1}, rb = {s2, s2, s1};
@@ -1417,7 +1423,8 @@ static void blk_correct(hamr_grid* g, int tau) {
   tot = (long long)L.n[0] * L.n[1] * L.n[2] * D.B.nact;
   {
     Launch l_(g, K_OTHER);
-    k_blk_correct_zones<<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, bufs_of(g), tau, lev_fac);
+    if (D.entropy || D.drift) k_blk_correct_zones<true><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, bufs_of(g), tau, lev_fac);
+    else k_blk_correct_zones<false><<<(unsigned)((tot + 127) / 128), 128, 0, g->stream>>>(D, bufs_of(g), tau, lev_fac);
   }
   launch_deref_sync(g, D, g->s[2], g->s[0]);   // the corrected new state of a block with cur == 0 / 2
 }
