@@ -519,3 +519,32 @@ def test_robust_path_under_lat(H, orc, case):
             assert abs(bg - bo) <= max(3, bo // 50)
         tot += bo
     assert len(set(o.levels())) > 1 and tot > 100 and g.divb() <= 1e-12
+
+
+def test_cfg4_full_size_with_entropy_backup_and_drift_floors(H, orc):
+    """BASELINE cfg 4 as written (1472 blocks of 16^3: x1 refinement, phi-derefinement 2x / 4x, LAT levels 1 / 2 / 4) with
+    both robust options: every zone of every block after one coarse step (4 finest steps), the level assignment equal"""
+    import bench
+    p, gen, _ = bench.workload("cfg4r")
+    g, o = H.Grid(p), orc.OrcGrid(p)
+    infos = []
+    for b in range(o.num_blocks()):
+        d = o.block_info(b)
+        infos.append((d["x_lo"], d["dx"], d["n"]))
+    assert len(infos) == 1472
+    for b, (hb, fb) in enumerate(gen(infos)):
+        assert g.set_block_prims(b, hb, fb) == 0 and o.set_block_prims(b, hb, fb) == 0
+    assert g.commit() == 0 and o.commit() == 0
+    assert g.levels() == list(o.levels()) and sorted(set(o.levels())) == [0, 1, 2]
+    g.step(1)
+    o.step(1)
+    assert g.levels() == list(o.levels())
+    worst = {}
+    for b, (x_lo, dx, n) in enumerate(infos):
+        e = parity_errors(I.block_as_grid(p, x_lo, dx, n), o.get_block_prims(b), g.get_block_prims(b))
+        for k, v in e.items():
+            worst[k] = max(worst.get(k, 0.0), v)
+    sg, so = g.stats(), o.stats()
+    print("cfg 4 + NEXT-2, one coarse step:", worst, sg, so, g.backup_count(), o.backup_count())
+    assert max(worst.values()) <= 4e-10, worst          # 4 finest steps
+    assert sg[0] == so[0] == 0 and sg[3] == so[3] and g.divb() <= 1e-12
