@@ -247,3 +247,52 @@ def test_bench_shard_line():
     assert line["metric"] == "zone_cycles_per_sec" and line["scaling"] == "strong" and line["value"] > 0
     assert line["config"]["slabs"] == [[0, 16], [16, 16]] and line["gpu_launches"] > 0
     assert line["divb"] <= TOL_DIVB and line["one_grid"]["ms_per_step"] > 0
+
+
+def _nccl_one_rank(port, out_path, mem):
+    import os
+    import sys
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    from paper_1912_10192_b200 import hamr, shard
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    torch.cuda.set_device(0)
+    torch.cuda.set_stream(torch.cuda.Stream())
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    p = I.torus_params()
+    hyd, bf = I.fm_torus(p, seed=0)
+    one = hamr.Grid(p, torch_arena=True)
+    assert one.set_prims(hyd, bf) == 0
+    one.step(5)
+    ds = shard.DistSlab(p, peer_memory=mem)
+    assert ds.red.on_stream and ds.ranges == [(0, 32)]
+    assert ds.set_prims(hyd, bf) == 0
+    ds.step(5)
+    same = all(np.array_equal(a, b) for a, b in zip(one.get_prims(), ds.slab.get_prims())) and ds.slab.t == one.t
+    ds.close()
+    dist.destroy_process_group()
+    with open(out_path, "w") as f:
+        f.write("same" if same else "different")
+
+
+@pytest.mark.parametrize("mem", ["symm", "ipc"])
+def test_dist_slab_on_a_one_rank_nccl_group(tmp_path, mem):
+    """the torch.distributed plumbing of shard.DistSlab with the NCCL backend (all-reduces enqueued on the grid's stream)
+    and both ways of mapping arenas (torch symmetric memory; CUDA IPC handles), on the one GPU there is: a group of ONE
+    rank, whose slab covers the grid; the run equals the one-grid run bit for bit"""
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    out = tmp_path / "r.txt"
+    ctx = mp.get_context("spawn")
+    q = ctx.Process(target=_nccl_one_rank, args=(port, str(out), mem))
+    q.start()
+    q.join(timeout=300)
+    if q.is_alive():
+        q.kill()
+        raise AssertionError("the rank did not finish")
+    assert q.exitcode == 0 and out.read_text() == "same"
