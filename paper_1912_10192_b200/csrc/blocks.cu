@@ -169,14 +169,13 @@ __device__ __noinline__ void blk_src_slow(const Dev* Dv, int b, int phys, int sd
   *out = blk_src(*Dv, b, phys, sd, id, norule != 0);
 }
 
-__device__ __forceinline__ GSrc blk_src_tab(const Dev& Dv, int b, int phys, int sd, const int id[3], bool norule) {
-  const Lay& L = Dv.L;
-  const int e3 = L.n[2] + 2 * NG + 1;
-  const bool inside = id[0] >= -NG && id[0] <= L.n[0] + NG && id[1] >= -NG && id[1] <= L.n[1] + NG && id[2] >= -NG &&
-                      id[2] <= L.n[2] + NG;
-  if (Dv.B.gsrc && inside) {
-    const int loc = ((id[0] + NG) * L.e2 + id[1] + NG) * e3 + id[2] + NG;
-    const unsigned long long w = __ldg(Dv.B.gsrc + ((size_t)b * 4 + (sd + 1)) * Dv.B.gloc + loc);
+// tb: the block's part of the table (NULL: no table); loc: the padded location of id[] (every caller's id[] lies inside
+// the padded block: the thread's own location, its + 1 neighbour along a dimension that is not the extra slot, or a
+// derefinement group slot of the same row)
+__device__ __forceinline__ GSrc blk_src_tab(const Dev& Dv, const unsigned long long* __restrict__ tb, int loc, int b,
+                                            int phys, int sd, const int id[3], bool norule) {
+  if (tb) {
+    const unsigned long long w = __ldg(tb + (size_t)(sd + 1) * Dv.B.gloc + loc);
     if (!(w >> 63)) {
       GSrc s;
       s.zl = (int)(unsigned)(w & 0xffffffffull);
@@ -461,6 +460,10 @@ __global__ void __launch_bounds__(256, GHOST_MINB) k_blk_ghosts(const __grid_con
   // bit 2: all neighbours on the block's own level: no finer-block faces, and every sample is a plain copy
   // of the neighbour's stage source (its time-n state for a predictor, its predictor state for a corrector)
   const bool same = (flags & 4) != 0;
+  // the block's part of the ghost-source table and this thread's location in it (its neighbours: fixed strides)
+  const unsigned long long* tb = Dv.B.gsrc ? Dv.B.gsrc + (size_t)b * 4 * Dv.B.gloc : nullptr;
+  const int lst[3] = {L.e2 * e3, e3, 1};
+  const int loc0 = ((id[0] + NG) * L.e2 + id[1] + NG) * e3 + id[2] + NG;
   int lastq = -1;
   QTime qt;
   qt.b0 = 0; qt.b1 = -1; qt.w = 0.0;
@@ -482,7 +485,7 @@ __global__ void __launch_bounds__(256, GHOST_MINB) k_blk_ghosts(const __grid_con
   // here is a neighbour of b on b's own level, so none of them rewrites those zones in this launch.
   bool pure = false;
   if (wP) {
-    const GSrc s = blk_src_tab(Dv, b, phys, -1, id, same);
+    const GSrc s = blk_src_tab(Dv, tb, loc0, b, phys, -1, id, same);
     if (s.ghost) { qt = qtime(s.q); lastq = s.q; }
 #pragma unroll
     for (int c = 0; c < 5; c++) vP[c] = fetch(c, s);
@@ -503,7 +506,7 @@ __global__ void __launch_bounds__(256, GHOST_MINB) k_blk_ghosts(const __grid_con
     if (extra[o1] || extra[o2]) { lo[d] = hi[d] = 0.0; continue; }
     const bool face_read = shell1[o1] && shell1[o2] && id[d] >= 0 && id[d] <= L.n[d];   // a flux kernel reads this face
     if (pure && !face_read) { lo[d] = hi[d] = 0.0; continue; }
-    GSrc s = blk_src_tab(Dv, b, phys, d, id, same);
+    GSrc s = blk_src_tab(Dv, tb, loc0, b, phys, d, id, same);
     if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
     lo[d] = fetch(5 + d, s);
     if (s.mod) { wF[d] = face_read; anymod = true; }
@@ -511,7 +514,7 @@ __global__ void __launch_bounds__(256, GHOST_MINB) k_blk_ghosts(const __grid_con
     if (!extra[d] && !pure) {
       int idp[3] = {id[0], id[1], id[2]};
       idp[d] += 1;
-      s = blk_src_tab(Dv, b, phys, d, idp, same);
+      s = blk_src_tab(Dv, tb, loc0 + lst[d], b, phys, d, idp, same);
       if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
       hi[d] = fetch(5 + d, s);
       anymod = anymod || s.mod;
@@ -540,11 +543,11 @@ __global__ void __launch_bounds__(256, GHOST_MINB) k_blk_ghosts(const __grid_con
         if (m > 1) {   // C-15: B_c^3 of a phi-derefined row is the group's value, from the group's two outer x3-faces
           const int k0 = id[2] - id[2] % m;
           int ig[3] = {id[0], id[1], k0};
-          GSrc s = blk_src_tab(Dv, b, phys, 2, ig, same);
+          GSrc s = blk_src_tab(Dv, tb, loc0 + (k0 - id[2]), b, phys, 2, ig, same);
           if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
           lo[2] = fetch(7, s);
           ig[2] = k0 + m;
-          s = blk_src_tab(Dv, b, phys, 2, ig, same);
+          s = blk_src_tab(Dv, tb, loc0 + (k0 + m - id[2]), b, phys, 2, ig, same);
           if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
           hi[2] = fetch(7, s);
         }
@@ -554,13 +557,13 @@ __global__ void __launch_bounds__(256, GHOST_MINB) k_blk_ghosts(const __grid_con
         const int Mhi = max(m, __ldg(Dv.mrow + min(J + 1, Dv.B.n2g + NG) + NG));
         if (Mlo != m) {
           int ig[3] = {id[0], id[1], deref_face2_slot(id[2], n3, m, Mlo)};
-          const GSrc s = blk_src_tab(Dv, b, phys, 1, ig, same);
+          const GSrc s = blk_src_tab(Dv, tb, loc0 + (ig[2] - id[2]), b, phys, 1, ig, same);
           if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
           lo[1] = fetch(6, s);
         }
         if (Mhi != m) {
           int ig[3] = {id[0], id[1] + 1, deref_face2_slot(id[2], n3, m, Mhi)};
-          const GSrc s = blk_src_tab(Dv, b, phys, 1, ig, same);
+          const GSrc s = blk_src_tab(Dv, tb, loc0 + lst[1] + (ig[2] - id[2]), b, phys, 1, ig, same);
           if (s.ghost && s.q != lastq) { qt = qtime(s.q); lastq = s.q; }
           hi[1] = fetch(6, s);
         }
