@@ -149,37 +149,42 @@ __global__ void __launch_bounds__(256) k_ghosts(Dev D, Fields s, int all, int pq
 //          axis): every k;   part B: active (i,j) columns: the 2 NG + 1 ghost slots in k.
 // nox3: the stage kernels of this grid never read x3 ghost zones (x3_ghosts_unused, flux.cu): part A covers
 // k in [0, n3) only and there is no part B.
-__global__ void __launch_bounds__(256) k_ghosts_shell(Dev D, Fields s, int nj, long long nA, int nox3, int pq) {
+__global__ void __launch_bounds__(256) k_ghosts_shell(Dev D, Fields s, int nj, long long nA_, int nox3, int pq) {
   const Lay& L = D.L;
-  const int e3 = nox3 ? L.n[2] : L.n[2] + 2 * NG + 1;
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  // 32-bit index arithmetic (an array holds < 2^31 doubles, checked at creation): 64-bit division is emulated
+  const unsigned e3 = nox3 ? L.n[2] : L.n[2] + 2 * NG + 1;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned nA = (unsigned)nA_;
   if (t < nA) {
-    const int k = (int)(t % e3) - (nox3 ? 0 : NG);
-    long long row = t / e3;
+    unsigned row = t / e3;
+    const int k = (int)(t - row * e3) - (nox3 ? 0 : NG);
     int i, j;
-    const long long lo_rows = (long long)NG * L.e2, mid_rows = (long long)L.n[0] * nj;
+    const unsigned e2 = L.e2, lo_rows = NG * e2, mid_rows = (unsigned)L.n[0] * nj;
     if (row < lo_rows) {
-      i = (int)(row / L.e2) - NG; j = (int)(row % L.e2) - NG;
+      const unsigned a = row / e2;
+      i = (int)a - NG; j = (int)(row - a * e2) - NG;
     } else if (row < lo_rows + mid_rows) {
       row -= lo_rows;
-      i = (int)(row / nj);
-      const int q = (int)(row % nj);  // -3, -2, -1, [0,] n2 .. n2 + 3
+      const unsigned a = row / (unsigned)nj;
+      i = (int)a;
+      const int q = (int)(row - a * nj);  // -3, -2, -1, [0,] n2 .. n2 + 3
       j = q < NG ? q - NG : (nj == 2 * NG + 2 ? (q == NG ? 0 : L.n[1] + q - NG - 1) : L.n[1] + q - NG);
     } else {
       row -= lo_rows + mid_rows;
-      i = L.n[0] + (int)(row / L.e2); j = (int)(row % L.e2) - NG;
+      const unsigned a = row / e2;
+      i = L.n[0] + (int)a; j = (int)(row - a * e2) - NG;
     }
     ghost_cell(D, s, 0, i, j, k, pq);
     return;
   }
   if (nox3) return;
-  const long long u = t - nA;
-  const long long nB = (long long)L.n[0] * L.n[1] * 8;
+  const unsigned u = t - nA;
+  const unsigned nB = (unsigned)L.n[0] * L.n[1] * 8;
   if (u >= nB) return;
   const int q = (int)(u & 7);
   if (q == 7) return;
-  const long long col = u >> 3;
-  const int i = (int)(col / L.n[1]), j = (int)(col % L.n[1]);
+  const unsigned col = u >> 3;
+  const int i = (int)(col / (unsigned)L.n[1]), j = (int)(col - (unsigned)i * L.n[1]);
   if (nj == 2 * NG + 2 && j == 0) return;  // the wall row was done in part A
   const int n3 = L.n[2];
   const int k = q < NG ? q - NG : n3 + q - NG;
